@@ -1,0 +1,6 @@
+"""CPU oracle package - TEST INFRASTRUCTURE (see oracle/lsa_oracle.py header)."""
+from .lsa_oracle import (  # noqa: F401
+    EPS_NORM, LsaOracle, PoolExhausted, ResidencyOracle, attention, chunk_scores,
+    merge_partials, partial_attention, query_tower, topk_select, trigger_fires,
+    validate_selection, widen,
+)

@@ -1,0 +1,415 @@
+"""Seeded synthetic LSA workloads (inputs only - none of the method's arithmetic).
+
+This module is the ONE piece shared by the CUDA path (tests, bench.py) and the CPU
+oracle (oracle/): it produces the stored, already-rounded input arrays that both sides
+read.  It never scores, selects, allocates pages or attends.  It depends on numpy and
+torch-CPU only and must stay importable without the CUDA extension.
+
+Shapes / distributions follow BASELINE.json `configs` (numbered 1..5 here) and
+SURVEY.md 8(d); the recipe is restated in DESIGN.md "Input recipe".  They stand in for
+the paper's long-context workloads (Table 1 context lengths 46K-512K, Fig. 1
+1M-token projection) - only the context-length range and the ~10 % recall ratio are
+taken from the paper, no item of any benchmark suite.
+
+Array conventions
+-----------------
+* dtype "f32": numpy float32 arrays.
+* dtype "bf16": numpy uint16 arrays holding bfloat16 bit patterns (numpy has no bf16).
+  `to_torch` / `as_f64` convert.  The stored bit patterns are the truth for both sides.
+* cold_csa[b] : [n_chunks, 2, C, D]   (K block then V block per chunk = one page)
+* chunk_emb[b]: [n_chunks, E]         hca_k/hca_v[b]: [n_hca, D]     win_k/win_v[b]: [W, D]
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+from typing import Dict, List, Optional, Tuple
+
+import numpy as np
+import torch
+
+BASE_SEED = 260609079 * 8  # seed = 260609079*8 + config_id
+
+
+# --------------------------------------------------------------------------------------
+# dtype helpers (storage only)
+# --------------------------------------------------------------------------------------
+def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """Round float32 -> bfloat16 bit patterns (round-to-nearest-even), as uint16."""
+    t = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32))
+    return t.to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16).copy()
+
+
+def bf16_bits_to_f32(bits: np.ndarray) -> np.ndarray:
+    return (bits.astype(np.uint32) << 16).view(np.float32)
+
+
+def store(x: np.ndarray, dtype: str) -> np.ndarray:
+    """Round a float array to the storage dtype of the config."""
+    if dtype == "f32":
+        return np.ascontiguousarray(x, dtype=np.float32)
+    if dtype == "bf16":
+        return f32_to_bf16_bits(np.asarray(x, dtype=np.float32))
+    raise ValueError(dtype)
+
+
+def as_f64(x: np.ndarray, dtype: str) -> np.ndarray:
+    """Exact widening of a stored array to float64."""
+    if dtype == "f32":
+        return x.astype(np.float64)
+    return bf16_bits_to_f32(x).astype(np.float64)
+
+
+def to_torch(x: np.ndarray, dtype: str) -> torch.Tensor:
+    """Stored numpy array -> torch CPU tensor of the matching dtype (shares memory)."""
+    if dtype == "f32":
+        return torch.from_numpy(x)
+    return torch.from_numpy(x.view(np.int16)).view(torch.bfloat16)
+
+
+def from_torch(t: torch.Tensor, dtype: str) -> np.ndarray:
+    t = t.detach().cpu().contiguous()
+    if dtype == "f32":
+        return t.numpy()
+    return t.view(torch.int16).numpy().view(np.uint16)
+
+
+def elem_size(dtype: str) -> int:
+    return 4 if dtype == "f32" else 2
+
+
+# --------------------------------------------------------------------------------------
+# configuration
+# --------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class LsaWorkloadConfig:
+    name: str
+    config_id: int
+    dtype: str                 # "f32" | "bf16"
+    B: int
+    L: List[int]               # per-sequence context length in tokens
+    H: int
+    D: int
+    C: int                     # CSA entries per chunk (= page rows)
+    W: int                     # window capacity (raw tokens)
+    Dh: int
+    E: int
+    k: int
+    tau: int
+    steps: int
+    hot_pages: int
+    recall_lag: int = 1
+    csa_ratio: int = 4         # BASELINE.json cfg 1 "assumed 4:1"
+    hca_ratio: int = 128       # PAPER.md l.31 "128:1"
+    emb_mode: str = "beta"     # "needle0" (cfg1) | "beta" (cfg 2-4) | "uniform" (cfg 5)
+    n_needles: int = 16
+    needle_cos: float = 0.8
+    needle_period: int = 4     # needles drift every this many triggers
+    h_noise: float = 0.05
+    stagger: bool = False      # cfg 4: per-sequence trigger phase
+    tie_frac: float = 0.0      # cfg 5: fraction of triggers carrying planted ties
+    q_gain: float = 1.0        # 1.0 = BASELINE recipe q ~ N(0,1)/sqrt(D)
+    kv_base_chunks: int = 0    # >0: cold pools are tiled from this many random chunks
+
+    # ---- derived per sequence -------------------------------------------------------
+    def n_hca(self, b: int) -> int:
+        return self.L[b] // self.hca_ratio
+
+    def n_csa(self, b: int) -> int:
+        return self.L[b] // self.csa_ratio
+
+    def n_chunks(self, b: int) -> int:
+        return -(-self.n_csa(b) // self.C)
+
+    def k_eff(self, b: int) -> int:
+        return min(self.k, self.n_chunks(b))
+
+    def step0(self, b: int) -> int:
+        if not self.stagger:
+            return 0
+        # sequence b first fires at global step (b*tau//B) mod tau
+        return (self.tau - (b * self.tau // self.B) % self.tau) % self.tau
+
+    @property
+    def page_elems(self) -> int:
+        return 2 * self.C * self.D
+
+    @property
+    def page_bytes(self) -> int:
+        return self.page_elems * elem_size(self.dtype)
+
+    @property
+    def seed(self) -> int:
+        return BASE_SEED + self.config_id
+
+    def keys_attended(self, b: int, selected: bool = True) -> int:
+        """N_b of SURVEY 8: HCA rows + selected chunks (full pages) + full window."""
+        return self.n_hca(b) + (self.k_eff(b) * self.C if selected else 0) + min(self.W, self.L[b])
+
+    def attn_bytes_per_step(self) -> int:
+        """Algorithmic bytes of S7 per step, all sequences."""
+        sz = elem_size(self.dtype)
+        return sum(self.keys_attended(b) * 2 * self.D * sz + 2 * self.H * self.D * sz
+                   for b in range(self.B))
+
+    def attn_flops_per_step(self) -> int:
+        return sum(4 * self.H * self.D * self.keys_attended(b) for b in range(self.B))
+
+
+def _ragged_lengths(seed: int, B: int, lo: int, hi: int) -> List[int]:
+    g = np.random.Generator(np.random.Philox(seed))
+    u = g.uniform(math.log(lo), math.log(hi), size=B)
+    return [int(math.floor(math.exp(x))) // 128 * 128 for x in u]
+
+
+def make_config(config_id: int, **overrides) -> LsaWorkloadConfig:
+    """The five BASELINE.json configs (1-based, file order)."""
+    if config_id == 1:
+        cfg = LsaWorkloadConfig(
+            name="cfg1_tiny_f32_8k", config_id=1, dtype="f32", B=1, L=[8192], H=16, D=128,
+            C=64, W=512, Dh=1024, E=256, k=4, tau=64, steps=128, hot_pages=8,
+            emb_mode="needle0", n_needles=4, needle_cos=0.9, needle_period=10**9)
+    elif config_id == 2:
+        cfg = LsaWorkloadConfig(
+            name="cfg2_bf16_128k", config_id=2, dtype="bf16", B=1, L=[131072], H=64, D=512,
+            C=128, W=8192, Dh=4096, E=512, k=16, tau=64, steps=1024, hot_pages=64)
+    elif config_id == 3:
+        cfg = LsaWorkloadConfig(
+            name="cfg3_bf16_1m", config_id=3, dtype="bf16", B=1, L=[1048576], H=64, D=512,
+            C=128, W=8192, Dh=4096, E=512, k=64, tau=64, steps=2048,
+            hot_pages=205)  # ceil(0.1 * 2048 chunks)
+    elif config_id == 4:
+        B = 32
+        L = _ragged_lengths(BASE_SEED + 4, B, 65536, 1048576)
+        cfg = LsaWorkloadConfig(
+            name="cfg4_bf16_b32_ragged", config_id=4, dtype="bf16", B=B, L=L, H=64, D=512,
+            C=128, W=8192, Dh=4096, E=512, k=32, tau=64, steps=512,
+            hot_pages=16 * 10**9 // (2 * 128 * 512 * 2),  # 16e9 B -> 61035 pages
+            stagger=True, kv_base_chunks=256)
+    elif config_id == 5:
+        B = 8
+        cfg = LsaWorkloadConfig(
+            name="cfg5_bf16_churn", config_id=5, dtype="bf16", B=B, L=[524288] * B, H=64,
+            D=512, C=128, W=8192, Dh=4096, E=512, k=128, tau=16, steps=1024,
+            hot_pages=2 * 128 * B,  # 2k pages per sequence
+            emb_mode="uniform", n_needles=0, tie_frac=0.10, kv_base_chunks=256)
+    else:
+        raise ValueError(f"config_id must be 1..5, got {config_id}")
+    return dataclasses.replace(cfg, **overrides) if overrides else cfg
+
+
+def make_small_config(dtype: str = "f32", **kw) -> LsaWorkloadConfig:
+    """A scaled-down shape for CPU tests and fast parity cases (not a BASELINE config)."""
+    base = dict(name="small", config_id=101, dtype=dtype, B=2, L=[4096, 2432], H=8, D=64, C=16,
+                W=64, Dh=128, E=64, k=3, tau=4, steps=12, hot_pages=16, emb_mode="beta",
+                n_needles=2, needle_cos=0.8, needle_period=2)
+    base.update(kw)
+    return LsaWorkloadConfig(**base)
+
+
+# --------------------------------------------------------------------------------------
+# generator
+# --------------------------------------------------------------------------------------
+def _rng(seed: int, *tags: int) -> np.random.Generator:
+    return np.random.Generator(np.random.Philox(key=np.random.SeedSequence([seed, *tags]).generate_state(2, np.uint64)))
+
+
+def _randn_stored(g: np.random.Generator, shape, scale: float, dtype: str) -> np.ndarray:
+    x = g.standard_normal(size=shape, dtype=np.float32)
+    x *= np.float32(scale)
+    return store(x, dtype)
+
+
+def _unit_rows(x: np.ndarray) -> np.ndarray:
+    return x / np.linalg.norm(x, axis=-1, keepdims=True)
+
+
+class LsaWorkload:
+    """All static inputs of one config plus per-step / per-trigger dynamic inputs."""
+
+    def __init__(self, cfg: LsaWorkloadConfig, build_kv: bool = True):
+        """build_kv=False skips every K/V array (indexer-only uses at full config sizes)."""
+        self.cfg = cfg
+        c = cfg
+        dt = c.dtype
+        s = c.seed
+        self.W_q = _randn_stored(_rng(s, 1), (c.E, c.Dh), 1.0 / math.sqrt(c.Dh), dt)
+        self.hca_k, self.hca_v, self.win_k, self.win_v = [], [], [], []
+        self.cold_csa: List[np.ndarray] = []
+        self.h0: List[np.ndarray] = []        # stored dtype [Dh]
+        self.u: List[np.ndarray] = []         # float64 [E]: planted query direction
+        self.base_cos: List[np.ndarray] = []  # float64 [n_chunks] (beta mode)
+        self.base_emb: List[np.ndarray] = []  # stored [n_chunks, E]
+        self._needle_cache: Dict[Tuple[int, int], np.ndarray] = {}
+        inv_sqrt_d = 1.0 / math.sqrt(c.D)
+        kv_base = None
+        if c.kv_base_chunks > 0 and build_kv:
+            kv_base = _randn_stored(_rng(s, 2), (c.kv_base_chunks, 2, c.C, c.D), inv_sqrt_d, dt)
+        Wf = as_f64(self.W_q, dt)
+        for b in range(c.B):
+            nch = c.n_chunks(b)
+            if build_kv:
+                self._build_kv(b, kv_base, inv_sqrt_d)
+
+            # planted query direction u_b and an h0 with  W_q h0 = s*u  built by least squares
+            # (np.linalg.lstsq min-norm solve - a construction, not the query tower itself).
+            g = _rng(s, 20, b)
+            u = _unit_rows(g.standard_normal(c.E))
+            gvec = g.standard_normal(c.Dh)
+            zg = Wf @ gvec
+            rhs = np.linalg.norm(zg) * u - zg
+            corr = np.linalg.lstsq(Wf, rhs, rcond=None)[0]
+            self.h0.append(store((gvec + corr).astype(np.float32), dt))
+            self.u.append(u)
+
+            ge = _rng(s, 21, b)
+            r = ge.standard_normal((nch, c.E))
+            if c.emb_mode == "beta":
+                cosv = ge.beta(2.0, 8.0, size=nch)
+                self.base_cos.append(cosv)
+                emb = self._plant(u, r, cosv)
+            else:                                   # "needle0" / "uniform": random unit rows
+                self.base_cos.append(np.zeros(nch))
+                emb = _unit_rows(r)
+            self.base_emb.append(store(emb.astype(np.float32), dt))
+
+    def _build_kv(self, b: int, kv_base: Optional[np.ndarray], inv_sqrt_d: float) -> None:
+        c, dt, s = self.cfg, self.cfg.dtype, self.cfg.seed
+        nh, nch, ncsa = c.n_hca(b), c.n_chunks(b), c.n_csa(b)
+        self.hca_k.append(_randn_stored(_rng(s, 10, b), (nh, c.D), inv_sqrt_d, dt))
+        self.hca_v.append(_randn_stored(_rng(s, 11, b), (nh, c.D), inv_sqrt_d, dt))
+        self.win_k.append(_randn_stored(_rng(s, 12, b), (c.W, c.D), inv_sqrt_d, dt))
+        self.win_v.append(_randn_stored(_rng(s, 13, b), (c.W, c.D), inv_sqrt_d, dt))
+        if kv_base is None:
+            cold = _randn_stored(_rng(s, 14, b), (nch, 2, c.C, c.D), inv_sqrt_d, dt)
+        else:
+            # tile the base block with a per-sequence stride so chunks differ per (b, c)
+            idx = (np.arange(nch, dtype=np.int64) * 7 + 13 * b) % c.kv_base_chunks
+            cold = kv_base[idx].copy()
+            # make every chunk unique in its first K element (cheap) so wrong copies are detectable
+            tagv = store((((np.arange(nch) % 251) / 251.0 - 0.5) * inv_sqrt_d).astype(np.float32), dt)
+            cold[:, 0, 0, 0] = tagv
+        tail = nch * c.C - ncsa
+        if tail:
+            cold[nch - 1, :, c.C - tail:, :] = 0   # rows past n_csa: zero padding
+        self.cold_csa.append(cold)
+
+    # ---- embeddings -----------------------------------------------------------------
+    @staticmethod
+    def _plant(u: np.ndarray, r: np.ndarray, cosv: np.ndarray) -> np.ndarray:
+        """rows = cos*u + sqrt(1-cos^2)*r_perp  with r_perp unit and orthogonal to u."""
+        r_perp = r - (r @ u)[:, None] * u[None, :]
+        r_perp = _unit_rows(r_perp)
+        return cosv[:, None] * u[None, :] + np.sqrt(1.0 - cosv ** 2)[:, None] * r_perp
+
+    def needle_ids(self, b: int, trigger_idx: int) -> np.ndarray:
+        """Chunk ids carrying needles during trigger `trigger_idx` (drift every needle_period)."""
+        c = self.cfg
+        if c.n_needles == 0:
+            return np.zeros(0, dtype=np.int64)
+        epoch = trigger_idx // c.needle_period
+        key = (b, epoch)
+        if key not in self._needle_cache:
+            g = _rng(c.seed, 30, b, epoch)
+            n = min(c.n_needles, c.n_chunks(b))
+            self._needle_cache[key] = np.sort(g.choice(c.n_chunks(b), size=n, replace=False))
+        return self._needle_cache[key]
+
+    def chunk_emb(self, b: int, trigger_idx: int) -> np.ndarray:
+        """Embedding table [n_chunks, E] (stored dtype) in force at trigger `trigger_idx`."""
+        c = self.cfg
+        emb = self.base_emb[b].copy()
+        ids = self.needle_ids(b, trigger_idx)
+        if len(ids):
+            g = _rng(c.seed, 31, b, trigger_idx // c.needle_period)
+            r = g.standard_normal((len(ids), c.E))
+            rows = self._plant(self.u[b], r, np.full(len(ids), c.needle_cos))
+            emb[ids] = store(rows.astype(np.float32), c.dtype)
+        return emb
+
+    def emb_row_updates(self, b: int, trigger_idx: int) -> Optional[Tuple[np.ndarray, np.ndarray]]:
+        """(row ids, new rows) to rewrite in place when the needle epoch changes, else None."""
+        c = self.cfg
+        if c.n_needles == 0 or trigger_idx == 0 or trigger_idx % c.needle_period != 0:
+            return None
+        old = self.needle_ids(b, trigger_idx - 1)
+        new = self.needle_ids(b, trigger_idx)
+        ids = np.union1d(old, new)
+        return ids, self.chunk_emb(b, trigger_idx)[ids]
+
+    # ---- per-step dynamic inputs ----------------------------------------------------
+    def q(self, step: int) -> np.ndarray:
+        c = self.cfg
+        return _randn_stored(_rng(c.seed, 40, step), (c.B, c.H, c.D), c.q_gain / math.sqrt(c.D), c.dtype)
+
+    def kv_new(self, step: int) -> Tuple[np.ndarray, np.ndarray]:
+        c = self.cfg
+        g = _rng(c.seed, 41, step)
+        s = 1.0 / math.sqrt(c.D)
+        return _randn_stored(g, (c.B, c.D), s, c.dtype), _randn_stored(g, (c.B, c.D), s, c.dtype)
+
+    def h(self, step: int) -> np.ndarray:
+        """Hidden states [B, Dh] at global step `step` (only consumed at trigger steps)."""
+        c = self.cfg
+        g = _rng(c.seed, 42, step)
+        if c.emb_mode == "uniform":            # cfg 5: redrawn i.i.d. -> scores resampled
+            return _randn_stored(g, (c.B, c.Dh), 1.0, c.dtype)
+        out = np.empty((c.B, c.Dh), dtype=np.float32)
+        for b in range(c.B):
+            out[b] = as_f64(self.h0[b], c.dtype) + c.h_noise * g.standard_normal(c.Dh)
+        return store(out, c.dtype)
+
+    # ---- schedule helpers (integer bookkeeping of the harness, not the method) -------
+    def seq_step(self, b: int, global_step: int) -> int:
+        return self.cfg.step0(b) + global_step
+
+    def fires(self, b: int, global_step: int) -> bool:
+        return self.seq_step(b, global_step) % self.cfg.tau == 0
+
+    def trigger_index(self, b: int, global_step: int) -> int:
+        """Number of triggers of sequence b at global steps < global_step.
+
+        At a firing step this is the 0-based index of that trigger (harness bookkeeping)."""
+        c = self.cfg
+        first = (-c.step0(b)) % c.tau          # first global step at which seq b fires
+        if global_step <= first:
+            return 0
+        return (global_step - first - 1) // c.tau + 1
+
+    def has_tie_trigger(self, b: int, trigger_idx: int) -> bool:
+        c = self.cfg
+        if c.tie_frac <= 0:
+            return False
+        g = _rng(c.seed, 50, b, trigger_idx)
+        return bool(g.uniform() < c.tie_frac)
+
+    def total_cold_bytes(self) -> int:
+        return sum(x.nbytes for x in self.cold_csa)
+
+
+def plant_boundary_ties(emb: np.ndarray, order: np.ndarray, k: int, dtype: str) -> np.ndarray:
+    """Return a copy of `emb` with an exact tie and a near tie planted across the k-th rank.
+
+    `order` is a ranking of chunk ids (best first) computed by the CALLER (tests use the
+    oracle; bench.py uses any fixed permutation).  Row order[k] becomes a bit copy of row
+    order[k-1] (exact tie across the boundary: the lower chunk id must win); row
+    order[k+1] becomes that row with one low-magnitude coordinate moved by one ulp
+    (score gap ~1e-6).  SURVEY 8(d) cfg 5, R14.
+    """
+    out = emb.copy()
+    n = len(order)
+    if k < 1 or k >= n:
+        return out
+    src = order[k - 1]
+    out[order[k]] = out[src]
+    if k + 1 < n:
+        row = out[src].copy()
+        mag = np.abs(as_f64(row, dtype))
+        mag[mag == 0] = np.inf
+        j = int(np.argmin(mag))
+        if dtype == "bf16":
+            row[j] = np.uint16(int(row[j]) ^ 1) if (int(row[j]) & 0x7FFF) != 0 else row[j]
+        else:
+            row[j] = np.nextafter(row[j], np.float32(0))
+        out[order[k + 1]] = row
+    return out
