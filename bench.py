@@ -1,0 +1,378 @@
+#!/usr/bin/env python
+"""bench.py - LSA decode-step throughput on B200 through the C ABI (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (lsa_step: table swap, window append, split-K attention
++ combine, and - every tau steps - query tower, chunk scoring, top-k, residency diff, chunk fetch on
+the side stream) over one decode token of every sequence of the config.  Default workload =
+BASELINE.json configs[2] (1-based config 3: bf16, B=1, 1M-token context), the one the metric is
+quoted on.  Inputs are synthetic and seeded (paper_2606_09079_b200/workloads.py).
+
+L2 hygiene: the per-step working set at B=1 (48 MiB) fits B200's L2, so R independent replicas of the
+layer state are stepped round-robin with R * bytes/step >= 2x L2 ("inputs larger than L2"); a real
+model touches >= 21 such layers per token.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload; the oracle is otherwise only used for the `cpu_baseline` leg on rank 0.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_09079_b200.workloads import LsaWorkload, make_config, to_torch  # noqa: E402
+
+METRIC = {1: ("lsa_decode_steps_per_s_8k_ctx_fp32", "steps/s"),
+          2: ("lsa_decode_steps_per_s_128k_ctx", "steps/s"),
+          3: ("lsa_decode_steps_per_s_1m_ctx", "steps/s"),
+          4: ("lsa_decode_tokens_per_s_b32_ragged", "tokens/s"),
+          5: ("lsa_decode_steps_per_s_churn_b8_512k", "steps/s")}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d["hbm_gbs"], source="MEASURED_PEAKS.json (of measured)")
+    return dict(hbm_gbs=6650.0, source="B200_PROFILING.md fallback (of fallback)")
+
+
+# ----------------------------------------------------------------------------------------------
+# reference arm / cpu baseline: the oracle on a bounded sample
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(wl, budget_s=20.0, max_steps=24):
+    """Run the oracle as it stands from step 0 (trigger + fetch + attention) for up to max_steps steps
+    or ~budget_s seconds; returns (steps, seconds, threads)."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from lsa_harness import make_oracle
+    threads = os.cpu_count() or 1
+    try:
+        from threadpoolctl import threadpool_info
+        nt = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
+        if nt:
+            threads = max(nt)
+    except Exception:
+        pass
+    orc = make_oracle(wl)
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_steps:
+        kn, vn = wl.kv_new(n)
+        orc.run_step(wl.q(n), wl.h(n), kn, vn)
+        n += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    return n, time.perf_counter() - t0, threads
+
+
+def run_reference(args, cfg, wl):
+    name, unit = METRIC[cfg.config_id]
+    per_step_units = cfg.B if unit == "tokens/s" else 1
+    for _ in range(max(args.warmup, 0) and 1):
+        oracle_sample(wl, budget_s=1.0, max_steps=1)
+    n, secs, threads = oracle_sample(wl, budget_s=max(5.0, min(60.0, 2.0 * args.steps)), max_steps=max(2, min(args.steps, 48)))
+    val = n * per_step_units / secs
+    line = dict(metric=name, value=val, unit=unit, n_gpus=args.gpus, steps=n, warmup=1, ms_per_step=1e3 * secs / n,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload=cfg.name, B=cfg.B, L=cfg.L if cfg.B <= 2 else f"{min(cfg.L)}..{max(cfg.L)}", H=cfg.H,
+                            D=cfg.D, k=cfg.k, tau=cfg.tau),
+                cpu_baseline=dict(value=val, unit=unit, cores=threads, kind="oracle",
+                                  sample=f"oracle steps 0..{n - 1} of {cfg.name} (trigger + fetch at step 0, attention every step)"),
+                e2e=dict(value=val, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------
+class Replica:
+    def __init__(self, wl, shared, sc, sf, lsa):
+        c = wl.cfg
+        dev = shared["dev"]
+        tdt = shared["tdt"]
+        self.hot_pool = torch.zeros((c.hot_pages, 2, c.C, c.D), dtype=tdt, device=dev)
+        self.emb = [e.clone() for e in shared["emb"]]
+        self.hca_k = [x.clone() for x in shared["hca_k"]]
+        self.hca_v = [x.clone() for x in shared["hca_v"]]
+        self.win_k = [x.clone() for x in shared["win_k"]]
+        self.win_v = [x.clone() for x in shared["win_v"]]
+        seqs = [dict(cold_csa=shared["cold"][b], n_csa=c.n_csa(b), chunk_emb=self.emb[b], hca_k=self.hca_k[b],
+                     hca_v=self.hca_v[b], win_k=self.win_k[b], win_v=self.win_v[b], w_len=min(c.W, c.L[b]), w_head=0,
+                     step0=c.step0(b)) for b in range(c.B)]
+        self.ctx = lsa.LsaContext(dtype=lsa.LSA_F32 if c.dtype == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W,
+                                  Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=shared["W_q"], seqs=seqs,
+                                  recall_lag=c.recall_lag, stream_compute=sc, stream_fetch=sf,
+                                  attn_impl=shared["attn_impl"])
+        self.step = 0
+
+
+def clocks_sampler_start(dev_index):
+    f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    try:
+        p = subprocess.Popen(["nvidia-smi", f"--id={dev_index}", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                             stdout=f, stderr=subprocess.DEVNULL)
+    except Exception:
+        return None, f
+    return p, f
+
+
+def clocks_sampler_stop(p, f):
+    if p is None:
+        return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+    p.terminate()
+    try:
+        p.wait(timeout=5)
+    except Exception:
+        p.kill()
+    f.flush()
+    f.seek(0)
+    sm, smax, reasons = [], [], set()
+    for line in f.read().splitlines():
+        parts = [x.strip() for x in line.split(",")]
+        if len(parts) < 7:
+            continue
+        try:
+            sm.append(float(parts[0])); smax.append(float(parts[1]))
+        except ValueError:
+            continue
+        for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), parts[3:7]):
+            if v.lower().startswith("active"):
+                reasons.add(name)
+    f.close()
+    os.unlink(f.name)
+    return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(smax) if smax else None,
+                samples=len(sm), reasons=sorted(reasons))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1536)
+    ap.add_argument("--warmup", type=int, default=192)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--attn", default="auto", choices=["auto", "simt", "tcgen05"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--replicas", type=int, default=0)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    cfg = make_config(args.config)
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, cfg, LsaWorkload(cfg))
+        return 0
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2606_09079_b200 import lsa
+
+    wl = LsaWorkload(cfg)
+    c = cfg
+    tdt = torch.float32 if c.dtype == "f32" else torch.bfloat16
+    name, unit = METRIC[c.config_id]
+    per_step_units = c.B if unit == "tokens/s" else 1
+    props = torch.cuda.get_device_properties(dev)
+    l2 = getattr(props, "L2_cache_size", 126 * 2**20)
+    attn_bytes = c.attn_bytes_per_step()
+    R = args.replicas or max(1, math.ceil(2 * l2 / attn_bytes))
+    warmup = max(args.warmup, 3, 2 * R)
+    attn_impl = dict(auto=lsa.LSA_ATTN_AUTO, simt=lsa.LSA_ATTN_SIMT, tcgen05=lsa.LSA_ATTN_TCGEN05)[args.attn]
+
+    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, W_q=to_torch(wl.W_q, c.dtype).to(dev),
+                  cold=[to_torch(x, c.dtype).pin_memory() for x in wl.cold_csa],
+                  emb=[to_torch(wl.chunk_emb(b, 0), c.dtype).to(dev) for b in range(c.B)],
+                  hca_k=[to_torch(x, c.dtype).to(dev) for x in wl.hca_k], hca_v=[to_torch(x, c.dtype).to(dev) for x in wl.hca_v],
+                  win_k=[to_torch(x, c.dtype).to(dev) for x in wl.win_k], win_v=[to_torch(x, c.dtype).to(dev) for x in wl.win_v])
+    sc, sf = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    reps = [Replica(wl, shared, sc, sf, lsa) for _ in range(R)]
+
+    # a rotating set of per-step inputs, resident in HBM before the timed region
+    NIN = 16
+    qs = [to_torch(wl.q(i), c.dtype).to(dev) for i in range(NIN)]
+    hs = [to_torch(wl.h(i * c.tau), c.dtype).to(dev) for i in range(NIN)]
+    kns, vns = zip(*[(to_torch(a, c.dtype).to(dev), to_torch(b_, c.dtype).to(dev)) for a, b_ in (wl.kv_new(i) for i in range(NIN))])
+    out = torch.empty((c.B, c.H, c.D), dtype=tdt, device=dev)
+    # needle drift (cfg 2-4): rows to rewrite at each trigger index, staged on the device
+    drift = {}
+    max_trig = (warmup + 3 * args.steps) // (c.tau * R) + 3
+    for trig in range(1, max_trig + 1):
+        for b in range(c.B):
+            upd = wl.emb_row_updates(b, trig)
+            if upd is not None:
+                drift[(b, trig)] = (torch.from_numpy(upd[0]).to(dev), to_torch(upd[1], c.dtype).to(dev))
+    torch.cuda.synchronize()
+
+    def one_step(i, host=None):
+        r = reps[i % R]
+        t = r.step
+        if drift:
+            for b in range(c.B):
+                if wl.fires(b, t):
+                    u = drift.get((b, wl.trigger_index(b, t)))
+                    if u is not None:
+                        with torch.cuda.stream(sf):
+                            r.emb[b][u[0]] = u[1]
+        j = i % NIN
+        if host is None:
+            r.ctx.step(qs[j], hs[(t // c.tau) % NIN], kns[j], vns[j], out)
+        else:
+            r.ctx.step_host(host["q"][j], host["h"][(t // c.tau) % NIN], host["kn"][j], host["vn"][j], host["out"])
+        r.step += 1
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    def timed(n, host=None, i0=0):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        w0 = time.perf_counter()
+        e0.record(sc)
+        for i in range(n):
+            one_step(i0 + i, host)
+        e1.record(sc)
+        sf.synchronize(); sc.synchronize()
+        wall = time.perf_counter() - w0
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev)
+            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, wall
+
+    # ---- warm-up, then the device-resident timed region ----
+    for i in range(warmup):
+        one_step(i)
+    i_next = warmup
+    st0 = reps[0].ctx.stats()
+    launches0 = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps)
+    samp, sampf = clocks_sampler_start(local_rank)
+    ms, wall = timed(args.steps, i0=i_next)
+    clocks = clocks_sampler_stop(samp, sampf)
+    i_next += args.steps
+    launches = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps) - launches0
+    value = world * args.steps * per_step_units / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers (H2D + D2H inside the timed region) ----
+    pin = lambda t: t.cpu().pin_memory()
+    host = dict(q=[pin(x) for x in qs], h=[pin(x) for x in hs], kn=[pin(x) for x in kns], vn=[pin(x) for x in vns],
+                out=torch.empty((c.B, c.H, c.D), dtype=tdt).pin_memory())
+    for i in range(max(3, R)):
+        one_step(i_next + i, host)
+    i_next += max(3, R)
+    n_e2e = max(64, args.steps // 4)
+    ms_e2e, _ = timed(n_e2e, host, i0=i_next)
+    i_next += n_e2e
+    es = 4 if c.dtype == "f32" else 2
+    h2d = (c.B * c.H * c.D + c.B * c.Dh + 2 * c.B * c.D) * es
+    d2h = c.B * c.H * c.D * es
+    e2e_value = world * n_e2e * per_step_units / (ms_e2e * 1e-3)
+
+    # ---- per-kernel device time of the dominant kernel (CUDA events on its own stream) ----
+    n_prof = min(args.steps, 512)
+    for r in reps:
+        r.ctx.profile_enable(n_prof // R + 8)
+    for i in range(n_prof):
+        one_step(i_next + i)
+    i_next += n_prof
+    phases = {}
+    for r in reps:
+        for ph, v in r.ctx.profile_read().items():
+            d = phases.setdefault(ph, dict(ms=0.0, count=0))
+            d["ms"] += v["ms"]; d["count"] += v["count"]
+        r.ctx.profile_enable(0)
+    attn_ms = phases["attention"]["ms"] / max(phases["attention"]["count"], 1)
+    comb_ms = phases["combine"]["ms"] / max(phases["combine"]["count"], 1) if phases["combine"]["count"] else 0.0
+    peaks = load_peaks()
+    achieved = attn_bytes / (attn_ms * 1e-3) / 1e9
+    stats = reps[0].ctx.stats()
+    roofline = dict(bound="hbm", achieved=achieved, peak=peaks["hbm_gbs"], unit="GB/s", frac=achieved / peaks["hbm_gbs"],
+                    traffic=None, kernel="lsa split-K decode attention (S7)" + (" incl. combine" if comb_ms == 0.0 else ""),
+                    algorithmic_bytes_per_launch=attn_bytes, kernel_ms=attn_ms, combine_ms=comb_ms,
+                    step_ms=ms / args.steps, frac_of_step=achieved and (attn_bytes / (ms / args.steps * 1e-3) / 1e9) / peaks["hbm_gbs"],
+                    peak_source=peaks["source"], frac_of_nominal_8tbs=achieved / 8000.0)
+
+    # ---- chunk fetch: H2D link peak (pinned cudaMemcpyAsync) and the device-pull fetch kernel ----
+    fetch = None
+    if rank == 0:
+        src = torch.empty(256 * 2**20, dtype=torch.uint8).pin_memory()
+        dst = torch.empty(256 * 2**20, dtype=torch.uint8, device=dev)
+        best = 0.0
+        for _ in range(6):
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); dst.copy_(src, non_blocking=True); b_.record(); torch.cuda.synchronize()
+            best = max(best, src.numel() / (a.elapsed_time(b_) * 1e-3) / 1e9)
+        r = reps[0]
+        r.ctx.profile_enable(64)
+        nb = 0
+        g = np.random.default_rng(1)
+        n_ch = c.n_chunks(0)
+        for it in range(8):
+            sel = np.full((1, c.k), -1, dtype=np.int32)
+            ke = c.k_eff(0)
+            sel[0, :ke] = g.choice(n_ch, size=ke, replace=False)
+            b0 = r.ctx.stats()["bytes_fetched"]
+            r.ctx.fetch_chunks([0], torch.from_numpy(sel).to(dev))
+            r.ctx.commit_tables()
+            nb += r.ctx.stats()["bytes_fetched"] - b0
+        pr = r.ctx.profile_read()
+        r.ctx.profile_enable(0)
+        fms = pr["fetch"]["ms"]
+        fetch = dict(h2d_peak_gbs=best, fetch_gbs=(nb / (fms * 1e-3) / 1e9) if fms > 0 else None,
+                     frac_of_h2d_peak=(nb / (fms * 1e-3) / 1e9 / best) if fms > 0 else None, bytes=nb, kernel_ms=fms,
+                     mode="device-pull kernel over the mapped pinned cold pool",
+                     residency_ms_per_trigger=pr["residency"]["ms"] / max(pr["residency"]["count"], 1))
+        del src, dst
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n, secs, threads = oracle_sample(wl, budget_s=15.0, max_steps=24)
+        cpu_baseline = dict(value=n * per_step_units / secs, unit=unit, cores=threads, kind="oracle",
+                            sample=f"oracle steps 0..{n - 1} of {c.name}: trigger + fetch at step 0, attention every step; {secs:.1f} s")
+
+    if rank == 0:
+        line = dict(metric=name, value=value, unit=unit, n_gpus=world, steps=args.steps, warmup=warmup,
+                    ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype=c.dtype, data="synthetic",
+                    config=dict(workload=c.name, B=c.B, L=c.L if c.B <= 2 else f"{min(c.L)}..{max(c.L)}", H=c.H, D=c.D, C=c.C,
+                                W=c.W, k=c.k, tau=c.tau, hot_pages=c.hot_pages, recall_lag=c.recall_lag,
+                                l2_policy=f"{R} layer-state replicas stepped round-robin; {R}x{attn_bytes / 2**20:.1f} MiB attended "
+                                          f"per rotation vs L2 {l2 / 2**20:.0f} MiB (inputs larger than L2)",
+                                parallelism=f"dp{world} (independent sequences per rank, no collective)",
+                                attn_impl={1: "simt", 2: "tcgen05"}.get(stats["attn_impl"], "?"), attn_ctas=stats["attn_ctas"]),
+                    e2e=dict(value=e2e_value, unit=unit, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=n_e2e,
+                             ms_per_step=ms_e2e / n_e2e),
+                    gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
+                    phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
+                    fetch=fetch, wall_s=wall,
+                    tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
+        print(json.dumps(line))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

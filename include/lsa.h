@@ -1,0 +1,193 @@
+/* lsa.h - C ABI of liblsa: the decode hot path of Lookahead Sparse Attention (LSA),
+ * arxiv/paper_2606_09079 "FlashMemory-DeepSeek-V4", hand-written CUDA for sm_100a (B200).
+ *
+ * Citations: `P:n` = PAPER.md line n; `BJ` = BASELINE.json north_star/configs; `R#` = the
+ * numbered readings in DESIGN.md.  Every step S0..S8 of DESIGN.md runs in CUDA kernels of this
+ * library; there is no CPU fallback.  No torch / C++ types cross this boundary.
+ *
+ * The path (BJ north_star):
+ *   every tau decode steps (S0) the Memory Indexer maps the hidden state h to a query embedding
+ *   (S1), scores it against one embedding per CSA chunk (S2), a per-sequence top-k picks the
+ *   chunks (S3), chunks missing from HBM are given pages of a shared paged hot pool (S4) and
+ *   copied from the pinned-host cold pool on a side stream (S5); the new page table becomes
+ *   visible `recall_lag` steps later (S6); every step split-K decode attention runs over
+ *   all HCA entries (+) the selected resident chunks (+) the window ring (S7) and a combine
+ *   kernel merges the splits (S8).
+ *
+ * Conventions
+ *   - All functions return LSA_OK (0) or a negative lsa_status; lsa_last_error gives text.
+ *   - "DEVICE" pointers are CUDA device memory of the current device, "PINNED HOST" is page-locked
+ *     host memory (cudaHostAlloc / cudaHostRegister, e.g. torch pin_memory), "HOST" is any host
+ *     memory.  Every buffer is CALLER-OWNED and must outlive the context; the library owns only
+ *     the opaque context (page tables, LRU state, split-K scratch, events).
+ *   - dtype is LSA_F32 or LSA_BF16 for q, K, V, W_q, h, chunk embeddings and out; scores, lse
+ *     and all accumulation are fp32.
+ *   - Row-major, innermost dimension contiguous, no padding, 16-byte aligned base pointers.
+ *   - The five path calls only ENQUEUE work on the caller's two streams and return; they never
+ *     block the host.  lsa_sync / lsa_get_* / lsa_step_host block.
+ *   - Not thread-safe per context.
+ */
+#ifndef LSA_H_
+#define LSA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LSA_VERSION 1
+
+typedef struct lsa_ctx lsa_ctx; /* opaque */
+
+enum lsa_status {
+  LSA_OK = 0,
+  LSA_ERR_INVALID_ARG = -1,    /* bad shape / null pointer / non-pinned cold pool / k > pages ... */
+  LSA_ERR_CUDA = -2,           /* a CUDA runtime call failed (text in lsa_last_error)             */
+  LSA_ERR_POOL_EXHAUSTED = -3, /* S4 found no unpinned page (cannot happen if hot_pages >= 2*sum k) */
+  LSA_ERR_OOM = -4,
+  LSA_ERR_STATE = -5,          /* call sequence not allowed (e.g. destroyed ctx)                  */
+  LSA_ERR_UNSUPPORTED = -6     /* shape has no compiled kernel */
+};
+
+enum lsa_dtype { LSA_F32 = 0, LSA_BF16 = 1 };
+enum lsa_attn_impl { LSA_ATTN_AUTO = 0, LSA_ATTN_SIMT = 1, LSA_ATTN_TCGEN05 = 2 };
+enum lsa_fetch_mode { LSA_FETCH_DEVICE_PULL = 0, LSA_FETCH_MEMCPY = 1 };
+
+/* Shape and resources of one LSA layer shared by B sequences (BJ configs). */
+typedef struct lsa_config {
+  uint32_t struct_size;  /* = sizeof(lsa_config), ABI check                                     */
+  int32_t dtype;         /* lsa_dtype                                                           */
+  int32_t B;             /* sequences                                                           */
+  int32_t H;             /* query heads, all sharing ONE K and ONE V head (MQA; R19)       */
+  int32_t D;             /* K/V/q head dim                                                      */
+  int32_t C;             /* compressed entries per CSA chunk = rows per page                    */
+  int32_t W;             /* window ring capacity in raw tokens ("last 8K tokens"; R6)      */
+  int32_t Dh;            /* indexer hidden size d                                        */
+  int32_t E;             /* query / chunk embedding dim (BJ)                                    */
+  int32_t k;             /* chunks selected per sequence = K_max (R2)                    */
+  int32_t tau;           /* trigger interval (tau = 64)                                   */
+  int32_t recall_lag;    /* 0: new table visible at the trigger step; 1: at t+1 (R9)      */
+  float sm_scale;        /* softmax scale; 0 -> 1/sqrt(D) (R18)                                 */
+  int64_t hot_pages;     /* P: pages in the hot pool; must be >= 2 * sum_b min(k, n_chunks_b)   */
+  void* hot_pool;        /* DEVICE [P][2][C][D]: page = K block [C][D] then V block [C][D]      */
+  const void* W_q;       /* DEVICE [E][Dh] query-tower weight (P:61-65 collapsed; R1)           */
+  void* stream_compute;  /* cudaStream_t: S6-S8 (and S1-S5 when recall_lag == 0 waits on them)  */
+  void* stream_fetch;    /* cudaStream_t: side band for S1-S5 ("async side band")         */
+  int32_t attn_impl;     /* lsa_attn_impl; AUTO picks tcgen05 for bf16,H=64,D=512,C=128          */
+  int32_t fetch_mode;    /* lsa_fetch_mode; DEVICE_PULL keeps the whole trigger path on device   */
+  int32_t max_ctas;      /* 0 -> one split-K wave sized from the SM count                       */
+  int32_t reserved;
+} lsa_config;
+
+/* One sequence (CPU cold mirror + always-resident tiers).  n_chunks = ceil(n_csa/C);
+ * the last chunk may be partial: rows >= n_csa - c*C of it are never attended (R22). */
+typedef struct lsa_seq_desc {
+  const void* cold_csa;  /* PINNED HOST [n_chunks][2][C][D]: chunk c = one page image            */
+  int64_t n_csa;         /* valid compressed (CSA) entries                                      */
+  const void* chunk_emb; /* DEVICE [n_chunks][E], rows L2-normalised by the producer (R3)        */
+  const void* hca_k;     /* DEVICE [n_hca][D] heavily-compressed (128:1) keys, always resident   */
+  const void* hca_v;     /* DEVICE [n_hca][D]                                                   */
+  int64_t n_hca;
+  void* win_k;           /* DEVICE ring [W][D] raw-token window keys                            */
+  void* win_v;           /* DEVICE ring [W][D]                                                  */
+  int32_t w_len;         /* filled ring rows [0, w_len) are attended                            */
+  int32_t w_head;        /* next ring slot to be written by lsa_step(k_new, v_new)              */
+  int64_t step0;         /* initial decode-step counter (staggered triggers, R26)               */
+} lsa_seq_desc;
+
+typedef struct lsa_stats {
+  uint64_t triggers;      /* per-sequence trigger events processed by S4                         */
+  uint64_t hits;          /* selected chunks already resident                                   */
+  uint64_t misses;        /* selected chunks fetched from the cold pool                          */
+  uint64_t evictions;     /* pages whose previous owner was evicted                              */
+  uint64_t bytes_fetched; /* misses * page_bytes                                                */
+  uint64_t steps;         /* lsa_step calls                                                     */
+  uint64_t attn_launches; /* kernels launched by S7+S8                                          */
+  uint64_t index_launches;/* kernels launched by S1-S5                                          */
+  int32_t pool_error;     /* nonzero if S4 ever ran out of pages                                 */
+  int32_t attn_impl;      /* implementation actually in use (lsa_attn_impl)                      */
+  int32_t attn_ctas;      /* CTAs of the last S7 launch                                          */
+  int32_t reserved;
+} lsa_stats;
+
+/* Create a context.  All pages start FREE, every chunk starts in the cold pool, the attended
+ * page table of every sequence is empty (BJ cfg 1 "all chunks start in the host cold pool"; R10).
+ * Errors: INVALID_ARG for null pointers, B/H/D/C/k/tau < 1, D % 8 != 0, hot_pages too small,
+ * non-pinned cold_csa; UNSUPPORTED if no kernel is compiled for (dtype,H,D). */
+int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs /* HOST [B] */, lsa_ctx** out);
+
+/* S1-S3 for n sequences: q_hat = normalize(W_q h_i), score_c = q_hat . Emb[c]
+ * (P:71-75), first min(k, n_chunks) chunk ids by (score desc, chunk idx asc) (R2, R14).
+ *   h         DEVICE [n][Dh], row i belongs to sequence seq_ids[i]
+ *   seq_ids   HOST   [n], strictly ascending
+ *   sel_idx   DEVICE [n][k] int32 out, score order, unused slots -1
+ *   sel_score DEVICE [n][k] fp32 out (may be NULL), unused slots -inf
+ * Pure: mutates no pool state.  Runs on stream_fetch. */
+int lsa_index_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n,
+                     int32_t* sel_idx, float* sel_score);
+
+/* S4-S5 for n sequences (ascending seq_ids): residency diff against the hot pool, page
+ * allocation (never-used pages lowest index first, else LRU by (last_used, page), never a page
+ * of any current or staged table; R11-R12), copy of every missing chunk cold -> hot on
+ * stream_fetch, and staging of the next page table in ascending chunk id (R13).  The
+ * staged table becomes current at the first lsa_step / lsa_decode_attention whose per-sequence
+ * step counter is >= (counter at this call) + recall_lag, or at lsa_commit_tables.
+ *   sel_idx DEVICE [n][k] int32 (-1 = unused slot), e.g. from lsa_index_select. */
+int lsa_fetch_chunks(lsa_ctx* ctx, const int32_t* seq_ids, int32_t n, const int32_t* sel_idx);
+
+/* Make every staged page table current now (stream_compute waits for its fetch). */
+int lsa_commit_tables(lsa_ctx* ctx);
+
+/* S6-S8 for all B sequences on stream_compute: (swap due tables, then) per head
+ * softmax(sm_scale q K^T) V over HCA rows (+) rows [0, valid(c)) of every page of the current
+ * table (+) window rows [0, w_len)  - one softmax over the union (R5).
+ *   q   DEVICE [B][H][D]   out DEVICE [B][H][D] (dtype)   lse DEVICE [B][H] fp32 or NULL.
+ * A sequence with no keys gets out = 0, lse = -inf.  Does not advance step counters. */
+int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, float* lse);
+
+/* One decode step for all sequences:
+ *  (a) staged tables that are due become current;  (b) sequences with step_b % tau == 0 run
+ *  S1-S5 on stream_fetch with h;  (c) recall_lag == 0: their tables become current;
+ *  (d) k_new/v_new (DEVICE [B][D], or both NULL) are written to ring slot w_head, so the new
+ *  token attends to itself;  (e) attention + combine -> out;  (f) step_b += 1.
+ *   h DEVICE [B][Dh] (row b = sequence b; only read at trigger steps; may be NULL otherwise). */
+int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
+             void* out);
+
+/* lsa_step with HOST buffers (pinned recommended): copies q,h,k_new,v_new host->device, runs the
+ * step, copies out device->host and blocks until it has landed.  Used for end-to-end timing. */
+int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new,
+                  const void* v_new, void* out);
+
+/* Replace the embedding table pointer of one sequence (DEVICE [n_chunks][E]). */
+int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb);
+
+/* Blocking read-back of a page table.  which: 0 = current, 1 = staged.  chunk_idx/page HOST [k].
+ * *n = entries (0 if none / nothing staged).  Entries are in ascending chunk id. */
+int lsa_get_page_table(lsa_ctx* ctx, int32_t seq, int32_t which, int32_t* chunk_idx,
+                       int32_t* page, int32_t* n);
+
+/* Blocking: page_of[seq][0..n_chunks) -> HOST int32 (-1 = cold). */
+int lsa_get_residency(lsa_ctx* ctx, int32_t seq, int32_t* page_of);
+
+int lsa_get_stats(lsa_ctx* ctx, lsa_stats* out); /* blocking */
+
+/* Per-phase device timing with CUDA events recorded on the launching stream (off by default;
+ * each enabled launch costs two event records).  capacity = event pairs kept per phase; 0 disables.
+ * lsa_profile_read blocks, returns the summed milliseconds and launch counts per phase since the
+ * last read and rearms.  Phases: */
+enum lsa_phase { LSA_PH_PRESTEP = 0, LSA_PH_ATTENTION = 1, LSA_PH_COMBINE = 2, LSA_PH_INDEX = 3,
+                 LSA_PH_RESIDENCY = 4, LSA_PH_FETCH = 5, LSA_PH_COUNT = 6 };
+int lsa_profile_enable(lsa_ctx* ctx, int32_t capacity);
+int lsa_profile_read(lsa_ctx* ctx, double* ms_sum /* HOST [6] */, int64_t* count /* HOST [6] */);
+int lsa_get_step(lsa_ctx* ctx, int32_t seq, int64_t* step);
+int lsa_sync(lsa_ctx* ctx);                      /* waits for both streams, reports device errors */
+const char* lsa_last_error(lsa_ctx* ctx);        /* ctx may be NULL: last init error             */
+void lsa_destroy(lsa_ctx* ctx);
+int lsa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSA_H_ */

@@ -1,0 +1,588 @@
+// lsa_api.cu - the C ABI of liblsa (include/lsa.h): host-side orchestration only.
+// Every step of the path runs in the kernels of lsa_index.cu / lsa_residency.cu /
+// lsa_attn_simt.cu / lsa_attn_tc.cu; this file validates arguments, keeps deterministic host
+// mirrors of the per-sequence counters (so no call ever waits for the device), orders the two
+// streams with events and launches.  Step order: DESIGN.md "Step order".
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/lsa.h"
+#include "lsa_attn_tc.h"
+#include "lsa_kernels.h"
+
+using namespace lsa;
+
+static thread_local std::string g_init_error;
+
+struct lsa_ctx {
+  lsa_config cfg{};
+  int B = 0, k = 0;
+  float sm_scale = 0.f;
+  long long page_bytes = 0;
+  int elem = 0;
+  cudaStream_t sc = nullptr, sf = nullptr;
+  cudaEvent_t ev_fetch = nullptr, ev_compute = nullptr;
+  int n_sms = 0;
+  // device state
+  SeqDev* d_seqs = nullptr;
+  PoolDev pool{};
+  std::vector<void*> owned;          // cudaMalloc'ed blocks to free
+  std::vector<SeqDev> seq_host;      // immutable fields (host copy)
+  int total_chunks = 0, n_chunks_max = 0;
+  // host mirrors (deterministic: advanced by the same rules the kernels apply)
+  std::vector<long long> step, visible_at;
+  std::vector<char> pending;
+  std::vector<int> k_eff;
+  // index scratch
+  float* d_z = nullptr;
+  float* d_scores = nullptr;
+  int32_t* d_sel = nullptr;
+  // attention
+  int attn_impl = LSA_ATTN_SIMT;
+  AttnGeom geom{};
+  float* part_o = nullptr;
+  float* part_ml = nullptr;
+  int fetch_ctas = 0;
+  TcPlan* tc = nullptr;
+  // host-buffer staging (lsa_step_host)
+  void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr;
+  // optional per-phase event timing
+  int prof_cap = 0;
+  std::vector<cudaEvent_t> prof_ev[LSA_PH_COUNT];   // 2*cap events per phase
+  int prof_n[LSA_PH_COUNT] = {0, 0, 0, 0, 0, 0};
+  // bookkeeping
+  unsigned long long n_steps = 0, attn_launches = 0, index_launches = 0;
+  int last_attn_ctas = 0;
+  std::string err;
+};
+
+#define LSA_FAIL(ctx, code, ...)                          \
+  do {                                                    \
+    char _b[512];                                         \
+    snprintf(_b, sizeof(_b), __VA_ARGS__);                \
+    if (ctx) (ctx)->err = _b; else g_init_error = _b;     \
+    return (code);                                        \
+  } while (0)
+
+#define LSA_CUDA(ctx, expr)                                                                   \
+  do {                                                                                        \
+    cudaError_t _e = (expr);                                                                  \
+    if (_e != cudaSuccess)                                                                    \
+      LSA_FAIL(ctx, LSA_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+  } while (0)
+
+// Records a start event now and an end event at scope exit on `st` when profiling is enabled.
+struct ProfScope {
+  lsa_ctx* c; int ph; cudaStream_t st; bool on;
+  ProfScope(lsa_ctx* c_, int ph_, cudaStream_t st_) : c(c_), ph(ph_), st(st_), on(false) {
+    if (c->prof_cap > 0 && c->prof_n[ph] < c->prof_cap) {
+      on = true;
+      cudaEventRecord(c->prof_ev[ph][2 * c->prof_n[ph]], st);
+    }
+  }
+  ~ProfScope() {
+    if (on) {
+      cudaEventRecord(c->prof_ev[ph][2 * c->prof_n[ph] + 1], st);
+      c->prof_n[ph] += 1;
+    }
+  }
+};
+
+template <typename T>
+static int dev_alloc(lsa_ctx* c, T** p, size_t n, bool zero = true) {
+  void* q = nullptr;
+  size_t bytes = std::max<size_t>(n, 1) * sizeof(T);
+  cudaError_t e = cudaMalloc(&q, bytes);
+  if (e != cudaSuccess) LSA_FAIL(c, LSA_ERR_OOM, "cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+  if (zero) {
+    e = cudaMemset(q, 0, bytes);
+    if (e != cudaSuccess) LSA_FAIL(c, LSA_ERR_CUDA, "cudaMemset failed: %s", cudaGetErrorString(e));
+  }
+  c->owned.push_back(q);
+  *p = reinterpret_cast<T*>(q);
+  return LSA_OK;
+}
+
+extern "C" int lsa_version(void) { return LSA_VERSION; }
+
+extern "C" const char* lsa_last_error(lsa_ctx* ctx) { return ctx ? ctx->err.c_str() : g_init_error.c_str(); }
+
+extern "C" void lsa_destroy(lsa_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->sc) cudaStreamSynchronize(ctx->sc);
+  if (ctx->sf) cudaStreamSynchronize(ctx->sf);
+  if (ctx->tc) tc_destroy(ctx->tc);
+  for (void* p : ctx->owned) cudaFree(p);
+  if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
+  if (ctx->ev_compute) cudaEventDestroy(ctx->ev_compute);
+  for (auto& v : ctx->prof_ev)
+    for (cudaEvent_t e : v) cudaEventDestroy(e);
+  delete ctx;
+}
+
+static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs) {
+  c->cfg = *cfg;
+  const int B = cfg->B, H = cfg->H, D = cfg->D, C = cfg->C, k = cfg->k;
+  c->B = B;
+  c->k = k;
+  c->elem = cfg->dtype == LSA_F32 ? 4 : 2;
+  c->page_bytes = 2ll * C * D * c->elem;
+  c->sm_scale = cfg->sm_scale > 0.f ? cfg->sm_scale : 1.0f / std::sqrt((float)D);
+  c->sc = (cudaStream_t)cfg->stream_compute;
+  c->sf = (cudaStream_t)cfg->stream_fetch;
+  int dev = 0;
+  LSA_CUDA(c, cudaGetDevice(&dev));
+  LSA_CUDA(c, cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev));
+  LSA_CUDA(c, cudaEventCreateWithFlags(&c->ev_fetch, cudaEventDisableTiming));
+  LSA_CUDA(c, cudaEventCreateWithFlags(&c->ev_compute, cudaEventDisableTiming));
+
+  c->seq_host.resize(B);
+  c->step.resize(B);
+  c->visible_at.assign(B, 0);
+  c->pending.assign(B, 0);
+  c->k_eff.resize(B);
+  long long sum_k = 0, total_keys_max = 0, n_keys_max = 0;
+  for (int b = 0; b < B; ++b) {
+    const lsa_seq_desc& s = seqs[b];
+    if (s.n_csa < 0 || s.n_hca < 0 || s.w_len < 0 || s.w_len > cfg->W || s.w_head < 0 || s.w_head >= std::max(cfg->W, 1))
+      LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: bad n_csa/n_hca/w_len/w_head", b);
+    const long long n_chunks = (s.n_csa + C - 1) / C;
+    if (n_chunks > 0 && (!s.cold_csa || !s.chunk_emb)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null cold_csa/chunk_emb", b);
+    if (s.n_hca > 0 && (!s.hca_k || !s.hca_v)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null hca_k/hca_v", b);
+    if (cfg->W > 0 && (!s.win_k || !s.win_v)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null win_k/win_v", b);
+    SeqDev d{};
+    if (n_chunks > 0) {
+      cudaPointerAttributes at{};
+      cudaError_t e = cudaPointerGetAttributes(&at, s.cold_csa);
+      if (e != cudaSuccess || at.type != cudaMemoryTypeHost || !at.devicePointer) {
+        cudaGetLastError();
+        LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: cold_csa must be pinned (page-locked, mapped) host memory", b);
+      }
+      d.cold = at.devicePointer;
+    }
+    d.emb = s.chunk_emb;
+    d.hca_k = s.hca_k;
+    d.hca_v = s.hca_v;
+    d.win_k = s.win_k;
+    d.win_v = s.win_v;
+    d.n_csa = s.n_csa;
+    d.n_chunks = (int)n_chunks;
+    d.n_hca = (int)s.n_hca;
+    d.k_eff = (int)std::min<long long>(k, n_chunks);
+    d.page_of_off = c->total_chunks;
+    d.w_len = s.w_len;
+    d.w_head = s.w_head;
+    c->total_chunks += (int)n_chunks;
+    c->n_chunks_max = std::max(c->n_chunks_max, (int)n_chunks);
+    c->seq_host[b] = d;
+    c->step[b] = s.step0;
+    c->k_eff[b] = d.k_eff;
+    sum_k += d.k_eff;
+    const long long nk = s.n_hca + (long long)d.k_eff * C + cfg->W;
+    total_keys_max += nk;
+    n_keys_max = std::max(n_keys_max, nk);
+  }
+  if (cfg->hot_pages < 2 * sum_k)
+    LSA_FAIL(c, LSA_ERR_INVALID_ARG, "hot_pages=%lld < 2*sum_b min(k,n_chunks_b)=%lld (current + staged tables are pinned)",
+             (long long)cfg->hot_pages, 2 * sum_k);
+  if (cfg->hot_pages > (1ll << kPageBits)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "hot_pages > 2^%d", kPageBits);
+
+  // ---- device state ----
+  const int P = (int)cfg->hot_pages;
+  int rc;
+  if ((rc = dev_alloc(c, &c->d_seqs, B))) return rc;
+  LSA_CUDA(c, cudaMemcpy(c->d_seqs, c->seq_host.data(), sizeof(SeqDev) * B, cudaMemcpyHostToDevice));
+  if ((rc = dev_alloc(c, &c->pool.page_of, c->total_chunks, false))) return rc;
+  LSA_CUDA(c, cudaMemset(c->pool.page_of, 0xff, sizeof(int) * std::max(c->total_chunks, 1)));
+  if ((rc = dev_alloc(c, &c->pool.owner_seq, P, false))) return rc;
+  LSA_CUDA(c, cudaMemset(c->pool.owner_seq, 0xff, sizeof(int) * P));
+  if ((rc = dev_alloc(c, &c->pool.owner_chunk, P))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.last_used, P))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.pin_mark, P))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.tbl_chunk, (size_t)B * 2 * k))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.tbl_page, (size_t)B * 2 * k))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.fetch_src, (size_t)B * k))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.fetch_page, (size_t)B * k))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.counters, 8))) return rc;
+  if ((rc = dev_alloc(c, &c->pool.epoch, 1))) return rc;
+  // ---- index scratch ----
+  if ((rc = dev_alloc(c, &c->d_z, (size_t)B * cfg->E))) return rc;
+  if ((rc = dev_alloc(c, &c->d_scores, (size_t)B * std::max(c->n_chunks_max, 1)))) return rc;
+  if ((rc = dev_alloc(c, &c->d_sel, (size_t)B * k))) return rc;
+
+  // ---- attention implementation + split geometry ----
+  int impl = cfg->attn_impl;
+  const bool tc_ok = tc_supported(cfg->dtype, H, D, C);
+  if (impl == LSA_ATTN_AUTO) impl = tc_ok ? LSA_ATTN_TCGEN05 : LSA_ATTN_SIMT;
+  if (impl == LSA_ATTN_TCGEN05 && !tc_ok)
+    LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "tcgen05 attention needs bf16, H=64, D=512, C=128 (got dtype=%d H=%d D=%d C=%d)", cfg->dtype, H, D, C);
+  if (impl == LSA_ATTN_SIMT && !simt_supported(cfg->dtype, H, D))
+    LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "no SIMT attention kernel compiled for H=%d D=%d", H, D);
+  c->attn_impl = impl;
+  if (impl == LSA_ATTN_SIMT) {
+    int occ = 0;
+    LSA_CUDA(c, simt_max_ctas_per_sm(cfg->dtype, H, D, k, &occ));
+    if (occ < 1) LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "SIMT attention kernel does not fit on an SM for H=%d D=%d", H, D);
+    const int target = cfg->max_ctas > 0 ? cfg->max_ctas : c->n_sms * occ;
+    const int tile = simt_tile_keys();
+    long long kpc = (total_keys_max + target - 1) / std::max(target, 1);
+    kpc = std::max<long long>(tile, (kpc + tile - 1) / tile * tile);
+    c->geom.keys_per_cta = (int)kpc;
+    c->geom.s_max = (int)std::max<long long>(1, (n_keys_max + kpc - 1) / kpc);
+    if ((rc = dev_alloc(c, &c->part_o, (size_t)B * c->geom.s_max * H * D, false))) return rc;
+    if ((rc = dev_alloc(c, &c->part_ml, (size_t)B * c->geom.s_max * H * 2, false))) return rc;
+  } else {
+    std::vector<long long> nk(B);
+    for (int b = 0; b < B; ++b) nk[b] = seqs[b].n_hca + (long long)c->k_eff[b] * C + cfg->W;
+    TcInit ti{};
+    ti.B = B; ti.k = k; ti.W = cfg->W; ti.P = P; ti.n_sms = c->n_sms; ti.max_ctas = cfg->max_ctas;
+    ti.hot_pool = cfg->hot_pool; ti.seq_host = c->seq_host.data(); ti.d_seqs = c->d_seqs; ti.pool = c->pool;
+    ti.sm_scale = c->sm_scale;
+    std::string msg;
+    int trc = tc_create(ti, &c->tc, &msg);
+    if (trc != 0) LSA_FAIL(c, trc, "tcgen05 attention init failed: %s", msg.c_str());
+  }
+  c->fetch_ctas = std::max(8, std::min(64, c->n_sms / 2));
+  LSA_CUDA(c, cudaDeviceSynchronize());
+  return LSA_OK;
+}
+
+extern "C" int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs, lsa_ctx** out) {
+  if (!cfg || !seqs || !out) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "null argument");
+  *out = nullptr;
+  if (cfg->struct_size != sizeof(lsa_config))
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "lsa_config.struct_size=%u, library expects %zu", cfg->struct_size, sizeof(lsa_config));
+  if (cfg->dtype != LSA_F32 && cfg->dtype != LSA_BF16) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad dtype %d", cfg->dtype);
+  if (cfg->B < 1 || cfg->B > 1024 || cfg->H < 1 || cfg->D < 1 || cfg->C < 1 || cfg->W < 0 || cfg->Dh < 1 || cfg->E < 1)
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "B (1..1024), H, D, C, Dh, E must be >= 1 and W >= 0");
+  if (cfg->k < 1 || cfg->k > kMaxK) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "k must be in [1, %d]", kMaxK);
+  if (cfg->tau < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "tau must be >= 1");
+  if (cfg->recall_lag != 0 && cfg->recall_lag != 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "recall_lag must be 0 or 1");
+  if (cfg->D % 8 || cfg->Dh % 8 || cfg->E % 8) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "D, Dh, E must be multiples of 8 (16-byte vector loads)");
+  if (!cfg->hot_pool || !cfg->W_q) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "null hot_pool / W_q");
+  if (cfg->hot_pages < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "hot_pages must be >= 1");
+  if (cfg->fetch_mode != LSA_FETCH_DEVICE_PULL && cfg->fetch_mode != LSA_FETCH_MEMCPY)
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad fetch_mode");
+  lsa_ctx* c = new (std::nothrow) lsa_ctx();
+  if (!c) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_OOM, "out of host memory");
+  int rc = init_impl(c, cfg, seqs);
+  if (rc != LSA_OK) {
+    g_init_error = c->err;
+    lsa_destroy(c);
+    return rc;
+  }
+  *out = c;
+  return LSA_OK;
+}
+
+// ---- S1-S3 ------------------------------------------------------------------------------------
+// rows[i] = row of `h` holding the hidden state of sequence ids[i]
+static int index_select_impl(lsa_ctx* c, const void* h, const int* ids, const int* rows, int n, int32_t* sel_idx,
+                             float* sel_score) {
+  const lsa_config& cfg = c->cfg;
+  for (int off = 0; off < n; off += kFireMax) {
+    const int m = std::min(kFireMax, n - off);
+    FireList fire{}, hrows{};
+    fire.n = hrows.n = m;
+    for (int i = 0; i < m; ++i) { fire.ids[i] = ids[off + i]; hrows.ids[i] = rows[off + i]; }
+    ProfScope prof(c, LSA_PH_INDEX, c->sf);
+    LSA_CUDA(c, launch_qtower(cfg.dtype, cfg.W_q, h, hrows, c->d_z, cfg.E, cfg.Dh, c->sf));
+    LSA_CUDA(c, launch_scores(cfg.dtype, c->d_seqs, fire, c->d_z, c->d_scores, cfg.E, std::max(c->n_chunks_max, 1), c->sf));
+    LSA_CUDA(c, launch_topk(c->d_seqs, fire, c->d_scores, std::max(c->n_chunks_max, 1), c->k,
+                            sel_idx + (size_t)off * c->k, sel_score ? sel_score + (size_t)off * c->k : nullptr, c->sf));
+    c->index_launches += 3;
+  }
+  return LSA_OK;
+}
+
+static int check_ids(lsa_ctx* c, const int32_t* seq_ids, int n) {
+  if (!seq_ids || n < 1 || n > c->B) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq_ids null or n out of range");
+  for (int i = 0; i < n; ++i) {
+    if (seq_ids[i] < 0 || seq_ids[i] >= c->B) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq id %d out of range", seq_ids[i]);
+    if (i && seq_ids[i] <= seq_ids[i - 1]) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq_ids must be strictly ascending");
+  }
+  return LSA_OK;
+}
+
+extern "C" int lsa_index_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n, int32_t* sel_idx,
+                                float* sel_score) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!h || !sel_idx) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null h / sel_idx");
+  int rc = check_ids(ctx, seq_ids, n);
+  if (rc) return rc;
+  std::vector<int> rows(n);
+  for (int i = 0; i < n; ++i) rows[i] = i;
+  return index_select_impl(ctx, h, seq_ids, rows.data(), n, sel_idx, sel_score);
+}
+
+// ---- S4-S5 ------------------------------------------------------------------------------------
+static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx) {
+  const lsa_config& cfg = c->cfg;
+  // the side band must see the tables as of "now" on the compute stream, and may not evict pages
+  // an earlier attention launch is still reading
+  LSA_CUDA(c, cudaEventRecord(c->ev_compute, c->sc));
+  LSA_CUDA(c, cudaStreamWaitEvent(c->sf, c->ev_compute, 0));
+  for (int off = 0; off < n; off += kFireMax) {
+    const int m = std::min(kFireMax, n - off);
+    FireList fire{};
+    fire.n = m;
+    for (int i = 0; i < m; ++i) fire.ids[i] = ids[off + i];
+    {
+      ProfScope prof(c, LSA_PH_RESIDENCY, c->sf);
+      LSA_CUDA(c, launch_residency(c->d_seqs, c->pool, fire, sel_idx + (size_t)off * c->k, c->B, c->k, (int)cfg.hot_pages,
+                                   c->page_bytes, c->sf));
+    }
+    {
+      ProfScope prof(c, LSA_PH_FETCH, c->sf);
+      LSA_CUDA(c, launch_fetch(c->pool, cfg.hot_pool, c->page_bytes, c->fetch_ctas, c->sf));
+    }
+    c->index_launches += 2;
+  }
+  LSA_CUDA(c, cudaEventRecord(c->ev_fetch, c->sf));
+  for (int i = 0; i < n; ++i) {
+    c->pending[ids[i]] = 1;
+    c->visible_at[ids[i]] = c->step[ids[i]] + cfg.recall_lag;
+  }
+  return LSA_OK;
+}
+
+extern "C" int lsa_fetch_chunks(lsa_ctx* ctx, const int32_t* seq_ids, int32_t n, const int32_t* sel_idx) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!sel_idx) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null sel_idx");
+  int rc = check_ids(ctx, seq_ids, n);
+  if (rc) return rc;
+  return fetch_impl(ctx, seq_ids, n, sel_idx);
+}
+
+// ---- S6 -----------------------------------------------------------------------------------------
+// Swap every staged table that is due (or all of them if force) and optionally append k_new/v_new.
+static int prestep_impl(lsa_ctx* c, bool force, const void* k_new, const void* v_new) {
+  uint32_t words[32] = {0};
+  bool any = false;
+  for (int b = 0; b < c->B; ++b) {
+    if (c->pending[b] && (force || c->step[b] >= c->visible_at[b])) {
+      words[b >> 5] |= 1u << (b & 31);
+      c->pending[b] = 0;
+      any = true;
+    }
+  }
+  if (!any && !k_new) return LSA_OK;
+  if (any) LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_fetch, 0));
+  ProfScope prof(c, LSA_PH_PRESTEP, c->sc);
+  LSA_CUDA(c, launch_prestep(c->cfg.dtype, c->d_seqs, c->B, c->cfg.D, c->cfg.W, any ? words : nullptr, 32, k_new, v_new, c->sc));
+  c->attn_launches += 1;
+  return LSA_OK;
+}
+
+extern "C" int lsa_commit_tables(lsa_ctx* ctx) {
+  if (!ctx) return LSA_ERR_STATE;
+  return prestep_impl(ctx, true, nullptr, nullptr);
+}
+
+// ---- S7-S8 --------------------------------------------------------------------------------------
+static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse) {
+  const lsa_config& cfg = c->cfg;
+  if (c->attn_impl == LSA_ATTN_SIMT) {
+    {
+      ProfScope prof(c, LSA_PH_ATTENTION, c->sc);
+      LSA_CUDA(c, launch_attn_simt(cfg.dtype, cfg.H, cfg.D, cfg.C, c->k, c->d_seqs, c->pool, cfg.hot_pool, q, c->sm_scale,
+                                   c->geom, c->B, c->part_o, c->part_ml, c->sc));
+    }
+    {
+      ProfScope prof(c, LSA_PH_COMBINE, c->sc);
+      LSA_CUDA(c, launch_combine(cfg.dtype, cfg.H, cfg.D, cfg.C, c->d_seqs, c->geom, c->B, c->part_o, c->part_ml, out, lse, c->sc));
+    }
+    c->attn_launches += 2;
+    c->last_attn_ctas = c->geom.s_max * c->B;
+  } else {
+    int launches = 0, ctas = 0;
+    std::string msg;
+    ProfScope prof(c, LSA_PH_ATTENTION, c->sc);   // attention + combine of the tcgen05 path
+    int rc = tc_attention(c->tc, q, out, lse, c->sc, &launches, &ctas, &msg);
+    if (rc != 0) LSA_FAIL(c, rc, "tcgen05 attention: %s", msg.c_str());
+    c->attn_launches += launches;
+    c->last_attn_ctas = ctas;
+  }
+  return LSA_OK;
+}
+
+extern "C" int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, float* lse) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!q || !out) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null q / out");
+  int rc = prestep_impl(ctx, false, nullptr, nullptr);
+  if (rc) return rc;
+  return attention_impl(ctx, q, out, lse);
+}
+
+extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
+  if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
+  if (k_new && c->cfg.W < 1) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new given but W == 0");
+  int ids[1024];
+  int n_fire = 0;
+  for (int b = 0; b < c->B; ++b)
+    if (c->step[b] % c->cfg.tau == 0) ids[n_fire++] = b;           // S0
+  if (n_fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
+  int rc;
+  if ((rc = prestep_impl(c, false, k_new, v_new))) return rc;       // (a) + (d)
+  if (n_fire) {                                                     // (b)
+    if ((rc = index_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))) return rc;
+    if ((rc = fetch_impl(c, ids, n_fire, c->d_sel))) return rc;
+    if (c->cfg.recall_lag == 0 && (rc = prestep_impl(c, false, nullptr, nullptr))) return rc;   // (c)
+  }
+  if ((rc = attention_impl(c, q, out, nullptr))) return rc;         // (e)
+  for (int b = 0; b < c->B; ++b) c->step[b] += 1;                   // (f)
+  c->n_steps += 1;
+  return LSA_OK;
+}
+
+extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
+  const lsa_config& cfg = c->cfg;
+  const size_t qb = (size_t)c->B * cfg.H * cfg.D * c->elem, hb = (size_t)c->B * cfg.Dh * c->elem,
+               nb = (size_t)c->B * cfg.D * c->elem;
+  if (!c->st_q) {
+    int rc;
+    unsigned char* p = nullptr;
+    if ((rc = dev_alloc(c, &p, 2 * qb + hb + 2 * nb + 5 * 256))) return rc;
+    auto take = [&p](size_t n) { void* r = p; p += (n + 255) / 256 * 256; return r; };
+    c->st_q = take(qb); c->st_out = take(qb); c->st_h = take(hb); c->st_kn = take(nb); c->st_vn = take(nb);
+  }
+  LSA_CUDA(c, cudaMemcpyAsync(c->st_q, q, qb, cudaMemcpyHostToDevice, c->sc));
+  if (h) LSA_CUDA(c, cudaMemcpyAsync(c->st_h, h, hb, cudaMemcpyHostToDevice, c->sc));
+  if (k_new) {
+    LSA_CUDA(c, cudaMemcpyAsync(c->st_kn, k_new, nb, cudaMemcpyHostToDevice, c->sc));
+    LSA_CUDA(c, cudaMemcpyAsync(c->st_vn, v_new, nb, cudaMemcpyHostToDevice, c->sc));
+  }
+  int rc = lsa_step(c, c->st_q, h ? c->st_h : nullptr, k_new ? c->st_kn : nullptr, k_new ? c->st_vn : nullptr, c->st_out);
+  if (rc) return rc;
+  LSA_CUDA(c, cudaMemcpyAsync(out, c->st_out, qb, cudaMemcpyDeviceToHost, c->sc));
+  LSA_CUDA(c, cudaStreamSynchronize(c->sc));
+  return LSA_OK;
+}
+
+// ---- support --------------------------------------------------------------------------------------
+extern "C" int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (seq < 0 || seq >= ctx->B || !chunk_emb) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad seq / null chunk_emb");
+  ctx->seq_host[seq].emb = chunk_emb;
+  // ordered after every index launch already enqueued on the side band
+  LSA_CUDA(ctx, cudaMemcpyAsync(reinterpret_cast<char*>(ctx->d_seqs + seq) + offsetof(SeqDev, emb), &ctx->seq_host[seq].emb,
+                                sizeof(void*), cudaMemcpyHostToDevice, ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  return LSA_OK;
+}
+
+extern "C" int lsa_sync(lsa_ctx* ctx) {
+  if (!ctx) return LSA_ERR_STATE;
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  unsigned long long err = 0;
+  LSA_CUDA(ctx, cudaMemcpy(&err, ctx->pool.counters + C_ERROR, sizeof(err), cudaMemcpyDeviceToHost));
+  if (err) LSA_FAIL(ctx, LSA_ERR_POOL_EXHAUSTED, "hot pool exhausted during a residency pass");
+  return LSA_OK;
+}
+
+extern "C" int lsa_get_page_table(lsa_ctx* ctx, int32_t seq, int32_t which, int32_t* chunk_idx, int32_t* page, int32_t* n) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (seq < 0 || seq >= ctx->B || (which != 0 && which != 1) || !chunk_idx || !page || !n)
+    LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad argument");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  SeqDev d{};
+  LSA_CUDA(ctx, cudaMemcpy(&d, ctx->d_seqs + seq, sizeof(SeqDev), cudaMemcpyDeviceToHost));
+  int buf = which == 0 ? d.cur_buf : 1 - d.cur_buf;
+  int cnt = (which == 1 && !d.pending) ? 0 : d.n_tbl[buf];
+  *n = cnt;
+  if (cnt > 0) {
+    LSA_CUDA(ctx, cudaMemcpy(chunk_idx, ctx->pool.tbl_chunk + ((size_t)seq * 2 + buf) * ctx->k, sizeof(int) * cnt, cudaMemcpyDeviceToHost));
+    LSA_CUDA(ctx, cudaMemcpy(page, ctx->pool.tbl_page + ((size_t)seq * 2 + buf) * ctx->k, sizeof(int) * cnt, cudaMemcpyDeviceToHost));
+  }
+  return LSA_OK;
+}
+
+extern "C" int lsa_get_residency(lsa_ctx* ctx, int32_t seq, int32_t* page_of) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (seq < 0 || seq >= ctx->B || !page_of) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad argument");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  const SeqDev& d = ctx->seq_host[seq];
+  if (d.n_chunks > 0)
+    LSA_CUDA(ctx, cudaMemcpy(page_of, ctx->pool.page_of + d.page_of_off, sizeof(int) * d.n_chunks, cudaMemcpyDeviceToHost));
+  return LSA_OK;
+}
+
+extern "C" int lsa_get_stats(lsa_ctx* ctx, lsa_stats* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!out) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null out");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  unsigned long long cnt[8];
+  LSA_CUDA(ctx, cudaMemcpy(cnt, ctx->pool.counters, sizeof(cnt), cudaMemcpyDeviceToHost));
+  memset(out, 0, sizeof(*out));
+  out->triggers = cnt[C_TRIGGERS];
+  out->hits = cnt[C_HITS];
+  out->misses = cnt[C_MISSES];
+  out->evictions = cnt[C_EVICTIONS];
+  out->bytes_fetched = cnt[C_BYTES];
+  out->pool_error = (int)cnt[C_ERROR];
+  out->steps = ctx->n_steps;
+  out->attn_launches = ctx->attn_launches;
+  out->index_launches = ctx->index_launches;
+  out->attn_impl = ctx->attn_impl;
+  out->attn_ctas = ctx->last_attn_ctas;
+  return LSA_OK;
+}
+
+extern "C" int lsa_get_step(lsa_ctx* ctx, int32_t seq, int64_t* step) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (seq < 0 || seq >= ctx->B || !step) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad argument");
+  *step = ctx->step[seq];
+  return LSA_OK;
+}
+
+extern "C" int lsa_profile_enable(lsa_ctx* ctx, int32_t capacity) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (capacity < 0 || capacity > (1 << 20)) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "capacity out of range");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  for (int ph = 0; ph < LSA_PH_COUNT; ++ph) {
+    while ((int)ctx->prof_ev[ph].size() < 2 * capacity) {
+      cudaEvent_t e;
+      LSA_CUDA(ctx, cudaEventCreate(&e));
+      ctx->prof_ev[ph].push_back(e);
+    }
+    ctx->prof_n[ph] = 0;
+  }
+  ctx->prof_cap = capacity;
+  return LSA_OK;
+}
+
+extern "C" int lsa_profile_read(lsa_ctx* ctx, double* ms_sum, int64_t* count) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!ms_sum || !count) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null output");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  for (int ph = 0; ph < LSA_PH_COUNT; ++ph) {
+    double sum = 0;
+    for (int i = 0; i < ctx->prof_n[ph]; ++i) {
+      float ms = 0.f;
+      LSA_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->prof_ev[ph][2 * i], ctx->prof_ev[ph][2 * i + 1]));
+      sum += ms;
+    }
+    ms_sum[ph] = sum;
+    count[ph] = ctx->prof_n[ph];
+    ctx->prof_n[ph] = 0;
+  }
+  return LSA_OK;
+}

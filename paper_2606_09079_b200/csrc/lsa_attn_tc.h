@@ -1,0 +1,29 @@
+// lsa_attn_tc.h - host interface of the tcgen05/TMA split-K decode attention (lsa_attn_tc.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+
+#include "lsa_common.cuh"
+
+namespace lsa {
+
+struct TcPlan;
+
+struct TcInit {
+  int B, k, W, P, n_sms, max_ctas;
+  void* hot_pool;
+  const SeqDev* seq_host;   // host copy of the immutable per-sequence fields
+  SeqDev* d_seqs;
+  PoolDev pool;
+  float sm_scale;
+};
+
+// bf16, H = 64 query heads sharing one K/V of D = 512, pages of C = 128 rows (BASELINE cfg 2-5)
+bool tc_supported(int dtype, int H, int D, int C);
+int tc_create(const TcInit& init, TcPlan** out, std::string* msg);   // 0 or an lsa_status
+int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, cudaStream_t st, int* launches, int* ctas,
+                 std::string* msg);
+void tc_destroy(TcPlan* plan);
+
+}  // namespace lsa

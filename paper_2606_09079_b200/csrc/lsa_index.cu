@@ -1,0 +1,148 @@
+// lsa_index.cu - S1 query tower, S2 chunk scoring, S3 per-sequence top-k  (sm_100a)
+//
+//   S1  z = W_q h ; q_hat = z / max(||z||, 1e-12)     PAPER.md l.61-65 Eq.(1)-(2) collapsed to one
+//       linear map + L2 norm (l.124 "standard dual-encoder"; BASELINE.json north_star; DESIGN R1)
+//   S2  score_c = q_hat . Emb[c]                       PAPER.md l.71-75 Eq.(4) in cosine form (R1,R3)
+//   S3  first min(k, n_chunks) by (score desc, idx asc) PAPER.md l.77-79 Eq.(5) with top-k (R2,R14)
+//
+// All three are HBM/latency bound (W_q 4 MiB + Emb <= 2 MiB per trigger): 16-byte loads, one warp per
+// output row, fp32 accumulation in a fixed order so bit-identical embedding rows give bit-identical
+// scores wherever they sit in the table (exact planted ties stay exact).
+#include "lsa_kernels.h"
+#include "lsa_select.cuh"
+
+namespace lsa {
+
+constexpr int kQtWarps = 4;   // rows of W_q per block
+constexpr int kQtSeqs = 4;    // sequences per pass (W_q row is read once for all of them)
+
+template <typename T>
+__global__ void __launch_bounds__(kQtWarps * 32)
+qtower_kernel(const T* __restrict__ W, const T* __restrict__ h, FireList rows, float* __restrict__ z, int E, int Dh) {
+  constexpr int V = Elem<T>::kVec;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int e = blockIdx.x * kQtWarps + warp;
+  const int i0 = blockIdx.y * kQtSeqs;
+  const int n = rows.n;
+  if (e >= E) return;
+  float acc[kQtSeqs];
+#pragma unroll
+  for (int s = 0; s < kQtSeqs; ++s) acc[s] = 0.f;
+  const T* wrow = W + (size_t)e * Dh;
+#pragma unroll 2
+  for (int d0 = lane * V; d0 < Dh; d0 += 32 * V) {
+    float wf[V];
+    Elem<T>::load16(wrow + d0, wf);
+#pragma unroll
+    for (int s = 0; s < kQtSeqs; ++s) {
+      if (i0 + s < n) {
+        float hf[V];
+        Elem<T>::load16(h + (size_t)rows.ids[i0 + s] * Dh + d0, hf);
+#pragma unroll
+        for (int j = 0; j < V; ++j) acc[s] = fmaf(wf[j], hf[j], acc[s]);
+      }
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < kQtSeqs; ++s) {
+    float v = warp_sum(acc[s]);
+    if (lane == 0 && i0 + s < n) z[(size_t)(i0 + s) * E + e] = v;
+  }
+}
+
+constexpr int kScWarps = 8;
+
+template <typename T>
+__global__ void __launch_bounds__(kScWarps * 32)
+score_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __restrict__ z,
+             float* __restrict__ scores, int E, int n_chunks_max) {
+  extern __shared__ float zs[];           // [E]
+  __shared__ float red[kScWarps];
+  __shared__ float inv_norm_s;
+  constexpr int V = Elem<T>::kVec;
+  const int i = blockIdx.y;
+  const SeqDev& sq = seqs[fire.ids[i]];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int c0 = blockIdx.x * kScWarps;
+  if (c0 >= sq.n_chunks) return;
+  float ss = 0.f;
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    float v = z[(size_t)i * E + e];
+    zs[e] = v;
+    ss = fmaf(v, v, ss);
+  }
+  ss = warp_sum(ss);
+  if (lane == 0) red[warp] = ss;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float t = 0.f;
+    for (int w = 0; w < kScWarps; ++w) t += red[w];
+    inv_norm_s = 1.0f / fmaxf(sqrtf(t), 1e-12f);
+  }
+  __syncthreads();
+  const int c = c0 + warp;
+  if (c >= sq.n_chunks) return;
+  const T* row = reinterpret_cast<const T*>(sq.emb) + (size_t)c * E;
+  float acc = 0.f;
+  for (int e0 = lane * V; e0 < E; e0 += 32 * V) {
+    float ef[V];
+    Elem<T>::load16(row + e0, ef);
+#pragma unroll
+    for (int j = 0; j < V; ++j) acc = fmaf(ef[j], zs[e0 + j], acc);
+  }
+  acc = warp_sum(acc);
+  if (lane == 0) scores[(size_t)i * n_chunks_max + c] = acc * inv_norm_s;
+}
+
+__global__ void __launch_bounds__(1024)
+topk_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __restrict__ scores,
+            int n_chunks_max, int k, int32_t* __restrict__ sel_idx, float* __restrict__ sel_score) {
+  __shared__ SelectSmem sm;
+  const int i = blockIdx.x;
+  const SeqDev& sq = seqs[fire.ids[i]];
+  const float* sc = scores + (size_t)i * n_chunks_max;
+  auto keyf = [sc](int c) -> unsigned long long {
+    return ((unsigned long long)(~float_to_ordered(sc[c])) << 32) | (unsigned)c;
+  };
+  const int m = block_select_smallest(keyf, sq.n_chunks, min(k, sq.n_chunks), sm);
+  for (int j = threadIdx.x; j < k; j += blockDim.x) {
+    int idx = -1;
+    float val = -INFINITY;
+    if (j < m) {
+      unsigned long long key = sm.keys[j];
+      idx = (int)(key & 0xffffffffull);
+      val = ordered_to_float(~(uint32_t)(key >> 32));
+    }
+    sel_idx[(size_t)i * k + j] = idx;
+    if (sel_score) sel_score[(size_t)i * k + j] = val;
+  }
+}
+
+cudaError_t launch_qtower(int dtype, const void* W, const void* h, const FireList& rows, float* z, int E, int Dh,
+                          cudaStream_t st) {
+  dim3 grid((E + kQtWarps - 1) / kQtWarps, (rows.n + kQtSeqs - 1) / kQtSeqs);
+  if (dtype == 0)
+    qtower_kernel<float><<<grid, kQtWarps * 32, 0, st>>>((const float*)W, (const float*)h, rows, z, E, Dh);
+  else
+    qtower_kernel<__nv_bfloat16><<<grid, kQtWarps * 32, 0, st>>>((const __nv_bfloat16*)W, (const __nv_bfloat16*)h, rows, z, E, Dh);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, const float* z, float* scores,
+                          int E, int n_chunks_max, cudaStream_t st) {
+  dim3 grid((n_chunks_max + kScWarps - 1) / kScWarps, fire.n);
+  size_t smem = (size_t)E * sizeof(float);
+  if (dtype == 0)
+    score_kernel<float><<<grid, kScWarps * 32, smem, st>>>(seqs, fire, z, scores, E, n_chunks_max);
+  else
+    score_kernel<__nv_bfloat16><<<grid, kScWarps * 32, smem, st>>>(seqs, fire, z, scores, E, n_chunks_max);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores, int n_chunks_max, int k,
+                        int32_t* sel_idx, float* sel_score, cudaStream_t st) {
+  topk_kernel<<<fire.n, 1024, 0, st>>>(seqs, fire, scores, n_chunks_max, k, sel_idx, sel_score);
+  return cudaGetLastError();
+}
+
+}  // namespace lsa

@@ -1,0 +1,47 @@
+// lsa_kernels.h - host-side launchers of the LSA kernels (internal to liblsa).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lsa_common.cuh"
+
+namespace lsa {
+
+struct AttnGeom {          // host-computed split geometry of one S7 launch
+  int keys_per_cta;        // virtual keys per split (multiple of the tile)
+  int s_max;               // gridDim.x : splits of the longest sequence
+};
+
+// ---- S1-S3 (lsa_index.cu) ---------------------------------------------------------------
+// z[i][e] = sum_d W[e][d] * h[rows.ids[i]][d]           (fp32 out, i < rows.n)
+cudaError_t launch_qtower(int dtype, const void* W, const void* h, const FireList& rows, float* z, int E,
+                          int Dh, cudaStream_t st);
+// scores[i][c] = (z_i . Emb_{b_i}[c]) / max(||z_i||, 1e-12)
+cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, const float* z,
+                          float* scores, int E, int n_chunks_max, cudaStream_t st);
+// sel_idx[i][0..k) / sel_score: first k_eff by (score desc, chunk idx asc), rest -1 / -inf
+cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores,
+                        int n_chunks_max, int k, int32_t* sel_idx, float* sel_score, cudaStream_t st);
+
+// ---- S4-S6 (lsa_residency.cu) -----------------------------------------------------------
+cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, const int32_t* sel_idx,
+                             int B, int k, int P, long long page_bytes, cudaStream_t st);
+cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas,
+                         cudaStream_t st);
+// swap tables of sequences whose bit is set in swap_mask; append k_new/v_new rows to the ring
+cudaError_t launch_prestep(int dtype, SeqDev* seqs, int B, int D, int W, const uint32_t* swap_mask_words,
+                           int n_words, const void* k_new, const void* v_new, cudaStream_t st);
+
+// ---- S7-S8, SIMT implementation (lsa_attn_simt.cu) ---------------------------------------
+bool simt_supported(int dtype, int H, int D);
+int simt_tile_keys();
+cudaError_t simt_smem_bytes(int dtype, int H, int D, int k, size_t* bytes);
+cudaError_t simt_max_ctas_per_sm(int dtype, int H, int D, int k, int* ctas);
+cudaError_t launch_attn_simt(int dtype, int H, int D, int C, int k, const SeqDev* seqs, PoolDev pool,
+                             const void* hot_pool, const void* q, float sm_scale, AttnGeom g, int B,
+                             float* part_o, float* part_ml, cudaStream_t st);
+cudaError_t launch_combine(int dtype, int H, int D, int C, const SeqDev* seqs, AttnGeom g, int B,
+                           const float* part_o, const float* part_ml, void* out, float* lse,
+                           cudaStream_t st);
+
+}  // namespace lsa

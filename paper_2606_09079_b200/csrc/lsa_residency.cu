@@ -1,0 +1,277 @@
+// lsa_residency.cu - S4 residency diff + page allocation, S5 chunk fetch, S6 table swap (sm_100a)
+//
+//   S4  hits = sel & resident, misses = sel \ resident; every miss gets the unpinned page with the
+//       smallest (last_used, page) - never-used pages (last_used 0) first, lowest index first - and
+//       its previous owner is evicted.  Pages of any current or staged table are pinned.
+//       PAPER.md l.185 (recalled subset lands in the "GPU reserve", page granular), l.187
+//       (residency bitmap + remap); BASELINE.json cfg 4 (shared pool, LRU); DESIGN R11-R13.
+//   S5  copy each missing chunk (one contiguous page image) from the pinned-host cold pool to its
+//       hot-pool page.  PAPER.md l.179/l.185 (CPU cold mirror), l.189 (async recall).
+//       Device-pull design: the kernel reads the cold pool through its mapped device address with
+//       16-byte loads, so the whole trigger path stays on the device - no host round trip, unlike
+//       the host-synchronising Level-1 recall the paper describes (l.187).
+//   S6  the staged table becomes the attended one ("materialize ... at step t+1").
+//
+// The residency pass is one 1024-thread block: the pool is shared by all sequences and the oracle
+// semantics are sequential in ascending sequence id, so there is no parallelism across sequences;
+// inside one sequence every pass (pin marking, hit lookup, victim selection, table write) is
+// block-parallel.
+#include "lsa_kernels.h"
+#include "lsa_select.cuh"
+
+namespace lsa {
+
+struct ResSmem {
+  SelectSmem sel;
+  int sel_up[kMaxK];      // selection sorted by chunk id
+  int next_page[kMaxK];
+  int miss_rank[kMaxK];   // rank among misses or -1 for a hit
+  int warp_cnt[32];
+  int n_sel;
+  int n_miss;
+  unsigned long long tick;
+  unsigned int epoch;
+};
+
+__global__ void __launch_bounds__(1024)
+residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const int32_t* __restrict__ sel_idx,
+                 int B, int k, int P, long long page_bytes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  ResSmem& sm = *reinterpret_cast<ResSmem*>(smem_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) pool.counters[C_FETCH_COUNT] = 0;
+  __syncthreads();
+
+  for (int fi = 0; fi < fire.n; ++fi) {
+    const int b = fire.ids[fi];
+    SeqDev& sq = seqs[b];
+    const int* my_sel = sel_idx + (size_t)fi * k;
+
+    // ---- selection -> ascending chunk id (R13) ----
+    {
+      int n_pad = next_pow2(k);
+      for (int i = tid; i < n_pad; i += blockDim.x) {
+        int c = (i < k) ? my_sel[i] : -1;
+        sm.sel.keys[i] = (c >= 0 && c < sq.n_chunks) ? (unsigned long long)c : kKeyMax;
+      }
+      __syncthreads();
+      block_bitonic_sort(sm.sel.keys, n_pad);
+      if (tid == 0) {
+        int n = 0;
+        while (n < k && sm.sel.keys[n] != kKeyMax) ++n;
+        sm.n_sel = n;
+        sm.tick = ++pool.counters[C_TICK];
+        sm.epoch = ++(*pool.epoch);
+        pool.counters[C_TRIGGERS] += 1;
+        sq.pending = 0;                 // a new selection supersedes an unswapped staged table
+      }
+      __syncthreads();
+      for (int i = tid; i < sm.n_sel; i += blockDim.x) sm.sel_up[i] = (int)sm.sel.keys[i];
+      __syncthreads();
+    }
+    const int n_sel = sm.n_sel;
+    const unsigned long long tick = sm.tick;
+    const unsigned int epoch = sm.epoch;
+
+    // ---- pin every page of a current table and of other sequences' staged tables ----
+    for (int idx = tid; idx < B * 2 * k; idx += blockDim.x) {
+      int bb = idx / (2 * k), r = idx % (2 * k), buf = r / k, j = r % k;
+      const SeqDev& o = seqs[bb];
+      bool is_cur = (buf == o.cur_buf);
+      bool live = is_cur ? true : (o.pending != 0);
+      if (live && j < o.n_tbl[buf]) pool.pin_mark[pool.tbl_page[((size_t)bb * 2 + buf) * k + j]] = epoch;
+    }
+    __syncthreads();
+
+    // ---- pass 1: hits ----
+    int my_miss = 0;
+    if (tid < n_sel) {
+      int c = sm.sel_up[tid];
+      int p = pool.page_of[sq.page_of_off + c];
+      if (p >= 0) {
+        pool.last_used[p] = tick;
+        pool.pin_mark[p] = epoch;
+        sm.next_page[tid] = p;
+      } else {
+        my_miss = 1;
+      }
+    }
+    // block exclusive scan of my_miss over tid < kMaxK (1024 threads = 32 warps)
+    unsigned bal = __ballot_sync(0xffffffffu, my_miss);
+    int wpre = __popc(bal & ((1u << lane) - 1));
+    if (lane == 0) sm.warp_cnt[warp] = __popc(bal);
+    __syncthreads();
+    if (warp == 0) {
+      int v = sm.warp_cnt[lane];
+      int incl = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+      }
+      sm.warp_cnt[lane] = incl - v;
+      if (lane == 31) sm.n_miss = incl;
+    }
+    __syncthreads();
+    if (tid < n_sel) sm.miss_rank[tid] = my_miss ? (sm.warp_cnt[warp] + wpre) : -1;
+    const int n_miss = sm.n_miss;
+    __syncthreads();
+
+    // ---- pass 2: the n_miss smallest (last_used, page) among unpinned pages ----
+    if (n_miss > 0) {
+      const unsigned long long* lu = pool.last_used;
+      const unsigned int* pm = pool.pin_mark;
+      auto keyf = [lu, pm, epoch](int p) -> unsigned long long {
+        return pm[p] == epoch ? kKeyMax : ((lu[p] << kPageBits) | (unsigned long long)p);
+      };
+      int got = block_select_smallest(keyf, P, n_miss, sm.sel);
+      __syncthreads();
+      bool bad = (got < n_miss) || (sm.sel.keys[n_miss - 1] == kKeyMax);
+      if (bad) {
+        if (tid == 0) pool.counters[C_ERROR] = 1;   // pool exhausted: leave state untouched
+        __syncthreads();
+        continue;
+      }
+      const unsigned long long base = pool.counters[C_FETCH_COUNT];
+      if (tid < n_sel && sm.miss_rank[tid] >= 0) {
+        const int r = sm.miss_rank[tid];
+        const int c = sm.sel_up[tid];
+        const int p = (int)(sm.sel.keys[r] & ((1ull << kPageBits) - 1));
+        const int ob = pool.owner_seq[p];
+        if (ob >= 0) {
+          pool.page_of[seqs[ob].page_of_off + pool.owner_chunk[p]] = -1;
+          atomicAdd(&pool.counters[C_EVICTIONS], 1ull);
+        }
+        pool.owner_seq[p] = b;
+        pool.owner_chunk[p] = c;
+        pool.page_of[sq.page_of_off + c] = p;
+        pool.last_used[p] = tick;
+        sm.next_page[tid] = p;
+        pool.fetch_src[base + r] = reinterpret_cast<const unsigned char*>(sq.cold) + (long long)c * page_bytes;
+        pool.fetch_page[base + r] = p;
+      }
+    }
+    __syncthreads();
+
+    // ---- stage the next table (ascending chunk id) ----
+    const int buf = 1 - sq.cur_buf;
+    if (tid < n_sel) {
+      pool.tbl_chunk[((size_t)b * 2 + buf) * k + tid] = sm.sel_up[tid];
+      pool.tbl_page[((size_t)b * 2 + buf) * k + tid] = sm.next_page[tid];
+    }
+    if (tid == 0) {
+      sq.n_tbl[buf] = n_sel;
+      sq.pending = 1;
+      pool.counters[C_FETCH_COUNT] += n_miss;
+      pool.counters[C_MISSES] += n_miss;
+      pool.counters[C_HITS] += n_sel - n_miss;
+      pool.counters[C_BYTES] += (unsigned long long)n_miss * (unsigned long long)page_bytes;
+    }
+    __threadfence();
+    __syncthreads();
+  }
+}
+
+// ---- S5: device-pull fetch ----------------------------------------------------------------
+constexpr int kFetchThreads = 256;
+constexpr int kFetchUnroll = 4;                                  // 16-byte loads in flight per thread
+constexpr int kFetchSlice = kFetchThreads * kFetchUnroll * 16;   // 16 KiB per (page, slice) item
+
+__device__ __forceinline__ uint4 ld_stream16(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+__global__ void __launch_bounds__(kFetchThreads)
+fetch_kernel(PoolDev pool, unsigned char* __restrict__ hot_pool, long long page_bytes) {
+  const int n_fetch = (int)pool.counters[C_FETCH_COUNT];
+  const int slices = (int)((page_bytes + kFetchSlice - 1) / kFetchSlice);
+  const long long items = (long long)n_fetch * slices;
+  for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+    const int f = (int)(it / slices), s = (int)(it % slices);
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(pool.fetch_src[f]) + (long long)s * kFetchSlice;
+    unsigned char* dst = hot_pool + (long long)pool.fetch_page[f] * page_bytes + (long long)s * kFetchSlice;
+    const long long left = page_bytes - (long long)s * kFetchSlice;
+    uint4 v[kFetchUnroll];
+#pragma unroll
+    for (int u = 0; u < kFetchUnroll; ++u) {
+      long long off = ((long long)u * kFetchThreads + threadIdx.x) * 16;
+      if (off < left) v[u] = ld_stream16(reinterpret_cast<const uint4*>(src + off));
+    }
+#pragma unroll
+    for (int u = 0; u < kFetchUnroll; ++u) {
+      long long off = ((long long)u * kFetchThreads + threadIdx.x) * 16;
+      if (off < left) *reinterpret_cast<uint4*>(dst + off) = v[u];
+    }
+  }
+}
+
+// ---- S6 + window append ---------------------------------------------------------------------
+// The swap mask is passed BY VALUE (32 words = up to 1024 sequences): a step needs no extra copy.
+struct SwapWords { uint32_t w[32]; };
+
+template <typename T>
+__global__ void __launch_bounds__(128)
+prestep_kernel_v(SeqDev* __restrict__ seqs, int D, int W, SwapWords sw, int use_swap,
+                 const T* __restrict__ k_new, const T* __restrict__ v_new) {
+  const int b = blockIdx.x;
+  SeqDev& sq = seqs[b];
+  const bool swap = use_swap && ((sw.w[(b >> 5) & 31] >> (b & 31)) & 1u);
+  if (k_new) {
+    const int slot = sq.w_head;
+    T* kd = reinterpret_cast<T*>(sq.win_k) + (size_t)slot * D;
+    T* vd = reinterpret_cast<T*>(sq.win_v) + (size_t)slot * D;
+    constexpr int V = Elem<T>::kVec;
+    for (int d = threadIdx.x * V; d < D; d += blockDim.x * V) {
+      *reinterpret_cast<uint4*>(kd + d) = *reinterpret_cast<const uint4*>(k_new + (size_t)b * D + d);
+      *reinterpret_cast<uint4*>(vd + d) = *reinterpret_cast<const uint4*>(v_new + (size_t)b * D + d);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (swap && sq.pending) {
+      sq.cur_buf = 1 - sq.cur_buf;
+      sq.pending = 0;
+    }
+    if (k_new) {
+      const int slot = sq.w_head;
+      sq.w_head = (slot + 1 == W) ? 0 : slot + 1;
+      sq.w_len = min(W, sq.w_len + 1);
+    }
+  }
+}
+
+cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, const int32_t* sel_idx, int B, int k,
+                             int P, long long page_bytes, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(residency_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(ResSmem));
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  residency_kernel<<<1, 1024, sizeof(ResSmem), st>>>(seqs, pool, fire, sel_idx, B, k, P, page_bytes);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas, cudaStream_t st) {
+  fetch_kernel<<<n_ctas, kFetchThreads, 0, st>>>(pool, reinterpret_cast<unsigned char*>(hot_pool), page_bytes);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_prestep(int dtype, SeqDev* seqs, int B, int D, int W, const uint32_t* swap_mask_words,
+                           int n_words, const void* k_new, const void* v_new, cudaStream_t st) {
+  SwapWords sw;
+  for (int i = 0; i < 32; ++i) sw.w[i] = (swap_mask_words && i < n_words) ? swap_mask_words[i] : 0u;
+  const int use_swap = swap_mask_words != nullptr;
+  if (dtype == 0)
+    prestep_kernel_v<float><<<B, 128, 0, st>>>(seqs, D, W, sw, use_swap, (const float*)k_new, (const float*)v_new);
+  else
+    prestep_kernel_v<__nv_bfloat16><<<B, 128, 0, st>>>(seqs, D, W, sw, use_swap, (const __nv_bfloat16*)k_new,
+                                                       (const __nv_bfloat16*)v_new);
+  return cudaGetLastError();
+}
+
+}  // namespace lsa

@@ -1,0 +1,298 @@
+"""Thin ctypes binding of liblsa (include/lsa.h): argument marshalling only.
+
+Every step of the LSA path runs in the CUDA kernels behind the C ABI; PyTorch is used here
+for device / pinned-host memory and streams.  There is no CPU fallback: importing this
+module without the built library raises, and so does calling it without a CUDA device.
+
+Functions mirror the C names: lsa_init_pools, lsa_index_select, lsa_fetch_chunks,
+lsa_decode_attention, lsa_step (+ support calls).  `LsaContext` owns the opaque handle and
+keeps the caller's tensors alive for the lifetime of the context (the library never copies
+them).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence, Tuple
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblsa.so")
+
+LSA_F32, LSA_BF16 = 0, 1
+LSA_ATTN_AUTO, LSA_ATTN_SIMT, LSA_ATTN_TCGEN05 = 0, 1, 2
+LSA_FETCH_DEVICE_PULL, LSA_FETCH_MEMCPY = 0, 1
+
+STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_ERR_POOL_EXHAUSTED",
+          -4: "LSA_ERR_OOM", -5: "LSA_ERR_STATE", -6: "LSA_ERR_UNSUPPORTED"}
+
+EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit_tables",
+           "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
+           "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
+           "lsa_profile_enable", "lsa_profile_read",
+           "lsa_last_error", "lsa_destroy", "lsa_version"]
+
+
+class LsaError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class lsa_config(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("dtype", C.c_int32), ("B", C.c_int32), ("H", C.c_int32),
+                ("D", C.c_int32), ("C", C.c_int32), ("W", C.c_int32), ("Dh", C.c_int32), ("E", C.c_int32),
+                ("k", C.c_int32), ("tau", C.c_int32), ("recall_lag", C.c_int32), ("sm_scale", C.c_float),
+                ("hot_pages", C.c_int64), ("hot_pool", C.c_void_p), ("W_q", C.c_void_p),
+                ("stream_compute", C.c_void_p), ("stream_fetch", C.c_void_p), ("attn_impl", C.c_int32),
+                ("fetch_mode", C.c_int32), ("max_ctas", C.c_int32), ("reserved", C.c_int32)]
+
+
+class lsa_seq_desc(C.Structure):
+    _fields_ = [("cold_csa", C.c_void_p), ("n_csa", C.c_int64), ("chunk_emb", C.c_void_p),
+                ("hca_k", C.c_void_p), ("hca_v", C.c_void_p), ("n_hca", C.c_int64), ("win_k", C.c_void_p),
+                ("win_v", C.c_void_p), ("w_len", C.c_int32), ("w_head", C.c_int32), ("step0", C.c_int64)]
+
+
+class lsa_stats(C.Structure):
+    _fields_ = [("triggers", C.c_uint64), ("hits", C.c_uint64), ("misses", C.c_uint64),
+                ("evictions", C.c_uint64), ("bytes_fetched", C.c_uint64), ("steps", C.c_uint64),
+                ("attn_launches", C.c_uint64), ("index_launches", C.c_uint64), ("pool_error", C.c_int32),
+                ("attn_impl", C.c_int32), ("attn_ctas", C.c_int32), ("reserved", C.c_int32)]
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2606_09079_b200.build` "
+            "(or __graft_entry__.build()).  There is no CPU fallback for the LSA path.")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32p, f32p = C.c_void_p, C.POINTER(C.c_int32), C.c_void_p
+    lib.lsa_init_pools.argtypes = [C.POINTER(lsa_config), C.POINTER(lsa_seq_desc), C.POINTER(vp)]
+    lib.lsa_index_select.argtypes = [vp, vp, i32p, C.c_int32, vp, f32p]
+    lib.lsa_fetch_chunks.argtypes = [vp, i32p, C.c_int32, vp]
+    lib.lsa_commit_tables.argtypes = [vp]
+    lib.lsa_decode_attention.argtypes = [vp, vp, vp, f32p]
+    lib.lsa_step.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.lsa_step_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.lsa_set_chunk_emb.argtypes = [vp, C.c_int32, vp]
+    lib.lsa_get_page_table.argtypes = [vp, C.c_int32, C.c_int32, i32p, i32p, i32p]
+    lib.lsa_get_residency.argtypes = [vp, C.c_int32, i32p]
+    lib.lsa_get_stats.argtypes = [vp, C.POINTER(lsa_stats)]
+    lib.lsa_get_step.argtypes = [vp, C.c_int32, C.POINTER(C.c_int64)]
+    lib.lsa_sync.argtypes = [vp]
+    lib.lsa_profile_enable.argtypes = [vp, C.c_int32]
+    lib.lsa_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    lib.lsa_last_error.argtypes = [vp]
+    lib.lsa_last_error.restype = C.c_char_p
+    lib.lsa_destroy.argtypes = [vp]
+    lib.lsa_destroy.restype = None
+    lib.lsa_version.argtypes = []
+    for name in EXPORTS:
+        if name not in ("lsa_last_error", "lsa_destroy"):
+            getattr(lib, name).restype = C.c_int
+    return lib
+
+
+_lib = _load()
+
+
+def _torch_dtype(dtype: int):
+    return torch.float32 if dtype == LSA_F32 else torch.bfloat16
+
+
+def _dev_ptr(t: Optional[torch.Tensor], dtype=None, what="tensor") -> Optional[int]:
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise LsaError(-1, f"{what} must be a CUDA tensor")
+    if not t.is_contiguous():
+        raise LsaError(-1, f"{what} must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise LsaError(-1, f"{what} must have dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _host_ptr(t: Optional[torch.Tensor], dtype=None, what="tensor") -> Optional[int]:
+    if t is None:
+        return None
+    if t.is_cuda or not t.is_contiguous():
+        raise LsaError(-1, f"{what} must be a contiguous host tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise LsaError(-1, f"{what} must have dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _ids(seq_ids: Sequence[int]):
+    arr = (C.c_int32 * len(seq_ids))(*[int(x) for x in seq_ids])
+    return arr, len(seq_ids)
+
+
+class LsaContext:
+    """Owns one lsa_ctx.  See include/lsa.h for the meaning of every argument."""
+
+    def __init__(self, *, dtype: int, H: int, D: int, C_: int, W: int, Dh: int, E: int, k: int, tau: int,
+                 hot_pool: torch.Tensor, W_q: torch.Tensor, seqs: Sequence[dict], recall_lag: int = 1,
+                 sm_scale: float = 0.0, stream_compute: Optional[torch.cuda.Stream] = None,
+                 stream_fetch: Optional[torch.cuda.Stream] = None, attn_impl: int = LSA_ATTN_AUTO,
+                 fetch_mode: int = LSA_FETCH_DEVICE_PULL, max_ctas: int = 0):
+        if not torch.cuda.is_available():
+            raise LsaError(-2, "no CUDA device: the LSA path has no CPU fallback")
+        td = _torch_dtype(dtype)
+        self.dtype, self.tdtype = dtype, td
+        self.B, self.H, self.D, self.C, self.W, self.Dh, self.E, self.k, self.tau = len(seqs), H, D, C_, W, Dh, E, k, tau
+        self.stream_compute = stream_compute or torch.cuda.Stream()
+        self.stream_fetch = stream_fetch or torch.cuda.Stream()
+        self._keep = [hot_pool, W_q, list(seqs)]
+        page_elems = 2 * C_ * D
+        if hot_pool.numel() % page_elems:
+            raise LsaError(-1, "hot_pool size is not a whole number of pages")
+        cfg = lsa_config()
+        cfg.struct_size = C.sizeof(lsa_config)
+        cfg.dtype, cfg.B, cfg.H, cfg.D, cfg.C, cfg.W = dtype, self.B, H, D, C_, W
+        cfg.Dh, cfg.E, cfg.k, cfg.tau, cfg.recall_lag, cfg.sm_scale = Dh, E, k, tau, recall_lag, sm_scale
+        cfg.hot_pages = hot_pool.numel() // page_elems
+        cfg.hot_pool = _dev_ptr(hot_pool, td, "hot_pool")
+        cfg.W_q = _dev_ptr(W_q, td, "W_q")
+        cfg.stream_compute = self.stream_compute.cuda_stream
+        cfg.stream_fetch = self.stream_fetch.cuda_stream
+        cfg.attn_impl, cfg.fetch_mode, cfg.max_ctas = attn_impl, fetch_mode, max_ctas
+        descs = (lsa_seq_desc * self.B)()
+        for b, s in enumerate(seqs):
+            d = descs[b]
+            cold = s.get("cold_csa")
+            if cold is not None and not cold.is_pinned():
+                raise LsaError(-1, f"seq {b}: cold_csa must be pinned host memory")
+            d.cold_csa = _host_ptr(cold, td, "cold_csa")
+            d.n_csa = int(s["n_csa"])
+            d.chunk_emb = _dev_ptr(s.get("chunk_emb"), td, "chunk_emb")
+            d.hca_k = _dev_ptr(s.get("hca_k"), td, "hca_k")
+            d.hca_v = _dev_ptr(s.get("hca_v"), td, "hca_v")
+            d.n_hca = 0 if s.get("hca_k") is None else s["hca_k"].shape[0]
+            d.win_k = _dev_ptr(s.get("win_k"), td, "win_k")
+            d.win_v = _dev_ptr(s.get("win_v"), td, "win_v")
+            d.w_len = int(s.get("w_len", 0))
+            d.w_head = int(s.get("w_head", 0))
+            d.step0 = int(s.get("step0", 0))
+        handle = C.c_void_p()
+        rc = _lib.lsa_init_pools(C.byref(cfg), descs, C.byref(handle))
+        if rc != 0:
+            raise LsaError(rc, (_lib.lsa_last_error(None) or b"").decode())
+        self._h = handle
+        self.hot_pages = int(cfg.hot_pages)
+
+    # -- helpers ---------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise LsaError(rc, (_lib.lsa_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.lsa_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the five path calls ---------------------------------------------------------------
+    def index_select(self, h: torch.Tensor, seq_ids: Sequence[int], want_scores: bool = True):
+        arr, n = _ids(seq_ids)
+        sel = torch.empty((n, self.k), dtype=torch.int32, device=h.device)
+        sc = torch.empty((n, self.k), dtype=torch.float32, device=h.device) if want_scores else None
+        self._check(_lib.lsa_index_select(self._h, _dev_ptr(h, self.tdtype, "h"), arr, n, sel.data_ptr(),
+                                          None if sc is None else sc.data_ptr()))
+        return sel, sc
+
+    def fetch_chunks(self, seq_ids: Sequence[int], sel_idx: torch.Tensor):
+        arr, n = _ids(seq_ids)
+        self._check(_lib.lsa_fetch_chunks(self._h, arr, n, _dev_ptr(sel_idx, torch.int32, "sel_idx")))
+
+    def commit_tables(self):
+        self._check(_lib.lsa_commit_tables(self._h))
+
+    def decode_attention(self, q: torch.Tensor, out: Optional[torch.Tensor] = None, want_lse: bool = False):
+        out = torch.empty_like(q) if out is None else out
+        lse = torch.empty((self.B, self.H), dtype=torch.float32, device=q.device) if want_lse else None
+        self._check(_lib.lsa_decode_attention(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(out, self.tdtype, "out"),
+                                              None if lse is None else lse.data_ptr()))
+        return (out, lse) if want_lse else out
+
+    def step(self, q, h, k_new=None, v_new=None, out=None):
+        out = torch.empty_like(q) if out is None else out
+        self._check(_lib.lsa_step(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(h, self.tdtype, "h"),
+                                  _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
+                                  _dev_ptr(out, self.tdtype, "out")))
+        return out
+
+    def step_host(self, q, h, k_new, v_new, out):
+        self._check(_lib.lsa_step_host(self._h, _host_ptr(q, self.tdtype, "q"), _host_ptr(h, self.tdtype, "h"),
+                                       _host_ptr(k_new, self.tdtype, "k_new"), _host_ptr(v_new, self.tdtype, "v_new"),
+                                       _host_ptr(out, self.tdtype, "out")))
+        return out
+
+    # -- support -----------------------------------------------------------------------------
+    def set_chunk_emb(self, seq: int, emb: torch.Tensor):
+        self._keep.append(emb)
+        self._check(_lib.lsa_set_chunk_emb(self._h, seq, _dev_ptr(emb, self.tdtype, "chunk_emb")))
+
+    def page_table(self, seq: int, which: int = 0) -> Tuple[List[int], List[int]]:
+        ch, pg, n = (C.c_int32 * self.k)(), (C.c_int32 * self.k)(), C.c_int32(0)
+        self._check(_lib.lsa_get_page_table(self._h, seq, which, ch, pg, C.byref(n)))
+        return list(ch[: n.value]), list(pg[: n.value])
+
+    def residency(self, seq: int, n_chunks: int) -> List[int]:
+        buf = (C.c_int32 * max(n_chunks, 1))()
+        self._check(_lib.lsa_get_residency(self._h, seq, buf))
+        return list(buf[:n_chunks])
+
+    def stats(self) -> dict:
+        st = lsa_stats()
+        self._check(_lib.lsa_get_stats(self._h, C.byref(st)))
+        return {f: getattr(st, f) for f, _ in lsa_stats._fields_ if f != "reserved"}
+
+    def get_step(self, seq: int) -> int:
+        v = C.c_int64(0)
+        self._check(_lib.lsa_get_step(self._h, seq, C.byref(v)))
+        return v.value
+
+    def sync(self):
+        self._check(_lib.lsa_sync(self._h))
+
+    PHASES = ("prestep", "attention", "combine", "index", "residency", "fetch")
+
+    def profile_enable(self, capacity: int):
+        self._check(_lib.lsa_profile_enable(self._h, capacity))
+
+    def profile_read(self) -> dict:
+        ms, cnt = (C.c_double * 6)(), (C.c_int64 * 6)()
+        self._check(_lib.lsa_profile_read(self._h, ms, cnt))
+        return {p: dict(ms=ms[i], count=cnt[i]) for i, p in enumerate(self.PHASES)}
+
+
+# C-named free functions (same names as the ABI) --------------------------------------------------
+def lsa_init_pools(**kw) -> LsaContext:
+    return LsaContext(**kw)
+
+
+def lsa_index_select(ctx: LsaContext, h, seq_ids, want_scores=True):
+    return ctx.index_select(h, seq_ids, want_scores)
+
+
+def lsa_fetch_chunks(ctx: LsaContext, seq_ids, sel_idx):
+    return ctx.fetch_chunks(seq_ids, sel_idx)
+
+
+def lsa_decode_attention(ctx: LsaContext, q, out=None, want_lse=False):
+    return ctx.decode_attention(q, out, want_lse)
+
+
+def lsa_step(ctx: LsaContext, q, h, k_new=None, v_new=None, out=None):
+    return ctx.step(q, h, k_new, v_new, out)
+
+
+def lsa_version() -> int:
+    return _lib.lsa_version()

@@ -38,3 +38,111 @@ def apply_emb_updates(wl: LsaWorkload, oracle: LsaOracle, global_step: int, gpu_
         oracle.chunk_emb[b][ids] = rows
         if gpu_embs is not None:
             gpu_embs[b][torch.from_numpy(ids).to(gpu_embs[b].device)] = to_torch(rows, c.dtype).to(gpu_embs[b].device)
+
+
+# ------------------------------------------------------------------------------------------
+# GPU side (only used by -m gpu tests and smoke)
+# ------------------------------------------------------------------------------------------
+class GpuRig:
+    """Device / pinned tensors of one workload plus the LsaContext built on them."""
+
+    def __init__(self, wl: LsaWorkload, trigger_idx: int = 0, device="cuda:0", **ctx_over):
+        import torch
+        from paper_2606_09079_b200 import lsa
+        from paper_2606_09079_b200.workloads import to_torch
+        c = wl.cfg
+        self.wl, self.cfg, self.device = wl, c, torch.device(device)
+        dt = c.dtype
+        tdt = torch.float32 if dt == "f32" else torch.bfloat16
+        dev = self.device
+        self.hot_pool = torch.zeros((c.hot_pages, 2, c.C, c.D), dtype=tdt, device=dev)
+        self.W_q = to_torch(wl.W_q, dt).to(dev)
+        self.cold = [to_torch(x, dt).pin_memory() for x in wl.cold_csa]
+        self.emb = [to_torch(wl.chunk_emb(b, trigger_idx), dt).to(dev) for b in range(c.B)]
+        self.hca_k = [to_torch(x, dt).to(dev) for x in wl.hca_k]
+        self.hca_v = [to_torch(x, dt).to(dev) for x in wl.hca_v]
+        self.win_k = [to_torch(x, dt).to(dev) for x in wl.win_k]
+        self.win_v = [to_torch(x, dt).to(dev) for x in wl.win_v]
+        seqs = []
+        for b in range(c.B):
+            seqs.append(dict(cold_csa=self.cold[b], n_csa=c.n_csa(b), chunk_emb=self.emb[b],
+                             hca_k=self.hca_k[b], hca_v=self.hca_v[b], win_k=self.win_k[b], win_v=self.win_v[b],
+                             w_len=min(c.W, c.L[b]), w_head=0, step0=c.step0(b)))
+        kw = dict(dtype=lsa.LSA_F32 if dt == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W, Dh=c.Dh, E=c.E,
+                  k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=self.W_q, seqs=seqs, recall_lag=c.recall_lag)
+        kw.update(ctx_over)
+        self.ctx = lsa.LsaContext(**kw)
+        self.tdt = tdt
+
+    def dev(self, arr):
+        from paper_2606_09079_b200.workloads import to_torch
+        return to_torch(arr, self.cfg.dtype).to(self.device)
+
+    def host(self, t):
+        from paper_2606_09079_b200.workloads import as_f64, from_torch
+        return as_f64(from_torch(t, self.cfg.dtype), self.cfg.dtype)
+
+
+def attn_tolerance(dtype: str):
+    """BASELINE.json north_star: abs 2e-2 / rel 1e-2 for bf16 inputs, 1e-4 for the fp32 config."""
+    return dict(atol=2e-2, rtol=1e-2) if dtype == "bf16" else dict(atol=1e-4, rtol=1e-4)
+
+
+def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=None, with_kv_new: bool = True,
+                 tie_emb_builder=None):
+    """Drive lsa_step and the oracle in lock-step: validate the GPU's
+    selection against the oracle's scores, feed it to the oracle's residency model, then compare page
+    tables / residency / fetched bytes bit-exactly and attention outputs within tolerance."""
+    import torch
+    from oracle import validate_selection
+    c = wl.cfg
+    orc = make_oracle(wl)
+    tol = attn_tolerance(c.dtype)
+    n_checked, max_err = 0, 0.0
+    for t in range(steps):
+        apply_emb_updates(wl, orc, t, rig.emb)
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t) if with_kv_new else (None, None)
+        firing = [b for b in range(c.B) if orc.step[b] % c.tau == 0]
+        bytes_before = rig.ctx.stats()["bytes_fetched"] if not firing else None
+        out_gpu = rig.ctx.step(rig.dev(q), rig.dev(h), None if kn is None else rig.dev(kn),
+                               None if vn is None else rig.dev(vn))
+        forced = {}
+        for b in firing:                      # GPU selection = chunk ids of the table it just staged
+            which = 0 if c.recall_lag == 0 else 1
+            chunks, pages = rig.ctx.page_table(b, which)
+            sc = orc.scores(b, h[b])
+            order = sorted(chunks, key=lambda ch: (-sc[ch], ch))
+            import numpy as _np
+            padded = _np.full(c.k, -1, dtype=_np.int64); padded[: len(order)] = order
+            msg = validate_selection(padded, sc, c.k)
+            assert msg is None, f"step {t} seq {b}: {msg}"
+            forced[b] = chunks
+        orc.step_begin(h, forced_selection=forced if firing else None)
+        for b in firing:
+            which = 0 if c.recall_lag == 0 else 1
+            chunks, pages = rig.ctx.page_table(b, which)
+            ref = orc.pool.cur[b] if c.recall_lag == 0 else orc.pool.nxt[b]
+            assert list(zip(chunks, pages)) == ref, f"step {t} seq {b}: page table mismatch"
+            assert rig.ctx.residency(b, c.n_chunks(b)) == orc.pool.page_of[b], f"step {t} seq {b}: residency mismatch"
+        if firing:
+            st = rig.ctx.stats()
+            assert (st["hits"], st["misses"], st["evictions"], st["bytes_fetched"], st["pool_error"]) == \
+                   (orc.pool.hits, orc.pool.misses, orc.pool.evictions, orc.pool.bytes_fetched, 0), f"step {t}: counters"
+            hot = rig.hot_pool.cpu()
+            from paper_2606_09079_b200.workloads import from_torch
+            hot_np = from_torch(hot, c.dtype)
+            owned = [p for p, o in enumerate(orc.pool.owner) if o is not None]
+            assert _np.array_equal(hot_np[owned], orc.pool.hot[owned]), f"step {t}: fetched bytes differ"
+        else:
+            assert rig.ctx.stats()["bytes_fetched"] == bytes_before      # P:185 zero transfers inside a window
+        attend = check_attention_at is None or t in check_attention_at
+        res = orc.step_end(q, kn, vn, attend=attend)
+        if attend:
+            got = rig.host(out_gpu)
+            import numpy as np
+            np.testing.assert_allclose(got, res[0], err_msg=f"attention mismatch at step {t}", **tol)
+            max_err = max(max_err, float(np.max(np.abs(got - res[0]))))
+            n_checked += 1
+    rig.ctx.sync()
+    return dict(checked=n_checked, max_abs_err=max_err, oracle=orc)

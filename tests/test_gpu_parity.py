@@ -1,0 +1,323 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): chunk indices, page tables, residency, counters and fetched bytes
+bit-exact (selection swaps only inside the 1e-5-relative band around the k-th oracle score, never
+among bit-identical scores); attention within abs 2e-2 / rel 1e-2 (bf16) or 1e-4 (fp32).
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from lsa_harness import GpuRig, attn_tolerance, make_oracle, run_lockstep
+from oracle import ResidencyOracle, attention, chunk_scores, query_tower, topk_select, validate_selection, widen
+from paper_2606_09079_b200.workloads import (LsaWorkload, as_f64, from_torch, make_config, make_small_config,
+                                             plant_boundary_ties, store, to_torch)
+
+pytestmark = pytest.mark.gpu
+
+
+def _lsa():
+    from paper_2606_09079_b200 import lsa
+    return lsa
+
+
+# ------------------------------------------------------------------------------- S1-S3
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_index_select_matches_oracle_order(dtype):
+    cfg = make_small_config(dtype, B=3, L=[65536, 32768, 1024], C=16, E=128, Dh=512, k=24, hot_pages=256)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    orc = make_oracle(wl)
+    for t in (0, 5):
+        h = wl.h(t)
+        sel, sc = rig.ctx.index_select(rig.dev(h), [0, 1, 2])
+        rig.ctx.sync()
+        sel, sc = sel.cpu().numpy(), sc.cpu().numpy().astype(np.float64)
+        for b in range(cfg.B):
+            osc = orc.scores(b, h[b])
+            assert validate_selection(sel[b], osc, cfg.k) is None
+            ke = cfg.k_eff(b)
+            np.testing.assert_allclose(sc[b, :ke], osc[sel[b, :ke]], atol=2e-6, rtol=1e-5)
+            assert np.all(sc[b, ke:] == -np.inf)
+    # subset call: rows of h follow seq_ids
+    h = wl.h(9)
+    sel2, _ = rig.ctx.index_select(rig.dev(h[[2, 0]][::-1].copy()), [0, 2])
+    sel_all, _ = rig.ctx.index_select(rig.dev(h), [0, 1, 2])
+    rig.ctx.sync()
+    assert torch.equal(sel2[0], sel_all[0]) and torch.equal(sel2[1], sel_all[2])
+
+
+def test_index_select_exact_ties_and_zero_query():
+    cfg = make_config(5, B=2, L=[524288, 524288], hot_pages=512)
+    wl = LsaWorkload(cfg, build_kv=False)
+    # index-only context: K/V tensors are tiny dummies
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    orc_scores = []
+    embs = []
+    h = wl.h(0)
+    for b in range(cfg.B):
+        emb = wl.chunk_emb(b, 0)
+        qh = query_tower(wl.W_q, h[b])
+        order = topk_select(chunk_scores(qh, emb), cfg.n_chunks(b))[0]
+        emb = plant_boundary_ties(emb, order, cfg.k, cfg.dtype)
+        if b == 1:            # many exact duplicates of the best row
+            emb[100:140] = emb[order[0]]
+        embs.append(emb)
+        orc_scores.append(chunk_scores(qh, emb))
+    cold = [torch.zeros((cfg.n_chunks(b), 2, cfg.C, cfg.D), dtype=torch.bfloat16).pin_memory() for b in range(cfg.B)]
+    emb_d = [to_torch(e, "bf16").to(dev) for e in embs]
+    z = torch.zeros((8, cfg.D), dtype=torch.bfloat16, device=dev)
+    seqs = [dict(cold_csa=cold[b], n_csa=cfg.n_csa(b), chunk_emb=emb_d[b], hca_k=z, hca_v=z, win_k=z.clone(),
+                 win_v=z.clone(), w_len=0) for b in range(cfg.B)]
+    ctx = lsa.LsaContext(dtype=lsa.LSA_BF16, H=cfg.H, D=cfg.D, C_=cfg.C, W=8, Dh=cfg.Dh, E=cfg.E, k=cfg.k, tau=cfg.tau,
+                         hot_pool=torch.zeros((cfg.hot_pages, 2, cfg.C, cfg.D), dtype=torch.bfloat16, device=dev),
+                         W_q=to_torch(wl.W_q, "bf16").to(dev), seqs=seqs)
+    sel, sc = ctx.index_select(to_torch(h, "bf16").to(dev), [0, 1])
+    ctx.sync()
+    sel = sel.cpu().numpy()
+    for b in range(cfg.B):
+        assert validate_selection(sel[b], orc_scores[b], cfg.k) is None
+    dup = set(range(100, 140))
+    got = [c for c in sel[1].tolist() if c in dup or orc_scores[1][c] == orc_scores[1][100]]
+    assert got == sorted(got)                          # equal scores come out in ascending chunk id
+    # zero hidden state: every score is 0 -> lowest chunk ids (R16)
+    sel0, sc0 = ctx.index_select(torch.zeros((2, cfg.Dh), dtype=torch.bfloat16, device=dev), [0, 1])
+    ctx.sync()
+    assert sel0[0].tolist() == list(range(cfg.k)) and torch.all(sc0 == 0)
+    ctx.close()
+
+
+def test_topk_radix_path_many_chunks():
+    """n_chunks > 4096 exercises the radix-select branch of S3."""
+    cfg = make_small_config("f32", B=1, L=[6000 * 16 * 4], C=16, D=64, H=8, E=64, Dh=128, k=50, hot_pages=128,
+                            emb_mode="uniform", n_needles=0)
+    wl = LsaWorkload(cfg)
+    assert cfg.n_chunks(0) == 6000
+    rig = GpuRig(wl)
+    orc = make_oracle(wl)
+    for t in range(3):
+        h = wl.h(t)
+        sel, sc = rig.ctx.index_select(rig.dev(h), [0])
+        rig.ctx.sync()
+        assert validate_selection(sel[0].cpu().numpy(), orc.scores(0, h[0]), cfg.k) is None
+
+
+# ------------------------------------------------------------------------------- S4-S5
+@pytest.mark.parametrize("lag", [0, 1])
+def test_fetch_chunks_lockstep_random_selections(lag):
+    cfg = make_small_config("bf16", B=3, L=[4096, 2432, 1280], C=16, k=5, hot_pages=30 + 3, recall_lag=lag)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    n_chunks = [cfg.n_chunks(b) for b in range(cfg.B)]
+    ref = ResidencyOracle(cfg.B, n_chunks, cfg.hot_pages, wl.cold_csa)
+    g = np.random.default_rng(5)
+    for it in range(25):
+        ids = sorted(g.choice(cfg.B, size=g.integers(1, cfg.B + 1), replace=False).tolist())
+        sel = np.full((len(ids), cfg.k), -1, dtype=np.int32)
+        for i, b in enumerate(ids):
+            ke = min(cfg.k, n_chunks[b])
+            sel[i, :ke] = g.choice(n_chunks[b], size=ke, replace=False)
+        rig.ctx.fetch_chunks(ids, torch.from_numpy(sel).to(rig.device))
+        for i, b in enumerate(ids):
+            ref.fetch(b, sel[i], 0, 0)
+        for b in ids:
+            ch, pg = rig.ctx.page_table(b, 1)
+            assert list(zip(ch, pg)) == ref.nxt[b]
+        rig.ctx.commit_tables()
+        for b in range(cfg.B):
+            ref.maybe_swap(b, 0)
+            ch, pg = rig.ctx.page_table(b, 0)
+            assert list(zip(ch, pg)) == ref.cur[b]
+            assert rig.ctx.residency(b, n_chunks[b]) == ref.page_of[b]
+        st = rig.ctx.stats()
+        assert (st["hits"], st["misses"], st["evictions"], st["bytes_fetched"]) == \
+               (ref.hits, ref.misses, ref.evictions, ref.bytes_fetched)
+        hot = from_torch(rig.hot_pool.cpu(), "bf16")
+        owned = [p for p, o in enumerate(ref.owner) if o is not None]
+        assert np.array_equal(hot[owned], ref.hot[owned])
+    assert ref.evictions > 0
+
+
+def test_residency_radix_path_many_pages():
+    """hot_pages > 4096 exercises the radix-select branch of S4 (victim selection)."""
+    cfg = make_small_config("f32", B=2, L=[6000 * 16 * 4, 3000 * 16 * 4], C=16, D=64, H=8, E=64, Dh=128, k=40,
+                            hot_pages=5000, emb_mode="uniform", n_needles=0, recall_lag=0)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    n_chunks = [cfg.n_chunks(b) for b in range(cfg.B)]
+    ref = ResidencyOracle(cfg.B, n_chunks, cfg.hot_pages, wl.cold_csa)
+    g = np.random.default_rng(6)
+    for it in range(140):                              # 140 * 80 selections > 5000 pages -> LRU kicks in
+        sel = np.stack([g.choice(n_chunks[b], size=cfg.k, replace=False) for b in range(2)]).astype(np.int32)
+        rig.ctx.fetch_chunks([0, 1], torch.from_numpy(sel).to(rig.device))
+        rig.ctx.commit_tables()
+        for b in range(2):
+            ref.fetch(b, sel[b], 0, 0)
+            ref.maybe_swap(b, 0)
+        if it % 20 == 19 or it > 130:
+            for b in range(2):
+                ch, pg = rig.ctx.page_table(b, 0)
+                assert list(zip(ch, pg)) == ref.cur[b], f"iteration {it}"
+    st = rig.ctx.stats()
+    assert ref.evictions > 0 and (st["hits"], st["misses"], st["evictions"]) == (ref.hits, ref.misses, ref.evictions)
+
+
+def test_init_rejects_unpinned_and_small_pool():
+    lsa = _lsa()
+    cfg = make_small_config("f32")
+    wl = LsaWorkload(cfg)
+    with pytest.raises(lsa.LsaError, match="hot_pages"):
+        GpuRig(LsaWorkload(make_small_config("f32", hot_pages=5)))
+    rig = GpuRig(wl)
+    z = torch.zeros((4, cfg.D), device=rig.device)
+    with pytest.raises(lsa.LsaError, match="pinned"):
+        lsa.LsaContext(dtype=0, H=cfg.H, D=cfg.D, C_=cfg.C, W=4, Dh=cfg.Dh, E=cfg.E, k=1, tau=4, hot_pool=rig.hot_pool,
+                       W_q=rig.W_q, seqs=[dict(cold_csa=torch.zeros((2, 2, cfg.C, cfg.D)), n_csa=20, chunk_emb=rig.emb[0],
+                                               hca_k=z, hca_v=z, win_k=z.clone(), win_v=z.clone())])
+    with pytest.raises(lsa.LsaError, match="UNSUPPORTED"):
+        lsa.LsaContext(dtype=0, H=24, D=64, C_=cfg.C, W=4, Dh=cfg.Dh, E=cfg.E, k=1, tau=4, hot_pool=rig.hot_pool,
+                       W_q=rig.W_q, seqs=[dict(cold_csa=rig.cold[0], n_csa=20, chunk_emb=rig.emb[0], hca_k=z, hca_v=z,
+                                               win_k=z.clone(), win_v=z.clone())])
+
+
+# ------------------------------------------------------------------------------- S7-S8
+def _direct_ctx(dtype, H, D, C, hca_k, hca_v, win_k, win_v, w_len, W, **kw):
+    """A context with no CSA chunks at all: attention over HCA + window only."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    tdt = torch.float32 if dtype == "f32" else torch.bfloat16
+    B = len(hca_k)
+    seqs = [dict(cold_csa=None, n_csa=0, chunk_emb=None, hca_k=hca_k[b], hca_v=hca_v[b], win_k=win_k[b], win_v=win_v[b],
+                 w_len=w_len[b]) for b in range(B)]
+    return lsa.LsaContext(dtype=0 if dtype == "f32" else 1, H=H, D=D, C_=C, W=W, Dh=64, E=64, k=1, tau=4,
+                          hot_pool=torch.zeros((2 * B, 2, C, D), dtype=tdt, device=dev),
+                          W_q=torch.zeros((64, 64), dtype=tdt, device=dev), seqs=seqs, **kw)
+
+
+@pytest.mark.parametrize("dtype,H,D", [("f32", 16, 128), ("bf16", 64, 512), ("bf16", 8, 64), ("f32", 64, 64)])
+def test_attention_edge_cases(dtype, H, D):
+    dev = torch.device("cuda:0")
+    tdt = torch.float32 if dtype == "f32" else torch.bfloat16
+    g = torch.Generator().manual_seed(1)
+    W = 40
+    rnd = lambda *s: (torch.randn(*s, generator=g)).to(tdt).to(dev)
+    # seq 0: exactly one key (in HCA), empty window; seq 1: no keys at all; seq 2: all keys equal;
+    # seq 3: ragged 37 HCA rows + 29 window rows with large logits
+    hk = [rnd(1, D), torch.zeros((0, D), dtype=tdt, device=dev), rnd(1, D).expand(33, D).contiguous(), rnd(37, D)]
+    hv = [rnd(1, D), torch.zeros((0, D), dtype=tdt, device=dev), rnd(33, D), rnd(37, D)]
+    wk = [rnd(W, D) for _ in range(4)]
+    wv = [rnd(W, D) for _ in range(4)]
+    w_len = [0, 0, 0, 29]
+    ctx = _direct_ctx(dtype, H, D, 16, hk, hv, wk, wv, w_len, W, sm_scale=0.5)
+    q = rnd(4, H, D)
+    out, lse = ctx.decode_attention(q, want_lse=True)
+    ctx.sync()
+    out64 = out.double().cpu().numpy()
+    lse = lse.cpu().numpy()
+    tol = attn_tolerance(dtype)
+    # single key -> exactly that key's value
+    assert torch.equal(out[0], hv[0].expand(H, D)), "single-key attention must return the value row bit-exactly"
+    # no keys -> zeros, lse = -inf
+    assert torch.all(out[1] == 0) and np.all(lse[1] == -np.inf)
+    # equal keys -> mean of V
+    np.testing.assert_allclose(out64[2], np.broadcast_to(hv[2].double().mean(0).cpu().numpy(), (H, D)), **tol)
+    # ragged + large logits vs oracle
+    K = np.concatenate([hk[3].double().cpu().numpy(), wk[3][:29].double().cpu().numpy()])
+    V = np.concatenate([hv[3].double().cpu().numpy(), wv[3][:29].double().cpu().numpy()])
+    ref, ref_lse, _ = attention(q[3].double().cpu().numpy(), K, V, 0.5)
+    np.testing.assert_allclose(out64[3], ref, **tol)
+    np.testing.assert_allclose(lse[3], ref_lse, atol=2e-2 if dtype == "bf16" else 1e-4, rtol=1e-3)
+    ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("lag", [0, 1])
+def test_lockstep_small(dtype, lag):
+    cfg = make_small_config(dtype, recall_lag=lag, steps=14, q_gain=8.0)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    r = run_lockstep(wl, rig, cfg.steps)
+    assert r["checked"] == cfg.steps
+
+
+@pytest.mark.parametrize("max_ctas", [1, 3, 0])
+def test_lockstep_small_split_counts(max_ctas):
+    """Split-K geometry must not change results: 1 split, 3 splits, one full wave."""
+    cfg = make_small_config("f32", steps=6, q_gain=8.0)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl, max_ctas=max_ctas)
+    run_lockstep(wl, rig, cfg.steps)
+
+
+def test_k_equals_all_chunks_is_dense_attention():
+    cfg = make_small_config("f32", B=2, L=[2048, 1216], k=32, hot_pages=128, recall_lag=0, tau=4, q_gain=8.0)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    q = wl.q(0)
+    out = rig.host(rig.ctx.step(rig.dev(q), rig.dev(wl.h(0))))
+    for b in range(cfg.B):
+        ncsa = cfg.n_csa(b)
+        cold = as_f64(wl.cold_csa[b], "f32")
+        Kd = np.concatenate([as_f64(wl.hca_k[b], "f32"), cold[:, 0].reshape(-1, cfg.D)[:ncsa], as_f64(wl.win_k[b], "f32")])
+        Vd = np.concatenate([as_f64(wl.hca_v[b], "f32"), cold[:, 1].reshape(-1, cfg.D)[:ncsa], as_f64(wl.win_v[b], "f32")])
+        ref = torch.nn.functional.scaled_dot_product_attention(
+            torch.from_numpy(as_f64(q[b], "f32"))[None], torch.from_numpy(Kd)[None], torch.from_numpy(Vd)[None],
+            scale=1 / math.sqrt(cfg.D))[0].numpy()
+        np.testing.assert_allclose(out[b], ref, atol=1e-4, rtol=1e-4)
+
+
+# ------------------------------------------------------------------------------- BASELINE configs
+def test_cfg1_every_step():
+    wl = LsaWorkload(make_config(1))
+    rig = GpuRig(wl)
+    r = run_lockstep(wl, rig, wl.cfg.steps)
+    assert r["checked"] == 128
+    st = rig.ctx.stats()
+    assert st["triggers"] == 2 and st["misses"] == 4 and st["hits"] == 4
+
+
+def _sample_steps(cfg, steps):
+    s = set()
+    for t in range(steps):
+        if t % cfg.tau == 0 or t % cfg.tau == 1 or t % 64 == 37:
+            s.add(t)
+    return s
+
+
+def test_cfg2_sampled():
+    wl = LsaWorkload(make_config(2))
+    rig = GpuRig(wl)
+    steps = 64 * 9 + 2                      # crosses two needle-drift epochs (every 4 triggers)
+    r = run_lockstep(wl, rig, steps, check_attention_at=_sample_steps(wl.cfg, steps))
+    assert r["checked"] >= 27
+
+
+def test_cfg3_sampled_bench_launch_config():
+    wl = LsaWorkload(make_config(3))
+    rig = GpuRig(wl)
+    steps = 64 * 5 + 2
+    r = run_lockstep(wl, rig, steps, check_attention_at=_sample_steps(wl.cfg, steps))
+    assert r["checked"] >= 15
+    assert rig.ctx.stats()["misses"] >= 64
+
+
+def test_cfg5_churn_sampled():
+    cfg = make_config(5)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    steps = 16 * 4 + 2
+    r = run_lockstep(wl, rig, steps, check_attention_at={0, 1, 16, 17, 33, 64, 65})
+    st = rig.ctx.stats()
+    assert st["evictions"] > 0 and st["misses"] > 3 * 8 * 128 * 0.6
+
+
+def test_cfg4_ragged_batch_sampled():
+    cfg = make_config(4)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    steps = 70
+    r = run_lockstep(wl, rig, steps, check_attention_at={0, 1, 3, 63, 64, 65, 69})
+    assert rig.ctx.stats()["triggers"] == 32 + 3      # every sequence once, sequences 0..2 twice
