@@ -80,6 +80,7 @@ class GpuRig:
 
     def host(self, t):
         from paper_2606_09079_b200.workloads import as_f64, from_torch
+        self.ctx.sync()          # the library's streams are not torch's current stream
         return as_f64(from_torch(t, self.cfg.dtype), self.cfg.dtype)
 
 
