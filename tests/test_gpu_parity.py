@@ -233,6 +233,57 @@ def test_attention_edge_cases(dtype, H, D):
     ctx.close()
 
 
+@pytest.mark.parametrize("max_ctas", [0, 1, 5])
+def test_tcgen05_attention_edge_cases(max_ctas):
+    """The tensor-core kernel (bf16, H=64, D=512, C=128): single key, no keys, equal keys, ragged
+    segments, and a running maximum that jumps by far more than 2^8 between tiles (O rescale path)."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 200
+    g = torch.Generator().manual_seed(2)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    qdir = torch.randn(D, generator=g)
+    qdir = qdir / qdir.norm()
+    ramp = (torch.arange(700).float()[:, None] / 700.0 * 90.0) * qdir[None, :]            # logits grow with the row id
+    ramp_k = (ramp + 0.05 * torch.randn(700, D, generator=g)).to(torch.bfloat16).to(dev)
+    hk = [rnd(1, D), torch.zeros((0, D), dtype=torch.bfloat16, device=dev), rnd(1, D).expand(333, D).contiguous(), rnd(37, D), ramp_k]
+    hv = [rnd(1, D), torch.zeros((0, D), dtype=torch.bfloat16, device=dev), rnd(333, D), rnd(37, D), rnd(700, D)]
+    wk = [rnd(W, D) for _ in range(5)]
+    wv = [rnd(W, D) for _ in range(5)]
+    w_len = [0, 0, 0, 29, 130]
+    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.5, max_ctas=max_ctas,
+                      attn_impl=lsa.LSA_ATTN_TCGEN05)
+    assert ctx.stats()["attn_impl"] == lsa.LSA_ATTN_TCGEN05
+    q = rnd(5, H, D)
+    q[4] = (qdir[None, :] * (1.0 + 0.1 * torch.rand(H, 1, generator=g))).to(torch.bfloat16).to(dev)
+    out, lse = ctx.decode_attention(q, want_lse=True)
+    ctx.sync()
+    out64, lse = out.double().cpu().numpy(), lse.cpu().numpy()
+    tol = attn_tolerance("bf16")
+    assert torch.equal(out[0], hv[0].expand(H, D)), "single-key attention must return the value row bit-exactly"
+    assert torch.all(out[1] == 0) and np.all(lse[1] == -np.inf)
+    np.testing.assert_allclose(out64[2], np.broadcast_to(hv[2].double().mean(0).cpu().numpy(), (H, D)), **tol)
+    for b in (3, 4):
+        K = np.concatenate([hk[b].double().cpu().numpy(), wk[b][: w_len[b]].double().cpu().numpy()])
+        V = np.concatenate([hv[b].double().cpu().numpy(), wv[b][: w_len[b]].double().cpu().numpy()])
+        ref, ref_lse, _ = attention(q[b].double().cpu().numpy(), K, V, 0.5)
+        np.testing.assert_allclose(out64[b], ref, **tol)
+        np.testing.assert_allclose(lse[b], ref_lse, atol=2e-2, rtol=1e-3)
+    ctx.close()
+
+
+@pytest.mark.parametrize("impl", ["simt", "tcgen05"])
+def test_flagship_shape_short_context_both_impls(impl):
+    """bf16 H=64 D=512 C=128 at a short context, with a partial last chunk, through both kernels."""
+    lsa = _lsa()
+    cfg = make_config(2, L=[16384 + 4 * 37], W=1024, k=6, hot_pages=16, steps=70, name="cfg2_short", q_gain=16.0, tau=32)
+    assert cfg.n_csa(0) % cfg.C != 0
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl, attn_impl=lsa.LSA_ATTN_SIMT if impl == "simt" else lsa.LSA_ATTN_TCGEN05)
+    r = run_lockstep(wl, rig, cfg.steps, check_attention_at={0, 1, 2, 31, 32, 33, 34, 64, 65, 69})
+    assert r["checked"] == 10
+
+
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("lag", [0, 1])
 def test_lockstep_small(dtype, lag):
