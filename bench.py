@@ -22,7 +22,6 @@ import math
 import os
 import subprocess
 import sys
-import tempfile
 import time
 
 import numpy as np
@@ -118,29 +117,41 @@ class Replica:
 
 
 def clocks_sampler_start(dev_index):
-    f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    """nvidia-smi polled every 100 ms while the timed region runs (B200_PROFILING.md clocks line); lines
+    are read from a pipe by a thread because nvidia-smi block-buffers when writing to a file."""
+    import threading
     q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
     try:
         p = subprocess.Popen(["nvidia-smi", f"--id={dev_index}", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100"],
-                             stdout=f, stderr=subprocess.DEVNULL)
+                             stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
     except Exception:
-        return None, f
-    return p, f
+        return None, None
+    lines = []
+
+    def pump():
+        for line in p.stdout:
+            lines.append((time.perf_counter(), line))
+
+    th = threading.Thread(target=pump, daemon=True)
+    th.start()
+    return p, (lines, th)
 
 
-def clocks_sampler_stop(p, f):
+def clocks_sampler_stop(p, state, t_begin=None, t_end=None):
     if p is None:
         return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+    lines, th = state
     p.terminate()
     try:
         p.wait(timeout=5)
     except Exception:
         p.kill()
-    f.flush()
-    f.seek(0)
+    th.join(timeout=5)
     sm, smax, reasons = [], [], set()
-    for line in f.read().splitlines():
+    for ts, line in lines:
+        if t_begin is not None and not (t_begin <= ts <= t_end + 0.15):
+            continue
         parts = [x.strip() for x in line.split(",")]
         if len(parts) < 7:
             continue
@@ -151,8 +162,6 @@ def clocks_sampler_stop(p, f):
         for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), parts[3:7]):
             if v.lower().startswith("active"):
                 reasons.add(name)
-    f.close()
-    os.unlink(f.name)
     return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(smax) if smax else None,
                 samples=len(sm), reasons=sorted(reasons))
 
@@ -263,14 +272,15 @@ def main():
         return ms, wall
 
     # ---- warm-up, then the device-resident timed region ----
+    samp, sampf = clocks_sampler_start(local_rank)
     for i in range(warmup):
         one_step(i)
     i_next = warmup
-    st0 = reps[0].ctx.stats()
     launches0 = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps)
-    samp, sampf = clocks_sampler_start(local_rank)
+    t_begin = time.perf_counter()
     ms, wall = timed(args.steps, i0=i_next)
-    clocks = clocks_sampler_stop(samp, sampf)
+    t_end = time.perf_counter()
+    clocks = clocks_sampler_stop(samp, sampf, t_begin, t_end)
     i_next += args.steps
     launches = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps) - launches0
     value = world * args.steps * per_step_units / (ms * 1e-3)

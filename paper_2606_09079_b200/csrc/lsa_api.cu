@@ -378,6 +378,8 @@ static int prestep_impl(lsa_ctx* c, bool force, const void* k_new, const void* v
   ProfScope prof(c, LSA_PH_PRESTEP, c->sc);
   LSA_CUDA(c, launch_prestep(c->cfg.dtype, c->d_seqs, c->B, c->cfg.D, c->cfg.W, any ? words : nullptr, 32, k_new, v_new, c->sc));
   c->attn_launches += 1;
+  if (k_new)                                      // host mirror of the ring fill (the kernel applies the same rule)
+    for (int b = 0; b < c->B; ++b) c->seq_host[b].w_len = std::min(c->cfg.W, c->seq_host[b].w_len + 1);
   return LSA_OK;
 }
 
@@ -405,7 +407,10 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse) {
     int launches = 0, ctas = 0;
     std::string msg;
     ProfScope prof(c, LSA_PH_ATTENTION, c->sc);   // attention + combine of the tcgen05 path
-    int rc = tc_attention(c->tc, q, out, lse, c->sc, &launches, &ctas, &msg);
+    long long tiles = 0;                          // host mirror: HCA + selected pages + window, in 128-key tiles
+    for (int b = 0; b < c->B; ++b)
+      tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
+    int rc = tc_attention(c->tc, q, out, lse, tiles, c->sc, &launches, &ctas, &msg);
     if (rc != 0) LSA_FAIL(c, rc, "tcgen05 attention: %s", msg.c_str());
     c->attn_launches += launches;
     c->last_attn_ctas = ctas;

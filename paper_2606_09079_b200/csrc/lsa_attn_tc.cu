@@ -1,78 +1,145 @@
 // lsa_attn_tc.cu - host side of the tcgen05 attention (tensor maps, launch) and the S8 combine kernel.
 // Kernel: lsa_attn_tc_kernel.cuh.  Design notes: lsa_attn_tc_defs.cuh.
+#include <cstdio>
+#include <cstdlib>
+
 #include "lsa_attn_tc_kernel.cuh"
 
 namespace lsa {
 
 // ---- S8: merge the split partials of one sequence  ----------------------------------------------
 //   m* = max m_i ; l* = sum l_i 2^(m_i-m*) ; out = sum o_i 2^(m_i-m*) / l* ; lse = ln2 (m* + log2 l*)
-// grid (2*H, B), 256 threads: block = one head, one half of D; thread = one output element.
-__global__ void __launch_bounds__(256)
+// Partials are stored as [d-block m][head half][head quad g][d_local 128][4 heads] (the order the
+// attention epilogue drains TMEM in).  grid (128, B): block = (m, half, g, 64 of the 128 d); 512 threads =
+// 64 d x 8 groups, group j accumulates partials j, j+8, ... with one float4 (4 heads) per thread, 1 KiB
+// contiguous per partial per group.  Launched with programmatic stream serialization: the launch and
+// prologue overlap the attention kernel's tail.
+constexpr int kCombineThreads = 512;
+// The combine grid is launched while attention CTAs still own most SMs (PDL).  Asking for more than half an
+// SM's shared memory keeps its blocks at one per SM, so the early ones cannot pile up on the few idle SMs.
+constexpr int kCombineSmemPad = 116 * 1024;
+
+__global__ void __launch_bounds__(kCombineThreads)
 combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
-  __shared__ float w_s[256];
-  __shared__ int red_i[8][3];
-  __shared__ float red_f[8];
-  __shared__ int s_lo, s_hi;
+  __shared__ float4 w_s[256];
+  __shared__ int slot_s[256];
+  __shared__ float4 red_f[16];
+  __shared__ int warp_cnt[16];
+  __shared__ float4 acc_s[8][64];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int h = blockIdx.x >> 1, d = (blockIdx.x & 1) * 256 + tid, b = blockIdx.y;
-  // group counts: before b, of b, total
-  int pre = 0, mine = 0, tot = 0;
-  for (int i = tid; i < p.B; i += 256) {
-    const int g = seq_groups(p.seqs[i]);
-    tot += g;
-    if (i < b) pre += g;
-    if (i == b) mine = g;
+  const int dh = blockIdx.x & 1, g = (blockIdx.x >> 1) & 7, hh = (blockIdx.x >> 4) & 1, m = blockIdx.x >> 5, b = blockIdx.y;
+  const int h0 = hh * 32 + g * 4;
+#ifdef LSA_TC_TRACE
+  const unsigned long long g_entry = gtime();
+#endif
+  griddep_wait();                                 // partials and piece_info are final from here on
+  griddep_launch_dependents();                    // the next kernel in the stream may start its own prologue
+#ifdef LSA_TC_TRACE
+  const unsigned long long g_dep = gtime();
+#endif                                 // partials and piece_info are final from here on
+  // thread c < n_cta looks at CTA c: did it write a partial for sequence b?  (n_cta <= 256)
+  bool active = false;
+  float4 mi = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY), li = make_float4(0.f, 0.f, 0.f, 0.f);
+  const size_t slot = (size_t)tid + b;
+  if (tid < n_cta) {
+    const int2 info = p.piece_info[tid];
+    const float4 m4 = *reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0);
+    const float4 l4 = *reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0);
+    active = info.x <= b && b < info.x + info.y;
+    if (active) { mi = m4; li = l4; }
   }
+  float4 mmax = mi;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
-    pre += __shfl_xor_sync(0xffffffffu, pre, o);
-    mine += __shfl_xor_sync(0xffffffffu, mine, o);
-    tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    mmax.x = fmaxf(mmax.x, __shfl_xor_sync(0xffffffffu, mmax.x, o));
+    mmax.y = fmaxf(mmax.y, __shfl_xor_sync(0xffffffffu, mmax.y, o));
+    mmax.z = fmaxf(mmax.z, __shfl_xor_sync(0xffffffffu, mmax.z, o));
+    mmax.w = fmaxf(mmax.w, __shfl_xor_sync(0xffffffffu, mmax.w, o));
   }
-  if (lane == 0) { red_i[warp][0] = pre; red_i[warp][1] = mine; red_i[warp][2] = tot; }
+  const unsigned bal = __ballot_sync(0xffffffffu, active);
+  if (lane == 0) { red_f[warp] = mmax; warp_cnt[warp] = __popc(bal); }
   __syncthreads();
-  pre = mine = tot = 0;
-  for (int w = 0; w < 8; ++w) { pre += red_i[w][0]; mine += red_i[w][1]; tot += red_i[w][2]; }
-  // which CTAs hold a piece of sequence b (same partition arithmetic as PieceCursor)
-  bool active = false;
-  if (tid < n_cta && mine > 0) {
-    const int f0 = (int)((long long)tid * tot / n_cta), f1 = (int)((long long)(tid + 1) * tot / n_cta);
-    active = f0 < f1 && f0 < pre + mine && f1 > pre;
+  float4 m_star = red_f[0];
+  int base = 0, n_act = 0;
+  for (int w = 0; w < 16; ++w) {
+    const float4 r = red_f[w];
+    m_star.x = fmaxf(m_star.x, r.x); m_star.y = fmaxf(m_star.y, r.y); m_star.z = fmaxf(m_star.z, r.z); m_star.w = fmaxf(m_star.w, r.w);
+    if (w < warp) base += warp_cnt[w];
+    n_act += warp_cnt[w];
   }
-  const size_t slot = (size_t)tid + b;
-  const float mi = active ? p.part_m[slot * kTcH + h] : -INFINITY;
-  float mmax = mi;
+  float4 wi = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (active) {                                   // compacted list of (slot, weights of the 4 heads)
+    wi.x = mi.x == -INFINITY ? 0.f : exp2f(mi.x - m_star.x);
+    wi.y = mi.y == -INFINITY ? 0.f : exp2f(mi.y - m_star.y);
+    wi.z = mi.z == -INFINITY ? 0.f : exp2f(mi.z - m_star.z);
+    wi.w = mi.w == -INFINITY ? 0.f : exp2f(mi.w - m_star.w);
+    const int pos = base + __popc(bal & ((1u << lane) - 1));
+    w_s[pos] = wi;
+    slot_s[pos] = (int)slot;
+  }
+  float4 lsum = make_float4(wi.x * li.x, wi.y * li.y, wi.z * li.z, wi.w * li.w);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) mmax = fmaxf(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
-  if (tid == 0) { s_lo = 1 << 30; s_hi = -1; }
-  __syncthreads();
-  if (lane == 0) red_f[warp] = mmax;
-  if (active) { atomicMin(&s_lo, tid); atomicMax(&s_hi, tid); }
-  __syncthreads();
-  float m_star = red_f[0];
-  for (int w = 1; w < 8; ++w) m_star = fmaxf(m_star, red_f[w]);
-  const float wi = (active && mi != -INFINITY) ? exp2f(mi - m_star) : 0.f;
-  w_s[tid] = wi;
-  float lsum = active ? wi * p.part_l[slot * kTcH + h] : 0.f;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) lsum += __shfl_xor_sync(0xffffffffu, lsum, o);
-  __syncthreads();
+  for (int o = 16; o > 0; o >>= 1) {
+    lsum.x += __shfl_xor_sync(0xffffffffu, lsum.x, o);
+    lsum.y += __shfl_xor_sync(0xffffffffu, lsum.y, o);
+    lsum.z += __shfl_xor_sync(0xffffffffu, lsum.z, o);
+    lsum.w += __shfl_xor_sync(0xffffffffu, lsum.w, o);
+  }
+  __syncthreads();                                // red_f is reused; w_s / slot_s are complete
   if (lane == 0) red_f[warp] = lsum;
   __syncthreads();
-  float l_star = 0.f;
-  for (int w = 0; w < 8; ++w) l_star += red_f[w];
-  const bool empty = !(l_star > 0.f);
-  float acc = 0.f;
-  const int lo = s_lo, hi = s_hi;
-  const float* po = p.part_o + ((size_t)b * kTcH + h) * kTcD + d;     // slot i+b -> + i * H * D
-#pragma unroll 4
-  for (int i = lo; i <= hi; ++i) {
-    const float w = w_s[i];                       // 0 for CTAs without a piece: their slot is never read
-    if (w != 0.f) acc = fmaf(w, po[(size_t)i * (kTcH * kTcD)], acc);
+  float4 l_star = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int w = 0; w < 16; ++w) {
+    const float4 r = red_f[w];
+    l_star.x += r.x; l_star.y += r.y; l_star.z += r.z; l_star.w += r.w;
   }
-  out[((size_t)b * kTcH + h) * kTcD + d] = __float2bfloat16_rn(empty ? 0.f : acc / l_star);
-  if (lse && (blockIdx.x & 1) == 0 && tid == 0)
-    lse[(size_t)b * kTcH + h] = empty ? -INFINITY : (m_star + log2f(l_star)) * 0.6931471805599453f;
+#ifdef LSA_TC_TRACE
+  const unsigned long long g_w = gtime();
+#endif
+  // ---- weighted sum of the partials ----
+  const int dl = tid & 63, grp = tid >> 6;
+  const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dh * 64 + dl;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  constexpr int U = 8;                            // independent 16-byte loads in flight per thread
+  for (int i0 = grp; i0 < n_act; i0 += 8 * U) {
+    float4 v[U], w[U];
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      const int i = i0 + 8 * j;
+      const bool ok = i < n_act;
+      w[j] = ok ? w_s[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+      v[j] = ok ? po[(size_t)slot_s[i] * (kTcH * kTcD / 4)] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      acc.x = fmaf(w[j].x, v[j].x, acc.x); acc.y = fmaf(w[j].y, v[j].y, acc.y);
+      acc.z = fmaf(w[j].z, v[j].z, acc.z); acc.w = fmaf(w[j].w, v[j].w, acc.w);
+    }
+  }
+#ifdef LSA_TC_TRACE
+  const unsigned long long g_l = gtime();
+#endif
+  acc_s[grp][dl] = acc;
+  __syncthreads();
+  if (tid < 256) {                                // thread = one output element: head h0 + e, d = m*128 + dh*64 + dl
+    const int e = tid >> 6;
+    const float* a = reinterpret_cast<const float*>(acc_s);
+    float s = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) s += a[(w * 64 + dl) * 4 + e];
+    const float ls = e == 0 ? l_star.x : e == 1 ? l_star.y : e == 2 ? l_star.z : l_star.w;
+    out[((size_t)b * kTcH + h0 + e) * kTcD + m * 128 + dh * 64 + dl] = __float2bfloat16_rn(ls > 0.f ? s / ls : 0.f);
+  }
+#ifdef LSA_TC_TRACE
+  __syncthreads();
+  if (tid == 0 && blockIdx.x == 0 && b == 0) { tlog_add(p.tlog, 3, g_entry); tlog_add(p.tlog, 4, g_dep); tlog_add(p.tlog, 6, g_w); tlog_add(p.tlog, 7, g_l); }
+  if (tid == 0 && blockIdx.x == gridDim.x - 1 && b == 0) tlog_add(p.tlog, 5, g_dep);
+#endif
+  if (lse && m == 0 && dh == 0 && tid < 4) {
+    const float ls = tid == 0 ? l_star.x : tid == 1 ? l_star.y : tid == 2 ? l_star.z : l_star.w;
+    const float ms = tid == 0 ? m_star.x : tid == 1 ? m_star.y : tid == 2 ? m_star.z : m_star.w;
+    lse[(size_t)b * kTcH + h0 + tid] = ls > 0.f ? (ms + log2f(ls)) * 0.6931471805599453f : -INFINITY;
+  }
 }
 
 // ---- host ------------------------------------------------------------------------------------------
@@ -87,18 +154,21 @@ struct TcPlan {
   const void* q_cached = nullptr;
   CUtensorMap* d_maps = nullptr;
   TcParams params{};
-  int grid = 0;
+  int grid_max = 0;
   size_t smem = 0;
 };
 
 bool tc_supported(int dtype, int H, int D, int C) { return dtype == 1 && H == kTcH && D == kTcD && C == kTcC; }
 
-static bool encode_rows(EncodeTiledFn enc, CUtensorMap* m, const void* ptr, uint64_t rows, uint32_t box_rows, std::string* msg) {
-  cuuint64_t dims[2] = {(cuuint64_t)kTcD, rows};
-  cuuint64_t strides[1] = {(cuuint64_t)kTcD * 2};
-  cuuint32_t box[2] = {64, box_rows};
-  cuuint32_t es[2] = {1, 1};
-  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, es,
+// A [rows][512] bf16 matrix seen as (64 columns, rows, 8 d-blocks): one box = [d-blocks][box_rows][128 B],
+// which is exactly the K-major / MN-major 128-byte-swizzle operand image tcgen05.mma reads.
+static bool encode_rows(EncodeTiledFn enc, CUtensorMap* m, const void* ptr, uint64_t rows, uint32_t box_rows, uint32_t box_dblocks,
+                        std::string* msg) {
+  cuuint64_t dims[3] = {64, rows, (cuuint64_t)kTcD / 64};
+  cuuint64_t strides[2] = {(cuuint64_t)kTcD * 2, 128};
+  cuuint32_t box[3] = {64, box_rows, box_dblocks};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, es,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
@@ -126,9 +196,9 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
   if (e != cudaSuccess || !fn) { *msg = "cuTensorMapEncodeTiled entry point not found"; delete pl; return -2; }
   pl->encode = (EncodeTiledFn)fn;
-  pl->grid = init.max_ctas > 0 ? std::min(init.max_ctas, init.n_sms) : init.n_sms;
-  if (pl->grid > 256) pl->grid = 256;
-  if (!encode_rows(pl->encode, &pl->map_pool, init.hot_pool, (uint64_t)init.P * 2 * kTcC, 32, msg)) { delete pl; return -2; }
+  pl->grid_max = init.max_ctas > 0 ? std::min(init.max_ctas, init.n_sms) : init.n_sms;
+  if (pl->grid_max > 256) pl->grid_max = 256;
+  if (!encode_rows(pl->encode, &pl->map_pool, init.hot_pool, (uint64_t)init.P * 2 * kTcC, kTcTile, 2, msg)) { delete pl; return -2; }
   std::vector<CUtensorMap> maps((size_t)init.B * 4);
   for (int b = 0; b < init.B; ++b) {
     const SeqDev& s = init.seq_host[b];
@@ -136,7 +206,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
     const uint64_t rows[4] = {(uint64_t)s.n_hca, (uint64_t)s.n_hca, (uint64_t)init.W, (uint64_t)init.W};
     for (int j = 0; j < 4; ++j) {
       const bool none = rows[j] == 0 || ptrs[j] == nullptr;     // never referenced: point at the pool
-      if (!encode_rows(pl->encode, &maps[(size_t)b * 4 + j], none ? init.hot_pool : ptrs[j], none ? 32 : rows[j], 32, msg)) {
+      if (!encode_rows(pl->encode, &maps[(size_t)b * 4 + j], none ? init.hot_pool : ptrs[j], none ? kTcTile : rows[j], kTcTile, 2, msg)) {
         delete pl;
         return -2;
       }
@@ -150,41 +220,101 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   }
   TC_CUDA(cudaMalloc(&pl->d_maps, maps.size() * sizeof(CUtensorMap)));
   TC_CUDA(cudaMemcpy(pl->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
-  const size_t slots = (size_t)pl->grid + init.B;
+  const size_t slots = (size_t)pl->grid_max + init.B;
   TcParams& p = pl->params;
   p.seqs = init.d_seqs; p.tbl_chunk = init.pool.tbl_chunk; p.tbl_page = init.pool.tbl_page; p.seq_maps = pl->d_maps;
-  p.B = init.B; p.k = init.k; p.pool_rows = init.P * 2 * kTcC;
+  p.B = init.B; p.k = init.k;
   p.scale_log2 = init.sm_scale * 1.4426950408889634f;
   TC_CUDA(cudaMalloc(&p.part_o, slots * kTcH * kTcD * sizeof(float)));
   TC_CUDA(cudaMalloc(&p.part_m, slots * kTcH * sizeof(float)));
   TC_CUDA(cudaMalloc(&p.part_l, slots * kTcH * sizeof(float)));
+  TC_CUDA(cudaMalloc(&p.piece_info, (size_t)pl->grid_max * sizeof(int2)));
+  TC_CUDA(cudaMemset(p.part_m, 0, slots * kTcH * sizeof(float)));
+  TC_CUDA(cudaMemset(p.part_l, 0, slots * kTcH * sizeof(float)));
+  TC_CUDA(cudaMemset(p.piece_info, 0, (size_t)pl->grid_max * sizeof(int2)));
+#ifdef LSA_TC_TRACE
+  TC_CUDA(cudaMalloc(&p.trace, (size_t)pl->grid_max * 3 * 32 * sizeof(long long)));
+  TC_CUDA(cudaMemset(p.trace, 0, (size_t)pl->grid_max * 3 * 32 * sizeof(long long)));
+  TC_CUDA(cudaMalloc(&p.tlog, (1 + 3 * 4096) * sizeof(unsigned long long)));
+  TC_CUDA(cudaMemset(p.tlog, 0, (1 + 3 * 4096) * sizeof(unsigned long long)));
+#endif
   pl->smem = sizeof(TcSmem) + 1024;
   TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
+  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
   *out = pl;
   return 0;
 }
 
-int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, cudaStream_t st, int* launches, int* ctas,
+// One CTA per SM streams at up to ~85 GB/s, twice its fair share of HBM, so the grid is sized to give every
+// CTA the same number of whole tiles (e.g. 192 tiles -> 96 CTAs x 2) instead of one CTA per SM with a ragged
+// last tile: fewer split partials for S8 to merge, no padded MMA work.
+static int pick_grid(const TcPlan* pl, long long tiles_est) {
+  const int g = pl->grid_max;
+  if (tiles_est <= 0) return 1;
+  const long long per = (tiles_est + g - 1) / g;
+  return (int)std::max<long long>(1, std::min<long long>(g, (tiles_est + per - 1) / per));
+}
+
+int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long tiles_est, cudaStream_t st, int* launches, int* ctas,
                  std::string* msg) {
   if (q != pl->q_cached) {
-    if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, 64, msg)) return -2;
+    if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
     pl->q_cached = q;
   }
-  attn_tc_kernel<<<pl->grid, kTcThreads, pl->smem, st>>>(pl->map_pool, pl->map_q, pl->params);
-  TC_CUDA(cudaGetLastError());
-  combine_tc_kernel<<<dim3(kTcH * 2, pl->init.B), 256, 0, st>>>(pl->params, pl->grid, (__nv_bfloat16*)out, lse);
-  TC_CUDA(cudaGetLastError());
+  const int grid = pick_grid(pl, tiles_est);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t lc{};
+  lc.gridDim = dim3(grid); lc.blockDim = dim3(kTcThreads); lc.dynamicSmemBytes = pl->smem; lc.stream = st;
+  lc.attrs = attr; lc.numAttrs = 1;
+#ifdef LSA_TC_TRACE
+  static const int no_pdl = getenv("LSA_NO_PDL") ? atoi(getenv("LSA_NO_PDL")) : 0;   // 1: combine, 2: attention, 3: both
+  if (no_pdl & 2) lc.numAttrs = 0;
+#endif
+  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel, pl->map_pool, pl->map_q, pl->params));
+  cudaLaunchConfig_t lc2{};
+  lc2.gridDim = dim3(128, pl->init.B); lc2.blockDim = dim3(kCombineThreads); lc2.dynamicSmemBytes = kCombineSmemPad; lc2.stream = st;
+  lc2.attrs = attr; lc2.numAttrs = 1;
+#ifdef LSA_TC_TRACE
+  if (no_pdl & 1) lc2.numAttrs = 0;
+#endif
+  TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel, pl->params, grid, (__nv_bfloat16*)out, lse));
   *launches = 2;
-  *ctas = pl->grid;
+  *ctas = grid;
   return 0;
 }
 
 void tc_destroy(TcPlan* pl) {
   if (!pl) return;
+#ifdef LSA_TC_TRACE
+  if (const char* path = getenv("LSA_TC_TRACE_FILE")) {
+    std::vector<long long> h((size_t)pl->grid_max * 3 * 32);
+    cudaMemcpy(h.data(), pl->params.trace, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+    if (FILE* f = fopen(path, "w")) {
+      for (int c = 0; c < pl->grid_max; ++c)
+        for (int r = 0; r < 3; ++r) {
+          fprintf(f, "%d %d", c, r);
+          for (int i = 0; i < 32; ++i) fprintf(f, " %lld", h[((size_t)c * 3 + r) * 32 + i]);
+          fprintf(f, "\n");
+        }
+      fclose(f);
+    }
+    std::vector<unsigned long long> tl(1 + 3 * 4096);
+    cudaMemcpy(tl.data(), pl->params.tlog, tl.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    if (FILE* f = fopen((std::string(path) + ".tlog").c_str(), "w")) {
+      for (unsigned long long i = 0; i < tl[0] && i < 4096; ++i) fprintf(f, "%llu %llu %llu\n", tl[1 + 3 * i], tl[2 + 3 * i], tl[3 + 3 * i]);
+      fclose(f);
+    }
+  }
+  cudaFree(pl->params.trace);
+  cudaFree(pl->params.tlog);
+#endif
   cudaFree(pl->d_maps);
   cudaFree(pl->params.part_o);
   cudaFree(pl->params.part_m);
   cudaFree(pl->params.part_l);
+  cudaFree(pl->params.piece_info);
   delete pl;
 }
 

@@ -22,8 +22,9 @@ struct TcInit {
 // bf16, H = 64 query heads sharing one K/V of D = 512, pages of C = 128 rows (BASELINE cfg 2-5)
 bool tc_supported(int dtype, int H, int D, int C);
 int tc_create(const TcInit& init, TcPlan** out, std::string* msg);   // 0 or an lsa_status
-int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, cudaStream_t st, int* launches, int* ctas,
-                 std::string* msg);
+// tiles_est: upper estimate of the batch's 128-key tiles (sizes the grid; the kernel partitions the exact list)
+int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, cudaStream_t st, int* launches,
+                 int* ctas, std::string* msg);
 void tc_destroy(TcPlan* plan);
 
 }  // namespace lsa

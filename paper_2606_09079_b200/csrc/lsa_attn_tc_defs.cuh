@@ -1,4 +1,4 @@
-// lsa_attn_tc.cu - S7 split-K decode attention on tcgen05 tensor cores + TMA, and S8 combine (sm_100a)
+// lsa_attn_tc_defs.cuh - S7 split-K decode attention on tcgen05 tensor cores + TMA, and S8 combine (sm_100a)
 //
 // Shape: bf16, H = 64 query heads sharing ONE K and ONE V of D = 512 (MQA, DESIGN R19),
 // pages of C = 128 rows (BASELINE.json configs 2-5).  Per key the path moves 2 KiB and does
@@ -7,18 +7,24 @@
 // Formulation ("keys on M"): with only 64 heads a head-major MMA would run at M = 64, i.e. half rate, and
 // its 64x512 fp32 accumulator would fill all 512 TMEM columns.  Instead each 128-key tile computes
 //     S^T[128 keys x 64 heads] = K_tile[128 x 512] . Q^T            (A = K, K-major;  B = Q, K-major)
-//     O^T[512 x 64 heads]     += V_tile^T[512 x 128] . P^T           (A = V, MN-major; B = P, K-major)
+//     O^T[512 x 64 heads]     += V_tile^T[512 x 128] . P^T           (A = V, MN-major; B = P, MN-major)
 //     L  [128 x 64 heads]     += 1[128 x 128]        . P^T           (row sums of P for free)
 // all at M = 128, N = 64: every K and V byte is read from shared memory exactly once, straight from the
-// swizzled TMA landing buffers, and O^T needs only 4 x 64 TMEM columns.
+// swizzled TMA landing buffers, and O^T needs only 4 x 64 TMEM columns.  At N = 64 one MMA reads
+// 4 KiB of A + 2 KiB of B from shared memory, i.e. it is paced by the 128 B/clk shared-memory port
+// (48 clk per MMA, measured) - 3456 clk per 128-key tile against >= 5700 clk of TMA time per tile.
 //
-// One persistent CTA per SM owns a contiguous range of 32-key groups of the batch's flat key list
-// (HCA rows, pages of the current table, window rows - per sequence, in that order) and emits one
-// (m, l, o) partial per sequence it touches; lsa_combine_tc merges them (S8).
-//   warp 0   : TMA producer   - Q tile, then K/V stages (4-deep ring of 32 KiB = 128 keys x 128 dims)
-//   warp 1   : MMA issuer     - one elected thread issues tcgen05.mma / tcgen05.commit
-//   warps 2-5: softmax        - thread <-> key: TMEM -> regs, masked scale, cross-lane max via
-//                               redux.sync, 2^(x-m) -> bf16 P tile in swizzled smem; lazy O rescale;
+// Work unit: a TILE = 128 consecutive rows of one tensor (HCA rows [128j, 128j+128), one page of the
+// current table, window rows [128j, ...)), so every TMA box is one 32 KiB [2 d-blocks][128 rows][128 B]
+// image (3-D tensor map: 64 columns x rows x 8 d-blocks).  The flat tile list of the batch (per sequence:
+// HCA tiles, pages in table order, window tiles) is cut into gridDim.x contiguous ranges; a CTA emits one
+// (m, l, o) partial per sequence it touches and lsa_combine_tc merges them (S8).
+//   warp 0    : TMA producer  - Q tile (one 64 KiB box), then K/V stages (4-deep ring of 32 KiB)
+//   warp 1    : MMA issuer    - one elected thread issues tcgen05.mma / tcgen05.commit
+//   warps 2-9 : softmax       - thread <-> (key, half of the heads): TMEM -> regs, masked scale,
+//                               2^(x-m) -> bf16 P tile (8 heads per 16-byte store, swizzled);
+//                               the running maximum is exact on the first tile of a piece and kept
+//                               until a logit exceeds it by 2^8 (one OR-reduction barrier per tile);
 //                               epilogue TMEM -> partial in global memory
 #pragma once
 #include <cuda.h>
@@ -32,21 +38,31 @@ namespace lsa {
 using namespace ptx;
 
 constexpr int kTcH = 64, kTcD = 512, kTcC = 128;
+constexpr int kTcTile = 128;                // keys per tile
 constexpr int kTcStages = 4;
-constexpr int kTcStageBytes = 32768;
-constexpr int kTcThreads = 192;
+constexpr int kTcStageBytes = 32768;        // [2 d-blocks][128 rows][128 B]
+constexpr int kTcSoftmaxWarps = 8;
+constexpr int kTcThreads = 64 + 32 * kTcSoftmaxWarps;
 constexpr int kTcMaxB = 256;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P may grow to 2^8 before O is rescaled
+
+// per-sequence shape as of this launch
+struct SeqView {
+  int b, t_hca, n_cur, n_hca, w_len, cur;
+  long long n_csa;
+};
 
 struct TcSmem {
   alignas(1024) unsigned char q[65536];                       // [8 d-blocks][64 heads][128 B], SW128
   alignas(1024) unsigned char stage[kTcStages][kTcStageBytes];// [2 d-blocks][128 keys][128 B], SW128
-  alignas(1024) unsigned char p[16384];                       // [2 key-blocks][64 heads][128 B], SW128
+  alignas(1024) unsigned char p[16384];                       // [128 keys][64 heads] bf16, SW128 (MN-major B)
   alignas(1024) unsigned char ones[4096];                     // 128 x 16 bf16 ones, no swizzle
-  float wmax[2][kTcH][4];                                     // per-warp tile maxima (ordered ints)
-  int gpre[kTcMaxB + 1];                                      // prefix of 32-key groups per sequence
+  alignas(16) float wmax[2][32][4];                           // [head half][head][lane quarter] tile maxima
+  alignas(16) float mtile[2][4][32];                          // [head half][lane quarter][head] merged tile maxima
+  SeqView view[kTcMaxB];                                      // per-sequence shape, read once by warp 0
+  int gpre[kTcMaxB + 1];                                      // prefix of tiles per sequence
   uint64_t full[kTcStages], empty[kTcStages];
-  uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_empty;
+  uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup;
   uint32_t tmem_base;
 };
 
@@ -55,98 +71,109 @@ struct TcParams {
   const int* tbl_chunk;
   const int* tbl_page;
   const CUtensorMap* seq_maps;   // [B][4]: hca_k, hca_v, win_k, win_v
-  int B, k, pool_rows;
+  int B, k;
   float scale_log2;
-  float* part_o;                 // [slots][H][D]
+  float* part_o;                 // [slots][4 d-blocks][2 head halves][8 head quads][128 d][4 heads]  (= H*D floats)
   float* part_m;                 // [slots][H]   (log2 domain)
   float* part_l;                 // [slots][H]
+  int2* piece_info;              // [grid]: (first sequence, number of sequences) this CTA wrote partials for
+#ifdef LSA_TC_TRACE
+  long long* trace;              // [grid][3 roles][32] clock64 stamps (debug builds only)
+  unsigned long long* tlog;      // [0] = entries; then (kernel id, globaltimer start, end) per launch of block 0
+#endif
 };
 
-__device__ __forceinline__ int seq_groups(const SeqDev& s) {
-  return (s.n_hca + 31) / 32 + s.n_tbl[s.cur_buf] * (kTcC / 32) + (s.w_len + 31) / 32;
+__host__ __device__ __forceinline__ int tc_tiles(int n_hca, int n_cur, int w_len) {
+  return (n_hca + kTcTile - 1) / kTcTile + n_cur + (w_len + kTcTile - 1) / kTcTile;
 }
+__device__ __forceinline__ int seq_tiles(const SeqDev& s) { return tc_tiles(s.n_hca, s.n_tbl[s.cur_buf], s.w_len); }
 
-// where a 32-key group of a sequence lives
-struct GroupSrc {
-  const CUtensorMap* mk;
-  const CUtensorMap* mv;
-  int row_k, row_v, n_valid;
-};
-
-struct SeqView {
-  int b, g_hca, n_cur, n_hca, w_len, cur;
-  long long n_csa;
-};
-
-__device__ __forceinline__ SeqView make_view(const TcParams& p, int b) {
-  const SeqDev& s = p.seqs[b];
+__device__ __forceinline__ SeqView make_view(const SeqDev& s, int b) {
   SeqView v;
-  v.b = b; v.n_hca = s.n_hca; v.g_hca = (s.n_hca + 31) / 32; v.cur = s.cur_buf; v.n_cur = s.n_tbl[s.cur_buf];
+  v.b = b; v.n_hca = s.n_hca; v.t_hca = (s.n_hca + kTcTile - 1) / kTcTile; v.cur = s.cur_buf; v.n_cur = s.n_tbl[s.cur_buf];
   v.w_len = s.w_len; v.n_csa = s.n_csa;
   return v;
 }
 
-__device__ __forceinline__ GroupSrc resolve_group(const TcParams& p, const CUtensorMap* map_pool, const SeqView& v, int g,
-                                                  int g_end) {
-  GroupSrc r;
-  if (g >= g_end) {                       // beyond this CTA's range: whole box out of bounds -> TMA zero fill
-    r.mk = r.mv = map_pool; r.row_k = r.row_v = p.pool_rows; r.n_valid = 0;
-    return r;
-  }
-  if (g < v.g_hca) {
+// where tile t of a sequence lives
+struct TileSrc {
+  const CUtensorMap* mk;
+  const CUtensorMap* mv;
+  int row_k, row_v;
+};
+
+__device__ __forceinline__ TileSrc tile_src(const TcParams& p, const CUtensorMap* map_pool, const SeqView& v, int t) {
+  TileSrc r;
+  if (t < v.t_hca) {
     r.mk = p.seq_maps + v.b * 4 + 0; r.mv = p.seq_maps + v.b * 4 + 1;
-    r.row_k = r.row_v = g * 32; r.n_valid = min(32, v.n_hca - g * 32);
+    r.row_k = r.row_v = t * kTcTile;
     return r;
   }
-  g -= v.g_hca;
-  if (g < v.n_cur * 4) {
-    const int slot = g >> 2, r0 = (g & 3) * 32;
-    const size_t ti = ((size_t)v.b * 2 + v.cur) * p.k + slot;
-    const int chunk = p.tbl_chunk[ti], page = p.tbl_page[ti];
-    const long long valid_rows = v.n_csa - (long long)chunk * kTcC;
+  t -= v.t_hca;
+  if (t < v.n_cur) {
+    const int page = p.tbl_page[((size_t)v.b * 2 + v.cur) * p.k + t];
     r.mk = r.mv = map_pool;
-    r.row_k = page * (2 * kTcC) + r0; r.row_v = r.row_k + kTcC;
-    r.n_valid = (int)max(0ll, min(32ll, valid_rows - r0));
+    r.row_k = page * (2 * kTcC); r.row_v = r.row_k + kTcC;
     return r;
   }
-  g -= v.n_cur * 4;
+  t -= v.n_cur;
   r.mk = p.seq_maps + v.b * 4 + 2; r.mv = p.seq_maps + v.b * 4 + 3;
-  r.row_k = r.row_v = g * 32; r.n_valid = min(32, v.w_len - g * 32);
+  r.row_k = r.row_v = t * kTcTile;
   return r;
 }
 
-// Iterates the (sequence, group range) pieces of this CTA's share [f0, f1) of the flat group list.
+// attended rows of tile t (the rest of its 128 rows is masked)
+__device__ __forceinline__ int tile_valid(const TcParams& p, const SeqView& v, int t) {
+  if (t < v.t_hca) return min(kTcTile, v.n_hca - t * kTcTile);
+  t -= v.t_hca;
+  if (t < v.n_cur) {
+    const int chunk = p.tbl_chunk[((size_t)v.b * 2 + v.cur) * p.k + t];
+    return (int)max(0ll, min((long long)kTcC, v.n_csa - (long long)chunk * kTcC));
+  }
+  t -= v.n_cur;
+  return min(kTcTile, v.w_len - t * kTcTile);
+}
+
+// Iterates the (sequence, tile range) pieces of this CTA's share [f0, f1) of the flat tile list.
+// 32-bit arithmetic: T < 2^21 tiles, n_cta <= 256.
 struct PieceCursor {
   const int* gpre;
   int B, f, f1, b;
   __device__ PieceCursor(const int* gpre_, int B_, int cta, int n_cta) : gpre(gpre_), B(B_) {
-    const long long T = gpre_[B_];
-    f = (int)((long long)cta * T / n_cta);
-    f1 = (int)((long long)(cta + 1) * T / n_cta);
+    const unsigned T = (unsigned)gpre_[B_];
+    f = (int)((unsigned)cta * T / (unsigned)n_cta);
+    f1 = (int)((unsigned)(cta + 1) * T / (unsigned)n_cta);
     b = 0;
   }
-  // returns false when exhausted; else fills b_out and the group range [g0, g1) inside sequence b_out
-  __device__ bool next(int& b_out, int& g0, int& g1) {
+  // returns false when exhausted; else fills b_out and the tile range [t0, t1) inside sequence b_out
+  __device__ bool next(int& b_out, int& t0, int& t1) {
     if (f >= f1) return false;
     while (gpre[b + 1] <= f) ++b;
     b_out = b;
-    g0 = f - gpre[b];
+    t0 = f - gpre[b];
     const int end = min(f1, gpre[b + 1]);
-    g1 = end - gpre[b];
+    t1 = end - gpre[b];
     f = end;
     return true;
   }
 };
+
+#ifdef LSA_TC_TRACE
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ void tlog_add(unsigned long long* tlog, unsigned long long id, unsigned long long t0) {
+  const unsigned long long i = atomicAdd(tlog, 1ull);
+  if (i < 4096) { tlog[1 + 3 * i] = id; tlog[2 + 3 * i] = t0; tlog[3 + 3 * i] = gtime(); }
+}
+#endif
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-__device__ __forceinline__ int float_ordered_s32(float f) {   // monotone float -> signed int
-  int b = __float_as_int(f);
-  return b >= 0 ? b : (b ^ 0x7fffffff);
-}
-__device__ __forceinline__ float s32_ordered_float(int i) { return __int_as_float(i >= 0 ? i : (i ^ 0x7fffffff)); }
 
 }  // namespace lsa

@@ -4,31 +4,55 @@
 
 namespace lsa {
 
+#ifdef LSA_TC_TRACE
+// debug builds only (_work/): per-CTA, per-role clock64 stamps relative to kernel entry
+#define TR(role, slot) do { if ((slot) < 32) p.trace[((size_t)blockIdx.x * 3 + (role)) * 32 + (slot)] = clock64() - t_entry; } while (0)
+#else
+#define TR(role, slot) do { } while (0)
+#endif
+
+// Order of the K/V stage groups of a piece with tiles t0..t1-1, for the producer and the MMA issuer alike:
+//   K(t0) | K(t0+1) V(t0) | K(t0+2) V(t0+1) | ... | V(t1-1)
+// K runs one tile ahead of V, so S(t+1) is computed (and K(t+2) is in flight) while the softmax of tile t
+// runs; with the 4-stage ring a V tile never waits behind the K tile that depends on its completion.
+
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_constant__ CUtensorMap map_q, TcParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   TcSmem& sm = *reinterpret_cast<TcSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int cta = blockIdx.x, n_cta = gridDim.x;
+#ifdef LSA_TC_TRACE
+  const long long t_entry = clock64();
+  const unsigned long long g_entry = gtime();
+#endif
 
-  // ---- one-time setup ---------------------------------------------------------------------------
+  // ---- setup: mbarriers first (one cheap block barrier), everything slower overlaps behind `setup` ----
   if (tid == 0) {
     for (int i = 0; i < kTcStages; ++i) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], 1); }
     mbar_init(&sm.q_full, 1); mbar_init(&sm.q_empty, 1);
-    for (int i = 0; i < 2; ++i) { mbar_init(&sm.s_full[i], 1); mbar_init(&sm.s_empty[i], 4); }
-    mbar_init(&sm.p_full, 4); mbar_init(&sm.pv_done, 1); mbar_init(&sm.o_empty, 4);
+    for (int i = 0; i < 2; ++i) { mbar_init(&sm.s_full[i], 1); mbar_init(&sm.s_empty[i], kTcSoftmaxWarps); }
+    mbar_init(&sm.p_full, kTcSoftmaxWarps); mbar_init(&sm.pv_done, 1); mbar_init(&sm.o_empty, kTcSoftmaxWarps);
+    for (int i = 0; i < 4; ++i) mbar_init(&sm.o_full[i], 1);
+    mbar_init(&sm.setup, kTcThreads / 32);
     fence_mbar_init();
     prefetch_tmap(&map_pool);
     prefetch_tmap(&map_q);
   }
-  if (warp == 1) tmem_alloc(&sm.tmem_base, 512);
-  for (int i = tid; i < 2048; i += kTcThreads) reinterpret_cast<uint16_t*>(sm.ones)[i] = 0x3f80;   // bf16 1.0
-  // prefix of groups per sequence (B <= 256): warp 0 scans
+  __syncthreads();
+  griddep_wait();                 // PDL: everything below may read what the previous kernel wrote
+  griddep_launch_dependents();    // the combine kernel may start its prologue; it waits for this grid itself
   if (warp == 0) {
+    // per-sequence shape and the prefix of tiles per sequence (B <= 256)
     int carry = 0;
     for (int base = 0; base < p.B; base += 32) {
       const int b = base + lane;
-      int g = b < p.B ? seq_groups(p.seqs[b]) : 0;
+      int g = 0;
+      if (b < p.B) {
+        const SeqView v = make_view(p.seqs[b], b);
+        sm.view[b] = v;
+        g = v.t_hca + v.n_cur + (v.w_len + kTcTile - 1) / kTcTile;
+      }
       int incl = g;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -39,247 +63,311 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       carry += __shfl_sync(0xffffffffu, incl, 31);
     }
     if (lane == 0) sm.gpre[0] = 0;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm.setup);
+  } else if (warp == 1) {
+    tmem_alloc(&sm.tmem_base, 512);
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm.setup);
+  } else {
+    for (int i = tid - 64; i < 2048; i += kTcThreads - 64) reinterpret_cast<uint16_t*>(sm.ones)[i] = 0x3f80;   // bf16 1.0
+    fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&sm.setup);
   }
-  fence_proxy_async_smem();
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = sm.tmem_base;
-  const uint32_t tS = tmem, tO = tmem + 128, tL = tmem + 384;
 
   if (warp == 0) {
-    // =========================== TMA producer ===========================
-    if (lane == 0) {
+    // =========================== TMA producer (does not wait for `setup`: it wrote gpre itself) ===========
+    if (elect_one()) {
       PieceCursor cur(sm.gpre, p.B, cta, n_cta);
-      int b, g0, g1, item = 0;
+      int b, t0, t1, item = 0;
       uint32_t ring = 0;                                  // stages issued so far
-      while (cur.next(b, g0, g1)) {
+      auto issue4 = [&](const CUtensorMap* m, int row) {
+#pragma unroll 1
+        for (int s4 = 0; s4 < 4; ++s4) {
+          const int st = ring % kTcStages;
+          mbar_wait(&sm.empty[st], ((ring / kTcStages) & 1) ^ 1, 11);
+          mbar_arrive_expect_tx(&sm.full[st], kTcStageBytes);
+          tma_load_3d(sm.stage[st], m, 0, row, s4 * 2, &sm.full[st]);
+          TR(0, 2 + ring);
+          ++ring;
+        }
+      };
+      TR(0, 0);
+      while (cur.next(b, t0, t1)) {
+        const SeqView v = sm.view[b];
+        TileSrc src = tile_src(p, &map_pool, v, t0);      // table look-up overlaps the Q issue
         if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 10);
         mbar_arrive_expect_tx(&sm.q_full, 65536);
-        for (int db = 0; db < 8; ++db) tma_load_2d(sm.q + db * 8192, &map_q, db * 64, b * kTcH, &sm.q_full);
-        const SeqView v = make_view(p, b);
-        const int n_tiles = (g1 - g0 + 3) >> 2;
-        for (int t = 0; t < n_tiles; ++t) {
-          GroupSrc src[4];
-#pragma unroll
-          for (int gi = 0; gi < 4; ++gi) src[gi] = resolve_group(p, &map_pool, v, g0 + t * 4 + gi, g1);
-#pragma unroll 1
-          for (int kv = 0; kv < 2; ++kv) {
-#pragma unroll 1
-            for (int s4 = 0; s4 < 4; ++s4) {
-              const int st = ring % kTcStages;
-              mbar_wait(&sm.empty[st], ((ring / kTcStages) & 1) ^ 1, 11);
-              mbar_arrive_expect_tx(&sm.full[st], kTcStageBytes);
-#pragma unroll
-              for (int db = 0; db < 2; ++db)
-#pragma unroll
-                for (int gi = 0; gi < 4; ++gi)
-                  tma_load_2d(sm.stage[st] + db * 16384 + gi * 4096, kv ? src[gi].mv : src[gi].mk, (s4 * 2 + db) * 64,
-                              kv ? src[gi].row_v : src[gi].row_k, &sm.full[st]);
-              ++ring;
-            }
+        tma_load_3d(sm.q, &map_q, 0, b * kTcH, 0, &sm.q_full);
+        TR(0, 1);
+        issue4(src.mk, src.row_k);
+        for (int t = t0; t < t1; ++t) {
+          TileSrc nxt = src;
+          if (t + 1 < t1) {
+            nxt = tile_src(p, &map_pool, v, t + 1);
+            issue4(nxt.mk, nxt.row_k);
           }
+          issue4(src.mv, src.row_v);
+          src = nxt;
         }
         ++item;
       }
     }
   } else if (warp == 1) {
     // =========================== MMA issuer ===========================
-    if (lane == 0) {
-      constexpr uint32_t id_kk = make_idesc_bf16(128, 64, 0, 0);   // A K-major  (K tile, ones)
-      constexpr uint32_t id_mn = make_idesc_bf16(128, 64, 1, 0);   // A MN-major (V tile)
-      const uint32_t q_addr = smem_u32(sm.q), p_addr = smem_u32(sm.p);
+    if (elect_one()) {
+      constexpr uint32_t id_s = make_idesc_bf16(128, 64, 0, 0);    // A = K tile (K-major),  B = Q   (K-major)
+      constexpr uint32_t id_pv = make_idesc_bf16(128, 64, 1, 1);   // A = V tile (MN-major), B = P^T (MN-major)
+      constexpr uint32_t id_l = make_idesc_bf16(128, 64, 0, 1);    // A = ones   (K-major),  B = P^T (MN-major)
+      mbar_wait(&sm.setup, 0, 19);
+      tc_fence_after();
+      const uint32_t tmem = sm.tmem_base;
+      const uint32_t tS = tmem, tO = tmem + 128, tL = tmem + 384;
+      // descriptors of stage 0 / the Q tile / the P tile; everything else is a constant added to the address field
+      const uint64_t dk0 = make_sdesc(smem_u32(sm.stage[0]), 16, 1024, kLayoutSw128);
+      const uint64_t dv0 = make_sdesc(smem_u32(sm.stage[0]), 16384, 1024, kLayoutSw128);
+      const uint64_t dq0 = make_sdesc(smem_u32(sm.q), 16, 1024, kLayoutSw128);
+      const uint64_t dp0 = make_sdesc(smem_u32(sm.p), 16384, 1024, kLayoutSw128);
       const uint64_t ones_desc = make_sdesc(smem_u32(sm.ones), 128, 256, kLayoutNone);
       PieceCursor cur(sm.gpre, p.B, cta, n_cta);
-      int b, g0, g1, item = 0;
-      uint32_t ring = 0, tcount = 0;
-      while (cur.next(b, g0, g1)) {
-        mbar_wait(&sm.q_full, item & 1, 20);
+      int b, t0, t1, item = 0;
+      uint32_t ring = 0, n_s = 0, n_pv = 0;               // stages consumed, S tiles issued, PV tiles issued
+      // S^T(tile n_s) = K Q^T into S buffer n_s & 1
+      auto issue_s = [&](bool last_of_piece) {
+        const int buf = n_s & 1;
+        mbar_wait(&sm.s_empty[buf], ((n_s >> 1) & 1) ^ 1, 21);
         tc_fence_after();
-        const int n_tiles = (g1 - g0 + 3) >> 2;
-        for (int t = 0; t < n_tiles; ++t) {
-          const int buf = tcount & 1;
-          // ---- S^T = K Q^T ----
-          mbar_wait(&sm.s_empty[buf], ((tcount >> 1) & 1) ^ 1, 21);
-          tc_fence_after();
 #pragma unroll 1
-          for (int s4 = 0; s4 < 4; ++s4) {
-            const int st = ring % kTcStages;
-            mbar_wait(&sm.full[st], (ring / kTcStages) & 1, 22);
-            tc_fence_after();
-            const uint32_t st_addr = smem_u32(sm.stage[st]);
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const uint64_t a = make_sdesc(st_addr + (ks >> 2) * 16384 + (ks & 3) * 32, 16, 1024, kLayoutSw128);
-              const uint64_t bq = make_sdesc(q_addr + (s4 * 2 + (ks >> 2)) * 8192 + (ks & 3) * 32, 16, 1024, kLayoutSw128);
-              umma_bf16(tS + buf * 64, a, bq, id_kk, (s4 | ks) != 0);
-            }
-            umma_commit(&sm.empty[st]);
-            ++ring;
-          }
-          umma_commit(&sm.s_full[buf]);
-          if (t == n_tiles - 1) umma_commit(&sm.q_empty);
-          // ---- O^T += V^T P^T ; L += 1 P^T ----
-          mbar_wait(&sm.p_full, tcount & 1, 23);
+        for (int s4 = 0; s4 < 4; ++s4) {
+          const int st = ring % kTcStages;
+          mbar_wait(&sm.full[st], (ring / kTcStages) & 1, 22);
           tc_fence_after();
-          if (t == 0 && item > 0) {
-            mbar_wait(&sm.o_empty, (item - 1) & 1, 24);
-            tc_fence_after();
-          }
-#pragma unroll 1
-          for (int m = 0; m < 4; ++m) {
-            const int st = ring % kTcStages;
-            mbar_wait(&sm.full[st], (ring / kTcStages) & 1, 25);
-            tc_fence_after();
-            const uint32_t st_addr = smem_u32(sm.stage[st]);
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const uint64_t a = make_sdesc(st_addr + ks * 2048, 16384, 1024, kLayoutSw128);
-              const uint64_t bp = make_sdesc(p_addr + (ks >> 2) * 8192 + (ks & 3) * 32, 16, 1024, kLayoutSw128);
-              umma_bf16(tO + m * 64, a, bp, id_mn, (t | ks) != 0);
-            }
-            umma_commit(&sm.empty[st]);
-            ++ring;
-          }
+          const uint64_t a0 = dk0 + (uint64_t)(st * (kTcStageBytes >> 4));
+          const uint64_t b0 = dq0 + (uint64_t)(s4 * (16384 >> 4));
 #pragma unroll
           for (int ks = 0; ks < 8; ++ks) {
-            const uint64_t bp = make_sdesc(p_addr + (ks >> 2) * 8192 + (ks & 3) * 32, 16, 1024, kLayoutSw128);
-            umma_bf16(tL, ones_desc, bp, id_kk, (t | ks) != 0);
+            const uint64_t a = a0 + (uint64_t)(((ks >> 2) * 16384 + (ks & 3) * 32) >> 4);
+            const uint64_t bq = b0 + (uint64_t)(((ks >> 2) * 8192 + (ks & 3) * 32) >> 4);
+            umma_bf16(tS + buf * 64, a, bq, id_s, (s4 | ks) != 0);
           }
-          umma_commit(&sm.pv_done);
-          ++tcount;
+          umma_commit(&sm.empty[st]);
+          ++ring;
+        }
+        umma_commit(&sm.s_full[buf]);
+        TR(1, 1 + n_s * 3);
+        if (last_of_piece) umma_commit(&sm.q_empty);
+        ++n_s;
+      };
+      // O^T (+)= V^T P^T ; L (+)= 1 P^T for tile n_pv.  On the last tile of a piece every 128-row block of O^T
+      // is committed on its own, so the epilogue drains block m while blocks m+1.. are still being computed.
+      auto issue_pv = [&](bool first_of_piece, bool last_of_piece) {
+        mbar_wait(&sm.p_full, n_pv & 1, 23);
+        tc_fence_after();
+        TR(1, 2 + n_pv * 3);
+        if (first_of_piece && item > 0) {                 // the previous piece's epilogue has drained O and L
+          mbar_wait(&sm.o_empty, (item - 1) & 1, 24);
+          tc_fence_after();
+        }
+        const uint32_t acc = first_of_piece ? 0u : 1u;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) umma_bf16(tL, ones_desc, dp0 + (uint64_t)((ks * 2048) >> 4), id_l, acc | (ks != 0));
+#pragma unroll 1
+        for (int m = 0; m < 4; ++m) {
+          const int st = ring % kTcStages;
+          mbar_wait(&sm.full[st], (ring / kTcStages) & 1, 25);
+          tc_fence_after();
+          const uint64_t a0 = dv0 + (uint64_t)(st * (kTcStageBytes >> 4));
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks)
+            umma_bf16(tO + m * 64, a0 + (uint64_t)((ks * 2048) >> 4), dp0 + (uint64_t)((ks * 2048) >> 4), id_pv, acc | (ks != 0));
+          umma_commit(&sm.empty[st]);
+          if (last_of_piece) umma_commit(&sm.o_full[m]);
+          ++ring;
+        }
+        umma_commit(&sm.pv_done);
+        TR(1, 3 + n_pv * 3);
+        ++n_pv;
+      };
+      while (cur.next(b, t0, t1)) {
+        mbar_wait(&sm.q_full, item & 1, 20);
+        tc_fence_after();
+        TR(1, 0);
+        issue_s(t0 + 1 == t1);
+        for (int t = t0; t < t1; ++t) {
+          if (t + 1 < t1) issue_s(t + 2 == t1);
+          issue_pv(t == t0, t + 1 == t1);
         }
         ++item;
       }
     }
   } else {
-    // =========================== softmax + epilogue (128 threads) ===========================
-    const int wq = warp & 3;                              // TMEM sub-partition of this warp
-    const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
-    const int key = wq * 32 + lane;                       // key row of the tile owned by this thread
+    // =========================== softmax + epilogue (8 warps) ===========================
+    const int q4 = warp & 3;                              // TMEM lane quarter this warp may access
+    const int hh = (warp - 2) >> 2;                       // half of the heads owned by this warp
+    const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
+    const int key = q4 * 32 + lane;                       // key row of the tile owned by this thread
+    const bool tr = (tid == 64);
+    mbar_wait(&sm.setup, 0, 29);
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+    const uint32_t tS = tmem, tO = tmem + 128, tL = tmem + 384;
     PieceCursor cur(sm.gpre, p.B, cta, n_cta);
-    int b, g0, g1;
-    uint32_t tcount = 0;
-    while (cur.next(b, g0, g1)) {
-      const SeqView v = make_view(p, b);
-      const int n_tiles = (g1 - g0 + 3) >> 2;
-      float m_run[kTcH];
-      for (int t = 0; t < n_tiles; ++t) {
+    int b, t0, t1, b_first = -1, b_last = -1;
+    uint32_t tcount = 0, piece = 0;
+    float m_run[32];
+    // merged maximum of every head of this warp's half over all 128 keys of the tile -> mt[32]
+    auto tile_max = [&](const float (&x)[32], float (&mt)[32]) {
+      float mine = -INFINITY;
+#pragma unroll
+      for (int h = 0; h < 32; ++h) {
+        const float r = redux_max_f32(x[h]);
+        if (lane == h) mine = r;
+      }
+      sm.wmax[hh][lane][q4] = mine;
+      named_bar_sync(1, 32 * kTcSoftmaxWarps);
+      const float4 w = *reinterpret_cast<const float4*>(sm.wmax[hh][lane]);
+      sm.mtile[hh][q4][lane] = fmaxf(fmaxf(w.x, w.y), fmaxf(w.z, w.w));
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const float4 t4 = *reinterpret_cast<const float4*>(&sm.mtile[hh][q4][4 * j]);
+        mt[4 * j] = t4.x; mt[4 * j + 1] = t4.y; mt[4 * j + 2] = t4.z; mt[4 * j + 3] = t4.w;
+      }
+      __syncwarp();
+    };
+    while (cur.next(b, t0, t1)) {
+      if (b_first < 0) b_first = b;
+      // sequences without keys between two pieces of this CTA get an empty partial (weight 0 in S8)
+      for (int e = b_last + 1; b_last >= 0 && e < b; ++e)
+        if (tid < 64 + kTcH) { p.part_m[((size_t)cta + e) * kTcH + tid - 64] = -INFINITY; p.part_l[((size_t)cta + e) * kTcH + tid - 64] = 0.f; }
+      b_last = b;
+      const SeqView v = sm.view[b];
+      int nv_next = tile_valid(p, v, t0);
+      for (int t = t0; t < t1; ++t) {
         const int buf = tcount & 1;
-        const GroupSrc src = resolve_group(p, &map_pool, v, g0 + t * 4 + wq, g1);
-        const bool valid = lane < src.n_valid;
-        float x[kTcH];
+        const bool valid = key < nv_next;
+        if (t + 1 < t1) nv_next = tile_valid(p, v, t + 1);        // global look-up overlaps the wait below
+        float x[32];
+        if (tr) TR(2, 0 + tcount * 5);
         mbar_wait(&sm.s_full[buf], (tcount >> 1) & 1, 30);
         tc_fence_after();
-        tmem_ld32(tS + buf * 64 + lane_addr, reinterpret_cast<uint32_t*>(x));
-        tmem_ld32(tS + buf * 64 + 32 + lane_addr, reinterpret_cast<uint32_t*>(x) + 32);
+        if (tr) TR(2, 1 + tcount * 5);
+        tmem_ld32(tS + buf * 64 + hh * 32 + lane_addr, reinterpret_cast<uint32_t*>(x));
         tmem_wait_ld();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.s_empty[buf]);
-        // masked, scaled logits (log2 domain) and the per-warp maximum of every head
+        // masked, scaled logits (log2 domain); inputs are finite, so a tile with >= 1 valid key has a finite maximum
 #pragma unroll
-        for (int h = 0; h < kTcH; ++h) {
-          x[h] = valid ? x[h] * p.scale_log2 : -INFINITY;
-          const int r = redux_max_s32(float_ordered_s32(x[h]));
-          if ((h & 31) == lane) reinterpret_cast<int*>(sm.wmax[buf][h])[wq] = r;
-        }
-        named_bar_sync(1, 128);
-        // tile maximum of every head (identical in all 128 threads); first tile of a piece adopts it,
-        // later tiles keep the stale running maximum unless it is exceeded by more than 2^8
-        bool need_rescale = false;
+        for (int h = 0; h < 32; ++h) x[h] = valid ? x[h] * p.scale_log2 : -INFINITY;
+        bool rescale = false;
+        float f[32];
+        if (t == t0) {
+          tile_max(x, m_run);
+        } else {
+          bool over = false;
 #pragma unroll
-        for (int h = 0; h < kTcH; ++h) {
-          const int4 w = *reinterpret_cast<const int4*>(sm.wmax[buf][h]);
-          const float mt = s32_ordered_float(max(max(w.x, w.y), max(w.z, w.w)));
-          if (t == 0) m_run[h] = mt;
-          else need_rescale |= (mt > m_run[h] + kRescaleThreshold);
+          for (int h = 0; h < 32; ++h) over |= (x[h] > m_run[h] + kRescaleThreshold);
+          rescale = named_bar_red_or(1, 32 * kTcSoftmaxWarps, over);
+          if (rescale) {                      // rare: adopt the new maximum, O^T and L are rescaled below
+            float mt[32];
+            tile_max(x, mt);
+#pragma unroll
+            for (int h = 0; h < 32; ++h) {
+              const float mn = fmaxf(m_run[h], mt[h]);
+              f[h] = ex2_approx(m_run[h] - mn);
+              m_run[h] = mn;
+            }
+          }
         }
-        // P tile buffer (and O) are free once the previous tile's PV MMAs have completed
+        if (tr) TR(2, 2 + tcount * 5);
+        // P^T values of this thread: 32 heads of one key, bf16 pairs (computed before waiting for the buffer)
+        uint32_t pw[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) pw[e] = pack_bf16x2(ex2_approx(x[2 * e] - m_run[2 * e]), ex2_approx(x[2 * e + 1] - m_run[2 * e + 1]));
+        // the P tile buffer (and O) are free once the previous tile's PV MMAs have completed
         if (tcount > 0) {
           mbar_wait(&sm.pv_done, (tcount - 1) & 1, 31);
           tc_fence_after();
         }
-        if (need_rescale) {             // rare: O^T and L are rescaled in TMEM, 32 columns at a time
-#pragma unroll
-          for (int c = 0; c < 10; ++c) {          // 4 x 64 O columns + 64 L columns
+        if (rescale) {
+#pragma unroll 1
+          for (int c = 0; c < 5; ++c) {             // 4 x 64 O columns + 64 L columns; this warp's 32 of each
             uint32_t vreg[32];
-            const uint32_t addr = tO + c * 32 + lane_addr;
+            const uint32_t addr = tO + c * 64 + hh * 32 + lane_addr;
             tmem_ld32(addr, vreg);
             tmem_wait_ld();
 #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const int h = (c & 1) * 32 + j;
-              const int4 w = *reinterpret_cast<const int4*>(sm.wmax[buf][h]);
-              const float mn = fmaxf(m_run[h], s32_ordered_float(max(max(w.x, w.y), max(w.z, w.w))));
-              const float f = (mn == -INFINITY) ? 1.f : ex2_approx(m_run[h] - mn);
-              vreg[j] = __float_as_uint(__uint_as_float(vreg[j]) * f);
-            }
+            for (int j = 0; j < 32; ++j) vreg[j] = __float_as_uint(__uint_as_float(vreg[j]) * f[j]);
             tmem_st32(addr, vreg);
           }
           tmem_wait_st();
-#pragma unroll
-          for (int h = 0; h < kTcH; ++h) {
-            const int4 w = *reinterpret_cast<const int4*>(sm.wmax[buf][h]);
-            m_run[h] = fmaxf(m_run[h], s32_ordered_float(max(max(w.x, w.y), max(w.z, w.w))));
-          }
         }
-        // P^T tile: bf16, K-major (keys contiguous per head), 128-byte swizzle
+        if (tr) TR(2, 3 + tcount * 5);
+        // P^T tile: bf16 [128 keys][64 heads], 128-byte swizzle; this thread's 32 heads = 4 x 16 B
         {
-          const int kb = key >> 6, kk = key & 63;
-          unsigned char* pbase = sm.p + kb * 8192 + (kk & 7) * 2;
-          const int chunk = kk >> 3;
+          unsigned char* prow = sm.p + key * 128;
 #pragma unroll
-          for (int h = 0; h < kTcH; ++h) {
-            const float mu = (m_run[h] == -INFINITY) ? 0.f : m_run[h];
-            const float pv = ex2_approx(x[h] - mu);
-            *reinterpret_cast<__nv_bfloat16*>(pbase + h * 128 + ((chunk ^ (h & 7)) << 4)) = __float2bfloat16_rn(pv);
-          }
+          for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<uint4*>(prow + (((hh * 4 + j) ^ (key & 7)) << 4)) = make_uint4(pw[4 * j], pw[4 * j + 1], pw[4 * j + 2], pw[4 * j + 3]);
         }
         fence_proxy_async_smem();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.p_full);
+        if (tr) TR(2, 4 + tcount * 5);
         ++tcount;
       }
       // ---- epilogue: O^T, L, m -> partial slot (cta + b) ----
-      mbar_wait(&sm.pv_done, (tcount - 1) & 1, 32);
-      tc_fence_after();
+      // layout [d-block m][head half][head quad g][d_local][4 heads]: one 16-byte store per (m, g), warp-contiguous
+      if (tr) TR(2, 20);
       const size_t slot = (size_t)cta + b;
-      float* po = p.part_o + slot * (kTcH * kTcD);
+      float4* po = reinterpret_cast<float4*>(p.part_o + slot * (kTcH * kTcD)) + (size_t)hh * (8 * 128) + key;
 #pragma unroll 1
-      for (int c = 0; c < 8; ++c) {               // c>>1 = d-tile, c&1 = head half
+      for (int m = 0; m < 4; ++m) {               // d = m * 128 + key
         uint32_t vreg[32];
-        tmem_ld32(tO + c * 32 + lane_addr, vreg);
+        mbar_wait(&sm.o_full[m], piece & 1, 32);
+        tc_fence_after();
+        tmem_ld32(tO + m * 64 + hh * 32 + lane_addr, vreg);
         tmem_wait_ld();
-        const int d = (c >> 1) * 128 + key;
 #pragma unroll
-        for (int j = 0; j < 32; ++j) po[(size_t)((c & 1) * 32 + j) * kTcD + d] = __uint_as_float(vreg[j]);
+        for (int g = 0; g < 8; ++g)
+          po[(size_t)m * (2 * 8 * 128) + g * 128] = make_float4(__uint_as_float(vreg[4 * g]), __uint_as_float(vreg[4 * g + 1]),
+                                                                 __uint_as_float(vreg[4 * g + 2]), __uint_as_float(vreg[4 * g + 3]));
       }
-      if (wq == 0) {                              // every lane of L holds the same row sums: lane 0 writes them
-#pragma unroll 1
-        for (int c = 0; c < 2; ++c) {
-          uint32_t vreg[32];
-          tmem_ld32(tL + c * 32 + lane_addr, vreg);
-          tmem_wait_ld();
-          if (lane == 0)
+      if (q4 == 0) {                              // every lane of L holds the same row sums: lane 0 writes them
+        uint32_t vreg[32];
+        tmem_ld32(tL + hh * 32 + lane_addr, vreg);
+        tmem_wait_ld();
+        if (lane == 0) {
 #pragma unroll
-            for (int j = 0; j < 32; ++j) p.part_l[slot * kTcH + c * 32 + j] = __uint_as_float(vreg[j]);
+          for (int j = 0; j < 32; ++j) {
+            p.part_l[slot * kTcH + hh * 32 + j] = __uint_as_float(vreg[j]);
+            p.part_m[slot * kTcH + hh * 32 + j] = m_run[j];
+          }
         }
-      }
-      if (wq == 1 && lane == 0) {
-#pragma unroll
-        for (int h = 0; h < kTcH; ++h) p.part_m[slot * kTcH + h] = m_run[h];
       }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&sm.o_empty);
+      if (tr) TR(2, 21);
+      ++piece;
     }
+    if (tid == 64) p.piece_info[cta] = make_int2(b_first < 0 ? 0 : b_first, b_first < 0 ? 0 : b_last - b_first + 1);
   }
   // ---- teardown ----
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 512);
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(sm.tmem_base, 512);
+  }
+  if (tid == 0) TR(0, 31);
+#ifdef LSA_TC_TRACE
+  if (tid == 0 && (cta == 0 || cta == n_cta - 1)) tlog_add(p.tlog, cta == 0 ? 1 : 2, g_entry);
+#endif
 }
 
 }  // namespace lsa
