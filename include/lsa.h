@@ -53,6 +53,11 @@ enum lsa_status {
 enum lsa_dtype { LSA_F32 = 0, LSA_BF16 = 1 };
 enum lsa_attn_impl { LSA_ATTN_AUTO = 0, LSA_ATTN_SIMT = 1, LSA_ATTN_TCGEN05 = 2 };
 enum lsa_fetch_mode { LSA_FETCH_DEVICE_PULL = 0, LSA_FETCH_MEMCPY = 1 };
+/* S8 (merge of the split-K partials, tcgen05 path): AUTO = KERNEL = a separate combine kernel chained to the
+ * attention kernel by programmatic dependent launch.  FUSED (B <= 4 only, else ignored) merges inside the
+ * attention kernel behind a grid-wide arrival counter: one launch per step; measured slower than KERNEL on
+ * B200, kept as a tested alternative. */
+enum lsa_merge_mode { LSA_MERGE_AUTO = 0, LSA_MERGE_KERNEL = 1, LSA_MERGE_FUSED = 2 };
 
 /* Shape and resources of one LSA layer shared by B sequences (BJ configs). */
 typedef struct lsa_config {
@@ -77,7 +82,7 @@ typedef struct lsa_config {
   int32_t attn_impl;     /* lsa_attn_impl; AUTO picks tcgen05 for bf16,H=64,D=512,C=128          */
   int32_t fetch_mode;    /* lsa_fetch_mode; DEVICE_PULL keeps the whole trigger path on device   */
   int32_t max_ctas;      /* 0 -> one split-K wave sized from the SM count                       */
-  int32_t reserved;
+  int32_t merge_mode;    /* lsa_merge_mode: where S8 runs (tcgen05 path)                        */
 } lsa_config;
 
 /* One sequence (CPU cold mirror + always-resident tiers).  n_chunks = ceil(n_csa/C);

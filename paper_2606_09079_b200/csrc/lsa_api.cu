@@ -243,6 +243,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
     for (int b = 0; b < B; ++b) nk[b] = seqs[b].n_hca + (long long)c->k_eff[b] * C + cfg->W;
     TcInit ti{};
     ti.B = B; ti.k = k; ti.W = cfg->W; ti.P = P; ti.n_sms = c->n_sms; ti.max_ctas = cfg->max_ctas;
+    ti.fuse_combine = cfg->merge_mode == LSA_MERGE_FUSED ? 1 : 0;
     ti.hot_pool = cfg->hot_pool; ti.seq_host = c->seq_host.data(); ti.d_seqs = c->d_seqs; ti.pool = c->pool;
     ti.sm_scale = c->sm_scale;
     std::string msg;
@@ -268,6 +269,8 @@ extern "C" int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs, l
   if (cfg->D % 8 || cfg->Dh % 8 || cfg->E % 8) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "D, Dh, E must be multiples of 8 (16-byte vector loads)");
   if (!cfg->hot_pool || !cfg->W_q) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "null hot_pool / W_q");
   if (cfg->hot_pages < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "hot_pages must be >= 1");
+  if (cfg->merge_mode < LSA_MERGE_AUTO || cfg->merge_mode > LSA_MERGE_FUSED)
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad merge_mode");
   if (cfg->fetch_mode != LSA_FETCH_DEVICE_PULL && cfg->fetch_mode != LSA_FETCH_MEMCPY)
     LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad fetch_mode");
   lsa_ctx* c = new (std::nothrow) lsa_ctx();

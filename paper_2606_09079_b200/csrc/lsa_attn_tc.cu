@@ -19,7 +19,14 @@ constexpr int kCombineThreads = 512;
 // SM's shared memory keeps its blocks at one per SM, so the early ones cannot pile up on the few idle SMs.
 constexpr int kCombineSmemPad = 116 * 1024;
 
-__global__ void __launch_bounds__(kCombineThreads)
+// kSpec (B <= kCombineSpecMaxB, where nearly every CTA holds a piece of every sequence): the partial loads of
+// all n_cta slots are issued before anything is known about them, together with the loads of piece_info,
+// m and l, so the kernel is ONE memory round trip deep; slots that turn out to be inactive are discarded
+// (selected away, never multiplied).  Otherwise the active list is built first and only those are read.
+constexpr int kCombineSpecMaxB = 4;
+
+template <bool kSpec>
+__global__ void __launch_bounds__(kCombineThreads, 1)
 combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
   __shared__ float4 w_s[256];
   __shared__ int slot_s[256];
@@ -29,6 +36,9 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int dh = blockIdx.x & 1, g = (blockIdx.x >> 1) & 7, hh = (blockIdx.x >> 4) & 1, m = blockIdx.x >> 5, b = blockIdx.y;
   const int h0 = hh * 32 + g * 4;
+  const int dl = tid & 63, grp = tid >> 6;
+  const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dh * 64 + dl;
+  constexpr int U = kSpec ? 16 : 8;               // independent 16-byte loads in flight per thread
 #ifdef LSA_TC_TRACE
   const unsigned long long g_entry = gtime();
 #endif
@@ -36,15 +46,23 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   griddep_launch_dependents();                    // the next kernel in the stream may start its own prologue
 #ifdef LSA_TC_TRACE
   const unsigned long long g_dep = gtime();
-#endif                                 // partials and piece_info are final from here on
+#endif
+  float4 v[U];
+  if (kSpec) {
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      const int c = grp + 8 * j;
+      v[j] = c < n_cta ? __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
   // thread c < n_cta looks at CTA c: did it write a partial for sequence b?  (n_cta <= 256)
   bool active = false;
   float4 mi = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY), li = make_float4(0.f, 0.f, 0.f, 0.f);
   const size_t slot = (size_t)tid + b;
   if (tid < n_cta) {
-    const int2 info = p.piece_info[tid];
-    const float4 m4 = *reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0);
-    const float4 l4 = *reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0);
+    const int2 info = __ldcg(p.piece_info + tid);
+    const float4 m4 = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
+    const float4 l4 = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
     active = info.x <= b && b < info.x + info.y;
     if (active) { mi = m4; li = l4; }
   }
@@ -68,11 +86,15 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
     n_act += warp_cnt[w];
   }
   float4 wi = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (active) {                                   // compacted list of (slot, weights of the 4 heads)
+  if (active) {
     wi.x = mi.x == -INFINITY ? 0.f : exp2f(mi.x - m_star.x);
     wi.y = mi.y == -INFINITY ? 0.f : exp2f(mi.y - m_star.y);
     wi.z = mi.z == -INFINITY ? 0.f : exp2f(mi.z - m_star.z);
     wi.w = mi.w == -INFINITY ? 0.f : exp2f(mi.w - m_star.w);
+  }
+  if (kSpec) {                                    // weights by CTA index; slot_s = 1 marks an active slot
+    if (tid < 256) { w_s[tid] = wi; slot_s[tid] = active ? 1 : 0; }
+  } else if (active) {                            // compacted list of (slot, weights of the 4 heads)
     const int pos = base + __popc(bal & ((1u << lane) - 1));
     w_s[pos] = wi;
     slot_s[pos] = (int)slot;
@@ -97,23 +119,39 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   const unsigned long long g_w = gtime();
 #endif
   // ---- weighted sum of the partials ----
-  const int dl = tid & 63, grp = tid >> 6;
-  const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dh * 64 + dl;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  constexpr int U = 8;                            // independent 16-byte loads in flight per thread
-  for (int i0 = grp; i0 < n_act; i0 += 8 * U) {
-    float4 v[U], w[U];
+  if (kSpec) {
 #pragma unroll
     for (int j = 0; j < U; ++j) {
-      const int i = i0 + 8 * j;
-      const bool ok = i < n_act;
-      w[j] = ok ? w_s[i] : make_float4(0.f, 0.f, 0.f, 0.f);
-      v[j] = ok ? po[(size_t)slot_s[i] * (kTcH * kTcD / 4)] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const int c = grp + 8 * j;
+      if (c < n_cta && slot_s[c]) {
+        const float4 w = w_s[c];
+        acc.x = fmaf(w.x, v[j].x, acc.x); acc.y = fmaf(w.y, v[j].y, acc.y);
+        acc.z = fmaf(w.z, v[j].z, acc.z); acc.w = fmaf(w.w, v[j].w, acc.w);
+      }
     }
+    for (int c = grp + 8 * U; c < n_cta; c += 8) {  // more than 8*U CTAs
+      if (slot_s[c]) {
+        const float4 w = w_s[c];
+        const float4 x = __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4));
+        acc.x = fmaf(w.x, x.x, acc.x); acc.y = fmaf(w.y, x.y, acc.y); acc.z = fmaf(w.z, x.z, acc.z); acc.w = fmaf(w.w, x.w, acc.w);
+      }
+    }
+  } else {
+    for (int i0 = grp; i0 < n_act; i0 += 8 * U) {
+      float4 w[U];
 #pragma unroll
-    for (int j = 0; j < U; ++j) {
-      acc.x = fmaf(w[j].x, v[j].x, acc.x); acc.y = fmaf(w[j].y, v[j].y, acc.y);
-      acc.z = fmaf(w[j].z, v[j].z, acc.z); acc.w = fmaf(w[j].w, v[j].w, acc.w);
+      for (int j = 0; j < U; ++j) {
+        const int i = i0 + 8 * j;
+        const bool ok = i < n_act;
+        w[j] = ok ? w_s[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        v[j] = ok ? __ldcg(po + (size_t)slot_s[i] * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int j = 0; j < U; ++j) {
+        acc.x = fmaf(w[j].x, v[j].x, acc.x); acc.y = fmaf(w[j].y, v[j].y, acc.y);
+        acc.z = fmaf(w[j].z, v[j].z, acc.z); acc.w = fmaf(w[j].w, v[j].w, acc.w);
+      }
     }
   }
 #ifdef LSA_TC_TRACE
@@ -154,6 +192,7 @@ struct TcPlan {
   const void* q_cached = nullptr;
   CUtensorMap* d_maps = nullptr;
   TcParams params{};
+  unsigned long long grid_total = 0;   // host mirror of the fused-S8 arrival counter
   int grid_max = 0;
   size_t smem = 0;
 };
@@ -232,6 +271,9 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   TC_CUDA(cudaMemset(p.part_m, 0, slots * kTcH * sizeof(float)));
   TC_CUDA(cudaMemset(p.part_l, 0, slots * kTcH * sizeof(float)));
   TC_CUDA(cudaMemset(p.piece_info, 0, (size_t)pl->grid_max * sizeof(int2)));
+  TC_CUDA(cudaMalloc(&p.grid_ctr, sizeof(unsigned int)));
+  TC_CUDA(cudaMemset(p.grid_ctr, 0, sizeof(unsigned int)));
+  p.fused = (init.B <= kTcFusedMaxB && init.fuse_combine) ? 1 : 0;   // opt-in (LSA_MERGE_FUSED)
 #ifdef LSA_TC_TRACE
   TC_CUDA(cudaMalloc(&p.trace, (size_t)pl->grid_max * 3 * 32 * sizeof(long long)));
   TC_CUDA(cudaMemset(p.trace, 0, (size_t)pl->grid_max * 3 * 32 * sizeof(long long)));
@@ -240,7 +282,8 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
 #endif
   pl->smem = sizeof(TcSmem) + 1024;
   TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
-  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
+  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
+  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
   *out = pl;
   return 0;
 }
@@ -261,7 +304,17 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
     if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
     pl->q_cached = q;
   }
-  const int grid = pick_grid(pl, tiles_est);
+  const int n_attn = pick_grid(pl, tiles_est);
+  // fused S8: the whole grid (one CTA per SM, all resident) also merges the partials, so idle SMs help
+  const int grid = pl->params.fused ? pl->grid_max : n_attn;
+  TcParams prm = pl->params;
+  prm.n_attn = n_attn;
+  if (prm.fused) {
+    pl->grid_total += (unsigned long long)grid;
+    prm.grid_target = (unsigned int)pl->grid_total;
+    prm.out = (__nv_bfloat16*)out;
+    prm.lse = lse;
+  }
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -272,16 +325,24 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   static const int no_pdl = getenv("LSA_NO_PDL") ? atoi(getenv("LSA_NO_PDL")) : 0;   // 1: combine, 2: attention, 3: both
   if (no_pdl & 2) lc.numAttrs = 0;
 #endif
-  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel, pl->map_pool, pl->map_q, pl->params));
+  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel, pl->map_pool, pl->map_q, prm));
+  if (prm.fused) {
+    *launches = 1;
+    *ctas = n_attn;
+    return 0;
+  }
   cudaLaunchConfig_t lc2{};
   lc2.gridDim = dim3(128, pl->init.B); lc2.blockDim = dim3(kCombineThreads); lc2.dynamicSmemBytes = kCombineSmemPad; lc2.stream = st;
   lc2.attrs = attr; lc2.numAttrs = 1;
 #ifdef LSA_TC_TRACE
   if (no_pdl & 1) lc2.numAttrs = 0;
 #endif
-  TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel, pl->params, grid, (__nv_bfloat16*)out, lse));
+  if (pl->init.B <= kCombineSpecMaxB)
+    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel<true>, prm, n_attn, (__nv_bfloat16*)out, lse));
+  else
+    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel<false>, prm, n_attn, (__nv_bfloat16*)out, lse));
   *launches = 2;
-  *ctas = grid;
+  *ctas = n_attn;
   return 0;
 }
 
@@ -315,6 +376,7 @@ void tc_destroy(TcPlan* pl) {
   cudaFree(pl->params.part_m);
   cudaFree(pl->params.part_l);
   cudaFree(pl->params.piece_info);
+  cudaFree(pl->params.grid_ctr);
   delete pl;
 }
 

@@ -12,6 +12,7 @@ struct TcPlan;
 
 struct TcInit {
   int B, k, W, P, n_sms, max_ctas;
+  int fuse_combine;         // 1: merge the split partials inside the attention kernel when B is small
   void* hot_pool;
   const SeqDev* seq_host;   // host copy of the immutable per-sequence fields
   SeqDev* d_seqs;

@@ -28,6 +28,7 @@
 //                               epilogue TMEM -> partial in global memory
 #pragma once
 #include <cuda.h>
+#include <cuda_bf16.h>
 
 #include <vector>
 
@@ -77,6 +78,13 @@ struct TcParams {
   float* part_m;                 // [slots][H]   (log2 domain)
   float* part_l;                 // [slots][H]
   int2* piece_info;              // [grid]: (first sequence, number of sequences) this CTA wrote partials for
+  // fused S8 (small batches): the grid meets at a counter barrier and merges the partials itself
+  int fused;                     // 1: no combine kernel follows
+  int n_attn;                    // CTAs that own tiles (the remaining CTAs of the grid only help with the merge)
+  unsigned int* grid_ctr;        // monotonically increasing arrival counter
+  unsigned int grid_target;      // value of the counter once every CTA of this launch has arrived
+  __nv_bfloat16* out;            // [B][H][D]      (fused mode)
+  float* lse;                    // [B][H] or null (fused mode)
 #ifdef LSA_TC_TRACE
   long long* trace;              // [grid][3 roles][32] clock64 stamps (debug builds only)
   unsigned long long* tlog;      // [0] = entries; then (kernel id, globaltimer start, end) per launch of block 0
@@ -143,6 +151,7 @@ struct PieceCursor {
     const unsigned T = (unsigned)gpre_[B_];
     f = (int)((unsigned)cta * T / (unsigned)n_cta);
     f1 = (int)((unsigned)(cta + 1) * T / (unsigned)n_cta);
+    if (cta >= n_cta) f = f1 = 0;                 // helper CTA: no tiles
     b = 0;
   }
   // returns false when exhausted; else fills b_out and the tile range [t0, t1) inside sequence b_out

@@ -1,6 +1,7 @@
 // lsa_attn_tc_kernel.cuh - the tcgen05 split-K decode attention kernel (see lsa_attn_tc_defs.cuh).
 #pragma once
 #include "lsa_attn_tc_defs.cuh"
+#include "lsa_attn_tc_fused.cuh"
 
 namespace lsa {
 
@@ -21,7 +22,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   TcSmem& sm = *reinterpret_cast<TcSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int cta = blockIdx.x, n_cta = gridDim.x;
+  const int cta = blockIdx.x, n_cta = p.n_attn;    // CTAs that own tiles; gridDim.x may be larger (fused S8)
 #ifdef LSA_TC_TRACE
   const long long t_entry = clock64();
   const unsigned long long g_entry = gtime();
@@ -359,14 +360,29 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
   }
   // ---- teardown ----
   tc_fence_before();
-  __syncthreads();
-  if (warp == 1) {
-    tc_fence_after();
-    tmem_dealloc(sm.tmem_base, 512);
+  if (p.fused) {
+    if (tid == 0) TR(0, 27);
+    grid_arrive_and_wait(p);                      // every partial of the launch is visible from here on
+    if (tid == 0) TR(0, 28);
+    if (warp == 1) {
+      tc_fence_after();
+      tmem_dealloc(sm.tmem_base, 512);
+    }
+    if (warp >= 2) fused_combine(p, sm.q, cta, gridDim.x, tid - 64);
+    if (tid == 64) TR(0, 29);
+#ifdef LSA_TC_TRACE
+    __syncthreads();
+#endif
+  } else {
+    __syncthreads();
+    if (warp == 1) {
+      tc_fence_after();
+      tmem_dealloc(sm.tmem_base, 512);
+    }
   }
   if (tid == 0) TR(0, 31);
 #ifdef LSA_TC_TRACE
-  if (tid == 0 && (cta == 0 || cta == n_cta - 1)) tlog_add(p.tlog, cta == 0 ? 1 : 2, g_entry);
+  if (tid == 0 && (cta == 0 || cta == gridDim.x - 1)) tlog_add(p.tlog, cta == 0 ? 1 : 2, g_entry);
 #endif
 }
 

@@ -233,10 +233,14 @@ def test_attention_edge_cases(dtype, H, D):
     ctx.close()
 
 
+@pytest.mark.parametrize("merge", ["kernel", "fused"])
+@pytest.mark.parametrize("keep", [(0, 1, 2, 3, 4), (0, 1, 2, 4), (4,)])
 @pytest.mark.parametrize("max_ctas", [0, 1, 5])
-def test_tcgen05_attention_edge_cases(max_ctas):
+def test_tcgen05_attention_edge_cases(max_ctas, keep, merge):
     """The tensor-core kernel (bf16, H=64, D=512, C=128): single key, no keys, equal keys, ragged
-    segments, and a running maximum that jumps by far more than 2^8 between tiles (O rescale path)."""
+    segments, and a running maximum that jumps by far more than 2^8 between tiles (O rescale path).
+    S8 as the separate combine kernel (two-phase for 5 sequences, single-round-trip for <= 4) and fused
+    behind the attention kernel's grid barrier (<= 4 sequences; ignored for 5)."""
     lsa = _lsa()
     dev = torch.device("cuda:0")
     H, D, W = 64, 512, 200
@@ -251,35 +255,45 @@ def test_tcgen05_attention_edge_cases(max_ctas):
     wk = [rnd(W, D) for _ in range(5)]
     wv = [rnd(W, D) for _ in range(5)]
     w_len = [0, 0, 0, 29, 130]
-    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.5, max_ctas=max_ctas,
-                      attn_impl=lsa.LSA_ATTN_TCGEN05)
-    assert ctx.stats()["attn_impl"] == lsa.LSA_ATTN_TCGEN05
     q = rnd(5, H, D)
     q[4] = (qdir[None, :] * (1.0 + 0.1 * torch.rand(H, 1, generator=g))).to(torch.bfloat16).to(dev)
-    out, lse = ctx.decode_attention(q, want_lse=True)
+    sel = lambda xs: [xs[i] for i in keep]
+    hk, hv, wk, wv, w_len, q = sel(hk), sel(hv), sel(wk), sel(wv), sel(w_len), q[list(keep)].contiguous()
+    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.5, max_ctas=max_ctas,
+                      attn_impl=lsa.LSA_ATTN_TCGEN05,
+                      merge_mode=lsa.LSA_MERGE_FUSED if merge == "fused" else lsa.LSA_MERGE_KERNEL)
+    assert ctx.stats()["attn_impl"] == lsa.LSA_ATTN_TCGEN05
+    for rep in range(3):                      # repeated launches: the arrival counter of the fused merge keeps counting
+        out, lse = ctx.decode_attention(q, want_lse=True)
     ctx.sync()
     out64, lse = out.double().cpu().numpy(), lse.cpu().numpy()
     tol = attn_tolerance("bf16")
-    assert torch.equal(out[0], hv[0].expand(H, D)), "single-key attention must return the value row bit-exactly"
-    assert torch.all(out[1] == 0) and np.all(lse[1] == -np.inf)
-    np.testing.assert_allclose(out64[2], np.broadcast_to(hv[2].double().mean(0).cpu().numpy(), (H, D)), **tol)
-    for b in (3, 4):
-        K = np.concatenate([hk[b].double().cpu().numpy(), wk[b][: w_len[b]].double().cpu().numpy()])
-        V = np.concatenate([hv[b].double().cpu().numpy(), wv[b][: w_len[b]].double().cpu().numpy()])
-        ref, ref_lse, _ = attention(q[b].double().cpu().numpy(), K, V, 0.5)
-        np.testing.assert_allclose(out64[b], ref, **tol)
-        np.testing.assert_allclose(lse[b], ref_lse, atol=2e-2, rtol=1e-3)
+    for i, orig in enumerate(keep):
+        if orig == 0:
+            assert torch.equal(out[i], hv[i].expand(H, D)), "single-key attention must return the value row bit-exactly"
+        elif orig == 1:
+            assert torch.all(out[i] == 0) and np.all(lse[i] == -np.inf)
+        elif orig == 2:
+            np.testing.assert_allclose(out64[i], np.broadcast_to(hv[i].double().mean(0).cpu().numpy(), (H, D)), **tol)
+        else:
+            K = np.concatenate([hk[i].double().cpu().numpy(), wk[i][: w_len[i]].double().cpu().numpy()])
+            V = np.concatenate([hv[i].double().cpu().numpy(), wv[i][: w_len[i]].double().cpu().numpy()])
+            ref, ref_lse, _ = attention(q[i].double().cpu().numpy(), K, V, 0.5)
+            np.testing.assert_allclose(out64[i], ref, **tol)
+            np.testing.assert_allclose(lse[i], ref_lse, atol=2e-2, rtol=1e-3)
     ctx.close()
 
 
-@pytest.mark.parametrize("impl", ["simt", "tcgen05"])
+@pytest.mark.parametrize("impl", ["simt", "tcgen05", "tcgen05_merge_fused"])
 def test_flagship_shape_short_context_both_impls(impl):
-    """bf16 H=64 D=512 C=128 at a short context, with a partial last chunk, through both kernels."""
+    """bf16 H=64 D=512 C=128 at a short context, with a partial last chunk, through both kernels; the
+    tensor-core kernel with S8 fused behind its grid barrier (B <= 4 default) and as a separate kernel."""
     lsa = _lsa()
     cfg = make_config(2, L=[16384 + 4 * 37], W=1024, k=6, hot_pages=16, steps=70, name="cfg2_short", q_gain=16.0, tau=32)
     assert cfg.n_csa(0) % cfg.C != 0
     wl = LsaWorkload(cfg)
-    rig = GpuRig(wl, attn_impl=lsa.LSA_ATTN_SIMT if impl == "simt" else lsa.LSA_ATTN_TCGEN05)
+    rig = GpuRig(wl, attn_impl=lsa.LSA_ATTN_SIMT if impl == "simt" else lsa.LSA_ATTN_TCGEN05,
+                 merge_mode=lsa.LSA_MERGE_FUSED if impl.endswith("merge_fused") else lsa.LSA_MERGE_AUTO)
     r = run_lockstep(wl, rig, cfg.steps, check_attention_at={0, 1, 2, 31, 32, 33, 34, 64, 65, 69})
     assert r["checked"] == 10
 
