@@ -30,6 +30,7 @@ import torch
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+from paper_2606_09079_b200.dist import max_over_ranks  # noqa: E402
 from paper_2606_09079_b200.workloads import LsaWorkload, make_config, to_torch  # noqa: E402
 
 METRIC = {1: ("lsa_decode_steps_per_s_8k_ctx_fp32", "steps/s"),
@@ -37,6 +38,11 @@ METRIC = {1: ("lsa_decode_steps_per_s_8k_ctx_fp32", "steps/s"),
           3: ("lsa_decode_steps_per_s_1m_ctx", "steps/s"),
           4: ("lsa_decode_tokens_per_s_b32_ragged", "tokens/s"),
           5: ("lsa_decode_steps_per_s_churn_b8_512k", "steps/s")}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one attn_tc_kernel launch, from the committed ncu --set full
+# capture of this command (profiles/); None where no capture has been taken for the config.
+TRAFFIC = {3: None}
 
 
 def load_peaks():
@@ -169,8 +175,8 @@ def clocks_sampler_stop(p, state, t_begin=None, t_end=None):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1536)
-    ap.add_argument("--warmup", type=int, default=192)
+    ap.add_argument("--steps", type=int, default=20000)
+    ap.add_argument("--warmup", type=int, default=256)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--attn", default="auto", choices=["auto", "simt", "tcgen05"])
@@ -264,11 +270,7 @@ def main():
         sf.synchronize(); sc.synchronize()
         wall = time.perf_counter() - w0
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=dev)
-            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(e0.elapsed_time(e1), dev)       # the job's time = the slowest rank's
         return ms, wall
 
     # ---- warm-up, then the device-resident timed region ----
@@ -319,7 +321,7 @@ def main():
     achieved = attn_bytes / (attn_ms * 1e-3) / 1e9
     stats = reps[0].ctx.stats()
     roofline = dict(bound="hbm", achieved=achieved, peak=peaks["hbm_gbs"], unit="GB/s", frac=achieved / peaks["hbm_gbs"],
-                    traffic=None, kernel="lsa split-K decode attention (S7)" + (" incl. combine" if comb_ms == 0.0 else ""),
+                    traffic=TRAFFIC.get(c.config_id), kernel="attn_tc_kernel: split-K decode attention (S7)" + (" incl. combine" if comb_ms == 0.0 else ""),
                     algorithmic_bytes_per_launch=attn_bytes, kernel_ms=attn_ms, combine_ms=comb_ms,
                     step_ms=ms / args.steps, frac_of_step=achieved and (attn_bytes / (ms / args.steps * 1e-3) / 1e9) / peaks["hbm_gbs"],
                     peak_source=peaks["source"], frac_of_nominal_8tbs=achieved / 8000.0)

@@ -409,11 +409,22 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse) {
   } else {
     int launches = 0, ctas = 0;
     std::string msg;
-    ProfScope prof(c, LSA_PH_ATTENTION, c->sc);   // attention + combine of the tcgen05 path
+    // profiling: attention = start .. mid, combine = mid .. end (the events between the two kernels cost the
+    // programmatic overlap of that pair, so phase times are upper bounds of what an unprofiled step sees)
+    const bool prof = c->prof_cap > 0 && c->prof_n[LSA_PH_ATTENTION] < c->prof_cap && c->prof_n[LSA_PH_COMBINE] < c->prof_cap;
+    const int ia = c->prof_n[LSA_PH_ATTENTION], ic = c->prof_n[LSA_PH_COMBINE];
+    if (prof) cudaEventRecord(c->prof_ev[LSA_PH_ATTENTION][2 * ia], c->sc);
     long long tiles = 0;                          // host mirror: HCA + selected pages + window, in 128-key tiles
     for (int b = 0; b < c->B; ++b)
       tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
-    int rc = tc_attention(c->tc, q, out, lse, tiles, c->sc, &launches, &ctas, &msg);
+    int rc = tc_attention(c->tc, q, out, lse, tiles, c->sc, &launches, &ctas, &msg,
+                          prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
+                          prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr);
+    if (prof) {
+      cudaEventRecord(c->prof_ev[LSA_PH_COMBINE][2 * ic + 1], c->sc);
+      c->prof_n[LSA_PH_ATTENTION] += 1;
+      c->prof_n[LSA_PH_COMBINE] += 1;
+    }
     if (rc != 0) LSA_FAIL(c, rc, "tcgen05 attention: %s", msg.c_str());
     c->attn_launches += launches;
     c->last_attn_ctas = ctas;

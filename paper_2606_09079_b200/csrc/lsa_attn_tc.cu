@@ -299,7 +299,7 @@ static int pick_grid(const TcPlan* pl, long long tiles_est) {
 }
 
 int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long tiles_est, cudaStream_t st, int* launches, int* ctas,
-                 std::string* msg) {
+                 std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1) {
   if (q != pl->q_cached) {
     if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
     pl->q_cached = q;
@@ -326,6 +326,8 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   if (no_pdl & 2) lc.numAttrs = 0;
 #endif
   TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel, pl->map_pool, pl->map_q, prm));
+  if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
+  if (ev_mid1) TC_CUDA(cudaEventRecord(ev_mid1, st));
   if (prm.fused) {
     *launches = 1;
     *ctas = n_attn;

@@ -24,8 +24,9 @@ struct TcInit {
 bool tc_supported(int dtype, int H, int D, int C);
 int tc_create(const TcInit& init, TcPlan** out, std::string* msg);   // 0 or an lsa_status
 // tiles_est: upper estimate of the batch's 128-key tiles (sizes the grid; the kernel partitions the exact list)
+// ev_mid0 / ev_mid1 (optional, profiling): recorded between the attention and the combine kernel
 int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, cudaStream_t st, int* launches,
-                 int* ctas, std::string* msg);
+                 int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr);
 void tc_destroy(TcPlan* plan);
 
 }  // namespace lsa
