@@ -42,7 +42,7 @@ METRIC = {1: ("lsa_decode_steps_per_s_8k_ctx_fp32", "steps/s"),
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one attn_tc_kernel launch, from the committed ncu --set full
 # capture of this command (profiles/); None where no capture has been taken for the config.
-TRAFFIC = {3: None}
+TRAFFIC = {3: 51.2e6}     # profiles/r01_attn_tc_kernel_ncu.md: 50.47 MB read + 0.3-1.1 MB written
 
 
 def load_peaks():

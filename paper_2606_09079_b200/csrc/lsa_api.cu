@@ -366,9 +366,10 @@ extern "C" int lsa_fetch_chunks(lsa_ctx* ctx, const int32_t* seq_ids, int32_t n,
 
 // ---- S6 -----------------------------------------------------------------------------------------
 // Swap every staged table that is due (or all of them if force) and optionally append k_new/v_new.
-static int prestep_impl(lsa_ctx* c, bool force, const void* k_new, const void* v_new) {
-  uint32_t words[32] = {0};
+// Which staged tables are due (or all of them if force)?  Clears their host-side pending flags.
+static bool due_mask(lsa_ctx* c, bool force, uint32_t words[32]) {
   bool any = false;
+  for (int i = 0; i < 32; ++i) words[i] = 0;
   for (int b = 0; b < c->B; ++b) {
     if (c->pending[b] && (force || c->step[b] >= c->visible_at[b])) {
       words[b >> 5] |= 1u << (b & 31);
@@ -376,13 +377,23 @@ static int prestep_impl(lsa_ctx* c, bool force, const void* k_new, const void* v
       any = true;
     }
   }
+  return any;
+}
+
+static void mirror_append(lsa_ctx* c) {            // host mirror of the ring fill (the kernels apply the same rule)
+  for (int b = 0; b < c->B; ++b) c->seq_host[b].w_len = std::min(c->cfg.W, c->seq_host[b].w_len + 1);
+}
+
+// Swap every staged table that is due (or all of them if force) and optionally append k_new/v_new.
+static int prestep_impl(lsa_ctx* c, bool force, const void* k_new, const void* v_new) {
+  uint32_t words[32];
+  const bool any = due_mask(c, force, words);
   if (!any && !k_new) return LSA_OK;
   if (any) LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_fetch, 0));
   ProfScope prof(c, LSA_PH_PRESTEP, c->sc);
   LSA_CUDA(c, launch_prestep(c->cfg.dtype, c->d_seqs, c->B, c->cfg.D, c->cfg.W, any ? words : nullptr, 32, k_new, v_new, c->sc));
   c->attn_launches += 1;
-  if (k_new)                                      // host mirror of the ring fill (the kernel applies the same rule)
-    for (int b = 0; b < c->B; ++b) c->seq_host[b].w_len = std::min(c->cfg.W, c->seq_host[b].w_len + 1);
+  if (k_new) mirror_append(c);
   return LSA_OK;
 }
 
@@ -392,7 +403,7 @@ extern "C" int lsa_commit_tables(lsa_ctx* ctx) {
 }
 
 // ---- S7-S8 --------------------------------------------------------------------------------------
-static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse) {
+static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, const TcPrestep* pre = nullptr) {
   const lsa_config& cfg = c->cfg;
   if (c->attn_impl == LSA_ATTN_SIMT) {
     {
@@ -417,7 +428,7 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse) {
     long long tiles = 0;                          // host mirror: HCA + selected pages + window, in 128-key tiles
     for (int b = 0; b < c->B; ++b)
       tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
-    int rc = tc_attention(c->tc, q, out, lse, tiles, c->sc, &launches, &ctas, &msg,
+    int rc = tc_attention(c->tc, q, out, lse, tiles, pre, c->sc, &launches, &ctas, &msg,
                           prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
                           prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr);
     if (prof) {
@@ -435,6 +446,15 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse) {
 extern "C" int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, float* lse) {
   if (!ctx) return LSA_ERR_STATE;
   if (!q || !out) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null q / out");
+  if (ctx->attn_impl == LSA_ATTN_TCGEN05) {        // S6 is folded into the attention launch
+    TcPrestep pre{};
+    uint32_t words[32];
+    if (due_mask(ctx, false, words)) {
+      LSA_CUDA(ctx, cudaStreamWaitEvent(ctx->sc, ctx->ev_fetch, 0));
+      for (int i = 0; i < 8; ++i) pre.swap[i] = words[i];
+    }
+    return attention_impl(ctx, q, out, lse, &pre);
+  }
   int rc = prestep_impl(ctx, false, nullptr, nullptr);
   if (rc) return rc;
   return attention_impl(ctx, q, out, lse);
@@ -452,6 +472,22 @@ extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* 
     if (c->step[b] % c->cfg.tau == 0) ids[n_fire++] = b;           // S0
   if (n_fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
   int rc;
+  if (n_fire == 0 && c->attn_impl == LSA_ATTN_TCGEN05) {
+    // no trigger this step: (a) and (d) ride on the attention launch itself (one kernel less per step).  On a
+    // trigger step the residency pass must see the swapped tables, so they stay a kernel of their own.
+    TcPrestep pre{};
+    uint32_t words[32];
+    if (due_mask(c, false, words)) {
+      LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_fetch, 0));
+      for (int i = 0; i < 8; ++i) pre.swap[i] = words[i];
+    }
+    pre.k_new = k_new; pre.v_new = v_new;
+    if (k_new) mirror_append(c);
+    if ((rc = attention_impl(c, q, out, nullptr, &pre))) return rc;
+    for (int b = 0; b < c->B; ++b) c->step[b] += 1;
+    c->n_steps += 1;
+    return LSA_OK;
+  }
   if ((rc = prestep_impl(c, false, k_new, v_new))) return rc;       // (a) + (d)
   if (n_fire) {                                                     // (b)
     if ((rc = index_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))) return rc;

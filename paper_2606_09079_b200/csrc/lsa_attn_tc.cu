@@ -47,6 +47,7 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
 #ifdef LSA_TC_TRACE
   const unsigned long long g_dep = gtime();
 #endif
+  if (blockIdx.x == 0 && tid == 0) commit_state(p, b);   // S6 / window append folded into the attention launch
   float4 v[U];
   if (kSpec) {
 #pragma unroll
@@ -262,7 +263,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   const size_t slots = (size_t)pl->grid_max + init.B;
   TcParams& p = pl->params;
   p.seqs = init.d_seqs; p.tbl_chunk = init.pool.tbl_chunk; p.tbl_page = init.pool.tbl_page; p.seq_maps = pl->d_maps;
-  p.B = init.B; p.k = init.k;
+  p.B = init.B; p.k = init.k; p.W = init.W; p.seqs_mut = init.d_seqs;
   p.scale_log2 = init.sm_scale * 1.4426950408889634f;
   TC_CUDA(cudaMalloc(&p.part_o, slots * kTcH * kTcD * sizeof(float)));
   TC_CUDA(cudaMalloc(&p.part_m, slots * kTcH * sizeof(float)));
@@ -298,8 +299,8 @@ static int pick_grid(const TcPlan* pl, long long tiles_est) {
   return (int)std::max<long long>(1, std::min<long long>(g, (tiles_est + per - 1) / per));
 }
 
-int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long tiles_est, cudaStream_t st, int* launches, int* ctas,
-                 std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1) {
+int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long tiles_est, const TcPrestep* pre, cudaStream_t st,
+                 int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1) {
   if (q != pl->q_cached) {
     if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
     pl->q_cached = q;
@@ -309,6 +310,11 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   const int grid = pl->params.fused ? pl->grid_max : n_attn;
   TcParams prm = pl->params;
   prm.n_attn = n_attn;
+  if (pre) {
+    for (int i = 0; i < kTcMaxB / 32; ++i) prm.swap[i] = pre->swap[i];
+    prm.k_new = (const __nv_bfloat16*)pre->k_new;
+    prm.v_new = (const __nv_bfloat16*)pre->v_new;
+  }
   if (prm.fused) {
     pl->grid_total += (unsigned long long)grid;
     prm.grid_target = (unsigned int)pl->grid_total;

@@ -23,10 +23,17 @@ struct TcInit {
 // bf16, H = 64 query heads sharing one K/V of D = 512, pages of C = 128 rows (BASELINE cfg 2-5)
 bool tc_supported(int dtype, int H, int D, int C);
 int tc_create(const TcInit& init, TcPlan** out, std::string* msg);   // 0 or an lsa_status
+// S6 + window append folded into the attention launch (steps without a trigger)
+struct TcPrestep {
+  unsigned int swap[8];     // bit b: the staged table of sequence b becomes current (B <= 256)
+  const void* k_new;        // DEVICE [B][D] or null
+  const void* v_new;
+};
+
 // tiles_est: upper estimate of the batch's 128-key tiles (sizes the grid; the kernel partitions the exact list)
 // ev_mid0 / ev_mid1 (optional, profiling): recorded between the attention and the combine kernel
-int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, cudaStream_t st, int* launches,
-                 int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr);
+int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, const TcPrestep* pre, cudaStream_t st,
+                 int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr);
 void tc_destroy(TcPlan* plan);
 
 }  // namespace lsa

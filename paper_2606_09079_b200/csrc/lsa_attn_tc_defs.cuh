@@ -50,6 +50,7 @@ constexpr float kRescaleThreshold = 8.0f;   // log2 units: P may grow to 2^8 bef
 // per-sequence shape as of this launch
 struct SeqView {
   int b, t_hca, n_cur, n_hca, w_len, cur;
+  int app_tile, app_slot;      // tile of this sequence holding the ring slot written by this launch (-1: no append)
   long long n_csa;
 };
 
@@ -63,7 +64,7 @@ struct TcSmem {
   SeqView view[kTcMaxB];                                      // per-sequence shape, read once by warp 0
   int gpre[kTcMaxB + 1];                                      // prefix of tiles per sequence
   uint64_t full[kTcStages], empty[kTcStages];
-  uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup;
+  uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup, app_done;
   uint32_t tmem_base;
 };
 
@@ -78,6 +79,13 @@ struct TcParams {
   float* part_m;                 // [slots][H]   (log2 domain)
   float* part_l;                 // [slots][H]
   int2* piece_info;              // [grid]: (first sequence, number of sequences) this CTA wrote partials for
+  // S6 + window append folded into this launch (steps without a trigger): every CTA applies them to its VIEW of
+  // the per-sequence records; the records themselves are updated once, after the grid, by commit_state()
+  SeqDev* seqs_mut;
+  unsigned int swap[kTcMaxB / 32];   // bit b: sequence b's staged table becomes current (if one is pending)
+  const __nv_bfloat16* k_new;        // [B][D] or null: row b is written to ring slot w_head of sequence b
+  const __nv_bfloat16* v_new;
+  int W;                             // ring capacity
   // fused S8 (small batches): the grid meets at a counter barrier and merges the partials itself
   int fused;                     // 1: no combine kernel follows
   int n_attn;                    // CTAs that own tiles (the remaining CTAs of the grid only help with the merge)
@@ -94,13 +102,33 @@ struct TcParams {
 __host__ __device__ __forceinline__ int tc_tiles(int n_hca, int n_cur, int w_len) {
   return (n_hca + kTcTile - 1) / kTcTile + n_cur + (w_len + kTcTile - 1) / kTcTile;
 }
-__device__ __forceinline__ int seq_tiles(const SeqDev& s) { return tc_tiles(s.n_hca, s.n_tbl[s.cur_buf], s.w_len); }
 
-__device__ __forceinline__ SeqView make_view(const SeqDev& s, int b) {
+__device__ __forceinline__ SeqView make_view(const TcParams& p, int b) {
+  const SeqDev& s = p.seqs[b];
   SeqView v;
-  v.b = b; v.n_hca = s.n_hca; v.t_hca = (s.n_hca + kTcTile - 1) / kTcTile; v.cur = s.cur_buf; v.n_cur = s.n_tbl[s.cur_buf];
-  v.w_len = s.w_len; v.n_csa = s.n_csa;
+  const bool swap = ((p.swap[b >> 5] >> (b & 31)) & 1u) && s.pending;
+  v.b = b; v.n_hca = s.n_hca; v.t_hca = (s.n_hca + kTcTile - 1) / kTcTile;
+  v.cur = swap ? 1 - s.cur_buf : s.cur_buf;
+  v.n_cur = s.n_tbl[v.cur];
+  v.n_csa = s.n_csa;
+  v.w_len = s.w_len; v.app_tile = -1; v.app_slot = 0;
+  if (p.k_new) {
+    v.app_slot = s.w_head;
+    v.w_len = min(p.W, s.w_len + 1);
+    v.app_tile = v.t_hca + v.n_cur + s.w_head / kTcTile;
+  }
   return v;
+}
+
+// The per-sequence records catch up with the view: one thread per sequence, after the whole grid has finished.
+__device__ __forceinline__ void commit_state(const TcParams& p, int b) {
+  SeqDev& s = p.seqs_mut[b];
+  if (((p.swap[b >> 5] >> (b & 31)) & 1u) && s.pending) { s.cur_buf = 1 - s.cur_buf; s.pending = 0; }
+  if (p.k_new) {
+    const int slot = s.w_head;
+    s.w_head = (slot + 1 == p.W) ? 0 : slot + 1;
+    s.w_len = min(p.W, s.w_len + 1);
+  }
 }
 
 // where tile t of a sequence lives

@@ -36,6 +36,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
     mbar_init(&sm.p_full, kTcSoftmaxWarps); mbar_init(&sm.pv_done, 1); mbar_init(&sm.o_empty, kTcSoftmaxWarps);
     for (int i = 0; i < 4; ++i) mbar_init(&sm.o_full[i], 1);
     mbar_init(&sm.setup, kTcThreads / 32);
+    mbar_init(&sm.app_done, kTcSoftmaxWarps);
     fence_mbar_init();
     prefetch_tmap(&map_pool);
     prefetch_tmap(&map_q);
@@ -50,7 +51,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       const int b = base + lane;
       int g = 0;
       if (b < p.B) {
-        const SeqView v = make_view(p.seqs[b], b);
+        const SeqView v = make_view(p, b);
         sm.view[b] = v;
         g = v.t_hca + v.n_cur + (v.w_len + kTcTile - 1) / kTcTile;
       }
@@ -84,6 +85,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       PieceCursor cur(sm.gpre, p.B, cta, n_cta);
       int b, t0, t1, item = 0;
       uint32_t ring = 0;                                  // stages issued so far
+      bool app_seen = false;
+      // the tile holding this launch's new window row is loaded only after the softmax warps have written it
+      auto app_gate = [&](const SeqView& v, int t) {
+        if (t == v.app_tile && !app_seen) { mbar_wait(&sm.app_done, 0, 12); app_seen = true; }
+      };
       auto issue4 = [&](const CUtensorMap* m, int row) {
 #pragma unroll 1
         for (int s4 = 0; s4 < 4; ++s4) {
@@ -103,11 +109,13 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
         mbar_arrive_expect_tx(&sm.q_full, 65536);
         tma_load_3d(sm.q, &map_q, 0, b * kTcH, 0, &sm.q_full);
         TR(0, 1);
+        app_gate(v, t0);
         issue4(src.mk, src.row_k);
         for (int t = t0; t < t1; ++t) {
           TileSrc nxt = src;
           if (t + 1 < t1) {
             nxt = tile_src(p, &map_pool, v, t + 1);
+            app_gate(v, t + 1);
             issue4(nxt.mk, nxt.row_k);
           }
           issue4(src.mv, src.row_v);
@@ -214,8 +222,26 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
     const uint32_t tS = tmem, tO = tmem + 128, tL = tmem + 384;
-    PieceCursor cur(sm.gpre, p.B, cta, n_cta);
     int b, t0, t1, b_first = -1, b_last = -1;
+    if (p.k_new) {
+      // window append ("decoded tokens stay resident"; DESIGN R6): the CTA that owns the tile holding ring
+      // slot w_head of a sequence writes k_new/v_new there before its producer loads that tile
+      PieceCursor pc(sm.gpre, p.B, cta, n_cta);
+      const int t = tid - 64;
+      while (pc.next(b, t0, t1)) {
+        const SeqView v = sm.view[b];
+        if (v.app_tile >= t0 && v.app_tile < t1 && t < 128) {
+          const SeqDev& s = p.seqs[b];
+          const uint4* src = reinterpret_cast<const uint4*>((t < 64 ? p.k_new : p.v_new) + (size_t)b * kTcD) + (t & 63);
+          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(t < 64 ? s.win_k : s.win_v) + (size_t)v.app_slot * kTcD) + (t & 63);
+          *dst = *src;
+        }
+      }
+      fence_proxy_async_all();                            // generic-proxy stores -> later TMA (async proxy) reads
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&sm.app_done);
+    }
+    PieceCursor cur(sm.gpre, p.B, cta, n_cta);
     uint32_t tcount = 0, piece = 0;
     float m_run[32];
     // merged maximum of every head of this warp's half over all 128 keys of the tile -> mt[32]
@@ -368,6 +394,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       tc_fence_after();
       tmem_dealloc(sm.tmem_base, 512);
     }
+    if (cta == 0 && tid < p.B) commit_state(p, tid);  // every CTA has read the records (they are behind the barrier)
     if (warp >= 2) fused_combine(p, sm.q, cta, gridDim.x, tid - 64);
     if (tid == 64) TR(0, 29);
 #ifdef LSA_TC_TRACE
