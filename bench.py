@@ -298,7 +298,7 @@ def main():
     ms_e2e, _ = timed(n_e2e, host, i0=i_next)
     i_next += n_e2e
     es = 4 if c.dtype == "f32" else 2
-    h2d = (c.B * c.H * c.D + c.B * c.Dh + 2 * c.B * c.D) * es
+    h2d = (c.B * c.H * c.D + 2 * c.B * c.D) * es + c.B * c.Dh * es // c.tau     # h crosses only at trigger steps (1 in tau)
     d2h = c.B * c.H * c.D * es
     e2e_value = world * n_e2e * per_step_units / (ms_e2e * 1e-3)
 

@@ -160,8 +160,9 @@ int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, float* lse);
 int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
              void* out);
 
-/* lsa_step with HOST buffers (pinned recommended): copies q,h,k_new,v_new host->device, runs the
- * step, copies out device->host and blocks until it has landed.  Used for end-to-end timing. */
+/* lsa_step with HOST buffers: packs q, k_new, v_new (and h, at trigger steps only) into one pinned staging
+ * image, copies it host->device in ONE transfer, runs the step, copies out device->host (pinned `out`
+ * recommended) and blocks until it has landed.  Used for end-to-end timing. */
 int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new,
                   const void* v_new, void* out);
 

@@ -52,7 +52,7 @@ struct lsa_ctx {
   int fetch_ctas = 0;
   TcPlan* tc = nullptr;
   // host-buffer staging (lsa_step_host)
-  void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr;
+  void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
   // optional per-phase event timing
   int prof_cap = 0;
   std::vector<cudaEvent_t> prof_ev[LSA_PH_COUNT];   // 2*cap events per phase
@@ -119,6 +119,7 @@ extern "C" void lsa_destroy(lsa_ctx* ctx) {
   if (ctx->sc) cudaStreamSynchronize(ctx->sc);
   if (ctx->sf) cudaStreamSynchronize(ctx->sf);
   if (ctx->tc) tc_destroy(ctx->tc);
+  if (ctx->st_pin) cudaFreeHost(ctx->st_pin);
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
   if (ctx->ev_compute) cudaEventDestroy(ctx->ev_compute);
@@ -504,23 +505,30 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
   if (!ctx) return LSA_ERR_STATE;
   lsa_ctx* c = ctx;
   if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
+  if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
   const lsa_config& cfg = c->cfg;
+  auto up = [](size_t n) { return (n + 255) / 256 * 256; };
   const size_t qb = (size_t)c->B * cfg.H * cfg.D * c->elem, hb = (size_t)c->B * cfg.Dh * c->elem,
                nb = (size_t)c->B * cfg.D * c->elem;
+  // one packed image [q | k_new | v_new | h] in pinned host memory -> ONE host-to-device copy per step
+  const size_t o_kn = up(qb), o_vn = o_kn + up(nb), o_h = o_vn + up(nb), in_bytes = o_h + up(hb);
   if (!c->st_q) {
     int rc;
     unsigned char* p = nullptr;
-    if ((rc = dev_alloc(c, &p, 2 * qb + hb + 2 * nb + 5 * 256))) return rc;
-    auto take = [&p](size_t n) { void* r = p; p += (n + 255) / 256 * 256; return r; };
-    c->st_q = take(qb); c->st_out = take(qb); c->st_h = take(hb); c->st_kn = take(nb); c->st_vn = take(nb);
+    if ((rc = dev_alloc(c, &p, in_bytes + up(qb)))) return rc;
+    c->st_q = p; c->st_kn = p + o_kn; c->st_vn = p + o_vn; c->st_h = p + o_h; c->st_out = p + in_bytes;
+    LSA_CUDA(c, cudaHostAlloc(&c->st_pin, in_bytes, cudaHostAllocDefault));
   }
-  LSA_CUDA(c, cudaMemcpyAsync(c->st_q, q, qb, cudaMemcpyHostToDevice, c->sc));
-  if (h) LSA_CUDA(c, cudaMemcpyAsync(c->st_h, h, hb, cudaMemcpyHostToDevice, c->sc));
-  if (k_new) {
-    LSA_CUDA(c, cudaMemcpyAsync(c->st_kn, k_new, nb, cudaMemcpyHostToDevice, c->sc));
-    LSA_CUDA(c, cudaMemcpyAsync(c->st_vn, v_new, nb, cudaMemcpyHostToDevice, c->sc));
-  }
-  int rc = lsa_step(c, c->st_q, h ? c->st_h : nullptr, k_new ? c->st_kn : nullptr, k_new ? c->st_vn : nullptr, c->st_out);
+  bool fire = false;
+  for (int b = 0; b < c->B; ++b) fire |= (c->step[b] % cfg.tau == 0);
+  if (fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
+  unsigned char* pin = static_cast<unsigned char*>(c->st_pin);
+  memcpy(pin, q, qb);
+  size_t upto = qb;
+  if (k_new) { memcpy(pin + o_kn, k_new, nb); memcpy(pin + o_vn, v_new, nb); upto = o_vn + nb; }
+  if (fire) { memcpy(pin + o_h, h, hb); upto = o_h + hb; }          // h is only read at trigger steps
+  LSA_CUDA(c, cudaMemcpyAsync(c->st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
+  int rc = lsa_step(c, c->st_q, fire ? c->st_h : nullptr, k_new ? c->st_kn : nullptr, k_new ? c->st_vn : nullptr, c->st_out);
   if (rc) return rc;
   LSA_CUDA(c, cudaMemcpyAsync(out, c->st_out, qb, cudaMemcpyDeviceToHost, c->sc));
   LSA_CUDA(c, cudaStreamSynchronize(c->sc));

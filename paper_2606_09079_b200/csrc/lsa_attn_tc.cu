@@ -19,13 +19,12 @@ constexpr int kCombineThreads = 512;
 // SM's shared memory keeps its blocks at one per SM, so the early ones cannot pile up on the few idle SMs.
 constexpr int kCombineSmemPad = 116 * 1024;
 
-// kSpec (B <= kCombineSpecMaxB, where nearly every CTA holds a piece of every sequence): the partial loads of
-// all n_cta slots are issued before anything is known about them, together with the loads of piece_info,
-// m and l, so the kernel is ONE memory round trip deep; slots that turn out to be inactive are discarded
-// (selected away, never multiplied).  Otherwise the active list is built first and only those are read.
+// For B <= kCombineSpecMaxB nearly every CTA holds a piece of every sequence: the partial loads of all n_cta
+// slots are issued before anything is known about them, together with the loads of piece_info, m and l, so
+// the kernel is ONE memory round trip deep; slots that turn out to be inactive are discarded (selected away,
+// never multiplied).  Larger batches use combine_tc_wide_kernel below.
 constexpr int kCombineSpecMaxB = 4;
 
-template <bool kSpec>
 __global__ void __launch_bounds__(kCombineThreads, 1)
 combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
   __shared__ float4 w_s[256];
@@ -38,7 +37,7 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   const int h0 = hh * 32 + g * 4;
   const int dl = tid & 63, grp = tid >> 6;
   const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dh * 64 + dl;
-  constexpr int U = kSpec ? 16 : 8;               // independent 16-byte loads in flight per thread
+  constexpr int U = 16;                           // independent 16-byte loads in flight per thread
 #ifdef LSA_TC_TRACE
   const unsigned long long g_entry = gtime();
 #endif
@@ -48,22 +47,25 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   const unsigned long long g_dep = gtime();
 #endif
   if (blockIdx.x == 0 && tid == 0) commit_state(p, b);   // S6 / window append folded into the attention launch
-  float4 v[U];
-  if (kSpec) {
-#pragma unroll
-    for (int j = 0; j < U; ++j) {
-      const int c = grp + 8 * j;
-      v[j] = c < n_cta ? __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-  }
   // thread c < n_cta looks at CTA c: did it write a partial for sequence b?  (n_cta <= 256)
+  // These small loads go first so that they are not queued behind the bulk of partial loads below.
   bool active = false;
   float4 mi = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY), li = make_float4(0.f, 0.f, 0.f, 0.f);
   const size_t slot = (size_t)tid + b;
+  int2 info = make_int2(0, 0);
+  float4 m4 = mi, l4 = li;
   if (tid < n_cta) {
-    const int2 info = __ldcg(p.piece_info + tid);
-    const float4 m4 = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
-    const float4 l4 = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
+    info = __ldcg(p.piece_info + tid);
+    m4 = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
+    l4 = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
+  }
+  float4 v[U];
+#pragma unroll
+  for (int j = 0; j < U; ++j) {
+    const int c = grp + 8 * j;
+    v[j] = c < n_cta ? __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  if (tid < n_cta) {
     active = info.x <= b && b < info.x + info.y;
     if (active) { mi = m4; li = l4; }
   }
@@ -93,13 +95,7 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
     wi.z = mi.z == -INFINITY ? 0.f : exp2f(mi.z - m_star.z);
     wi.w = mi.w == -INFINITY ? 0.f : exp2f(mi.w - m_star.w);
   }
-  if (kSpec) {                                    // weights by CTA index; slot_s = 1 marks an active slot
-    if (tid < 256) { w_s[tid] = wi; slot_s[tid] = active ? 1 : 0; }
-  } else if (active) {                            // compacted list of (slot, weights of the 4 heads)
-    const int pos = base + __popc(bal & ((1u << lane) - 1));
-    w_s[pos] = wi;
-    slot_s[pos] = (int)slot;
-  }
+  if (tid < 256) { w_s[tid] = wi; slot_s[tid] = active ? 1 : 0; }   // weights by CTA index; slot_s marks active slots
   float4 lsum = make_float4(wi.x * li.x, wi.y * li.y, wi.z * li.z, wi.w * li.w);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -121,7 +117,7 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
 #endif
   // ---- weighted sum of the partials ----
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (kSpec) {
+  {
 #pragma unroll
     for (int j = 0; j < U; ++j) {
       const int c = grp + 8 * j;
@@ -136,22 +132,6 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
         const float4 w = w_s[c];
         const float4 x = __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4));
         acc.x = fmaf(w.x, x.x, acc.x); acc.y = fmaf(w.y, x.y, acc.y); acc.z = fmaf(w.z, x.z, acc.z); acc.w = fmaf(w.w, x.w, acc.w);
-      }
-    }
-  } else {
-    for (int i0 = grp; i0 < n_act; i0 += 8 * U) {
-      float4 w[U];
-#pragma unroll
-      for (int j = 0; j < U; ++j) {
-        const int i = i0 + 8 * j;
-        const bool ok = i < n_act;
-        w[j] = ok ? w_s[i] : make_float4(0.f, 0.f, 0.f, 0.f);
-        v[j] = ok ? __ldcg(po + (size_t)slot_s[i] * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-      }
-#pragma unroll
-      for (int j = 0; j < U; ++j) {
-        acc.x = fmaf(w[j].x, v[j].x, acc.x); acc.y = fmaf(w[j].y, v[j].y, acc.y);
-        acc.z = fmaf(w[j].z, v[j].z, acc.z); acc.w = fmaf(w[j].w, v[j].w, acc.w);
       }
     }
   }
@@ -175,6 +155,107 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   if (tid == 0 && blockIdx.x == gridDim.x - 1 && b == 0) tlog_add(p.tlog, 5, g_dep);
 #endif
   if (lse && m == 0 && dh == 0 && tid < 4) {
+    const float ls = tid == 0 ? l_star.x : tid == 1 ? l_star.y : tid == 2 ? l_star.z : l_star.w;
+    const float ms = tid == 0 ? m_star.x : tid == 1 ? m_star.y : tid == 2 ? m_star.z : m_star.w;
+    lse[(size_t)b * kTcH + h0 + tid] = ls > 0.f ? (ms + log2f(ls)) * 0.6931471805599453f : -INFINITY;
+  }
+}
+
+// S8 for larger batches (B > kCombineSpecMaxB): a sequence is touched by only a few CTAs, so there is nothing to
+// split - grid (16, B): block = 4 heads x all 512 d, thread = one float4 column (4 heads of one d) and walks
+// the sequence's active partials itself (all loads of a batch of 8 in flight), no cross-thread reduction.
+__global__ void __launch_bounds__(512)
+combine_tc_wide_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
+  __shared__ float4 w_s[256];
+  __shared__ int slot_s[256];
+  __shared__ float4 red_f[16];
+  __shared__ int warp_cnt[16];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = blockIdx.x & 7, hh = blockIdx.x >> 3, b = blockIdx.y;
+  const int h0 = hh * 32 + g * 4;
+  const int m = tid >> 7, dl = tid & 127;
+  griddep_wait();
+  griddep_launch_dependents();
+  if (blockIdx.x == 0 && tid == 0) commit_state(p, b);
+  bool active = false;
+  float4 mi = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY), li = make_float4(0.f, 0.f, 0.f, 0.f);
+  const size_t slot = (size_t)tid + b;
+  if (tid < n_cta) {
+    const int2 info = __ldcg(p.piece_info + tid);
+    active = info.x <= b && b < info.x + info.y;
+    if (active) {
+      mi = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
+      li = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
+    }
+  }
+  float4 mmax = mi;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    mmax.x = fmaxf(mmax.x, __shfl_xor_sync(0xffffffffu, mmax.x, o));
+    mmax.y = fmaxf(mmax.y, __shfl_xor_sync(0xffffffffu, mmax.y, o));
+    mmax.z = fmaxf(mmax.z, __shfl_xor_sync(0xffffffffu, mmax.z, o));
+    mmax.w = fmaxf(mmax.w, __shfl_xor_sync(0xffffffffu, mmax.w, o));
+  }
+  const unsigned bal = __ballot_sync(0xffffffffu, active);
+  if (lane == 0) { red_f[warp] = mmax; warp_cnt[warp] = __popc(bal); }
+  __syncthreads();
+  float4 m_star = red_f[0];
+  int base = 0, n_act = 0;
+  for (int w = 0; w < 16; ++w) {
+    const float4 r = red_f[w];
+    m_star.x = fmaxf(m_star.x, r.x); m_star.y = fmaxf(m_star.y, r.y); m_star.z = fmaxf(m_star.z, r.z); m_star.w = fmaxf(m_star.w, r.w);
+    if (w < warp) base += warp_cnt[w];
+    n_act += warp_cnt[w];
+  }
+  float4 wi = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (active) {
+    wi.x = mi.x == -INFINITY ? 0.f : exp2f(mi.x - m_star.x);
+    wi.y = mi.y == -INFINITY ? 0.f : exp2f(mi.y - m_star.y);
+    wi.z = mi.z == -INFINITY ? 0.f : exp2f(mi.z - m_star.z);
+    wi.w = mi.w == -INFINITY ? 0.f : exp2f(mi.w - m_star.w);
+    const int pos = base + __popc(bal & ((1u << lane) - 1));
+    w_s[pos] = wi;
+    slot_s[pos] = (int)slot;
+  }
+  float4 lsum = make_float4(wi.x * li.x, wi.y * li.y, wi.z * li.z, wi.w * li.w);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lsum.x += __shfl_xor_sync(0xffffffffu, lsum.x, o);
+    lsum.y += __shfl_xor_sync(0xffffffffu, lsum.y, o);
+    lsum.z += __shfl_xor_sync(0xffffffffu, lsum.z, o);
+    lsum.w += __shfl_xor_sync(0xffffffffu, lsum.w, o);
+  }
+  __syncthreads();
+  if (lane == 0) red_f[warp] = lsum;
+  __syncthreads();
+  float4 l_star = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int w = 0; w < 16; ++w) {
+    const float4 r = red_f[w];
+    l_star.x += r.x; l_star.y += r.y; l_star.z += r.z; l_star.w += r.w;
+  }
+  const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dl;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  constexpr int U = 8;
+  for (int i0 = 0; i0 < n_act; i0 += U) {
+    float4 v[U], w[U];
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      const bool ok = i0 + j < n_act;
+      w[j] = ok ? w_s[i0 + j] : make_float4(0.f, 0.f, 0.f, 0.f);
+      v[j] = ok ? __ldcg(po + (size_t)slot_s[i0 + j] * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      acc.x = fmaf(w[j].x, v[j].x, acc.x); acc.y = fmaf(w[j].y, v[j].y, acc.y);
+      acc.z = fmaf(w[j].z, v[j].z, acc.z); acc.w = fmaf(w[j].w, v[j].w, acc.w);
+    }
+  }
+  __nv_bfloat16* o = out + ((size_t)b * kTcH + h0) * kTcD + m * 128 + dl;
+  o[0] = __float2bfloat16_rn(l_star.x > 0.f ? acc.x / l_star.x : 0.f);
+  o[kTcD] = __float2bfloat16_rn(l_star.y > 0.f ? acc.y / l_star.y : 0.f);
+  o[2 * kTcD] = __float2bfloat16_rn(l_star.z > 0.f ? acc.z / l_star.z : 0.f);
+  o[3 * kTcD] = __float2bfloat16_rn(l_star.w > 0.f ? acc.w / l_star.w : 0.f);
+  if (lse && tid < 4) {
     const float ls = tid == 0 ? l_star.x : tid == 1 ? l_star.y : tid == 2 ? l_star.z : l_star.w;
     const float ms = tid == 0 ? m_star.x : tid == 1 ? m_star.y : tid == 2 ? m_star.z : m_star.w;
     lse[(size_t)b * kTcH + h0 + tid] = ls > 0.f ? (ms + log2f(ls)) * 0.6931471805599453f : -INFINITY;
@@ -283,8 +364,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
 #endif
   pl->smem = sizeof(TcSmem) + 1024;
   TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
-  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
-  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
+  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
   *out = pl;
   return 0;
 }
@@ -345,10 +425,12 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
 #ifdef LSA_TC_TRACE
   if (no_pdl & 1) lc2.numAttrs = 0;
 #endif
-  if (pl->init.B <= kCombineSpecMaxB)
-    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel<true>, prm, n_attn, (__nv_bfloat16*)out, lse));
-  else
-    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel<false>, prm, n_attn, (__nv_bfloat16*)out, lse));
+  if (pl->init.B <= kCombineSpecMaxB) {
+    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel, prm, n_attn, (__nv_bfloat16*)out, lse));
+  } else {
+    lc2.gridDim = dim3(16, pl->init.B); lc2.dynamicSmemBytes = 0;
+    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_wide_kernel, prm, n_attn, (__nv_bfloat16*)out, lse));
+  }
   *launches = 2;
   *ctas = n_attn;
   return 0;

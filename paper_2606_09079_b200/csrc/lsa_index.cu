@@ -29,7 +29,7 @@ qtower_kernel(const T* __restrict__ W, const T* __restrict__ h, FireList rows, f
 #pragma unroll
   for (int s = 0; s < kQtSeqs; ++s) acc[s] = 0.f;
   const T* wrow = W + (size_t)e * Dh;
-#pragma unroll 2
+#pragma unroll 8
   for (int d0 = lane * V; d0 < Dh; d0 += 32 * V) {
     float wf[V];
     Elem<T>::load16(wrow + d0, wf);

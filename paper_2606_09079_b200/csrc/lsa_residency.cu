@@ -118,25 +118,32 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
     __syncthreads();
 
     // ---- pass 2: the n_miss smallest (last_used, page) among unpinned pages ----
+    // Pages never return to the never-used state and never-used pages (last_used = 0) sort first, lowest index
+    // first, so the used pages are always the prefix [0, n_used) with n_used = misses - evictions so far.  While
+    // enough never-used pages are left, the victims are simply the next n_miss indices (no scan of the pool).
     if (n_miss > 0) {
-      const unsigned long long* lu = pool.last_used;
-      const unsigned int* pm = pool.pin_mark;
-      auto keyf = [lu, pm, epoch](int p) -> unsigned long long {
-        return pm[p] == epoch ? kKeyMax : ((lu[p] << kPageBits) | (unsigned long long)p);
-      };
-      int got = block_select_smallest(keyf, P, n_miss, sm.sel);
-      __syncthreads();
-      bool bad = (got < n_miss) || (sm.sel.keys[n_miss - 1] == kKeyMax);
-      if (bad) {
-        if (tid == 0) pool.counters[C_ERROR] = 1;   // pool exhausted: leave state untouched
+      const long long n_used = (long long)(pool.counters[C_MISSES] - pool.counters[C_EVICTIONS]);
+      const bool fast = n_used + n_miss <= (long long)P;
+      if (!fast) {
+        const unsigned long long* lu = pool.last_used;
+        const unsigned int* pm = pool.pin_mark;
+        auto keyf = [lu, pm, epoch](int p) -> unsigned long long {
+          return pm[p] == epoch ? kKeyMax : ((lu[p] << kPageBits) | (unsigned long long)p);
+        };
+        int got = block_select_smallest(keyf, P, n_miss, sm.sel);
         __syncthreads();
-        continue;
+        bool bad = (got < n_miss) || (sm.sel.keys[n_miss - 1] == kKeyMax);
+        if (bad) {
+          if (tid == 0) pool.counters[C_ERROR] = 1;   // pool exhausted: leave state untouched
+          __syncthreads();
+          continue;
+        }
       }
       const unsigned long long base = pool.counters[C_FETCH_COUNT];
       if (tid < n_sel && sm.miss_rank[tid] >= 0) {
         const int r = sm.miss_rank[tid];
         const int c = sm.sel_up[tid];
-        const int p = (int)(sm.sel.keys[r] & ((1ull << kPageBits) - 1));
+        const int p = fast ? (int)n_used + r : (int)(sm.sel.keys[r] & ((1ull << kPageBits) - 1));
         const int ob = pool.owner_seq[p];
         if (ob >= 0) {
           pool.page_of[seqs[ob].page_of_off + pool.owner_chunk[p]] = -1;

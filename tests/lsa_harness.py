@@ -16,7 +16,7 @@ def make_oracle(wl: LsaWorkload, trigger_idx: int = 0, **over) -> LsaOracle:
         n_csa=[c.n_csa(b) for b in range(c.B)],
         chunk_emb=[wl.chunk_emb(b, trigger_idx) for b in range(c.B)],
         hca_k=wl.hca_k, hca_v=wl.hca_v, win_k=wl.win_k, win_v=wl.win_v,
-        w_len=[min(c.W, c.L[b]) for b in range(c.B)], w_head=[0] * c.B,
+        w_len=[min(c.W, c.L[b]) for b in range(c.B)], w_head=[min(c.W, c.L[b]) % c.W for b in range(c.B)],
         step0=[c.step0(b) for b in range(c.B)])
     kw.update(over)
     return LsaOracle(**kw)
@@ -67,7 +67,7 @@ class GpuRig:
         for b in range(c.B):
             seqs.append(dict(cold_csa=self.cold[b], n_csa=c.n_csa(b), chunk_emb=self.emb[b],
                              hca_k=self.hca_k[b], hca_v=self.hca_v[b], win_k=self.win_k[b], win_v=self.win_v[b],
-                             w_len=min(c.W, c.L[b]), w_head=0, step0=c.step0(b)))
+                             w_len=min(c.W, c.L[b]), w_head=min(c.W, c.L[b]) % c.W, step0=c.step0(b)))
         kw = dict(dtype=lsa.LSA_F32 if dt == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W, Dh=c.Dh, E=c.E,
                   k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=self.W_q, seqs=seqs, recall_lag=c.recall_lag)
         kw.update(ctx_over)

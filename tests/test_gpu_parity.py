@@ -298,6 +298,30 @@ def test_flagship_shape_short_context_both_impls(impl):
     assert r["checked"] == 10
 
 
+@pytest.mark.parametrize("merge", ["kernel", "fused"])
+def test_flagship_shape_growing_window_and_ring_wrap(merge):
+    """S6 and the window append ride on the attention launch on steps without a trigger (tensor-core path).
+    Growing ring: w_len starts at a multiple of 128, so the first appended token opens a new tile and later
+    ones extend a ragged tile; full ring: w_head wraps and the oldest row is replaced.  Two sequences, so the
+    appended rows land in tiles owned by different CTAs."""
+    lsa = _lsa()
+    mm = lsa.LSA_MERGE_FUSED if merge == "fused" else lsa.LSA_MERGE_KERNEL
+    # (a) growing: L = 8576 = 67 * 128 < W
+    cfg = make_config(2, B=2, L=[8576, 4096 + 4 * 30], W=9000, k=5, hot_pages=24, steps=12, name="cfg2_growing", q_gain=16.0, tau=4)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl, attn_impl=lsa.LSA_ATTN_TCGEN05, merge_mode=mm)
+    r = run_lockstep(wl, rig, cfg.steps)
+    assert r["checked"] == cfg.steps
+    rig.ctx.close()
+    # (b) full ring of 300 rows (not a multiple of 128): 310 steps wrap w_head once
+    cfg = make_config(2, B=2, L=[16384, 8192], W=300, k=4, hot_pages=16, steps=310, name="cfg2_wrap", q_gain=16.0, tau=64)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl, attn_impl=lsa.LSA_ATTN_TCGEN05, merge_mode=mm)
+    r = run_lockstep(wl, rig, cfg.steps, check_attention_at={0, 1, 2, 63, 64, 65, 127, 128, 129, 255, 256, 298, 299, 300, 301, 309})
+    assert r["checked"] == 16
+    rig.ctx.close()
+
+
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("lag", [0, 1])
 def test_lockstep_small(dtype, lag):
