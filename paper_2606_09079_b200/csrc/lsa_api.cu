@@ -53,6 +53,8 @@ struct lsa_ctx {
   TcPlan* tc = nullptr;
   // host-buffer staging (lsa_step_host)
   void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
+  const void* out_host_cached = nullptr;
+  void* out_dev_alias = nullptr;
   // optional per-phase event timing
   int prof_cap = 0;
   std::vector<cudaEvent_t> prof_ev[LSA_PH_COUNT];   // 2*cap events per phase
@@ -528,9 +530,21 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
   if (k_new) { memcpy(pin + o_kn, k_new, nb); memcpy(pin + o_vn, v_new, nb); upto = o_vn + nb; }
   if (fire) { memcpy(pin + o_h, h, hb); upto = o_h + hb; }          // h is only read at trigger steps
   LSA_CUDA(c, cudaMemcpyAsync(c->st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
-  int rc = lsa_step(c, c->st_q, fire ? c->st_h : nullptr, k_new ? c->st_kn : nullptr, k_new ? c->st_vn : nullptr, c->st_out);
+  // result: if `out` is pinned and mapped, S8 writes it in place over the host link (no device-to-host copy
+  // operation in the chain); otherwise through a device buffer and one copy
+  if (out != c->out_host_cached) {
+    cudaPointerAttributes at{};
+    c->out_dev_alias = nullptr;
+    if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+      c->out_dev_alias = at.devicePointer;
+    else
+      cudaGetLastError();
+    c->out_host_cached = out;
+  }
+  void* out_dev = c->out_dev_alias ? c->out_dev_alias : c->st_out;
+  int rc = lsa_step(c, c->st_q, fire ? c->st_h : nullptr, k_new ? c->st_kn : nullptr, k_new ? c->st_vn : nullptr, out_dev);
   if (rc) return rc;
-  LSA_CUDA(c, cudaMemcpyAsync(out, c->st_out, qb, cudaMemcpyDeviceToHost, c->sc));
+  if (!c->out_dev_alias) LSA_CUDA(c, cudaMemcpyAsync(out, c->st_out, qb, cudaMemcpyDeviceToHost, c->sc));
   LSA_CUDA(c, cudaStreamSynchronize(c->sc));
   return LSA_OK;
 }

@@ -22,7 +22,7 @@ __device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
 }
 
 // All kTcThreads threads call this after their last global store of the launch.
-__device__ __forceinline__ void grid_arrive_and_wait(const TcParams& p) {
+__device__ __noinline__ void grid_arrive_and_wait(const TcParams& p) {
   __threadfence();
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -58,7 +58,7 @@ __device__ __forceinline__ float w_of(float m, float M) { return m == -INFINITY 
 
 // Called by the 256 merge threads (t = 0..255) of every CTA after the grid barrier.
 // scratch: >= 24 KiB of shared memory no longer used by the attention phase (the Q tile buffer).
-__device__ __forceinline__ void fused_combine(const TcParams& p, unsigned char* scratch, int cta, int n_cta, int t) {
+__device__ __noinline__ void fused_combine(const TcParams& p, unsigned char* scratch, int cta, int n_cta, int t) {
   const int w = t >> 5, lane = t & 31;
   int* cnt = reinterpret_cast<int*>(scratch);                    // [kTcFusedMaxB]
   int* wcnt = cnt + 8;                                           // [kTcFusedMaxB][8]

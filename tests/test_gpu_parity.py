@@ -322,6 +322,32 @@ def test_flagship_shape_growing_window_and_ring_wrap(merge):
     rig.ctx.close()
 
 
+@pytest.mark.parametrize("pinned_out", [True, False])
+def test_step_host_equals_step(pinned_out):
+    """lsa_step_host (host buffers: one packed H2D copy, result written in place when `out` is pinned and
+    mapped, else one D2H copy) gives bit-identical outputs, page tables and counters to lsa_step."""
+    lsa = _lsa()
+    cfg = make_config(2, B=2, L=[16384 + 4 * 37, 8192], W=1024, k=6, hot_pages=32, steps=40, name="cfg2_host", q_gain=16.0, tau=8)
+    wl = LsaWorkload(cfg)
+    a, b_ = GpuRig(wl), GpuRig(wl)
+    out_h = torch.empty((cfg.B, cfg.H, cfg.D), dtype=torch.bfloat16)
+    if pinned_out:
+        out_h = out_h.pin_memory()
+    for t in range(cfg.steps):
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t)
+        ref = a.ctx.step(a.dev(q), a.dev(h), a.dev(kn), a.dev(vn))
+        a.ctx.sync()
+        to_h = lambda x: to_torch(x, cfg.dtype).pin_memory()
+        b_.ctx.step_host(to_h(q), to_h(h) if t % 2 == 0 or t % cfg.tau == 0 else None, to_h(kn), to_h(vn), out_h)
+        assert torch.equal(ref.cpu(), out_h), f"step {t}"
+    for s_ in range(cfg.B):
+        assert a.ctx.page_table(s_) == b_.ctx.page_table(s_)
+    sa, sb = a.ctx.stats(), b_.ctx.stats()
+    assert (sa["hits"], sa["misses"], sa["bytes_fetched"]) == (sb["hits"], sb["misses"], sb["bytes_fetched"])
+    a.ctx.close(); b_.ctx.close()
+
+
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("lag", [0, 1])
 def test_lockstep_small(dtype, lag):
