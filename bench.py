@@ -319,10 +319,16 @@ def main():
     comb_ms = phases["combine"]["ms"] / max(phases["combine"]["count"], 1) if phases["combine"]["count"] else 0.0
     peaks = load_peaks()
     achieved = attn_bytes / (attn_ms * 1e-3) / 1e9
+    ph_dev = phases.get("attention_dev", dict(ms=0.0, count=0))
+    attn_dev_ms = ph_dev["ms"] / ph_dev["count"] if ph_dev["count"] else None
     stats = reps[0].ctx.stats()
     roofline = dict(bound="hbm", achieved=achieved, peak=peaks["hbm_gbs"], unit="GB/s", frac=achieved / peaks["hbm_gbs"],
                     traffic=TRAFFIC.get(c.config_id), kernel="attn_tc_kernel: split-K decode attention (S7)" + (" incl. combine" if comb_ms == 0.0 else ""),
                     algorithmic_bytes_per_launch=attn_bytes, kernel_ms=attn_ms, combine_ms=comb_ms,
+                    # the same kernel by the device's %globaltimer (first CTA past its launch dependency -> last CTA
+                    # done): the CUDA-event figure above also holds the launch gap the events themselves open
+                    kernel_ms_device_clock=attn_dev_ms,
+                    frac_device_clock=(attn_bytes / (attn_dev_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if attn_dev_ms else None,
                     step_ms=ms / args.steps, frac_of_step=achieved and (attn_bytes / (ms / args.steps * 1e-3) / 1e9) / peaks["hbm_gbs"],
                     peak_source=peaks["source"], frac_of_nominal_8tbs=achieved / 8000.0)
 

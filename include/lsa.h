@@ -184,9 +184,12 @@ int lsa_get_stats(lsa_ctx* ctx, lsa_stats* out); /* blocking */
  * lsa_profile_read blocks, returns the summed milliseconds and launch counts per phase since the
  * last read and rearms.  Phases: */
 enum lsa_phase { LSA_PH_PRESTEP = 0, LSA_PH_ATTENTION = 1, LSA_PH_COMBINE = 2, LSA_PH_INDEX = 3,
-                 LSA_PH_RESIDENCY = 4, LSA_PH_FETCH = 5, LSA_PH_COUNT = 6 };
+                 LSA_PH_RESIDENCY = 4, LSA_PH_FETCH = 5,
+                 LSA_PH_ATTENTION_DEV = 6, /* tcgen05 attention kernel's own working time by %globaltimer: first CTA
+                                              past its launch dependency -> last CTA done (no event in the way) */
+                 LSA_PH_COUNT = 7 };
 int lsa_profile_enable(lsa_ctx* ctx, int32_t capacity);
-int lsa_profile_read(lsa_ctx* ctx, double* ms_sum /* HOST [6] */, int64_t* count /* HOST [6] */);
+int lsa_profile_read(lsa_ctx* ctx, double* ms_sum /* HOST [LSA_PH_COUNT] */, int64_t* count /* HOST [LSA_PH_COUNT] */);
 int lsa_get_step(lsa_ctx* ctx, int32_t seq, int64_t* step);
 int lsa_sync(lsa_ctx* ctx);                      /* waits for both streams, reports device errors */
 const char* lsa_last_error(lsa_ctx* ctx);        /* ctx may be NULL: last init error             */

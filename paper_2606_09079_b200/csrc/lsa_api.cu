@@ -58,7 +58,9 @@ struct lsa_ctx {
   // optional per-phase event timing
   int prof_cap = 0;
   std::vector<cudaEvent_t> prof_ev[LSA_PH_COUNT];   // 2*cap events per phase
-  int prof_n[LSA_PH_COUNT] = {0, 0, 0, 0, 0, 0};
+  int prof_n[LSA_PH_COUNT] = {0, 0, 0, 0, 0, 0, 0};
+  unsigned long long* d_ktime = nullptr;            // [prof_cap][2] attention-kernel globaltimer stamps
+  int ktime_cap = 0;
   // bookkeeping
   unsigned long long n_steps = 0, attn_launches = 0, index_launches = 0;
   int last_attn_ctas = 0;
@@ -433,7 +435,8 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
       tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
     int rc = tc_attention(c->tc, q, out, lse, tiles, pre, c->sc, &launches, &ctas, &msg,
                           prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
-                          prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr);
+                          prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr,
+                          prof && c->d_ktime ? c->d_ktime + 2 * ia : nullptr);
     if (prof) {
       cudaEventRecord(c->prof_ev[LSA_PH_COMBINE][2 * ic + 1], c->sc);
       c->prof_n[LSA_PH_ATTENTION] += 1;
@@ -633,13 +636,23 @@ extern "C" int lsa_profile_enable(lsa_ctx* ctx, int32_t capacity) {
   if (capacity < 0 || capacity > (1 << 20)) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "capacity out of range");
   LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
   LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
-  for (int ph = 0; ph < LSA_PH_COUNT; ++ph) {
+  for (int ph = 0; ph < LSA_PH_ATTENTION_DEV; ++ph) {
     while ((int)ctx->prof_ev[ph].size() < 2 * capacity) {
       cudaEvent_t e;
       LSA_CUDA(ctx, cudaEventCreate(&e));
       ctx->prof_ev[ph].push_back(e);
     }
     ctx->prof_n[ph] = 0;
+  }
+  if (capacity > ctx->ktime_cap) {
+    int rc = dev_alloc(ctx, &ctx->d_ktime, (size_t)2 * capacity, false);
+    if (rc) return rc;
+    ctx->ktime_cap = capacity;
+  }
+  if (capacity > 0) {
+    std::vector<unsigned long long> init((size_t)2 * capacity);
+    for (int i = 0; i < capacity; ++i) { init[2 * i] = ~0ull; init[2 * i + 1] = 0ull; }
+    LSA_CUDA(ctx, cudaMemcpy(ctx->d_ktime, init.data(), init.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice));
   }
   ctx->prof_cap = capacity;
   return LSA_OK;
@@ -650,7 +663,22 @@ extern "C" int lsa_profile_read(lsa_ctx* ctx, double* ms_sum, int64_t* count) {
   if (!ms_sum || !count) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null output");
   LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
   LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
-  for (int ph = 0; ph < LSA_PH_COUNT; ++ph) {
+  {                                                 // device-clock working time of the tcgen05 attention kernel
+    const int n = ctx->d_ktime ? std::min(ctx->prof_n[LSA_PH_ATTENTION], ctx->ktime_cap) : 0;
+    std::vector<unsigned long long> kt((size_t)2 * std::max(n, 1));
+    if (n > 0) LSA_CUDA(ctx, cudaMemcpy(kt.data(), ctx->d_ktime, (size_t)2 * n * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    double sum = 0;
+    int cnt = 0;
+    for (int i = 0; i < n; ++i)
+      if (kt[2 * i] != ~0ull && kt[2 * i + 1] > kt[2 * i]) { sum += (double)(kt[2 * i + 1] - kt[2 * i]) * 1e-6; ++cnt; }
+    ms_sum[LSA_PH_ATTENTION_DEV] = sum;
+    count[LSA_PH_ATTENTION_DEV] = cnt;
+    if (n > 0) {
+      for (int i = 0; i < n; ++i) { kt[2 * i] = ~0ull; kt[2 * i + 1] = 0ull; }
+      LSA_CUDA(ctx, cudaMemcpy(ctx->d_ktime, kt.data(), (size_t)2 * n * sizeof(unsigned long long), cudaMemcpyHostToDevice));
+    }
+  }
+  for (int ph = 0; ph < LSA_PH_ATTENTION_DEV; ++ph) {
     double sum = 0;
     for (int i = 0; i < ctx->prof_n[ph]; ++i) {
       float ms = 0.f;

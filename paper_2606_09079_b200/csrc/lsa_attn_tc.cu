@@ -380,7 +380,7 @@ static int pick_grid(const TcPlan* pl, long long tiles_est) {
 }
 
 int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long tiles_est, const TcPrestep* pre, cudaStream_t st,
-                 int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1) {
+                 int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1, unsigned long long* ktime) {
   if (q != pl->q_cached) {
     if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
     pl->q_cached = q;
@@ -390,6 +390,7 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   const int grid = pl->params.fused ? pl->grid_max : n_attn;
   TcParams prm = pl->params;
   prm.n_attn = n_attn;
+  prm.ktime = ktime;
   if (pre) {
     for (int i = 0; i < kTcMaxB / 32; ++i) prm.swap[i] = pre->swap[i];
     prm.k_new = (const __nv_bfloat16*)pre->k_new;

@@ -33,7 +33,8 @@ struct TcPrestep {
 // tiles_est: upper estimate of the batch's 128-key tiles (sizes the grid; the kernel partitions the exact list)
 // ev_mid0 / ev_mid1 (optional, profiling): recorded between the attention and the combine kernel
 int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, const TcPrestep* pre, cudaStream_t st,
-                 int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr);
+                 int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr,
+                 unsigned long long* ktime = nullptr /* DEVICE [2] = {~0, 0}: kernel working-time stamps */);
 void tc_destroy(TcPlan* plan);
 
 }  // namespace lsa

@@ -93,6 +93,9 @@ struct TcParams {
   unsigned int grid_target;      // value of the counter once every CTA of this launch has arrived
   __nv_bfloat16* out;            // [B][H][D]      (fused mode)
   float* lse;                    // [B][H] or null (fused mode)
+  // profiling only (null otherwise): [0] = min over CTAs of %globaltimer once past the launch dependency,
+  // [1] = max over CTAs at exit - the kernel's own working time, with programmatic overlap left intact
+  unsigned long long* ktime;
 #ifdef LSA_TC_TRACE
   long long* trace;              // [grid][3 roles][32] clock64 stamps (debug builds only)
   unsigned long long* tlog;      // [0] = entries; then (kernel id, globaltimer start, end) per launch of block 0
@@ -195,12 +198,12 @@ struct PieceCursor {
   }
 };
 
-#ifdef LSA_TC_TRACE
 __device__ __forceinline__ unsigned long long gtime() {
   unsigned long long t;
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
   return t;
 }
+#ifdef LSA_TC_TRACE
 __device__ __forceinline__ void tlog_add(unsigned long long* tlog, unsigned long long id, unsigned long long t0) {
   const unsigned long long i = atomicAdd(tlog, 1ull);
   if (i < 4096) { tlog[1 + 3 * i] = id; tlog[2 + 3 * i] = t0; tlog[3 + 3 * i] = gtime(); }

@@ -44,6 +44,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
   __syncthreads();
   griddep_wait();                 // PDL: everything below may read what the previous kernel wrote
   griddep_launch_dependents();    // the combine kernel may start its prologue; it waits for this grid itself
+  if (p.ktime && tid == 0) atomicMin(p.ktime, gtime());
   if (warp == 0) {
     // per-sequence shape and the prefix of tiles per sequence (B <= 256)
     int carry = 0;
@@ -408,6 +409,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
     }
   }
   if (tid == 0) TR(0, 31);
+  if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
 #ifdef LSA_TC_TRACE
   if (tid == 0 && (cta == 0 || cta == gridDim.x - 1)) tlog_add(p.tlog, cta == 0 ? 1 : 2, g_entry);
 #endif

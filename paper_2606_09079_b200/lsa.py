@@ -263,13 +263,13 @@ class LsaContext:
     def sync(self):
         self._check(_lib.lsa_sync(self._h))
 
-    PHASES = ("prestep", "attention", "combine", "index", "residency", "fetch")
+    PHASES = ("prestep", "attention", "combine", "index", "residency", "fetch", "attention_dev")
 
     def profile_enable(self, capacity: int):
         self._check(_lib.lsa_profile_enable(self._h, capacity))
 
     def profile_read(self) -> dict:
-        ms, cnt = (C.c_double * 6)(), (C.c_int64 * 6)()
+        ms, cnt = (C.c_double * 7)(), (C.c_int64 * 7)()
         self._check(_lib.lsa_profile_read(self._h, ms, cnt))
         return {p: dict(ms=ms[i], count=cnt[i]) for i, p in enumerate(self.PHASES)}
 
