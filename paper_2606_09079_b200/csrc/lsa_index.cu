@@ -21,6 +21,8 @@ __global__ void __launch_bounds__(kQtWarps * 32)
 qtower_kernel(const T* __restrict__ W, const T* __restrict__ h, FireList rows, float* __restrict__ z, int E, int Dh) {
   constexpr int V = Elem<T>::kVec;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  pdl_wait();
+  pdl_launch_dependents();
   const int e = blockIdx.x * kQtWarps + warp;
   const int i0 = blockIdx.y * kQtSeqs;
   const int n = rows.n;
@@ -61,6 +63,8 @@ score_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __rest
   __shared__ float inv_norm_s;
   constexpr int V = Elem<T>::kVec;
   const int i = blockIdx.y;
+  pdl_wait();
+  pdl_launch_dependents();
   const SeqDev& sq = seqs[fire.ids[i]];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int c0 = blockIdx.x * kScWarps;
@@ -99,6 +103,8 @@ topk_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __restr
             int n_chunks_max, int k, int32_t* __restrict__ sel_idx, float* __restrict__ sel_score) {
   __shared__ SelectSmem sm;
   const int i = blockIdx.x;
+  pdl_wait();
+  pdl_launch_dependents();
   const SeqDev& sq = seqs[fire.ids[i]];
   const float* sc = scores + (size_t)i * n_chunks_max;
   auto keyf = [sc](int c) -> unsigned long long {
@@ -122,10 +128,8 @@ cudaError_t launch_qtower(int dtype, const void* W, const void* h, const FireLis
                           cudaStream_t st) {
   dim3 grid((E + kQtWarps - 1) / kQtWarps, (rows.n + kQtSeqs - 1) / kQtSeqs);
   if (dtype == 0)
-    qtower_kernel<float><<<grid, kQtWarps * 32, 0, st>>>((const float*)W, (const float*)h, rows, z, E, Dh);
-  else
-    qtower_kernel<__nv_bfloat16><<<grid, kQtWarps * 32, 0, st>>>((const __nv_bfloat16*)W, (const __nv_bfloat16*)h, rows, z, E, Dh);
-  return cudaGetLastError();
+    return launch_pdl(qtower_kernel<float>, grid, dim3(kQtWarps * 32), 0, st, (const float*)W, (const float*)h, rows, z, E, Dh);
+  return launch_pdl(qtower_kernel<__nv_bfloat16>, grid, dim3(kQtWarps * 32), 0, st, (const __nv_bfloat16*)W, (const __nv_bfloat16*)h, rows, z, E, Dh);
 }
 
 cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, const float* z, float* scores,
@@ -133,16 +137,13 @@ cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, c
   dim3 grid((n_chunks_max + kScWarps - 1) / kScWarps, fire.n);
   size_t smem = (size_t)E * sizeof(float);
   if (dtype == 0)
-    score_kernel<float><<<grid, kScWarps * 32, smem, st>>>(seqs, fire, z, scores, E, n_chunks_max);
-  else
-    score_kernel<__nv_bfloat16><<<grid, kScWarps * 32, smem, st>>>(seqs, fire, z, scores, E, n_chunks_max);
-  return cudaGetLastError();
+    return launch_pdl(score_kernel<float>, grid, dim3(kScWarps * 32), smem, st, seqs, fire, z, scores, E, n_chunks_max);
+  return launch_pdl(score_kernel<__nv_bfloat16>, grid, dim3(kScWarps * 32), smem, st, seqs, fire, z, scores, E, n_chunks_max);
 }
 
 cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores, int n_chunks_max, int k,
                         int32_t* sel_idx, float* sel_score, cudaStream_t st) {
-  topk_kernel<<<fire.n, 1024, 0, st>>>(seqs, fire, scores, n_chunks_max, k, sel_idx, sel_score);
-  return cudaGetLastError();
+  return launch_pdl(topk_kernel, dim3(fire.n), dim3(1024), 0, st, seqs, fire, scores, n_chunks_max, k, sel_idx, sel_score);
 }
 
 }  // namespace lsa

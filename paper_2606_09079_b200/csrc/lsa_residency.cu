@@ -39,6 +39,8 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ResSmem& sm = *reinterpret_cast<ResSmem*>(smem_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_wait();
+  pdl_launch_dependents();
   if (tid == 0) pool.counters[C_FETCH_COUNT] = 0;
   __syncthreads();
 
@@ -193,6 +195,7 @@ __device__ __forceinline__ uint4 ld_stream16(const uint4* p) {
 
 __global__ void __launch_bounds__(kFetchThreads)
 fetch_kernel(PoolDev pool, unsigned char* __restrict__ hot_pool, long long page_bytes) {
+  pdl_wait();                      // the fetch list of the residency pass is complete
   const int n_fetch = (int)pool.counters[C_FETCH_COUNT];
   const int slices = (int)((page_bytes + kFetchSlice - 1) / kFetchSlice);
   const long long items = (long long)n_fetch * slices;
@@ -259,13 +262,11 @@ cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, c
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  residency_kernel<<<1, 1024, sizeof(ResSmem), st>>>(seqs, pool, fire, sel_idx, B, k, P, page_bytes);
-  return cudaGetLastError();
+  return launch_pdl(residency_kernel, dim3(1), dim3(1024), sizeof(ResSmem), st, seqs, pool, fire, sel_idx, B, k, P, page_bytes);
 }
 
 cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas, cudaStream_t st) {
-  fetch_kernel<<<n_ctas, kFetchThreads, 0, st>>>(pool, reinterpret_cast<unsigned char*>(hot_pool), page_bytes);
-  return cudaGetLastError();
+  return launch_pdl(fetch_kernel, dim3(n_ctas), dim3(kFetchThreads), 0, st, pool, reinterpret_cast<unsigned char*>(hot_pool), page_bytes);
 }
 
 cudaError_t launch_prestep(int dtype, SeqDev* seqs, int B, int D, int W, const uint32_t* swap_mask_words,
