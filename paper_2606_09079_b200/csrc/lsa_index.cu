@@ -31,17 +31,31 @@ qtower_kernel(const T* __restrict__ W, const T* __restrict__ h, FireList rows, f
 #pragma unroll
   for (int s = 0; s < kQtSeqs; ++s) acc[s] = 0.f;
   const T* wrow = W + (size_t)e * Dh;
-#pragma unroll 8
-  for (int d0 = lane * V; d0 < Dh; d0 += 32 * V) {
-    float wf[V];
-    Elem<T>::load16(wrow + d0, wf);
+  // 8 independent 16-byte loads of the weight row are issued before any of them is used (the row is read once
+  // from HBM; h comes from L1/L2), so a 4096-wide row is two memory round trips, not sixteen
+  constexpr int kU = 8;
+  for (int d0 = lane * V; d0 < Dh; d0 += 32 * V * kU) {
+    uint4 wraw[kU];
 #pragma unroll
-    for (int s = 0; s < kQtSeqs; ++s) {
-      if (i0 + s < n) {
-        float hf[V];
-        Elem<T>::load16(h + (size_t)rows.ids[i0 + s] * Dh + d0, hf);
+    for (int u = 0; u < kU; ++u) {
+      const int d = d0 + u * 32 * V;
+      wraw[u] = d < Dh ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+    }
 #pragma unroll
-        for (int j = 0; j < V; ++j) acc[s] = fmaf(wf[j], hf[j], acc[s]);
+    for (int u = 0; u < kU; ++u) {
+      const int d = d0 + u * 32 * V;
+      if (d < Dh) {
+        float wf[V];
+        Elem<T>::unpack16(wraw[u], wf);
+#pragma unroll
+        for (int s = 0; s < kQtSeqs; ++s) {
+          if (i0 + s < n) {
+            float hf[V];
+            Elem<T>::load16(h + (size_t)rows.ids[i0 + s] * Dh + d, hf);
+#pragma unroll
+            for (int j = 0; j < V; ++j) acc[s] = fmaf(wf[j], hf[j], acc[s]);
+          }
+        }
       }
     }
   }

@@ -1,7 +1,7 @@
 // lsa_select.cuh - block-wide "m smallest of n unique 64-bit keys, sorted" used by
 //   S3 top-k      (key = ~ordered(score) << 32 | chunk idx  -> score desc, idx asc; BJ north_star)
 //   S4 allocation (key = last_used << 20 | page             -> never-used first, then LRU; R12)
-// n <= kSortCap: bitonic sort in shared memory.  Larger n: 8-bit MSB radix select of the m-th key,
+// n <= kSortAll: bitonic sort in shared memory.  Larger n: 8-bit MSB radix select of the m-th key,
 // compaction of the m winners, bitonic sort of those.  Deterministic: keys are unique.
 #pragma once
 #include "lsa_common.cuh"
@@ -9,6 +9,7 @@
 namespace lsa {
 
 constexpr unsigned long long kKeyMax = 0xffffffffffffffffull;
+constexpr int kSortAll = kSortCap;         // up to this many keys the whole set is sorted; above, radix select first
 
 struct SelectSmem {
   unsigned long long keys[kSortCap];
@@ -29,13 +30,13 @@ __device__ __forceinline__ int next_pow2(int n) {
 __device__ inline void block_bitonic_sort(unsigned long long* keys, int n_pad) {
   for (int k = 2; k <= n_pad; k <<= 1) {
     for (int j = k >> 1; j > 0; j >>= 1) {
-      for (int i = threadIdx.x; i < n_pad; i += blockDim.x) {
-        int ixj = i ^ j;
-        if (ixj > i) {
-          unsigned long long a = keys[i], b = keys[ixj];
-          bool up = ((i & k) == 0);
-          if ((a > b) == up) { keys[i] = b; keys[ixj] = a; }
-        }
+      // one thread per compare-exchange pair: i has bit j clear, its partner is i | j
+      for (int t = threadIdx.x; t < (n_pad >> 1); t += blockDim.x) {
+        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+        const int ixj = i | j;
+        unsigned long long a = keys[i], b = keys[ixj];
+        const bool up = ((i & k) == 0);
+        if ((a > b) == up) { keys[i] = b; keys[ixj] = a; }
       }
       __syncthreads();
     }
@@ -49,7 +50,7 @@ template <class KeyF>
 __device__ inline int block_select_smallest(KeyF keyf, int n, int m, SelectSmem& sm) {
   if (m > n) m = n;
   if (m <= 0) return 0;
-  if (n <= kSortCap) {
+  if (n <= kSortAll) {
     int n_pad = next_pow2(n);
     for (int i = threadIdx.x; i < n_pad; i += blockDim.x) sm.keys[i] = i < n ? keyf(i) : kKeyMax;
     __syncthreads();
