@@ -4,3 +4,4 @@ from .lsa_oracle import (  # noqa: F401
     merge_partials, partial_attention, query_tower, topk_select, trigger_fires,
     validate_selection, widen,
 )
+from . import l1_oracle  # noqa: F401,E402  (paper-exact Level-1 indexer, NEXT-1)
