@@ -166,6 +166,41 @@ int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, cons
 int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new,
                   const void* v_new, void* out);
 
+/* ---- paper-exact Level-1 Memory Indexer (Eq.(1)-(5), l.142 Eq.(13))) --------
+ * An alternative to lsa_index_select with the scorer the paper states: per indexer layer
+ *   c = h W^DQ (1), q = c W^IUQ split into n_h heads of c_I (2), w = h W^w (3),
+ *   I_s = sigmoid(sum_h w_h ReLU(q_h . K_s)) for every compressed entry s (4),
+ * an entry is recalled if I_s >= threshold in ANY layer (5, 13); recall is page granular (l.185): chunk
+ * c = entries [c*C, (c+1)*C) is selected iff one of its entries is, with score = max I over its entries and
+ * layers, and if more than k (= K_max) chunks qualify the k best by (score desc, chunk id asc) are kept.
+ * All weights are stored TRANSPOSED, [out][in] row-major, bf16.  Supported: dtype bf16, C = 128, c_I = 128,
+ * n_h = 64 (else LSA_ERR_UNSUPPORTED); d_c % 8 == 0; 1..4 layers. */
+typedef struct lsa_l1_layer {
+  const void* W_dq;      /* DEVICE [d_c][Dh]          = (W^DQ)^T                                         */
+  const void* W_iuq;     /* DEVICE [n_h*c_I][d_c]     = (W^IUQ)^T, head h = rows [h*c_I, (h+1)*c_I)      */
+  const void* W_w;       /* DEVICE [n_h][Dh]          = (W^w)^T                                          */
+} lsa_l1_layer;
+
+typedef struct lsa_l1_config {
+  uint32_t struct_size;  /* = sizeof(lsa_l1_config)                                                      */
+  int32_t n_layers;      /* indexer layers whose sets are OR-ed (the paper uses 3: layers 10, 12, 20)    */
+  int32_t d_c;           /* low-rank query dim (paper: r = 2048, l.153)                                  */
+  int32_t c_I;           /* index-key dim per head                                                       */
+  int32_t n_h;           /* indexer heads                                                                */
+  float threshold;       /* 0 -> 0.5 (l.77); must be in (0, 1)                                           */
+  lsa_l1_layer layers[4];
+} lsa_l1_config;
+
+/* index_k: HOST array of B * n_layers DEVICE pointers; index_k[b * n_layers + l] = compressed indexer keys
+ * K^IComp of sequence b for layer l, [n_csa_b][c_I] bf16, caller-owned, must outlive the context (the
+ * index-K of the Memory-Indexer layers stays on the GPU).  May be called once per context. */
+int lsa_l1_init(lsa_ctx* ctx, const lsa_l1_config* cfg, const void* const* index_k);
+
+/* Eq.(1)-(5), (13) for n sequences on stream_fetch; same argument conventions and output format as
+ * lsa_index_select (sel_idx DEVICE [n][k], valid ids first in (score desc, id asc) order, then -1;
+ * sel_score DEVICE [n][k] = I of the chunk, -inf padding, may be NULL), so the result feeds lsa_fetch_chunks. */
+int lsa_l1_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n, int32_t* sel_idx, float* sel_score);
+
 /* Replace the embedding table pointer of one sequence (DEVICE [n_chunks][E]). */
 int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb);
 

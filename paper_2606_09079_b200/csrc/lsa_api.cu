@@ -16,6 +16,7 @@
 #include "../../include/lsa.h"
 #include "lsa_attn_tc.h"
 #include "lsa_kernels.h"
+#include "lsa_l1.h"
 
 using namespace lsa;
 
@@ -51,6 +52,8 @@ struct lsa_ctx {
   float* part_ml = nullptr;
   int fetch_ctas = 0;
   TcPlan* tc = nullptr;
+  L1Plan* l1 = nullptr;               // paper-exact Level-1 indexer (lsa_l1_init)
+  float l1_threshold = 0.5f;
   // host-buffer staging (lsa_step_host)
   void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
   const void* out_host_cached = nullptr;
@@ -123,6 +126,7 @@ extern "C" void lsa_destroy(lsa_ctx* ctx) {
   if (ctx->sc) cudaStreamSynchronize(ctx->sc);
   if (ctx->sf) cudaStreamSynchronize(ctx->sf);
   if (ctx->tc) tc_destroy(ctx->tc);
+  if (ctx->l1) l1_destroy(ctx->l1);
   if (ctx->st_pin) cudaFreeHost(ctx->st_pin);
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
@@ -328,6 +332,49 @@ extern "C" int lsa_index_select(lsa_ctx* ctx, const void* h, const int32_t* seq_
   std::vector<int> rows(n);
   for (int i = 0; i < n; ++i) rows[i] = i;
   return index_select_impl(ctx, h, seq_ids, rows.data(), n, sel_idx, sel_score);
+}
+
+// ---- paper-exact Level-1 indexer (NEXT-1) ---------------------------------------------------------
+extern "C" int lsa_l1_init(lsa_ctx* ctx, const lsa_l1_config* cfg, const void* const* index_k) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (!cfg || !index_k) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null argument");
+  if (cfg->struct_size != sizeof(lsa_l1_config)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "lsa_l1_config.struct_size mismatch");
+  if (c->l1) LSA_FAIL(c, LSA_ERR_STATE, "lsa_l1_init was already called on this context");
+  if (cfg->n_layers < 1 || cfg->n_layers > 4 || cfg->d_c < 8 || cfg->d_c % 8) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "n_layers must be 1..4, d_c a multiple of 8");
+  const float thr = cfg->threshold == 0.f ? 0.5f : cfg->threshold;
+  if (!(thr > 0.f && thr < 1.f)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "threshold must be in (0, 1)");
+  if (!l1_supported(c->cfg.dtype, c->cfg.C, cfg->c_I, cfg->n_h))
+    LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "Level-1 indexer needs bf16, C=128, c_I=128, n_h=64 (got dtype=%d C=%d c_I=%d n_h=%d)", c->cfg.dtype, c->cfg.C,
+             cfg->c_I, cfg->n_h);
+  L1Init in{};
+  in.B = c->B; in.n_layers = cfg->n_layers; in.Dh = c->cfg.Dh; in.d_c = cfg->d_c; in.n_chunks_max = c->n_chunks_max; in.n_sms = c->n_sms;
+  for (int l = 0; l < cfg->n_layers; ++l) {
+    if (!cfg->layers[l].W_dq || !cfg->layers[l].W_iuq || !cfg->layers[l].W_w) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null weight pointer in layer %d", l);
+    in.layers[l].W_dq = cfg->layers[l].W_dq; in.layers[l].W_iuq = cfg->layers[l].W_iuq; in.layers[l].W_w = cfg->layers[l].W_w;
+  }
+  in.index_k = index_k;
+  in.seq_host = c->seq_host.data();
+  std::string msg;
+  const int rc = l1_create(in, &c->l1, &msg);
+  if (rc != 0) LSA_FAIL(c, rc, "Level-1 indexer init failed: %s", msg.c_str());
+  c->l1_threshold = thr;
+  return LSA_OK;
+}
+
+extern "C" int lsa_l1_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n, int32_t* sel_idx, float* sel_score) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!ctx->l1) LSA_FAIL(ctx, LSA_ERR_STATE, "lsa_l1_init has not been called");
+  if (!h || !sel_idx) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null h / sel_idx");
+  int rc = check_ids(ctx, seq_ids, n);
+  if (rc) return rc;
+  std::string msg;
+  int launches = 0;
+  ProfScope prof(ctx, LSA_PH_INDEX, ctx->sf);
+  rc = l1_select(ctx->l1, ctx->d_seqs, h, seq_ids, n, ctx->k, ctx->l1_threshold, sel_idx, sel_score, ctx->sf, &launches, &msg);
+  ctx->index_launches += launches;
+  if (rc != 0) LSA_FAIL(ctx, rc == -1 ? LSA_ERR_INVALID_ARG : LSA_ERR_CUDA, "Level-1 indexer: %s", msg.c_str());
+  return LSA_OK;
 }
 
 // ---- S4-S5 ------------------------------------------------------------------------------------

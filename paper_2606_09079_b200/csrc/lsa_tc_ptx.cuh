@@ -33,7 +33,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 }
 // Bounded wait: a protocol bug traps (-> launch failure) instead of hanging the GPU.  The slow path is kept out of
 // line: the kernel waits at ~25 sites and its straight-line code is executed once per launch, instruction-cache cold.
-__device__ __noinline__ void mbar_wait_slow(uint64_t* bar, uint32_t parity, int tag) {
+static __device__ __noinline__ void mbar_wait_slow(uint64_t* bar, uint32_t parity, int tag) {
   const long long t0 = clock64();
   while (!mbar_try_wait(bar, parity)) {
     if (clock64() - t0 > 4000000000ll) {   // ~2 s at 2 GHz

@@ -31,7 +31,7 @@ STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_E
 EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit_tables",
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
-           "lsa_profile_enable", "lsa_profile_read",
+           "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select",
            "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
@@ -63,6 +63,15 @@ class lsa_stats(C.Structure):
                 ("attn_impl", C.c_int32), ("attn_ctas", C.c_int32), ("reserved", C.c_int32)]
 
 
+class lsa_l1_layer(C.Structure):
+    _fields_ = [("W_dq", C.c_void_p), ("W_iuq", C.c_void_p), ("W_w", C.c_void_p)]
+
+
+class lsa_l1_config(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_int32), ("d_c", C.c_int32), ("c_I", C.c_int32),
+                ("n_h", C.c_int32), ("threshold", C.c_float), ("layers", lsa_l1_layer * 4)]
+
+
 def _load() -> C.CDLL:
     if not os.path.exists(LIB_PATH):
         raise ImportError(
@@ -85,6 +94,8 @@ def _load() -> C.CDLL:
     lib.lsa_sync.argtypes = [vp]
     lib.lsa_profile_enable.argtypes = [vp, C.c_int32]
     lib.lsa_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    lib.lsa_l1_init.argtypes = [vp, C.POINTER(lsa_l1_config), C.POINTER(vp)]
+    lib.lsa_l1_select.argtypes = [vp, vp, i32p, C.c_int32, vp, f32p]
     lib.lsa_last_error.argtypes = [vp]
     lib.lsa_last_error.restype = C.c_char_p
     lib.lsa_destroy.argtypes = [vp]
@@ -206,6 +217,34 @@ class LsaContext:
         sc = torch.empty((n, self.k), dtype=torch.float32, device=h.device) if want_scores else None
         self._check(_lib.lsa_index_select(self._h, _dev_ptr(h, self.tdtype, "h"), arr, n, sel.data_ptr(),
                                           None if sc is None else sc.data_ptr()))
+        return sel, sc
+
+    def l1_init(self, layers: Sequence[dict], index_k: Sequence[Sequence[torch.Tensor]], d_c: int, c_I: int = 128,
+                n_h: int = 64, threshold: float = 0.5):
+        """Paper-exact Level-1 indexer (Eq. 1-5, 13).  layers[l] = dict(W_dq [d_c][Dh], W_iuq [n_h*c_I][d_c],
+        W_w [n_h][Dh]) bf16 CUDA tensors; index_k[b][l] = [n_csa_b][c_I] bf16 CUDA tensor."""
+        cfg = lsa_l1_config()
+        cfg.struct_size = C.sizeof(lsa_l1_config)
+        cfg.n_layers, cfg.d_c, cfg.c_I, cfg.n_h, cfg.threshold = len(layers), d_c, c_I, n_h, threshold
+        for l, lay in enumerate(layers):
+            cfg.layers[l].W_dq = _dev_ptr(lay["W_dq"], self.tdtype, "W_dq")
+            cfg.layers[l].W_iuq = _dev_ptr(lay["W_iuq"], self.tdtype, "W_iuq")
+            cfg.layers[l].W_w = _dev_ptr(lay["W_w"], self.tdtype, "W_w")
+        L = len(layers)
+        ptrs = (C.c_void_p * (self.B * L))()
+        for b in range(self.B):
+            for l in range(L):
+                t = index_k[b][l]
+                ptrs[b * L + l] = _dev_ptr(t, self.tdtype, "index_k") if t is not None and t.numel() else None
+        self._keep += [list(layers), [list(x) for x in index_k]]
+        self._check(_lib.lsa_l1_init(self._h, C.byref(cfg), ptrs))
+
+    def l1_select(self, h: torch.Tensor, seq_ids: Sequence[int], want_scores: bool = True):
+        arr, n = _ids(seq_ids)
+        sel = torch.empty((n, self.k), dtype=torch.int32, device=h.device)
+        sc = torch.empty((n, self.k), dtype=torch.float32, device=h.device) if want_scores else None
+        self._check(_lib.lsa_l1_select(self._h, _dev_ptr(h, self.tdtype, "h"), arr, n, sel.data_ptr(),
+                                       None if sc is None else sc.data_ptr()))
         return sel, sc
 
     def fetch_chunks(self, seq_ids: Sequence[int], sel_idx: torch.Tensor):

@@ -413,3 +413,55 @@ def plant_boundary_ties(emb: np.ndarray, order: np.ndarray, k: int, dtype: str) 
             row[j] = np.nextafter(row[j], np.float32(0))
         out[order[k + 1]] = row
     return out
+
+
+# --------------------------------------------------------------------------------------
+# inputs of the paper-exact Level-1 indexer (Eq.(1)-(5), (13))
+# --------------------------------------------------------------------------------------
+class L1Inputs:
+    """Seeded weights and compressed indexer keys for `n_layers` Memory-Indexer layers on top of an
+    LsaWorkload (which supplies h_t, Dh, n_csa, C).  Shapes the paper leaves open (R28) are parameters:
+    d_c (paper: r = 2048), c_I = 128, n_h = 64.  All arrays are stored bf16 bit patterns, transposed
+    [out][in] (oracle/l1_oracle.py reading L1).
+
+    Structure: W_w is built so that w = W_w h0 is about +1 on `n_pos` heads and -0.5 on the others, random keys
+    therefore score clearly below the threshold; in about `hot_frac` of the chunks one entry is aligned with a
+    positive head's query (match ~ `hot_gain`), so it scores clearly above.  Near-threshold entries arise
+    naturally from the noise.  The alignment uses q0 = W_iuq (W_dq h0), computed here only to PLACE inputs."""
+
+    def __init__(self, wl: "LsaWorkload", n_layers: int = 3, d_c: int = 256, c_I: int = 128, n_h: int = 64, n_pos: int = 8,
+                 hot_frac: float = 0.06, hot_gain: float = 14.0, tag: int = 900):
+        c = wl.cfg
+        assert c.dtype == "bf16"
+        self.n_layers, self.d_c, self.c_I, self.n_h = n_layers, d_c, c_I, n_h
+        self.layers: List[dict] = []
+        self.index_k: List[List[np.ndarray]] = [[] for _ in range(c.B)]
+        self.hot_chunks: List[List[np.ndarray]] = [[] for _ in range(c.B)]
+        s = c.seed
+        for l in range(n_layers):
+            W_dq = _randn_stored(_rng(s, tag, l, 1), (d_c, c.Dh), 1.0 / math.sqrt(c.Dh), "bf16")
+            W_iuq = _randn_stored(_rng(s, tag, l, 2), (n_h * c_I, d_c), 1.0 / math.sqrt(d_c), "bf16")
+            g = _rng(s, tag, l, 3)
+            a = np.full(n_h, -0.5)
+            a[g.choice(n_h, size=n_pos, replace=False)] = 1.0
+            # one W_w for all sequences: built from the mean direction of the sequences' h0
+            hbar = np.mean([as_f64(wl.h0[b], "bf16") for b in range(c.B)], axis=0)
+            W_w = np.outer(a, hbar) / float(hbar @ hbar) + 0.02 * g.standard_normal((n_h, c.Dh)) / math.sqrt(c.Dh)
+            W_w = store(W_w.astype(np.float32), "bf16")
+            self.layers.append(dict(W_dq=W_dq, W_iuq=W_iuq, W_w=W_w))
+            Wd, Wu = as_f64(W_dq, "bf16"), as_f64(W_iuq, "bf16")
+            for b in range(c.B):
+                n, nch = c.n_csa(b), c.n_chunks(b)
+                q0 = (Wu @ (Wd @ as_f64(wl.h0[b], "bf16"))).reshape(n_h, c_I)
+                scale = 1.0 / np.mean(np.linalg.norm(q0, axis=1))
+                gk = _rng(s, tag, l, 10 + b)
+                K = gk.standard_normal((n, c_I)) * scale
+                hot = np.nonzero(gk.random(nch) < hot_frac)[0]
+                pos_heads = np.nonzero(a > 0)[0]
+                for ch in hot:
+                    lo, hi = ch * c.C, min(n, (ch + 1) * c.C)
+                    e = int(gk.integers(lo, hi))
+                    p = int(pos_heads[gk.integers(len(pos_heads))])
+                    K[e] = hot_gain * q0[p] / float(q0[p] @ q0[p])
+                self.index_k[b].append(store(K.astype(np.float32), "bf16"))
+                self.hot_chunks[b].append(hot)
