@@ -182,6 +182,7 @@ def main():
     ap.add_argument("--attn", default="auto", choices=["auto", "simt", "tcgen05"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", type=int, default=0)
+    ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -364,6 +365,35 @@ def main():
                      residency_ms_per_trigger=pr["residency"]["ms"] / max(pr["residency"]["count"], 1))
         del src, dst
 
+    # ---- optional: the paper-exact Level-1 indexer (NEXT-1) at this config's context length ----
+    l1 = None
+    if args.l1 and rank == 0 and c.dtype == "bf16" and c.C == 128:
+        from paper_2606_09079_b200.workloads import L1Inputs
+        L, d_c = 3, 2048                                   # paper: layers {10,12,20}, low-rank query dim r = 2048
+        l1in = L1Inputs(wl, n_layers=L, d_c=d_c)
+        r = reps[0]
+        layers = [{k_: to_torch(v, "bf16").to(dev) for k_, v in lay.items()} for lay in l1in.layers]
+        index_k = [[to_torch(K, "bf16").to(dev) for K in l1in.index_k[b]] for b in range(c.B)]
+        r.ctx.l1_init(layers, index_k, d_c=d_c)
+        hd = to_torch(wl.h(0), c.dtype).to(dev)
+        ids = list(range(c.B))
+        for _ in range(3):
+            r.ctx.l1_select(hd, ids, want_scores=False)
+        r.ctx.sync()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_it = 20
+        e0.record(sf)
+        for _ in range(n_it):
+            r.ctx.l1_select(hd, ids, want_scores=False)
+        e1.record(sf)
+        sf.synchronize()
+        l1_ms = e0.elapsed_time(e1) / n_it
+        key_bytes = sum(c.n_csa(b) for b in range(c.B)) * 128 * 2 * L
+        w_bytes = L * (d_c * c.Dh + 64 * 128 * d_c + 64 * c.Dh) * 2
+        l1 = dict(ms_per_trigger=l1_ms, layers=L, d_c=d_c, c_I=128, n_h=64, index_key_bytes=key_bytes, weight_bytes=w_bytes,
+                  gbs=(key_bytes + w_bytes) / (l1_ms * 1e-3) / 1e9, frac_of_hbm_peak=(key_bytes + w_bytes) / (l1_ms * 1e-3) / 1e9 / load_peaks()["hbm_gbs"],
+                  note="Eq.(1)-(5),(13) for all sequences of the config, warm L2 for the weights (same call repeated)")
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n, secs, threads = oracle_sample(wl, budget_s=15.0, max_steps=24)
@@ -384,7 +414,7 @@ def main():
                              ms_per_step=ms_e2e / n_e2e),
                     gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, wall_s=wall,
+                    fetch=fetch, l1_indexer=l1, wall_s=wall,
                     tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
         print(json.dumps(line))
     if world > 1:

@@ -31,9 +31,9 @@ qtower_kernel(const T* __restrict__ W, const T* __restrict__ h, FireList rows, f
 #pragma unroll
   for (int s = 0; s < kQtSeqs; ++s) acc[s] = 0.f;
   const T* wrow = W + (size_t)e * Dh;
-  // 8 independent 16-byte loads of the weight row are issued before any of them is used (the row is read once
-  // from HBM; h comes from L1/L2), so a 4096-wide row is two memory round trips, not sixteen
-  constexpr int kU = 8;
+  // 16 independent 16-byte loads of the weight row are issued before any of them is used (the row is read once
+  // from HBM; h comes from L1/L2), so a 4096-wide bf16 row is one memory round trip, not sixteen
+  constexpr int kU = 16;
   for (int d0 = lane * V; d0 < Dh; d0 += 32 * V * kU) {
     uint4 wraw[kU];
 #pragma unroll

@@ -56,28 +56,45 @@ template <> __device__ __forceinline__ __nv_bfloat16 l1_out<__nv_bfloat16>(float
 
 constexpr int kGvWarps = 4, kGvSeqs = 4;
 
-// W bf16 [E][Din]; x [n][ldx] (row i at x + i*ldx); out [n][ldo] (row i at out + i*ldo)
+// W bf16 [E][Din]; x [n][ldx] (row i at x + i*ldx); out [n][ldo] (row i at out + i*ldo).
+// The block first stages its (up to 4) x rows in shared memory - read from L2 inside the FMA loop they would be
+// 16 dependent round trips per lane - then every warp streams one weight row with all its loads in flight.
 template <typename XT, typename OT>
 __global__ void __launch_bounds__(kGvWarps * 32)
 l1_gemv_kernel(const __nv_bfloat16* __restrict__ W, const XT* __restrict__ x, long long ldx, OT* __restrict__ out, long long ldo,
                int n, int E, int Din) {
+  extern __shared__ __align__(16) unsigned char gv_smem[];
+  XT* xs = reinterpret_cast<XT*>(gv_smem);                 // [kGvSeqs][Din]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  pdl_wait();
-  pdl_launch_dependents();
   const int e = blockIdx.x * kGvWarps + warp;
   const int i0 = blockIdx.y * kGvSeqs;
+  const __nv_bfloat16* wrow = W + (size_t)min(e, E - 1) * Din;
+  constexpr int kU = 16;
+  uint4 wraw[kU];
+#pragma unroll
+  for (int u = 0; u < kU; ++u) {                            // weights never depend on the previous kernel
+    const int d = lane * 8 + u * 256;
+    wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+  }
+  pdl_wait();
+  pdl_launch_dependents();
+  constexpr int kPer16 = 16 / (int)sizeof(XT);
+  for (int s = 0; s < kGvSeqs; ++s)
+    if (i0 + s < n)
+      for (int d = threadIdx.x * kPer16; d < Din; d += kGvWarps * 32 * kPer16)
+        *reinterpret_cast<uint4*>(xs + (size_t)s * Din + d) = *reinterpret_cast<const uint4*>(x + (size_t)(i0 + s) * ldx + d);
+  __syncthreads();
   if (e >= E) return;
   float acc[kGvSeqs];
 #pragma unroll
   for (int s = 0; s < kGvSeqs; ++s) acc[s] = 0.f;
-  const __nv_bfloat16* wrow = W + (size_t)e * Din;
-  constexpr int kU = 8;
   for (int d0 = lane * 8; d0 < Din; d0 += 256 * kU) {
-    uint4 wraw[kU];
+    if (d0 != lane * 8) {                                   // rows longer than 4096: further batches
 #pragma unroll
-    for (int u = 0; u < kU; ++u) {
-      const int d = d0 + u * 256;
-      wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+      for (int u = 0; u < kU; ++u) {
+        const int d = d0 + u * 256;
+        wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+      }
     }
 #pragma unroll
     for (int u = 0; u < kU; ++u) {
@@ -89,7 +106,7 @@ l1_gemv_kernel(const __nv_bfloat16* __restrict__ W, const XT* __restrict__ x, lo
         for (int s = 0; s < kGvSeqs; ++s) {
           if (i0 + s < n) {
             float xf[8];
-            L1X<XT>::load8(x + (size_t)(i0 + s) * ldx + d, xf);
+            L1X<XT>::load8(xs + (size_t)s * Din + d, xf);
 #pragma unroll
             for (int j = 0; j < 8; ++j) acc[s] = fmaf(wf[j], xf[j], acc[s]);
           }
@@ -381,6 +398,9 @@ int l1_create(const L1Init& init, L1Plan** out, std::string* msg) {
   if (!l1_encode(pl->encode, &pl->map_q, pl->q, pieces * kL1H, kL1H, msg)) { delete pl; return -2; }
   pl->smem = sizeof(L1Smem) + 1024;
   L1_CUDA(cudaFuncSetAttribute(l1_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
+  if ((size_t)kGvSeqs * init.Dh * 2 > 200 * 1024 || (size_t)kGvSeqs * init.d_c * 4 > 200 * 1024) { *msg = "Dh / d_c too large for the staged projections"; delete pl; return -6; }
+  L1_CUDA(cudaFuncSetAttribute(l1_gemv_kernel<__nv_bfloat16, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  L1_CUDA(cudaFuncSetAttribute(l1_gemv_kernel<float, __nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   *out = pl;
   return 0;
 }
@@ -407,13 +427,13 @@ int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, i
       const __nv_bfloat16* Ww = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_w);
       float* cq = pl->cq + (size_t)l * pl->cap * d_c;
       // Eq.(1): c^Q [m][d_c] fp32
-      L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((d_c + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, 0, st,
+      L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((d_c + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * Dh * 2, st,
                          Wdq, hb + (size_t)off * Dh, (long long)Dh, cq, (long long)d_c, m, d_c, Dh));
       // Eq.(3): w -> piece (i, l)
-      L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((kL1H + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, 0, st,
+      L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((kL1H + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * Dh * 2, st,
                          Ww, hb + (size_t)off * Dh, (long long)Dh, pl->wbuf + (size_t)l * kL1H, (long long)L * kL1H, m, kL1H, Dh));
       // Eq.(2): q -> piece (i, l), rounded to bf16
-      L1_CUDA(launch_pdl(l1_gemv_kernel<float, __nv_bfloat16>, dim3((kL1H * kL1CI + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, 0, st,
+      L1_CUDA(launch_pdl(l1_gemv_kernel<float, __nv_bfloat16>, dim3((kL1H * kL1CI + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * d_c * 4, st,
                          Wiuq, (const float*)cq, (long long)d_c, pl->q + (size_t)l * kL1H * kL1CI, (long long)L * kL1H * kL1CI, m,
                          kL1H * kL1CI, d_c));
       *launches += 3;
