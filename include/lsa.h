@@ -201,6 +201,11 @@ int lsa_l1_init(lsa_ctx* ctx, const lsa_l1_config* cfg, const void* const* index
  * sel_score DEVICE [n][k] = I of the chunk, -inf padding, may be NULL), so the result feeds lsa_fetch_chunks. */
 int lsa_l1_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n, int32_t* sel_idx, float* sel_score);
 
+/* Which indexer lsa_step runs at trigger steps: BASELINE.json's dual encoder (S1-S3, default) or the
+ * paper-exact Level-1 indexer (needs lsa_l1_init). */
+enum lsa_indexer { LSA_INDEXER_DUAL_ENCODER = 0, LSA_INDEXER_LEVEL1 = 1 };
+int lsa_set_indexer(lsa_ctx* ctx, int32_t indexer);
+
 /* Replace the embedding table pointer of one sequence (DEVICE [n_chunks][E]). */
 int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb);
 

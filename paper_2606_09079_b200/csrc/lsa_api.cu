@@ -54,6 +54,7 @@ struct lsa_ctx {
   TcPlan* tc = nullptr;
   L1Plan* l1 = nullptr;               // paper-exact Level-1 indexer (lsa_l1_init)
   float l1_threshold = 0.5f;
+  int indexer = 0;                     // lsa_indexer used by lsa_step at trigger steps
   // host-buffer staging (lsa_step_host)
   void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
   const void* out_host_cached = nullptr;
@@ -362,18 +363,32 @@ extern "C" int lsa_l1_init(lsa_ctx* ctx, const lsa_l1_config* cfg, const void* c
   return LSA_OK;
 }
 
+static int l1_select_impl(lsa_ctx* ctx, const void* h, const int* ids, const int* rows, int n, int32_t* sel_idx, float* sel_score) {
+  std::string msg;
+  int launches = 0;
+  ProfScope prof(ctx, LSA_PH_INDEX, ctx->sf);
+  const int rc = l1_select(ctx->l1, ctx->d_seqs, h, ids, rows, n, ctx->k, ctx->l1_threshold, sel_idx, sel_score, ctx->sf, &launches, &msg);
+  ctx->index_launches += launches;
+  if (rc != 0) LSA_FAIL(ctx, rc == -1 ? LSA_ERR_INVALID_ARG : LSA_ERR_CUDA, "Level-1 indexer: %s", msg.c_str());
+  return LSA_OK;
+}
+
 extern "C" int lsa_l1_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n, int32_t* sel_idx, float* sel_score) {
   if (!ctx) return LSA_ERR_STATE;
   if (!ctx->l1) LSA_FAIL(ctx, LSA_ERR_STATE, "lsa_l1_init has not been called");
   if (!h || !sel_idx) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null h / sel_idx");
   int rc = check_ids(ctx, seq_ids, n);
   if (rc) return rc;
-  std::string msg;
-  int launches = 0;
-  ProfScope prof(ctx, LSA_PH_INDEX, ctx->sf);
-  rc = l1_select(ctx->l1, ctx->d_seqs, h, seq_ids, n, ctx->k, ctx->l1_threshold, sel_idx, sel_score, ctx->sf, &launches, &msg);
-  ctx->index_launches += launches;
-  if (rc != 0) LSA_FAIL(ctx, rc == -1 ? LSA_ERR_INVALID_ARG : LSA_ERR_CUDA, "Level-1 indexer: %s", msg.c_str());
+  std::vector<int> rows(n);
+  for (int i = 0; i < n; ++i) rows[i] = i;
+  return l1_select_impl(ctx, h, seq_ids, rows.data(), n, sel_idx, sel_score);
+}
+
+extern "C" int lsa_set_indexer(lsa_ctx* ctx, int32_t indexer) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (indexer != LSA_INDEXER_DUAL_ENCODER && indexer != LSA_INDEXER_LEVEL1) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad indexer");
+  if (indexer == LSA_INDEXER_LEVEL1 && !ctx->l1) LSA_FAIL(ctx, LSA_ERR_STATE, "lsa_l1_init has not been called");
+  ctx->indexer = indexer;
   return LSA_OK;
 }
 
@@ -543,7 +558,9 @@ extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* 
   }
   if ((rc = prestep_impl(c, false, k_new, v_new))) return rc;       // (a) + (d)
   if (n_fire) {                                                     // (b)
-    if ((rc = index_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))) return rc;
+    if (c->indexer == LSA_INDEXER_LEVEL1 ? (rc = l1_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))
+                                         : (rc = index_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr)))
+      return rc;
     if ((rc = fetch_impl(c, ids, n_fire, c->d_sel))) return rc;
     if (c->cfg.recall_lag == 0 && (rc = prestep_impl(c, false, nullptr, nullptr))) return rc;   // (c)
   }

@@ -56,13 +56,13 @@ template <> __device__ __forceinline__ __nv_bfloat16 l1_out<__nv_bfloat16>(float
 
 constexpr int kGvWarps = 4, kGvSeqs = 4;
 
-// W bf16 [E][Din]; x [n][ldx] (row i at x + i*ldx); out [n][ldo] (row i at out + i*ldo).
+// W bf16 [E][Din]; x rows of stride ldx (input i is row xrows.ids[i]); out [n][ldo] (row i at out + i*ldo).
 // The block first stages its (up to 4) x rows in shared memory - read from L2 inside the FMA loop they would be
 // 16 dependent round trips per lane - then every warp streams one weight row with all its loads in flight.
 template <typename XT, typename OT>
 __global__ void __launch_bounds__(kGvWarps * 32)
-l1_gemv_kernel(const __nv_bfloat16* __restrict__ W, const XT* __restrict__ x, long long ldx, OT* __restrict__ out, long long ldo,
-               int n, int E, int Din) {
+l1_gemv_kernel(const __nv_bfloat16* __restrict__ W, const XT* __restrict__ x, long long ldx, FireList xrows, OT* __restrict__ out,
+               long long ldo, int n, int E, int Din) {
   extern __shared__ __align__(16) unsigned char gv_smem[];
   XT* xs = reinterpret_cast<XT*>(gv_smem);                 // [kGvSeqs][Din]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -82,7 +82,7 @@ l1_gemv_kernel(const __nv_bfloat16* __restrict__ W, const XT* __restrict__ x, lo
   for (int s = 0; s < kGvSeqs; ++s)
     if (i0 + s < n)
       for (int d = threadIdx.x * kPer16; d < Din; d += kGvWarps * 32 * kPer16)
-        *reinterpret_cast<uint4*>(xs + (size_t)s * Din + d) = *reinterpret_cast<const uint4*>(x + (size_t)(i0 + s) * ldx + d);
+        *reinterpret_cast<uint4*>(xs + (size_t)s * Din + d) = *reinterpret_cast<const uint4*>(x + (size_t)xrows.ids[i0 + s] * ldx + d);
   __syncthreads();
   if (e >= E) return;
   float acc[kGvSeqs];
@@ -411,9 +411,9 @@ void l1_destroy(L1Plan* pl) {
   delete pl;
 }
 
-// h DEVICE [n][Dh] (row i belongs to sequence ids[i]); sel_idx DEVICE [n][k]
-int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, int n, int k, float threshold, int32_t* sel_idx,
-              float* sel_score, cudaStream_t st, int* launches, std::string* msg) {
+// h DEVICE rows of Dh (row hrows[i] belongs to sequence ids[i]); sel_idx DEVICE [n][k]
+int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, const int* hrows, int n, int k, float threshold,
+              int32_t* sel_idx, float* sel_score, cudaStream_t st, int* launches, std::string* msg) {
   const L1Init& in = pl->init;
   const int L = in.n_layers, Dh = in.Dh, d_c = in.d_c;
   const float logit_thr = (float)std::log((double)threshold / (1.0 - (double)threshold));
@@ -421,6 +421,9 @@ int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, i
   for (int off = 0; off < n; off += pl->cap) {
     const int m = std::min(pl->cap, n - off);
     const dim3 blk(kGvWarps * 32);
+    FireList hr{}, ident{};
+    hr.n = ident.n = m;
+    for (int i = 0; i < m; ++i) { hr.ids[i] = hrows[off + i]; ident.ids[i] = i; }
     for (int l = 0; l < L; ++l) {
       const __nv_bfloat16* Wdq = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_dq);
       const __nv_bfloat16* Wiuq = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_iuq);
@@ -428,13 +431,13 @@ int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, i
       float* cq = pl->cq + (size_t)l * pl->cap * d_c;
       // Eq.(1): c^Q [m][d_c] fp32
       L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((d_c + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * Dh * 2, st,
-                         Wdq, hb + (size_t)off * Dh, (long long)Dh, cq, (long long)d_c, m, d_c, Dh));
+                         Wdq, hb, (long long)Dh, hr, cq, (long long)d_c, m, d_c, Dh));
       // Eq.(3): w -> piece (i, l)
       L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((kL1H + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * Dh * 2, st,
-                         Ww, hb + (size_t)off * Dh, (long long)Dh, pl->wbuf + (size_t)l * kL1H, (long long)L * kL1H, m, kL1H, Dh));
+                         Ww, hb, (long long)Dh, hr, pl->wbuf + (size_t)l * kL1H, (long long)L * kL1H, m, kL1H, Dh));
       // Eq.(2): q -> piece (i, l), rounded to bf16
       L1_CUDA(launch_pdl(l1_gemv_kernel<float, __nv_bfloat16>, dim3((kL1H * kL1CI + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * d_c * 4, st,
-                         Wiuq, (const float*)cq, (long long)d_c, pl->q + (size_t)l * kL1H * kL1CI, (long long)L * kL1H * kL1CI, m,
+                         Wiuq, (const float*)cq, (long long)d_c, ident, pl->q + (size_t)l * kL1H * kL1CI, (long long)L * kL1H * kL1CI, m,
                          kL1H * kL1CI, d_c));
       *launches += 3;
     }

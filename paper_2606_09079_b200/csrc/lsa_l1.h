@@ -25,8 +25,8 @@ struct L1Init {
 
 bool l1_supported(int dtype, int C, int c_I, int n_h);
 int l1_create(const L1Init& init, L1Plan** out, std::string* msg);     // 0 or an lsa_status
-int l1_select(L1Plan* plan, const SeqDev* d_seqs, const void* h, const int* ids, int n, int k, float threshold, int32_t* sel_idx,
-              float* sel_score, cudaStream_t st, int* launches, std::string* msg);
+int l1_select(L1Plan* plan, const SeqDev* d_seqs, const void* h, const int* ids, const int* hrows, int n, int k, float threshold,
+              int32_t* sel_idx, float* sel_score, cudaStream_t st, int* launches, std::string* msg);
 void l1_destroy(L1Plan* plan);
 
 }  // namespace lsa

@@ -24,6 +24,7 @@ LSA_F32, LSA_BF16 = 0, 1
 LSA_ATTN_AUTO, LSA_ATTN_SIMT, LSA_ATTN_TCGEN05 = 0, 1, 2
 LSA_FETCH_DEVICE_PULL, LSA_FETCH_MEMCPY = 0, 1
 LSA_MERGE_AUTO, LSA_MERGE_KERNEL, LSA_MERGE_FUSED = 0, 1, 2
+LSA_INDEXER_DUAL_ENCODER, LSA_INDEXER_LEVEL1 = 0, 1
 
 STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_ERR_POOL_EXHAUSTED",
           -4: "LSA_ERR_OOM", -5: "LSA_ERR_STATE", -6: "LSA_ERR_UNSUPPORTED"}
@@ -31,7 +32,7 @@ STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_E
 EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit_tables",
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
-           "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select",
+           "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
            "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
@@ -96,6 +97,7 @@ def _load() -> C.CDLL:
     lib.lsa_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     lib.lsa_l1_init.argtypes = [vp, C.POINTER(lsa_l1_config), C.POINTER(vp)]
     lib.lsa_l1_select.argtypes = [vp, vp, i32p, C.c_int32, vp, f32p]
+    lib.lsa_set_indexer.argtypes = [vp, C.c_int32]
     lib.lsa_last_error.argtypes = [vp]
     lib.lsa_last_error.restype = C.c_char_p
     lib.lsa_destroy.argtypes = [vp]
@@ -238,6 +240,9 @@ class LsaContext:
                 ptrs[b * L + l] = _dev_ptr(t, self.tdtype, "index_k") if t is not None and t.numel() else None
         self._keep += [list(layers), [list(x) for x in index_k]]
         self._check(_lib.lsa_l1_init(self._h, C.byref(cfg), ptrs))
+
+    def set_indexer(self, indexer: int):
+        self._check(_lib.lsa_set_indexer(self._h, indexer))
 
     def l1_select(self, h: torch.Tensor, seq_ids: Sequence[int], want_scores: bool = True):
         arr, n = _ids(seq_ids)

@@ -90,7 +90,7 @@ def attn_tolerance(dtype: str):
 
 
 def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=None, with_kv_new: bool = True,
-                 tie_emb_builder=None):
+                 tie_emb_builder=None, l1=None, l1_band: float = 3e-2):
     """Drive lsa_step and the oracle in lock-step: validate the GPU's
     selection against the oracle's scores, feed it to the oracle's residency model, then compare page
     tables / residency / fetched bytes bit-exactly and attention outputs within tolerance."""
@@ -112,11 +112,17 @@ def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=
         for b in firing:                      # GPU selection = chunk ids of the table it just staged
             which = 0 if c.recall_lag == 0 else 1
             chunks, pages = rig.ctx.page_table(b, which)
-            sc = orc.scores(b, h[b])
-            order = sorted(chunks, key=lambda ch: (-sc[ch], ch))
             import numpy as _np
-            padded = _np.full(c.k, -1, dtype=_np.int64); padded[: len(order)] = order
-            msg = validate_selection(padded, sc, c.k)
+            if l1 is not None:            # paper-exact Level-1 indexer drives the step (lsa_set_indexer)
+                from oracle.l1_oracle import l1_index_select, validate_l1_selection
+                _, _, cs, _ = l1_index_select(h[b], l1.layers, l1.index_k[b], l1.n_h, c.C, c.k)
+                padded = _np.full(c.k, -1, dtype=_np.int64); padded[: len(chunks)] = chunks
+                msg = validate_l1_selection(padded, cs, c.k, 0.5, l1_band)
+            else:
+                sc = orc.scores(b, h[b])
+                order = sorted(chunks, key=lambda ch: (-sc[ch], ch))
+                padded = _np.full(c.k, -1, dtype=_np.int64); padded[: len(order)] = order
+                msg = validate_selection(padded, sc, c.k)
             assert msg is None, f"step {t} seq {b}: {msg}"
             forced[b] = chunks
         orc.step_begin(h, forced_selection=forced if firing else None)

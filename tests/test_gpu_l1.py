@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 import torch
 
-from lsa_harness import GpuRig
+from lsa_harness import GpuRig, run_lockstep
 from oracle.l1_oracle import l1_index_select, validate_l1_selection
 from paper_2606_09079_b200.workloads import L1Inputs, LsaWorkload, make_small_config, to_torch
 
@@ -63,6 +63,21 @@ def test_l1_select_matches_oracle(k, n_layers):
         hot = rig.hot_pool.cpu()
         for c_, p_ in zip(chunks, pages):
             assert torch.equal(hot[p_], rig.cold[b][c_])
+    rig.ctx.close()
+
+
+def test_lsa_step_with_level1_indexer_lockstep():
+    """lsa_set_indexer(LEVEL1): the paper-exact indexer drives lsa_step (trigger -> Eq.1-5,13 -> residency ->
+    fetch -> attention).  The GPU's selection is validated against the L1 oracle, then page tables, residency,
+    counters, fetched bytes (bit-exact) and attention outputs (BASELINE tolerance) are checked in lock-step."""
+    from paper_2606_09079_b200 import lsa
+    cfg = make_small_config("bf16", B=3, L=[20096, 4992, 512], C=128, H=8, D=64, Dh=512, E=64, k=10, hot_pages=64, W=64, tau=4, steps=14)
+    wl, l1, rig = _rig(cfg, 2, 128)
+    rig.ctx.set_indexer(lsa.LSA_INDEXER_LEVEL1)
+    r = run_lockstep(wl, rig, cfg.steps, l1=l1)
+    assert r["checked"] == cfg.steps
+    st = rig.ctx.stats()
+    assert st["misses"] > 0 and st["hits"] > 0            # h drifts slowly: later triggers mostly hit
     rig.ctx.close()
 
 
