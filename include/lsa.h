@@ -25,6 +25,9 @@
  *   - Row-major, innermost dimension contiguous, no padding, 16-byte aligned base pointers.
  *   - The five path calls only ENQUEUE work on the caller's two streams and return; they never
  *     block the host.  lsa_sync / lsa_get_* / lsa_step_host block.
+ *   - Stream order is the caller's contract for its own buffers: q, k_new, v_new and out are read / written
+ *     on stream_compute, h and sel_idx on stream_fetch; whatever produces them must be ordered before the
+ *     call on that stream (lsa_step_host does this itself for its staging copies).
  *   - Not thread-safe per context.
  */
 #ifndef LSA_H_
@@ -160,9 +163,10 @@ int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, float* lse);
 int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
              void* out);
 
-/* lsa_step with HOST buffers: packs q, k_new, v_new (and h, at trigger steps only) into one pinned staging
- * image, copies it host->device in ONE transfer, runs the step, copies out device->host (pinned `out`
- * recommended) and blocks until it has landed.  Used for end-to-end timing. */
+/* lsa_step with HOST buffers.  Pinned + mapped inputs (e.g. torch pin_memory) are pulled over the host link by
+ * one small kernel and a pinned `out` is written in place by S8; pageable buffers go through one packed
+ * host->device copy and one device->host copy.  h is only read at trigger steps.  Blocks until the result
+ * has landed.  Used for end-to-end timing. */
 int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new,
                   const void* v_new, void* out);
 

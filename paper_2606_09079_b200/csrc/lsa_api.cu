@@ -11,6 +11,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/lsa.h"
@@ -58,6 +59,7 @@ struct lsa_ctx {
   // host-buffer staging (lsa_step_host)
   void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
   const void* out_host_cached = nullptr;
+  std::vector<std::pair<const void*, void*>> alias_cache;   // host pointer -> device alias (or null)
   void* out_dev_alias = nullptr;
   // optional per-phase event timing
   int prof_cap = 0;
@@ -570,6 +572,33 @@ extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* 
   return LSA_OK;
 }
 
+// lsa_step_host: one launch pulls the step's inputs out of pinned, mapped host buffers (16-byte loads over the
+// host link) into the device staging area - no CPU-side packing, no copy-engine operation in the chain.
+struct HostGather {
+  const uint4* src[4];
+  uint4* dst[4];
+  unsigned n16[4];     // 16-byte units per part (0 = absent)
+};
+__global__ void __launch_bounds__(256) host_gather_kernel(HostGather g) {
+  const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+    for (unsigned i = tid; i < g.n16[p]; i += nthr) g.dst[p][i] = g.src[p][i];
+}
+
+// device alias of a pinned + mapped host pointer, or null (cached: the attribute query costs about a microsecond)
+static void* host_alias(lsa_ctx* c, const void* p) {
+  if (!p) return nullptr;
+  for (const auto& e : c->alias_cache) if (e.first == p) return e.second;
+  cudaPointerAttributes at{};
+  void* d = nullptr;
+  if (cudaPointerGetAttributes(&at, p) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer) d = at.devicePointer;
+  else cudaGetLastError();
+  if (c->alias_cache.size() >= 256) c->alias_cache.clear();
+  c->alias_cache.emplace_back(p, d);
+  return d;
+}
+
 extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
   if (!ctx) return LSA_ERR_STATE;
   lsa_ctx* c = ctx;
@@ -591,12 +620,33 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
   bool fire = false;
   for (int b = 0; b < c->B; ++b) fire |= (c->step[b] % cfg.tau == 0);
   if (fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
-  unsigned char* pin = static_cast<unsigned char*>(c->st_pin);
-  memcpy(pin, q, qb);
-  size_t upto = qb;
-  if (k_new) { memcpy(pin + o_kn, k_new, nb); memcpy(pin + o_vn, v_new, nb); upto = o_vn + nb; }
-  if (fire) { memcpy(pin + o_h, h, hb); upto = o_h + hb; }          // h is only read at trigger steps
-  LSA_CUDA(c, cudaMemcpyAsync(c->st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
+  void* aq = host_alias(c, q);
+  void* akn = k_new ? host_alias(c, k_new) : nullptr;
+  void* avn = v_new ? host_alias(c, v_new) : nullptr;
+  void* ah = fire ? host_alias(c, h) : nullptr;
+  if (aq && (!k_new || (akn && avn)) && (!fire || ah) && qb % 16 == 0 && nb % 16 == 0 && hb % 16 == 0) {
+    HostGather g{};
+    g.src[0] = (const uint4*)aq; g.dst[0] = (uint4*)c->st_q; g.n16[0] = (unsigned)(qb / 16);
+    if (k_new) {
+      g.src[1] = (const uint4*)akn; g.dst[1] = (uint4*)c->st_kn; g.n16[1] = (unsigned)(nb / 16);
+      g.src[2] = (const uint4*)avn; g.dst[2] = (uint4*)c->st_vn; g.n16[2] = (unsigned)(nb / 16);
+    }
+    if (fire) { g.src[3] = (const uint4*)ah; g.dst[3] = (uint4*)c->st_h; g.n16[3] = (unsigned)(hb / 16); }
+    const unsigned total = g.n16[0] + g.n16[1] + g.n16[2] + g.n16[3];
+    host_gather_kernel<<<std::max(1u, std::min(64u, (total + 255u) / 256u)), 256, 0, c->sc>>>(g);
+    LSA_CUDA(c, cudaGetLastError());
+  } else {                         // pageable inputs: pack into the pinned staging image, one host-to-device copy
+    unsigned char* pin = static_cast<unsigned char*>(c->st_pin);
+    memcpy(pin, q, qb);
+    size_t upto = qb;
+    if (k_new) { memcpy(pin + o_kn, k_new, nb); memcpy(pin + o_vn, v_new, nb); upto = o_vn + nb; }
+    if (fire) { memcpy(pin + o_h, h, hb); upto = o_h + hb; }          // h is only read at trigger steps
+    LSA_CUDA(c, cudaMemcpyAsync(c->st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
+  }
+  if (fire) {                      // the indexer reads the staged h on the fetch stream: order it behind the copy
+    LSA_CUDA(c, cudaEventRecord(c->ev_compute, c->sc));
+    LSA_CUDA(c, cudaStreamWaitEvent(c->sf, c->ev_compute, 0));
+  }
   // result: if `out` is pinned and mapped, S8 writes it in place over the host link (no device-to-host copy
   // operation in the chain); otherwise through a device buffer and one copy
   if (out != c->out_host_cached) {

@@ -324,8 +324,8 @@ def test_flagship_shape_growing_window_and_ring_wrap(merge):
 
 @pytest.mark.parametrize("pinned_out", [True, False])
 def test_step_host_equals_step(pinned_out):
-    """lsa_step_host (host buffers: one packed H2D copy, result written in place when `out` is pinned and
-    mapped, else one D2H copy) gives bit-identical outputs, page tables and counters to lsa_step."""
+    """lsa_step_host gives bit-identical outputs, page tables and counters to lsa_step, with pinned buffers
+    (inputs pulled by a gather kernel, result written in place) and pageable ones (packed copy in, copy out)."""
     lsa = _lsa()
     cfg = make_config(2, B=2, L=[16384 + 4 * 37, 8192], W=1024, k=6, hot_pages=32, steps=40, name="cfg2_host", q_gain=16.0, tau=8)
     wl = LsaWorkload(cfg)
@@ -338,7 +338,7 @@ def test_step_host_equals_step(pinned_out):
         kn, vn = wl.kv_new(t)
         ref = a.ctx.step(a.dev(q), a.dev(h), a.dev(kn), a.dev(vn))
         a.ctx.sync()
-        to_h = lambda x: to_torch(x, cfg.dtype).pin_memory()
+        to_h = (lambda x: to_torch(x, cfg.dtype).pin_memory()) if pinned_out else (lambda x: to_torch(x, cfg.dtype))
         b_.ctx.step_host(to_h(q), to_h(h) if t % 2 == 0 or t % cfg.tau == 0 else None, to_h(kn), to_h(vn), out_h)
         assert torch.equal(ref.cpu(), out_h), f"step {t}"
     for s_ in range(cfg.B):
