@@ -118,7 +118,7 @@ class Replica:
         self.ctx = lsa.LsaContext(dtype=lsa.LSA_F32 if c.dtype == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W,
                                   Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=shared["W_q"], seqs=seqs,
                                   recall_lag=c.recall_lag, stream_compute=sc, stream_fetch=sf,
-                                  attn_impl=shared["attn_impl"])
+                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0))
         self.step = 0
 
 
@@ -182,6 +182,7 @@ def main():
     ap.add_argument("--attn", default="auto", choices=["auto", "simt", "tcgen05"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", type=int, default=0)
+    ap.add_argument("--max-ctas", type=int, default=0, help="cap on attention CTAs (0 = library default)")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -214,7 +215,7 @@ def main():
     warmup = max(args.warmup, 3, 2 * R)
     attn_impl = dict(auto=lsa.LSA_ATTN_AUTO, simt=lsa.LSA_ATTN_SIMT, tcgen05=lsa.LSA_ATTN_TCGEN05)[args.attn]
 
-    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, W_q=to_torch(wl.W_q, c.dtype).to(dev),
+    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, max_ctas=args.max_ctas, W_q=to_torch(wl.W_q, c.dtype).to(dev),
                   cold=[to_torch(x, c.dtype).pin_memory() for x in wl.cold_csa],
                   emb=[to_torch(wl.chunk_emb(b, 0), c.dtype).to(dev) for b in range(c.B)],
                   hca_k=[to_torch(x, c.dtype).to(dev) for x in wl.hca_k], hca_v=[to_torch(x, c.dtype).to(dev) for x in wl.hca_v],

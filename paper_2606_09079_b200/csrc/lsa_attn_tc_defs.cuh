@@ -17,8 +17,10 @@
 // Work unit: a TILE = 128 consecutive rows of one tensor (HCA rows [128j, 128j+128), one page of the
 // current table, window rows [128j, ...)), so every TMA box is one 32 KiB [2 d-blocks][128 rows][128 B]
 // image (3-D tensor map: 64 columns x rows x 8 d-blocks).  The flat tile list of the batch (per sequence:
-// HCA tiles, pages in table order, window tiles) is cut into gridDim.x contiguous ranges; a CTA emits one
-// (m, l, o) partial per sequence it touches and lsa_combine_tc merges them (S8).
+// HCA tiles, pages in table order, window tiles) is cut into n_attn contiguous ranges (n_attn <= SM count,
+// chosen so every CTA gets the same number of whole tiles); a CTA emits one (m, l, o) partial per sequence it
+// touches and a combine kernel (lsa_attn_tc.cu) merges them (S8).  S6 and the window append ride on the launch
+// on steps without a trigger (make_view / commit_state below).
 //   warp 0    : TMA producer  - Q tile (one 64 KiB box), then K/V stages (4-deep ring of 32 KiB)
 //   warp 1    : MMA issuer    - one elected thread issues tcgen05.mma / tcgen05.commit
 //   warps 2-9 : softmax       - thread <-> (key, half of the heads): TMEM -> regs, masked scale,
@@ -101,10 +103,6 @@ struct TcParams {
   unsigned long long* tlog;      // [0] = entries; then (kernel id, globaltimer start, end) per launch of block 0
 #endif
 };
-
-__host__ __device__ __forceinline__ int tc_tiles(int n_hca, int n_cur, int w_len) {
-  return (n_hca + kTcTile - 1) / kTcTile + n_cur + (w_len + kTcTile - 1) / kTcTile;
-}
 
 __device__ __forceinline__ SeqView make_view(const TcParams& p, int b) {
   const SeqDev& s = p.seqs[b];
