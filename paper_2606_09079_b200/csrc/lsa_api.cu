@@ -257,7 +257,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
     ti.B = B; ti.k = k; ti.W = cfg->W; ti.P = P; ti.n_sms = c->n_sms; ti.max_ctas = cfg->max_ctas;
     ti.fuse_combine = cfg->merge_mode == LSA_MERGE_FUSED ? 1 : 0;
     ti.hot_pool = cfg->hot_pool; ti.seq_host = c->seq_host.data(); ti.d_seqs = c->d_seqs; ti.pool = c->pool;
-    ti.sm_scale = c->sm_scale;
+    ti.sm_scale = c->sm_scale; ti.stream = c->sc;
     std::string msg;
     int trc = tc_create(ti, &c->tc, &msg);
     if (trc != 0) LSA_FAIL(c, trc, "tcgen05 attention init failed: %s", msg.c_str());

@@ -18,6 +18,7 @@ struct TcInit {
   SeqDev* d_seqs;
   PoolDev pool;
   float sm_scale;
+  cudaStream_t stream;      // compute stream of the context: contexts of one stream share the split-K workspace
 };
 
 // bf16, H = 64 query heads sharing one K/V of D = 512, pages of C = 128 rows (BASELINE cfg 2-5)

@@ -284,6 +284,57 @@ def test_tcgen05_attention_edge_cases(max_ctas, keep, merge):
     ctx.close()
 
 
+@pytest.mark.parametrize("merge", ["kernel", "fused"])
+def test_tcgen05_contexts_of_one_stream_share_the_workspace(merge):
+    """Contexts on the same compute stream share the split-K workspace (lsa_attn_tc.cu): launches of three
+    contexts with different batch sizes and key counts, interleaved back to back without a host sync, must each
+    match the oracle - also after one of them was closed while the others keep running."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 256
+    g = torch.Generator().manual_seed(11)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    st = torch.cuda.Stream(dev)
+    shapes = [[1500, 700], [3000], [130, 0, 900, 257, 64]]          # HCA rows per sequence, per context
+    rigs = []
+    for n_rows in shapes:
+        B = len(n_rows)
+        hk, hv = [rnd(n, D) for n in n_rows], [rnd(n, D) for n in n_rows]
+        wk, wv = [rnd(W, D) for _ in range(B)], [rnd(W, D) for _ in range(B)]
+        w_len = [(37 * (b + 1)) % W for b in range(B)]
+        ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.05, attn_impl=lsa.LSA_ATTN_TCGEN05,
+                          stream_compute=st, merge_mode=lsa.LSA_MERGE_FUSED if merge == "fused" else lsa.LSA_MERGE_KERNEL)
+        rigs.append(dict(ctx=ctx, hk=hk, hv=hv, wk=wk, wv=wv, w_len=w_len, q=rnd(B, H, D),
+                         out=torch.empty((B, H, D), dtype=torch.bfloat16, device=dev)))
+    tol = attn_tolerance("bf16")
+    torch.cuda.synchronize()
+
+    def check(r):
+        out64 = r["out"].double().cpu().numpy()
+        for b in range(len(r["hk"])):
+            K = np.concatenate([r["hk"][b].double().cpu().numpy(), r["wk"][b][: r["w_len"][b]].double().cpu().numpy()])
+            V = np.concatenate([r["hv"][b].double().cpu().numpy(), r["wv"][b][: r["w_len"][b]].double().cpu().numpy()])
+            ref, _, _ = attention(r["q"][b].double().cpu().numpy(), K, V, 0.05)
+            np.testing.assert_allclose(out64[b], ref, **tol)
+
+    for rep in range(4):
+        for r in rigs:
+            r["ctx"].decode_attention(r["q"], r["out"])
+    st.synchronize()
+    for r in rigs:
+        check(r)
+    rigs[0]["ctx"].close()                      # the first context created the workspace; the others keep it alive
+    for rep in range(3):
+        for r in rigs[1:]:
+            with torch.cuda.stream(st):
+                r["out"].zero_()
+            r["ctx"].decode_attention(r["q"], r["out"])
+    st.synchronize()
+    for r in rigs[1:]:
+        check(r)
+        r["ctx"].close()
+
+
 @pytest.mark.parametrize("impl", ["simt", "tcgen05", "tcgen05_merge_fused"])
 def test_flagship_shape_short_context_both_impls(impl):
     """bf16 H=64 D=512 C=128 at a short context, with a partial last chunk, through both kernels; the
