@@ -269,11 +269,12 @@ def main():
         for i in range(n):
             one_step(i0 + i, host)
         e1.record(sc)
+        enq = time.perf_counter() - w0                      # host time to enqueue the n steps (no waiting)
         sf.synchronize(); sc.synchronize()
         wall = time.perf_counter() - w0
         barrier()
         ms = max_over_ranks(e0.elapsed_time(e1), dev)       # the job's time = the slowest rank's
-        return ms, wall
+        return ms, wall, enq
 
     # ---- warm-up, then the device-resident timed region ----
     samp, sampf = clocks_sampler_start(local_rank)
@@ -282,7 +283,7 @@ def main():
     i_next = warmup
     launches0 = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps)
     t_begin = time.perf_counter()
-    ms, wall = timed(args.steps, i0=i_next)
+    ms, wall, enq = timed(args.steps, i0=i_next)
     t_end = time.perf_counter()
     clocks = clocks_sampler_stop(samp, sampf, t_begin, t_end)
     i_next += args.steps
@@ -297,7 +298,7 @@ def main():
         one_step(i_next + i, host)
     i_next += max(3, R)
     n_e2e = max(64, args.steps // 4)
-    ms_e2e, _ = timed(n_e2e, host, i0=i_next)
+    ms_e2e, _, enq_e2e = timed(n_e2e, host, i0=i_next)
     i_next += n_e2e
     es = 4 if c.dtype == "f32" else 2
     h2d = (c.B * c.H * c.D + 2 * c.B * c.D) * es + c.B * c.Dh * es // c.tau     # h crosses only at trigger steps (1 in tau)
@@ -415,7 +416,8 @@ def main():
                              ms_per_step=ms_e2e / n_e2e),
                     gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, l1_indexer=l1, wall_s=wall,
+                    fetch=fetch, l1_indexer=l1, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
+                    host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
         print(json.dumps(line))
     if world > 1:

@@ -10,25 +10,37 @@ namespace lsa {
 
 // ---- S8: merge the split partials of one sequence  ----------------------------------------------
 //   m* = max m_i ; l* = sum l_i 2^(m_i-m*) ; out = sum o_i 2^(m_i-m*) / l* ; lse = ln2 (m* + log2 l*)
-// Partials are stored as [d-block m][head half][head quad g][d_local 128][4 heads] (the order the
-// attention epilogue drains TMEM in).  grid (128, B): block = (m, half, g, 64 of the 128 d); 512 threads =
-// 64 d x 8 groups, group j accumulates partials j, j+8, ... with one float4 (4 heads) per thread, 1 KiB
-// contiguous per partial per group.  Launched with programmatic stream serialization: the launch and
-// prologue overlap the attention kernel's tail.
+// Partials are stored as [d-block m][head half][head quad g][d_local 128][4 heads] fp16 with one power-of-two
+// scale per (m, half, 32 d) block (lsa_attn_tc_defs.cuh, "split-K partial format") - the order the attention
+// epilogue drains TMEM in.  grid (128, B): block = (m, half, g, 64 of the 128 d), i.e. 512 contiguous bytes of
+// every slot; 512 threads = 64 d x 8 groups, group j accumulates partials j, j+8, ... (4 heads per thread).
+// Launched with programmatic stream serialization: the launch and prologue overlap the attention kernel's tail.
 constexpr int kCombineThreads = 512;
 // The combine grid is launched while attention CTAs still own most SMs (PDL).  Asking for more than half an
 // SM's shared memory keeps its blocks at one per SM, so the early ones cannot pile up on the few idle SMs.
 constexpr int kCombineSmemPad = 116 * 1024;
+constexpr int kCombineSmemMax = 128 * 1024;        // landing buffer of 256 slots x 512 B
 
-// For B <= kCombineSpecMaxB nearly every CTA holds a piece of every sequence: the partial loads of all n_cta
-// slots are issued before anything is known about them, together with the loads of piece_info, m and l, so
-// the kernel is ONE memory round trip deep; slots that turn out to be inactive are discarded (selected away,
-// never multiplied).  Larger batches use combine_tc_wide_kernel below.
+// For B <= kCombineSpecMaxB nearly every CTA holds a piece of every sequence: the copies of all n_cta slots are
+// issued before anything is known about them, together with the loads of piece_info, m, l and the scales, so the
+// kernel is ONE memory round trip deep; slots that turn out to be inactive are discarded (selected away, never
+// multiplied).  Larger batches use combine_tc_wide_kernel below.
 constexpr int kCombineSpecMaxB = 4;
 
+// The partials themselves come in by TMA: one 2-D box = the block's 512 bytes of kCombRows consecutive slots, so
+// the whole read is n_cta / 32 bulk copies issued by one thread of a warp that has nothing else to wait for,
+// landing in shared memory behind one mbarrier, instead of 16 loads per thread queued in the LSU.
+constexpr int kCombRows = 32;                     // slots per TMA box
+constexpr int kCombRowBytes = 512;                // (m, hh, g, half of d): 64 d x 4 heads fp16
+constexpr int kCombBoxBytes = kCombRows * kCombRowBytes;
+
 __global__ void __launch_bounds__(kCombineThreads, 1)
-combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
+combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int n_cta, __nv_bfloat16* __restrict__ out,
+                  float* __restrict__ lse) {
+  extern __shared__ __align__(128) unsigned char comb_rows[];   // [slot row][512 B]
+  __shared__ __align__(8) uint64_t bar;
   __shared__ float4 w_s[256];
+  __shared__ float2 sc_s[256];
   __shared__ int slot_s[256];
   __shared__ float4 red_f[16];
   __shared__ int warp_cnt[16];
@@ -37,16 +49,28 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   const int dh = blockIdx.x & 1, g = (blockIdx.x >> 1) & 7, hh = (blockIdx.x >> 4) & 1, m = blockIdx.x >> 5, b = blockIdx.y;
   const int h0 = hh * 32 + g * 4;
   const int dl = tid & 63, grp = tid >> 6;
-  const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dh * 64 + dl;
-  constexpr int U = 16;                           // independent 16-byte loads in flight per thread
 #ifdef LSA_TC_TRACE
   const unsigned long long g_entry = gtime();
 #endif
+  const int n_box = (n_cta + kCombRows - 1) / kCombRows;
+  if (tid == 0) {
+    mbar_init(&bar, 1);
+    fence_mbar_init();
+    prefetch_tmap(&map_part);
+  }
+  __syncthreads();
   griddep_wait();                                 // partials and piece_info are final from here on
   griddep_launch_dependents();                    // the next kernel in the stream may start its own prologue
 #ifdef LSA_TC_TRACE
   const unsigned long long g_dep = gtime();
+  const long long c_dep = clock64();
 #endif
+  if (tid == kCombineThreads - 32) {              // rows b .. b + 32 n_box - 1 of column block (m, hh, g, dh); a warp
+                                                  // that has no small loads to wait for issues the copies
+    mbar_arrive_expect_tx(&bar, (uint32_t)(n_box * kCombBoxBytes));
+    for (int i = 0; i < n_box; ++i)
+      tma_load_2d(comb_rows + i * kCombBoxBytes, &map_part, (((m * 2 + hh) * 8 + g) * 2 + dh) * (kCombRowBytes / 4), b + i * kCombRows, &bar);
+  }
   if (blockIdx.x == 0 && tid == 0) commit_state(p, b);   // S6 / window append folded into the attention launch
   // thread c < n_cta looks at CTA c: did it write a partial for sequence b?  (n_cta <= 256)
   // These small loads go first so that they are not queued behind the bulk of partial loads below.
@@ -55,21 +79,21 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   const size_t slot = (size_t)tid + b;
   int2 info = make_int2(0, 0);
   float4 m4 = mi, l4 = li;
+  float2 s2 = make_float2(0.f, 0.f);              // scales of this CTA's two lane quarters (d = dh*64 + 0..31 / 32..63)
   if (tid < n_cta) {
     info = __ldcg(p.piece_info + tid);
     m4 = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
     l4 = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
-  }
-  float4 v[U];
-#pragma unroll
-  for (int j = 0; j < U; ++j) {
-    const int c = grp + 8 * j;
-    v[j] = c < n_cta ? __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    s2 = __ldcg(reinterpret_cast<const float2*>(p.part_s + part_scale_idx(slot, m, hh, dh * 2)));
   }
   if (tid < n_cta) {
-    active = info.x <= b && b < info.x + info.y;
+    // a piece without valid keys (m = -inf for every head) wrote no O: its slot is skipped like an inactive one
+    active = info.x <= b && b < info.x + info.y && m4.x != -INFINITY;
     if (active) { mi = m4; li = l4; }
   }
+#ifdef LSA_TC_TRACE
+  const long long c_small = mi.x > 1e30f ? 0ll : clock64();   // after the small loads have returned (thread 0)
+#endif
   float4 mmax = mi;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -96,7 +120,7 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
     wi.z = mi.z == -INFINITY ? 0.f : exp2f(mi.z - m_star.z);
     wi.w = mi.w == -INFINITY ? 0.f : exp2f(mi.w - m_star.w);
   }
-  if (tid < 256) { w_s[tid] = wi; slot_s[tid] = active ? 1 : 0; }   // weights by CTA index; slot_s marks active slots
+  if (tid < 256) { w_s[tid] = wi; sc_s[tid] = s2; slot_s[tid] = active ? 1 : 0; }   // by CTA index; slot_s marks active slots
   float4 lsum = make_float4(wi.x * li.x, wi.y * li.y, wi.z * li.z, wi.w * li.w);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -114,30 +138,30 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
     l_star.x += r.x; l_star.y += r.y; l_star.z += r.z; l_star.w += r.w;
   }
 #ifdef LSA_TC_TRACE
-  const unsigned long long g_w = gtime();
+  const long long c_w = clock64();
 #endif
-  // ---- weighted sum of the partials ----
+  // ---- weighted sum of the partials (row c of the landing buffer = slot b + c = CTA c) ----
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  mbar_wait(&bar, 0, 40);
+#ifdef LSA_TC_TRACE
+  const long long c_land = clock64();
+#endif
   {
-#pragma unroll
-    for (int j = 0; j < U; ++j) {
-      const int c = grp + 8 * j;
-      if (c < n_cta && slot_s[c]) {
-        const float4 w = w_s[c];
-        acc.x = fmaf(w.x, v[j].x, acc.x); acc.y = fmaf(w.y, v[j].y, acc.y);
-        acc.z = fmaf(w.z, v[j].z, acc.z); acc.w = fmaf(w.w, v[j].w, acc.w);
-      }
-    }
-    for (int c = grp + 8 * U; c < n_cta; c += 8) {  // more than 8*U CTAs
+    const uint2* rows = reinterpret_cast<const uint2*>(comb_rows) + dl;
+#pragma unroll 4
+    for (int c = grp; c < n_cta; c += 8) {
       if (slot_s[c]) {
         const float4 w = w_s[c];
-        const float4 x = __ldcg(po + (size_t)(c + b) * (kTcH * kTcD / 4));
-        acc.x = fmaf(w.x, x.x, acc.x); acc.y = fmaf(w.y, x.y, acc.y); acc.z = fmaf(w.z, x.z, acc.z); acc.w = fmaf(w.w, x.w, acc.w);
+        const float sc = dl < 32 ? sc_s[c].x : sc_s[c].y;
+        const uint2 x = rows[c * (kCombRowBytes / 8)];
+        const float2 a01 = unpack_f16x2(x.x), a23 = unpack_f16x2(x.y);
+        acc.x = fmaf(w.x * sc, a01.x, acc.x); acc.y = fmaf(w.y * sc, a01.y, acc.y);
+        acc.z = fmaf(w.z * sc, a23.x, acc.z); acc.w = fmaf(w.w * sc, a23.y, acc.w);
       }
     }
   }
 #ifdef LSA_TC_TRACE
-  const unsigned long long g_l = gtime();
+  const long long c_l = clock64();
 #endif
   acc_s[grp][dl] = acc;
   __syncthreads();
@@ -152,7 +176,12 @@ combine_tc_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, float*
   }
 #ifdef LSA_TC_TRACE
   __syncthreads();
-  if (tid == 0 && blockIdx.x == 0 && b == 0) { tlog_add(p.tlog, 3, g_entry); tlog_add(p.tlog, 4, g_dep); tlog_add(p.tlog, 6, g_w); tlog_add(p.tlog, 7, g_l); }
+  if (tid == 0 && blockIdx.x == 0 && b == 0) {
+    const long long c_end = clock64();
+    tlog_add(p.tlog, 3, g_entry); tlog_add(p.tlog, 4, g_dep);
+    tlog_pair(p.tlog, 8, 0, c_small - c_dep); tlog_pair(p.tlog, 6, 0, c_w - c_dep); tlog_pair(p.tlog, 9, 0, c_land - c_dep);
+    tlog_pair(p.tlog, 7, 0, c_l - c_dep); tlog_pair(p.tlog, 10, 0, c_end - c_dep);
+  }
   if (tid == 0 && blockIdx.x == gridDim.x - 1 && b == 0) tlog_add(p.tlog, 5, g_dep);
 #endif
   if (lse && m == 0 && dh == 0 && tid < 4) {
@@ -187,6 +216,7 @@ combine_tc_wide_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, f
     if (active) {
       mi = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
       li = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
+      active = mi.x != -INFINITY;                 // a piece without valid keys wrote no O: skip its slot
     }
   }
   float4 mmax = mi;
@@ -234,21 +264,26 @@ combine_tc_wide_kernel(TcParams p, int n_cta, __nv_bfloat16* __restrict__ out, f
     const float4 r = red_f[w];
     l_star.x += r.x; l_star.y += r.y; l_star.z += r.z; l_star.w += r.w;
   }
-  const float4* po = reinterpret_cast<const float4*>(p.part_o) + (size_t)((m * 2 + hh) * 8 + g) * 128 + dl;
+  const uint2* po = p.part_o + (size_t)((m * 2 + hh) * 8 + g) * 128 + dl;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   constexpr int U = 8;
   for (int i0 = 0; i0 < n_act; i0 += U) {
-    float4 v[U], w[U];
+    uint2 v[U];
+    float4 w[U];
+    float sc[U];
 #pragma unroll
     for (int j = 0; j < U; ++j) {
       const bool ok = i0 + j < n_act;
+      const int sl = ok ? slot_s[i0 + j] : 0;
       w[j] = ok ? w_s[i0 + j] : make_float4(0.f, 0.f, 0.f, 0.f);
-      v[j] = ok ? __ldcg(po + (size_t)slot_s[i0 + j] * (kTcH * kTcD / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      v[j] = ok ? __ldcg(po + (size_t)sl * (kTcH * kTcD / 4)) : make_uint2(0u, 0u);
+      sc[j] = ok ? __ldcg(p.part_s + part_scale_idx(sl, m, hh, dl >> 5)) : 0.f;   // the same word for a whole warp
     }
 #pragma unroll
     for (int j = 0; j < U; ++j) {
-      acc.x = fmaf(w[j].x, v[j].x, acc.x); acc.y = fmaf(w[j].y, v[j].y, acc.y);
-      acc.z = fmaf(w[j].z, v[j].z, acc.z); acc.w = fmaf(w[j].w, v[j].w, acc.w);
+      const float2 a01 = unpack_f16x2(v[j].x), a23 = unpack_f16x2(v[j].y);
+      acc.x = fmaf(w[j].x * sc[j], a01.x, acc.x); acc.y = fmaf(w[j].y * sc[j], a01.y, acc.y);
+      acc.z = fmaf(w[j].z * sc[j], a23.x, acc.z); acc.w = fmaf(w[j].w * sc[j], a23.y, acc.w);
     }
   }
   __nv_bfloat16* o = out + ((size_t)b * kTcH + h0) * kTcD + m * 128 + dl;
@@ -273,7 +308,7 @@ struct TcWorkspace;
 struct TcPlan {
   TcInit init{};
   EncodeTiledFn encode = nullptr;
-  CUtensorMap map_pool{}, map_q{};
+  CUtensorMap map_pool{}, map_q{}, map_part{};
   const void* q_cached = nullptr;
   CUtensorMap* d_maps = nullptr;
   TcParams params{};
@@ -296,14 +331,15 @@ struct TcWorkspace {
   cudaStream_t stream = nullptr;
   size_t slots = 0, grid_max = 0;
   int refs = 0;
-  float *part_o = nullptr, *part_m = nullptr, *part_l = nullptr;
+  uint2* part_o = nullptr;
+  float *part_s = nullptr, *part_m = nullptr, *part_l = nullptr;
   int2* piece_info = nullptr;
 };
 static std::mutex g_ws_mu;
 static std::vector<TcWorkspace*> g_ws;
 
 static void ws_free(TcWorkspace* w) {
-  cudaFree(w->part_o); cudaFree(w->part_m); cudaFree(w->part_l); cudaFree(w->piece_info);
+  cudaFree(w->part_o); cudaFree(w->part_s); cudaFree(w->part_m); cudaFree(w->part_l); cudaFree(w->piece_info);
   delete w;
 }
 
@@ -315,7 +351,8 @@ static TcWorkspace* ws_acquire(cudaStream_t st, size_t slots, size_t grid_max, s
     if (w->device == device && w->stream == st && w->slots >= slots && w->grid_max >= grid_max) { ++w->refs; return w; }
   TcWorkspace* w = new TcWorkspace();
   w->device = device; w->stream = st; w->slots = slots; w->grid_max = grid_max; w->refs = 1;
-  cudaError_t e = cudaMalloc(&w->part_o, slots * kTcH * kTcD * sizeof(float));
+  cudaError_t e = cudaMalloc(&w->part_o, slots * (kTcH * kTcD / 4) * sizeof(uint2));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_s, slots * kTcPartScales * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&w->part_m, slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&w->part_l, slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, grid_max * sizeof(int2));
@@ -409,7 +446,17 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   p.scale_log2 = init.sm_scale * 1.4426950408889634f;
   pl->ws = ws_acquire(init.stream, slots, (size_t)pl->grid_max, msg);
   if (!pl->ws) { cudaFree(pl->d_maps); delete pl; return -2; }
-  p.part_o = pl->ws->part_o; p.part_m = pl->ws->part_m; p.part_l = pl->ws->part_l; p.piece_info = pl->ws->piece_info;
+  {   // the workspace's O partials as a 2-D u32 tensor [slots][H*D/2]; box = 512 B of kCombRows slots
+    cuuint64_t dims[2] = {(cuuint64_t)kTcH * kTcD / 2, (cuuint64_t)pl->ws->slots};
+    cuuint64_t strides[1] = {(cuuint64_t)kTcH * kTcD * 2};
+    cuuint32_t box[2] = {kCombRowBytes / 4, kCombRows};
+    cuuint32_t es[2] = {1, 1};
+    CUresult r = pl->encode(&pl->map_part, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, pl->ws->part_o, dims, strides, box, es,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { *msg = "cuTensorMapEncodeTiled (partials) failed"; return -2; }
+  }
+  p.part_o = pl->ws->part_o; p.part_s = pl->ws->part_s; p.part_m = pl->ws->part_m; p.part_l = pl->ws->part_l; p.piece_info = pl->ws->piece_info;
   TC_CUDA(cudaMalloc(&p.grid_ctr, sizeof(unsigned int)));
   TC_CUDA(cudaMemset(p.grid_ctr, 0, sizeof(unsigned int)));
   p.fused = (init.B <= kTcFusedMaxB && init.fuse_combine) ? 1 : 0;   // opt-in (LSA_MERGE_FUSED)
@@ -421,7 +468,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
 #endif
   pl->smem = sizeof(TcSmem) + 1024;
   TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
-  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemPad));
+  TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemMax));
   *out = pl;
   return 0;
 }
@@ -484,7 +531,9 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   if (no_pdl & 1) lc2.numAttrs = 0;
 #endif
   if (pl->init.B <= kCombineSpecMaxB) {
-    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel, prm, n_attn, (__nv_bfloat16*)out, lse));
+    const int land = (n_attn + kCombRows - 1) / kCombRows * kCombBoxBytes;
+    if (land > kCombineSmemPad) lc2.dynamicSmemBytes = land;
+    TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_kernel, pl->map_part, prm, n_attn, (__nv_bfloat16*)out, lse));
   } else {
     lc2.gridDim = dim3(16, pl->init.B); lc2.dynamicSmemBytes = 0;
     TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_wide_kernel, prm, n_attn, (__nv_bfloat16*)out, lse));

@@ -49,6 +49,27 @@ constexpr int kTcThreads = 64 + 32 * kTcSoftmaxWarps;
 constexpr int kTcMaxB = 256;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P may grow to 2^8 before O is rescaled
 
+// ---- split-K partial format --------------------------------------------------------------------
+// The un-normalised O^T of a piece goes to the workspace as fp16 with one power-of-two scale per warp of the
+// epilogue (32 d-rows x 32 heads): the block's largest magnitude lands in [2^14, 2^15), so every element within
+// 2^-28 of it keeps fp16's 11-bit mantissa (relative error <= 2^-12, 8x below the rounding of the bf16 result)
+// and smaller ones keep an absolute error below 2^-39 of the block maximum.  Half the bytes of fp32 partials:
+// both the store at the end of the attention kernel (per-SM store bandwidth) and the combine kernel's read
+// (L2 bandwidth) are bound by them at small B.  m and l stay fp32.
+constexpr int kTcPartScales = 32;           // scales per slot: [4 d-blocks m][2 head halves hh][4 lane quarters]
+__device__ __forceinline__ int part_scale_idx(size_t slot, int m, int hh, int q4) {
+  return (int)(((slot * 4 + m) * 2 + hh) * 4 + q4);
+}
+// amax = largest |value| of the block.  Returns the multiplier (2^e) applied before the fp16 conversion and,
+// through *inv, its exact inverse 2^-e; both are normal fp32 numbers for every amax (0, denormal, inf, NaN too).
+__device__ __forceinline__ float part_scale(float amax, float* inv) {
+  const int eb = (int)((__float_as_uint(amax) >> 23) & 0xffu);      // biased exponent of amax
+  int sb = 268 - eb;                                                // 127 + 14 - (eb - 127)
+  sb = sb > 253 ? 253 : sb;                                         // tiny or zero blocks: keep the inverse normal
+  *inv = __uint_as_float((uint32_t)(254 - sb) << 23);
+  return __uint_as_float((uint32_t)sb << 23);
+}
+
 // per-sequence shape as of this launch
 struct SeqView {
   int b, t_hca, n_cur, n_hca, w_len, cur;
@@ -77,7 +98,8 @@ struct TcParams {
   const CUtensorMap* seq_maps;   // [B][4]: hca_k, hca_v, win_k, win_v
   int B, k;
   float scale_log2;
-  float* part_o;                 // [slots][4 d-blocks][2 head halves][8 head quads][128 d][4 heads]  (= H*D floats)
+  uint2* part_o;                 // [slots][4 d-blocks m][2 head halves hh][8 head quads g][128 d][4 heads] fp16, scaled:
+  float* part_s;                 // [slots][m][hh][4 lane quarters]: o = fp16 value * part_s (a power of two), see part_scale()
   float* part_m;                 // [slots][H]   (log2 domain)
   float* part_l;                 // [slots][H]
   int2* piece_info;              // [grid]: (first sequence, number of sequences) this CTA wrote partials for
@@ -205,6 +227,11 @@ __device__ __forceinline__ unsigned long long gtime() {
 __device__ __forceinline__ void tlog_add(unsigned long long* tlog, unsigned long long id, unsigned long long t0) {
   const unsigned long long i = atomicAdd(tlog, 1ull);
   if (i < 4096) { tlog[1 + 3 * i] = id; tlog[2 + 3 * i] = t0; tlog[3 + 3 * i] = gtime(); }
+}
+// raw pair (e.g. SM clock offsets): reading %globaltimer costs about a microsecond, clock64() a few cycles
+__device__ __forceinline__ void tlog_pair(unsigned long long* tlog, unsigned long long id, unsigned long long a, unsigned long long b) {
+  const unsigned long long i = atomicAdd(tlog, 1ull);
+  if (i < 4096) { tlog[1 + 3 * i] = id; tlog[2 + 3 * i] = a; tlog[3 + 3 * i] = b; }
 }
 #endif
 

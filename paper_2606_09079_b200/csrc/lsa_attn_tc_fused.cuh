@@ -85,7 +85,7 @@ __device__ __noinline__ void fused_combine(const TcParams& p, unsigned char* scr
   }
   named_bar_sync(2, 256);
   // ---- units ----
-  const float4* part_o4 = reinterpret_cast<const float4*>(p.part_o);
+  const uint2* part_o4 = p.part_o;                               // 4 heads of one d per element
   constexpr int U = 12;                                          // 16-byte loads in flight per thread
   int it = 0;
   for (int u = cta; u < p.B * 256; u += n_cta, ++it) {
@@ -95,29 +95,44 @@ __device__ __noinline__ void fused_combine(const TcParams& p, unsigned char* scr
     const int* lst = list + b * 256;
     const int n_w = n > w ? (n - w + 7) >> 3 : 0;                // partials w, w+8, ... of this warp (<= 32)
     const int col = cc * 32 + lane;                              // float4 column inside a partial
-    float4 v[U];
+    uint2 v[U];
 #pragma unroll
     for (int j = 0; j < U; ++j)
-      v[j] = j < n_w ? __ldcg(part_o4 + (size_t)lst[w + 8 * j] * (kTcH * kTcD / 4) + col) : make_float4(0.f, 0.f, 0.f, 0.f);
+      v[j] = j < n_w ? __ldcg(part_o4 + (size_t)lst[w + 8 * j] * (kTcH * kTcD / 4) + col) : make_uint2(0u, 0u);
     float4 mj = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY), lj = make_float4(0.f, 0.f, 0.f, 0.f);
+    float sj = 0.f;                                              // scale of the unit's fp16 block in partial `lane`
     if (lane < n_w) {
       const size_t s = (size_t)lst[w + 8 * lane];
       mj = __ldcg(reinterpret_cast<const float4*>(p.part_m + s * kTcH + h0));
       lj = __ldcg(reinterpret_cast<const float4*>(p.part_l + s * kTcH + h0));
+      sj = __ldcg(p.part_s + part_scale_idx(s, m, hh, dq));
     }
     const float4 M = warp_max4(mj);
     const float4 wj = make_float4(w_of(mj.x, M.x), w_of(mj.y, M.y), w_of(mj.z, M.z), w_of(mj.w, M.w));
     const float4 L = warp_sum4(make_float4(wj.x * lj.x, wj.y * lj.y, wj.z * lj.z, wj.w * lj.w));
+    // a piece without valid keys (m = -inf) wrote no O: its weight is 0 and its data is never multiplied
+    const float4 ws = make_float4(wj.x * sj, wj.y * sj, wj.z * sj, wj.w * sj);
+    const unsigned live = __ballot_sync(0xffffffffu, mj.x != -INFINITY);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
     for (int j = 0; j < U; ++j) {
-      acc.x = fmaf(__shfl_sync(0xffffffffu, wj.x, j), v[j].x, acc.x); acc.y = fmaf(__shfl_sync(0xffffffffu, wj.y, j), v[j].y, acc.y);
-      acc.z = fmaf(__shfl_sync(0xffffffffu, wj.z, j), v[j].z, acc.z); acc.w = fmaf(__shfl_sync(0xffffffffu, wj.w, j), v[j].w, acc.w);
+      const float2 a01 = unpack_f16x2(v[j].x), a23 = unpack_f16x2(v[j].y);
+      const float fx = __shfl_sync(0xffffffffu, ws.x, j), fy = __shfl_sync(0xffffffffu, ws.y, j);
+      const float fz = __shfl_sync(0xffffffffu, ws.z, j), fw = __shfl_sync(0xffffffffu, ws.w, j);
+      if ((live >> j) & 1u) {
+        acc.x = fmaf(fx, a01.x, acc.x); acc.y = fmaf(fy, a01.y, acc.y);
+        acc.z = fmaf(fz, a23.x, acc.z); acc.w = fmaf(fw, a23.y, acc.w);
+      }
     }
     for (int j = U; j < n_w; ++j) {                              // more than 8*U partials: rare, one at a time
-      const float4 x = __ldcg(part_o4 + (size_t)lst[w + 8 * j] * (kTcH * kTcD / 4) + col);
-      acc.x = fmaf(__shfl_sync(0xffffffffu, wj.x, j), x.x, acc.x); acc.y = fmaf(__shfl_sync(0xffffffffu, wj.y, j), x.y, acc.y);
-      acc.z = fmaf(__shfl_sync(0xffffffffu, wj.z, j), x.z, acc.z); acc.w = fmaf(__shfl_sync(0xffffffffu, wj.w, j), x.w, acc.w);
+      const uint2 x = __ldcg(part_o4 + (size_t)lst[w + 8 * j] * (kTcH * kTcD / 4) + col);
+      const float2 a01 = unpack_f16x2(x.x), a23 = unpack_f16x2(x.y);
+      const float fx = __shfl_sync(0xffffffffu, ws.x, j), fy = __shfl_sync(0xffffffffu, ws.y, j);
+      const float fz = __shfl_sync(0xffffffffu, ws.z, j), fw = __shfl_sync(0xffffffffu, ws.w, j);
+      if ((live >> j) & 1u) {
+        acc.x = fmaf(fx, a01.x, acc.x); acc.y = fmaf(fy, a01.y, acc.y);
+        acc.z = fmaf(fz, a23.x, acc.z); acc.w = fmaf(fw, a23.y, acc.w);
+      }
     }
     float4* mb = mrg + ((it & 1) * 8 + w) * 34;
     mb[lane] = acc;

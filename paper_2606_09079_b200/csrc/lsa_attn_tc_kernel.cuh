@@ -352,7 +352,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       // layout [d-block m][head half][head quad g][d_local][4 heads]: one 16-byte store per (m, g), warp-contiguous
       if (tr) TR(2, 20);
       const size_t slot = (size_t)cta + b;
-      float4* po = reinterpret_cast<float4*>(p.part_o + slot * (kTcH * kTcD)) + (size_t)hh * (8 * 128) + key;
+      uint2* po = p.part_o + slot * (kTcH * kTcD / 4) + (size_t)hh * (8 * 128) + key;
 #pragma unroll 1
       for (int m = 0; m < 4; ++m) {               // d = m * 128 + key
         uint32_t vreg[32];
@@ -360,10 +360,17 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
         tc_fence_after();
         tmem_ld32(tO + m * 64 + hh * 32 + lane_addr, vreg);
         tmem_wait_ld();
+        float amax = 0.f;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) amax = fmaxf(amax, fabsf(__uint_as_float(vreg[j])));
+        float inv;
+        const float sc = part_scale(redux_max_f32(amax), &inv);   // one scale per warp: 32 d-rows x 32 heads
+        if (lane == 0) p.part_s[part_scale_idx(slot, m, hh, q4)] = inv;
 #pragma unroll
         for (int g = 0; g < 8; ++g)
-          po[(size_t)m * (2 * 8 * 128) + g * 128] = make_float4(__uint_as_float(vreg[4 * g]), __uint_as_float(vreg[4 * g + 1]),
-                                                                 __uint_as_float(vreg[4 * g + 2]), __uint_as_float(vreg[4 * g + 3]));
+          po[(size_t)m * (2 * 8 * 128) + g * 128] =
+              make_uint2(pack_f16x2(__uint_as_float(vreg[4 * g]) * sc, __uint_as_float(vreg[4 * g + 1]) * sc),
+                         pack_f16x2(__uint_as_float(vreg[4 * g + 2]) * sc, __uint_as_float(vreg[4 * g + 3]) * sc));
       }
       if (q4 == 0) {                              // every lane of L holds the same row sums: lane 0 writes them
         uint32_t vreg[32];

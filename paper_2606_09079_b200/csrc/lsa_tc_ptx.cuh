@@ -184,4 +184,16 @@ __device__ __forceinline__ bool elect_one() {
 }
 
 }  // namespace ptx
+// two floats -> packed fp16 pair (low half = a), round to nearest even; and back
+__device__ __forceinline__ uint32_t pack_f16x2(float a, float b) {
+  uint32_t r;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a));
+  return r;
+}
+__device__ __forceinline__ float2 unpack_f16x2(uint32_t v) {
+  float2 r;
+  asm("{ .reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi; }" : "=f"(r.x), "=f"(r.y) : "r"(v));
+  return r;
+}
+
 }  // namespace lsa
