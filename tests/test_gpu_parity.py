@@ -285,6 +285,43 @@ def test_tcgen05_attention_edge_cases(max_ctas, keep, merge):
 
 
 @pytest.mark.parametrize("merge", ["kernel", "fused"])
+@pytest.mark.parametrize("v_scale", [2.0 ** -40, 1.0, 2.0 ** 40])
+def test_tcgen05_partials_keep_precision_at_any_magnitude(v_scale, merge):
+    """The split-K partials are fp16 with a power-of-two scale per block (lsa_attn_tc_defs.cuh): values far
+    outside fp16's own range (V ~ 2^-40 or 2^40) and a row whose columns differ by 2^20 must come out with the
+    same RELATIVE accuracy as values near 1.  Several CTAs per sequence so the partials really are merged."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 128
+    g = torch.Generator().manual_seed(21)
+    rnd = lambda *s: torch.randn(*s, generator=g)
+    n_rows = [2000, 777]
+    col_gain = torch.ones(D)
+    col_gain[::7] = 2.0 ** 20                                     # wide dynamic range inside one row of V
+    hk = [rnd(n, D).to(torch.bfloat16).to(dev) for n in n_rows]
+    hv = [(rnd(n, D) * col_gain * v_scale).to(torch.bfloat16).to(dev) for n in n_rows]
+    wk = [rnd(W, D).to(torch.bfloat16).to(dev) for _ in n_rows]
+    wv = [(rnd(W, D) * col_gain * v_scale).to(torch.bfloat16).to(dev) for _ in n_rows]
+    w_len = [100, 0]
+    q = rnd(2, H, D).to(torch.bfloat16).to(dev)                   # logits ~ N(0, 5.6^2): a few keys dominate, |out| ~ |V|
+    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.25, attn_impl=lsa.LSA_ATTN_TCGEN05,
+                      merge_mode=lsa.LSA_MERGE_FUSED if merge == "fused" else lsa.LSA_MERGE_KERNEL)
+    out = ctx.decode_attention(q)
+    ctx.sync()
+    assert ctx.stats()["attn_ctas"] > 4
+    out64 = out.double().cpu().numpy()
+    for b in range(2):
+        K = np.concatenate([hk[b].double().cpu().numpy(), wk[b][: w_len[b]].double().cpu().numpy()])
+        V = np.concatenate([hv[b].double().cpu().numpy(), wv[b][: w_len[b]].double().cpu().numpy()])
+        ref, _, _ = attention(q[b].double().cpu().numpy(), K, V, 0.25)
+        gain = (col_gain.double() * v_scale).numpy()[None, :]
+        assert np.abs(ref / gain).mean() > 0.1
+        # relative to each column's magnitude, tighter than the north star's bf16 bar (abs 2e-2 / rel 1e-2)
+        np.testing.assert_allclose(out64[b] / gain, ref / gain, atol=1e-2, rtol=1e-2)
+    ctx.close()
+
+
+@pytest.mark.parametrize("merge", ["kernel", "fused"])
 def test_tcgen05_contexts_of_one_stream_share_the_workspace(merge):
     """Contexts on the same compute stream share the split-K workspace (lsa_attn_tc.cu): launches of three
     contexts with different batch sizes and key counts, interleaved back to back without a host sync, must each
