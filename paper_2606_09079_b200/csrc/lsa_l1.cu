@@ -8,7 +8,8 @@
 //
 // Kernels
 //   l1_gemv_kernel      Eq.(1)-(3): one warp per output row, 16-byte loads, fp32 accumulation.  c^Q stays fp32;
-//                       q is rounded to bf16 (it is the B operand of the tensor-core match below).
+//                       q is rounded to bf16 (it is the B operand of the tensor-core match below).  Two launches
+//                       per trigger: Eq.(1)+(3) of every layer, then Eq.(2) of every layer.
 //   l1_score_kernel     Eq.(4) over all entries, the only heavy part: 64 MiB of index keys per layer at 1M
 //                       context against 4.3 GFLOP -> HBM-bound with the match on tensor cores.  Same
 //                       "entries on M" formulation as the attention kernel: per 128-entry tile
@@ -57,67 +58,95 @@ template <> __device__ __forceinline__ __nv_bfloat16 l1_out<__nv_bfloat16>(float
 constexpr int kGvWarps = 4, kGvSeqs = 4;
 
 // W bf16 [E][Din]; x rows of stride ldx (input i is row xrows.ids[i]); out [n][ldo] (row i at out + i*ldo).
-// The block first stages its (up to 4) x rows in shared memory - read from L2 inside the FMA loop they would be
-// 16 dependent round trips per lane - then every warp streams one weight row with all its loads in flight.
+// One launch carries several independent products that share Din ("jobs": the three layers' Eq.(1) and Eq.(3) in
+// one launch, their Eq.(2) in another) - a single layer's matrix is one wave of blocks and leaves HBM half idle.
+// Blocks are persistent: a block stages its (up to 4) x rows in shared memory ONCE - read from L2 inside the
+// FMA loop they would be 16 dependent round trips per lane - and its warps then walk weight rows r, r + stride,
+// ... with all loads of a row in flight; the other warps of the SM cover a warp's latency.
+//   shared_x = 1: every job reads the same x; the rows of all jobs form one flat list, gridDim.z = 1
+//   shared_x = 0: job = blockIdx.z has its own x
+constexpr int kGvMaxJobs = 8;
+struct GvJobs {
+  const __nv_bfloat16* W[kGvMaxJobs];   // [E][Din]
+  const void* x[kGvMaxJobs];            // input rows (XT)
+  void* out[kGvMaxJobs];                // row i at out + i * ldo (OT)
+  long long ldo[kGvMaxJobs];
+  int E[kGvMaxJobs];
+  int n_jobs, shared_x;
+};
+
 template <typename XT, typename OT>
 __global__ void __launch_bounds__(kGvWarps * 32)
-l1_gemv_kernel(const __nv_bfloat16* __restrict__ W, const XT* __restrict__ x, long long ldx, FireList xrows, OT* __restrict__ out,
-               long long ldo, int n, int E, int Din) {
+l1_gemv_kernel(GvJobs jobs, long long ldx, FireList xrows, int n, int Din) {
   extern __shared__ __align__(16) unsigned char gv_smem[];
   XT* xs = reinterpret_cast<XT*>(gv_smem);                 // [kGvSeqs][Din]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int e = blockIdx.x * kGvWarps + warp;
   const int i0 = blockIdx.y * kGvSeqs;
-  const __nv_bfloat16* wrow = W + (size_t)min(e, E - 1) * Din;
+  const int j_lo = jobs.shared_x ? 0 : (int)blockIdx.z, j_hi = jobs.shared_x ? jobs.n_jobs : j_lo + 1;
+  int total = 0;
+  for (int j = j_lo; j < j_hi; ++j) total += jobs.E[j];
+  const int stride = gridDim.x * kGvWarps;
+  int r = blockIdx.x * kGvWarps + warp;
+  // row r of the flat list -> (job, row inside the job)
+  auto locate = [&](int rr, int& j, int& e) {
+    j = j_lo; e = rr;
+    while (j + 1 < j_hi && e >= jobs.E[j]) { e -= jobs.E[j]; ++j; }
+  };
   constexpr int kU = 16;
   uint4 wraw[kU];
+  auto load_row = [&](const __nv_bfloat16* wrow, int d0) {
 #pragma unroll
-  for (int u = 0; u < kU; ++u) {                            // weights never depend on the previous kernel
-    const int d = lane * 8 + u * 256;
-    wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+    for (int u = 0; u < kU; ++u) {
+      const int d = d0 + u * 256;
+      wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+    }
+  };
+  int j = 0, e = 0;
+  if (r < total) {                                          // weights never depend on the previous kernel
+    locate(r, j, e);
+    load_row(jobs.W[j] + (size_t)e * Din, lane * 8);
   }
   pdl_wait();
   pdl_launch_dependents();
   constexpr int kPer16 = 16 / (int)sizeof(XT);
+  const XT* x = reinterpret_cast<const XT*>(jobs.x[j_lo]);
   for (int s = 0; s < kGvSeqs; ++s)
     if (i0 + s < n)
       for (int d = threadIdx.x * kPer16; d < Din; d += kGvWarps * 32 * kPer16)
         *reinterpret_cast<uint4*>(xs + (size_t)s * Din + d) = *reinterpret_cast<const uint4*>(x + (size_t)xrows.ids[i0 + s] * ldx + d);
   __syncthreads();
-  if (e >= E) return;
-  float acc[kGvSeqs];
+  for (bool first = true; r < total; r += stride, first = false) {
+    if (!first) locate(r, j, e);
+    const __nv_bfloat16* wrow = jobs.W[j] + (size_t)e * Din;
+    float acc[kGvSeqs];
 #pragma unroll
-  for (int s = 0; s < kGvSeqs; ++s) acc[s] = 0.f;
-  for (int d0 = lane * 8; d0 < Din; d0 += 256 * kU) {
-    if (d0 != lane * 8) {                                   // rows longer than 4096: further batches
+    for (int s = 0; s < kGvSeqs; ++s) acc[s] = 0.f;
+    for (int d0 = lane * 8; d0 < Din; d0 += 256 * kU) {
+      if (!first || d0 != lane * 8) load_row(wrow, d0);     // (the first batch of the first row is already here)
 #pragma unroll
       for (int u = 0; u < kU; ++u) {
         const int d = d0 + u * 256;
-        wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
-      }
-    }
+        if (d < Din) {
+          float wf[8];
+          Elem<__nv_bfloat16>::unpack16(wraw[u], wf);
 #pragma unroll
-    for (int u = 0; u < kU; ++u) {
-      const int d = d0 + u * 256;
-      if (d < Din) {
-        float wf[8];
-        Elem<__nv_bfloat16>::unpack16(wraw[u], wf);
+          for (int s = 0; s < kGvSeqs; ++s) {
+            if (i0 + s < n) {
+              float xf[8];
+              L1X<XT>::load8(xs + (size_t)s * Din + d, xf);
 #pragma unroll
-        for (int s = 0; s < kGvSeqs; ++s) {
-          if (i0 + s < n) {
-            float xf[8];
-            L1X<XT>::load8(xs + (size_t)s * Din + d, xf);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) acc[s] = fmaf(wf[j], xf[j], acc[s]);
+              for (int jj = 0; jj < 8; ++jj) acc[s] = fmaf(wf[jj], xf[jj], acc[s]);
+            }
           }
         }
       }
     }
-  }
+    OT* out = reinterpret_cast<OT*>(jobs.out[j]);
 #pragma unroll
-  for (int s = 0; s < kGvSeqs; ++s) {
-    const float v = warp_sum(acc[s]);
-    if (lane == 0 && i0 + s < n) out[(size_t)(i0 + s) * ldo + e] = l1_out<OT>(v);
+    for (int s = 0; s < kGvSeqs; ++s) {
+      const float v = warp_sum(acc[s]);
+      if (lane == 0 && i0 + s < n) out[(size_t)(i0 + s) * jobs.ldo[j] + e] = l1_out<OT>(v);
+    }
   }
 }
 
@@ -340,6 +369,7 @@ struct L1Plan {
   int cap = 0;                         // sequences per launch
   size_t smem = 0;
   int n_sms = 0;
+  int occ13 = 1, occ2 = 1;             // resident GEMV blocks per SM (Eq.(1)+(3) launch, Eq.(2) launch)
 };
 
 // [rows][128] bf16 seen as (64 columns, rows, 2 d-blocks): a box lands as [2][box_rows][128 B], 128-byte swizzle
@@ -401,6 +431,9 @@ int l1_create(const L1Init& init, L1Plan** out, std::string* msg) {
   if ((size_t)kGvSeqs * init.Dh * 2 > 200 * 1024 || (size_t)kGvSeqs * init.d_c * 4 > 200 * 1024) { *msg = "Dh / d_c too large for the staged projections"; delete pl; return -6; }
   L1_CUDA(cudaFuncSetAttribute(l1_gemv_kernel<__nv_bfloat16, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   L1_CUDA(cudaFuncSetAttribute(l1_gemv_kernel<float, __nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  // persistent GEMV blocks: exactly one resident wave (a second, partial wave would double the kernel's time)
+  L1_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->occ13, l1_gemv_kernel<__nv_bfloat16, float>, kGvWarps * 32, (size_t)kGvSeqs * init.Dh * 2));
+  L1_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->occ2, l1_gemv_kernel<float, __nv_bfloat16>, kGvWarps * 32, (size_t)kGvSeqs * init.d_c * 4));
   *out = pl;
   return 0;
 }
@@ -424,23 +457,32 @@ int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, c
     FireList hr{}, ident{};
     hr.n = ident.n = m;
     for (int i = 0; i < m; ++i) { hr.ids[i] = hrows[off + i]; ident.ids[i] = i; }
+    // Eq.(1) c^Q [m][d_c] fp32 and Eq.(3) w -> piece (i, l), all layers in one launch (both read h)
+    GvJobs j13{}, j2{};
     for (int l = 0; l < L; ++l) {
-      const __nv_bfloat16* Wdq = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_dq);
-      const __nv_bfloat16* Wiuq = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_iuq);
-      const __nv_bfloat16* Ww = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_w);
       float* cq = pl->cq + (size_t)l * pl->cap * d_c;
-      // Eq.(1): c^Q [m][d_c] fp32
-      L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((d_c + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * Dh * 2, st,
-                         Wdq, hb, (long long)Dh, hr, cq, (long long)d_c, m, d_c, Dh));
-      // Eq.(3): w -> piece (i, l)
-      L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3((kL1H + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * Dh * 2, st,
-                         Ww, hb, (long long)Dh, hr, pl->wbuf + (size_t)l * kL1H, (long long)L * kL1H, m, kL1H, Dh));
+      j13.W[l] = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_dq);
+      j13.x[l] = hb; j13.out[l] = cq; j13.ldo[l] = d_c; j13.E[l] = d_c;
+      j13.W[L + l] = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_w);
+      j13.x[L + l] = hb; j13.out[L + l] = pl->wbuf + (size_t)l * kL1H; j13.ldo[L + l] = (long long)L * kL1H; j13.E[L + l] = kL1H;
       // Eq.(2): q -> piece (i, l), rounded to bf16
-      L1_CUDA(launch_pdl(l1_gemv_kernel<float, __nv_bfloat16>, dim3((kL1H * kL1CI + kGvWarps - 1) / kGvWarps, (m + kGvSeqs - 1) / kGvSeqs), blk, (size_t)kGvSeqs * d_c * 4, st,
-                         Wiuq, (const float*)cq, (long long)d_c, ident, pl->q + (size_t)l * kL1H * kL1CI, (long long)L * kL1H * kL1CI, m,
-                         kL1H * kL1CI, d_c));
-      *launches += 3;
+      j2.W[l] = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_iuq);
+      j2.x[l] = cq; j2.out[l] = pl->q + (size_t)l * kL1H * kL1CI; j2.ldo[l] = (long long)L * kL1H * kL1CI; j2.E[l] = kL1H * kL1CI;
     }
+    j13.n_jobs = 2 * L; j13.shared_x = 1;
+    j2.n_jobs = L; j2.shared_x = 0;
+    const unsigned gy = (unsigned)((m + kGvSeqs - 1) / kGvSeqs);
+    // persistent blocks: as many as fit on the machine at once (shared memory bounds the occupancy)
+    auto blocks_x = [&](int per_sm, int rows, int z) {
+      const int fit = std::max(1, pl->n_sms * std::max(1, per_sm) / (int)(gy * z));
+      return (unsigned)std::max(1, std::min(fit, (rows + kGvWarps - 1) / kGvWarps));
+    };
+    const size_t sm13 = (size_t)kGvSeqs * Dh * 2, sm2 = (size_t)kGvSeqs * d_c * 4;
+    L1_CUDA(launch_pdl(l1_gemv_kernel<__nv_bfloat16, float>, dim3(blocks_x(pl->occ13, L * (d_c + kL1H), 1), gy, 1), blk, sm13, st, j13,
+                       (long long)Dh, hr, m, Dh));
+    L1_CUDA(launch_pdl(l1_gemv_kernel<float, __nv_bfloat16>, dim3(blocks_x(pl->occ2, kL1H * kL1CI, L), gy, L), blk, sm2, st, j2,
+                       (long long)d_c, ident, m, d_c));
+    *launches += 2;
     L1ScoreParams sp{};
     sp.k_maps = pl->d_maps; sp.wbuf = pl->wbuf; sp.chunk_pre = pl->chunk_pre;
     sp.n_pieces = m * L; sp.n_chunks_max = std::max(in.n_chunks_max, 1);
