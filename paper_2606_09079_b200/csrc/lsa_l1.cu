@@ -75,8 +75,87 @@ struct GvJobs {
   int n_jobs, shared_x;
 };
 
+constexpr int kGvU = 8;                       // 16-byte loads per lane and batch: one batch = 2048 weights of a row
+constexpr int kGvBatch = kGvU * 256;
+
+// The warp's rows as a sequence of batches (row, d0); batch t+1 is loaded into the other register buffer before
+// batch t is multiplied, so a warp always has 4 KiB in flight.  NS = sequences handled per block (1: the common
+// single-trigger case without the 4x predicated code; 4: rows i0 .. i0+3, those >= n masked).
+__device__ __forceinline__ void gv_locate(const GvJobs& jobs, int j_lo, int j_hi, int rr, int& j, int& e) {
+  j = j_lo; e = rr;                                        // row rr of the flat list -> (job, row inside the job)
+  while (j + 1 < j_hi && e >= jobs.E[j]) { e -= jobs.E[j]; ++j; }
+}
+__device__ __forceinline__ void gv_load(uint4* w, const __nv_bfloat16* wrow, int d0, int Din, int lane) {
+#pragma unroll
+  for (int u = 0; u < kGvU; ++u) {
+    const int d = d0 + lane * 8 + u * 256;
+    w[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
+  }
+}
+
+// wa holds batch 0 of row r0 = (j, e) already (loaded by the caller before the launch dependency resolved).
+template <typename XT, typename OT, int NS>
+__device__ __forceinline__ void gv_rows(const GvJobs& jobs, const XT* xs, int j_lo, int j_hi, int total, int stride, int r0,
+                                        int i0, int n, int Din, int lane, uint4 (&wa)[kGvU], int j, int e) {
+  auto locate = [&](int rr, int& jj, int& ee) { gv_locate(jobs, j_lo, j_hi, rr, jj, ee); };
+  auto load = [&](uint4* w, const __nv_bfloat16* wrow, int d0) { gv_load(w, wrow, d0, Din, lane); };
+  float acc[NS][2];
+#pragma unroll
+  for (int s = 0; s < NS; ++s) acc[s][0] = acc[s][1] = 0.f;
+  auto mul = [&](const uint4* w, int d0) {
+#pragma unroll
+    for (int u = 0; u < kGvU; ++u) {
+      const int d = d0 + lane * 8 + u * 256;
+      if (d < Din) {
+        float wf[8];
+        Elem<__nv_bfloat16>::unpack16(w[u], wf);
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+          if (NS == 1 || i0 + s < n) {
+            float xf[8];
+            L1X<XT>::load8(xs + (size_t)s * Din + d, xf);
+#pragma unroll
+            for (int jj = 0; jj < 8; ++jj) acc[s][jj & 1] = fmaf(wf[jj], xf[jj], acc[s][jj & 1]);
+          }
+        }
+      }
+    }
+  };
+  auto finish = [&](int j, int e) {
+    OT* out = reinterpret_cast<OT*>(jobs.out[j]);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      const float v = warp_sum(acc[s][0] + acc[s][1]);
+      if (lane == 0 && i0 + s < n) out[(size_t)(i0 + s) * jobs.ldo[j] + e] = l1_out<OT>(v);
+      acc[s][0] = acc[s][1] = 0.f;
+    }
+  };
+  // state of the batch in flight / being multiplied
+  int r = r0, d0 = 0;
+  const __nv_bfloat16* wrow = r < total ? jobs.W[j] + (size_t)e * Din : nullptr;
+  uint4 wb[kGvU];
+  // one step: issue the loads of the next batch into `nxt`, multiply `cur`
+  auto step = [&](uint4* cur, uint4* nxt) {
+    int r2 = r, d2 = d0 + kGvBatch, j2 = j, e2 = e;
+    const __nv_bfloat16* wrow2 = wrow;
+    if (d2 >= Din) {
+      r2 = r + stride; d2 = 0;
+      if (r2 < total) { locate(r2, j2, e2); wrow2 = jobs.W[j2] + (size_t)e2 * Din; }
+    }
+    if (r2 < total) load(nxt, wrow2, d2);
+    mul(cur, d0);
+    if (r2 != r) finish(j, e);
+    r = r2; d0 = d2; j = j2; e = e2; wrow = wrow2;
+  };
+  while (r < total) {
+    step(wa, wb);
+    if (r >= total) break;
+    step(wb, wa);
+  }
+}
+
 template <typename XT, typename OT>
-__global__ void __launch_bounds__(kGvWarps * 32)
+__global__ void __launch_bounds__(kGvWarps * 32, 4)
 l1_gemv_kernel(GvJobs jobs, long long ldx, FireList xrows, int n, int Din) {
   extern __shared__ __align__(16) unsigned char gv_smem[];
   XT* xs = reinterpret_cast<XT*>(gv_smem);                 // [kGvSeqs][Din]
@@ -85,26 +164,12 @@ l1_gemv_kernel(GvJobs jobs, long long ldx, FireList xrows, int n, int Din) {
   const int j_lo = jobs.shared_x ? 0 : (int)blockIdx.z, j_hi = jobs.shared_x ? jobs.n_jobs : j_lo + 1;
   int total = 0;
   for (int j = j_lo; j < j_hi; ++j) total += jobs.E[j];
-  const int stride = gridDim.x * kGvWarps;
-  int r = blockIdx.x * kGvWarps + warp;
-  // row r of the flat list -> (job, row inside the job)
-  auto locate = [&](int rr, int& j, int& e) {
-    j = j_lo; e = rr;
-    while (j + 1 < j_hi && e >= jobs.E[j]) { e -= jobs.E[j]; ++j; }
-  };
-  constexpr int kU = 16;
-  uint4 wraw[kU];
-  auto load_row = [&](const __nv_bfloat16* wrow, int d0) {
-#pragma unroll
-    for (int u = 0; u < kU; ++u) {
-      const int d = d0 + u * 256;
-      wraw[u] = d < Din ? *reinterpret_cast<const uint4*>(wrow + d) : make_uint4(0u, 0u, 0u, 0u);
-    }
-  };
-  int j = 0, e = 0;
-  if (r < total) {                                          // weights never depend on the previous kernel
-    locate(r, j, e);
-    load_row(jobs.W[j] + (size_t)e * Din, lane * 8);
+  const int stride = gridDim.x * kGvWarps, r0 = blockIdx.x * kGvWarps + warp;
+  uint4 wa[kGvU];
+  int j0 = j_lo, e0 = 0;
+  if (r0 < total) {                                         // weights never depend on the previous kernel
+    gv_locate(jobs, j_lo, j_hi, r0, j0, e0);
+    gv_load(wa, jobs.W[j0] + (size_t)e0 * Din, 0, Din, lane);
   }
   pdl_wait();
   pdl_launch_dependents();
@@ -115,39 +180,8 @@ l1_gemv_kernel(GvJobs jobs, long long ldx, FireList xrows, int n, int Din) {
       for (int d = threadIdx.x * kPer16; d < Din; d += kGvWarps * 32 * kPer16)
         *reinterpret_cast<uint4*>(xs + (size_t)s * Din + d) = *reinterpret_cast<const uint4*>(x + (size_t)xrows.ids[i0 + s] * ldx + d);
   __syncthreads();
-  for (bool first = true; r < total; r += stride, first = false) {
-    if (!first) locate(r, j, e);
-    const __nv_bfloat16* wrow = jobs.W[j] + (size_t)e * Din;
-    float acc[kGvSeqs];
-#pragma unroll
-    for (int s = 0; s < kGvSeqs; ++s) acc[s] = 0.f;
-    for (int d0 = lane * 8; d0 < Din; d0 += 256 * kU) {
-      if (!first || d0 != lane * 8) load_row(wrow, d0);     // (the first batch of the first row is already here)
-#pragma unroll
-      for (int u = 0; u < kU; ++u) {
-        const int d = d0 + u * 256;
-        if (d < Din) {
-          float wf[8];
-          Elem<__nv_bfloat16>::unpack16(wraw[u], wf);
-#pragma unroll
-          for (int s = 0; s < kGvSeqs; ++s) {
-            if (i0 + s < n) {
-              float xf[8];
-              L1X<XT>::load8(xs + (size_t)s * Din + d, xf);
-#pragma unroll
-              for (int jj = 0; jj < 8; ++jj) acc[s] = fmaf(wf[jj], xf[jj], acc[s]);
-            }
-          }
-        }
-      }
-    }
-    OT* out = reinterpret_cast<OT*>(jobs.out[j]);
-#pragma unroll
-    for (int s = 0; s < kGvSeqs; ++s) {
-      const float v = warp_sum(acc[s]);
-      if (lane == 0 && i0 + s < n) out[(size_t)(i0 + s) * jobs.ldo[j] + e] = l1_out<OT>(v);
-    }
-  }
+  if (n - i0 == 1) gv_rows<XT, OT, 1>(jobs, xs, j_lo, j_hi, total, stride, r0, i0, n, Din, lane, wa, j0, e0);
+  else gv_rows<XT, OT, kGvSeqs>(jobs, xs, j_lo, j_hi, total, stride, r0, i0, n, Din, lane, wa, j0, e0);
 }
 
 // ---- Eq.(4): entry scoring on tensor cores -----------------------------------------------------------------
