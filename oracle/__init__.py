@@ -5,3 +5,4 @@ from .lsa_oracle import (  # noqa: F401
     validate_selection, widen,
 )
 from . import l1_oracle  # noqa: F401,E402  (paper-exact Level-1 indexer, NEXT-1)
+from . import l2_oracle  # noqa: F401,E402  (Level-2 in-window Top-k, NEXT-2)

@@ -465,3 +465,27 @@ class L1Inputs:
                     K[e] = hot_gain * q0[p] / float(q0[p] @ q0[p])
                 self.index_k[b].append(store(K.astype(np.float32), "bf16"))
                 self.hot_chunks[b].append(hot)
+
+
+class L2Inputs:
+    """Seeded inputs of Level 2 (the native Lightning Indexer inside the resident set, Eq.(6)) on top of
+    an LsaWorkload: one layer's compressed indexer keys per sequence, and per decode step the indexer queries
+    q_idx [B][n_h][c_I] (bf16) and head weights w_idx [B][n_h] (fp32) of the token being decoded - inputs of the
+    path like q (oracle/l2_oracle.py reading M3).  Keys and queries are N(0,1)/sqrt(sqrt(c_I)) each, so a
+    per-head match is ~N(0,1); weights are N(0.5, 1)/n_h (mostly positive, some negative heads)."""
+
+    def __init__(self, wl: "LsaWorkload", c_I: int = 128, n_h: int = 64, tag: int = 1200):
+        c = wl.cfg
+        assert c.dtype == "bf16"
+        self.cfg, self.c_I, self.n_h, self.tag = c, c_I, n_h, tag
+        s = c_I ** -0.25
+        self.index_k: List[np.ndarray] = [_randn_stored(_rng(c.seed, tag, 1, b), (c.n_csa(b), c_I), s, "bf16") for b in range(c.B)]
+
+    def q_idx(self, step: int) -> np.ndarray:
+        c = self.cfg
+        return _randn_stored(_rng(c.seed, self.tag, 2, step), (c.B, self.n_h, self.c_I), self.c_I ** -0.25, "bf16")
+
+    def w_idx(self, step: int) -> np.ndarray:
+        c = self.cfg
+        g = _rng(c.seed, self.tag, 3, step)
+        return ((0.5 + g.standard_normal((c.B, self.n_h))) / self.n_h).astype(np.float32)
