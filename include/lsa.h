@@ -210,6 +210,37 @@ int lsa_l1_select(lsa_ctx* ctx, const void* h, const int32_t* seq_ids, int32_t n
 enum lsa_indexer { LSA_INDEXER_DUAL_ENCODER = 0, LSA_INDEXER_LEVEL1 = 1 };
 int lsa_set_indexer(lsa_ctx* ctx, int32_t indexer);
 
+/* ---- Level 2: the native Lightning Indexer inside the resident set (Eq.(6), l.187) ----
+ * Every decode step i, per sequence: Score_native(i, s) = sum_h w_{i,h} ReLU(q_{i,h} . K_s^IComp) - Eq.(4) without
+ * the sigmoid (l.75) - for the entries s of C_t^MemComp = the valid rows of the pages of the CURRENT page table;
+ * the first min(k2, |C_t^MemComp|) entries by (score descending, entry id s = chunk*C + row ascending) form
+ * C_i^CoreComp, and core attention runs over HCA (+) C_i^CoreComp (+) window (l.85; HCA per BJ north_star).
+ * Supported: dtype bf16, C = 128, c_I = 128, n_h = 64, tcgen05 attention path, 1 <= k2 <= 4096 (else
+ * LSA_ERR_UNSUPPORTED / INVALID_ARG). */
+typedef struct lsa_l2_config {
+  uint32_t struct_size;  /* = sizeof(lsa_l2_config)                                                      */
+  int32_t c_I;           /* index-key dim per head                                                       */
+  int32_t n_h;           /* indexer heads                                                                */
+  int32_t k2;            /* Top-k entries kept per sequence and step (Eq.(6))                            */
+} lsa_l2_config;
+
+/* index_k: HOST array of B DEVICE pointers; index_k[b] = this layer's compressed indexer keys of sequence b,
+ * [n_csa_b][c_I] bf16, caller-owned, must outlive the context.  May be called once per context. */
+int lsa_l2_init(lsa_ctx* ctx, const lsa_l2_config* cfg, const void* const* index_k);
+
+/* Eq.(6) for all B sequences on stream_compute: staged tables that are due become current first (S6), then the
+ * entries of the current tables are scored and the Top-k2 marked.  The selection applies to the NEXT
+ * lsa_decode_attention call only (one-shot), which then attends HCA (+) the marked rows (+) window.
+ *   q_idx DEVICE [B][n_h][c_I] bf16   w_idx DEVICE [B][n_h] fp32 (both read on stream_compute)
+ *   sel_entries DEVICE [B][k2] int32 or NULL: entry ids in (score desc, id asc) order, then -1
+ *   sel_score   DEVICE [B][k2] fp32  or NULL: their native scores, -inf padding */
+int lsa_l2_select(lsa_ctx* ctx, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score);
+
+/* lsa_step with Level 2 between (d) and (e): the step's attention runs over HCA (+) the Top-k2 entries of the
+ * current tables (+) window.  Other arguments and the step order as lsa_step. */
+int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
+                const void* q_idx, const float* w_idx, void* out);
+
 /* Replace the embedding table pointer of one sequence (DEVICE [n_chunks][E]). */
 int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb);
 

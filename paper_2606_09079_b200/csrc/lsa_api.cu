@@ -18,6 +18,7 @@
 #include "lsa_attn_tc.h"
 #include "lsa_kernels.h"
 #include "lsa_l1.h"
+#include "lsa_l2.h"
 
 using namespace lsa;
 
@@ -55,6 +56,8 @@ struct lsa_ctx {
   TcPlan* tc = nullptr;
   L1Plan* l1 = nullptr;               // paper-exact Level-1 indexer (lsa_l1_init)
   float l1_threshold = 0.5f;
+  L2Plan* l2 = nullptr;               // Level 2 (lsa_l2_init)
+  bool l2_armed = false;              // a Level-2 selection waits for the next attention launch
   int indexer = 0;                     // lsa_indexer used by lsa_step at trigger steps
   // host-buffer staging (lsa_step_host)
   void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
@@ -130,6 +133,7 @@ extern "C" void lsa_destroy(lsa_ctx* ctx) {
   if (ctx->sf) cudaStreamSynchronize(ctx->sf);
   if (ctx->tc) tc_destroy(ctx->tc);
   if (ctx->l1) l1_destroy(ctx->l1);
+  if (ctx->l2) l2_destroy(ctx->l2);
   if (ctx->st_pin) cudaFreeHost(ctx->st_pin);
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
@@ -497,6 +501,8 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
     long long tiles = 0;                          // host mirror: HCA + selected pages + window, in 128-key tiles
     for (int b = 0; b < c->B; ++b)
       tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
+    tc_set_l2_mask(c->tc, c->l2_armed ? l2_mask(c->l2) : nullptr);      // one-shot: the selection of this step
+    c->l2_armed = false;
     int rc = tc_attention(c->tc, q, out, lse, tiles, pre, c->sc, &launches, &ctas, &msg,
                           prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
                           prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr,
@@ -530,8 +536,10 @@ extern "C" int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, floa
   return attention_impl(ctx, q, out, lse);
 }
 
-extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
-  if (!ctx) return LSA_ERR_STATE;
+static int l2_select_impl(lsa_ctx* c, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score);
+
+static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out,
+                     const void* q_idx, const float* w_idx) {
   lsa_ctx* c = ctx;
   if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
   if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
@@ -542,7 +550,7 @@ extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* 
     if (c->step[b] % c->cfg.tau == 0) ids[n_fire++] = b;           // S0
   if (n_fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
   int rc;
-  if (n_fire == 0 && c->attn_impl == LSA_ATTN_TCGEN05) {
+  if (n_fire == 0 && c->attn_impl == LSA_ATTN_TCGEN05 && !q_idx) {
     // no trigger this step: (a) and (d) ride on the attention launch itself (one kernel less per step).  On a
     // trigger step the residency pass must see the swapped tables, so they stay a kernel of their own.
     TcPrestep pre{};
@@ -566,10 +574,63 @@ extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* 
     if ((rc = fetch_impl(c, ids, n_fire, c->d_sel))) return rc;
     if (c->cfg.recall_lag == 0 && (rc = prestep_impl(c, false, nullptr, nullptr))) return rc;   // (c)
   }
+  if (q_idx && (rc = l2_select_impl(c, q_idx, w_idx, nullptr, nullptr))) return rc;   // Level 2 sees the tables attention will
   if ((rc = attention_impl(c, q, out, nullptr))) return rc;         // (e)
   for (int b = 0; b < c->B; ++b) c->step[b] += 1;                   // (f)
   c->n_steps += 1;
   return LSA_OK;
+}
+
+extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  return step_impl(ctx, q, h, k_new, v_new, out, nullptr, nullptr);
+}
+
+// ---- Level 2 (NEXT-2) ---------------------------------------------------------------------------------------
+extern "C" int lsa_l2_init(lsa_ctx* ctx, const lsa_l2_config* cfg, const void* const* index_k) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (!cfg || !index_k) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null argument");
+  if (cfg->struct_size != sizeof(lsa_l2_config)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "lsa_l2_config.struct_size mismatch");
+  if (c->l2) LSA_FAIL(c, LSA_ERR_STATE, "lsa_l2_init was already called on this context");
+  if (cfg->k2 < 1 || cfg->k2 > kSortCap) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k2 must be in 1..%d", kSortCap);
+  if (c->attn_impl != LSA_ATTN_TCGEN05 || !l2_supported(c->cfg.dtype, c->cfg.C, cfg->c_I, cfg->n_h))
+    LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "Level 2 needs the tcgen05 attention path, bf16, C=128, c_I=128, n_h=64 (got dtype=%d C=%d c_I=%d n_h=%d)",
+             c->cfg.dtype, c->cfg.C, cfg->c_I, cfg->n_h);
+  L2Init in{};
+  in.B = c->B; in.k = c->k; in.k2 = cfg->k2; in.n_sms = c->n_sms;
+  in.index_k = index_k; in.seq_host = c->seq_host.data(); in.tbl_chunk = c->pool.tbl_chunk;
+  std::string msg;
+  const int rc = l2_create(in, &c->l2, &msg);
+  if (rc != 0) LSA_FAIL(c, rc == -1 ? LSA_ERR_INVALID_ARG : LSA_ERR_CUDA, "Level 2 init failed: %s", msg.c_str());
+  return LSA_OK;
+}
+
+static int l2_select_impl(lsa_ctx* c, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score) {
+  if (!c->l2) LSA_FAIL(c, LSA_ERR_STATE, "lsa_l2_init has not been called");
+  if (!q_idx || !w_idx) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q_idx / w_idx");
+  int rc = prestep_impl(c, false, nullptr, nullptr);                // the tables the next attention launch will read
+  if (rc) return rc;
+  std::string msg;
+  int launches = 0;
+  rc = l2_select(c->l2, c->d_seqs, q_idx, w_idx, sel_entries, sel_score, c->sc, &launches, &msg);
+  c->attn_launches += launches;
+  if (rc != 0) LSA_FAIL(c, LSA_ERR_CUDA, "Level 2: %s", msg.c_str());
+  c->l2_armed = true;
+  return LSA_OK;
+}
+
+extern "C" int lsa_l2_select(lsa_ctx* ctx, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score) {
+  if (!ctx) return LSA_ERR_STATE;
+  return l2_select_impl(ctx, q_idx, w_idx, sel_entries, sel_score);
+}
+
+extern "C" int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, const void* q_idx,
+                           const float* w_idx, void* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!ctx->l2) LSA_FAIL(ctx, LSA_ERR_STATE, "lsa_l2_init has not been called");
+  if (!q_idx || !w_idx) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null q_idx / w_idx");
+  return step_impl(ctx, q, h, k_new, v_new, out, q_idx, w_idx);
 }
 
 // lsa_step_host: one launch pulls the step's inputs out of pinned, mapped host buffers (16-byte loads over the

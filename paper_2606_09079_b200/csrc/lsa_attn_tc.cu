@@ -543,6 +543,8 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   return 0;
 }
 
+void tc_set_l2_mask(TcPlan* pl, const uint32_t* mask) { pl->params.l2_mask = mask; }
+
 void tc_destroy(TcPlan* pl) {
   if (!pl) return;
 #ifdef LSA_TC_TRACE

@@ -1,6 +1,7 @@
 // lsa_attn_tc.h - host interface of the tcgen05/TMA split-K decode attention (lsa_attn_tc.cu).
 #pragma once
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 #include <string>
 
@@ -36,6 +37,8 @@ struct TcPrestep {
 int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, const TcPrestep* pre, cudaStream_t st,
                  int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr,
                  unsigned long long* ktime = nullptr /* DEVICE [2] = {~0, 0}: kernel working-time stamps */);
+// Level 2: key mask [B][k][4] words used by the launches that follow (null: off); see TcParams::l2_mask
+void tc_set_l2_mask(TcPlan* plan, const uint32_t* mask);
 void tc_destroy(TcPlan* plan);
 
 }  // namespace lsa

@@ -110,6 +110,9 @@ struct TcParams {
   const __nv_bfloat16* k_new;        // [B][D] or null: row b is written to ring slot w_head of sequence b
   const __nv_bfloat16* v_new;
   int W;                             // ring capacity
+  // Level 2 (Eq.(6); lsa_l2.cu): key mask of the pages of the current table, [B][k][4] words (bit r of word
+  // r / 32 = row r of the page is one of the Top-k entries), or null: every valid row is attended
+  const uint32_t* l2_mask;
   // fused S8 (small batches): the grid meets at a counter barrier and merges the partials itself
   int fused;                     // 1: no combine kernel follows
   int n_attn;                    // CTAs that own tiles (the remaining CTAs of the grid only help with the merge)
@@ -191,6 +194,14 @@ __device__ __forceinline__ int tile_valid(const TcParams& p, const SeqView& v, i
   }
   t -= v.n_cur;
   return min(kTcTile, v.w_len - t * kTcTile);
+}
+
+// Level-2 key mask of tile t for the 32 rows [32 * q4, 32 * q4 + 32): all ones outside the page segment
+__device__ __forceinline__ uint32_t tile_keymask(const TcParams& p, const SeqView& v, int t, int q4) {
+  if (!p.l2_mask) return 0xffffffffu;
+  t -= v.t_hca;
+  if (t < 0 || t >= v.n_cur) return 0xffffffffu;
+  return p.l2_mask[((size_t)v.b * p.k + t) * 4 + q4];
 }
 
 // Iterates the (sequence, tile range) pieces of this CTA's share [f0, f1) of the flat tile list.

@@ -273,10 +273,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       b_last = b;
       const SeqView v = sm.view[b];
       int nv_next = tile_valid(p, v, t0);
+      uint32_t km_next = tile_keymask(p, v, t0, q4);
       for (int t = t0; t < t1; ++t) {
         const int buf = tcount & 1;
-        const bool valid = key < nv_next;
-        if (t + 1 < t1) nv_next = tile_valid(p, v, t + 1);        // global look-up overlaps the wait below
+        const bool valid = key < nv_next && ((km_next >> lane) & 1u);
+        if (t + 1 < t1) { nv_next = tile_valid(p, v, t + 1); km_next = tile_keymask(p, v, t + 1, q4); }   // global look-ups overlap the wait below
         float x[32];
         if (tr) TR(2, 0 + tcount * 5);
         mbar_wait(&sm.s_full[buf], (tcount >> 1) & 1, 30);
@@ -294,6 +295,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
         float f[32];
         if (t == t0) {
           tile_max(x, m_run);
+          // a first tile without any attended key (Level-2 mask) leaves -inf: keep the maximum finite so that
+          // 2^(x - m) is 0, not NaN; the first real logit then triggers the rescale path
+#pragma unroll
+          for (int h = 0; h < 32; ++h) m_run[h] = fmaxf(m_run[h], -1e30f);
         } else {
           bool over = false;
 #pragma unroll
@@ -380,7 +385,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             p.part_l[slot * kTcH + hh * 32 + j] = __uint_as_float(vreg[j]);
-            p.part_m[slot * kTcH + hh * 32 + j] = m_run[j];
+            p.part_m[slot * kTcH + hh * 32 + j] = m_run[j] <= -1e30f ? -INFINITY : m_run[j];   // no attended key: S8 skips the slot
           }
         }
       }

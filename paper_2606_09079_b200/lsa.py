@@ -33,6 +33,7 @@ EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
+           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2",
            "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
@@ -68,6 +69,10 @@ class lsa_l1_layer(C.Structure):
     _fields_ = [("W_dq", C.c_void_p), ("W_iuq", C.c_void_p), ("W_w", C.c_void_p)]
 
 
+class lsa_l2_config(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("c_I", C.c_int32), ("n_h", C.c_int32), ("k2", C.c_int32)]
+
+
 class lsa_l1_config(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_int32), ("d_c", C.c_int32), ("c_I", C.c_int32),
                 ("n_h", C.c_int32), ("threshold", C.c_float), ("layers", lsa_l1_layer * 4)]
@@ -98,6 +103,9 @@ def _load() -> C.CDLL:
     lib.lsa_l1_init.argtypes = [vp, C.POINTER(lsa_l1_config), C.POINTER(vp)]
     lib.lsa_l1_select.argtypes = [vp, vp, i32p, C.c_int32, vp, f32p]
     lib.lsa_set_indexer.argtypes = [vp, C.c_int32]
+    lib.lsa_l2_init.argtypes = [vp, C.POINTER(lsa_l2_config), C.POINTER(vp)]
+    lib.lsa_l2_select.argtypes = [vp, vp, vp, vp, vp]
+    lib.lsa_step_l2.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsa_last_error.argtypes = [vp]
     lib.lsa_last_error.restype = C.c_char_p
     lib.lsa_destroy.argtypes = [vp]
@@ -240,6 +248,34 @@ class LsaContext:
                 ptrs[b * L + l] = _dev_ptr(t, self.tdtype, "index_k") if t is not None and t.numel() else None
         self._keep += [list(layers), [list(x) for x in index_k]]
         self._check(_lib.lsa_l1_init(self._h, C.byref(cfg), ptrs))
+
+    def l2_init(self, index_k: Sequence[torch.Tensor], k2: int, c_I: int = 128, n_h: int = 64):
+        """Level 2 (Eq. 6): index_k[b] = [n_csa_b][c_I] bf16 CUDA tensor of this layer's compressed indexer keys."""
+        cfg = lsa_l2_config()
+        cfg.struct_size = C.sizeof(lsa_l2_config)
+        cfg.c_I, cfg.n_h, cfg.k2 = c_I, n_h, k2
+        ptrs = (C.c_void_p * self.B)()
+        for b in range(self.B):
+            t = index_k[b]
+            ptrs[b] = _dev_ptr(t, self.tdtype, "index_k") if t is not None and t.numel() else None
+        self._keep += [list(index_k)]
+        self._check(_lib.lsa_l2_init(self._h, C.byref(cfg), ptrs))
+        self.k2 = k2
+
+    def l2_select(self, q_idx: torch.Tensor, w_idx: torch.Tensor, want_entries: bool = True):
+        sel = torch.empty((self.B, self.k2), dtype=torch.int32, device=q_idx.device) if want_entries else None
+        sc = torch.empty((self.B, self.k2), dtype=torch.float32, device=q_idx.device) if want_entries else None
+        self._check(_lib.lsa_l2_select(self._h, _dev_ptr(q_idx, self.tdtype, "q_idx"), _dev_ptr(w_idx, torch.float32, "w_idx"),
+                                       None if sel is None else sel.data_ptr(), None if sc is None else sc.data_ptr()))
+        return sel, sc
+
+    def step_l2(self, q, h, k_new, v_new, q_idx, w_idx, out=None):
+        out = torch.empty_like(q) if out is None else out
+        self._check(_lib.lsa_step_l2(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(h, self.tdtype, "h"),
+                                     _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
+                                     _dev_ptr(q_idx, self.tdtype, "q_idx"), _dev_ptr(w_idx, torch.float32, "w_idx"),
+                                     _dev_ptr(out, self.tdtype, "out")))
+        return out
 
     def set_indexer(self, indexer: int):
         self._check(_lib.lsa_set_indexer(self._h, indexer))

@@ -45,7 +45,7 @@ def test_struct_layout_matches_header(lib_path, tmp_path):
     """Compile include/lsa.h with gcc and compare sizeof/offsetof with the ctypes mirror."""
     import subprocess
     from paper_2606_09079_b200 import lsa
-    structs = {"lsa_config": lsa.lsa_config, "lsa_seq_desc": lsa.lsa_seq_desc, "lsa_stats": lsa.lsa_stats,
+    structs = {"lsa_config": lsa.lsa_config, "lsa_seq_desc": lsa.lsa_seq_desc, "lsa_stats": lsa.lsa_stats, "lsa_l2_config": lsa.lsa_l2_config,
                "lsa_l1_layer": lsa.lsa_l1_layer, "lsa_l1_config": lsa.lsa_l1_config}
     lines = ['#include <stdio.h>', '#include <stddef.h>', f'#include "{HEADER}"', 'int main(void){']
     for name, cls in structs.items():
