@@ -184,6 +184,8 @@ def main():
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--max-ctas", type=int, default=0, help="cap on attention CTAs (0 = library default)")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
+    ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
+    ap.add_argument("--l2-k2", type=int, default=2048, help="Level-2 Top-k (entries per sequence and step)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -396,6 +398,47 @@ def main():
                   gbs=(key_bytes + w_bytes) / (l1_ms * 1e-3) / 1e9, frac_of_hbm_peak=(key_bytes + w_bytes) / (l1_ms * 1e-3) / 1e9 / load_peaks()["hbm_gbs"],
                   note="Eq.(1)-(5),(13) for all sequences of the config, warm L2 for the weights (same call repeated)")
 
+    # ---- optional: the step with Level 2 (NEXT-2): lsa_step_l2 through the same replica rotation ----
+    level2 = None
+    if args.l2 and rank == 0 and c.dtype == "bf16" and c.C == 128 and stats["attn_impl"] == 2:
+        from paper_2606_09079_b200.workloads import L2Inputs
+        l2in = L2Inputs(wl)
+        ik = [to_torch(K, "bf16").to(dev) for K in l2in.index_k]
+        for r in reps:
+            r.ctx.l2_init(ik, args.l2_k2)
+        qis = [to_torch(l2in.q_idx(i), "bf16").to(dev) for i in range(NIN)]
+        wis = [torch.from_numpy(l2in.w_idx(i)).to(dev) for i in range(NIN)]
+
+        def l2_step(i):
+            r = reps[i % R]
+            t, j = r.step, i % NIN
+            r.ctx.step_l2(qs[j], hs[(t // c.tau) % NIN], kns[j], vns[j], qis[j], wis[j], out)
+            r.step += 1
+        for i in range(max(3, 2 * R)):
+            l2_step(i_next + i)
+        i_next += max(3, 2 * R)
+        n_l2 = max(256, args.steps // 4)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(sc)
+        for i in range(n_l2):
+            l2_step(i_next + i)
+        e1.record(sc)
+        sf.synchronize(); sc.synchronize()
+        i_next += n_l2
+        l2_ms = e0.elapsed_time(e1) / n_l2
+        # the two Level-2 kernels alone (score + Top-k), same rotation
+        e0.record(sc)
+        for i in range(n_l2):
+            reps[i % R].ctx.l2_select(qis[i % NIN], wis[i % NIN], want_entries=False)
+        e1.record(sc)
+        sc.synchronize()
+        sel_ms = e0.elapsed_time(e1) / n_l2
+        key_bytes = sum(c.k_eff(b) for b in range(c.B)) * c.C * 128 * 2
+        level2 = dict(value=per_step_units / (l2_ms * 1e-3), unit=unit, ms_per_step=l2_ms, k2=args.l2_k2,
+                      resident_entries=sum(c.k_eff(b) for b in range(c.B)) * c.C, select_ms=sel_ms, index_key_bytes_per_step=key_bytes,
+                      note="lsa_step_l2: prestep + Level-2 score + Top-k2 + masked attention + combine; select_ms = the two Level-2 kernels alone")
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n, secs, threads = oracle_sample(wl, budget_s=15.0, max_steps=24)
@@ -416,7 +459,7 @@ def main():
                              ms_per_step=ms_e2e / n_e2e),
                     gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, l1_indexer=l1, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
+                    fetch=fetch, l1_indexer=l1, level2=level2, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
                     host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
         print(json.dumps(line))

@@ -236,6 +236,10 @@ int lsa_l2_init(lsa_ctx* ctx, const lsa_l2_config* cfg, const void* const* index
  *   sel_score   DEVICE [B][k2] fp32  or NULL: their native scores, -inf padding */
 int lsa_l2_select(lsa_ctx* ctx, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score);
 
+/* Blocking read-back of the row mask the last lsa_l2_select / lsa_step_l2 wrote for sequence seq:
+ * words HOST [k][4] uint32, bit r of word [j][r / 32] = row r of the j-th page of the current table is selected. */
+int lsa_l2_get_mask(lsa_ctx* ctx, int32_t seq, uint32_t* words);
+
 /* lsa_step with Level 2 between (d) and (e): the step's attention runs over HCA (+) the Top-k2 entries of the
  * current tables (+) window.  Other arguments and the step order as lsa_step. */
 int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,

@@ -625,6 +625,15 @@ extern "C" int lsa_l2_select(lsa_ctx* ctx, const void* q_idx, const float* w_idx
   return l2_select_impl(ctx, q_idx, w_idx, sel_entries, sel_score);
 }
 
+extern "C" int lsa_l2_get_mask(lsa_ctx* ctx, int32_t seq, uint32_t* words) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!ctx->l2) LSA_FAIL(ctx, LSA_ERR_STATE, "lsa_l2_init has not been called");
+  if (seq < 0 || seq >= ctx->B || !words) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad seq / null words");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  LSA_CUDA(ctx, cudaMemcpy(words, l2_mask(ctx->l2) + (size_t)seq * ctx->k * 4, (size_t)ctx->k * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  return LSA_OK;
+}
+
 extern "C" int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, const void* q_idx,
                            const float* w_idx, void* out) {
   if (!ctx) return LSA_ERR_STATE;

@@ -467,7 +467,8 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   TC_CUDA(cudaMemset(p.tlog, 0, (1 + 3 * 4096) * sizeof(unsigned long long)));
 #endif
   pl->smem = sizeof(TcSmem) + 1024;
-  TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
+  TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
+  TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
   TC_CUDA(cudaFuncSetAttribute(combine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCombineSmemMax));
   *out = pl;
   return 0;
@@ -516,7 +517,8 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   static const int no_pdl = getenv("LSA_NO_PDL") ? atoi(getenv("LSA_NO_PDL")) : 0;   // 1: combine, 2: attention, 3: both
   if (no_pdl & 2) lc.numAttrs = 0;
 #endif
-  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel, pl->map_pool, pl->map_q, prm));
+  if (prm.l2_mask) TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel<true>, pl->map_pool, pl->map_q, prm));
+  else TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel<false>, pl->map_pool, pl->map_q, prm));
   if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
   if (ev_mid1) TC_CUDA(cudaEventRecord(ev_mid1, st));
   if (prm.fused) {

@@ -17,6 +17,9 @@ namespace lsa {
 // K runs one tile ahead of V, so S(t+1) is computed (and K(t+2) is in flight) while the softmax of tile t
 // runs; with the 4-stage ring a V tile never waits behind the K tile that depends on its completion.
 
+// kMask: the Level-2 row mask (TcParams::l2_mask, lsa_l2.cu) is applied to the page tiles; the unmasked
+// instantiation carries none of that code.
+template <bool kMask>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_constant__ CUtensorMap map_q, TcParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -273,11 +276,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       b_last = b;
       const SeqView v = sm.view[b];
       int nv_next = tile_valid(p, v, t0);
-      uint32_t km_next = tile_keymask(p, v, t0, q4);
+      uint32_t km_next = kMask ? tile_keymask(p, v, t0, q4) : 0xffffffffu;
       for (int t = t0; t < t1; ++t) {
         const int buf = tcount & 1;
-        const bool valid = key < nv_next && ((km_next >> lane) & 1u);
-        if (t + 1 < t1) { nv_next = tile_valid(p, v, t + 1); km_next = tile_keymask(p, v, t + 1, q4); }   // global look-ups overlap the wait below
+        const bool valid = kMask ? (key < nv_next && ((km_next >> lane) & 1u)) : key < nv_next;
+        if (t + 1 < t1) {                                         // global look-ups overlap the wait below
+          nv_next = tile_valid(p, v, t + 1);
+          if (kMask) km_next = tile_keymask(p, v, t + 1, q4);
+        }
         float x[32];
         if (tr) TR(2, 0 + tcount * 5);
         mbar_wait(&sm.s_full[buf], (tcount >> 1) & 1, 30);
@@ -297,8 +303,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
           tile_max(x, m_run);
           // a first tile without any attended key (Level-2 mask) leaves -inf: keep the maximum finite so that
           // 2^(x - m) is 0, not NaN; the first real logit then triggers the rescale path
+          if (kMask) {
 #pragma unroll
-          for (int h = 0; h < 32; ++h) m_run[h] = fmaxf(m_run[h], -1e30f);
+            for (int h = 0; h < 32; ++h) m_run[h] = fmaxf(m_run[h], -1e30f);
+          }
         } else {
           bool over = false;
 #pragma unroll
@@ -385,7 +393,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             p.part_l[slot * kTcH + hh * 32 + j] = __uint_as_float(vreg[j]);
-            p.part_m[slot * kTcH + hh * 32 + j] = m_run[j] <= -1e30f ? -INFINITY : m_run[j];   // no attended key: S8 skips the slot
+            p.part_m[slot * kTcH + hh * 32 + j] = (kMask && m_run[j] <= -1e30f) ? -INFINITY : m_run[j];   // no attended key: S8 skips the slot
           }
         }
       }

@@ -228,6 +228,128 @@ l2_topk_kernel(const SeqDev* __restrict__ seqs, const int* __restrict__ tbl_chun
   }
 }
 
+
+// Mask-only fast path (no entry list asked for, k * 128 <= 16384): a thread keeps PER consecutive scores in registers
+// (position = tid * PER + j, so thread order is entry-id order); the k2-th largest 32-bit ordered score is found by a
+// 4-pass 8-bit MSB radix select (warp-aggregated shared-memory histograms, bins scanned by one warp), and ties AT the
+// cut-off are resolved by position with one block-wide scan - the same (score desc, entry id asc) rule as the
+// general kernel, without sorting the winners.  Each mask word is written exactly once.
+template <int PER>
+__global__ void __launch_bounds__(1024)
+l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ score, int k, int k2, uint32_t* __restrict__ mask) {
+  __shared__ unsigned hist[256];
+  __shared__ unsigned wsum[33];
+  __shared__ unsigned s_prefix, s_need;
+  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_wait();
+  pdl_launch_dependents();
+  const SeqDev& sq = seqs[b];
+  const int n = sq.n_tbl[sq.cur_buf] * kL2C;                 // multiple of 128, PER divides 128
+  const float* sc = score + (size_t)b * k * kL2C;
+  uint32_t* mk = mask + (size_t)b * k * 4;
+  const int base = tid * PER;
+  uint32_t key[PER];                                         // 0 = not an entry (float_to_ordered never returns 0)
+#pragma unroll
+  for (int j = 0; j < PER; j += 4) {
+    float4 v = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+    if (base + j < n) v = *reinterpret_cast<const float4*>(sc + base + j);
+    key[j] = v.x == -INFINITY ? 0u : float_to_ordered(v.x);
+    key[j + 1] = v.y == -INFINITY ? 0u : float_to_ordered(v.y);
+    key[j + 2] = v.z == -INFINITY ? 0u : float_to_ordered(v.z);
+    key[j + 3] = v.w == -INFINITY ? 0u : float_to_ordered(v.w);
+  }
+  // block-wide exclusive scan of one value per thread (thread order); returns the prefix, *total = the block sum
+  auto block_scan = [&](unsigned v, unsigned* total) -> unsigned {
+    unsigned incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+    __syncthreads();                                         // wsum may still be read from an earlier call
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+      const unsigned w = wsum[lane];
+      unsigned wi = w;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, wi, o); if (lane >= o) wi += t; }
+      wsum[lane] = wi - w;
+      if (lane == 31) wsum[32] = wi;
+    }
+    __syncthreads();
+    *total = wsum[32];
+    return wsum[warp] + incl - v;
+  };
+  unsigned n_valid_thr = 0;
+#pragma unroll
+  for (int j = 0; j < PER; ++j) n_valid_thr += key[j] != 0u;
+  unsigned n_valid;
+  block_scan(n_valid_thr, &n_valid);
+  const unsigned want = min((unsigned)k2, n_valid);
+  uint32_t thr = 0xffffffffu;                                // want == 0: nothing reaches the cut-off
+  unsigned need_eq = 0;
+  if (want > 0) {
+    if (tid == 0) { s_prefix = 0u; s_need = want; }
+    uint32_t pmask = 0u;
+    for (int byte = 3; byte >= 0; --byte) {
+      if (tid < 256) hist[tid] = 0u;
+      __syncthreads();
+      const uint32_t prefix = s_prefix;
+#pragma unroll
+      for (int j = 0; j < PER; ++j) {
+        const bool act = (key[j] & pmask) == prefix;          // key 0 only matches while prefix == 0 and lands in bin 0 ...
+        const unsigned bin = (key[j] >> (8 * byte)) & 255u;   // ... behind every real key, and want <= n_valid keeps it out
+        const unsigned amask = __ballot_sync(0xffffffffu, act);
+        if (act) {
+          const unsigned peers = __match_any_sync(amask, bin);
+          if (lane == __ffs(peers) - 1) atomicAdd(&hist[bin], __popc(peers));
+        }
+      }
+      __syncthreads();
+      if (warp == 0) {                                        // lane l owns bins 255 - 8l .. 248 - 8l (descending)
+        unsigned h[8], mine = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { h[i] = hist[255 - 8 * lane - i]; mine += h[i]; }
+        unsigned incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+        const unsigned need = s_need;
+        const unsigned before = incl - mine;                  // keys in higher bins than this lane's
+        if (before < need && need <= incl) {                  // the cut-off digit is one of this lane's bins
+          unsigned cum = before;
+          int d = 0;
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            if (cum + h[i] >= need) { d = 255 - 8 * lane - i; break; }
+            cum += h[i];
+          }
+          s_need = need - cum;
+          s_prefix = prefix | ((uint32_t)d << (8 * byte));
+        }
+      }
+      pmask |= 0xffu << (8 * byte);
+      __syncthreads();
+    }
+    thr = s_prefix;
+    need_eq = s_need;                                         // how many of the keys == thr are taken (lowest positions)
+  }
+  unsigned n_eq_thr = 0;
+#pragma unroll
+  for (int j = 0; j < PER; ++j) n_eq_thr += (key[j] == thr);
+  unsigned dummy;
+  unsigned eq_before = block_scan(n_eq_thr, &dummy);
+  uint32_t bits = 0u;
+#pragma unroll
+  for (int j = 0; j < PER; ++j) {
+    bool take = want > 0 && key[j] > thr;
+    if (want > 0 && key[j] == thr) { take = eq_before < need_eq; ++eq_before; }
+    if (take) bits |= 1u << ((base + j) & 31);
+  }
+#pragma unroll
+  for (int o = 1; o < 32 / PER; o <<= 1) bits |= __shfl_xor_sync(0xffffffffu, bits, o);
+  const int word = base >> 5;
+  if ((lane & (32 / PER - 1)) == 0 && word < k * 4) mk[word] = bits;
+  for (int w = 1024 * PER / 32 + tid; w < k * 4; w += 1024) mk[w] = 0u;
+}
+
 // ---- host -------------------------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -319,8 +441,16 @@ int l2_select(L2Plan* pl, const SeqDev* d_seqs, const void* q_idx, const float* 
   const long long tiles = (long long)in.B * in.k;
   const int grid = (int)std::max(1ll, std::min<long long>(in.n_sms, tiles));
   L2_CUDA(launch_pdl(l2_score_kernel, dim3(grid), dim3(kL2Threads), pl->smem, st, pl->map_q, sp));
-  L2_CUDA(launch_pdl(l2_topk_kernel, dim3(in.B), dim3(1024), 0, st, d_seqs, in.tbl_chunk, (const float*)pl->score, in.k, in.k2, pl->mask,
-                     sel_entries, sel_score));
+  const int n_max = in.k * kL2C;
+  if (!sel_entries && !sel_score && n_max <= 16384) {       // mask only: keys in registers, no sort
+    const float* sc = pl->score;
+    if (n_max <= 4096) L2_CUDA(launch_pdl(l2_topk_mask_kernel<4>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, in.k, in.k2, pl->mask));
+    else if (n_max <= 8192) L2_CUDA(launch_pdl(l2_topk_mask_kernel<8>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, in.k, in.k2, pl->mask));
+    else L2_CUDA(launch_pdl(l2_topk_mask_kernel<16>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, in.k, in.k2, pl->mask));
+  } else {
+    L2_CUDA(launch_pdl(l2_topk_kernel, dim3(in.B), dim3(1024), 0, st, d_seqs, in.tbl_chunk, (const float*)pl->score, in.k, in.k2, pl->mask,
+                       sel_entries, sel_score));
+  }
   *launches += 2;
   return 0;
 }

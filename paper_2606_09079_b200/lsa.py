@@ -33,7 +33,7 @@ EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
-           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2",
+           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask",
            "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
@@ -105,6 +105,7 @@ def _load() -> C.CDLL:
     lib.lsa_set_indexer.argtypes = [vp, C.c_int32]
     lib.lsa_l2_init.argtypes = [vp, C.POINTER(lsa_l2_config), C.POINTER(vp)]
     lib.lsa_l2_select.argtypes = [vp, vp, vp, vp, vp]
+    lib.lsa_l2_get_mask.argtypes = [vp, C.c_int32, vp]
     lib.lsa_step_l2.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsa_last_error.argtypes = [vp]
     lib.lsa_last_error.restype = C.c_char_p
@@ -268,6 +269,14 @@ class LsaContext:
         self._check(_lib.lsa_l2_select(self._h, _dev_ptr(q_idx, self.tdtype, "q_idx"), _dev_ptr(w_idx, torch.float32, "w_idx"),
                                        None if sel is None else sel.data_ptr(), None if sc is None else sc.data_ptr()))
         return sel, sc
+
+    def l2_mask(self, seq: int):
+        """Blocking: the row mask of the last Level-2 selection, as a bool array [k][C = 128]."""
+        import numpy as np
+        words = np.zeros(self.k * 4, dtype=np.uint32)
+        self._check(_lib.lsa_l2_get_mask(self._h, seq, words.ctypes.data))
+        bits = (words[:, None] >> np.arange(32, dtype=np.uint32)[None, :]) & 1
+        return bits.reshape(self.k, 128).astype(bool)
 
     def step_l2(self, q, h, k_new, v_new, q_idx, w_idx, out=None):
         out = torch.empty_like(q) if out is None else out

@@ -52,12 +52,21 @@ def _oracle_l2(orc, cfg, l2, t, k2):
     return sels, ids, scs
 
 
-@pytest.mark.parametrize("k,k2", [(12, 37), (12, 1), (40, 700), (40, 4096)])
-def test_l2_select_and_attention_match_oracle(k, k2):
+def _mask_of(cfg, orc, b, entries):
+    m = np.zeros((cfg.k, cfg.C), dtype=bool)
+    slot = {c: j for j, (c, _) in enumerate(orc.pool.cur[b])}          # tables are in ascending chunk id
+    for s in entries:
+        m[slot[int(s) // cfg.C], int(s) % cfg.C] = True
+    return m
+
+
+@pytest.mark.parametrize("k,k2,L", [(12, 37, (20096, 4992)), (12, 1, (20096, 4992)), (40, 700, (20096, 4992)), (40, 4096, (20096, 4992)),
+                                    (72, 1500, (40960, 4992))])
+def test_l2_select_and_attention_match_oracle(k, k2, L):
     """API level: lsa_l2_select then lsa_decode_attention.  k = 12: 1536 + 1248 entries (sort-all path); k = 40: 5024
     entries in sequence 0 (radix-select path), whose last chunk is partial (32 valid rows); k2 = 4096 covers all of
     sequence 1 (1248 entries): every valid row selected.  k2 = 1 / 37 leave most pages without a selected row."""
-    cfg, wl, l2, rig = _rig(k, k2)
+    cfg, wl, l2, rig = _rig(k, k2, L=L)
     orc = make_oracle(wl)
     tol = attn_tolerance("bf16")
     compared = 0
@@ -78,6 +87,13 @@ def test_l2_select_and_attention_match_oracle(k, k2):
         out = rig.ctx.decode_attention(rig.dev(q))
         out_plain = rig.ctx.decode_attention(rig.dev(q))      # the selection is one-shot
         rig.ctx.sync()
+        masks = [rig.ctx.l2_mask(b) for b in range(cfg.B)]    # written by the general (sorting) kernel
+        rig.ctx.l2_select(qi, wi, want_entries=False)         # mask-only fast kernel (keys in registers, radix select)
+        out_fast = rig.ctx.decode_attention(rig.dev(q))
+        for b in range(cfg.B):
+            assert np.array_equal(rig.ctx.l2_mask(b), masks[b]), f"t {t} seq {b}: the two Top-k kernels disagree"
+            assert np.array_equal(masks[b], _mask_of(cfg, orc, b, [e for e in sel[b].cpu().tolist() if e >= 0]))
+        assert torch.equal(out_fast, out)
         sel, sc = sel.cpu().numpy(), sc.cpu().numpy().astype(np.float64)
         o_sels, o_ids, o_scs = _oracle_l2(orc, cfg, l2, t, k2)
         same = True
@@ -113,6 +129,9 @@ def test_l2_before_any_trigger_attends_hca_and_window_only():
     q = wl.q(0)
     sel, sc = rig.ctx.l2_select(qi, wi)                       # empty tables: nothing to select
     out = rig.ctx.decode_attention(rig.dev(q))
+    rig.ctx.l2_select(qi, wi, want_entries=False)
+    assert not rig.ctx.l2_mask(0).any() and not rig.ctx.l2_mask(1).any()
+    assert torch.equal(rig.ctx.decode_attention(rig.dev(q)), out)
     rig.ctx.sync()
     assert torch.all(sel == -1) and torch.all(sc == -float("inf"))
     ref, _ = l2_decode_attention(orc, q, [[] for _ in range(cfg.B)])
