@@ -36,8 +36,11 @@ struct L2ScoreParams {
   const CUtensorMap* k_maps;     // [B]: index keys [n_csa][128] bf16 as (64, rows, 2 d-blocks)
   const float* w_idx;            // [B][64]
   float* score;                  // [B][k * 128]; rows past the chunk's valid entries get -inf
+  unsigned* ghist;               // [B][4096] or null: entries per top-12-bit bin of the ordered score (for the mask-only
+                                 // Top-k kernel, which zeroes it again); null when the general Top-k kernel follows
   int B, k;
 };
+constexpr int kL2Bins = 4096;
 
 struct L2Smem {
   alignas(1024) unsigned char q[16384];                          // [2 d-blocks][64 heads][128 B], SW128
@@ -179,6 +182,15 @@ l2_score_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant
         for (int h = 0; h < kL2H; ++h) pre = fmaf(w[h], fmaxf(x[h], 0.f), pre);          // Score_native (l.71-75)
         if (first + row >= n_csa) pre = -INFINITY;                                         // not an entry (M1)
         p.score[((size_t)b * p.k + t) * kL2C + row] = pre;
+        if (p.ghist) {                                                                     // first radix digit, counted where the scores are
+          const bool ok = pre != -INFINITY;
+          const unsigned bin = float_to_ordered(pre) >> 20;
+          const unsigned am = __ballot_sync(0xffffffffu, ok);
+          if (ok) {
+            const unsigned peers = __match_any_sync(am, bin);
+            if (lane == __ffs(peers) - 1) atomicAdd(p.ghist + (size_t)b * kL2Bins + bin, (unsigned)__popc(peers));
+          }
+        }
         ++n_s;
       }
     }
@@ -229,17 +241,76 @@ l2_topk_kernel(const SeqDev* __restrict__ seqs, const int* __restrict__ tbl_chun
 }
 
 
-// Mask-only fast path (no entry list asked for, k * 128 <= 16384): a thread keeps PER consecutive scores in registers
-// (position = tid * PER + j, so thread order is entry-id order); the k2-th largest 32-bit ordered score is found by a
-// 4-pass 8-bit MSB radix select (warp-aggregated shared-memory histograms, bins scanned by one warp), and ties AT the
-// cut-off are resolved by position with one block-wide scan - the same (score desc, entry id asc) rule as the
-// general kernel, without sorting the winners.  Each mask word is written exactly once.
+// Mask-only fast path (no entry list asked for, k * 128 <= 16384).  The first radix digit - the top 12 bits of the
+// ordered score - is counted by the score kernel's CTAs, which hold the scores in registers (warp-aggregated global
+// atomics into ghist[b][4096]); this kernel (one block per sequence, a thread keeps PER consecutive scores in registers:
+// position = tid * PER + j, so thread order is entry-id order)
+//   1. reads and re-zeroes the histogram, 4 bins per thread; one block scan gives the number of entries and the bin
+//      that holds the k2-th largest score,
+//   2. collects the keys of that bin (about n / 20 of them) into shared memory and finishes the select on those with
+//      3 passes of 8 bits (match.any-aggregated shared-memory histograms, bins scanned by one warp); a bin with more than
+//      kL2Cand keys runs the same passes over the register keys instead,
+//   3. marks key > cut-off, and resolves ties AT the cut-off by position with one block scan - the same
+//      (score desc, entry id asc) rule as the general kernel, without sorting the winners.
+// Each mask word is written exactly once.  History: 8-pass radix + sort of the winners 61 us per select at 8192 entries;
+// all 4 passes in this block 16.7 us (ncu: ~35 k cycles behind ~560 MATCH.ANY + ATOMS on one SM); see profiles/r01_level2.md.
+constexpr int kL2Cand = 2048;
+
+// byte_hi .. 0: 8-bit MSB radix passes over this thread's N keys; keys with (key & pmask) != *s_prefix are out.
+// In: *s_prefix / *s_need = digits fixed so far / rank wanted among the matching keys.  Out: the full key / how many
+// keys equal to it are taken.  All threads of the block call it.
+template <int N>
+__device__ __forceinline__ void l2_radix_passes(const uint32_t (&key)[N], uint32_t pmask, int byte_hi, unsigned* hist, unsigned* s_prefix,
+                                                unsigned* s_need, int tid, int lane, int warp) {
+  for (int byte = byte_hi; byte >= 0; --byte) {
+    if (tid < 256) hist[tid] = 0u;
+    __syncthreads();
+    const uint32_t prefix = *s_prefix;
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      const bool act = (key[j] & pmask) == prefix;
+      const unsigned bin = (key[j] >> (8 * byte)) & 255u;
+      const unsigned amask = __ballot_sync(0xffffffffu, act);
+      if (act) {
+        const unsigned peers = __match_any_sync(amask, bin);
+        if (lane == __ffs(peers) - 1) atomicAdd(&hist[bin], (unsigned)__popc(peers));
+      }
+    }
+    __syncthreads();
+    if (warp == 0) {                                        // lane l owns bins 255 - 8l .. 248 - 8l (descending)
+      unsigned h[8], mine = 0;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { h[i] = hist[255 - 8 * lane - i]; mine += h[i]; }
+      unsigned incl = mine;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+      const unsigned need = *s_need;
+      const unsigned before = incl - mine;                  // keys in higher bins than this lane's
+      if (before < need && need <= incl) {                  // the cut-off digit is one of this lane's bins
+        unsigned cum = before;
+        int d = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          if (cum + h[i] >= need) { d = 255 - 8 * lane - i; break; }
+          cum += h[i];
+        }
+        *s_need = need - cum;
+        *s_prefix = prefix | ((uint32_t)d << (8 * byte));
+      }
+    }
+    pmask |= 0xffu << (8 * byte);
+    __syncthreads();
+  }
+}
+
 template <int PER>
 __global__ void __launch_bounds__(1024)
-l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ score, int k, int k2, uint32_t* __restrict__ mask) {
+l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ score, unsigned* __restrict__ ghist, int k, int k2,
+                    uint32_t* __restrict__ mask) {
   __shared__ unsigned hist[256];
   __shared__ unsigned wsum[33];
-  __shared__ unsigned s_prefix, s_need;
+  __shared__ uint32_t cand[kL2Cand];
+  __shared__ unsigned s_prefix, s_need, s_m, s_cnt;
   const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   pdl_wait();
   pdl_launch_dependents();
@@ -248,6 +319,9 @@ l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ s
   const float* sc = score + (size_t)b * k * kL2C;
   uint32_t* mk = mask + (size_t)b * k * 4;
   const int base = tid * PER;
+  uint4* gh = reinterpret_cast<uint4*>(ghist + (size_t)b * kL2Bins) + tid;     // bins 4 tid .. 4 tid + 3
+  const uint4 h4 = *gh;
+  *gh = make_uint4(0u, 0u, 0u, 0u);                          // ready for the next step's score kernel
   uint32_t key[PER];                                         // 0 = not an entry (float_to_ordered never returns 0)
 #pragma unroll
   for (int j = 0; j < PER; j += 4) {
@@ -278,59 +352,52 @@ l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ s
     *total = wsum[32];
     return wsum[warp] + incl - v;
   };
-  unsigned n_valid_thr = 0;
-#pragma unroll
-  for (int j = 0; j < PER; ++j) n_valid_thr += key[j] != 0u;
+  // 1. the 12-bit digit of the cut-off: bins ascend with tid, the select wants the LARGEST keys
+  const unsigned hs = h4.x + h4.y + h4.z + h4.w;
   unsigned n_valid;
-  block_scan(n_valid_thr, &n_valid);
+  const unsigned below = block_scan(hs, &n_valid);
   const unsigned want = min((unsigned)k2, n_valid);
   uint32_t thr = 0xffffffffu;                                // want == 0: nothing reaches the cut-off
   unsigned need_eq = 0;
   if (want > 0) {
-    if (tid == 0) { s_prefix = 0u; s_need = want; }
-    uint32_t pmask = 0u;
-    for (int byte = 3; byte >= 0; --byte) {
-      if (tid < 256) hist[tid] = 0u;
-      __syncthreads();
-      const uint32_t prefix = s_prefix;
+    if (tid == 0) s_cnt = 0u;
+    unsigned cum = n_valid - below - hs;                     // entries in the bins above this thread's four
+    const unsigned hb[4] = {h4.w, h4.z, h4.y, h4.x};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      if (cum < want && want <= cum + hb[i]) { s_prefix = (uint32_t)(4 * tid + 3 - i) << 20; s_need = want - cum; s_m = hb[i]; }
+      cum += hb[i];
+    }
+    __syncthreads();
+    const uint32_t top = s_prefix;
+    if (s_m <= (unsigned)kL2Cand) {
+      // 2. the keys of that bin -> shared memory (any order: only their values matter from here on)
 #pragma unroll
       for (int j = 0; j < PER; ++j) {
-        const bool act = (key[j] & pmask) == prefix;          // key 0 only matches while prefix == 0 and lands in bin 0 ...
-        const unsigned bin = (key[j] >> (8 * byte)) & 255u;   // ... behind every real key, and want <= n_valid keeps it out
-        const unsigned amask = __ballot_sync(0xffffffffu, act);
-        if (act) {
-          const unsigned peers = __match_any_sync(amask, bin);
-          if (lane == __ffs(peers) - 1) atomicAdd(&hist[bin], __popc(peers));
+        const bool is = (key[j] & 0xfff00000u) == top && key[j] != 0u;
+        const unsigned bal = __ballot_sync(0xffffffffu, is);
+        if (is) {
+          const int leader = __ffs(bal) - 1;
+          unsigned pos0 = 0;
+          if (lane == leader) pos0 = atomicAdd(&s_cnt, (unsigned)__popc(bal));
+          pos0 = __shfl_sync(bal, pos0, leader);
+          const unsigned idx = pos0 + __popc(bal & ((1u << lane) - 1u));
+          if (idx < (unsigned)kL2Cand) cand[idx] = key[j];
         }
       }
       __syncthreads();
-      if (warp == 0) {                                        // lane l owns bins 255 - 8l .. 248 - 8l (descending)
-        unsigned h[8], mine = 0;
+      const unsigned m = min(s_cnt, (unsigned)kL2Cand);
+      uint32_t ck[kL2Cand / 1024];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { h[i] = hist[255 - 8 * lane - i]; mine += h[i]; }
-        unsigned incl = mine;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
-        const unsigned need = s_need;
-        const unsigned before = incl - mine;                  // keys in higher bins than this lane's
-        if (before < need && need <= incl) {                  // the cut-off digit is one of this lane's bins
-          unsigned cum = before;
-          int d = 0;
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            if (cum + h[i] >= need) { d = 255 - 8 * lane - i; break; }
-            cum += h[i];
-          }
-          s_need = need - cum;
-          s_prefix = prefix | ((uint32_t)d << (8 * byte));
-        }
-      }
-      pmask |= 0xffu << (8 * byte);
-      __syncthreads();
+      for (int j = 0; j < kL2Cand / 1024; ++j) ck[j] = (unsigned)(tid + 1024 * j) < m ? cand[tid + 1024 * j] : ~top;   // padding never matches
+      l2_radix_passes(ck, 0xfff00000u, 2, hist, &s_prefix, &s_need, tid, lane, warp);
+    } else {
+      l2_radix_passes(key, 0xfff00000u, 2, hist, &s_prefix, &s_need, tid, lane, warp);
     }
     thr = s_prefix;
     need_eq = s_need;                                         // how many of the keys == thr are taken (lowest positions)
   }
+  // 3. mark
   unsigned n_eq_thr = 0;
 #pragma unroll
   for (int j = 0; j < PER; ++j) n_eq_thr += (key[j] == thr);
@@ -363,6 +430,7 @@ struct L2Plan {
   const void* q_cached = nullptr;
   float* score = nullptr;              // [B][k * 128]
   uint32_t* mask = nullptr;            // [B][k][4]
+  unsigned* ghist = nullptr;           // [B][4096], all zero between steps
   size_t smem = 0;
 };
 
@@ -403,6 +471,8 @@ int l2_create(const L2Init& init, L2Plan** out, std::string* msg) {
   L2_CUDA(cudaMalloc(&pl->score, (size_t)B * init.k * kL2C * sizeof(float)));
   L2_CUDA(cudaMalloc(&pl->mask, (size_t)B * init.k * 4 * sizeof(uint32_t)));
   L2_CUDA(cudaMemset(pl->mask, 0, (size_t)B * init.k * 4 * sizeof(uint32_t)));
+  L2_CUDA(cudaMalloc(&pl->ghist, (size_t)B * kL2Bins * sizeof(unsigned)));
+  L2_CUDA(cudaMemset(pl->ghist, 0, (size_t)B * kL2Bins * sizeof(unsigned)));
   std::vector<CUtensorMap> maps((size_t)B);
   for (int b = 0; b < B; ++b) {
     const void* ptr = init.index_k[b];
@@ -424,7 +494,7 @@ const uint32_t* l2_mask(const L2Plan* pl) { return pl->mask; }
 
 void l2_destroy(L2Plan* pl) {
   if (!pl) return;
-  cudaFree(pl->d_maps); cudaFree(pl->score); cudaFree(pl->mask);
+  cudaFree(pl->d_maps); cudaFree(pl->score); cudaFree(pl->mask); cudaFree(pl->ghist);
   delete pl;
 }
 
@@ -438,15 +508,17 @@ int l2_select(L2Plan* pl, const SeqDev* d_seqs, const void* q_idx, const float* 
   L2ScoreParams sp{};
   sp.seqs = d_seqs; sp.tbl_chunk = in.tbl_chunk; sp.k_maps = pl->d_maps; sp.w_idx = w_idx; sp.score = pl->score;
   sp.B = in.B; sp.k = in.k;
+  const int n_max = in.k * kL2C;
+  const bool mask_only = !sel_entries && !sel_score && n_max <= 16384;     // keys in registers, no sort
+  sp.ghist = mask_only ? pl->ghist : nullptr;
   const long long tiles = (long long)in.B * in.k;
   const int grid = (int)std::max(1ll, std::min<long long>(in.n_sms, tiles));
   L2_CUDA(launch_pdl(l2_score_kernel, dim3(grid), dim3(kL2Threads), pl->smem, st, pl->map_q, sp));
-  const int n_max = in.k * kL2C;
-  if (!sel_entries && !sel_score && n_max <= 16384) {       // mask only: keys in registers, no sort
+  if (mask_only) {
     const float* sc = pl->score;
-    if (n_max <= 4096) L2_CUDA(launch_pdl(l2_topk_mask_kernel<4>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, in.k, in.k2, pl->mask));
-    else if (n_max <= 8192) L2_CUDA(launch_pdl(l2_topk_mask_kernel<8>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, in.k, in.k2, pl->mask));
-    else L2_CUDA(launch_pdl(l2_topk_mask_kernel<16>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, in.k, in.k2, pl->mask));
+    if (n_max <= 4096) L2_CUDA(launch_pdl(l2_topk_mask_kernel<4>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, pl->ghist, in.k, in.k2, pl->mask));
+    else if (n_max <= 8192) L2_CUDA(launch_pdl(l2_topk_mask_kernel<8>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, pl->ghist, in.k, in.k2, pl->mask));
+    else L2_CUDA(launch_pdl(l2_topk_mask_kernel<16>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, pl->ghist, in.k, in.k2, pl->mask));
   } else {
     L2_CUDA(launch_pdl(l2_topk_kernel, dim3(in.B), dim3(1024), 0, st, d_seqs, in.tbl_chunk, (const float*)pl->score, in.k, in.k2, pl->mask,
                        sel_entries, sel_score));
