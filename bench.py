@@ -437,7 +437,7 @@ def main():
         key_bytes = sum(c.k_eff(b) for b in range(c.B)) * c.C * 128 * 2
         level2 = dict(value=per_step_units / (l2_ms * 1e-3), unit=unit, ms_per_step=l2_ms, k2=args.l2_k2,
                       resident_entries=sum(c.k_eff(b) for b in range(c.B)) * c.C, select_ms=sel_ms, index_key_bytes_per_step=key_bytes,
-                      note="lsa_step_l2: prestep + Level-2 score + Top-k2 + masked attention + combine; select_ms = the two Level-2 kernels alone")
+                      note="lsa_step_l2: Level-2 score + Top-k2 + masked attention (S6 / append folded in) + combine; select_ms = the two Level-2 kernels alone, PDL-chained")
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

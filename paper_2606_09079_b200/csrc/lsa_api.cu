@@ -536,7 +536,8 @@ extern "C" int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, floa
   return attention_impl(ctx, q, out, lse);
 }
 
-static int l2_select_impl(lsa_ctx* c, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score);
+static int l2_select_impl(lsa_ctx* c, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score,
+                          const unsigned* folded_swap = nullptr);
 
 static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out,
                      const void* q_idx, const float* w_idx) {
@@ -550,7 +551,7 @@ static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_n
     if (c->step[b] % c->cfg.tau == 0) ids[n_fire++] = b;           // S0
   if (n_fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
   int rc;
-  if (n_fire == 0 && c->attn_impl == LSA_ATTN_TCGEN05 && !q_idx) {
+  if (n_fire == 0 && c->attn_impl == LSA_ATTN_TCGEN05) {
     // no trigger this step: (a) and (d) ride on the attention launch itself (one kernel less per step).  On a
     // trigger step the residency pass must see the swapped tables, so they stay a kernel of their own.
     TcPrestep pre{};
@@ -559,6 +560,8 @@ static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_n
       LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_fetch, 0));
       for (int i = 0; i < 8; ++i) pre.swap[i] = words[i];
     }
+    // Level 2 scores the tables as this launch will see them (the swap rides on the attention launch)
+    if (q_idx && (rc = l2_select_impl(c, q_idx, w_idx, nullptr, nullptr, pre.swap))) return rc;
     pre.k_new = k_new; pre.v_new = v_new;
     if (k_new) mirror_append(c);
     if ((rc = attention_impl(c, q, out, nullptr, &pre))) return rc;
@@ -606,14 +609,15 @@ extern "C" int lsa_l2_init(lsa_ctx* ctx, const lsa_l2_config* cfg, const void* c
   return LSA_OK;
 }
 
-static int l2_select_impl(lsa_ctx* c, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score) {
+static int l2_select_impl(lsa_ctx* c, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score,
+                          const unsigned* folded_swap) {
   if (!c->l2) LSA_FAIL(c, LSA_ERR_STATE, "lsa_l2_init has not been called");
   if (!q_idx || !w_idx) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q_idx / w_idx");
-  int rc = prestep_impl(c, false, nullptr, nullptr);                // the tables the next attention launch will read
+  int rc = folded_swap ? 0 : prestep_impl(c, false, nullptr, nullptr);   // the tables the next attention launch will read
   if (rc) return rc;
   std::string msg;
   int launches = 0;
-  rc = l2_select(c->l2, c->d_seqs, q_idx, w_idx, sel_entries, sel_score, c->sc, &launches, &msg);
+  rc = l2_select(c->l2, c->d_seqs, q_idx, w_idx, sel_entries, sel_score, folded_swap, c->sc, &launches, &msg);
   c->attn_launches += launches;
   if (rc != 0) LSA_FAIL(c, LSA_ERR_CUDA, "Level 2: %s", msg.c_str());
   c->l2_armed = true;

@@ -39,8 +39,17 @@ struct L2ScoreParams {
   unsigned* ghist;               // [B][4096] or null: entries per top-12-bit bin of the ordered score (for the mask-only
                                  // Top-k kernel, which zeroes it again); null when the general Top-k kernel follows
   int B, k;
+  unsigned swap[8];              // bit b: sequence b's staged table is the one this step attends (S6 folded into the
+                                 // attention launch that follows: the records still show it as pending)
 };
 constexpr int kL2Bins = 4096;
+
+struct L2Swap { unsigned w[8]; };
+// which table buffer the attention launch of this step will read
+__device__ __forceinline__ int l2_cur_buf(const SeqDev& s, const unsigned* swap, int b) {
+  const bool sw = ((swap[b >> 5] >> (b & 31)) & 1u) && s.pending;
+  return sw ? 1 - s.cur_buf : s.cur_buf;
+}
 
 struct L2Smem {
   alignas(1024) unsigned char q[16384];                          // [2 d-blocks][64 heads][128 B], SW128
@@ -66,7 +75,7 @@ struct L2Cursor {
       t0 = f - b * p.k;
       const int end = min(f1, (b + 1) * p.k);
       const SeqDev& s = p.seqs[b];
-      cur = s.cur_buf;
+      cur = l2_cur_buf(s, p.swap, b);
       t1 = min(end - b * p.k, s.n_tbl[cur]);
       f = end;
       if (t0 < t1) return true;
@@ -207,14 +216,14 @@ l2_score_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant
 // One block per sequence.  The table is in ascending chunk id, so position i = slot * 128 + row orders the entries
 // exactly as their ids s = chunk * 128 + row do: key = (~ordered(score), i) gives (score desc, entry id asc).
 __global__ void __launch_bounds__(1024)
-l2_topk_kernel(const SeqDev* __restrict__ seqs, const int* __restrict__ tbl_chunk, const float* __restrict__ score, int k, int k2,
+l2_topk_kernel(const SeqDev* __restrict__ seqs, L2Swap swap, const int* __restrict__ tbl_chunk, const float* __restrict__ score, int k, int k2,
                uint32_t* __restrict__ mask, int32_t* __restrict__ sel_entries, float* __restrict__ sel_score) {
   __shared__ SelectSmem sm;
   const int b = blockIdx.x;
   pdl_wait();
   pdl_launch_dependents();
   const SeqDev& sq = seqs[b];
-  const int cur = sq.cur_buf, n_cur = sq.n_tbl[cur];
+  const int cur = l2_cur_buf(sq, swap.w, b), n_cur = sq.n_tbl[cur];
   const float* sc = score + (size_t)b * k * kL2C;
   uint32_t* mk = mask + (size_t)b * k * 4;
   for (int i = threadIdx.x; i < k * 4; i += blockDim.x) mk[i] = 0u;
@@ -305,7 +314,7 @@ __device__ __forceinline__ void l2_radix_passes(const uint32_t (&key)[N], uint32
 
 template <int PER>
 __global__ void __launch_bounds__(1024)
-l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ score, unsigned* __restrict__ ghist, int k, int k2,
+l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, L2Swap swap, const float* __restrict__ score, unsigned* __restrict__ ghist, int k, int k2,
                     uint32_t* __restrict__ mask) {
   __shared__ unsigned hist[256];
   __shared__ unsigned wsum[33];
@@ -315,7 +324,7 @@ l2_topk_mask_kernel(const SeqDev* __restrict__ seqs, const float* __restrict__ s
   pdl_wait();
   pdl_launch_dependents();
   const SeqDev& sq = seqs[b];
-  const int n = sq.n_tbl[sq.cur_buf] * kL2C;                 // multiple of 128, PER divides 128
+  const int n = sq.n_tbl[l2_cur_buf(sq, swap.w, b)] * kL2C;  // multiple of 128, PER divides 128
   const float* sc = score + (size_t)b * k * kL2C;
   uint32_t* mk = mask + (size_t)b * k * 4;
   const int base = tid * PER;
@@ -499,7 +508,7 @@ void l2_destroy(L2Plan* pl) {
 }
 
 int l2_select(L2Plan* pl, const SeqDev* d_seqs, const void* q_idx, const float* w_idx, int32_t* sel_entries, float* sel_score,
-              cudaStream_t st, int* launches, std::string* msg) {
+              const unsigned* swap_words, cudaStream_t st, int* launches, std::string* msg) {
   const L2Init& in = pl->init;
   if (q_idx != pl->q_cached) {
     if (!l2_encode(pl->encode, &pl->map_q, q_idx, (uint64_t)in.B * kL2H, kL2H, msg)) return -2;
@@ -508,6 +517,8 @@ int l2_select(L2Plan* pl, const SeqDev* d_seqs, const void* q_idx, const float* 
   L2ScoreParams sp{};
   sp.seqs = d_seqs; sp.tbl_chunk = in.tbl_chunk; sp.k_maps = pl->d_maps; sp.w_idx = w_idx; sp.score = pl->score;
   sp.B = in.B; sp.k = in.k;
+  L2Swap sw{};
+  for (int i = 0; i < 8; ++i) sw.w[i] = sp.swap[i] = swap_words ? swap_words[i] : 0u;
   const int n_max = in.k * kL2C;
   const bool mask_only = !sel_entries && !sel_score && n_max <= 16384;     // keys in registers, no sort
   sp.ghist = mask_only ? pl->ghist : nullptr;
@@ -516,11 +527,11 @@ int l2_select(L2Plan* pl, const SeqDev* d_seqs, const void* q_idx, const float* 
   L2_CUDA(launch_pdl(l2_score_kernel, dim3(grid), dim3(kL2Threads), pl->smem, st, pl->map_q, sp));
   if (mask_only) {
     const float* sc = pl->score;
-    if (n_max <= 4096) L2_CUDA(launch_pdl(l2_topk_mask_kernel<4>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, pl->ghist, in.k, in.k2, pl->mask));
-    else if (n_max <= 8192) L2_CUDA(launch_pdl(l2_topk_mask_kernel<8>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, pl->ghist, in.k, in.k2, pl->mask));
-    else L2_CUDA(launch_pdl(l2_topk_mask_kernel<16>, dim3(in.B), dim3(1024), 0, st, d_seqs, sc, pl->ghist, in.k, in.k2, pl->mask));
+    if (n_max <= 4096) L2_CUDA(launch_pdl(l2_topk_mask_kernel<4>, dim3(in.B), dim3(1024), 0, st, d_seqs, sw, sc, pl->ghist, in.k, in.k2, pl->mask));
+    else if (n_max <= 8192) L2_CUDA(launch_pdl(l2_topk_mask_kernel<8>, dim3(in.B), dim3(1024), 0, st, d_seqs, sw, sc, pl->ghist, in.k, in.k2, pl->mask));
+    else L2_CUDA(launch_pdl(l2_topk_mask_kernel<16>, dim3(in.B), dim3(1024), 0, st, d_seqs, sw, sc, pl->ghist, in.k, in.k2, pl->mask));
   } else {
-    L2_CUDA(launch_pdl(l2_topk_kernel, dim3(in.B), dim3(1024), 0, st, d_seqs, in.tbl_chunk, (const float*)pl->score, in.k, in.k2, pl->mask,
+    L2_CUDA(launch_pdl(l2_topk_kernel, dim3(in.B), dim3(1024), 0, st, d_seqs, sw, in.tbl_chunk, (const float*)pl->score, in.k, in.k2, pl->mask,
                        sel_entries, sel_score));
   }
   *launches += 2;
