@@ -122,6 +122,46 @@ def test_l2_select_and_attention_match_oracle(k, k2, L):
     rig.ctx.close()
 
 
+def test_l2_all_scores_tied_selects_lowest_entry_ids():
+    """Degenerate case: zero head weights make every native score exactly 0, so Eq.(6) is decided by the tie rule alone
+    (M2): the k2 lowest entry ids of the resident set.  All 5024 keys of sequence 0 share one radix bin - more than the
+    mask-only kernel's shared-memory candidate buffer holds - so its register fallback runs; both kernels must agree."""
+    k2 = 700
+    cfg, wl, l2, rig = _rig(40, k2)
+    orc = make_oracle(wl)
+    for t in range(2):
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t)
+        firing = [b for b in range(cfg.B) if orc.step[b] % cfg.tau == 0]
+        rig.ctx.step(rig.dev(q), rig.dev(h), rig.dev(kn), rig.dev(vn))
+        orc.step_begin(h, forced_selection=_forced(rig, orc, cfg, h, firing) if firing else None)
+        orc.step_end(q, kn, vn, attend=False)
+    for b in range(cfg.B):
+        orc.pool.maybe_swap(b, orc.step[b])
+    qi, _ = _dev_l2(rig, l2, 2)
+    wi = torch.zeros((cfg.B, 64), dtype=torch.float32, device=rig.device)
+    sel, sc = rig.ctx.l2_select(qi, wi)
+    out = rig.ctx.decode_attention(rig.dev(wl.q(2)))
+    masks = [rig.ctx.l2_mask(b) for b in range(cfg.B)]
+    rig.ctx.l2_select(qi, wi, want_entries=False)
+    out_fast = rig.ctx.decode_attention(rig.dev(wl.q(2)))
+    rig.ctx.sync()
+    o_sels = []
+    for b in range(cfg.B):
+        o_sel, ids, o_sc = l2_select(l2.q_idx(2)[b], np.zeros(64, dtype=np.float32), l2.index_k[b], [c for c, _ in orc.pool.cur[b]],
+                                     cfg.n_csa(b), cfg.C, k2)
+        assert np.all(o_sc == 0.0) and o_sel.tolist() == ids[:k2].tolist()          # the oracle's own tie rule
+        got = sel[b].cpu().numpy()
+        assert got[got >= 0].tolist() == o_sel.tolist()                             # exact ties: the order is fixed too
+        assert torch.all(sc[b][: len(o_sel)] == 0.0)
+        assert np.array_equal(rig.ctx.l2_mask(b), masks[b]) and np.array_equal(masks[b], _mask_of(cfg, orc, b, o_sel))
+        o_sels.append(o_sel)
+    assert torch.equal(out, out_fast)
+    ref, _ = l2_decode_attention(orc, wl.q(2), o_sels)
+    np.testing.assert_allclose(rig.host(out), ref, **attn_tolerance("bf16"))
+    rig.ctx.close()
+
+
 def test_l2_before_any_trigger_attends_hca_and_window_only():
     cfg, wl, l2, rig = _rig(12, 64)
     orc = make_oracle(wl)
@@ -168,6 +208,40 @@ def test_lsa_step_l2_lockstep(recall_lag):
     # Level 2 changes the result: the same step without it differs from the Level-2 output
     plain = rig.host(rig.ctx.decode_attention(rig.dev(q)))
     assert np.abs(plain - got).max() > 10 * max(max_err, 1e-4)
+    rig.ctx.close()
+
+
+def test_l2_cfg3_full_size_bench_launch_config():
+    """BASELINE config 3 (1M context, k = 64 -> 8192 resident entries) with k2 = 2048, the configuration `bench.py --l2`
+    times: trigger step, the step whose table swap rides on the masked attention launch, and a plain step."""
+    cfg = make_config(3)
+    wl = LsaWorkload(cfg)
+    l2 = L2Inputs(wl)
+    rig = GpuRig(wl)
+    k2 = 2048
+    rig.ctx.l2_init([to_torch(K, "bf16").to(rig.device) for K in l2.index_k], k2)
+    orc = make_oracle(wl)
+    tol = attn_tolerance("bf16")
+    for t in range(3):
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t)
+        qi, wi = _dev_l2(rig, l2, t)
+        firing = [b for b in range(cfg.B) if orc.step[b] % cfg.tau == 0]
+        out = rig.ctx.step_l2(rig.dev(q), rig.dev(h), rig.dev(kn), rig.dev(vn), qi, wi)
+        orc.step_begin(h, forced_selection=_forced(rig, orc, cfg, h, firing) if firing else None)
+        o_sels, o_ids, o_scs = _oracle_l2(orc, cfg, l2, t, k2)
+        orc.step_end(q, kn, vn, attend=False)
+        if t > 0:
+            assert len(o_ids[0]) == 8192 and len(o_sels[0]) == k2
+            mask = rig.ctx.l2_mask(0)
+            assert mask.sum() == k2
+            got_set = {int(orc.pool.cur[0][j][0]) * cfg.C + int(r) for j, r in zip(*np.nonzero(mask))}
+            padded = np.full(k2, -1, dtype=np.int64); padded[:] = sorted(got_set)
+            assert validate_l2_selection(padded, o_ids[0], o_scs[0], k2) is None
+            if got_set != set(o_sels[0].tolist()):
+                continue                                              # a near-tie at the cut-off went the other way
+        ref, _ = l2_decode_attention(orc, q, o_sels)
+        np.testing.assert_allclose(rig.host(out), ref, err_msg=f"step {t}", **tol)
     rig.ctx.close()
 
 
