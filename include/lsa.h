@@ -230,7 +230,8 @@ int lsa_l2_init(lsa_ctx* ctx, const lsa_l2_config* cfg, const void* const* index
 
 /* Eq.(6) for all B sequences on stream_compute: staged tables that are due become current first (S6), then the
  * entries of the current tables are scored and the Top-k2 marked.  The selection applies to the NEXT
- * lsa_decode_attention call only (one-shot), which then attends HCA (+) the marked rows (+) window.
+ * lsa_decode_attention call only (one-shot), which then attends HCA (+) the marked rows (+) window; an lsa_step
+ * in between discards it (a step may change the tables: use lsa_step_l2).
  *   q_idx DEVICE [B][n_h][c_I] bf16   w_idx DEVICE [B][n_h] fp32 (both read on stream_compute)
  *   sel_entries DEVICE [B][k2] int32 or NULL: entry ids in (score desc, id asc) order, then -1
  *   sel_score   DEVICE [B][k2] fp32  or NULL: their native scores, -inf padding */

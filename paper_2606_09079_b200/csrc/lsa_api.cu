@@ -545,6 +545,7 @@ static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_n
   if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
   if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
   if (k_new && c->cfg.W < 1) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new given but W == 0");
+  if (!q_idx) c->l2_armed = false;        // a selection left by lsa_l2_select belongs to lsa_decode_attention, not to a step
   int ids[1024];
   int n_fire = 0;
   for (int b = 0; b < c->B; ++b)
