@@ -18,11 +18,13 @@ from paper_2606_09079_b200.workloads import L2Inputs, LsaWorkload, make_config, 
 pytestmark = pytest.mark.gpu
 
 
-def _rig(k, k2, B=2, L=(20096, 4992), steps=8, tau=4, **over):
+def _rig(k, k2, B=2, L=(20096, 4992), steps=8, tau=4, dup_rows=0, **over):
     cfg = make_config(2, B=B, L=list(L), W=1024, k=k, tau=tau, steps=steps, q_gain=16.0,
                       hot_pages=2 * sum(min(k, -(-(l // 4) // 128)) for l in L) + 4, name="l2_parity", **over)
     wl = LsaWorkload(cfg)
     l2 = L2Inputs(wl)
+    if dup_rows:                                              # only `dup_rows` distinct index keys per sequence: exact score ties
+        l2.index_k = [K[np.arange(len(K)) % dup_rows].copy() for K in l2.index_k]
     rig = GpuRig(wl)
     rig.ctx.l2_init([to_torch(K, "bf16").to(rig.device) for K in l2.index_k], k2)
     return cfg, wl, l2, rig
@@ -119,6 +121,52 @@ def test_l2_select_and_attention_match_oracle(k, k2, L):
         if all(k2 >= len(o_ids[b]) for b in range(cfg.B)):
             assert torch.equal(out, out_plain)                # every valid row marked: the same arithmetic, bit for bit
     assert compared >= 1
+    rig.ctx.close()
+
+
+@pytest.mark.parametrize("k,k2", [(12, 300), (40, 1000)])
+def test_l2_duplicate_keys_exact_ties_at_the_cutoff(k, k2):
+    """Only 97 distinct index keys per sequence: the native scores come in groups of exactly equal values (identical
+    inputs, identical arithmetic - on the GPU and in the oracle alike), and the k2-th score falls inside such a group, so
+    the deterministic tie-break (score desc, entry id asc; M2) decides which members are kept.  Both Top-k kernels must
+    return exactly the oracle's list."""
+    cfg, wl, l2, rig = _rig(k, k2, dup_rows=97)
+    orc = make_oracle(wl)
+    for t in range(2):
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t)
+        firing = [b for b in range(cfg.B) if orc.step[b] % cfg.tau == 0]
+        rig.ctx.step(rig.dev(q), rig.dev(h), rig.dev(kn), rig.dev(vn))
+        orc.step_begin(h, forced_selection=_forced(rig, orc, cfg, h, firing) if firing else None)
+        orc.step_end(q, kn, vn, attend=False)
+    for b in range(cfg.B):
+        orc.pool.maybe_swap(b, orc.step[b])
+    qi, wi = _dev_l2(rig, l2, 2)
+    sel, sc = rig.ctx.l2_select(qi, wi)
+    out = rig.ctx.decode_attention(rig.dev(wl.q(2)))
+    masks = [rig.ctx.l2_mask(b) for b in range(cfg.B)]
+    rig.ctx.l2_select(qi, wi, want_entries=False)
+    out_fast = rig.ctx.decode_attention(rig.dev(wl.q(2)))
+    rig.ctx.sync()
+    o_sels, o_ids, o_scs = _oracle_l2(orc, cfg, l2, 2, k2)
+    for b in range(cfg.B):
+        n = min(k2, len(o_ids[b]))
+        by_id = dict(zip(o_ids[b].tolist(), o_scs[b].tolist()))
+        got = sel[b].cpu().numpy()
+        # identical index-key rows must give identical oracle scores (same BLAS path for every row); if a host BLAS
+        # ever rounded them differently the oracle's order inside a group would be arbitrary: fall back to the band rule
+        groups_exact = all(len({by_id[e] for e in o_ids[b].tolist() if e % 97 == r}) <= 1 for r in range(97))
+        if not groups_exact:
+            assert validate_l2_selection(got, o_ids[b], o_scs[b], k2) is None
+            continue
+        if n < len(o_ids[b]):
+            ranked = sorted(by_id, key=lambda e: (-by_id[e], e))
+            assert by_id[ranked[n - 1]] == by_id[ranked[n]], "the cut-off must fall inside a tie group for this test to bite"
+        assert got[:n].tolist() == o_sels[b].tolist(), f"seq {b}"
+        assert np.array_equal(masks[b], _mask_of(cfg, orc, b, o_sels[b])) and np.array_equal(rig.ctx.l2_mask(b), masks[b])
+    assert torch.equal(out, out_fast)
+    ref, _ = l2_decode_attention(orc, wl.q(2), o_sels)
+    np.testing.assert_allclose(rig.host(out), ref, **attn_tolerance("bf16"))
     rig.ctx.close()
 
 
