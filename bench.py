@@ -184,6 +184,7 @@ def main():
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--max-ctas", type=int, default=0, help="cap on attention CTAs (0 = library default)")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
+    ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
     ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
     ap.add_argument("--l2-k2", type=int, default=2048, help="Level-2 Top-k (entries per sequence and step)")
     args = ap.parse_args()
@@ -439,6 +440,59 @@ def main():
                       resident_entries=sum(c.k_eff(b) for b in range(c.B)) * c.C, select_ms=sel_ms, index_key_bytes_per_step=key_bytes,
                       note="lsa_step_l2: Level-2 score + Top-k2 + masked attention (S6 / append folded in) + combine; select_ms = the two Level-2 kernels alone, PDL-chained")
 
+    # ---- optional: lsa_step_graph (NEXT-3) through the same replica rotation, fixed input buffers ----
+    graph = None
+    if args.graph and rank == 0 and stats["attn_impl"] == 2:
+        def g_step(i):
+            r = reps[i % R]
+            t = r.step
+            r.ctx.step_graph(qs[0], hs[(t // c.tau) % NIN], kns[0], vns[0], out)
+            r.step += 1
+        for i in range(max(3, 2 * R)):
+            g_step(i_next + i)
+        i_next += max(3, 2 * R)
+        n_g = max(256, args.steps // 2)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        w0 = time.perf_counter()
+        e0.record(sc)
+        for i in range(n_g):
+            g_step(i_next + i)
+        e1.record(sc)
+        enq_g = time.perf_counter() - w0
+        sf.synchronize(); sc.synchronize()
+        i_next += n_g
+        g_ms = e0.elapsed_time(e1) / n_g
+        # host cost of one call while the launch queue has room (256 steps = 512 launches, then drain)
+        def host_cost(fn):
+            best = None
+            for _ in range(3):
+                sf.synchronize(); sc.synchronize()
+                r0 = reps[0]
+                while r0.step % c.tau < 2 or r0.step % c.tau > c.tau - 10:      # stay inside one trigger window on every replica
+                    for r in reps:
+                        r.ctx.step(qs[0], hs[(r.step // c.tau) % NIN], kns[0], vns[0], out); r.step += 1
+                    sc.synchronize(); sf.synchronize()
+                w = time.perf_counter()
+                for i in range(8 * R if 8 * R < c.tau - 12 else R):
+                    fn(i)
+                dt = (time.perf_counter() - w) / (8 * R if 8 * R < c.tau - 12 else R)
+                best = dt if best is None else min(best, dt)
+            sc.synchronize(); sf.synchronize()
+            return best * 1e6
+
+        def s_step(i):
+            r = reps[i % R]
+            r.ctx.step(qs[0], hs[(r.step // c.tau) % NIN], kns[0], vns[0], out)
+            r.step += 1
+        host_us_graph = host_cost(lambda i: g_step(i)) if c.tau >= 32 else None
+        host_us_step = host_cost(s_step) if c.tau >= 32 else None
+        gs = [r.ctx.graph_stats() for r in reps]
+        graph = dict(value=per_step_units / (g_ms * 1e-3), unit=unit, ms_per_step=g_ms, host_enqueue_ms_per_step=enq_g * 1e3 / n_g,
+                     captures=sum(g_["captures"] for g_ in gs), replays=sum(g_["replays"] for g_ in gs),
+                     host_us_per_call=dict(lsa_step=host_us_step, lsa_step_graph=host_us_graph),
+                     note="lsa_step_graph: steps without a trigger or a table swap replay one captured graph (attention + combine) per context")
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n, secs, threads = oracle_sample(wl, budget_s=15.0, max_steps=24)
@@ -459,7 +513,7 @@ def main():
                              ms_per_step=ms_e2e / n_e2e),
                     gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, l1_indexer=l1, level2=level2, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
+                    fetch=fetch, l1_indexer=l1, level2=level2, step_graph=graph, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
                     host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
         print(json.dumps(line))

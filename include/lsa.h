@@ -163,6 +163,18 @@ int lsa_decode_attention(lsa_ctx* ctx, const void* q, void* out, float* lse);
 int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
              void* out);
 
+/* lsa_step with the fixed-shape part replayed from a CUDA graph ("CUDA-graph-compatible recall": the captured
+ * graph holds only fixed-shape GPU work, Level-1 scoring and copying run out-of-graph in the side band).  On a step
+ * without a trigger and without a table swap, the launches of (a)/(d)/(e) - S6, the window append, attention and
+ * combine - are one captured graph, replayed as long as q, k_new, v_new, out and the split geometry stay the same
+ * (the state they read - window fill, ring head, tables - lives in device records, so the same graph serves every
+ * such step); any other step, or a context with profiling / fused merge enabled, runs exactly as lsa_step and
+ * the graph is re-captured when the key changes.  Results are identical to lsa_step. */
+int lsa_step_graph(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
+                   void* out);
+/* captures / replays so far (HOST pointers, either may be NULL) */
+int lsa_graph_stats(lsa_ctx* ctx, uint64_t* captures, uint64_t* replays);
+
 /* lsa_step with HOST buffers.  Pinned + mapped inputs (e.g. torch pin_memory) are pulled over the host link by
  * one small kernel and a pinned `out` is written in place by S8; pageable buffers go through one packed
  * host->device copy and one device->host copy.  h is only read at trigger steps.  Blocks until the result

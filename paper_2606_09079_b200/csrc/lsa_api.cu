@@ -58,6 +58,11 @@ struct lsa_ctx {
   float l1_threshold = 0.5f;
   L2Plan* l2 = nullptr;               // Level 2 (lsa_l2_init)
   bool l2_armed = false;              // a Level-2 selection waits for the next attention launch
+  // lsa_step_graph: the captured non-trigger step and the key it is valid for
+  cudaGraphExec_t sg_exec = nullptr;
+  const void *sg_q = nullptr, *sg_kn = nullptr, *sg_vn = nullptr, *sg_out = nullptr;
+  long long sg_tiles = -1;
+  unsigned long long sg_launches = 0, sg_captures = 0, sg_replays = 0;
   int indexer = 0;                     // lsa_indexer used by lsa_step at trigger steps
   // host-buffer staging (lsa_step_host)
   void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
@@ -134,6 +139,7 @@ extern "C" void lsa_destroy(lsa_ctx* ctx) {
   if (ctx->tc) tc_destroy(ctx->tc);
   if (ctx->l1) l1_destroy(ctx->l1);
   if (ctx->l2) l2_destroy(ctx->l2);
+  if (ctx->sg_exec) cudaGraphExecDestroy(ctx->sg_exec);
   if (ctx->st_pin) cudaFreeHost(ctx->st_pin);
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
@@ -588,6 +594,55 @@ static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_n
 extern "C" int lsa_step(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
   if (!ctx) return LSA_ERR_STATE;
   return step_impl(ctx, q, h, k_new, v_new, out, nullptr, nullptr);
+}
+
+// ---- NEXT-3: the non-trigger step as a CUDA graph ------------------------------------------------------------
+extern "C" int lsa_step_graph(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
+  if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
+  bool plain = c->attn_impl != LSA_ATTN_TCGEN05 || c->prof_cap > 0 || c->cfg.merge_mode == LSA_MERGE_FUSED || (k_new && c->cfg.W < 1);
+  for (int b = 0; b < c->B && !plain; ++b)
+    plain = (c->step[b] % c->cfg.tau == 0) || (c->pending[b] && c->step[b] >= c->visible_at[b]);   // trigger, or a swap is due
+  if (plain) return step_impl(c, q, h, k_new, v_new, out, nullptr, nullptr);
+  c->l2_armed = false;
+  if (k_new) mirror_append(c);
+  long long tiles = 0;                              // same host mirror attention_impl sizes the grid from
+  for (int b = 0; b < c->B; ++b) tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
+  if (!c->sg_exec || q != c->sg_q || k_new != c->sg_kn || v_new != c->sg_vn || out != c->sg_out || tiles != c->sg_tiles) {
+    if (c->sg_exec) { cudaGraphExecDestroy(c->sg_exec); c->sg_exec = nullptr; }
+    const unsigned long long before = c->attn_launches;
+    LSA_CUDA(c, cudaStreamBeginCapture(c->sc, cudaStreamCaptureModeThreadLocal));
+    TcPrestep pre{};
+    pre.k_new = k_new; pre.v_new = v_new;
+    const int rc = attention_impl(c, q, out, nullptr, &pre);
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->sc, &g);
+    c->sg_launches = c->attn_launches - before;
+    c->attn_launches = before;                      // nothing ran during the capture
+    if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess || !g) LSA_FAIL(c, LSA_ERR_CUDA, "stream capture of the step failed: %s", cudaGetErrorString(e));
+    const cudaError_t ei = cudaGraphInstantiate(&c->sg_exec, g, 0);
+    cudaGraphDestroy(g);
+    if (ei != cudaSuccess) { c->sg_exec = nullptr; LSA_FAIL(c, LSA_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(ei)); }
+    c->sg_q = q; c->sg_kn = k_new; c->sg_vn = v_new; c->sg_out = out; c->sg_tiles = tiles;
+    c->sg_captures += 1;
+  } else {
+    c->sg_replays += 1;
+  }
+  LSA_CUDA(c, cudaGraphLaunch(c->sg_exec, c->sc));
+  c->attn_launches += c->sg_launches;
+  for (int b = 0; b < c->B; ++b) c->step[b] += 1;
+  c->n_steps += 1;
+  return LSA_OK;
+}
+
+extern "C" int lsa_graph_stats(lsa_ctx* ctx, uint64_t* captures, uint64_t* replays) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (captures) *captures = ctx->sg_captures;
+  if (replays) *replays = ctx->sg_replays;
+  return LSA_OK;
 }
 
 // ---- Level 2 (NEXT-2) ---------------------------------------------------------------------------------------

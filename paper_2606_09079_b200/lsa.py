@@ -33,7 +33,7 @@ EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
-           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask",
+           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats",
            "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
@@ -106,6 +106,8 @@ def _load() -> C.CDLL:
     lib.lsa_l2_init.argtypes = [vp, C.POINTER(lsa_l2_config), C.POINTER(vp)]
     lib.lsa_l2_select.argtypes = [vp, vp, vp, vp, vp]
     lib.lsa_l2_get_mask.argtypes = [vp, C.c_int32, vp]
+    lib.lsa_step_graph.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.lsa_graph_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.lsa_step_l2.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsa_last_error.argtypes = [vp]
     lib.lsa_last_error.restype = C.c_char_p
@@ -317,6 +319,19 @@ class LsaContext:
                                   _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
                                   _dev_ptr(out, self.tdtype, "out")))
         return out
+
+    def step_graph(self, q, h, k_new=None, v_new=None, out=None):
+        """lsa_step with the non-trigger step replayed from a CUDA graph (keep q / k_new / v_new / out at fixed addresses)."""
+        out = torch.empty_like(q) if out is None else out
+        self._check(_lib.lsa_step_graph(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(h, self.tdtype, "h"),
+                                        _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
+                                        _dev_ptr(out, self.tdtype, "out")))
+        return out
+
+    def graph_stats(self):
+        cap, rep = C.c_uint64(0), C.c_uint64(0)
+        self._check(_lib.lsa_graph_stats(self._h, C.byref(cap), C.byref(rep)))
+        return dict(captures=cap.value, replays=rep.value)
 
     def step_host(self, q, h, k_new, v_new, out):
         self._check(_lib.lsa_step_host(self._h, _host_ptr(q, self.tdtype, "q"), _host_ptr(h, self.tdtype, "h"),

@@ -90,7 +90,7 @@ def attn_tolerance(dtype: str):
 
 
 def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=None, with_kv_new: bool = True,
-                 tie_emb_builder=None, l1=None, l1_band: float = 3e-2):
+                 tie_emb_builder=None, l1=None, l1_band: float = 3e-2, step_fn=None):
     """Drive lsa_step and the oracle in lock-step: validate the GPU's
     selection against the oracle's scores, feed it to the oracle's residency model, then compare page
     tables / residency / fetched bytes bit-exactly and attention outputs within tolerance."""
@@ -106,8 +106,11 @@ def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=
         kn, vn = wl.kv_new(t) if with_kv_new else (None, None)
         firing = [b for b in range(c.B) if orc.step[b] % c.tau == 0]
         bytes_before = rig.ctx.stats()["bytes_fetched"] if not firing else None
-        out_gpu = rig.ctx.step(rig.dev(q), rig.dev(h), None if kn is None else rig.dev(kn),
-                               None if vn is None else rig.dev(vn))
+        if step_fn is not None:               # another entry point with lsa_step's semantics (e.g. lsa_step_graph)
+            out_gpu = step_fn(q, h, kn, vn)
+        else:
+            out_gpu = rig.ctx.step(rig.dev(q), rig.dev(h), None if kn is None else rig.dev(kn),
+                                   None if vn is None else rig.dev(vn))
         forced = {}
         for b in firing:                      # GPU selection = chunk ids of the table it just staged
             which = 0 if c.recall_lag == 0 else 1

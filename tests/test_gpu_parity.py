@@ -436,6 +436,34 @@ def test_step_host_equals_step(pinned_out):
     a.ctx.close(); b_.ctx.close()
 
 
+def test_step_graph_replays_and_matches_oracle():
+    """lsa_step_graph (NEXT-3): steps without a trigger or a table swap replay one captured CUDA graph (S6 fold,
+    window append, attention, combine); trigger steps and the step that swaps the tables run as lsa_step.  Same lock-step
+    checks as lsa_step: page tables / residency / fetched bytes bit-exact, attention within tolerance, every step."""
+    cfg = make_config(2, B=2, L=[16384 + 4 * 37, 8192], W=1024, k=6, hot_pages=32, steps=40, name="cfg2_graph", q_gain=16.0, tau=8)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    dev = rig.device
+    qd = torch.empty((cfg.B, cfg.H, cfg.D), dtype=torch.bfloat16, device=dev)
+    hd = torch.empty((cfg.B, cfg.Dh), dtype=torch.bfloat16, device=dev)
+    knd = torch.empty((cfg.B, cfg.D), dtype=torch.bfloat16, device=dev)
+    vnd = torch.empty_like(knd)
+    outd = torch.empty_like(qd)
+
+    def step_fn(q, h, kn, vn):
+        rig.ctx.sync()                                   # the previous step has finished reading the fixed buffers
+        qd.copy_(rig.dev(q)); hd.copy_(rig.dev(h)); knd.copy_(rig.dev(kn)); vnd.copy_(rig.dev(vn))
+        torch.cuda.synchronize()                         # the library's streams are not torch's current stream
+        return rig.ctx.step_graph(qd, hd, knd, vnd, outd)
+
+    r = run_lockstep(wl, rig, cfg.steps, step_fn=step_fn)
+    assert r["checked"] == cfg.steps
+    gs = rig.ctx.graph_stats()
+    # 40 steps, tau = 8: 5 trigger steps + 5 swap steps run plain; the other 30 share ONE graph (window full: fixed geometry)
+    assert gs["captures"] == 1 and gs["replays"] == 29, gs
+    rig.ctx.close()
+
+
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("lag", [0, 1])
 def test_lockstep_small(dtype, lag):
