@@ -184,6 +184,7 @@ def main():
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--max-ctas", type=int, default=0, help="cap on attention CTAs (0 = library default)")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
+    ap.add_argument("--export", action="store_true", help="also time lsa_export_chunks (NEXT-4: KV export HBM -> pinned cold pool)")
     ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
     ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
     ap.add_argument("--l2-k2", type=int, default=2048, help="Level-2 Top-k (entries per sequence and step)")
@@ -440,6 +441,28 @@ def main():
                       resident_entries=sum(c.k_eff(b) for b in range(c.B)) * c.C, select_ms=sel_ms, index_key_bytes_per_step=key_bytes,
                       note="lsa_step_l2: Level-2 score + Top-k2 + masked attention (S6 / append folded in) + combine; select_ms = the two Level-2 kernels alone, PDL-chained")
 
+    # ---- optional: KV export into the cold pool (NEXT-4, first half) against the pinned D2H copy rate ----
+    export = None
+    if args.export and rank == 0:
+        n_ch = min(c.n_chunks(0), max(1, (256 * 2**20) // c.page_bytes))
+        src = shared["cold"][0][:n_ch].to(dev)                   # the same bytes go back: the pool's content is unchanged
+        nb = src.numel() * src.element_size()
+        dstp = torch.empty(nb, dtype=torch.uint8).pin_memory()
+        flat = src.view(torch.uint8).reshape(-1)
+        best_d2h = 0.0
+        for _ in range(5):
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); dstp.copy_(flat, non_blocking=True); b_.record(); torch.cuda.synchronize()
+            best_d2h = max(best_d2h, nb / (a.elapsed_time(b_) * 1e-3) / 1e9)
+        best_exp = 0.0
+        for _ in range(5):
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(sf); reps[0].ctx.export_chunks(0, 0, src); b_.record(sf); sf.synchronize()
+            best_exp = max(best_exp, nb / (a.elapsed_time(b_) * 1e-3) / 1e9)
+        export = dict(bytes=nb, chunks=n_ch, export_gbs=best_exp, d2h_peak_gbs=best_d2h, frac_of_d2h_peak=best_exp / best_d2h,
+                      mode="device kernel storing over the mapped pinned cold pool")
+        del src, dstp
+
     # ---- optional: lsa_step_graph (NEXT-3) through the same replica rotation, fixed input buffers ----
     graph = None
     if args.graph and rank == 0 and stats["attn_impl"] == 2:
@@ -513,7 +536,7 @@ def main():
                              ms_per_step=ms_e2e / n_e2e),
                     gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, l1_indexer=l1, level2=level2, step_graph=graph, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
+                    fetch=fetch, l1_indexer=l1, level2=level2, step_graph=graph, export=export, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
                     host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
         print(json.dumps(line))

@@ -258,6 +258,13 @@ int lsa_l2_get_mask(lsa_ctx* ctx, int32_t seq, uint32_t* words);
 int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
                 const void* q_idx, const float* w_idx, void* out);
 
+/* NEXT-4 (first half; P:179, P:199 VRAM -> DRAM): KV export into the cold pool.  Copies n_chunks page images
+ * src DEVICE [n_chunks][2][C][D] (dtype) into chunks [first_chunk, first_chunk + n_chunks) of sequence seq's pinned-host
+ * cold pool (which must be writable), by a device kernel over the mapped pool on stream_fetch - ordered before every
+ * later trigger's fetch.  Meant for admission, before the chunks are first selected: a chunk that is already resident
+ * keeps its old hot copy until it is evicted.  Enqueues and returns; bit-exact. */
+int lsa_export_chunks(lsa_ctx* ctx, int32_t seq, int32_t first_chunk, int32_t n_chunks, const void* src);
+
 /* Replace the embedding table pointer of one sequence (DEVICE [n_chunks][E]). */
 int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb);
 

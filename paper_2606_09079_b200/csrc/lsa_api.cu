@@ -796,6 +796,23 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
   return LSA_OK;
 }
 
+// ---- NEXT-4 (first half): KV export into the cold pool -------------------------------------------------------
+extern "C" int lsa_export_chunks(lsa_ctx* ctx, int32_t seq, int32_t first_chunk, int32_t n_chunks, const void* src) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (seq < 0 || seq >= c->B) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "bad seq");
+  if (first_chunk < 0 || n_chunks < 0 || (long long)first_chunk + n_chunks > c->seq_host[seq].n_chunks)
+    LSA_FAIL(c, LSA_ERR_INVALID_ARG, "chunks [%d, %d) outside the sequence's %d chunks", first_chunk, first_chunk + n_chunks, c->seq_host[seq].n_chunks);
+  if (n_chunks == 0) return LSA_OK;
+  if (!src) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null src");
+  const long long bytes = (long long)n_chunks * c->page_bytes;
+  void* dst = const_cast<unsigned char*>(reinterpret_cast<const unsigned char*>(c->seq_host[seq].cold)) + (long long)first_chunk * c->page_bytes;
+  const int ctas = (int)std::max<long long>(1, std::min<long long>(c->fetch_ctas > 0 ? c->fetch_ctas : 64, (bytes + 16383) / 16384));
+  LSA_CUDA(c, launch_export(src, dst, bytes, ctas, c->sf));
+  c->index_launches += 1;
+  return LSA_OK;
+}
+
 // ---- support --------------------------------------------------------------------------------------
 extern "C" int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb) {
   if (!ctx) return LSA_ERR_STATE;

@@ -28,6 +28,8 @@ cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, c
                              int B, int k, int P, long long page_bytes, cudaStream_t st);
 cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas,
                          cudaStream_t st);
+// NEXT-4: copy `bytes` (multiple of 16) from device memory into the mapped pinned cold pool
+cudaError_t launch_export(const void* src, void* dst_mapped, long long bytes, int n_ctas, cudaStream_t st);
 // swap tables of sequences whose bit is set in swap_mask; append k_new/v_new rows to the ring
 cudaError_t launch_prestep(int dtype, SeqDev* seqs, int B, int D, int W, const uint32_t* swap_mask_words,
                            int n_words, const void* k_new, const void* v_new, cudaStream_t st);

@@ -218,6 +218,32 @@ fetch_kernel(PoolDev pool, unsigned char* __restrict__ hot_pool, long long page_
   }
 }
 
+// ---- NEXT-4 (first half): KV export, HBM -> pinned-host cold pool ("P-server streams full KV into D's pinned host
+// memory"; P:199 VRAM -> DRAM).  The mirror image of fetch_kernel: 16-byte stores over the mapped pinned pool, the
+// loads of a slice all in flight before its stores.
+__global__ void __launch_bounds__(kFetchThreads)
+export_kernel(const unsigned char* __restrict__ src, unsigned char* __restrict__ dst, long long bytes) {
+  const long long slice = (long long)kFetchUnroll * kFetchThreads * 16;
+  for (long long base = (long long)blockIdx.x * slice; base < bytes; base += (long long)gridDim.x * slice) {
+    uint4 v[kFetchUnroll];
+#pragma unroll
+    for (int u = 0; u < kFetchUnroll; ++u) {
+      const long long off = base + ((long long)u * kFetchThreads + threadIdx.x) * 16;
+      if (off < bytes) v[u] = *reinterpret_cast<const uint4*>(src + off);
+    }
+#pragma unroll
+    for (int u = 0; u < kFetchUnroll; ++u) {
+      const long long off = base + ((long long)u * kFetchThreads + threadIdx.x) * 16;
+      if (off < bytes) *reinterpret_cast<uint4*>(dst + off) = v[u];
+    }
+  }
+}
+
+cudaError_t launch_export(const void* src, void* dst_mapped, long long bytes, int n_ctas, cudaStream_t st) {
+  export_kernel<<<n_ctas, kFetchThreads, 0, st>>>(reinterpret_cast<const unsigned char*>(src), reinterpret_cast<unsigned char*>(dst_mapped), bytes);
+  return cudaGetLastError();
+}
+
 // ---- S6 + window append ---------------------------------------------------------------------
 // The swap mask is passed BY VALUE (32 words = up to 1024 sequences): a step needs no extra copy.
 struct SwapWords { uint32_t w[32]; };

@@ -33,7 +33,7 @@ EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
-           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats",
+           "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats", "lsa_export_chunks",
            "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
@@ -106,6 +106,7 @@ def _load() -> C.CDLL:
     lib.lsa_l2_init.argtypes = [vp, C.POINTER(lsa_l2_config), C.POINTER(vp)]
     lib.lsa_l2_select.argtypes = [vp, vp, vp, vp, vp]
     lib.lsa_l2_get_mask.argtypes = [vp, C.c_int32, vp]
+    lib.lsa_export_chunks.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, vp]
     lib.lsa_step_graph.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.lsa_graph_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.lsa_step_l2.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
@@ -319,6 +320,10 @@ class LsaContext:
                                   _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
                                   _dev_ptr(out, self.tdtype, "out")))
         return out
+
+    def export_chunks(self, seq: int, first_chunk: int, src: torch.Tensor):
+        """KV export (VRAM -> pinned cold pool): src = [n][2][C][D] CUDA tensor of page images for chunks first_chunk.."""
+        self._check(_lib.lsa_export_chunks(self._h, seq, first_chunk, int(src.shape[0]), _dev_ptr(src, self.tdtype, "src")))
 
     def step_graph(self, q, h, k_new=None, v_new=None, out=None):
         """lsa_step with the non-trigger step replayed from a CUDA graph (keep q / k_new / v_new / out at fixed addresses)."""

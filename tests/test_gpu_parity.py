@@ -436,6 +436,36 @@ def test_step_host_equals_step(pinned_out):
     a.ctx.close(); b_.ctx.close()
 
 
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_export_chunks_fills_the_cold_pool_bit_exactly(dtype):
+    """NEXT-4, first half (P:179, P:199 VRAM -> DRAM): parts of the pinned cold pool start zeroed; lsa_export_chunks copies
+    their page images from HBM (bit-exact, ragged chunk ranges), and the lock-step run that follows - whose fetches read
+    the cold pool - matches the oracle, which holds the true data throughout."""
+    from paper_2606_09079_b200 import lsa
+    cfg = make_small_config(dtype, steps=10, q_gain=8.0)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    true = [x.clone() for x in rig.cold]
+    n0, n1 = cfg.n_chunks(0), cfg.n_chunks(1)
+    rig.cold[0][: n0 - 5].zero_()
+    rig.cold[1].zero_()
+    srcs = [true[0][:7].to(rig.device), true[0][7: n0 - 5].to(rig.device), true[1].to(rig.device)]
+    torch.cuda.synchronize()
+    rig.ctx.export_chunks(0, 0, srcs[0])
+    rig.ctx.export_chunks(0, 7, srcs[1])
+    rig.ctx.export_chunks(1, 0, srcs[2])
+    rig.ctx.export_chunks(1, n1, srcs[2][:0])                       # empty range at the end: a no-op
+    rig.ctx.sync()
+    assert torch.equal(rig.cold[0], true[0]) and torch.equal(rig.cold[1], true[1])
+    with pytest.raises(lsa.LsaError):
+        rig.ctx.export_chunks(1, n1 - 1, srcs[2][:2])               # past the last chunk
+    with pytest.raises(lsa.LsaError):
+        rig.ctx.export_chunks(2, 0, srcs[2])                        # no such sequence
+    r = run_lockstep(wl, rig, cfg.steps)
+    assert r["checked"] == cfg.steps and rig.ctx.stats()["misses"] > 0
+    rig.ctx.close()
+
+
 def test_step_graph_replays_and_matches_oracle():
     """lsa_step_graph (NEXT-3): steps without a trigger or a table swap replay one captured CUDA graph (S6 fold,
     window append, attention, combine); trigger steps and the step that swaps the tables run as lsa_step.  Same lock-step
