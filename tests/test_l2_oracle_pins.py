@@ -152,3 +152,20 @@ def test_selection_only_from_resident_valid_rows_and_validator():
     sc2 = np.array([5.0, 4.0, 3.0, 3.0 - 1e-7, 1.0]); ids2 = np.arange(5)
     assert validate_l2_selection([0, 1, 3], ids2, sc2, 3) is None
     assert validate_l2_selection([0, 1, 4], ids2, sc2, 3) is not None
+
+
+def test_l2_inputs_are_seeded_and_shaped():
+    """The Level-2 input generator holds none of the method's arithmetic: shapes, determinism and the stated distributions."""
+    cfg = make_small_config("bf16", steps=2)
+    wl = LsaWorkload(cfg, build_kv=False)
+    a, b = L2Inputs(wl, c_I=16, n_h=4), L2Inputs(wl, c_I=16, n_h=4)
+    for x, y in zip(a.index_k, b.index_k):
+        assert x.dtype == np.uint16 and np.array_equal(x, y)
+    assert [k.shape for k in a.index_k] == [(cfg.n_csa(i), 16) for i in range(cfg.B)]
+    assert np.array_equal(a.q_idx(3), b.q_idx(3)) and not np.array_equal(a.q_idx(3), a.q_idx(4))
+    assert a.q_idx(0).shape == (cfg.B, 4, 16) and a.w_idx(0).shape == (cfg.B, 4) and a.w_idx(0).dtype == np.float32
+    big = L2Inputs(wl, c_I=128, n_h=64)
+    w = np.concatenate([big.w_idx(t).ravel() for t in range(40)])
+    assert abs(w.mean() * 64 - 0.5) < 0.1 and abs(w.std() * 64 - 1.0) < 0.1
+    m = widen(big.index_k[0][:512]) @ widen(big.q_idx(0)[0]).T              # per-head matches ~ N(0, 1)
+    assert abs(m.std() - 1.0) < 0.1 and abs(m.mean()) < 0.05
