@@ -178,6 +178,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20000)
     ap.add_argument("--warmup", type=int, default=256)
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--recall-lag", type=int, default=None, help="override the config's recall_lag (default 1 = the paper's t+1; up to tau-1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--attn", default="auto", choices=["auto", "simt", "tcgen05"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -193,7 +194,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
-    cfg = make_config(args.config)
+    cfg = make_config(args.config) if args.recall_lag is None else make_config(args.config, recall_lag=args.recall_lag)
     if args.impl == "reference":
         if rank == 0:
             run_reference(args, cfg, LsaWorkload(cfg))
@@ -338,6 +339,39 @@ def main():
                     frac_device_clock=(attn_bytes / (attn_dev_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if attn_dev_ms else None,
                     step_ms=ms / args.steps, frac_of_step=achieved and (attn_bytes / (ms / args.steps * 1e-3) / 1e9) / peaks["hbm_gbs"],
                     peak_source=peaks["source"], frac_of_nominal_8tbs=achieved / 8000.0)
+
+    # ---- how much of the trigger side band (S1-S5) hides behind attention (SURVEY 8(d) "fetch overlap") ----
+    # exposed time per trigger = tau * (mean step time over all steps - step time between triggers); hidden fraction =
+    # 1 - exposed / (side-band kernel time per trigger).  With recall_lag = 1 the new table is needed by step t + 1, so
+    # at most one step's attention can hide it.
+    side_band = None
+    if not c.stagger and c.tau >= 8 and all(ph in phases and phases[ph]["count"] for ph in ("index", "residency", "fetch")):
+        t_al = (max(r.step for r in reps) // c.tau + 1) * c.tau + 2
+        for idx, r in enumerate(reps):
+            while r.step < t_al:
+                one_step(idx)
+        nt_ms, n_win = 0.0, 6
+        for _ in range(n_win):
+            sf.synchronize(); sc.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(sc)
+            for _s in range(c.tau - 3):                      # phases 2 .. tau - 2 of every replica: no trigger, no swap
+                for idx in range(R):
+                    one_step(idx)
+            e1.record(sc)
+            sc.synchronize()
+            nt_ms += e0.elapsed_time(e1) / (R * (c.tau - 3))
+            for _s in range(3):                               # tau - 1, trigger, swap: untimed
+                for idx in range(R):
+                    one_step(idx)
+        nt_ms /= n_win
+        per = {ph: phases[ph]["ms"] / phases[ph]["count"] for ph in ("index", "residency", "fetch")}
+        side_ms = sum(per.values())
+        exposed = c.tau * (ms / args.steps - nt_ms)
+        side_band = dict(step_ms_all=ms / args.steps, step_ms_between_triggers=nt_ms, exposed_ms_per_trigger=exposed,
+                         side_band_ms_per_trigger=side_ms, phases_ms_per_trigger=per,
+                         hidden_fraction=(1.0 - exposed / side_ms) if side_ms > 0 else None, recall_lag=c.recall_lag,
+                         note="hidden_fraction = 1 - exposed / side-band kernel time; recall_lag = 1 lets only the trigger step's own attention hide it")
 
     # ---- chunk fetch: H2D link peak (pinned cudaMemcpyAsync) and the device-pull fetch kernel ----
     fetch = None
@@ -536,7 +570,7 @@ def main():
                              ms_per_step=ms_e2e / n_e2e),
                     gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, l1_indexer=l1, level2=level2, step_graph=graph, export=export, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
+                    fetch=fetch, side_band=side_band, l1_indexer=l1, level2=level2, step_graph=graph, export=export, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
                     host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
         print(json.dumps(line))

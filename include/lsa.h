@@ -75,7 +75,8 @@ typedef struct lsa_config {
   int32_t E;             /* query / chunk embedding dim (BJ)                                    */
   int32_t k;             /* chunks selected per sequence = K_max (R2)                    */
   int32_t tau;           /* trigger interval (tau = 64)                                   */
-  int32_t recall_lag;    /* 0: new table visible at the trigger step; 1: at t+1 (R9)      */
+  int32_t recall_lag;    /* 0: new table visible at the trigger step; 1: at t+1 (R9);     */
+                         /* 2..tau-1: at t+lag - a longer fetch hides behind more steps          */
   float sm_scale;        /* softmax scale; 0 -> 1/sqrt(D) (R18)                                 */
   int64_t hot_pages;     /* P: pages in the hot pool; must be >= 2 * sum_b min(k, n_chunks_b)   */
   void* hot_pool;        /* DEVICE [P][2][C][D]: page = K block [C][D] then V block [C][D]      */

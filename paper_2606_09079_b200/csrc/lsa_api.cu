@@ -287,7 +287,9 @@ extern "C" int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs, l
     LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "B (1..1024), H, D, C, Dh, E must be >= 1 and W >= 0");
   if (cfg->k < 1 || cfg->k > kMaxK) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "k must be in [1, %d]", kMaxK);
   if (cfg->tau < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "tau must be >= 1");
-  if (cfg->recall_lag != 0 && cfg->recall_lag != 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "recall_lag must be 0 or 1");
+  // one staged table per sequence: it must have become current before the next trigger stages another
+  if (cfg->recall_lag < 0 || (cfg->recall_lag > 1 && cfg->recall_lag >= cfg->tau))
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "recall_lag must be 0, 1, or at most tau - 1");
   if (cfg->D % 8 || cfg->Dh % 8 || cfg->E % 8) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "D, Dh, E must be multiples of 8 (16-byte vector loads)");
   if (!cfg->hot_pool || !cfg->W_q) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "null hot_pool / W_q");
   if (cfg->hot_pages < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "hot_pages must be >= 1");

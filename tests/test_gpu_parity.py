@@ -436,6 +436,21 @@ def test_step_host_equals_step(pinned_out):
     a.ctx.close(); b_.ctx.close()
 
 
+def test_recall_lag_deeper_than_one_step_flagship_shape_and_bounds():
+    """recall_lag in 2..tau-1 (a longer fetch hides behind more steps; default stays the paper's t+1): lock-step on
+    the tcgen05 path - the swap then rides on the attention launch lag steps after the trigger - and the init bound."""
+    from paper_2606_09079_b200 import lsa
+    cfg = make_config(2, B=2, L=[16384 + 4 * 37, 8192], W=1024, k=6, hot_pages=32, steps=26, name="cfg2_lag5", q_gain=16.0, tau=8,
+                      recall_lag=5)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    r = run_lockstep(wl, rig, cfg.steps)
+    assert r["checked"] == cfg.steps
+    rig.ctx.close()
+    with pytest.raises(lsa.LsaError):
+        GpuRig(LsaWorkload(make_small_config("bf16", tau=4, recall_lag=4)))      # a second table would be staged before the swap
+
+
 @pytest.mark.parametrize("dtype", ["bf16", "f32"])
 def test_export_chunks_fills_the_cold_pool_bit_exactly(dtype):
     """NEXT-4, first half (P:179, P:199 VRAM -> DRAM): parts of the pinned cold pool start zeroed; lsa_export_chunks copies
@@ -495,7 +510,7 @@ def test_step_graph_replays_and_matches_oracle():
 
 
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
-@pytest.mark.parametrize("lag", [0, 1])
+@pytest.mark.parametrize("lag", [0, 1, 3])
 def test_lockstep_small(dtype, lag):
     cfg = make_small_config(dtype, recall_lag=lag, steps=14, q_gain=8.0)
     wl = LsaWorkload(cfg)

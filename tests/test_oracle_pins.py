@@ -314,13 +314,13 @@ def test_full_path_cfg1_selects_needles_and_window_rule():
 def test_recall_lag_visibility():
     """attention at the trigger step uses the old table, step t+1 the new one."""
     wl = LsaWorkload(make_small_config("f32", B=1, L=[4096], tau=4, k=3, hot_pages=8))
-    for lag in (0, 1):
+    for lag in (0, 1, 3):
         orc = make_oracle(wl, recall_lag=lag)
         sizes = []
         for t in range(6):
             orc.run_step(wl.q(t), wl.h(t))
             sizes.append(len(orc.pool.cur[0]))
-        assert sizes == ([3] * 6 if lag == 0 else [0, 3, 3, 3, 3, 3])
+        assert sizes == [0] * lag + [3] * (6 - lag)          # visible from step t + lag on
     # direct check that the table used at the trigger step is the OLD one
     orc = make_oracle(wl, recall_lag=1)
     orc.step_begin(wl.h(0))
