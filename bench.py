@@ -118,7 +118,8 @@ class Replica:
         self.ctx = lsa.LsaContext(dtype=lsa.LSA_F32 if c.dtype == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W,
                                   Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=shared["W_q"], seqs=seqs,
                                   recall_lag=c.recall_lag, stream_compute=sc, stream_fetch=sf,
-                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0))
+                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0),
+                                  step_overlap=shared.get("overlap", 0))
         self.step = 0
 
 
@@ -184,6 +185,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--max-ctas", type=int, default=0, help="cap on attention CTAs (0 = library default)")
+    ap.add_argument("--overlap", type=int, default=0, help="lsa_config.step_overlap: 1 = the steps' inputs are independent of the previous step's output")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
     ap.add_argument("--export", action="store_true", help="also time lsa_export_chunks (NEXT-4: KV export HBM -> pinned cold pool)")
     ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
@@ -220,7 +222,7 @@ def main():
     warmup = max(args.warmup, 3, 2 * R)
     attn_impl = dict(auto=lsa.LSA_ATTN_AUTO, simt=lsa.LSA_ATTN_SIMT, tcgen05=lsa.LSA_ATTN_TCGEN05)[args.attn]
 
-    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, max_ctas=args.max_ctas, W_q=to_torch(wl.W_q, c.dtype).to(dev),
+    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, max_ctas=args.max_ctas, overlap=args.overlap, W_q=to_torch(wl.W_q, c.dtype).to(dev),
                   cold=[to_torch(x, c.dtype).pin_memory() for x in wl.cold_csa],
                   emb=[to_torch(wl.chunk_emb(b, 0), c.dtype).to(dev) for b in range(c.B)],
                   hca_k=[to_torch(x, c.dtype).to(dev) for x in wl.hca_k], hca_v=[to_torch(x, c.dtype).to(dev) for x in wl.hca_v],

@@ -39,7 +39,7 @@
 extern "C" {
 #endif
 
-#define LSA_VERSION 1
+#define LSA_VERSION 2
 
 typedef struct lsa_ctx lsa_ctx; /* opaque */
 
@@ -55,7 +55,6 @@ enum lsa_status {
 
 enum lsa_dtype { LSA_F32 = 0, LSA_BF16 = 1 };
 enum lsa_attn_impl { LSA_ATTN_AUTO = 0, LSA_ATTN_SIMT = 1, LSA_ATTN_TCGEN05 = 2 };
-enum lsa_fetch_mode { LSA_FETCH_DEVICE_PULL = 0, LSA_FETCH_MEMCPY = 1 };
 /* S8 (merge of the split-K partials, tcgen05 path): AUTO = KERNEL = a separate combine kernel chained to the
  * attention kernel by programmatic dependent launch.  FUSED (B <= 4 only, else ignored) merges inside the
  * attention kernel behind a grid-wide arrival counter: one launch per step; measured slower than KERNEL on
@@ -84,7 +83,10 @@ typedef struct lsa_config {
   void* stream_compute;  /* cudaStream_t: S6-S8 (and S1-S5 when recall_lag == 0 waits on them)  */
   void* stream_fetch;    /* cudaStream_t: side band for S1-S5 ("async side band")         */
   int32_t attn_impl;     /* lsa_attn_impl; AUTO picks tcgen05 for bf16,H=64,D=512,C=128          */
-  int32_t fetch_mode;    /* lsa_fetch_mode; DEVICE_PULL keeps the whole trigger path on device   */
+  int32_t step_overlap;  /* 0 (default): q / k_new / v_new may be produced by the work enqueued on stream_compute  */
+                         /* just before the call.  1: the caller guarantees they do NOT depend on the previous  */
+                         /* lsa_step's output (independent layers / requests): B <= 4 steps then run underneath  */
+                         /* the previous step's S8 instead of after it              */
   int32_t max_ctas;      /* 0 -> one split-K wave sized from the SM count                       */
   int32_t merge_mode;    /* lsa_merge_mode: where S8 runs (tcgen05 path)                        */
 } lsa_config;

@@ -43,6 +43,13 @@ struct lsa_ctx {
   std::vector<long long> step, visible_at;
   std::vector<char> pending;
   std::vector<int> k_eff;
+  // mirrors the small-batch attention path passes by value (lsa_attn_tc_small.cuh): attended table buffer, entries per
+  // buffer (-1: only the device knows, the selection was given on the device), ring head, appends so far
+  std::vector<int> cur_buf, w_head;
+  std::vector<int> n_tbl[2];
+  std::vector<unsigned int> app_count;
+  bool no_small = false;               // lsa_step_graph: the captured launch must read the device records
+  bool serialize_next = false;         // something the next attention launch reads was enqueued on another stream
   // index scratch
   float* d_z = nullptr;
   float* d_scores = nullptr;
@@ -170,6 +177,11 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   c->visible_at.assign(B, 0);
   c->pending.assign(B, 0);
   c->k_eff.resize(B);
+  c->cur_buf.assign(B, 0);
+  c->w_head.assign(B, 0);
+  c->n_tbl[0].assign(B, 0);
+  c->n_tbl[1].assign(B, 0);
+  c->app_count.assign(B, 0u);
   long long sum_k = 0, total_keys_max = 0, n_keys_max = 0;
   for (int b = 0; b < B; ++b) {
     const lsa_seq_desc& s = seqs[b];
@@ -206,6 +218,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
     c->seq_host[b] = d;
     c->step[b] = s.step0;
     c->k_eff[b] = d.k_eff;
+    c->w_head[b] = s.w_head;
     sum_k += d.k_eff;
     const long long nk = s.n_hca + (long long)d.k_eff * C + cfg->W;
     total_keys_max += nk;
@@ -295,8 +308,8 @@ extern "C" int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs, l
   if (cfg->hot_pages < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "hot_pages must be >= 1");
   if (cfg->merge_mode < LSA_MERGE_AUTO || cfg->merge_mode > LSA_MERGE_FUSED)
     LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad merge_mode");
-  if (cfg->fetch_mode != LSA_FETCH_DEVICE_PULL && cfg->fetch_mode != LSA_FETCH_MEMCPY)
-    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad fetch_mode");
+  if (cfg->step_overlap != 0 && cfg->step_overlap != 1)
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "step_overlap must be 0 or 1");
   lsa_ctx* c = new (std::nothrow) lsa_ctx();
   if (!c) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_OOM, "out of host memory");
   int rc = init_impl(c, cfg, seqs);
@@ -407,7 +420,9 @@ extern "C" int lsa_set_indexer(lsa_ctx* ctx, int32_t indexer) {
 }
 
 // ---- S4-S5 ------------------------------------------------------------------------------------
-static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx) {
+// sel_is_topk: the selection is S3's own output, i.e. exactly k_eff valid ids per sequence (the host then knows the
+// size of the staged table without asking the device)
+static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx, bool sel_is_topk = false) {
   const lsa_config& cfg = c->cfg;
   // the side band must see the tables as of "now" on the compute stream, and may not evict pages
   // an earlier attention launch is still reading
@@ -433,6 +448,7 @@ static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx)
   for (int i = 0; i < n; ++i) {
     c->pending[ids[i]] = 1;
     c->visible_at[ids[i]] = c->step[ids[i]] + cfg.recall_lag;
+    c->n_tbl[1 - c->cur_buf[ids[i]]][ids[i]] = sel_is_topk ? c->k_eff[ids[i]] : -1;
   }
   return LSA_OK;
 }
@@ -455,14 +471,19 @@ static bool due_mask(lsa_ctx* c, bool force, uint32_t words[32]) {
     if (c->pending[b] && (force || c->step[b] >= c->visible_at[b])) {
       words[b >> 5] |= 1u << (b & 31);
       c->pending[b] = 0;
+      c->cur_buf[b] ^= 1;                         // the device flips its record under the same condition
       any = true;
     }
   }
   return any;
 }
 
-static void mirror_append(lsa_ctx* c) {            // host mirror of the ring fill (the kernels apply the same rule)
-  for (int b = 0; b < c->B; ++b) c->seq_host[b].w_len = std::min(c->cfg.W, c->seq_host[b].w_len + 1);
+static void mirror_append(lsa_ctx* c) {            // host mirror of the ring (the kernels apply the same rule)
+  for (int b = 0; b < c->B; ++b) {
+    c->seq_host[b].w_len = std::min(c->cfg.W, c->seq_host[b].w_len + 1);
+    c->w_head[b] = c->w_head[b] + 1 == c->cfg.W ? 0 : c->w_head[b] + 1;
+    c->app_count[b] += 1u;
+  }
 }
 
 // Swap every staged table that is due (or all of them if force) and optionally append k_new/v_new.
@@ -473,6 +494,7 @@ static int prestep_impl(lsa_ctx* c, bool force, const void* k_new, const void* v
   if (any) LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_fetch, 0));
   ProfScope prof(c, LSA_PH_PRESTEP, c->sc);
   LSA_CUDA(c, launch_prestep(c->cfg.dtype, c->d_seqs, c->B, c->cfg.D, c->cfg.W, any ? words : nullptr, 32, k_new, v_new, c->sc));
+  c->serialize_next = true;        // the next attention launch reads what this kernel writes: no early start
   c->attn_launches += 1;
   if (k_new) mirror_append(c);
   return LSA_OK;
@@ -509,12 +531,38 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
     long long tiles = 0;                          // host mirror: HCA + selected pages + window, in 128-key tiles
     for (int b = 0; b < c->B; ++b)
       tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
-    tc_set_l2_mask(c->tc, c->l2_armed ? l2_mask(c->l2) : nullptr);      // one-shot: the selection of this step
-    c->l2_armed = false;
-    int rc = tc_attention(c->tc, q, out, lse, tiles, pre, c->sc, &launches, &ctas, &msg,
-                          prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
-                          prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr,
-                          prof && c->d_ktime ? c->d_ktime + 2 * ia : nullptr);
+    int rc;
+    if (tc_small_supported(c->tc) && !c->l2_armed && !c->no_small) {
+      // small batches: the launch gets the host's mirrors by value and does not wait for its predecessor.  The
+      // mirrors already hold the state AFTER this step's swap and append (due_mask / mirror_append ran).
+      TcSmallStep stp{};
+      const bool app = pre && pre->k_new;
+      for (int b = 0; b < c->B; ++b) {
+        TcSmallSeq& q_ = stp.seq[b];
+        q_.cur = c->cur_buf[b];
+        q_.n_cur = c->n_tbl[q_.cur][b];
+        q_.w_len = c->seq_host[b].w_len;
+        q_.app_slot = app ? (c->w_head[b] == 0 ? c->cfg.W - 1 : c->w_head[b] - 1) : -1;
+        q_.app_count = app ? c->app_count[b] - 1u : c->app_count[b];
+      }
+      stp.swap = pre ? pre->swap[0] : 0u;
+      stp.k_new = app ? pre->k_new : nullptr;
+      stp.v_new = app ? pre->v_new : nullptr;
+      stp.serialize = (!pre || stp.swap || c->serialize_next) ? 1 : 0;
+      stp.wait_inputs = c->cfg.step_overlap ? 0 : 1;
+      c->serialize_next = false;
+      rc = tc_attention_small(c->tc, q, out, lse, stp, c->sc, &launches, &ctas, &msg,
+                              prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
+                              prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr,
+                              prof && c->d_ktime ? c->d_ktime + 2 * ia : nullptr);
+    } else {
+      tc_set_l2_mask(c->tc, c->l2_armed ? l2_mask(c->l2) : nullptr);      // one-shot: the selection of this step
+      c->l2_armed = false;
+      rc = tc_attention(c->tc, q, out, lse, tiles, pre, c->sc, &launches, &ctas, &msg,
+                        prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
+                        prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr,
+                        prof && c->d_ktime ? c->d_ktime + 2 * ia : nullptr);
+    }
     if (prof) {
       cudaEventRecord(c->prof_ev[LSA_PH_COMBINE][2 * ic + 1], c->sc);
       c->prof_n[LSA_PH_ATTENTION] += 1;
@@ -583,7 +631,7 @@ static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_n
     if (c->indexer == LSA_INDEXER_LEVEL1 ? (rc = l1_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))
                                          : (rc = index_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr)))
       return rc;
-    if ((rc = fetch_impl(c, ids, n_fire, c->d_sel))) return rc;
+    if ((rc = fetch_impl(c, ids, n_fire, c->d_sel, c->indexer != LSA_INDEXER_LEVEL1))) return rc;
     if (c->cfg.recall_lag == 0 && (rc = prestep_impl(c, false, nullptr, nullptr))) return rc;   // (c)
   }
   if (q_idx && (rc = l2_select_impl(c, q_idx, w_idx, nullptr, nullptr))) return rc;   // Level 2 sees the tables attention will
@@ -607,6 +655,7 @@ extern "C" int lsa_step_graph(lsa_ctx* ctx, const void* q, const void* h, const 
   bool plain = c->attn_impl != LSA_ATTN_TCGEN05 || c->prof_cap > 0 || c->cfg.merge_mode == LSA_MERGE_FUSED || (k_new && c->cfg.W < 1);
   for (int b = 0; b < c->B && !plain; ++b)
     plain = (c->step[b] % c->cfg.tau == 0) || (c->pending[b] && c->step[b] >= c->visible_at[b]);   // trigger, or a swap is due
+  c->no_small = true;             // the captured launch reads the device records: this context stays on the general kernels
   if (plain) return step_impl(c, q, h, k_new, v_new, out, nullptr, nullptr);
   c->l2_armed = false;
   if (k_new) mirror_append(c);
@@ -767,6 +816,7 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
     const unsigned total = g.n16[0] + g.n16[1] + g.n16[2] + g.n16[3];
     host_gather_kernel<<<std::max(1u, std::min(64u, (total + 255u) / 256u)), 256, 0, c->sc>>>(g);
     LSA_CUDA(c, cudaGetLastError());
+    c->serialize_next = true;
   } else {                         // pageable inputs: pack into the pinned staging image, one host-to-device copy
     unsigned char* pin = static_cast<unsigned char*>(c->st_pin);
     memcpy(pin, q, qb);
@@ -774,6 +824,7 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
     if (k_new) { memcpy(pin + o_kn, k_new, nb); memcpy(pin + o_vn, v_new, nb); upto = o_vn + nb; }
     if (fire) { memcpy(pin + o_h, h, hb); upto = o_h + hb; }          // h is only read at trigger steps
     LSA_CUDA(c, cudaMemcpyAsync(c->st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
+    c->serialize_next = true;
   }
   if (fire) {                      // the indexer reads the staged h on the fetch stream: order it behind the copy
     LSA_CUDA(c, cudaEventRecord(c->ev_compute, c->sc));

@@ -5,6 +5,7 @@
 #include <mutex>
 
 #include "lsa_attn_tc_kernel.cuh"
+#include "lsa_attn_tc_small.cuh"
 
 namespace lsa {
 
@@ -308,9 +309,11 @@ struct TcWorkspace;
 struct TcPlan {
   TcInit init{};
   EncodeTiledFn encode = nullptr;
-  CUtensorMap map_pool{}, map_q{}, map_part{};
+  CUtensorMap map_pool{}, map_pool64{}, map_q{}, map_part{};
   const void* q_cached = nullptr;
   CUtensorMap* d_maps = nullptr;
+  CUtensorMap* d_maps8 = nullptr;      // small path: [B][8], 128-row and 64-row boxes
+  bool small_ok = false;
   TcParams params{};
   unsigned long long grid_total = 0;   // host mirror of the fused-S8 arrival counter
   int grid_max = 0;
@@ -331,15 +334,20 @@ struct TcWorkspace {
   cudaStream_t stream = nullptr;
   size_t slots = 0, grid_max = 0;
   int refs = 0;
-  uint2* part_o = nullptr;
+  uint2* part_o = nullptr;              // two buffers of `slots` each: the small path alternates, the general path uses the first
   float *part_s = nullptr, *part_m = nullptr, *part_l = nullptr;
-  int2* piece_info = nullptr;
+  int2* piece_info = nullptr;           // two buffers of grid_max
+  // small path: launches so far, the combine blocks they add up to, and the totals one and two launches ago
+  unsigned int* comb_ctr = nullptr;     // DEVICE: combine blocks finished
+  unsigned long long n_small = 0;
+  unsigned int comb_total = 0, comb_total_prev = 0;
+  bool last_small = false;              // the last launch on this workspace did not wait for its predecessor
 };
 static std::mutex g_ws_mu;
 static std::vector<TcWorkspace*> g_ws;
 
 static void ws_free(TcWorkspace* w) {
-  cudaFree(w->part_o); cudaFree(w->part_s); cudaFree(w->part_m); cudaFree(w->part_l); cudaFree(w->piece_info);
+  cudaFree(w->part_o); cudaFree(w->part_s); cudaFree(w->part_m); cudaFree(w->part_l); cudaFree(w->piece_info); cudaFree(w->comb_ctr);
   delete w;
 }
 
@@ -351,14 +359,16 @@ static TcWorkspace* ws_acquire(cudaStream_t st, size_t slots, size_t grid_max, s
     if (w->device == device && w->stream == st && w->slots >= slots && w->grid_max >= grid_max) { ++w->refs; return w; }
   TcWorkspace* w = new TcWorkspace();
   w->device = device; w->stream = st; w->slots = slots; w->grid_max = grid_max; w->refs = 1;
-  cudaError_t e = cudaMalloc(&w->part_o, slots * (kTcH * kTcD / 4) * sizeof(uint2));
-  if (e == cudaSuccess) e = cudaMalloc(&w->part_s, slots * kTcPartScales * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&w->part_m, slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&w->part_l, slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, grid_max * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMemset(w->part_m, 0, slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMemset(w->part_l, 0, slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMemset(w->piece_info, 0, grid_max * sizeof(int2));
+  cudaError_t e = cudaMalloc(&w->part_o, 2 * slots * (kTcH * kTcD / 4) * sizeof(uint2));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_s, 2 * slots * kTcPartScales * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_m, 2 * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_l, 2 * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, 2 * grid_max * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMalloc(&w->comb_ctr, sizeof(unsigned int));
+  if (e == cudaSuccess) e = cudaMemset(w->part_m, 0, 2 * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemset(w->part_l, 0, 2 * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemset(w->piece_info, 0, 2 * grid_max * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMemset(w->comb_ctr, 0, sizeof(unsigned int));
   if (e != cudaSuccess) {
     *msg = std::string("split-K workspace: ") + cudaGetErrorString(e);
     ws_free(w);
@@ -439,6 +449,28 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   }
   TC_CUDA(cudaMalloc(&pl->d_maps, maps.size() * sizeof(CUtensorMap)));
   TC_CUDA(cudaMemcpy(pl->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+  if (init.B <= kSmB && !init.fuse_combine) {
+    // small path: every source also as 64-row boxes (a lone half tile), lsa_attn_tc_small.cuh
+    if (!encode_rows(pl->encode, &pl->map_pool64, init.hot_pool, (uint64_t)init.P * 2 * kTcC, kSmHalf, 2, msg)) { delete pl; return -2; }
+    std::vector<CUtensorMap> maps8((size_t)init.B * 8);
+    for (int b = 0; b < init.B; ++b) {
+      const SeqDev& s = init.seq_host[b];
+      const void* ptrs[4] = {s.hca_k, s.hca_v, s.win_k, s.win_v};
+      const uint64_t rows[4] = {(uint64_t)s.n_hca, (uint64_t)s.n_hca, (uint64_t)init.W, (uint64_t)init.W};
+      for (int j = 0; j < 4; ++j) {
+        maps8[(size_t)b * 8 + j] = maps[(size_t)b * 4 + j];
+        const bool none = rows[j] == 0 || ptrs[j] == nullptr;
+        if (!encode_rows(pl->encode, &maps8[(size_t)b * 8 + 4 + j], none ? init.hot_pool : ptrs[j], none ? kTcTile : rows[j], kSmHalf, 2, msg)) {
+          delete pl;
+          return -2;
+        }
+      }
+    }
+    TC_CUDA(cudaMalloc(&pl->d_maps8, maps8.size() * sizeof(CUtensorMap)));
+    TC_CUDA(cudaMemcpy(pl->d_maps8, maps8.data(), maps8.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+    TC_CUDA(cudaFuncSetAttribute(attn_tc_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(SmSmem) + 1024)));
+    pl->small_ok = true;
+  }
   const size_t slots = (size_t)pl->grid_max + init.B;
   TcParams& p = pl->params;
   p.seqs = init.d_seqs; p.tbl_chunk = init.pool.tbl_chunk; p.tbl_page = init.pool.tbl_page; p.seq_maps = pl->d_maps;
@@ -513,6 +545,10 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   cudaLaunchConfig_t lc{};
   lc.gridDim = dim3(grid); lc.blockDim = dim3(kTcThreads); lc.dynamicSmemBytes = pl->smem; lc.stream = st;
   lc.attrs = attr; lc.numAttrs = 1;
+  if (pl->ws->last_small) {       // the small path's launches do not wait for one another: this one waits for all of them
+    lc.numAttrs = 0;
+    pl->ws->last_small = false;
+  }
 #ifdef LSA_TC_TRACE
   static const int no_pdl = getenv("LSA_NO_PDL") ? atoi(getenv("LSA_NO_PDL")) : 0;   // 1: combine, 2: attention, 3: both
   if (no_pdl & 2) lc.numAttrs = 0;
@@ -540,6 +576,66 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
     lc2.gridDim = dim3(16, pl->init.B); lc2.dynamicSmemBytes = 0;
     TC_CUDA(cudaLaunchKernelEx(&lc2, combine_tc_wide_kernel, prm, n_attn, (__nv_bfloat16*)out, lse));
   }
+  *launches = 2;
+  *ctas = n_attn;
+  return 0;
+}
+
+bool tc_small_supported(const TcPlan* pl) { return pl && pl->small_ok; }
+
+int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const TcSmallStep& step, cudaStream_t st, int* launches,
+                       int* ctas, std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1, unsigned long long* ktime) {
+  if (q != pl->q_cached) {
+    if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
+    pl->q_cached = q;
+  }
+  TcWorkspace* ws = pl->ws;
+  const int B = pl->init.B;
+  SmParams prm{};
+  long long halves = 0;                              // upper estimate of the flat half-tile list (sizes the grid)
+  for (int b = 0; b < B; ++b) {
+    const SeqDev& s = pl->init.seq_host[b];
+    const TcSmallSeq& h = step.seq[b];
+    SmSeq& d = prm.seq[b];
+    d.n_hca = s.n_hca; d.cur = h.cur; d.n_cur = h.n_cur; d.w_len = h.w_len; d.app_slot = h.app_slot; d.app_count = h.app_count;
+    d.n_csa = s.n_csa;
+    halves += (s.n_hca + kSmHalf - 1) / kSmHalf + 2 * (h.n_cur >= 0 ? h.n_cur : s.k_eff) + (h.w_len + kSmHalf - 1) / kSmHalf;
+  }
+  const int n_attn = (int)std::max<long long>(1, std::min<long long>(pl->grid_max, halves));
+  const int buf = (int)(ws->n_small & 1);
+  const bool first_after_general = !ws->last_small;  // the general path's combine may still read buffer 0: wait for the stream
+  prm.seqs = pl->init.d_seqs; prm.tbl_chunk = pl->init.pool.tbl_chunk; prm.tbl_page = pl->init.pool.tbl_page; prm.seq_maps = pl->d_maps8;
+  prm.B = B; prm.k = pl->init.k; prm.n_attn = n_attn; prm.scale_log2 = pl->params.scale_log2;
+  prm.part_o = ws->part_o + (size_t)buf * ws->slots * (kTcH * kTcD / 4);
+  prm.part_s = ws->part_s + (size_t)buf * ws->slots * kTcPartScales;
+  prm.part_m = ws->part_m + (size_t)buf * ws->slots * kTcH;
+  prm.part_l = ws->part_l + (size_t)buf * ws->slots * kTcH;
+  prm.piece_info = ws->piece_info + (size_t)buf * ws->grid_max;
+  prm.comb_ctr = ws->comb_ctr; prm.comb_need = ws->comb_total_prev;      // combines up to two launches ago
+  prm.k_new = (const __nv_bfloat16*)step.k_new; prm.v_new = (const __nv_bfloat16*)step.v_new;
+  prm.ktime = ktime;
+  prm.wait_inputs = step.wait_inputs;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t lc{};
+  lc.gridDim = dim3(n_attn); lc.blockDim = dim3(kTcThreads); lc.dynamicSmemBytes = sizeof(SmSmem) + 1024; lc.stream = st;
+  lc.attrs = attr; lc.numAttrs = (step.serialize || first_after_general) ? 0 : 1;
+  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel, pl->map_pool, pl->map_pool64, pl->map_q, prm));
+  if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
+  if (ev_mid1) TC_CUDA(cudaEventRecord(ev_mid1, st));
+  SmCombParams cp{};
+  cp.part_o = prm.part_o; cp.part_s = prm.part_s; cp.part_m = prm.part_m; cp.part_l = prm.part_l; cp.piece_info = prm.piece_info;
+  cp.comb_ctr = ws->comb_ctr; cp.comb_prev = ws->comb_total;
+  cp.seqs_mut = pl->init.d_seqs; cp.swap = step.swap; cp.append = step.k_new ? 1 : 0; cp.W = pl->init.W;
+  cudaLaunchConfig_t lc2{};
+  lc2.gridDim = dim3(128, B); lc2.blockDim = dim3(kCombSmThreads); lc2.dynamicSmemBytes = 0; lc2.stream = st;
+  lc2.attrs = attr; lc2.numAttrs = 1;
+  TC_CUDA(cudaLaunchKernelEx(&lc2, combine_small_kernel, cp, n_attn, (__nv_bfloat16*)out, lse));
+  ws->comb_total_prev = ws->comb_total;
+  ws->comb_total += 128u * (unsigned)B;
+  ws->n_small += 1;
+  ws->last_small = true;
   *launches = 2;
   *ctas = n_attn;
   return 0;
@@ -573,6 +669,7 @@ void tc_destroy(TcPlan* pl) {
   cudaFree(pl->params.tlog);
 #endif
   cudaFree(pl->d_maps);
+  cudaFree(pl->d_maps8);
   ws_release(pl->ws);
   cudaFree(pl->params.grid_ctr);
   delete pl;

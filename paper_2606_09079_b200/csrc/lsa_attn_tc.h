@@ -37,6 +37,29 @@ struct TcPrestep {
 int tc_attention(TcPlan* plan, const void* q, void* out, float* lse, long long tiles_est, const TcPrestep* pre, cudaStream_t st,
                  int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr,
                  unsigned long long* ktime = nullptr /* DEVICE [2] = {~0, 0}: kernel working-time stamps */);
+// ---- small batches (B <= 4): lsa_attn_tc_small.cuh --------------------------------------------------------------
+// The host's mirror of one sequence as the launch will see it (swap and append already applied).
+struct TcSmallSeq {
+  int cur;                  // table buffer attended
+  int n_cur;                // its entries, or -1 when only the device knows (selection given on the device)
+  int w_len;                // attended ring rows, this launch's append included
+  int app_slot;             // ring slot written by this launch, or -1
+  unsigned int app_count;   // appends enqueued before this launch
+};
+struct TcSmallStep {
+  TcSmallSeq seq[4];
+  unsigned int swap;        // bit b: sequence b's staged table becomes current with this launch (records catch up in S8)
+  const void* k_new;        // DEVICE [B][D] or null
+  const void* v_new;
+  int serialize;            // 1: the launch waits for everything before it in the stream (trigger and swap steps); 0: its
+                            // CTAs start as the previous step's leave their SMs, while that step is still being merged
+  int wait_inputs;          // 1: q / k_new / v_new may have been produced by the kernel just before this launch
+};
+bool tc_small_supported(const TcPlan* plan);
+int tc_attention_small(TcPlan* plan, const void* q, void* out, float* lse, const TcSmallStep& step, cudaStream_t st,
+                       int* launches, int* ctas, std::string* msg, cudaEvent_t ev_mid0 = nullptr, cudaEvent_t ev_mid1 = nullptr,
+                       unsigned long long* ktime = nullptr);
+
 // Level 2: key mask [B][k][4] words used by the launches that follow (null: off); see TcParams::l2_mask
 void tc_set_l2_mask(TcPlan* plan, const uint32_t* mask);
 void tc_destroy(TcPlan* plan);

@@ -154,6 +154,7 @@ __device__ __forceinline__ void commit_state(const TcParams& p, int b) {
     const int slot = s.w_head;
     s.w_head = (slot + 1 == p.W) ? 0 : slot + 1;
     s.w_len = min(p.W, s.w_len + 1);
+    s.app_epoch += 1;          // the row was written by the attention grid, which has completed
   }
 }
 

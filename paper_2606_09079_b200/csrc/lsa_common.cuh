@@ -33,6 +33,8 @@ struct SeqDev {
   int cur_buf;             // which of the two table buffers is attended
   int pending;             // a staged table sits in buffer 1-cur_buf
   int n_tbl[2];            // entries per table buffer
+  unsigned int app_epoch;  // ring rows appended so far; bumped with release semantics AFTER the row is written, so a
+                           // launch that does not wait for its predecessor (lsa_attn_tc_small.cuh) can order its reads
 };
 
 struct PoolDev {

@@ -275,6 +275,7 @@ prestep_kernel_v(SeqDev* __restrict__ seqs, int D, int W, SwapWords sw, int use_
       const int slot = sq.w_head;
       sq.w_head = (slot + 1 == W) ? 0 : slot + 1;
       sq.w_len = min(W, sq.w_len + 1);
+      sq.app_epoch += 1;         // visible with the row: this launch is stream-ordered before its readers
     }
   }
 }

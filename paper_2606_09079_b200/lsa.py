@@ -22,7 +22,6 @@ LIB_PATH = os.path.join(_HERE, "liblsa.so")
 
 LSA_F32, LSA_BF16 = 0, 1
 LSA_ATTN_AUTO, LSA_ATTN_SIMT, LSA_ATTN_TCGEN05 = 0, 1, 2
-LSA_FETCH_DEVICE_PULL, LSA_FETCH_MEMCPY = 0, 1
 LSA_MERGE_AUTO, LSA_MERGE_KERNEL, LSA_MERGE_FUSED = 0, 1, 2
 LSA_INDEXER_DUAL_ENCODER, LSA_INDEXER_LEVEL1 = 0, 1
 
@@ -49,7 +48,7 @@ class lsa_config(C.Structure):
                 ("k", C.c_int32), ("tau", C.c_int32), ("recall_lag", C.c_int32), ("sm_scale", C.c_float),
                 ("hot_pages", C.c_int64), ("hot_pool", C.c_void_p), ("W_q", C.c_void_p),
                 ("stream_compute", C.c_void_p), ("stream_fetch", C.c_void_p), ("attn_impl", C.c_int32),
-                ("fetch_mode", C.c_int32), ("max_ctas", C.c_int32), ("merge_mode", C.c_int32)]
+                ("step_overlap", C.c_int32), ("max_ctas", C.c_int32), ("merge_mode", C.c_int32)]
 
 
 class lsa_seq_desc(C.Structure):
@@ -162,7 +161,7 @@ class LsaContext:
                  hot_pool: torch.Tensor, W_q: torch.Tensor, seqs: Sequence[dict], recall_lag: int = 1,
                  sm_scale: float = 0.0, stream_compute: Optional[torch.cuda.Stream] = None,
                  stream_fetch: Optional[torch.cuda.Stream] = None, attn_impl: int = LSA_ATTN_AUTO,
-                 fetch_mode: int = LSA_FETCH_DEVICE_PULL, max_ctas: int = 0, merge_mode: int = LSA_MERGE_AUTO):
+                 step_overlap: int = 0, max_ctas: int = 0, merge_mode: int = LSA_MERGE_AUTO):
         if not torch.cuda.is_available():
             raise LsaError(-2, "no CUDA device: the LSA path has no CPU fallback")
         td = _torch_dtype(dtype)
@@ -183,7 +182,7 @@ class LsaContext:
         cfg.W_q = _dev_ptr(W_q, td, "W_q")
         cfg.stream_compute = self.stream_compute.cuda_stream
         cfg.stream_fetch = self.stream_fetch.cuda_stream
-        cfg.attn_impl, cfg.fetch_mode, cfg.max_ctas, cfg.merge_mode = attn_impl, fetch_mode, max_ctas, merge_mode
+        cfg.attn_impl, cfg.step_overlap, cfg.max_ctas, cfg.merge_mode = attn_impl, step_overlap, max_ctas, merge_mode
         descs = (lsa_seq_desc * self.B)()
         for b, s in enumerate(seqs):
             d = descs[b]

@@ -597,3 +597,101 @@ def test_cfg4_ragged_batch_sampled():
     steps = 70
     r = run_lockstep(wl, rig, steps, check_attention_at={0, 1, 3, 63, 64, 65, 69})
     assert rig.ctx.stats()["triggers"] == 32 + 3      # every sequence once, sequences 0..2 twice
+
+
+# ------------------------------------------------------------------------------- S7-S8, small batches (lsa_attn_tc_small.cuh)
+@pytest.mark.parametrize("overlap", [0, 1])
+@pytest.mark.parametrize("max_ctas", [0, 3, 7])
+def test_small_batch_half_tile_split_edge_cases(max_ctas, overlap):
+    """B <= 4 on the tensor-core path: pieces are cut at 64-row half tiles.  Row counts around the 64 / 128
+    boundaries in the HCA and window segments, cut by 3, 7 and one CTA per SM, so that lone halves, merged
+    halves and ragged tails all occur at piece starts and ends; every sequence against the oracle's attention."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 400
+    g = torch.Generator().manual_seed(31)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    for n_rows, w_len in [([63, 64, 65, 127], [1, 64, 65, 0]), ([128, 129, 191, 192], [127, 128, 129, 193]),
+                          ([1000], [333]), ([0, 257], [64, 0]), ([5, 0, 70], [0, 0, 300])]:
+        B = len(n_rows)
+        hk, hv = [rnd(n, D) for n in n_rows], [rnd(n, D) for n in n_rows]
+        wk, wv = [rnd(W, D) for _ in range(B)], [rnd(W, D) for _ in range(B)]
+        q = rnd(B, H, D)
+        ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.08, max_ctas=max_ctas,
+                          attn_impl=lsa.LSA_ATTN_TCGEN05, step_overlap=overlap)
+        for rep in range(3):
+            out, lse = ctx.decode_attention(q, want_lse=True)
+        ctx.sync()
+        out64, lse = out.double().cpu().numpy(), lse.cpu().numpy()
+        for b in range(B):
+            K = np.concatenate([hk[b].double().cpu().numpy(), wk[b][: w_len[b]].double().cpu().numpy()])
+            V = np.concatenate([hv[b].double().cpu().numpy(), wv[b][: w_len[b]].double().cpu().numpy()])
+            if len(K) == 0:
+                assert torch.all(out[b] == 0) and np.all(lse[b] == -np.inf)
+                continue
+            ref, ref_lse, _ = attention(q[b].double().cpu().numpy(), K, V, 0.08)
+            np.testing.assert_allclose(out64[b], ref, err_msg=f"rows {n_rows} w_len {w_len} seq {b}", **attn_tolerance("bf16"))
+            np.testing.assert_allclose(lse[b], ref_lse, atol=2e-2, rtol=1e-3)
+        ctx.close()
+
+
+@pytest.mark.parametrize("overlap", [0, 1])
+def test_small_batch_steps_back_to_back_without_sync(overlap):
+    """The small-batch launches do not wait for the previous step's merge (double-buffered partials, the ring row
+    ordered by SeqDev::app_epoch): 48 steps of two contexts interleaved on one stream, each with its own q and its
+    own output buffer, no host synchronisation in between; every output is then compared with the oracle, which
+    sees the window grow by one row per step."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W, steps = 64, 512, 640, 48
+    g = torch.Generator().manual_seed(32)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    st = torch.cuda.Stream(dev)
+    rigs = []
+    for n_rows, w_len in [([900, 300], [600, 61]), ([2000], [127])]:
+        B = len(n_rows)
+        hk, hv = [rnd(n, D) for n in n_rows], [rnd(n, D) for n in n_rows]
+        wk, wv = [rnd(W, D) for _ in range(B)], [rnd(W, D) for _ in range(B)]
+        w0k, w0v = [x.clone() for x in wk], [x.clone() for x in wv]
+        lsa_mod = lsa
+        seqs = [dict(cold_csa=None, n_csa=0, chunk_emb=None, hca_k=hk[b], hca_v=hv[b], win_k=wk[b], win_v=wv[b], w_len=w_len[b],
+                     w_head=w_len[b] % W, step0=1) for b in range(B)]
+        ctx = lsa_mod.LsaContext(dtype=1, H=H, D=D, C_=128, W=W, Dh=64, E=64, k=1, tau=1 << 20, sm_scale=0.06,
+                                 hot_pool=torch.zeros((2 * B, 2, 128, D), dtype=torch.bfloat16, device=dev),
+                                 W_q=torch.zeros((64, 64), dtype=torch.bfloat16, device=dev), seqs=seqs, stream_compute=st,
+                                 attn_impl=lsa.LSA_ATTN_TCGEN05, step_overlap=overlap)
+        rigs.append(dict(ctx=ctx, B=B, hk=hk, hv=hv, w0k=w0k, w0v=w0v, w_len=w_len,
+                         q=[rnd(B, H, D) for _ in range(steps)], kn=[rnd(B, D) for _ in range(steps)], vn=[rnd(B, D) for _ in range(steps)],
+                         out=[torch.empty((B, H, D), dtype=torch.bfloat16, device=dev) for _ in range(steps)]))
+    torch.cuda.synchronize()
+    for t in range(steps):
+        for r in rigs:
+            r["ctx"].step(r["q"][t], None, r["kn"][t], r["vn"][t], r["out"][t])
+    st.synchronize()
+    tol = attn_tolerance("bf16")
+    for r in rigs:
+        wk = [x.double().cpu().numpy().copy() for x in r["w0k"]]
+        wv = [x.double().cpu().numpy().copy() for x in r["w0v"]]
+        w_len, head = list(r["w_len"]), [w % W for w in r["w_len"]]
+        for t in range(steps):
+            for b in range(r["B"]):
+                wk[b][head[b]] = r["kn"][t][b].double().cpu().numpy()
+                wv[b][head[b]] = r["vn"][t][b].double().cpu().numpy()
+                head[b] = (head[b] + 1) % W
+                w_len[b] = min(W, w_len[b] + 1)
+                K = np.concatenate([r["hk"][b].double().cpu().numpy(), wk[b][: w_len[b]]])
+                V = np.concatenate([r["hv"][b].double().cpu().numpy(), wv[b][: w_len[b]]])
+                ref, _, _ = attention(r["q"][t][b].double().cpu().numpy(), K, V, 0.06)
+                np.testing.assert_allclose(r["out"][t][b].double().cpu().numpy(), ref, err_msg=f"step {t} seq {b}", **tol)
+        r["ctx"].close()
+
+
+def test_small_batch_step_overlap_lockstep():
+    """lsa_config.step_overlap = 1 (inputs independent of the previous step's output): the whole path in lock-step with
+    the oracle over several trigger periods - triggers, swaps (serialised launches) and the overlapped steps between them."""
+    cfg = make_config(2, B=2, L=[16384 + 4 * 37, 8192], W=1024, k=6, hot_pages=32, steps=40, name="cfg2_overlap", q_gain=16.0, tau=8)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl, step_overlap=1)
+    r = run_lockstep(wl, rig, cfg.steps)
+    assert r["checked"] == cfg.steps
+    rig.ctx.close()
