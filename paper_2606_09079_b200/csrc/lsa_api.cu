@@ -532,8 +532,9 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
     for (int b = 0; b < c->B; ++b)
       tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
     int rc;
-    if (tc_small_supported(c->tc) && !c->l2_armed && !c->no_small) {
-      // small batches: the launch gets the host's mirrors by value and does not wait for its predecessor.  The
+    if (c->cfg.step_overlap && tc_small_supported(c->tc) && !c->l2_armed && !c->no_small) {
+      // small batches whose steps do not depend on one another (lsa_config.step_overlap): one launch per step that
+      // gets the host's mirrors by value, does not wait for its predecessor and merges its own partials.  The
       // mirrors already hold the state AFTER this step's swap and append (due_mask / mirror_append ran).
       TcSmallStep stp{};
       const bool app = pre && pre->k_new;

@@ -313,6 +313,7 @@ struct TcPlan {
   const void* q_cached = nullptr;
   CUtensorMap* d_maps = nullptr;
   CUtensorMap* d_maps8 = nullptr;      // small path: [B][8], 128-row and 64-row boxes
+  SmMaps0 maps0{};                     // those of sequence 0, passed by value
   bool small_ok = false;
   TcParams params{};
   unsigned long long grid_total = 0;   // host mirror of the fused-S8 arrival counter
@@ -337,17 +338,19 @@ struct TcWorkspace {
   uint2* part_o = nullptr;              // two buffers of `slots` each: the small path alternates, the general path uses the first
   float *part_s = nullptr, *part_m = nullptr, *part_l = nullptr;
   int2* piece_info = nullptr;           // two buffers of grid_max
-  // small path: launches so far, the combine blocks they add up to, and the totals one and two launches ago
-  unsigned int* comb_ctr = nullptr;     // DEVICE: combine blocks finished
+  // small path (lsa_attn_tc_small.cuh): launches so far; the CTAs that arrive per buffer / leave in total, as the
+  // host has enqueued them (the kernels wait for these totals)
+  unsigned int* ctrs = nullptr;         // DEVICE [3]: arrivals buffer 0, arrivals buffer 1, CTAs that have left
   unsigned long long n_small = 0;
-  unsigned int comb_total = 0, comb_total_prev = 0;
+  unsigned int arr_total[2] = {0, 0};
+  unsigned int done_total = 0, done_total_prev = 0;     // after the last launch / after the one before it
   bool last_small = false;              // the last launch on this workspace did not wait for its predecessor
 };
 static std::mutex g_ws_mu;
 static std::vector<TcWorkspace*> g_ws;
 
 static void ws_free(TcWorkspace* w) {
-  cudaFree(w->part_o); cudaFree(w->part_s); cudaFree(w->part_m); cudaFree(w->part_l); cudaFree(w->piece_info); cudaFree(w->comb_ctr);
+  cudaFree(w->part_o); cudaFree(w->part_s); cudaFree(w->part_m); cudaFree(w->part_l); cudaFree(w->piece_info); cudaFree(w->ctrs);
   delete w;
 }
 
@@ -364,11 +367,11 @@ static TcWorkspace* ws_acquire(cudaStream_t st, size_t slots, size_t grid_max, s
   if (e == cudaSuccess) e = cudaMalloc(&w->part_m, 2 * slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&w->part_l, 2 * slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, 2 * grid_max * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMalloc(&w->comb_ctr, sizeof(unsigned int));
+  if (e == cudaSuccess) e = cudaMalloc(&w->ctrs, 3 * sizeof(unsigned int));
   if (e == cudaSuccess) e = cudaMemset(w->part_m, 0, 2 * slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMemset(w->part_l, 0, 2 * slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMemset(w->piece_info, 0, 2 * grid_max * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMemset(w->comb_ctr, 0, sizeof(unsigned int));
+  if (e == cudaSuccess) e = cudaMemset(w->ctrs, 0, 3 * sizeof(unsigned int));
   if (e != cudaSuccess) {
     *msg = std::string("split-K workspace: ") + cudaGetErrorString(e);
     ws_free(w);
@@ -466,6 +469,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
         }
       }
     }
+    for (int j = 0; j < 8; ++j) pl->maps0.m[j] = maps8[j];
     TC_CUDA(cudaMalloc(&pl->d_maps8, maps8.size() * sizeof(CUtensorMap)));
     TC_CUDA(cudaMemcpy(pl->d_maps8, maps8.data(), maps8.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
     TC_CUDA(cudaFuncSetAttribute(attn_tc_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(SmSmem) + 1024)));
@@ -601,17 +605,28 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
     d.n_csa = s.n_csa;
     halves += (s.n_hca + kSmHalf - 1) / kSmHalf + 2 * (h.n_cur >= 0 ? h.n_cur : s.k_eff) + (h.w_len + kSmHalf - 1) / kSmHalf;
   }
-  const int n_attn = (int)std::max<long long>(1, std::min<long long>(pl->grid_max, halves));
+  // Two launches are in flight at a time (the next one starts on the SMs this one leaves free), so a launch takes just
+  // under half the SMs - the rest is headroom for the trigger side band - and every CTA the same number of half tiles
+  const long long g_cap = pl->init.max_ctas > 0 ? pl->grid_max : std::max(1, (pl->init.n_sms - 20) / 2);
+  const long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
+  const int n_attn = (int)std::max<long long>(1, std::min<long long>(g_cap, (halves + per - 1) / per));
   const int buf = (int)(ws->n_small & 1);
   const bool first_after_general = !ws->last_small;  // the general path's combine may still read buffer 0: wait for the stream
   prm.seqs = pl->init.d_seqs; prm.tbl_chunk = pl->init.pool.tbl_chunk; prm.tbl_page = pl->init.pool.tbl_page; prm.seq_maps = pl->d_maps8;
   prm.B = B; prm.k = pl->init.k; prm.n_attn = n_attn; prm.scale_log2 = pl->params.scale_log2;
   prm.part_o = ws->part_o + (size_t)buf * ws->slots * (kTcH * kTcD / 4);
-  prm.part_s = ws->part_s + (size_t)buf * ws->slots * kTcPartScales;
-  prm.part_m = ws->part_m + (size_t)buf * ws->slots * kTcH;
+  prm.part_s = ws->part_s + (size_t)buf * ws->slots * kTcPartScales;     // same space, transposed: [32][slots]
+  prm.part_m = ws->part_m + (size_t)buf * ws->slots * kTcH;              // [64][slots]
   prm.part_l = ws->part_l + (size_t)buf * ws->slots * kTcH;
+  prm.n_slots = (int)ws->slots;
   prm.piece_info = ws->piece_info + (size_t)buf * ws->grid_max;
-  prm.comb_ctr = ws->comb_ctr; prm.comb_need = ws->comb_total_prev;      // combines up to two launches ago
+  prm.arr_ctr = ws->ctrs + buf; prm.arr_target = (ws->arr_total[buf] += (unsigned)n_attn);
+  prm.done_ctr = ws->ctrs + 2;
+  prm.done_need_buf = ws->done_total_prev;           // the launch two back (same buffer) has been merged
+  prm.done_need_prev = ws->done_total;               // the previous launch has been merged
+  ws->done_total_prev = ws->done_total;
+  ws->done_total += (unsigned)n_attn;
+  prm.out = (__nv_bfloat16*)out; prm.lse = lse; prm.swap = step.swap; prm.W = pl->init.W;
   prm.k_new = (const __nv_bfloat16*)step.k_new; prm.v_new = (const __nv_bfloat16*)step.v_new;
   prm.ktime = ktime;
   prm.wait_inputs = step.wait_inputs;
@@ -621,22 +636,12 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   cudaLaunchConfig_t lc{};
   lc.gridDim = dim3(n_attn); lc.blockDim = dim3(kTcThreads); lc.dynamicSmemBytes = sizeof(SmSmem) + 1024; lc.stream = st;
   lc.attrs = attr; lc.numAttrs = (step.serialize || first_after_general) ? 0 : 1;
-  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel, pl->map_pool, pl->map_pool64, pl->map_q, prm));
+  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel, pl->map_pool, pl->map_pool64, pl->map_q, pl->maps0, prm));
   if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
   if (ev_mid1) TC_CUDA(cudaEventRecord(ev_mid1, st));
-  SmCombParams cp{};
-  cp.part_o = prm.part_o; cp.part_s = prm.part_s; cp.part_m = prm.part_m; cp.part_l = prm.part_l; cp.piece_info = prm.piece_info;
-  cp.comb_ctr = ws->comb_ctr; cp.comb_prev = ws->comb_total;
-  cp.seqs_mut = pl->init.d_seqs; cp.swap = step.swap; cp.append = step.k_new ? 1 : 0; cp.W = pl->init.W;
-  cudaLaunchConfig_t lc2{};
-  lc2.gridDim = dim3(128, B); lc2.blockDim = dim3(kCombSmThreads); lc2.dynamicSmemBytes = 0; lc2.stream = st;
-  lc2.attrs = attr; lc2.numAttrs = 1;
-  TC_CUDA(cudaLaunchKernelEx(&lc2, combine_small_kernel, cp, n_attn, (__nv_bfloat16*)out, lse));
-  ws->comb_total_prev = ws->comb_total;
-  ws->comb_total += 128u * (unsigned)B;
   ws->n_small += 1;
   ws->last_small = true;
-  *launches = 2;
+  *launches = 1;
   *ctas = n_attn;
   return 0;
 }

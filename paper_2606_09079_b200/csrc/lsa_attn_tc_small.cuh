@@ -22,11 +22,17 @@
 //    A caller whose inputs do not depend on the previous step's output (lsa_config.step_overlap) drops that wait
 //    too: the whole kernel then runs underneath the previous step's merge.
 //
-// 3. The merge (combine_small_kernel) needs 4 KiB of shared memory and < 64 registers per thread, so its blocks are
-//    co-resident with attention CTAs (which leave ~12 KiB of an SM's shared memory free): it waits for ITS
-//    attention grid with griddepcontrol.wait and runs underneath the next step's attention kernel instead of
-//    between the two.  A counter the combine blocks bump on exit (comb_ctr) protects the buffer reuse two launches
-//    later and orders consecutive combines (they write the same records and, typically, the same `out`).
+// 3. S8 runs inside the launch.  A second kernel in the programmatic chain must sit resident and wait for the attention
+//    grid; measured, those waiting blocks pile up on the SMs the next step's CTAs need, and the host pays a second
+//    launch.  Instead every CTA publishes its partials, arrives at a counter (one per workspace buffer), waits for the
+//    launch's other CTAs and merges its share of the output: unit = 4 heads x 32 d; the 8 softmax warps take partials
+//    w, w+8, ... of every CTA of the launch (inactive ones are selected away, so no list is built first) - one
+//    round trip of loads per unit.  A second counter (done_ctr) is bumped on exit: it protects the reuse of the
+//    buffer two launches later and orders the merges of consecutive launches (records, `out`).  All CTAs of a
+//    launch are resident at the same time (grid <= SM count, one CTA per SM; a programmatically dependent launch
+//    starts only after every CTA of its predecessor has started), so the counter barrier cannot starve; waits are
+//    bounded and trap.  Contexts that run CONCURRENTLY on different streams could each hold part of the SMs and
+//    wait for the rest: such contexts must share stream_compute (they then share the workspace) or be run in turn.
 #pragma once
 #include <type_traits>
 
@@ -56,18 +62,30 @@ struct SmParams {
   const CUtensorMap* seq_maps;   // [B][8]: (hca_k, hca_v, win_k, win_v) with 128-row boxes, then with 64-row boxes
   int B, k, n_attn;
   float scale_log2;
-  uint2* part_o;                 // the workspace buffer of this launch (same layout as TcParams)
-  float* part_s;
-  float* part_m;
+  uint2* part_o;                 // the workspace buffer of this launch: O^T partials in TcParams' layout ...
+  float* part_s;                 // ... but m, l and the block scales TRANSPOSED, [64 heads][n_slots] / [32 blocks][n_slots]:
+  float* part_m;                 // S8 reads one head (block) of EVERY slot, which is then one coalesced line per 32 slots
   float* part_l;
+  int n_slots;                   // row length of the transposed arrays
   int2* piece_info;
-  const unsigned int* comb_ctr;  // combine blocks finished so far on this workspace
-  unsigned int comb_need;        // value it must have reached before this launch may overwrite its buffer
+  unsigned int* arr_ctr;         // arrival counter of this launch's workspace buffer (cumulative over its launches)
+  unsigned int arr_target;       // its value once every CTA of this launch has arrived
+  unsigned int* done_ctr;        // CTAs that have left, all launches of the workspace
+  unsigned int done_need_buf;    // value it has reached once the launch that used this buffer last has been merged
+  unsigned int done_need_prev;   // value it has reached once the previous launch has been merged
+  __nv_bfloat16* out;            // [B][H][D]
+  float* lse;                    // [B][H] or null
+  unsigned int swap;             // bit b: sequence b's staged table becomes current with this launch (records catch up here)
+  int W;                         // ring capacity
   const __nv_bfloat16* k_new;    // [B][D] or null
   const __nv_bfloat16* v_new;
   int wait_inputs;               // 1: griddepcontrol.wait before q / k_new / v_new are read
   unsigned long long* ktime;     // profiling only, see TcParams
 };
+
+// the eight tensor maps of sequence 0 travel with the launch (param space: no descriptor fetch from global memory
+// in front of the first TMA); sequences 1.. use SmParams::seq_maps
+struct SmMaps0 { CUtensorMap m[8]; };
 
 struct SmSmem {
   alignas(1024) unsigned char q[65536];                       // [8 d-blocks][64 heads][128 B], SW128
@@ -79,6 +97,9 @@ struct SmSmem {
   SmSeq seq[kSmB];
   int hh_hca[kSmB], hh_pg[kSmB];                              // half tiles of the HCA rows / of the pages
   int gpre[kSmB + 1];                                         // prefix of half tiles per sequence
+  int pg_page[32], pg_chunk[32];                              // table entries of the pages in this CTA's range
+  int pg_off[kSmB], pg_cnt;                                   // entry of (sequence b, table position t) = pg_off[b] + t
+  int k0_early;                                               // the setup already requested K of the first sub-tile
   uint64_t full[kTcStages], empty[kTcStages];
   uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup, app_done;
   uint32_t tmem_base;
@@ -158,19 +179,146 @@ struct SubCursor {
   }
 };
 
+// table entry of a page sub-tile: prefetched into shared memory by the setup, else (more than 32 pages in the range) global
+__device__ __forceinline__ int sub_entry(const SmParams& p, const SmSmem& sm, const SubTile& s, const int* tbl, const int* pre) {
+  const int i = sm.pg_off[s.b] + s.t;
+  if (i >= 0 && i < sm.pg_cnt) return pre[i];
+  return tbl[((size_t)s.b * 2 + sm.seq[s.b].cur) * p.k + s.t];
+}
+
 // attended rows of a sub-tile (the rest of its rows is masked)
 __device__ __forceinline__ int sub_valid(const SmParams& p, const SmSmem& sm, const SubTile& s) {
   const SmSeq& q = sm.seq[s.b];
   if (s.kind == 0) return min(s.rows, q.n_hca - s.row0);
   if (s.kind == 2) return min(s.rows, q.w_len - s.row0);
-  const int chunk = p.tbl_chunk[((size_t)s.b * 2 + q.cur) * p.k + s.t];
+  const int chunk = sub_entry(p, sm, s, p.tbl_chunk, sm.pg_chunk);
   const int vc = (int)max(0ll, min((long long)kTcC, q.n_csa - (long long)chunk * kTcC));
   return max(0, min(s.rows, vc - s.row0));
 }
 
+
+__device__ __forceinline__ float4 sm_warp_max4(float4 v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    v.x = fmaxf(v.x, __shfl_xor_sync(0xffffffffu, v.x, o)); v.y = fmaxf(v.y, __shfl_xor_sync(0xffffffffu, v.y, o));
+    v.z = fmaxf(v.z, __shfl_xor_sync(0xffffffffu, v.z, o)); v.w = fmaxf(v.w, __shfl_xor_sync(0xffffffffu, v.w, o));
+  }
+  return v;
+}
+__device__ __forceinline__ float4 sm_warp_sum4(float4 v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    v.x += __shfl_xor_sync(0xffffffffu, v.x, o); v.y += __shfl_xor_sync(0xffffffffu, v.y, o);
+    v.z += __shfl_xor_sync(0xffffffffu, v.z, o); v.w += __shfl_xor_sync(0xffffffffu, v.w, o);
+  }
+  return v;
+}
+__device__ __forceinline__ float sm_w_of(float m, float M) { return m == -INFINITY ? 0.f : exp2f(m - M); }
+
+// S8 (see the header, item 3).  Called by the 256 softmax threads (t = 0..255) of every CTA once all partials of the
+// launch are visible.  Unit = (sequence b, 32 consecutive uint2 columns cc of the partial layout) = 4 heads x 32 d, 256
+// per sequence; CTA c takes units [c * NU / n_cta, (c + 1) * NU / n_cta), two at a time: warps 0-3 the first, warps 4-7
+// the second, warp (w & 3) the slots of CTAs (w & 3), (w & 3) + 4, ...  EVERYTHING a pair of units needs is requested
+// before anything is waited for - the fp16 columns of all slots, and (lane l: CTAs l, l + 32, ...) piece_info, m, l and
+// the block scale, which every warp fetches for itself so that no weight crosses a warp - so the merge is one memory
+// round trip deep.  Inactive slots get scale 0 and are selected away, never multiplied.
+// scratch: >= 4 KiB of shared memory the attention phase no longer uses (the Q tile buffer).
+constexpr int kMrgData = 40;                  // slots per warp: kSG * 40 >= n_cta
+// kSG = warps per unit: 4 (two units at a time, n_cta <= 160) or 2 (four units at a time, n_cta <= 80)
+template <int kSG>
+__device__ __noinline__ void small_merge(const SmParams& p, unsigned char* scratch, int cta, int n_cta, int t) {
+  constexpr int kMrgW = kSG == 4 ? 5 : 3;     // slots per lane: ceil(n_cta max / 32)
+  constexpr int kPer = 8 / kSG;               // units per iteration
+  const int w = t >> 5, lane = t & 31, sg = w % kSG, half = w / kSG;
+  float4* red = reinterpret_cast<float4*>(scratch);              // [units per iteration][kSG slot groups][32 lanes]
+  const int NU = p.B * 256;
+  const int u0 = (int)((unsigned)cta * (unsigned)NU / (unsigned)n_cta), u1 = (int)((unsigned)(cta + 1) * (unsigned)NU / (unsigned)n_cta);
+  for (int ub = u0; ub < u1; ub += kPer) {
+    const int u = ub + half;
+    const bool on = u < u1;
+    const int b = on ? u >> 8 : 0, cc = u & 255;
+    const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
+    // ---- requests ----
+    const uint2* col = p.part_o + (size_t)b * (kTcH * kTcD / 4) + cc * 32 + lane;      // slot (c + b), this lane's column
+    uint2 v[kMrgData];
+#pragma unroll
+    for (int j = 0; j < kMrgData; ++j)
+      v[j] = (on && sg + kSG * j < n_cta) ? *(col + (size_t)(sg + kSG * j) * (kTcH * kTcD / 4)) : make_uint2(0u, 0u);
+    float4 mj[kMrgW], lj[kMrgW];
+    float sj[kMrgW];
+#pragma unroll
+    for (int r = 0; r < kMrgW; ++r) {
+      const int c = lane + 32 * r;
+      mj[r] = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY); lj[r] = make_float4(0.f, 0.f, 0.f, 0.f); sj[r] = 0.f;
+      if (on && c < n_cta) {
+        const size_t s = (size_t)c + b, ns = (size_t)p.n_slots;
+        const int2 info = p.piece_info[c];
+        const float* pm = p.part_m + (size_t)h0 * ns + s;
+        const float* pl = p.part_l + (size_t)h0 * ns + s;
+        const float4 m4 = make_float4(pm[0], pm[ns], pm[2 * ns], pm[3 * ns]);
+        const float4 l4 = make_float4(pl[0], pl[ns], pl[2 * ns], pl[3 * ns]);
+        const float s1 = p.part_s[(size_t)((m * 2 + hh) * 4 + dq) * ns + s];
+        // CTA c wrote a partial for sequence b, and the piece had an attended key (else it wrote no O)
+        if (info.x <= b && b < info.x + info.y && m4.x != -INFINITY) { mj[r] = m4; lj[r] = l4; sj[r] = s1; }
+      }
+    }
+    // ---- weights (every warp for itself) ----
+    float4 M = mj[0];
+#pragma unroll
+    for (int r = 1; r < kMrgW; ++r) { M.x = fmaxf(M.x, mj[r].x); M.y = fmaxf(M.y, mj[r].y); M.z = fmaxf(M.z, mj[r].z); M.w = fmaxf(M.w, mj[r].w); }
+    M = sm_warp_max4(M);
+    float4 L = make_float4(0.f, 0.f, 0.f, 0.f), ws[kMrgW];
+#pragma unroll
+    for (int r = 0; r < kMrgW; ++r) {
+      const float4 wj = make_float4(sm_w_of(mj[r].x, M.x), sm_w_of(mj[r].y, M.y), sm_w_of(mj[r].z, M.z), sm_w_of(mj[r].w, M.w));
+      L.x = fmaf(wj.x, lj[r].x, L.x); L.y = fmaf(wj.y, lj[r].y, L.y); L.z = fmaf(wj.z, lj[r].z, L.z); L.w = fmaf(wj.w, lj[r].w, L.w);
+      ws[r] = make_float4(wj.x * sj[r], wj.y * sj[r], wj.z * sj[r], wj.w * sj[r]);
+    }
+    L = sm_warp_sum4(L);
+    // ---- weighted sum of this warp's slots ----
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int j = 0; j < kMrgData; ++j) {
+      constexpr int kRound = 32 / kSG;                           // slot sg + kSG j is held by lane src, round j / kRound
+      const int src = (sg + kSG * j) & 31;
+      const float fx = __shfl_sync(0xffffffffu, ws[j / kRound].x, src), fy = __shfl_sync(0xffffffffu, ws[j / kRound].y, src);
+      const float fz = __shfl_sync(0xffffffffu, ws[j / kRound].z, src), fw = __shfl_sync(0xffffffffu, ws[j / kRound].w, src);
+      const float sc = __shfl_sync(0xffffffffu, sj[j / kRound], src);
+      if (sc != 0.f) {
+        const float2 a01 = unpack_f16x2(v[j].x), a23 = unpack_f16x2(v[j].y);
+        acc.x = fmaf(fx, a01.x, acc.x); acc.y = fmaf(fy, a01.y, acc.y);
+        acc.z = fmaf(fz, a23.x, acc.z); acc.w = fmaf(fw, a23.y, acc.w);
+      }
+    }
+    red[(half * kSG + sg) * 32 + lane] = acc;
+    named_bar_sync(2, 256);
+    if (sg == 0 && on) {                                         // one warp per unit: 4 heads x 32 d
+      float4 num = red[(half * kSG) * 32 + lane];
+#pragma unroll
+      for (int i = 1; i < kSG; ++i) {
+        const float4 a = red[(half * kSG + i) * 32 + lane];
+        num.x += a.x; num.y += a.y; num.z += a.z; num.w += a.w;
+      }
+      __nv_bfloat16* o = p.out + ((size_t)b * kTcH + h0) * kTcD + m * 128 + dq * 32 + lane;
+      o[0] = __float2bfloat16_rn(L.x > 0.f ? num.x / L.x : 0.f);
+      o[kTcD] = __float2bfloat16_rn(L.y > 0.f ? num.y / L.y : 0.f);
+      o[2 * kTcD] = __float2bfloat16_rn(L.z > 0.f ? num.z / L.z : 0.f);
+      o[3 * kTcD] = __float2bfloat16_rn(L.w > 0.f ? num.w / L.w : 0.f);
+      if (p.lse && m == 0 && dq == 0 && lane == 0) {
+        float* ls = p.lse + (size_t)b * kTcH + h0;
+        ls[0] = L.x > 0.f ? (M.x + log2f(L.x)) * 0.6931471805599453f : -INFINITY;
+        ls[1] = L.y > 0.f ? (M.y + log2f(L.y)) * 0.6931471805599453f : -INFINITY;
+        ls[2] = L.z > 0.f ? (M.z + log2f(L.z)) * 0.6931471805599453f : -INFINITY;
+        ls[3] = L.w > 0.f ? (M.w + log2f(L.w)) * 0.6931471805599453f : -INFINITY;
+      }
+    }
+    named_bar_sync(2, 256);                                      // `red` is reused by the next pair
+  }
+}
+
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_constant__ CUtensorMap map_pool64,
-                     const __grid_constant__ CUtensorMap map_q, const __grid_constant__ SmParams p) {
+                     const __grid_constant__ CUtensorMap map_q, const __grid_constant__ SmMaps0 maps0, const __grid_constant__ SmParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   SmSmem& sm = *reinterpret_cast<SmSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -193,17 +341,17 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   griddep_launch_dependents();    // the combine blocks of this step (and, behind them, the next step's CTAs) may be placed
   if (p.ktime && tid == 0) atomicMin(p.ktime, gtime());
   if (warp == 0) {
-    // per-sequence shape -> half tiles per segment and their prefix (B <= 4); ring rows appended by earlier
-    // launches are visible once app_epoch has caught up with the host's count
-    int g = 0;
+    // per-sequence shape -> half tiles per segment and their prefix (B <= 4).  Everything this CTA needs from global
+    // memory before its first TMA is requested in ONE round trip: the table entries of the pages in its range, the
+    // tensor maps of its sequences, and - only if its range holds window rows - the append counter.
+    int g = 0, hca = 0, pg = 0;
+    SmSeq q{};
     if (lane < p.B) {
-      SmSeq q = p.seq[lane];
-      if (q.n_cur < 0) q.n_cur = __ldcg(&p.seqs[lane].n_tbl[q.cur]);
-      wait_counter(&p.seqs[lane].app_epoch, q.app_count, 50);
-      sm.seq[lane] = q;
-      const int hca = (q.n_hca + kSmHalf - 1) / kSmHalf, pg = 2 * q.n_cur, win = (q.w_len + kSmHalf - 1) / kSmHalf;
-      sm.hh_hca[lane] = hca; sm.hh_pg[lane] = pg;
-      g = hca + pg + win;
+      q = p.seq[lane];
+      if (q.n_cur < 0) q.n_cur = __ldcg(&p.seqs[lane].n_tbl[q.cur]);       // selection given on the device: its size too
+      hca = (q.n_hca + kSmHalf - 1) / kSmHalf; pg = 2 * q.n_cur;
+      g = hca + pg + (q.w_len + kSmHalf - 1) / kSmHalf;
+      sm.seq[lane] = q; sm.hh_hca[lane] = hca; sm.hh_pg[lane] = pg;
     }
     int incl = g;
 #pragma unroll
@@ -213,6 +361,53 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     }
     if (lane < p.B) sm.gpre[lane + 1] = incl;
     if (lane == 0) sm.gpre[0] = 0;
+    const unsigned T = (unsigned)__shfl_sync(0xffffffffu, incl, p.B - 1);
+    const int f0 = (int)((unsigned)cta * T / (unsigned)n_cta), f1 = (int)((unsigned)(cta + 1) * T / (unsigned)n_cta);
+    __syncwarp();
+    // A range that starts in HCA rows needs nothing from global memory: its first K sub-tile is requested right here,
+    // ahead of the table / counter look-ups below (sm.k0_early tells the producer loop)
+    {
+      SubCursor c0(sm, p.B, cta, n_cta);
+      SubTile s0;
+      const bool early = c0.next(s0) && s0.kind == 0;
+      if (lane == 0) sm.k0_early = early ? 1 : 0;
+      if (early && elect_one()) {
+        const uint64_t pol = l2_policy_evict_first();
+        const CUtensorMap* mk = (s0.b == 0 ? maps0.m : p.seq_maps + s0.b * 8) + (s0.rows == kTcTile ? 0 : 4);
+#pragma unroll 1
+        for (int s4 = 0; s4 < 4; ++s4) {
+          mbar_arrive_expect_tx(&sm.full[s4], (uint32_t)s0.rows * 256u);
+          tma_load_3d_hint(sm.stage[s4], mk, 0, s0.row0, s4 * 2, &sm.full[s4], pol);
+        }
+      }
+    }
+    int cnt = 0;                                       // page slots of this CTA's range, all sequences
+#pragma unroll
+    for (int b = 0; b < kSmB; ++b) {
+      const int end_b = __shfl_sync(0xffffffffu, incl, b), g_b = __shfl_sync(0xffffffffu, g, b);
+      const int hca_b = __shfl_sync(0xffffffffu, hca, b), pg_b = __shfl_sync(0xffffffffu, pg, b), cur_b = __shfl_sync(0xffffffffu, q.cur, b);
+      if (b < p.B) {
+        const int base = end_b - g_b + hca_b;          // first page half tile of sequence b in the flat list
+        const int lo = max(f0, base), hi = min(f1, base + pg_b);
+        int off = -(1 << 30);
+        if (lo < hi) {
+          const int t_lo = (lo - base) >> 1, n = ((hi - 1 - base) >> 1) - t_lo + 1;
+          off = cnt - t_lo;
+          if (lane >= cnt && lane < cnt + n) {
+            const size_t e = ((size_t)b * 2 + cur_b) * p.k + t_lo + lane - cnt;
+            sm.pg_page[lane] = __ldcg(p.tbl_page + e);
+            sm.pg_chunk[lane] = __ldcg(p.tbl_chunk + e);
+          }
+          cnt += n;
+        }
+        if (lane == 0) sm.pg_off[b] = off;
+        // window rows in the range: ring rows appended by earlier launches are visible once app_epoch has caught
+        // up with the host's count (normally it has)
+        if (lane == b && f1 > base + pg_b && f0 < end_b) wait_counter(&p.seqs[b].app_epoch, q.app_count, 50);
+        if (b > 0 && f0 < end_b && f1 > end_b - g_b && lane < 8) prefetch_tmap(p.seq_maps + b * 8 + lane);
+      }
+    }
+    if (lane == 0) sm.pg_cnt = min(cnt, 32);
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm.setup);
   } else if (warp == 1) {
@@ -224,7 +419,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     for (int i = tid - 64; i < 2048; i += kTcThreads - 64) reinterpret_cast<uint16_t*>(sm.ones)[i] = 0x3f80;   // bf16 1.0
     fence_proxy_async_smem();
     // the partials of two launches ago (same buffer) have been merged
-    if (tid == 64) wait_counter(p.comb_ctr, p.comb_need, 51);
+    if (tid == 64) wait_counter(p.done_ctr, p.done_need_buf, 51);
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm.setup);
   }
@@ -232,20 +427,20 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   if (warp == 0) {
     // =========================== TMA producer ===========================
     if (elect_one()) {
-      fence_proxy_async_all();                            // ring rows written by other CTAs' generic stores -> TMA reads
       SubCursor cur(sm, p.B, cta, n_cta);
       SubTile s, nx;
-      uint32_t ring = 0;
+      uint32_t ring = sm.k0_early ? 4u : 0u;
       int item = 0;
-      bool app_seen = false, waited = false;
+      bool app_seen = false, waited = false, k0_pending = sm.k0_early != 0;
+      const uint64_t pol_stream = l2_policy_evict_first();   // K/V rows: read once per step
       auto src_of = [&](const SubTile& t, const CUtensorMap*& mk, const CUtensorMap*& mv, int& rk, int& rv) {
         const int big = t.rows == kTcTile ? 0 : 4;
         if (t.kind == 1) {
-          const int page = p.tbl_page[((size_t)t.b * 2 + sm.seq[t.b].cur) * p.k + t.t];
+          const int page = sub_entry(p, sm, t, p.tbl_page, sm.pg_page);
           mk = mv = (t.rows == kTcTile ? &map_pool : &map_pool64);
           rk = page * (2 * kTcC) + t.row0; rv = rk + kTcC;
         } else {
-          mk = p.seq_maps + t.b * 8 + big + (t.kind == 0 ? 0 : 2);
+          mk = (t.b == 0 ? maps0.m : p.seq_maps + t.b * 8) + big + (t.kind == 0 ? 0 : 2);
           mv = mk + 1;
           rk = rv = t.row0;
         }
@@ -256,8 +451,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         const SmSeq& q = sm.seq[t.b];
         if (t.kind == 2 && p.k_new && q.app_slot >= t.row0 && q.app_slot < t.row0 + t.rows) {
           if (!app_seen) { mbar_wait(&sm.app_done, 0, 12); app_seen = true; }   // every row of this CTA is written by then
-          st_release_u32(&p.seqs[t.b].app_epoch, q.app_count + 1u);
-          fence_proxy_async_all();
+          st_release_u32(&p.seqs[t.b].app_epoch, q.app_count + 1u);   // (the writers fenced generic -> async proxy)
         }
       };
       auto issue4 = [&](const CUtensorMap* m, int row, int rows) {
@@ -266,7 +460,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
           const int st = ring % kTcStages;
           mbar_wait(&sm.empty[st], ((ring / kTcStages) & 1) ^ 1, 11);
           mbar_arrive_expect_tx(&sm.full[st], (uint32_t)rows * 256u);
-          tma_load_3d(sm.stage[st], m, 0, row, s4 * 2, &sm.full[st]);
+          tma_load_3d_hint(sm.stage[st], m, 0, row, s4 * 2, &sm.full[st], pol_stream);
           ++ring;
         }
       };
@@ -277,9 +471,11 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         src_of(s, mk, mv, rk, rv);
         if (s.first) {
           app_gate(s);
-          issue4(mk, rk, s.rows);                          // K of the piece's first sub-tile: in flight before Q is known
+          if (!k0_pending) issue4(mk, rk, s.rows);         // K of the piece's first sub-tile: in flight before Q is known
+          k0_pending = false;
           if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 10);
           if (p.wait_inputs && !waited) { griddep_wait(); waited = true; }   // q is the caller's: whatever the stream ran last
+                                                    // after griddep_wait
           mbar_arrive_expect_tx(&sm.q_full, 65536);
           tma_load_3d(sm.q, &map_q, 0, s.b * kTcH, 0, &sm.q_full);
         }
@@ -295,6 +491,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (s.last) ++item;
         s = nx;
       }
+                                                    // all loads issued
     }
   } else if (warp == 1) {
     // =========================== MMA issuer ===========================
@@ -386,6 +583,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (s.last) ++item;
         s = nx;
       }
+                                                    // last PV issued (last V landed)
     }
   } else {
     // =========================== softmax + epilogue (8 warps) ===========================
@@ -450,7 +648,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (b_first < 0) b_first = b;
         // sequences without keys between two pieces of this CTA get an empty partial (weight 0 in S8)
         for (int e = b_last + 1; b_last >= 0 && e < b; ++e)
-          if (tid < 64 + kTcH) { p.part_m[((size_t)cta + e) * kTcH + tid - 64] = -INFINITY; p.part_l[((size_t)cta + e) * kTcH + tid - 64] = 0.f; }
+          if (tid < 64 + kTcH) { p.part_m[(size_t)(tid - 64) * p.n_slots + cta + e] = -INFINITY; p.part_l[(size_t)(tid - 64) * p.n_slots + cta + e] = 0.f; }
         b_last = b;
       }
       const bool first = s.first, last = s.last;
@@ -541,7 +739,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         for (int j = 0; j < 32; ++j) amax = fmaxf(amax, fabsf(__uint_as_float(vreg[j])));
         float inv;
         const float sc = part_scale(redux_max_f32(amax), &inv);   // one scale per warp: 32 d-rows x 32 heads
-        if (lane == 0) p.part_s[part_scale_idx(slot, m, hh, q4)] = inv;
+        if (lane == 0) p.part_s[(size_t)((m * 2 + hh) * 4 + q4) * p.n_slots + slot] = inv;
 #pragma unroll
         for (int g = 0; g < 8; ++g)
           po[(size_t)m * (2 * 8 * 128) + g * 128] =
@@ -555,8 +753,8 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (lane == 0) {
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
-            p.part_l[slot * kTcH + hh * 32 + j] = __uint_as_float(vreg[j]);
-            p.part_m[slot * kTcH + hh * 32 + j] = m_run[j] <= -1e30f ? -INFINITY : m_run[j];   // no attended key: S8 skips the slot
+            p.part_l[(size_t)(hh * 32 + j) * p.n_slots + slot] = __uint_as_float(vreg[j]);
+            p.part_m[(size_t)(hh * 32 + j) * p.n_slots + slot] = m_run[j] <= -1e30f ? -INFINITY : m_run[j];   // no attended key: S8 skips the slot
           }
         }
       }
@@ -567,188 +765,39 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     }
     if (tid == 64) p.piece_info[cta] = make_int2(b_first < 0 ? 0 : b_first, b_first < 0 ? 0 : b_last - b_first + 1);
   }
-  // ---- teardown ----
+  // ---- S8: publish, meet the other CTAs of the launch, merge this CTA's share ----
   tc_fence_before();
+  if (warp >= 2) __threadfence();                   // this thread's partial stores are visible device-wide
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(sm.tmem_base, 512);
   }
-  if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
-}
-
-// ---- S8 under the next step's attention ---------------------------------------------------------------------------
-// grid (128, B) x 128 threads; block = (m, hh, g, dh) = 512 contiguous bytes (64 d x 4 heads fp16) of every slot, as in
-// combine_tc_kernel.  A warp reads a whole 512-byte row per load (16 bytes per lane = 2 d x 4 heads), the four warps take
-// slots w, w+4, ...; weights and scales go through 4 KiB of shared memory.
-constexpr int kCombSmThreads = 128;
-constexpr int kCombSmUnroll = 8;
-
-struct SmCombParams {
-  const uint2* part_o;
-  const float* part_s;
-  const float* part_m;
-  const float* part_l;
-  const int2* piece_info;
-  unsigned int* comb_ctr;
-  unsigned int comb_prev;        // blocks of every earlier combine on this workspace: they have finished before this one writes
-  SeqDev* seqs_mut;              // S6 / window append folded into the attention launch: the records catch up here
-  unsigned int swap;             // bit b: sequence b's staged table became current in this step
-  int append;                    // 1: the step appended a ring row
-  int W;
-};
-
-__global__ void __launch_bounds__(kCombSmThreads)
-combine_small_kernel(const __grid_constant__ SmCombParams p, int n_cta, __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
-  __shared__ float4 w_s[256];                     // weights by CTA; reused for the cross-warp sum at the end
-  __shared__ float2 sc_s[256];
-  __shared__ float4 red_f[4];
-  float4 (*acc_s)[32][2] = reinterpret_cast<float4 (*)[32][2]>(w_s);   // [4 warps][32 lanes][2]
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int dh = blockIdx.x & 1, g = (blockIdx.x >> 1) & 7, hh = (blockIdx.x >> 4) & 1, m = blockIdx.x >> 5, b = blockIdx.y;
-  const int h0 = hh * 32 + g * 4;
-  griddep_launch_dependents();                    // the next step's attention CTAs may be placed as SMs free up
-  griddep_wait();                                 // this step's partials and piece_info are final from here on
-  if (tid == 0) wait_counter(p.comb_ctr, p.comb_prev, 52);   // every earlier combine has finished (records, `out`)
+  if (tid == 0) {
+    red_release_add_u32(p.arr_ctr, 1u);
+    wait_counter(p.arr_ctr, p.arr_target, 53);      // every partial of the launch is visible from here on
+    wait_counter(p.done_ctr, p.done_need_prev, 54); // the previous launch has been merged (records, `out`)
+  }
   __syncthreads();
-  if (blockIdx.x == 0 && tid == 0) {              // the per-sequence record catches up with the launch's view
-    SeqDev& s = p.seqs_mut[b];
-    if (((p.swap >> b) & 1u) && s.pending) { s.cur_buf = 1 - s.cur_buf; s.pending = 0; }
-    if (p.append) {
-      const int slot = s.w_head;
-      s.w_head = (slot + 1 == p.W) ? 0 : slot + 1;
-      s.w_len = min(p.W, s.w_len + 1);
+  if (cta == 0 && tid < p.B) {                      // the per-sequence record catches up with the launch's view
+    SeqDev& sd = p.seqs[tid];
+    if (((p.swap >> tid) & 1u) && sd.pending) { sd.cur_buf = 1 - sd.cur_buf; sd.pending = 0; }
+    if (p.k_new) {
+      const int slot = sd.w_head;
+      sd.w_head = (slot + 1 == p.W) ? 0 : slot + 1;
+      sd.w_len = min(p.W, sd.w_len + 1);
     }
   }
-  // thread c (and c + 128) looks at CTA c: did it write a partial for sequence b?  (n_cta <= 256)
-  float4 mi[2], li[2];
-  float2 s2[2];
-  bool act[2];
-  float4 mmax = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
-#pragma unroll
-  for (int r = 0; r < 2; ++r) {
-    const int c = tid + r * kCombSmThreads;
-    mi[r] = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
-    li[r] = make_float4(0.f, 0.f, 0.f, 0.f);
-    s2[r] = make_float2(0.f, 0.f);
-    act[r] = false;
-    if (c < n_cta) {
-      const size_t slot = (size_t)c + b;
-      const int2 info = __ldcg(p.piece_info + c);
-      const float4 m4 = __ldcg(reinterpret_cast<const float4*>(p.part_m + slot * kTcH + h0));
-      const float4 l4 = __ldcg(reinterpret_cast<const float4*>(p.part_l + slot * kTcH + h0));
-      s2[r] = __ldcg(reinterpret_cast<const float2*>(p.part_s + part_scale_idx(slot, m, hh, dh * 2)));
-      // a piece without valid keys (m = -inf for every head) wrote no O: its slot is skipped like an inactive one
-      act[r] = info.x <= b && b < info.x + info.y && m4.x != -INFINITY;
-      if (act[r]) { mi[r] = m4; li[r] = l4; }
-    }
-    mmax.x = fmaxf(mmax.x, mi[r].x); mmax.y = fmaxf(mmax.y, mi[r].y); mmax.z = fmaxf(mmax.z, mi[r].z); mmax.w = fmaxf(mmax.w, mi[r].w);
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    mmax.x = fmaxf(mmax.x, __shfl_xor_sync(0xffffffffu, mmax.x, o));
-    mmax.y = fmaxf(mmax.y, __shfl_xor_sync(0xffffffffu, mmax.y, o));
-    mmax.z = fmaxf(mmax.z, __shfl_xor_sync(0xffffffffu, mmax.z, o));
-    mmax.w = fmaxf(mmax.w, __shfl_xor_sync(0xffffffffu, mmax.w, o));
-  }
-  if (lane == 0) red_f[warp] = mmax;
-  __syncthreads();
-  float4 m_star = red_f[0];
-#pragma unroll
-  for (int w = 1; w < 4; ++w) {
-    const float4 r = red_f[w];
-    m_star.x = fmaxf(m_star.x, r.x); m_star.y = fmaxf(m_star.y, r.y); m_star.z = fmaxf(m_star.z, r.z); m_star.w = fmaxf(m_star.w, r.w);
-  }
-  float4 lsum = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-  for (int r = 0; r < 2; ++r) {
-    const int c = tid + r * kCombSmThreads;
-    float4 wi = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (act[r]) {
-      wi.x = mi[r].x == -INFINITY ? 0.f : exp2f(mi[r].x - m_star.x);
-      wi.y = mi[r].y == -INFINITY ? 0.f : exp2f(mi[r].y - m_star.y);
-      wi.z = mi[r].z == -INFINITY ? 0.f : exp2f(mi[r].z - m_star.z);
-      wi.w = mi[r].w == -INFINITY ? 0.f : exp2f(mi[r].w - m_star.w);
-    }
-    // an inactive slot keeps scale 0: its (possibly stale) data is multiplied by 0 weights below only if finite,
-    // so it is skipped by the scale test instead
-    if (c < 256) { w_s[c] = wi; sc_s[c] = act[r] ? s2[r] : make_float2(0.f, 0.f); }
-    lsum.x += wi.x * li[r].x; lsum.y += wi.y * li[r].y; lsum.z += wi.z * li[r].z; lsum.w += wi.w * li[r].w;
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    lsum.x += __shfl_xor_sync(0xffffffffu, lsum.x, o);
-    lsum.y += __shfl_xor_sync(0xffffffffu, lsum.y, o);
-    lsum.z += __shfl_xor_sync(0xffffffffu, lsum.z, o);
-    lsum.w += __shfl_xor_sync(0xffffffffu, lsum.w, o);
-  }
-  __syncthreads();                                // red_f is reused; w_s / sc_s are complete
-  if (lane == 0) red_f[warp] = lsum;
-  __syncthreads();
-  float4 l_star = red_f[0];
-#pragma unroll
-  for (int w = 1; w < 4; ++w) {
-    const float4 r = red_f[w];
-    l_star.x += r.x; l_star.y += r.y; l_star.z += r.z; l_star.w += r.w;
-  }
-  // ---- weighted sum: lane = d pair (dh*64 + 2*lane, +1) x 4 heads; warp w takes slots w, w+4, ... ----
-  const uint4* rows = reinterpret_cast<const uint4*>(p.part_o) + ((((size_t)m * 2 + hh) * 8 + g) * 2 + dh) * 32 + lane;
-  constexpr size_t kSlot16 = (size_t)kTcH * kTcD * 2 / 16;          // 16-byte units per slot
-  float a0[4] = {0.f, 0.f, 0.f, 0.f}, a1[4] = {0.f, 0.f, 0.f, 0.f};
-  const bool hi = lane >= 16;                                       // lane quarter of this d pair (scale block)
-  for (int c0 = warp; c0 < n_cta; c0 += 4 * kCombSmUnroll) {
-    uint4 v[kCombSmUnroll];
-#pragma unroll
-    for (int j = 0; j < kCombSmUnroll; ++j) {
-      const int c = c0 + 4 * j;
-      const float2 sc = c < n_cta ? sc_s[c] : make_float2(0.f, 0.f);
-      v[j] = (hi ? sc.y : sc.x) != 0.f ? __ldcg(rows + ((size_t)c + b) * kSlot16) : make_uint4(0u, 0u, 0u, 0u);
-    }
-#pragma unroll
-    for (int j = 0; j < kCombSmUnroll; ++j) {
-      const int c = c0 + 4 * j;
-      if (c < n_cta) {
-        const float2 sc2 = sc_s[c];
-        const float sc = hi ? sc2.y : sc2.x;
-        if (sc != 0.f) {
-          const float4 w = w_s[c];
-          const float2 x01 = unpack_f16x2(v[j].x), x23 = unpack_f16x2(v[j].y), y01 = unpack_f16x2(v[j].z), y23 = unpack_f16x2(v[j].w);
-          a0[0] = fmaf(w.x * sc, x01.x, a0[0]); a0[1] = fmaf(w.y * sc, x01.y, a0[1]);
-          a0[2] = fmaf(w.z * sc, x23.x, a0[2]); a0[3] = fmaf(w.w * sc, x23.y, a0[3]);
-          a1[0] = fmaf(w.x * sc, y01.x, a1[0]); a1[1] = fmaf(w.y * sc, y01.y, a1[1]);
-          a1[2] = fmaf(w.z * sc, y23.x, a1[2]); a1[3] = fmaf(w.w * sc, y23.y, a1[3]);
-        }
-      }
-    }
-  }
-  __syncthreads();                                // every warp is done with w_s
-  acc_s[warp][lane][0] = make_float4(a0[0], a0[1], a0[2], a0[3]);
-  acc_s[warp][lane][1] = make_float4(a1[0], a1[1], a1[2], a1[3]);
-  __syncthreads();
-  {                                               // thread = (head e, d pair): 4 heads x 32 pairs
-    const int e = tid >> 5;
-    float s0 = 0.f, s1 = 0.f;
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      s0 += reinterpret_cast<const float*>(&acc_s[w][lane][0])[e];
-      s1 += reinterpret_cast<const float*>(&acc_s[w][lane][1])[e];
-    }
-    const float ls = e == 0 ? l_star.x : e == 1 ? l_star.y : e == 2 ? l_star.z : l_star.w;
-    __nv_bfloat162 o2;
-    o2.x = __float2bfloat16_rn(ls > 0.f ? s0 / ls : 0.f);
-    o2.y = __float2bfloat16_rn(ls > 0.f ? s1 / ls : 0.f);
-    *reinterpret_cast<__nv_bfloat162*>(out + ((size_t)b * kTcH + h0 + e) * kTcD + m * 128 + dh * 64 + 2 * lane) = o2;
-  }
-  if (lse && m == 0 && dh == 0 && tid < 4) {
-    const float ls = tid == 0 ? l_star.x : tid == 1 ? l_star.y : tid == 2 ? l_star.z : l_star.w;
-    const float ms = tid == 0 ? m_star.x : tid == 1 ? m_star.y : tid == 2 ? m_star.z : m_star.w;
-    lse[(size_t)b * kTcH + h0 + tid] = ls > 0.f ? (ms + log2f(ls)) * 0.6931471805599453f : -INFINITY;
+  if (warp >= 2) {
+    if (n_cta <= 80) small_merge<2>(p, sm.q, cta, n_cta, tid - 64);
+    else small_merge<4>(p, sm.q, cta, n_cta, tid - 64);
   }
   __syncthreads();
   if (tid == 0) {
     __threadfence();
-    red_release_add_u32(p.comb_ctr, 1u);
+    red_release_add_u32(p.done_ctr, 1u);
   }
+  if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
 }
 
 }  // namespace lsa

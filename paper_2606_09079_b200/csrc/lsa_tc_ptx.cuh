@@ -75,6 +75,19 @@ __device__ __forceinline__ void tma_load_3d(void* smem_dst, const void* tmap, in
       ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
 }
 
+// The same with an L2 eviction-priority hint (createpolicy): K/V rows are read once per step and would otherwise push
+// everything small and hot - code, Q, split partials, page tables - out of L2.
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void tma_load_3d_hint(void* smem_dst, const void* tmap, int c0, int c1, int c2, uint64_t* bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
+      ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
+
 // ---- programmatic dependent launch (PDL) ----------------------------------------------------------------
 // wait: blocks until every grid this one depends on has completed and its writes are visible (no-op
 // when the launch carries no programmatic dependency).  launch_dependents: lets the next grid in the
