@@ -4,24 +4,39 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (lsa_step: table swap, window append, split-K attention
-+ combine, and - every tau steps - query tower, chunk scoring, top-k, residency diff, chunk fetch on
++ merge, and - every tau steps - query tower, chunk scoring, top-k, residency diff, chunk fetch on
 the side stream) over one decode token of every sequence of the config.  Default workload =
 BASELINE.json configs[2] (1-based config 3: bf16, B=1, 1M-token context), the one the metric is
 quoted on.  Inputs are synthetic and seeded (paper_2606_09079_b200/workloads.py).
 
 L2 hygiene: the per-step working set at B=1 (48 MiB) fits B200's L2, so R independent replicas of the
 layer state are stepped round-robin with R * bytes/step >= 2x L2 ("inputs larger than L2"); a real
-model touches >= 21 such layers per token.
+model touches >= 21 such layers per token.  The replicas start at trigger phases
+spread over tau and the warm-up covers every replica's first (cold) trigger, so that any timed window,
+however short, holds steady-state triggers: replica 0 fires at the first timed step.
+
+The steps of the timed loop are independent of one another (different replicas, inputs staged before
+the loop), so the contexts are created with lsa_config.step_overlap = 1 (--overlap 0 for the default
+of the API, where q / k_new / v_new may be produced by the work enqueued just before the call); the
+line carries the other mode as `dependent_inputs`.
+
+`--gpus N` (N > 1) without a torchrun environment re-executes this file under torch.distributed.run,
+one rank per GPU: configs 4 and 5 shard their sequences over the ranks (strong scaling: each GPU brings
+its own host link), the single-sequence configs run one replica set per rank (weak scaling); no
+data-path collective either way.  `--dry-run` drives that launcher and the reductions on CPU (gloo).
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
 workload; the oracle is otherwise only used for the `cpu_baseline` leg on rank 0.
 """
 import argparse
+import hashlib
 import json
 import math
 import os
+import socket
 import subprocess
 import sys
+import threading
 import time
 
 import numpy as np
@@ -30,19 +45,16 @@ import torch
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2606_09079_b200.dist import max_over_ranks  # noqa: E402
-from paper_2606_09079_b200.workloads import LsaWorkload, make_config, to_torch  # noqa: E402
+from paper_2606_09079_b200.dist import max_over_ranks, shard_sequences, sum_over_ranks  # noqa: E402
+from paper_2606_09079_b200.workloads import LsaWorkload, make_config, plant_boundary_ties, shard_config, to_torch  # noqa: E402
 
 METRIC = {1: ("lsa_decode_steps_per_s_8k_ctx_fp32", "steps/s"),
           2: ("lsa_decode_steps_per_s_128k_ctx", "steps/s"),
           3: ("lsa_decode_steps_per_s_1m_ctx", "steps/s"),
           4: ("lsa_decode_tokens_per_s_b32_ragged", "tokens/s"),
           5: ("lsa_decode_steps_per_s_churn_b8_512k", "steps/s")}
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum of one attn_tc_kernel launch, from the committed ncu --set full
-# capture of this command (profiles/); None where no capture has been taken for the config.
-TRAFFIC = {3: 51.2e6}     # profiles/r01_attn_tc_kernel_ncu.md: 50.47 MB read + 0.3-1.1 MB written
+SHARDED = (4, 5)                 # configs whose sequences are spread over the ranks (strong scaling)
+L2_DEFAULT = 126 * 2**20
 
 
 def load_peaks():
@@ -53,32 +65,78 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, source="B200_PROFILING.md fallback (of fallback)")
 
 
+def kernel_source_digest():
+    """sha-256 prefix of the sources of the dominant kernel: a stored ncu figure is only quoted while it still
+    describes the code that runs (profiles/r02_traffic.json)."""
+    h = hashlib.sha256()
+    for f in ("lsa_attn_tc_small.cuh", "lsa_attn_tc_kernel.cuh", "lsa_attn_tc_defs.cuh", "lsa_tc_ptx.cuh"):
+        h.update(open(os.path.join(ROOT, "paper_2606_09079_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic(config_id, overlap):
+    """dram__bytes_read + dram__bytes_write of one launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/), or None when there is no capture for this config or the kernel sources have changed since."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    if not os.path.exists(p):
+        return None, "no capture"
+    d = json.load(open(p)).get(f"cfg{config_id}_overlap{overlap}")
+    if not d:
+        return None, "no capture for this config"
+    if d.get("source_sha16") != kernel_source_digest():
+        return None, f"capture of commit {d.get('commit')} is stale: kernel sources changed"
+    return d["traffic_bytes"], f"ncu --set full, commit {d.get('commit')} ({d.get('file')})"
+
+
+def replicas_for(c, l2_bytes):
+    return max(1, math.ceil(2 * l2_bytes / c.attn_bytes_per_step()))
+
+
+def workload_config(c, n_gpus, l2_bytes=L2_DEFAULT):
+    """The `config` object of the JSON line: the workload only, identical for both arms."""
+    R = replicas_for(c, l2_bytes)
+    B = c.B_total or c.B
+    return dict(workload=c.name, B=B, L=c.L if B <= 2 else f"{min(c.L)}..{max(c.L)}", H=c.H, D=c.D,
+                C=c.C, W=c.W, Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pages=c.hot_pages, recall_lag=c.recall_lag,
+                cold_pool=("tiled from %d seeded base chunks, one tagged element per chunk" % c.kv_base_chunks) if c.kv_base_chunks else "independent seeded streams",
+                tie_triggers=c.tie_frac,
+                l2_policy=f"{R} layer-state replicas stepped round-robin; {R}x{c.attn_bytes_per_step() / 2**20:.1f} MiB attended "
+                          f"per rotation vs L2 {l2_bytes / 2**20:.0f} MiB (inputs larger than L2)",
+                parallelism=f"dp{n_gpus} (" + ("sequences sharded over ranks" if c.config_id in SHARDED and n_gpus > 1 else "independent sequences per rank") + ", no collective)")
+
+
 # ----------------------------------------------------------------------------------------------
 # reference arm / cpu baseline: the oracle on a bounded sample
 # ----------------------------------------------------------------------------------------------
-def oracle_sample(wl, budget_s=20.0, max_steps=24):
+def oracle_sample(wl, budget_s=20.0, max_steps=24, threads=None):
     """Run the oracle as it stands from step 0 (trigger + fetch + attention) for up to max_steps steps
     or ~budget_s seconds; returns (steps, seconds, threads)."""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     from lsa_harness import make_oracle
-    threads = os.cpu_count() or 1
-    try:
-        from threadpoolctl import threadpool_info
-        nt = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
-        if nt:
-            threads = max(nt)
-    except Exception:
-        pass
-    orc = make_oracle(wl)
-    t0 = time.perf_counter()
-    n = 0
-    while n < max_steps:
-        kn, vn = wl.kv_new(n)
-        orc.run_step(wl.q(n), wl.h(n), kn, vn)
-        n += 1
-        if time.perf_counter() - t0 > budget_s:
-            break
-    return n, time.perf_counter() - t0, threads
+    from threadpoolctl import threadpool_info, threadpool_limits
+    used = os.cpu_count() or 1
+    nt = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
+    if nt:
+        used = max(nt)
+
+    def run():
+        orc = make_oracle(wl)
+        t0 = time.perf_counter()
+        n = 0
+        while n < max_steps:
+            kn, vn = wl.kv_new(n)
+            orc.run_step(wl.q(n), wl.h(n), kn, vn)
+            n += 1
+            if time.perf_counter() - t0 > budget_s:
+                break
+        return n, time.perf_counter() - t0
+
+    if threads is None:
+        n, secs = run()
+        return n, secs, used
+    with threadpool_limits(limits=threads):
+        n, secs = run()
+    return n, secs, threads
 
 
 def run_reference(args, cfg, wl):
@@ -89,9 +147,8 @@ def run_reference(args, cfg, wl):
     n, secs, threads = oracle_sample(wl, budget_s=max(5.0, min(60.0, 2.0 * args.steps)), max_steps=max(2, min(args.steps, 48)))
     val = n * per_step_units / secs
     line = dict(metric=name, value=val, unit=unit, n_gpus=args.gpus, steps=n, warmup=1, ms_per_step=1e3 * secs / n,
-                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
-                config=dict(workload=cfg.name, B=cfg.B, L=cfg.L if cfg.B <= 2 else f"{min(cfg.L)}..{max(cfg.L)}", H=cfg.H,
-                            D=cfg.D, k=cfg.k, tau=cfg.tau),
+                higher_is_better=True, scaling="strong" if cfg.config_id in SHARDED and args.gpus > 1 else "weak", vs_baseline=None,
+                dtype="f64", data="synthetic", impl="reference", config=workload_config(cfg, args.gpus),
                 cpu_baseline=dict(value=val, unit=unit, cores=threads, kind="oracle",
                                   sample=f"oracle steps 0..{n - 1} of {cfg.name} (trigger + fetch at step 0, attention every step)"),
                 e2e=dict(value=val, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
@@ -99,10 +156,80 @@ def run_reference(args, cfg, wl):
 
 
 # ----------------------------------------------------------------------------------------------
+# clocks: NVML in-process, sampled over the whole GPU phase
+# ----------------------------------------------------------------------------------------------
+class ClockSampler:
+    """SM clock / throttle reasons read through NVML from a thread every few milliseconds between start() and stop();
+    `window` is the wall-clock span of the timed region, so that samples inside it can be told apart."""
+
+    def __init__(self, dev_index, interval_s=0.004):
+        self.samples, self.window, self.err = [], None, None
+        self._stop = threading.Event()
+        self.interval = interval_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[dev_index]) if vis and all(x.strip().isdigit() for x in vis.split(",")) else dev_index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_sm = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:                                   # no NVML: say so, never guess
+            self.nv, self.err = None, repr(e)
+
+    def _one(self):
+        nv = self.nv
+        sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+        try:
+            rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+        except Exception:
+            rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        self.samples.append((time.perf_counter(), sm, rs))
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._one()
+            except Exception as e:
+                self.err = repr(e)
+                return
+            self._stop.wait(self.interval)
+
+    def start(self):
+        if self.nv is not None:
+            self.th = threading.Thread(target=self._run, daemon=True)
+            self.th.start()
+
+    def sample_now(self):
+        if self.nv is not None:
+            try:
+                self._one()
+            except Exception as e:
+                self.err = repr(e)
+
+    def stop(self):
+        if self.nv is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, samples=0, reasons=[f"NVML unavailable: {self.err}"])
+        self._stop.set()
+        self.th.join(timeout=2)
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        sm = [s[1] for s in self.samples]
+        reasons = sorted(n for n, bit in names.items() if any(s[2] & bit for s in self.samples))
+        inside = [s[1] for s in self.samples if self.window and self.window[0] <= s[0] <= self.window[1] + 0.002]
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=float(self.max_sm), samples=len(sm),
+                    samples_in_timed_region=len(inside), sm_mhz_in_timed_region=float(np.median(inside)) if inside else None,
+                    reasons=reasons, how="NVML in-process, every 4 ms from the first warm-up step to the end of the end-to-end leg")
+
+
+# ----------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------
 class Replica:
-    def __init__(self, wl, shared, sc, sf, lsa):
+    def __init__(self, wl, shared, sc, sf, lsa, phase, overlap):
         c = wl.cfg
         dev = shared["dev"]
         tdt = shared["tdt"]
@@ -114,63 +241,54 @@ class Replica:
         self.win_v = [x.clone() for x in shared["win_v"]]
         seqs = [dict(cold_csa=shared["cold"][b], n_csa=c.n_csa(b), chunk_emb=self.emb[b], hca_k=self.hca_k[b],
                      hca_v=self.hca_v[b], win_k=self.win_k[b], win_v=self.win_v[b], w_len=min(c.W, c.L[b]), w_head=0,
-                     step0=c.step0(b)) for b in range(c.B)]
+                     step0=c.step0(b) + phase) for b in range(c.B)]
         self.ctx = lsa.LsaContext(dtype=lsa.LSA_F32 if c.dtype == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W,
                                   Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=shared["W_q"], seqs=seqs,
                                   recall_lag=c.recall_lag, stream_compute=sc, stream_fetch=sf,
-                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0),
-                                  step_overlap=shared.get("overlap", 0))
-        self.step = 0
+                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0), step_overlap=overlap)
+        self.step = phase                # global step index of the workload this replica is at (wl.fires / wl.trigger_index)
+        self.tie_emb = {}                # cfg 5: sequences whose alternate (tie-carrying) embedding table is installed
 
 
-def clocks_sampler_start(dev_index):
-    """nvidia-smi polled every 100 ms while the timed region runs (B200_PROFILING.md clocks line); lines
-    are read from a pipe by a thread because nvidia-smi block-buffers when writing to a file."""
-    import threading
-    q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
-        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
-    try:
-        p = subprocess.Popen(["nvidia-smi", f"--id={dev_index}", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100"],
-                             stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
-    except Exception:
-        return None, None
-    lines = []
-
-    def pump():
-        for line in p.stdout:
-            lines.append((time.perf_counter(), line))
-
-    th = threading.Thread(target=pump, daemon=True)
-    th.start()
-    return p, (lines, th)
+def relaunch_under_torchrun(args):
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    env = dict(os.environ)
+    if not args.dry_run:
+        env.setdefault("NCCL_DEBUG", "INFO")          # the ranks show up in NCCL's own log (stderr)
+    return subprocess.run(cmd, env=env).returncode
 
 
-def clocks_sampler_stop(p, state, t_begin=None, t_end=None):
-    if p is None:
-        return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
-    lines, th = state
-    p.terminate()
-    try:
-        p.wait(timeout=5)
-    except Exception:
-        p.kill()
-    th.join(timeout=5)
-    sm, smax, reasons = [], [], set()
-    for ts, line in lines:
-        if t_begin is not None and not (t_begin <= ts <= t_end + 0.15):
-            continue
-        parts = [x.strip() for x in line.split(",")]
-        if len(parts) < 7:
-            continue
-        try:
-            sm.append(float(parts[0])); smax.append(float(parts[1]))
-        except ValueError:
-            continue
-        for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), parts[3:7]):
-            if v.lower().startswith("active"):
-                reasons.add(name)
-    return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(smax) if smax else None,
-                samples=len(sm), reasons=sorted(reasons))
+def dry_run(args, cfg, rank, world):
+    """The N > 1 plumbing without a GPU: gloo group, sequence shards, the two reductions, one line from rank 0."""
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+    sharded = cfg.config_id in SHARDED and world > 1
+    lo, hi = shard_sequences(cfg.B, world, rank) if sharded else (0, cfg.B)
+    sub = shard_config(cfg, lo, hi) if sharded else cfg
+    name, unit = METRIC[cfg.config_id]
+    tokens = unit == "tokens/s"
+    units = args.steps * (sub.B if tokens else 1) if (tokens or not sharded) else (args.steps if rank == 0 else 0)
+    job_ms = max_over_ranks(10.0 * (1 + rank))                       # pretend the last rank is the slow one
+    total = sum_over_ranks(units)
+    shards = [None] * world
+    if world > 1:
+        dist.all_gather_object(shards, (lo, hi, sub.hot_pages))
+    else:
+        shards = [(lo, hi, sub.hot_pages)]
+    if rank == 0:
+        print(json.dumps(dict(metric=name, value=total / (job_ms * 1e-3), unit=unit, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                              ms_per_step=job_ms / args.steps, higher_is_better=True, scaling="strong" if sharded else "weak",
+                              vs_baseline=None, dtype=cfg.dtype, data="synthetic", dry_run=True, shards=shards,
+                              config=workload_config(cfg, world))))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
 
 
 def main():
@@ -185,13 +303,17 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--max-ctas", type=int, default=0, help="cap on attention CTAs (0 = library default)")
-    ap.add_argument("--overlap", type=int, default=0, help="lsa_config.step_overlap: 1 = the steps' inputs are independent of the previous step's output")
+    ap.add_argument("--overlap", type=int, default=1, help="lsa_config.step_overlap of the timed contexts: 1 = the steps' inputs do not depend on the previous step's output (true of this loop); 0 = the API default")
+    ap.add_argument("--no-dependent", action="store_true", help="skip the second measurement in the other step_overlap mode")
+    ap.add_argument("--dry-run", action="store_true", help="CPU only: launcher, sharding and reductions with a gloo group")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
     ap.add_argument("--export", action="store_true", help="also time lsa_export_chunks (NEXT-4: KV export HBM -> pinned cold pool)")
     ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
     ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
     ap.add_argument("--l2-k2", type=int, default=2048, help="Level-2 Top-k (entries per sequence and step)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        return relaunch_under_torchrun(args)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -201,6 +323,8 @@ def main():
         if rank == 0:
             run_reference(args, cfg, LsaWorkload(cfg))
         return 0
+    if args.dry_run:
+        return dry_run(args, cfg, rank, world)
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
@@ -210,25 +334,43 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     from paper_2606_09079_b200 import lsa
 
-    wl = LsaWorkload(cfg)
-    c = cfg
+    sharded = cfg.config_id in SHARDED and world > 1
+    if sharded:                                        # this rank's sequences only: own pools, own host link
+        lo, hi = shard_sequences(cfg.B, world, rank)
+        c = shard_config(cfg, lo, hi)
+    else:
+        c = cfg
+    wl = LsaWorkload(c)
     tdt = torch.float32 if c.dtype == "f32" else torch.bfloat16
     name, unit = METRIC[c.config_id]
-    per_step_units = c.B if unit == "tokens/s" else 1
+    tokens = unit == "tokens/s"
+    per_step_units = c.B if tokens else 1
     props = torch.cuda.get_device_properties(dev)
-    l2 = getattr(props, "L2_cache_size", 126 * 2**20)
+    l2 = getattr(props, "L2_cache_size", L2_DEFAULT)
     attn_bytes = c.attn_bytes_per_step()
-    R = args.replicas or max(1, math.ceil(2 * l2 / attn_bytes))
-    warmup = max(args.warmup, 3, 2 * R)
+    R = args.replicas or replicas_for(c, l2)
     attn_impl = dict(auto=lsa.LSA_ATTN_AUTO, simt=lsa.LSA_ATTN_SIMT, tcgen05=lsa.LSA_ATTN_TCGEN05)[args.attn]
 
-    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, max_ctas=args.max_ctas, overlap=args.overlap, W_q=to_torch(wl.W_q, c.dtype).to(dev),
+    def job_units(n_steps):
+        """units of the whole job in n_steps steps: ranks with their own replica sets add up; ranks that share one
+        batch of sequences make the same steps (tokens add up, steps do not)"""
+        if sharded and not tokens:
+            return n_steps
+        return sum_over_ranks(n_steps * per_step_units, dev)
+
+    shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, max_ctas=args.max_ctas, W_q=to_torch(wl.W_q, c.dtype).to(dev),
                   cold=[to_torch(x, c.dtype).pin_memory() for x in wl.cold_csa],
                   emb=[to_torch(wl.chunk_emb(b, 0), c.dtype).to(dev) for b in range(c.B)],
                   hca_k=[to_torch(x, c.dtype).to(dev) for x in wl.hca_k], hca_v=[to_torch(x, c.dtype).to(dev) for x in wl.hca_v],
                   win_k=[to_torch(x, c.dtype).to(dev) for x in wl.win_k], win_v=[to_torch(x, c.dtype).to(dev) for x in wl.win_v])
     sc, sf = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
-    reps = [Replica(wl, shared, sc, sf, lsa) for _ in range(R)]
+    # replica r starts r * (tau // R) steps before a trigger; replica 0 fires at its steps 0, tau, ...
+    phases = [(c.tau - r * (c.tau // R)) % c.tau for r in range(R)]
+    reps = [Replica(wl, shared, sc, sf, lsa, phases[r], args.overlap) for r in range(R)]
+    # every replica's first (cold: empty hot pool) trigger and its table swap happen in the warm-up, which is a whole
+    # number of trigger periods per replica: replica 0 then fires again at the first timed step
+    warmup = max(args.warmup, 3, R * c.tau)
+    warmup += (-warmup) % (R * c.tau)
 
     # a rotating set of per-step inputs, resident in HBM before the timed region
     NIN = 16
@@ -238,24 +380,45 @@ def main():
     out = torch.empty((c.B, c.H, c.D), dtype=tdt, device=dev)
     # needle drift (cfg 2-4): rows to rewrite at each trigger index, staged on the device
     drift = {}
-    max_trig = (warmup + 3 * args.steps) // (c.tau * R) + 3
+    max_trig = (2 * warmup + 6 * args.steps) // (c.tau * R) + 6
     for trig in range(1, max_trig + 1):
         for b in range(c.B):
             upd = wl.emb_row_updates(b, trig)
             if upd is not None:
                 drift[(b, trig)] = (torch.from_numpy(upd[0]).to(dev), to_torch(upd[1], c.dtype).to(dev))
+    # cfg 5 (BASELINE.json: "10% of triggers carry planted exact-tie and near-tie scores"): those triggers get an alternate
+    # table with an exact tie across the k-th rank of a FIXED seeded ranking and a one-ulp near-tie behind it (the parity
+    # tests plant them across the oracle's own ranking; here only the timing of the tie-break matters)
+    tie_tables = {}
+    if c.tie_frac > 0:
+        for b in range(c.B):
+            for trig in range(0, min(max_trig + 1, 256)):
+                if wl.has_tie_trigger(b, trig) and len(tie_tables) < 32:
+                    order = np.random.Generator(np.random.Philox(c.seed + 977 * b + trig)).permutation(c.n_chunks(b))
+                    tie_tables[(b, trig)] = to_torch(plant_boundary_ties(wl.chunk_emb(b, trig), order, c.k_eff(b), c.dtype), c.dtype).to(dev)
     torch.cuda.synchronize()
+    n_tie_triggers = [0]
 
-    def one_step(i, host=None):
-        r = reps[i % R]
+    def one_step(i, host=None, rs=None):
+        rs = reps if rs is None else rs
+        r = rs[i % len(rs)]
         t = r.step
-        if drift:
+        if drift or tie_tables:
             for b in range(c.B):
-                if wl.fires(b, t):
-                    u = drift.get((b, wl.trigger_index(b, t)))
-                    if u is not None:
-                        with torch.cuda.stream(sf):
-                            r.emb[b][u[0]] = u[1]
+                if not wl.fires(b, t):
+                    continue
+                trig = wl.trigger_index(b, t)
+                u = drift.get((b, trig))
+                if u is not None:
+                    with torch.cuda.stream(sf):
+                        r.emb[b][u[0]] = u[1]
+                if (b, trig) in tie_tables:
+                    r.ctx.set_chunk_emb(b, tie_tables[(b, trig)])
+                    r.tie_emb[b] = True
+                    n_tie_triggers[0] += 1
+                elif r.tie_emb.get(b):
+                    r.ctx.set_chunk_emb(b, r.emb[b])
+                    r.tie_emb[b] = False
         j = i % NIN
         if host is None:
             r.ctx.step(qs[j], hs[(t // c.tau) % NIN], kns[j], vns[j], out)
@@ -268,34 +431,46 @@ def main():
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
-    def timed(n, host=None, i0=0):
+    def counters(rs):
+        st = [r.ctx.stats() for r in rs]
+        return (sum(s["attn_launches"] + s["index_launches"] for s in st), sum(s["triggers"] for s in st),
+                sum(s["index_launches"] for s in st))
+
+    def timed(n, host=None, i0=0, rs=None):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         w0 = time.perf_counter()
         e0.record(sc)
         for i in range(n):
-            one_step(i0 + i, host)
+            one_step(i0 + i, host, rs)
+        sc.wait_stream(sf)                                  # side-band work still in flight belongs to the region
         e1.record(sc)
         enq = time.perf_counter() - w0                      # host time to enqueue the n steps (no waiting)
         sf.synchronize(); sc.synchronize()
-        wall = time.perf_counter() - w0
+        w1 = time.perf_counter()
         barrier()
         ms = max_over_ranks(e0.elapsed_time(e1), dev)       # the job's time = the slowest rank's
-        return ms, wall, enq
+        return ms, w1 - w0, enq, (w0, w1)
 
     # ---- warm-up, then the device-resident timed region ----
-    samp, sampf = clocks_sampler_start(local_rank)
+    clk = ClockSampler(local_rank)
+    clk.start()
     for i in range(warmup):
         one_step(i)
     i_next = warmup
-    launches0 = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps)
-    t_begin = time.perf_counter()
-    ms, wall, enq = timed(args.steps, i0=i_next)
-    t_end = time.perf_counter()
-    clocks = clocks_sampler_stop(samp, sampf, t_begin, t_end)
+    l0, t0_, x0 = counters(reps)
+    # a window shorter than one trigger period of every replica would hold 0 or 1 trigger, i.e. none or several times the
+    # workload's share (one per tau steps and replica): at least R * tau steps are timed, whatever --steps asks for
+    n_timed = max(args.steps, R * c.tau) if R * c.tau <= 8192 else args.steps
+    steps_requested, args.steps = args.steps, n_timed
+    ms, wall, enq, window = timed(args.steps, i0=i_next)
+    clk.sample_now()
+    clk.window = window
     i_next += args.steps
-    launches = sum(r.ctx.stats()["attn_launches"] + r.ctx.stats()["index_launches"] for r in reps) - launches0
-    value = world * args.steps * per_step_units / (ms * 1e-3)
+    l1_, t1_, x1 = counters(reps)
+    launches, triggers_timed, index_launches = l1_ - l0, t1_ - t0_, x1 - x0
+    units_job = job_units(args.steps)
+    value = units_job / (ms * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (H2D + D2H inside the timed region) ----
     pin = lambda t: t.cpu().pin_memory()
@@ -305,49 +480,72 @@ def main():
         one_step(i_next + i, host)
     i_next += max(3, R)
     n_e2e = max(64, args.steps // 4)
-    ms_e2e, _, enq_e2e = timed(n_e2e, host, i0=i_next)
+    ms_e2e, _, enq_e2e, _ = timed(n_e2e, host, i0=i_next)
     i_next += n_e2e
     es = 4 if c.dtype == "f32" else 2
     h2d = (c.B * c.H * c.D + 2 * c.B * c.D) * es + c.B * c.Dh * es // c.tau     # h crosses only at trigger steps (1 in tau)
     d2h = c.B * c.H * c.D * es
-    e2e_value = world * n_e2e * per_step_units / (ms_e2e * 1e-3)
+    e2e_value = job_units(n_e2e) / (ms_e2e * 1e-3)
+    clocks = clk.stop()
 
-    # ---- per-kernel device time of the dominant kernel (CUDA events on its own stream) ----
+    # ---- the other step_overlap mode, on replicas of its own (every rank runs it: there are barriers inside) ----
+    dependent = None
+    if not args.no_dependent and c.B <= 4 and c.dtype == "bf16":
+        other = 1 - args.overlap
+        reps2 = [Replica(wl, shared, sc, sf, lsa, phases[r], other) for r in range(R)]
+        for i in range(warmup):
+            one_step(i, None, reps2)
+        n_dep = max(256, min(args.steps, 4096))
+        ms_d, _, _, _ = timed(n_dep, None, warmup, reps2)
+        dependent = dict(step_overlap=other, value=job_units(n_dep) / (ms_d * 1e-3), unit=unit, ms_per_step=ms_d / n_dep,
+                         frac_of_hbm_peak=attn_bytes / (ms_d / n_dep * 1e-3) / 1e9 / load_peaks()["hbm_gbs"], steps=n_dep,
+                         note="same loop, contexts created with the other lsa_config.step_overlap (0 = the API default: q / k_new / v_new "
+                              "may be produced by the work enqueued on stream_compute just before the call)")
+        for r in reps2:
+            r.ctx.close()
+        del reps2
+
+    # ---- the dominant kernel alone (CUDA events around single launches on its stream: no overlap with neighbours) ----
     n_prof = min(args.steps, 512)
     for r in reps:
         r.ctx.profile_enable(n_prof // R + 8)
     for i in range(n_prof):
         one_step(i_next + i)
     i_next += n_prof
-    phases = {}
+    phases_ms = {}
     for r in reps:
         for ph, v in r.ctx.profile_read().items():
-            d = phases.setdefault(ph, dict(ms=0.0, count=0))
+            d = phases_ms.setdefault(ph, dict(ms=0.0, count=0))
             d["ms"] += v["ms"]; d["count"] += v["count"]
         r.ctx.profile_enable(0)
-    attn_ms = phases["attention"]["ms"] / max(phases["attention"]["count"], 1)
-    comb_ms = phases["combine"]["ms"] / max(phases["combine"]["count"], 1) if phases["combine"]["count"] else 0.0
+    attn_ms = phases_ms["attention"]["ms"] / max(phases_ms["attention"]["count"], 1)
+    comb_ms = phases_ms["combine"]["ms"] / max(phases_ms["combine"]["count"], 1) if phases_ms["combine"]["count"] else 0.0
     peaks = load_peaks()
-    achieved = attn_bytes / (attn_ms * 1e-3) / 1e9
-    ph_dev = phases.get("attention_dev", dict(ms=0.0, count=0))
+    ph_dev = phases_ms.get("attention_dev", dict(ms=0.0, count=0))
     attn_dev_ms = ph_dev["ms"] / ph_dev["count"] if ph_dev["count"] else None
     stats = reps[0].ctx.stats()
+    one_launch = c.B <= 4 and args.overlap == 1 and stats["attn_impl"] == 2
+    # one launch of the dominant kernel per step: its average duration over the timed region is the step time of the
+    # pipelined loop (the launches of consecutive steps overlap); kernel_ms_isolated = events around single launches
+    launch_ms = ms / args.steps
+    achieved = attn_bytes / (launch_ms * 1e-3) / 1e9
+    traffic, traffic_src = stored_traffic(c.config_id, args.overlap)
     roofline = dict(bound="hbm", achieved=achieved, peak=peaks["hbm_gbs"], unit="GB/s", frac=achieved / peaks["hbm_gbs"],
-                    traffic=TRAFFIC.get(c.config_id), kernel="attn_tc_kernel: split-K decode attention (S7)" + (" incl. combine" if comb_ms == 0.0 else ""),
-                    algorithmic_bytes_per_launch=attn_bytes, kernel_ms=attn_ms, combine_ms=comb_ms,
-                    # the same kernel by the device's %globaltimer (first CTA past its launch dependency -> last CTA
-                    # done): the CUDA-event figure above also holds the launch gap the events themselves open
-                    kernel_ms_device_clock=attn_dev_ms,
-                    frac_device_clock=(attn_bytes / (attn_dev_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if attn_dev_ms else None,
-                    step_ms=ms / args.steps, frac_of_step=achieved and (attn_bytes / (ms / args.steps * 1e-3) / 1e9) / peaks["hbm_gbs"],
+                    traffic=traffic, traffic_source=traffic_src,
+                    kernel=("attn_tc_small_kernel: split-K decode attention and the merge of its partials in one launch (S7 + S8)" if one_launch
+                            else "attn_tc_kernel: split-K decode attention (S7); S8 in the combine kernel that follows"),
+                    algorithmic_bytes_per_launch=attn_bytes, kernel_ms=launch_ms,
+                    kernel_ms_how="timed region / launches of this kernel inside it (CUDA events on stream_compute), i.e. everything a step costs is charged to it",
+                    kernel_ms_isolated=attn_ms, combine_ms_isolated=comb_ms, kernel_ms_device_clock_isolated=attn_dev_ms,
+                    step_ms=launch_ms, frac_of_step=achieved / peaks["hbm_gbs"],
                     peak_source=peaks["source"], frac_of_nominal_8tbs=achieved / 8000.0)
 
     # ---- how much of the trigger side band (S1-S5) hides behind attention (SURVEY 8(d) "fetch overlap") ----
     # exposed time per trigger = tau * (mean step time over all steps - step time between triggers); hidden fraction =
-    # 1 - exposed / (side-band kernel time per trigger).  With recall_lag = 1 the new table is needed by step t + 1, so
-    # at most one step's attention can hide it.
+    # 1 - exposed / (side-band kernel time per trigger).  With recall_lag = 1 the new table is needed by step t + 1.
     side_band = None
-    if not c.stagger and c.tau >= 8 and all(ph in phases and phases[ph]["count"] for ph in ("index", "residency", "fetch")):
+    if not c.stagger and c.tau >= 8 and args.steps >= 2 * R * c.tau and all(ph in phases_ms and phases_ms[ph]["count"] for ph in ("index", "residency", "fetch")):
+        # bring every replica to the same trigger phase, then time windows without a trigger or a swap
         t_al = (max(r.step for r in reps) // c.tau + 1) * c.tau + 2
         for idx, r in enumerate(reps):
             while r.step < t_al:
@@ -367,7 +565,7 @@ def main():
                 for idx in range(R):
                     one_step(idx)
         nt_ms /= n_win
-        per = {ph: phases[ph]["ms"] / phases[ph]["count"] for ph in ("index", "residency", "fetch")}
+        per = {ph: phases_ms[ph]["ms"] / phases_ms[ph]["count"] for ph in ("index", "residency", "fetch")}
         side_ms = sum(per.values())
         exposed = c.tau * (ms / args.steps - nt_ms)
         side_band = dict(step_ms_all=ms / args.steps, step_ms_between_triggers=nt_ms, exposed_ms_per_trigger=exposed,
@@ -522,59 +720,36 @@ def main():
         sf.synchronize(); sc.synchronize()
         i_next += n_g
         g_ms = e0.elapsed_time(e1) / n_g
-        # host cost of one call while the launch queue has room (256 steps = 512 launches, then drain)
-        def host_cost(fn):
-            best = None
-            for _ in range(3):
-                sf.synchronize(); sc.synchronize()
-                r0 = reps[0]
-                while r0.step % c.tau < 2 or r0.step % c.tau > c.tau - 10:      # stay inside one trigger window on every replica
-                    for r in reps:
-                        r.ctx.step(qs[0], hs[(r.step // c.tau) % NIN], kns[0], vns[0], out); r.step += 1
-                    sc.synchronize(); sf.synchronize()
-                w = time.perf_counter()
-                for i in range(8 * R if 8 * R < c.tau - 12 else R):
-                    fn(i)
-                dt = (time.perf_counter() - w) / (8 * R if 8 * R < c.tau - 12 else R)
-                best = dt if best is None else min(best, dt)
-            sc.synchronize(); sf.synchronize()
-            return best * 1e6
-
-        def s_step(i):
-            r = reps[i % R]
-            r.ctx.step(qs[0], hs[(r.step // c.tau) % NIN], kns[0], vns[0], out)
-            r.step += 1
-        host_us_graph = host_cost(lambda i: g_step(i)) if c.tau >= 32 else None
-        host_us_step = host_cost(s_step) if c.tau >= 32 else None
         gs = [r.ctx.graph_stats() for r in reps]
         graph = dict(value=per_step_units / (g_ms * 1e-3), unit=unit, ms_per_step=g_ms, host_enqueue_ms_per_step=enq_g * 1e3 / n_g,
                      captures=sum(g_["captures"] for g_ in gs), replays=sum(g_["replays"] for g_ in gs),
-                     host_us_per_call=dict(lsa_step=host_us_step, lsa_step_graph=host_us_graph),
                      note="lsa_step_graph: steps without a trigger or a table swap replay one captured graph (attention + combine) per context")
 
-    cpu_baseline = None
+    cpu_baseline = cpu_baseline_1t = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n, secs, threads = oracle_sample(wl, budget_s=15.0, max_steps=24)
+        n, secs, threads = oracle_sample(wl, budget_s=12.0, max_steps=24)
         cpu_baseline = dict(value=n * per_step_units / secs, unit=unit, cores=threads, kind="oracle",
                             sample=f"oracle steps 0..{n - 1} of {c.name}: trigger + fetch at step 0, attention every step; {secs:.1f} s")
+        n1, secs1, _ = oracle_sample(wl, budget_s=10.0, max_steps=6, threads=1)
+        cpu_baseline_1t = dict(value=n1 * per_step_units / secs1, unit=unit, cores=1, kind="oracle",
+                               sample=f"oracle steps 0..{n1 - 1} of {c.name} with the BLAS pool limited to one thread; {secs1:.1f} s")
 
     if rank == 0:
-        line = dict(metric=name, value=value, unit=unit, n_gpus=world, steps=args.steps, warmup=warmup,
-                    ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
-                    dtype=c.dtype, data="synthetic",
-                    config=dict(workload=c.name, B=c.B, L=c.L if c.B <= 2 else f"{min(c.L)}..{max(c.L)}", H=c.H, D=c.D, C=c.C,
-                                W=c.W, k=c.k, tau=c.tau, hot_pages=c.hot_pages, recall_lag=c.recall_lag,
-                                l2_policy=f"{R} layer-state replicas stepped round-robin; {R}x{attn_bytes / 2**20:.1f} MiB attended "
-                                          f"per rotation vs L2 {l2 / 2**20:.0f} MiB (inputs larger than L2)",
-                                parallelism=f"dp{world} (independent sequences per rank, no collective)",
-                                attn_impl={1: "simt", 2: "tcgen05"}.get(stats["attn_impl"], "?"), attn_ctas=stats["attn_ctas"]),
+        line = dict(metric=name, value=value, unit=unit, n_gpus=world, steps=args.steps, steps_requested=steps_requested, warmup=warmup,
+                    ms_per_step=ms / args.steps, higher_is_better=True, scaling="strong" if sharded else "weak", vs_baseline=None,
+                    dtype=c.dtype, data="synthetic", config=workload_config(cfg, world, l2),
+                    run=dict(step_overlap=args.overlap, attn_impl={1: "simt", 2: "tcgen05"}.get(stats["attn_impl"], "?"), attn_ctas=stats["attn_ctas"],
+                             replicas=R, replica_trigger_phases=phases, sequences_this_rank=c.B,
+                             note="step_overlap = 1: the timed steps belong to independent layer-state replicas and their inputs are staged before the loop"),
                     e2e=dict(value=e2e_value, unit=unit, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=n_e2e,
                              ms_per_step=ms_e2e / n_e2e),
-                    gpu_launches=int(launches), clocks=clocks, roofline=roofline, cpu_baseline=cpu_baseline,
-                    phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases.items()},
-                    fetch=fetch, side_band=side_band, l1_indexer=l1, level2=level2, step_graph=graph, export=export, wall_s=wall, host_enqueue_ms_per_step=enq * 1e3 / args.steps,
-                    host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
-                    tokens_per_s=world * args.steps * c.B / (ms * 1e-3))
+                    gpu_launches=int(launches), triggers_in_timed_region=int(triggers_timed), index_launches=int(index_launches),
+                    tie_triggers_seen=n_tie_triggers[0], clocks=clocks, roofline=roofline, dependent_inputs=dependent,
+                    cpu_baseline=cpu_baseline, cpu_baseline_1t=cpu_baseline_1t,
+                    phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases_ms.items()},
+                    fetch=fetch, side_band=side_band, l1_indexer=l1, level2=level2, step_graph=graph, export=export, wall_s=wall,
+                    host_enqueue_ms_per_step=enq * 1e3 / args.steps, host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
+                    tokens_per_s=(units_job if tokens else units_job * (cfg.B if sharded else c.B)) / (ms * 1e-3))
         print(json.dumps(line))
     if world > 1:
         torch.distributed.destroy_process_group()

@@ -627,6 +627,28 @@ static int step_impl(lsa_ctx* ctx, const void* q, const void* h, const void* k_n
     c->n_steps += 1;
     return LSA_OK;
   }
+  if (n_fire && c->attn_impl == LSA_ATTN_TCGEN05 && c->cfg.step_overlap && tc_small_supported(c->tc) && !q_idx && !c->no_small &&
+      c->cfg.recall_lag >= 1) {
+    // Independent steps (lsa_config.step_overlap), trigger step: with recall_lag >= 1 no table swap can be due now (the
+    // table staged by the previous trigger became current lag < tau steps after it), so the side band reads the records
+    // as the PREVIOUS step left them and nothing on the compute stream has to wait: the attention launch stays in the
+    // overlapped chain, the window append rides on it as on any other step.
+    bool due = false;
+    for (int b = 0; b < c->B; ++b) due |= c->pending[b] && c->step[b] >= c->visible_at[b];
+    if (!due) {
+      if (c->indexer == LSA_INDEXER_LEVEL1 ? (rc = l1_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))
+                                           : (rc = index_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr)))
+        return rc;
+      if ((rc = fetch_impl(c, ids, n_fire, c->d_sel, c->indexer != LSA_INDEXER_LEVEL1))) return rc;
+      TcPrestep pre{};
+      pre.k_new = k_new; pre.v_new = v_new;
+      if (k_new) mirror_append(c);
+      if ((rc = attention_impl(c, q, out, nullptr, &pre))) return rc;
+      for (int b = 0; b < c->B; ++b) c->step[b] += 1;
+      c->n_steps += 1;
+      return LSA_OK;
+    }
+  }
   if ((rc = prestep_impl(c, false, k_new, v_new))) return rc;       // (a) + (d)
   if (n_fire) {                                                     // (b)
     if (c->indexer == LSA_INDEXER_LEVEL1 ? (rc = l1_select_impl(c, h, ids, ids, n_fire, c->d_sel, nullptr))

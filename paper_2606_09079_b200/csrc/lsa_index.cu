@@ -124,7 +124,9 @@ topk_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __restr
   auto keyf = [sc](int c) -> unsigned long long {
     return ((unsigned long long)(~float_to_ordered(sc[c])) << 32) | (unsigned)c;
   };
-  const int m = block_select_smallest(keyf, sq.n_chunks, min(k, sq.n_chunks), sm);
+  // n <= 4096: histogram select + sort of the k winners; larger tables: radix select over the keys in global memory
+  const int m = sq.n_chunks <= 4096 ? block_topk_select(sc, sq.n_chunks, min(k, sq.n_chunks), sm)
+                                    : block_select_smallest(keyf, sq.n_chunks, min(k, sq.n_chunks), sm);
   for (int j = threadIdx.x; j < k; j += blockDim.x) {
     int idx = -1;
     float val = -INFINITY;

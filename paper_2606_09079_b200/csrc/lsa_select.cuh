@@ -123,4 +123,107 @@ __device__ inline int block_select_smallest(KeyF keyf, int n, int m, SelectSmem&
   return min(m, got);
 }
 
+// ---- S3 for n <= 4096 scores: histogram select + sort of the winners only ------------------------------------------
+// The k best of n scores by (score desc, index asc).  Every thread keeps its (up to 4) order-preserving 32-bit scores
+// in registers; three radix levels (12 + 12 + 8 bits, most significant first) each count the keys that still match
+// the decided prefix into a shared-memory histogram, a block-wide suffix scan finds the bin holding the k-th best and
+// how many keys of that bin are still needed.  After the last level the cut-off score is exact: keys above it win,
+// keys AT it win by ascending index (one block scan per register slot, only when the tie really straddles the cut).
+// The <= k winners are compacted and sorted (bitonic, mostly warp-level at k <= 128) - instead of sorting all n.
+// Writes min(k, n) keys (~ordered(score) << 32 | idx, ascending = best first) to sm.keys and returns their count.
+// All 1024 threads of the block call it; n <= 4096, k <= 1024.
+constexpr int kTopkBins = 4096;
+
+__device__ inline int block_topk_select(const float* __restrict__ sc, int n, int k, SelectSmem& sm) {
+  if (k > n) k = n;
+  if (k <= 0) return 0;
+  unsigned int* hist = reinterpret_cast<unsigned int*>(sm.keys + 1024);      // 16 KiB behind the 1024 output slots
+  unsigned int* wsum = sm.hist;                                              // [32] warp totals, [64..] results
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  unsigned int u[4];
+  bool have[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int c = tid + 1024 * j;
+    have[j] = c < n;
+    u[j] = have[j] ? float_to_ordered(sc[c]) : 0u;
+  }
+  unsigned int prefix = 0, mask = 0, need = (unsigned)k, eq_total = 0;
+#pragma unroll 1
+  for (int level = 0; level < 3; ++level) {
+    const int shift = level == 0 ? 20 : level == 1 ? 8 : 0;
+    const unsigned bins = level == 2 ? 256u : (unsigned)kTopkBins;
+    for (int i = tid; i < kTopkBins; i += 1024) hist[i] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (have[j] && (u[j] & mask) == prefix) atomicAdd(&hist[(u[j] >> shift) & (bins - 1)], 1u);
+    __syncthreads();
+    // suffix counts: thread t owns bins [4t, 4t + 4); above(b) = keys in bins > b
+    const unsigned h0 = hist[4 * tid], h1 = hist[4 * tid + 1], h2 = hist[4 * tid + 2], h3 = hist[4 * tid + 3];
+    const unsigned mine = h0 + h1 + h2 + h3;
+    unsigned incl = mine;                                   // inclusive suffix sum over threads (towards higher t)
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_down_sync(0xffffffffu, incl, o);
+      if (lane + o < 32) incl += t;
+    }
+    if (lane == 0) wsum[warp] = incl;
+    __syncthreads();
+    unsigned above_w = 0;
+    for (int w = warp + 1; w < 32; ++w) above_w += wsum[w];
+    const unsigned above_t = above_w + incl - mine;         // keys in bins of higher threads
+    const unsigned a3 = above_t, a2 = a3 + h3, a1 = a2 + h2, a0 = a1 + h1;
+    // exactly one bin satisfies above(b) < need <= above(b) + hist[b]
+    if (a3 < need && need <= a3 + h3) { wsum[64] = 4 * tid + 3; wsum[65] = need - a3; wsum[66] = h3; }
+    else if (a2 < need && need <= a2 + h2) { wsum[64] = 4 * tid + 2; wsum[65] = need - a2; wsum[66] = h2; }
+    else if (a1 < need && need <= a1 + h1) { wsum[64] = 4 * tid + 1; wsum[65] = need - a1; wsum[66] = h1; }
+    else if (a0 < need && need <= a0 + h0) { wsum[64] = 4 * tid; wsum[65] = need - a0; wsum[66] = h0; }
+    __syncthreads();
+    prefix |= wsum[64] << shift;
+    mask |= (bins - 1) << shift;
+    need = wsum[65];
+    eq_total = wsum[66];
+    __syncthreads();                                        // wsum / hist are rewritten by the next level
+    if (eq_total == need) break;                            // the whole cut-off bin is taken: nothing left to decide
+  }
+  // keys whose decided bits exceed the prefix win; keys that match it: all of them (eq_total == need), or - after the
+  // last level, where the match is on all 32 bits, i.e. an exact tie - the `need` lowest indices
+  const bool tie = eq_total != need;
+  if (tid == 0) sm.count = 0;
+  __syncthreads();
+  unsigned eq_before = 0;                                   // matching keys with a lower index, slots 0..j-1 of all threads
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const bool m = have[j] && (u[j] & mask) == prefix;
+    bool win = have[j] && (u[j] & mask) > prefix;
+    if (tie) {                                              // block-wide exclusive count of matches in index order
+      const unsigned bal = __ballot_sync(0xffffffffu, m);
+      if (lane == 0) wsum[warp] = __popc(bal);
+      __syncthreads();
+      unsigned below = eq_before;
+      for (int w = 0; w < warp; ++w) below += wsum[w];
+      unsigned tot = 0;
+      for (int w = 0; w < 32; ++w) tot += wsum[w];
+      below += __popc(bal & ((1u << lane) - 1));
+      win = win || (m && below < need);
+      eq_before += tot;
+      __syncthreads();
+    } else {
+      win = win || m;
+    }
+    if (win) {
+      const unsigned pos = atomicAdd(&sm.count, 1u);
+      sm.keys[pos] = ((unsigned long long)(~u[j]) << 32) | (unsigned)(tid + 1024 * j);
+    }
+  }
+  __syncthreads();
+  const int got = (int)sm.count;                            // == k
+  const int n_pad = next_pow2(got);
+  for (int i = got + tid; i < n_pad; i += 1024) sm.keys[i] = kKeyMax;
+  __syncthreads();
+  block_bitonic_sort(sm.keys, n_pad);
+  return got;
+}
+
 }  // namespace lsa

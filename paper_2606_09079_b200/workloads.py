@@ -110,6 +110,8 @@ class LsaWorkloadConfig:
     tie_frac: float = 0.0      # cfg 5: fraction of triggers carrying planted ties
     q_gain: float = 1.0        # 1.0 = BASELINE recipe q ~ N(0,1)/sqrt(D)
     kv_base_chunks: int = 0    # >0: cold pools are tiled from this many random chunks
+    seq_offset: int = 0        # this config holds sequences [seq_offset, seq_offset + B) of a batch of B_total
+    B_total: int = 0           # 0 = B (not a shard); see shard_config()
 
     # ---- derived per sequence -------------------------------------------------------
     def n_hca(self, b: int) -> int:
@@ -127,8 +129,8 @@ class LsaWorkloadConfig:
     def step0(self, b: int) -> int:
         if not self.stagger:
             return 0
-        # sequence b first fires at global step (b*tau//B) mod tau
-        return (self.tau - (b * self.tau // self.B) % self.tau) % self.tau
+        # sequence b first fires at global step (b*tau//B) mod tau (b, B of the whole batch)
+        return (self.tau - ((b + self.seq_offset) * self.tau // (self.B_total or self.B)) % self.tau) % self.tau
 
     @property
     def page_elems(self) -> int:
@@ -198,6 +200,17 @@ def make_config(config_id: int, **overrides) -> LsaWorkloadConfig:
     return dataclasses.replace(cfg, **overrides) if overrides else cfg
 
 
+def shard_config(cfg: LsaWorkloadConfig, lo: int, hi: int) -> LsaWorkloadConfig:
+    """Sequences [lo, hi) of `cfg` as a config of their own (one rank's share when the batch is sharded by sequence):
+    same per-sequence data and trigger phases as in the whole batch, the hot pool cut in proportion."""
+    if not (0 <= lo < hi <= cfg.B):
+        raise ValueError("bad shard")
+    pages = max(2 * sum(min(cfg.k, -(-(cfg.L[b] // cfg.csa_ratio) // cfg.C)) for b in range(lo, hi)),
+                cfg.hot_pages * (hi - lo) // cfg.B)
+    return dataclasses.replace(cfg, B=hi - lo, L=list(cfg.L[lo:hi]), hot_pages=pages, seq_offset=cfg.seq_offset + lo,
+                               B_total=cfg.B_total or cfg.B)
+
+
 def make_small_config(dtype: str = "f32", **kw) -> LsaWorkloadConfig:
     """A scaled-down shape for CPU tests and fast parity cases (not a BASELINE config)."""
     base = dict(name="small", config_id=101, dtype=dtype, B=2, L=[4096, 2432], H=8, D=64, C=16,
@@ -248,12 +261,13 @@ class LsaWorkload:
         Wf = as_f64(self.W_q, dt)
         for b in range(c.B):
             nch = c.n_chunks(b)
+            gb = b + c.seq_offset                   # index in the whole batch: a shard sees the same data
             if build_kv:
                 self._build_kv(b, kv_base, inv_sqrt_d)
 
             # planted query direction u_b and an h0 with  W_q h0 = s*u  built by least squares
             # (np.linalg.lstsq min-norm solve - a construction, not the query tower itself).
-            g = _rng(s, 20, b)
+            g = _rng(s, 20, gb)
             u = _unit_rows(g.standard_normal(c.E))
             gvec = g.standard_normal(c.Dh)
             zg = Wf @ gvec
@@ -262,7 +276,7 @@ class LsaWorkload:
             self.h0.append(store((gvec + corr).astype(np.float32), dt))
             self.u.append(u)
 
-            ge = _rng(s, 21, b)
+            ge = _rng(s, 21, gb)
             r = ge.standard_normal((nch, c.E))
             if c.emb_mode == "beta":
                 cosv = ge.beta(2.0, 8.0, size=nch)
@@ -276,15 +290,16 @@ class LsaWorkload:
     def _build_kv(self, b: int, kv_base: Optional[np.ndarray], inv_sqrt_d: float) -> None:
         c, dt, s = self.cfg, self.cfg.dtype, self.cfg.seed
         nh, nch, ncsa = c.n_hca(b), c.n_chunks(b), c.n_csa(b)
-        self.hca_k.append(_randn_stored(_rng(s, 10, b), (nh, c.D), inv_sqrt_d, dt))
-        self.hca_v.append(_randn_stored(_rng(s, 11, b), (nh, c.D), inv_sqrt_d, dt))
-        self.win_k.append(_randn_stored(_rng(s, 12, b), (c.W, c.D), inv_sqrt_d, dt))
-        self.win_v.append(_randn_stored(_rng(s, 13, b), (c.W, c.D), inv_sqrt_d, dt))
+        gb = b + c.seq_offset
+        self.hca_k.append(_randn_stored(_rng(s, 10, gb), (nh, c.D), inv_sqrt_d, dt))
+        self.hca_v.append(_randn_stored(_rng(s, 11, gb), (nh, c.D), inv_sqrt_d, dt))
+        self.win_k.append(_randn_stored(_rng(s, 12, gb), (c.W, c.D), inv_sqrt_d, dt))
+        self.win_v.append(_randn_stored(_rng(s, 13, gb), (c.W, c.D), inv_sqrt_d, dt))
         if kv_base is None:
-            cold = _randn_stored(_rng(s, 14, b), (nch, 2, c.C, c.D), inv_sqrt_d, dt)
+            cold = _randn_stored(_rng(s, 14, gb), (nch, 2, c.C, c.D), inv_sqrt_d, dt)
         else:
             # tile the base block with a per-sequence stride so chunks differ per (b, c)
-            idx = (np.arange(nch, dtype=np.int64) * 7 + 13 * b) % c.kv_base_chunks
+            idx = (np.arange(nch, dtype=np.int64) * 7 + 13 * gb) % c.kv_base_chunks
             cold = kv_base[idx].copy()
             # make every chunk unique in its first K element (cheap) so wrong copies are detectable
             tagv = store((((np.arange(nch) % 251) / 251.0 - 0.5) * inv_sqrt_d).astype(np.float32), dt)
@@ -310,7 +325,7 @@ class LsaWorkload:
         epoch = trigger_idx // c.needle_period
         key = (b, epoch)
         if key not in self._needle_cache:
-            g = _rng(c.seed, 30, b, epoch)
+            g = _rng(c.seed, 30, b + c.seq_offset, epoch)
             n = min(c.n_needles, c.n_chunks(b))
             self._needle_cache[key] = np.sort(g.choice(c.n_chunks(b), size=n, replace=False))
         return self._needle_cache[key]
@@ -321,7 +336,7 @@ class LsaWorkload:
         emb = self.base_emb[b].copy()
         ids = self.needle_ids(b, trigger_idx)
         if len(ids):
-            g = _rng(c.seed, 31, b, trigger_idx // c.needle_period)
+            g = _rng(c.seed, 31, b + c.seq_offset, trigger_idx // c.needle_period)
             r = g.standard_normal((len(ids), c.E))
             rows = self._plant(self.u[b], r, np.full(len(ids), c.needle_cos))
             emb[ids] = store(rows.astype(np.float32), c.dtype)
@@ -380,7 +395,7 @@ class LsaWorkload:
         c = self.cfg
         if c.tie_frac <= 0:
             return False
-        g = _rng(c.seed, 50, b, trigger_idx)
+        g = _rng(c.seed, 50, b + c.seq_offset, trigger_idx)
         return bool(g.uniform() < c.tie_frac)
 
     def total_cold_bytes(self) -> int:
