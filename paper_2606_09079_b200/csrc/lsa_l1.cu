@@ -73,6 +73,8 @@ struct GvJobs {
   long long ldo[kGvMaxJobs];
   int E[kGvMaxJobs];
   int n_jobs, shared_x;
+  long long lo_off;                     // bf16 outputs only, 0 = off: element e also gets its rounding residual
+                                        // bf16(v - float(bf16(v))) at out + lo_off, so that hi + lo carries ~16 bits
 };
 
 constexpr int kGvU = 8;                       // 16-byte loads per lane and batch: one batch = 2048 weights of a row
@@ -126,7 +128,13 @@ __device__ __forceinline__ void gv_rows(const GvJobs& jobs, const XT* xs, int j_
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
       const float v = warp_sum(acc[s][0] + acc[s][1]);
-      if (lane == 0 && i0 + s < n) out[(size_t)(i0 + s) * jobs.ldo[j] + e] = l1_out<OT>(v);
+      if (lane == 0 && i0 + s < n) {
+        const OT hi = l1_out<OT>(v);
+        out[(size_t)(i0 + s) * jobs.ldo[j] + e] = hi;
+        if constexpr (sizeof(OT) == 2) {
+          if (jobs.lo_off) out[(size_t)(i0 + s) * jobs.ldo[j] + e + jobs.lo_off] = __float2bfloat16_rn(v - __bfloat162float(hi));
+        }
+      }
       acc[s][0] = acc[s][1] = 0.f;
     }
   };
@@ -201,7 +209,7 @@ struct L1ScoreParams {
 };
 
 struct L1Smem {
-  alignas(1024) unsigned char q[16384];                          // [2 d-blocks][64 heads][128 B], SW128
+  alignas(1024) unsigned char q[32768];                          // [2 d-blocks][hi: 64 heads, lo: 64 heads][128 B], SW128
   alignas(1024) unsigned char stage[kL1Stages][kL1StageBytes];   // [2 d-blocks][128 entries][128 B], SW128
   float wm[2][4];                                                // per S buffer: the 4 warps' maxima
   uint64_t full[kL1Stages], empty[kL1Stages];
@@ -259,8 +267,8 @@ l1_score_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant
       uint32_t ring = 0;
       while (cur.next(piece, t0, t1)) {
         if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 40);
-        mbar_arrive_expect_tx(&sm.q_full, 16384);
-        tma_load_3d(sm.q, &map_q, 0, piece * kL1H, 0, &sm.q_full);
+        mbar_arrive_expect_tx(&sm.q_full, 32768);
+        tma_load_3d(sm.q, &map_q, 0, piece * 2 * kL1H, 0, &sm.q_full);
         const CUtensorMap* mk = p.k_maps + p.pieces[piece].map_idx;
         for (int t = t0; t < t1; ++t) {
           const int st = ring % kL1Stages;
@@ -290,10 +298,13 @@ l1_score_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant
           mbar_wait(&sm.full[st], (ring / kL1Stages) & 1, 44);
           tc_fence_after();
           const uint64_t a0 = dk0 + (uint64_t)(st * (kL1StageBytes >> 4));
+          // the query is kept as two bf16 terms (q = hi + lo, the Eq.(2) kernel writes both): K . hi, then K . lo into
+          // the same accumulator - the match then carries the fp32 query, not its 8-bit rounding
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks) {
-            const uint64_t off_a = (uint64_t)(((ks >> 2) * 16384 + (ks & 3) * 32) >> 4);
-            const uint64_t off_b = (uint64_t)(((ks >> 2) * 8192 + (ks & 3) * 32) >> 4);
+          for (int ks = 0; ks < 16; ++ks) {
+            const int kk = ks & 7, part = ks >> 3;
+            const uint64_t off_a = (uint64_t)(((kk >> 2) * 16384 + (kk & 3) * 32) >> 4);
+            const uint64_t off_b = (uint64_t)(((kk >> 2) * 16384 + part * 8192 + (kk & 3) * 32) >> 4);
             umma_bf16(tS + buf * 64, a0 + off_a, dq0 + off_b, id_s, ks != 0);
           }
           umma_commit(&sm.empty[st]);
@@ -397,7 +408,7 @@ struct L1Plan {
   CUtensorMap* d_maps = nullptr;       // [B * L]
   CUtensorMap map_q{};
   float* cq = nullptr;                 // [L][cap][d_c]
-  __nv_bfloat16* q = nullptr;          // [cap * L][64 * 128]
+  __nv_bfloat16* q = nullptr;          // [cap * L][2: hi, lo][64 * 128]
   float* wbuf = nullptr;               // [cap * L][64]
   float* chunk_pre = nullptr;          // [cap * L][n_chunks_max]
   int cap = 0;                         // sequences per launch
@@ -456,10 +467,10 @@ int l1_create(const L1Init& init, L1Plan** out, std::string* msg) {
   L1_CUDA(cudaMemcpy(pl->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
   const size_t pieces = (size_t)pl->cap * L;
   L1_CUDA(cudaMalloc(&pl->cq, (size_t)L * pl->cap * init.d_c * sizeof(float)));
-  L1_CUDA(cudaMalloc(&pl->q, pieces * kL1H * kL1CI * sizeof(__nv_bfloat16)));
+  L1_CUDA(cudaMalloc(&pl->q, pieces * 2 * kL1H * kL1CI * sizeof(__nv_bfloat16)));
   L1_CUDA(cudaMalloc(&pl->wbuf, pieces * kL1H * sizeof(float)));
   L1_CUDA(cudaMalloc(&pl->chunk_pre, pieces * (size_t)std::max(init.n_chunks_max, 1) * sizeof(float)));
-  if (!l1_encode(pl->encode, &pl->map_q, pl->q, pieces * kL1H, kL1H, msg)) { delete pl; return -2; }
+  if (!l1_encode(pl->encode, &pl->map_q, pl->q, pieces * 2 * kL1H, 2 * kL1H, msg)) { delete pl; return -2; }
   pl->smem = sizeof(L1Smem) + 1024;
   L1_CUDA(cudaFuncSetAttribute(l1_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
   if ((size_t)kGvSeqs * init.Dh * 2 > 200 * 1024 || (size_t)kGvSeqs * init.d_c * 4 > 200 * 1024) { *msg = "Dh / d_c too large for the staged projections"; delete pl; return -6; }
@@ -499,12 +510,12 @@ int l1_select(L1Plan* pl, const SeqDev* d_seqs, const void* h, const int* ids, c
       j13.x[l] = hb; j13.out[l] = cq; j13.ldo[l] = d_c; j13.E[l] = d_c;
       j13.W[L + l] = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_w);
       j13.x[L + l] = hb; j13.out[L + l] = pl->wbuf + (size_t)l * kL1H; j13.ldo[L + l] = (long long)L * kL1H; j13.E[L + l] = kL1H;
-      // Eq.(2): q -> piece (i, l), rounded to bf16
+      // Eq.(2): q -> piece (i, l) as two bf16 terms (hi, lo)
       j2.W[l] = reinterpret_cast<const __nv_bfloat16*>(in.layers[l].W_iuq);
-      j2.x[l] = cq; j2.out[l] = pl->q + (size_t)l * kL1H * kL1CI; j2.ldo[l] = (long long)L * kL1H * kL1CI; j2.E[l] = kL1H * kL1CI;
+      j2.x[l] = cq; j2.out[l] = pl->q + (size_t)l * 2 * kL1H * kL1CI; j2.ldo[l] = (long long)L * 2 * kL1H * kL1CI; j2.E[l] = kL1H * kL1CI;
     }
     j13.n_jobs = 2 * L; j13.shared_x = 1;
-    j2.n_jobs = L; j2.shared_x = 0;
+    j2.n_jobs = L; j2.shared_x = 0; j2.lo_off = (long long)kL1H * kL1CI;
     const unsigned gy = (unsigned)((m + kGvSeqs - 1) / kGvSeqs);
     // persistent blocks: as many as fit on the machine at once (shared memory bounds the occupancy)
     auto blocks_x = [&](int per_sm, int rows, int z) {

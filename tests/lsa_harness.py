@@ -89,8 +89,40 @@ def attn_tolerance(dtype: str):
     return dict(atol=2e-2, rtol=1e-2) if dtype == "bf16" else dict(atol=1e-4, rtol=1e-4)
 
 
+def apply_tie_triggers(wl: LsaWorkload, oracle: LsaOracle, rig, global_step: int, h, state: dict) -> int:
+    """BASELINE.json cfg 5: "10% of triggers carry planted exact-tie and near-tie scores".  At a trigger the workload marks
+    (LsaWorkload.has_tie_trigger) both sides get the table in force with an exact tie planted across the k-th rank of the
+    ORACLE's ranking (rank k+1's row becomes a bit copy of rank k's: the lower chunk id must win) and a one-ulp near-tie
+    behind it; the next trigger of that sequence restores the plain table.  Returns the number of tie triggers applied."""
+    from oracle import chunk_scores, query_tower
+    from paper_2606_09079_b200.workloads import plant_boundary_ties, to_torch
+    c = wl.cfg
+    n = 0
+    for b in range(c.B):
+        if not wl.fires(b, global_step):
+            continue
+        trig = wl.trigger_index(b, global_step)
+        if wl.has_tie_trigger(b, trig):
+            base = state.get(("plain", b), oracle.chunk_emb[b])
+            state[("plain", b)] = base
+            sc = chunk_scores(query_tower(oracle.W_q, h[b]), base)
+            order = np.array(sorted(range(len(sc)), key=lambda ch: (-sc[ch], ch)))
+            tied = plant_boundary_ties(base, order, c.k_eff(b), c.dtype)
+            oracle.chunk_emb[b] = tied
+            if rig is not None:
+                t = to_torch(tied, c.dtype).to(rig.device)
+                state[("dev", b)] = t                       # keep the tensor alive while the library reads it
+                rig.ctx.set_chunk_emb(b, t)
+            n += 1
+        elif ("plain", b) in state:
+            oracle.chunk_emb[b] = state.pop(("plain", b))
+            if rig is not None:
+                rig.ctx.set_chunk_emb(b, rig.emb[b])
+    return n
+
+
 def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=None, with_kv_new: bool = True,
-                 tie_emb_builder=None, l1=None, l1_band: float = 3e-2, step_fn=None):
+                 l1=None, l1_band: float = 3e-2, step_fn=None):
     """Drive lsa_step and the oracle in lock-step: validate the GPU's
     selection against the oracle's scores, feed it to the oracle's residency model, then compare page
     tables / residency / fetched bytes bit-exactly and attention outputs within tolerance."""
@@ -99,10 +131,12 @@ def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=
     c = wl.cfg
     orc = make_oracle(wl)
     tol = attn_tolerance(c.dtype)
-    n_checked, max_err = 0, 0.0
+    n_checked, max_err, n_ties, tie_state = 0, 0.0, 0, {}
     for t in range(steps):
         apply_emb_updates(wl, orc, t, rig.emb)
         q, h = wl.q(t), wl.h(t)
+        if c.tie_frac > 0:
+            n_ties += apply_tie_triggers(wl, orc, rig, t, h, tie_state)
         kn, vn = wl.kv_new(t) if with_kv_new else (None, None)
         firing = [b for b in range(c.B) if orc.step[b] % c.tau == 0]
         bytes_before = rig.ctx.stats()["bytes_fetched"] if not firing else None
@@ -155,4 +189,4 @@ def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=
             max_err = max(max_err, float(np.max(np.abs(got - res[0]))))
             n_checked += 1
     rig.ctx.sync()
-    return dict(checked=n_checked, max_abs_err=max_err, oracle=orc)
+    return dict(checked=n_checked, max_abs_err=max_err, oracle=orc, tie_triggers=n_ties)

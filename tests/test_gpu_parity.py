@@ -584,10 +584,12 @@ def test_cfg5_churn_sampled():
     cfg = make_config(5)
     wl = LsaWorkload(cfg)
     rig = GpuRig(wl)
-    steps = 16 * 4 + 2
-    r = run_lockstep(wl, rig, steps, check_attention_at={0, 1, 16, 17, 33, 64, 65})
+    steps = 16 * 6 + 2                      # the seeded draws mark sequence 2's triggers 5 and 6 (steps 80 and 96) as tie triggers
+    r = run_lockstep(wl, rig, steps, check_attention_at={0, 1, 16, 17, 33, 64, 65, 81, 97})
     st = rig.ctx.stats()
     assert st["evictions"] > 0 and st["misses"] > 3 * 8 * 128 * 0.6
+    # BASELINE.json configs[4]: 10 % of the triggers carry a planted exact tie and a one-ulp near-tie across the k-th rank
+    assert r["tie_triggers"] >= 2
 
 
 def test_cfg4_ragged_batch_sampled():
