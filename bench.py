@@ -398,6 +398,7 @@ def main():
                     tie_tables[(b, trig)] = to_torch(plant_boundary_ties(wl.chunk_emb(b, trig), order, c.k_eff(b), c.dtype), c.dtype).to(dev)
     torch.cuda.synchronize()
     n_tie_triggers = [0]
+    drift_needs_host_sync = False        # (the drift / tie updates of one_step are not replayed by the async leg: it keeps the tables)
 
     def one_step(i, host=None, rs=None):
         rs = reps if rs is None else rs
@@ -473,19 +474,55 @@ def main():
     value = units_job / (ms * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (H2D + D2H inside the timed region) ----
+    # Every step's q, k_new, v_new (and h at trigger steps) are pulled out of pinned host memory and its result lands in
+    # pinned host memory, where the host waits for it.  e2e: lsa_step_host_async, up to E2E_DEPTH steps in flight, each
+    # with an output buffer of its own, every ticket waited for inside the region (a serving loop with several independent
+    # requests in flight); e2e_sync: lsa_step_host, the host blocks on every step.
+    E2E_DEPTH = 6
     pin = lambda t: t.cpu().pin_memory()
     host = dict(q=[pin(x) for x in qs], h=[pin(x) for x in hs], kn=[pin(x) for x in kns], vn=[pin(x) for x in vns],
                 out=torch.empty((c.B, c.H, c.D), dtype=tdt).pin_memory())
+    outs = [torch.empty((c.B, c.H, c.D), dtype=tdt).pin_memory() for _ in range(E2E_DEPTH + 1)]
     for i in range(max(3, R)):
         one_step(i_next + i, host)
     i_next += max(3, R)
     n_e2e = max(64, args.steps // 4)
-    ms_e2e, _, enq_e2e, _ = timed(n_e2e, host, i0=i_next)
+    ms_sync, _, enq_e2e, _ = timed(n_e2e, host, i0=i_next)
     i_next += n_e2e
+
+    def timed_async(n, i0):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        tickets = []
+        barrier()
+        e0.record(sc)
+        for i in range(n):
+            r = reps[(i0 + i) % R]
+            t, j = r.step, (i0 + i) % NIN
+            tickets.append((r, r.ctx.step_host_async(host["q"][j], host["h"][(t // c.tau) % NIN], host["kn"][j], host["vn"][j],
+                                                     outs[i % len(outs)])))
+            r.step += 1
+            if len(tickets) > E2E_DEPTH:
+                rr, tk = tickets.pop(0)
+                rr.ctx.host_wait(tk)
+        for rr, tk in tickets:
+            rr.ctx.host_wait(tk)
+        sc.wait_stream(sf)
+        e1.record(sc)
+        sf.synchronize(); sc.synchronize()
+        barrier()
+        return max_over_ranks(e0.elapsed_time(e1), dev)
+
+    if c.B <= 4 and args.overlap == 1 and c.dtype == "bf16" and not drift_needs_host_sync:
+        timed_async(max(3, R), i_next); i_next += max(3, R)
+        ms_e2e = timed_async(n_e2e, i_next); i_next += n_e2e
+        e2e_mode = f"lsa_step_host_async, up to {E2E_DEPTH} steps in flight, every ticket waited for inside the region"
+    else:
+        ms_e2e, e2e_mode = ms_sync, "lsa_step_host (the host blocks on every step)"
     es = 4 if c.dtype == "f32" else 2
     h2d = (c.B * c.H * c.D + 2 * c.B * c.D) * es + c.B * c.Dh * es // c.tau     # h crosses only at trigger steps (1 in tau)
     d2h = c.B * c.H * c.D * es
     e2e_value = job_units(n_e2e) / (ms_e2e * 1e-3)
+    e2e_sync_value = job_units(n_e2e) / (ms_sync * 1e-3)
     clocks = clk.stop()
 
     # ---- the other step_overlap mode, on replicas of its own (every rank runs it: there are barriers inside) ----
@@ -742,7 +779,8 @@ def main():
                              replicas=R, replica_trigger_phases=phases, sequences_this_rank=c.B,
                              note="step_overlap = 1: the timed steps belong to independent layer-state replicas and their inputs are staged before the loop"),
                     e2e=dict(value=e2e_value, unit=unit, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=n_e2e,
-                             ms_per_step=ms_e2e / n_e2e),
+                             ms_per_step=ms_e2e / n_e2e, mode=e2e_mode,
+                             sync=dict(value=e2e_sync_value, ms_per_step=ms_sync / n_e2e, mode="lsa_step_host: the host blocks on every step")),
                     gpu_launches=int(launches), triggers_in_timed_region=int(triggers_timed), index_launches=int(index_launches),
                     tie_triggers_seen=n_tie_triggers[0], clocks=clocks, roofline=roofline, dependent_inputs=dependent,
                     cpu_baseline=cpu_baseline, cpu_baseline_1t=cpu_baseline_1t,

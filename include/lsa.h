@@ -47,7 +47,9 @@ enum lsa_status {
   LSA_OK = 0,
   LSA_ERR_INVALID_ARG = -1,    /* bad shape / null pointer / non-pinned cold pool / k > pages ... */
   LSA_ERR_CUDA = -2,           /* a CUDA runtime call failed (text in lsa_last_error)             */
-  LSA_ERR_POOL_EXHAUSTED = -3, /* S4 found no unpinned page (cannot happen if hot_pages >= 2*sum k) */
+  LSA_ERR_POOL_EXHAUSTED = -3, /* S4 found no unpinned page (cannot happen if hot_pages >= 2*sum k): reported by lsa_sync / */
+                               /* lsa_get_stats; the pass that failed changed no table, residency or counter, but the   */
+                               /* host's step bookkeeping has moved on - destroy the context                              */
   LSA_ERR_OOM = -4,
   LSA_ERR_STATE = -5,          /* call sequence not allowed (e.g. destroyed ctx)                  */
   LSA_ERR_UNSUPPORTED = -6     /* shape has no compiled kernel */
@@ -181,9 +183,20 @@ int lsa_graph_stats(lsa_ctx* ctx, uint64_t* captures, uint64_t* replays);
 /* lsa_step with HOST buffers.  Pinned + mapped inputs (e.g. torch pin_memory) are pulled over the host link by
  * one small kernel and a pinned `out` is written in place by S8; pageable buffers go through one packed
  * host->device copy and one device->host copy.  h is only read at trigger steps.  Blocks until the result
- * has landed.  Used for end-to-end timing. */
+ * has landed.  Used for end-to-end timing.  Pinned buffers are recognised once per address (the device alias is
+ * cached): a buffer passed here must stay registered, at that address, while the context lives. */
 int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new,
                   const void* v_new, void* out);
+
+/* lsa_step_host without the wait: the step is enqueued (inputs pulled from the pinned host buffers, result written to the
+ * pinned `out` in place) and *ticket identifies it; lsa_host_wait(ctx, ticket) returns once that step's `out` has landed
+ * (a completion word in pinned memory, written by the step's last CTA, is read - no stream synchronisation).  Steps
+ * complete in order.  Up to 8 steps may be in flight: q, k_new, v_new, h and out of a step must stay untouched until its
+ * ticket has been waited for.  Needs lsa_config.step_overlap = 1, B <= 4 on the tcgen05 path and pinned + mapped buffers;
+ * otherwise the call completes synchronously and returns ticket 0 (which lsa_host_wait accepts). */
+int lsa_step_host_async(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out,
+                        uint64_t* ticket);
+int lsa_host_wait(lsa_ctx* ctx, uint64_t ticket);
 
 /* ---- paper-exact Level-1 Memory Indexer (Eq.(1)-(5), l.142 Eq.(13))) --------
  * An alternative to lsa_index_select with the scorer the paper states: per indexer layer

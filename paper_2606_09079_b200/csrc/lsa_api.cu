@@ -50,6 +50,15 @@ struct lsa_ctx {
   std::vector<unsigned int> app_count;
   bool no_small = false;               // lsa_step_graph: the captured launch must read the device records
   bool serialize_next = false;         // something the next attention launch reads was enqueued on another stream
+  bool inputs_from_prev_kernel = false;// lsa_step_host: q / k_new / v_new come from the gather kernel just enqueued
+  unsigned int* host_flag = nullptr;   // lsa_step_host: pinned completion word (host address / device alias below)
+  unsigned int* host_flag_dev = nullptr;
+  unsigned int host_flag_seq = 0;
+  bool host_flag_armed = false;        // the launch just enqueued will write host_flag_seq to the flag
+  bool next_alone = false;             // the caller will block on the step being enqueued
+  unsigned int* gather_ctr = nullptr;  // DEVICE: finished blocks of the gather kernels of lsa_step_host_async
+  unsigned int gather_total = 0;       // as enqueued
+  bool inputs_by_counter = false;      // the next attention launch waits for gather_total instead of for the stream
   // index scratch
   float* d_z = nullptr;
   float* d_scores = nullptr;
@@ -72,7 +81,9 @@ struct lsa_ctx {
   unsigned long long sg_launches = 0, sg_captures = 0, sg_replays = 0;
   int indexer = 0;                     // lsa_indexer used by lsa_step at trigger steps
   // host-buffer staging (lsa_step_host)
-  void *st_q = nullptr, *st_h = nullptr, *st_kn = nullptr, *st_vn = nullptr, *st_out = nullptr, *st_pin = nullptr;
+  void *st_q = nullptr, *st_out = nullptr, *st_pin = nullptr;
+  unsigned long long st_calls = 0;                  // lsa_step_host calls so far: image st_calls % kStRing is next
+  uint64_t st_ticket[8] = {0, 0, 0, 0, 0, 0, 0, 0}; // ticket of the step that used each image last (0: none / complete)
   const void* out_host_cached = nullptr;
   std::vector<std::pair<const void*, void*>> alias_cache;   // host pointer -> device alias (or null)
   void* out_dev_alias = nullptr;
@@ -148,6 +159,7 @@ extern "C" void lsa_destroy(lsa_ctx* ctx) {
   if (ctx->l2) l2_destroy(ctx->l2);
   if (ctx->sg_exec) cudaGraphExecDestroy(ctx->sg_exec);
   if (ctx->st_pin) cudaFreeHost(ctx->st_pin);
+  if (ctx->host_flag) cudaFreeHost(ctx->host_flag);
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
   if (ctx->ev_compute) cudaEventDestroy(ctx->ev_compute);
@@ -550,8 +562,18 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
       stp.k_new = app ? pre->k_new : nullptr;
       stp.v_new = app ? pre->v_new : nullptr;
       stp.serialize = (!pre || stp.swap || c->serialize_next) ? 1 : 0;
-      stp.wait_inputs = c->cfg.step_overlap ? 0 : 1;
+      stp.wait_inputs = (c->cfg.step_overlap && !c->inputs_from_prev_kernel) ? 0 : 1;
+      if (c->inputs_by_counter) { stp.wait_inputs = 0; stp.in_ctr = c->gather_ctr; stp.in_need = c->gather_total; }
+      c->inputs_by_counter = false;
+      stp.alone = c->next_alone ? 1 : 0;
       c->serialize_next = false;
+      c->inputs_from_prev_kernel = false;
+      c->next_alone = false;
+      if (c->host_flag_dev) {                       // lsa_step_host spins on the flag instead of synchronising the stream
+        stp.host_flag = c->host_flag_dev;
+        stp.host_flag_val = ++c->host_flag_seq;
+        c->host_flag_armed = true;
+      }
       rc = tc_attention_small(c->tc, q, out, lse, stp, c->sc, &launches, &ctas, &msg,
                               prof ? c->prof_ev[LSA_PH_ATTENTION][2 * ia + 1] : nullptr,
                               prof ? c->prof_ev[LSA_PH_COMBINE][2 * ic] : nullptr,
@@ -782,12 +804,22 @@ struct HostGather {
   const uint4* src[4];
   uint4* dst[4];
   unsigned n16[4];     // 16-byte units per part (0 = absent)
+  unsigned int* ctr;   // or null: every block adds 1 (release) once its share is written - the attention launch that runs
+                       // beside it waits for the total instead of for the grid
 };
 __global__ void __launch_bounds__(256) host_gather_kernel(HostGather g) {
+  // the attention launch that follows may start its K/V stream now; it waits for this grid before it reads q / k_new
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
 #pragma unroll
   for (int p = 0; p < 4; ++p)
     for (unsigned i = tid; i < g.n16[p]; i += nthr) g.dst[p][i] = g.src[p][i];
+  if (g.ctr) {
+    asm volatile("fence.proxy.async;" ::: "memory");      // the image is read by TMA (async proxy)
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(g.ctr) : "memory");
+  }
 }
 
 // device alias of a pinned + mapped host pointer, or null (cached: the attribute query costs about a microsecond)
@@ -803,24 +835,58 @@ static void* host_alias(lsa_ctx* c, const void* p) {
   return d;
 }
 
-extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
-  if (!ctx) return LSA_ERR_STATE;
-  lsa_ctx* c = ctx;
+constexpr int kStRing = 8;            // staging images in rotation: lsa_step_host_async calls in flight at most
+
+static int host_wait_impl(lsa_ctx* c, uint64_t ticket) {
+  if (ticket == 0 || !c->host_flag) { LSA_CUDA(c, cudaStreamSynchronize(c->sc)); return LSA_OK; }
+  volatile unsigned int* f = c->host_flag;
+  const unsigned int want = (unsigned int)ticket;
+  for (long long spin = 0; (int)(*f - want) < 0; ++spin) {
+    if (spin > 20000000ll) { LSA_CUDA(c, cudaStreamSynchronize(c->sc)); break; }     // bounded: fall back to the stream
+#if defined(__x86_64__)
+    __builtin_ia32_pause();
+#endif
+  }
+  return LSA_OK;
+}
+
+// ticket: null = block until the result has landed; else the step is only enqueued and *ticket identifies it
+static int step_host_impl(lsa_ctx* c, const void* q, const void* h, const void* k_new, const void* v_new, void* out, uint64_t* ticket) {
   if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
   if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
   const lsa_config& cfg = c->cfg;
   auto up = [](size_t n) { return (n + 255) / 256 * 256; };
   const size_t qb = (size_t)c->B * cfg.H * cfg.D * c->elem, hb = (size_t)c->B * cfg.Dh * c->elem,
                nb = (size_t)c->B * cfg.D * c->elem;
-  // one packed image [q | k_new | v_new | h] in pinned host memory -> ONE host-to-device copy per step
+  // one packed image [q | k_new | v_new | h] per step; kStRing of them in rotation, so that the image of a step still
+  // in flight is not overwritten by the next ones
   const size_t o_kn = up(qb), o_vn = o_kn + up(nb), o_h = o_vn + up(nb), in_bytes = o_h + up(hb);
   if (!c->st_q) {
     int rc;
     unsigned char* p = nullptr;
-    if ((rc = dev_alloc(c, &p, in_bytes + up(qb)))) return rc;
-    c->st_q = p; c->st_kn = p + o_kn; c->st_vn = p + o_vn; c->st_h = p + o_h; c->st_out = p + in_bytes;
+    if ((rc = dev_alloc(c, &p, kStRing * in_bytes + up(qb)))) return rc;
+    c->st_q = p; c->st_out = p + kStRing * in_bytes;
     LSA_CUDA(c, cudaHostAlloc(&c->st_pin, in_bytes, cudaHostAllocDefault));
+    if (c->cfg.step_overlap && c->attn_impl == LSA_ATTN_TCGEN05 && tc_small_supported(c->tc)) {
+      void* f = nullptr;
+      LSA_CUDA(c, cudaHostAlloc(&f, 64, cudaHostAllocMapped));
+      memset(f, 0, 64);
+      c->host_flag = static_cast<unsigned int*>(f);
+      void* fd = nullptr;
+      LSA_CUDA(c, cudaHostGetDevicePointer(&fd, f, 0));
+      c->host_flag_dev = static_cast<unsigned int*>(fd);
+      if ((rc = dev_alloc(c, &c->gather_ctr, 1))) return rc;
+    }
   }
+  const int slot = (int)(c->st_calls % kStRing);
+  if (c->st_ticket[slot]) {                       // the step that used this image last has completed (normally long ago)
+    int rc = host_wait_impl(c, c->st_ticket[slot]);
+    if (rc) return rc;
+    c->st_ticket[slot] = 0;
+  }
+  c->st_calls += 1;
+  unsigned char* img = static_cast<unsigned char*>(c->st_q) + (size_t)slot * in_bytes;
+  void *st_q = img, *st_kn = img + o_kn, *st_vn = img + o_vn, *st_h = img + o_h;
   bool fire = false;
   for (int b = 0; b < c->B; ++b) fire |= (c->step[b] % cfg.tau == 0);
   if (fire && !h) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "h is NULL at a trigger step");
@@ -828,25 +894,41 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
   void* akn = k_new ? host_alias(c, k_new) : nullptr;
   void* avn = v_new ? host_alias(c, v_new) : nullptr;
   void* ah = fire ? host_alias(c, h) : nullptr;
+  bool gathered = false;
   if (aq && (!k_new || (akn && avn)) && (!fire || ah) && qb % 16 == 0 && nb % 16 == 0 && hb % 16 == 0) {
     HostGather g{};
-    g.src[0] = (const uint4*)aq; g.dst[0] = (uint4*)c->st_q; g.n16[0] = (unsigned)(qb / 16);
+    g.src[0] = (const uint4*)aq; g.dst[0] = (uint4*)st_q; g.n16[0] = (unsigned)(qb / 16);
     if (k_new) {
-      g.src[1] = (const uint4*)akn; g.dst[1] = (uint4*)c->st_kn; g.n16[1] = (unsigned)(nb / 16);
-      g.src[2] = (const uint4*)avn; g.dst[2] = (uint4*)c->st_vn; g.n16[2] = (unsigned)(nb / 16);
+      g.src[1] = (const uint4*)akn; g.dst[1] = (uint4*)st_kn; g.n16[1] = (unsigned)(nb / 16);
+      g.src[2] = (const uint4*)avn; g.dst[2] = (uint4*)st_vn; g.n16[2] = (unsigned)(nb / 16);
     }
-    if (fire) { g.src[3] = (const uint4*)ah; g.dst[3] = (uint4*)c->st_h; g.n16[3] = (unsigned)(hb / 16); }
+    if (fire) { g.src[3] = (const uint4*)ah; g.dst[3] = (uint4*)st_h; g.n16[3] = (unsigned)(hb / 16); }
     const unsigned total = g.n16[0] + g.n16[1] + g.n16[2] + g.n16[3];
-    host_gather_kernel<<<std::max(1u, std::min(64u, (total + 255u) / 256u)), 256, 0, c->sc>>>(g);
-    LSA_CUDA(c, cudaGetLastError());
-    c->serialize_next = true;
+    const dim3 grid(std::max(1u, std::min(64u, (total + 255u) / 256u)));
+    // it reads host buffers and writes an image no step in flight uses: with the overlapped path it need not wait for
+    // the previous step either (programmatic launch, no griddepcontrol.wait inside)
+    if (c->host_flag_dev && ticket && !fire) {
+      // asynchronous step: the gather runs beside the previous step (programmatic launch, no wait inside) and the
+      // attention launch waits for ITS blocks only - a grid dependency would wait for the previous step as well
+      g.ctr = c->gather_ctr;
+      c->gather_total += grid.x;
+      c->inputs_by_counter = true;
+      LSA_CUDA(c, launch_pdl(host_gather_kernel, grid, dim3(256), 0, c->sc, g));
+    } else if (c->host_flag_dev) LSA_CUDA(c, launch_pdl(host_gather_kernel, grid, dim3(256), 0, c->sc, g));
+    else {
+      host_gather_kernel<<<grid, 256, 0, c->sc>>>(g);
+      LSA_CUDA(c, cudaGetLastError());
+    }
+    c->inputs_from_prev_kernel = true;
+    gathered = true;
   } else {                         // pageable inputs: pack into the pinned staging image, one host-to-device copy
+    LSA_CUDA(c, cudaStreamSynchronize(c->sc));                        // the one pinned image is reused every call
     unsigned char* pin = static_cast<unsigned char*>(c->st_pin);
     memcpy(pin, q, qb);
     size_t upto = qb;
     if (k_new) { memcpy(pin + o_kn, k_new, nb); memcpy(pin + o_vn, v_new, nb); upto = o_vn + nb; }
     if (fire) { memcpy(pin + o_h, h, hb); upto = o_h + hb; }          // h is only read at trigger steps
-    LSA_CUDA(c, cudaMemcpyAsync(c->st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
+    LSA_CUDA(c, cudaMemcpyAsync(st_q, pin, upto, cudaMemcpyHostToDevice, c->sc));
     c->serialize_next = true;
   }
   if (fire) {                      // the indexer reads the staged h on the fetch stream: order it behind the copy
@@ -856,20 +938,45 @@ extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const v
   // result: if `out` is pinned and mapped, S8 writes it in place over the host link (no device-to-host copy
   // operation in the chain); otherwise through a device buffer and one copy
   if (out != c->out_host_cached) {
-    cudaPointerAttributes at{};
-    c->out_dev_alias = nullptr;
-    if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
-      c->out_dev_alias = at.devicePointer;
-    else
-      cudaGetLastError();
+    c->out_dev_alias = host_alias(c, out);
     c->out_host_cached = out;
   }
   void* out_dev = c->out_dev_alias ? c->out_dev_alias : c->st_out;
-  int rc = lsa_step(c, c->st_q, fire ? c->st_h : nullptr, k_new ? c->st_kn : nullptr, k_new ? c->st_vn : nullptr, out_dev);
+  c->host_flag_armed = false;
+  c->next_alone = ticket == nullptr;
+  int rc = lsa_step(c, st_q, fire ? st_h : nullptr, k_new ? st_kn : nullptr, k_new ? st_vn : nullptr, out_dev);
+  c->next_alone = false;
   if (rc) return rc;
-  if (!c->out_dev_alias) LSA_CUDA(c, cudaMemcpyAsync(out, c->st_out, qb, cudaMemcpyDeviceToHost, c->sc));
-  LSA_CUDA(c, cudaStreamSynchronize(c->sc));
-  return LSA_OK;
+  const bool flagged = c->host_flag_armed && c->out_dev_alias && gathered;
+  c->host_flag_armed = false;
+  if (!flagged) {                  // no completion word on this path: finish synchronously (a ticket of 0 is always complete)
+    if (!c->out_dev_alias) LSA_CUDA(c, cudaMemcpyAsync(out, c->st_out, qb, cudaMemcpyDeviceToHost, c->sc));
+    LSA_CUDA(c, cudaStreamSynchronize(c->sc));
+    if (ticket) *ticket = 0;
+    return LSA_OK;
+  }
+  // the launch's last CTA writes the step's sequence number to a pinned word once `out` (pinned, written in place) is
+  // complete: the host reads that word instead of synchronising the stream
+  c->st_ticket[slot] = c->host_flag_seq;
+  if (ticket) { *ticket = c->host_flag_seq; return LSA_OK; }
+  return host_wait_impl(c, c->host_flag_seq);
+}
+
+extern "C" int lsa_step_host(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out) {
+  if (!ctx) return LSA_ERR_STATE;
+  return step_host_impl(ctx, q, h, k_new, v_new, out, nullptr);
+}
+
+extern "C" int lsa_step_host_async(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new, void* out,
+                                   uint64_t* ticket) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!ticket) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null ticket");
+  return step_host_impl(ctx, q, h, k_new, v_new, out, ticket);
+}
+
+extern "C" int lsa_host_wait(lsa_ctx* ctx, uint64_t ticket) {
+  if (!ctx) return LSA_ERR_STATE;
+  return host_wait_impl(ctx, ticket);
 }
 
 // ---- NEXT-4 (first half): KV export into the cold pool -------------------------------------------------------

@@ -50,9 +50,6 @@ combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int 
   const int dh = blockIdx.x & 1, g = (blockIdx.x >> 1) & 7, hh = (blockIdx.x >> 4) & 1, m = blockIdx.x >> 5, b = blockIdx.y;
   const int h0 = hh * 32 + g * 4;
   const int dl = tid & 63, grp = tid >> 6;
-#ifdef LSA_TC_TRACE
-  const unsigned long long g_entry = gtime();
-#endif
   const int n_box = (n_cta + kCombRows - 1) / kCombRows;
   if (tid == 0) {
     mbar_init(&bar, 1);
@@ -62,10 +59,6 @@ combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int 
   __syncthreads();
   griddep_wait();                                 // partials and piece_info are final from here on
   griddep_launch_dependents();                    // the next kernel in the stream may start its own prologue
-#ifdef LSA_TC_TRACE
-  const unsigned long long g_dep = gtime();
-  const long long c_dep = clock64();
-#endif
   if (tid == kCombineThreads - 32) {              // rows b .. b + 32 n_box - 1 of column block (m, hh, g, dh); a warp
                                                   // that has no small loads to wait for issues the copies
     mbar_arrive_expect_tx(&bar, (uint32_t)(n_box * kCombBoxBytes));
@@ -92,9 +85,6 @@ combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int 
     active = info.x <= b && b < info.x + info.y && m4.x != -INFINITY;
     if (active) { mi = m4; li = l4; }
   }
-#ifdef LSA_TC_TRACE
-  const long long c_small = mi.x > 1e30f ? 0ll : clock64();   // after the small loads have returned (thread 0)
-#endif
   float4 mmax = mi;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -138,15 +128,9 @@ combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int 
     const float4 r = red_f[w];
     l_star.x += r.x; l_star.y += r.y; l_star.z += r.z; l_star.w += r.w;
   }
-#ifdef LSA_TC_TRACE
-  const long long c_w = clock64();
-#endif
   // ---- weighted sum of the partials (row c of the landing buffer = slot b + c = CTA c) ----
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   mbar_wait(&bar, 0, 40);
-#ifdef LSA_TC_TRACE
-  const long long c_land = clock64();
-#endif
   {
     const uint2* rows = reinterpret_cast<const uint2*>(comb_rows) + dl;
 #pragma unroll 4
@@ -161,9 +145,6 @@ combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int 
       }
     }
   }
-#ifdef LSA_TC_TRACE
-  const long long c_l = clock64();
-#endif
   acc_s[grp][dl] = acc;
   __syncthreads();
   if (tid < 256) {                                // thread = one output element: head h0 + e, d = m*128 + dh*64 + dl
@@ -175,16 +156,6 @@ combine_tc_kernel(const __grid_constant__ CUtensorMap map_part, TcParams p, int 
     const float ls = e == 0 ? l_star.x : e == 1 ? l_star.y : e == 2 ? l_star.z : l_star.w;
     out[((size_t)b * kTcH + h0 + e) * kTcD + m * 128 + dh * 64 + dl] = __float2bfloat16_rn(ls > 0.f ? s / ls : 0.f);
   }
-#ifdef LSA_TC_TRACE
-  __syncthreads();
-  if (tid == 0 && blockIdx.x == 0 && b == 0) {
-    const long long c_end = clock64();
-    tlog_add(p.tlog, 3, g_entry); tlog_add(p.tlog, 4, g_dep);
-    tlog_pair(p.tlog, 8, 0, c_small - c_dep); tlog_pair(p.tlog, 6, 0, c_w - c_dep); tlog_pair(p.tlog, 9, 0, c_land - c_dep);
-    tlog_pair(p.tlog, 7, 0, c_l - c_dep); tlog_pair(p.tlog, 10, 0, c_end - c_dep);
-  }
-  if (tid == 0 && blockIdx.x == gridDim.x - 1 && b == 0) tlog_add(p.tlog, 5, g_dep);
-#endif
   if (lse && m == 0 && dh == 0 && tid < 4) {
     const float ls = tid == 0 ? l_star.x : tid == 1 ? l_star.y : tid == 2 ? l_star.z : l_star.w;
     const float ms = tid == 0 ? m_star.x : tid == 1 ? m_star.y : tid == 2 ? m_star.z : m_star.w;
@@ -314,6 +285,7 @@ struct TcPlan {
   CUtensorMap* d_maps = nullptr;
   CUtensorMap* d_maps8 = nullptr;      // small path: [B][8], 128-row and 64-row boxes
   SmMaps0 maps0{};                     // those of sequence 0, passed by value
+  std::vector<std::pair<const void*, CUtensorMap>> q_maps;   // Q tensor maps by buffer address
   bool small_ok = false;
   TcParams params{};
   unsigned long long grid_total = 0;   // host mirror of the fused-S8 arrival counter
@@ -496,12 +468,6 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   TC_CUDA(cudaMalloc(&p.grid_ctr, sizeof(unsigned int)));
   TC_CUDA(cudaMemset(p.grid_ctr, 0, sizeof(unsigned int)));
   p.fused = (init.B <= kTcFusedMaxB && init.fuse_combine) ? 1 : 0;   // opt-in (LSA_MERGE_FUSED)
-#ifdef LSA_TC_TRACE
-  TC_CUDA(cudaMalloc(&p.trace, (size_t)pl->grid_max * 3 * 32 * sizeof(long long)));
-  TC_CUDA(cudaMemset(p.trace, 0, (size_t)pl->grid_max * 3 * 32 * sizeof(long long)));
-  TC_CUDA(cudaMalloc(&p.tlog, (1 + 3 * 4096) * sizeof(unsigned long long)));
-  TC_CUDA(cudaMemset(p.tlog, 0, (1 + 3 * 4096) * sizeof(unsigned long long)));
-#endif
   pl->smem = sizeof(TcSmem) + 1024;
   TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
   TC_CUDA(cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
@@ -553,10 +519,6 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
     lc.numAttrs = 0;
     pl->ws->last_small = false;
   }
-#ifdef LSA_TC_TRACE
-  static const int no_pdl = getenv("LSA_NO_PDL") ? atoi(getenv("LSA_NO_PDL")) : 0;   // 1: combine, 2: attention, 3: both
-  if (no_pdl & 2) lc.numAttrs = 0;
-#endif
   if (prm.l2_mask) TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel<true>, pl->map_pool, pl->map_q, prm));
   else TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_kernel<false>, pl->map_pool, pl->map_q, prm));
   if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
@@ -569,9 +531,6 @@ int tc_attention(TcPlan* pl, const void* q, void* out, float* lse, long long til
   cudaLaunchConfig_t lc2{};
   lc2.gridDim = dim3(128, pl->init.B); lc2.blockDim = dim3(kCombineThreads); lc2.dynamicSmemBytes = kCombineSmemPad; lc2.stream = st;
   lc2.attrs = attr; lc2.numAttrs = 1;
-#ifdef LSA_TC_TRACE
-  if (no_pdl & 1) lc2.numAttrs = 0;
-#endif
   if (pl->init.B <= kCombineSpecMaxB) {
     const int land = (n_attn + kCombRows - 1) / kCombRows * kCombBoxBytes;
     if (land > kCombineSmemPad) lc2.dynamicSmemBytes = land;
@@ -589,8 +548,15 @@ bool tc_small_supported(const TcPlan* pl) { return pl && pl->small_ok; }
 
 int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const TcSmallStep& step, cudaStream_t st, int* launches,
                        int* ctas, std::string* msg, cudaEvent_t ev_mid0, cudaEvent_t ev_mid1, unsigned long long* ktime) {
-  if (q != pl->q_cached) {
-    if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
+  if (q != pl->q_cached) {                          // a few q buffers in rotation (staging images, input rings): keep their maps
+    bool hit = false;
+    for (auto& e : pl->q_maps)
+      if (e.first == q) { pl->map_q = e.second; hit = true; break; }
+    if (!hit) {
+      if (!encode_rows(pl->encode, &pl->map_q, q, (uint64_t)pl->init.B * kTcH, kTcH, 8, msg)) return -2;
+      if (pl->q_maps.size() >= 32) pl->q_maps.clear();
+      pl->q_maps.emplace_back(q, pl->map_q);
+    }
     pl->q_cached = q;
   }
   TcWorkspace* ws = pl->ws;
@@ -607,7 +573,10 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   }
   // Two launches are in flight at a time (the next one starts on the SMs this one leaves free), so a launch takes just
   // under half the SMs - the rest is headroom for the trigger side band - and every CTA the same number of half tiles
-  const long long g_cap = pl->init.max_ctas > 0 ? pl->grid_max : std::max(1, (pl->init.n_sms - 20) / 2);
+  // (a launch that waits for the stream anyway - trigger-free swap steps, host-synchronous steps - has no neighbour to
+  // share the machine with and takes every SM)
+  const bool alone = step.serialize || step.alone;
+  const long long g_cap = (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 20) / 2);
   const long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
   const int n_attn = (int)std::max<long long>(1, std::min<long long>(g_cap, (halves + per - 1) / per));
   const int buf = (int)(ws->n_small & 1);
@@ -626,10 +595,13 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   prm.done_need_prev = ws->done_total;               // the previous launch has been merged
   ws->done_total_prev = ws->done_total;
   ws->done_total += (unsigned)n_attn;
+  prm.done_after = ws->done_total;
+  prm.host_flag = step.host_flag; prm.host_flag_val = step.host_flag_val;
   prm.out = (__nv_bfloat16*)out; prm.lse = lse; prm.swap = step.swap; prm.W = pl->init.W;
   prm.k_new = (const __nv_bfloat16*)step.k_new; prm.v_new = (const __nv_bfloat16*)step.v_new;
   prm.ktime = ktime;
   prm.wait_inputs = step.wait_inputs;
+  prm.in_ctr = step.in_ctr; prm.in_need = step.in_need;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -650,29 +622,6 @@ void tc_set_l2_mask(TcPlan* pl, const uint32_t* mask) { pl->params.l2_mask = mas
 
 void tc_destroy(TcPlan* pl) {
   if (!pl) return;
-#ifdef LSA_TC_TRACE
-  if (const char* path = getenv("LSA_TC_TRACE_FILE")) {
-    std::vector<long long> h((size_t)pl->grid_max * 3 * 32);
-    cudaMemcpy(h.data(), pl->params.trace, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
-    if (FILE* f = fopen(path, "w")) {
-      for (int c = 0; c < pl->grid_max; ++c)
-        for (int r = 0; r < 3; ++r) {
-          fprintf(f, "%d %d", c, r);
-          for (int i = 0; i < 32; ++i) fprintf(f, " %lld", h[((size_t)c * 3 + r) * 32 + i]);
-          fprintf(f, "\n");
-        }
-      fclose(f);
-    }
-    std::vector<unsigned long long> tl(1 + 3 * 4096);
-    cudaMemcpy(tl.data(), pl->params.tlog, tl.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
-    if (FILE* f = fopen((std::string(path) + ".tlog").c_str(), "w")) {
-      for (unsigned long long i = 0; i < tl[0] && i < 4096; ++i) fprintf(f, "%llu %llu %llu\n", tl[1 + 3 * i], tl[2 + 3 * i], tl[3 + 3 * i]);
-      fclose(f);
-    }
-  }
-  cudaFree(pl->params.trace);
-  cudaFree(pl->params.tlog);
-#endif
   cudaFree(pl->d_maps);
   cudaFree(pl->d_maps8);
   ws_release(pl->ws);

@@ -54,6 +54,11 @@ struct TcSmallStep {
   int serialize;            // 1: the launch waits for everything before it in the stream (trigger and swap steps); 0: its
                             // CTAs start as the previous step's leave their SMs, while that step is still being merged
   int wait_inputs;          // 1: q / k_new / v_new may have been produced by the kernel just before this launch
+  const unsigned int* in_ctr;   // q / k_new / v_new are complete once *in_ctr has reached in_need (null: see wait_inputs)
+  unsigned int in_need;
+  int alone;                // 1: the caller blocks on this step (no neighbour launch to share the SMs with): use them all
+  unsigned int* host_flag;  // PINNED HOST word (device alias) set to host_flag_val when `out` is complete, or null
+  unsigned int host_flag_val;
 };
 bool tc_small_supported(const TcPlan* plan);
 int tc_attention_small(TcPlan* plan, const void* q, void* out, float* lse, const TcSmallStep& step, cudaStream_t st,

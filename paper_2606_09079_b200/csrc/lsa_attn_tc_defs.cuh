@@ -123,10 +123,6 @@ struct TcParams {
   // profiling only (null otherwise): [0] = min over CTAs of %globaltimer once past the launch dependency,
   // [1] = max over CTAs at exit - the kernel's own working time, with programmatic overlap left intact
   unsigned long long* ktime;
-#ifdef LSA_TC_TRACE
-  long long* trace;              // [grid][3 roles][32] clock64 stamps (debug builds only)
-  unsigned long long* tlog;      // [0] = entries; then (kernel id, globaltimer start, end) per launch of block 0
-#endif
 };
 
 __device__ __forceinline__ SeqView make_view(const TcParams& p, int b) {
@@ -235,17 +231,6 @@ __device__ __forceinline__ unsigned long long gtime() {
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
   return t;
 }
-#ifdef LSA_TC_TRACE
-__device__ __forceinline__ void tlog_add(unsigned long long* tlog, unsigned long long id, unsigned long long t0) {
-  const unsigned long long i = atomicAdd(tlog, 1ull);
-  if (i < 4096) { tlog[1 + 3 * i] = id; tlog[2 + 3 * i] = t0; tlog[3 + 3 * i] = gtime(); }
-}
-// raw pair (e.g. SM clock offsets): reading %globaltimer costs about a microsecond, clock64() a few cycles
-__device__ __forceinline__ void tlog_pair(unsigned long long* tlog, unsigned long long id, unsigned long long a, unsigned long long b) {
-  const unsigned long long i = atomicAdd(tlog, 1ull);
-  if (i < 4096) { tlog[1 + 3 * i] = id; tlog[2 + 3 * i] = a; tlog[3 + 3 * i] = b; }
-}
-#endif
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;

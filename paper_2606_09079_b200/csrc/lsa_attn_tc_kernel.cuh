@@ -5,12 +5,6 @@
 
 namespace lsa {
 
-#ifdef LSA_TC_TRACE
-// debug builds only (_work/): per-CTA, per-role clock64 stamps relative to kernel entry
-#define TR(role, slot) do { if ((slot) < 32) p.trace[((size_t)blockIdx.x * 3 + (role)) * 32 + (slot)] = clock64() - t_entry; } while (0)
-#else
-#define TR(role, slot) do { } while (0)
-#endif
 
 // Order of the K/V stage groups of a piece with tiles t0..t1-1, for the producer and the MMA issuer alike:
 //   K(t0) | K(t0+1) V(t0) | K(t0+2) V(t0+1) | ... | V(t1-1)
@@ -26,10 +20,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
   TcSmem& sm = *reinterpret_cast<TcSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int cta = blockIdx.x, n_cta = p.n_attn;    // CTAs that own tiles; gridDim.x may be larger (fused S8)
-#ifdef LSA_TC_TRACE
-  const long long t_entry = clock64();
-  const unsigned long long g_entry = gtime();
-#endif
 
   // ---- setup: mbarriers first (one cheap block barrier), everything slower overlaps behind `setup` ----
   if (tid == 0) {
@@ -101,18 +91,15 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
           mbar_wait(&sm.empty[st], ((ring / kTcStages) & 1) ^ 1, 11);
           mbar_arrive_expect_tx(&sm.full[st], kTcStageBytes);
           tma_load_3d(sm.stage[st], m, 0, row, s4 * 2, &sm.full[st]);
-          TR(0, 2 + ring);
           ++ring;
         }
       };
-      TR(0, 0);
       while (cur.next(b, t0, t1)) {
         const SeqView v = sm.view[b];
         TileSrc src = tile_src(p, &map_pool, v, t0);      // table look-up overlaps the Q issue
         if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 10);
         mbar_arrive_expect_tx(&sm.q_full, 65536);
         tma_load_3d(sm.q, &map_q, 0, b * kTcH, 0, &sm.q_full);
-        TR(0, 1);
         app_gate(v, t0);
         issue4(src.mk, src.row_k);
         for (int t = t0; t < t1; ++t) {
@@ -169,7 +156,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
           ++ring;
         }
         umma_commit(&sm.s_full[buf]);
-        TR(1, 1 + n_s * 3);
         if (last_of_piece) umma_commit(&sm.q_empty);
         ++n_s;
       };
@@ -178,7 +164,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       auto issue_pv = [&](bool first_of_piece, bool last_of_piece) {
         mbar_wait(&sm.p_full, n_pv & 1, 23);
         tc_fence_after();
-        TR(1, 2 + n_pv * 3);
         if (first_of_piece && item > 0) {                 // the previous piece's epilogue has drained O and L
           mbar_wait(&sm.o_empty, (item - 1) & 1, 24);
           tc_fence_after();
@@ -200,13 +185,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
           ++ring;
         }
         umma_commit(&sm.pv_done);
-        TR(1, 3 + n_pv * 3);
         ++n_pv;
       };
       while (cur.next(b, t0, t1)) {
         mbar_wait(&sm.q_full, item & 1, 20);
         tc_fence_after();
-        TR(1, 0);
         issue_s(t0 + 1 == t1);
         for (int t = t0; t < t1; ++t) {
           if (t + 1 < t1) issue_s(t + 2 == t1);
@@ -221,7 +204,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
     const int hh = (warp - 2) >> 2;                       // half of the heads owned by this warp
     const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
     const int key = q4 * 32 + lane;                       // key row of the tile owned by this thread
-    const bool tr = (tid == 64);
     mbar_wait(&sm.setup, 0, 29);
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
@@ -285,10 +267,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
           if (kMask) km_next = tile_keymask(p, v, t + 1, q4);
         }
         float x[32];
-        if (tr) TR(2, 0 + tcount * 5);
         mbar_wait(&sm.s_full[buf], (tcount >> 1) & 1, 30);
         tc_fence_after();
-        if (tr) TR(2, 1 + tcount * 5);
         tmem_ld32(tS + buf * 64 + hh * 32 + lane_addr, reinterpret_cast<uint32_t*>(x));
         tmem_wait_ld();
         tc_fence_before();
@@ -323,7 +303,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
             }
           }
         }
-        if (tr) TR(2, 2 + tcount * 5);
         // P^T values of this thread: 32 heads of one key, bf16 pairs (computed before waiting for the buffer)
         uint32_t pw[16];
 #pragma unroll
@@ -346,7 +325,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
           }
           tmem_wait_st();
         }
-        if (tr) TR(2, 3 + tcount * 5);
         // P^T tile: bf16 [128 keys][64 heads], 128-byte swizzle; this thread's 32 heads = 4 x 16 B
         {
           unsigned char* prow = sm.p + key * 128;
@@ -358,12 +336,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.p_full);
-        if (tr) TR(2, 4 + tcount * 5);
         ++tcount;
       }
       // ---- epilogue: O^T, L, m -> partial slot (cta + b) ----
       // layout [d-block m][head half][head quad g][d_local][4 heads]: one 16-byte store per (m, g), warp-contiguous
-      if (tr) TR(2, 20);
       const size_t slot = (size_t)cta + b;
       uint2* po = p.part_o + slot * (kTcH * kTcD / 4) + (size_t)hh * (8 * 128) + key;
 #pragma unroll 1
@@ -400,7 +376,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&sm.o_empty);
-      if (tr) TR(2, 21);
       ++piece;
     }
     if (tid == 64) p.piece_info[cta] = make_int2(b_first < 0 ? 0 : b_first, b_first < 0 ? 0 : b_last - b_first + 1);
@@ -408,19 +383,13 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
   // ---- teardown ----
   tc_fence_before();
   if (p.fused) {
-    if (tid == 0) TR(0, 27);
     grid_arrive_and_wait(p);                      // every partial of the launch is visible from here on
-    if (tid == 0) TR(0, 28);
     if (warp == 1) {
       tc_fence_after();
       tmem_dealloc(sm.tmem_base, 512);
     }
     if (cta == 0 && tid < p.B) commit_state(p, tid);  // every CTA has read the records (they are behind the barrier)
     if (warp >= 2) fused_combine(p, sm.q, cta, gridDim.x, tid - 64);
-    if (tid == 64) TR(0, 29);
-#ifdef LSA_TC_TRACE
-    __syncthreads();
-#endif
   } else {
     __syncthreads();
     if (warp == 1) {
@@ -428,11 +397,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_consta
       tmem_dealloc(sm.tmem_base, 512);
     }
   }
-  if (tid == 0) TR(0, 31);
   if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
-#ifdef LSA_TC_TRACE
-  if (tid == 0 && (cta == 0 || cta == gridDim.x - 1)) tlog_add(p.tlog, cta == 0 ? 1 : 2, g_entry);
-#endif
 }
 
 }  // namespace lsa

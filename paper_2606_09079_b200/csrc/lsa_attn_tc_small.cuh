@@ -73,6 +73,10 @@ struct SmParams {
   unsigned int* done_ctr;        // CTAs that have left, all launches of the workspace
   unsigned int done_need_buf;    // value it has reached once the launch that used this buffer last has been merged
   unsigned int done_need_prev;   // value it has reached once the previous launch has been merged
+  unsigned int done_after;       // its value once this launch's last CTA has left
+  unsigned int* host_flag;       // lsa_step_host: PINNED HOST word (mapped) that receives host_flag_val when the launch's
+  unsigned int host_flag_val;    // last CTA leaves, i.e. when `out` is complete - the host spins on it instead of
+                                 // synchronising the stream; null otherwise
   __nv_bfloat16* out;            // [B][H][D]
   float* lse;                    // [B][H] or null
   unsigned int swap;             // bit b: sequence b's staged table becomes current with this launch (records catch up here)
@@ -80,6 +84,8 @@ struct SmParams {
   const __nv_bfloat16* k_new;    // [B][D] or null
   const __nv_bfloat16* v_new;
   int wait_inputs;               // 1: griddepcontrol.wait before q / k_new / v_new are read
+  const unsigned int* in_ctr;    // lsa_step_host_async: q / k_new / v_new are staged by a gather kernel that runs beside the
+  unsigned int in_need;          // previous step; they are complete once this counter (its finished blocks) reaches in_need
   unsigned long long* ktime;     // profiling only, see TcParams
 };
 
@@ -475,6 +481,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
           k0_pending = false;
           if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 10);
           if (p.wait_inputs && !waited) { griddep_wait(); waited = true; }   // q is the caller's: whatever the stream ran last
+          if (p.in_ctr && !waited) { wait_counter(p.in_ctr, p.in_need, 55); fence_proxy_async_all(); waited = true; }
                                                     // after griddep_wait
           mbar_arrive_expect_tx(&sm.q_full, 65536);
           tma_load_3d(sm.q, &map_q, 0, s.b * kTcH, 0, &sm.q_full);
@@ -606,6 +613,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         const SmSeq& q = sm.seq[a.b];
         if (a.kind == 2 && q.app_slot >= a.row0 && q.app_slot < a.row0 + a.rows && t < 128) {
           if (p.wait_inputs && !waited) { griddep_wait(); waited = true; }   // k_new / v_new are the caller's
+          if (p.in_ctr && !waited) { wait_counter(p.in_ctr, p.in_need, 56); waited = true; }
           const SeqDev& sd = p.seqs[a.b];
           const uint4* src = reinterpret_cast<const uint4*>((t < 64 ? p.k_new : p.v_new) + (size_t)a.b * kTcD) + (t & 63);
           uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(t < 64 ? sd.win_k : sd.win_v) + (size_t)q.app_slot * kTcD) + (t & 63);
@@ -794,8 +802,19 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   }
   __syncthreads();
   if (tid == 0) {
-    __threadfence();
-    red_release_add_u32(p.done_ctr, 1u);
+    if (p.host_flag) {
+      // `out` may live in pinned host memory: this CTA's rows are visible system-wide before it is counted, and the
+      // CTA that completes the count tells the host
+      __threadfence_system();
+      const unsigned int old = atomicAdd(p.done_ctr, 1u);
+      if (old + 1u == p.done_after) {
+        __threadfence_system();
+        *reinterpret_cast<volatile unsigned int*>(p.host_flag) = p.host_flag_val;
+      }
+    } else {
+      __threadfence();
+      red_release_add_u32(p.done_ctr, 1u);
+    }
   }
   if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
 }

@@ -62,10 +62,8 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
         int n = 0;
         while (n < k && sm.sel.keys[n] != kKeyMax) ++n;
         sm.n_sel = n;
-        sm.tick = ++pool.counters[C_TICK];
-        sm.epoch = ++(*pool.epoch);
-        pool.counters[C_TRIGGERS] += 1;
-        sq.pending = 0;                 // a new selection supersedes an unswapped staged table
+        sm.tick = pool.counters[C_TICK] + 1;     // committed below, once the pass is known to succeed
+        sm.epoch = ++(*pool.epoch);              // scratch stamp of pin_mark: harmless if the pass is abandoned
       }
       __syncthreads();
       for (int i = tid; i < sm.n_sel; i += blockDim.x) sm.sel_up[i] = (int)sm.sel.keys[i];
@@ -80,7 +78,7 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
       int bb = idx / (2 * k), r = idx % (2 * k), buf = r / k, j = r % k;
       const SeqDev& o = seqs[bb];
       bool is_cur = (buf == o.cur_buf);
-      bool live = is_cur ? true : (o.pending != 0);
+      bool live = is_cur ? true : (o.pending != 0 && bb != b);   // this sequence's own unswapped staged table is superseded
       if (live && j < o.n_tbl[buf]) pool.pin_mark[pool.tbl_page[((size_t)bb * 2 + buf) * k + j]] = epoch;
     }
     __syncthreads();
@@ -91,7 +89,6 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
       int c = sm.sel_up[tid];
       int p = pool.page_of[sq.page_of_off + c];
       if (p >= 0) {
-        pool.last_used[p] = tick;
         pool.pin_mark[p] = epoch;
         sm.next_page[tid] = p;
       } else {
@@ -123,20 +120,26 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
     // Pages never return to the never-used state and never-used pages (last_used = 0) sort first, lowest index
     // first, so the used pages are always the prefix [0, n_used) with n_used = misses - evictions so far.  While
     // enough never-used pages are left, the victims are simply the next n_miss indices (no scan of the pool).
+    bool fast = true;
+    long long n_used = 0;
     if (n_miss > 0) {
-      const long long n_used = (long long)(pool.counters[C_MISSES] - pool.counters[C_EVICTIONS]);
-      const bool fast = n_used + n_miss <= (long long)P;
+      n_used = (long long)(pool.counters[C_MISSES] - pool.counters[C_EVICTIONS]);
+      fast = n_used + n_miss <= (long long)P;
       if (!fast) {
         const unsigned long long* lu = pool.last_used;
         const unsigned int* pm = pool.pin_mark;
         auto keyf = [lu, pm, epoch](int p) -> unsigned long long {
           return pm[p] == epoch ? kKeyMax : ((lu[p] << kPageBits) | (unsigned long long)p);
         };
-        int got = block_select_smallest(keyf, P, n_miss, sm.sel);
+        // pools of up to 4096 pages: histogram select + sort of the victims only (the full sort took ~20 us per sequence)
+        int got = (P <= 4096 && blockDim.x == 1024) ? block_select_smallest_hist(keyf, P, n_miss, sm.sel)
+                                                    : block_select_smallest(keyf, P, n_miss, sm.sel);
         __syncthreads();
         bool bad = (got < n_miss) || (sm.sel.keys[n_miss - 1] == kKeyMax);
         if (bad) {
-          if (tid == 0) pool.counters[C_ERROR] = 1;   // pool exhausted: leave state untouched
+          // pool exhausted: nothing has been changed yet (pin_mark / epoch are scratch) - tables, residency, LRU
+          // stamps and counters stay as they were; lsa_sync / lsa_get_stats report the error
+          if (tid == 0) pool.counters[C_ERROR] = 1;
           __syncthreads();
           continue;
         }
@@ -162,7 +165,12 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
     }
     __syncthreads();
 
-    // ---- stage the next table (ascending chunk id) ----
+    // ---- the pass succeeds: commit the tick, the hits' LRU stamps, and stage the next table (ascending chunk id) ----
+    if (tid < n_sel && sm.miss_rank[tid] < 0) pool.last_used[sm.next_page[tid]] = tick;
+    if (tid == 0) {
+      pool.counters[C_TICK] = tick;
+      pool.counters[C_TRIGGERS] += 1;
+    }
     const int buf = 1 - sq.cur_buf;
     if (tid < n_sel) {
       pool.tbl_chunk[((size_t)b * 2 + buf) * k + tid] = sm.sel_up[tid];

@@ -226,4 +226,87 @@ __device__ inline int block_topk_select(const float* __restrict__ sc, int n, int
   return got;
 }
 
+// ---- the m smallest of n <= 4096 UNIQUE 64-bit keys (S4: LRU victims), same scheme ---------------------------------
+// Keys live in registers (4 per thread); 12-bit radix levels from the highest bit any key has set (kKeyMax =
+// "excluded" is ignored) down, until the cut-off bin is taken whole - unique keys always end there.  The winners are
+// compacted and sorted.  Returns the number written to sm.keys (< m if fewer than m keys are not excluded).
+template <class KeyF>
+__device__ inline int block_select_smallest_hist(KeyF keyf, int n, int m, SelectSmem& sm) {
+  if (m > n) m = n;
+  if (m <= 0) return 0;
+  unsigned int* hist = reinterpret_cast<unsigned int*>(sm.keys + 1024);
+  unsigned int* wsum = sm.hist;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  unsigned long long u[4];
+  bool have[4];
+  unsigned long long any = 0;
+  unsigned cnt = 0;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int c = tid + 1024 * j;
+    u[j] = c < n ? keyf(c) : kKeyMax;
+    have[j] = u[j] != kKeyMax;
+    if (have[j]) { any |= u[j]; ++cnt; }
+  }
+  // highest set bit over all keys, and how many keys there are
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { any |= __shfl_xor_sync(0xffffffffu, any, o); cnt += __shfl_xor_sync(0xffffffffu, cnt, o); }
+  if (lane == 0) { sm.keys[warp] = any; wsum[warp] = cnt; }
+  __syncthreads();
+  any = 0; cnt = 0;
+  for (int w = 0; w < 32; ++w) { any |= sm.keys[w]; cnt += wsum[w]; }
+  __syncthreads();
+  if ((unsigned)m > cnt) m = (int)cnt;
+  if (m == 0) return 0;
+  int top = 64 - __clzll((long long)(any | 1ull));           // bits in use
+  unsigned long long prefix = 0, mask = 0;
+  unsigned need = (unsigned)m, in_bin = 0;
+#pragma unroll 1
+  for (int shift = ((top + 11) / 12 - 1) * 12; shift >= 0; shift -= 12) {
+    for (int i = tid; i < kTopkBins; i += 1024) hist[i] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (have[j] && (u[j] & mask) == prefix) atomicAdd(&hist[(unsigned)(u[j] >> shift) & (kTopkBins - 1)], 1u);
+    __syncthreads();
+    // prefix counts: thread t owns bins [4t, 4t + 4); below(b) = keys in bins < b
+    const unsigned h0 = hist[4 * tid], h1 = hist[4 * tid + 1], h2 = hist[4 * tid + 2], h3 = hist[4 * tid + 3];
+    const unsigned mine = h0 + h1 + h2 + h3;
+    unsigned incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    unsigned below_w = 0;
+    for (int w = 0; w < warp; ++w) below_w += wsum[w];
+    const unsigned b0 = below_w + incl - mine, b1 = b0 + h0, b2 = b1 + h1, b3 = b2 + h2;
+    if (b0 < need && need <= b0 + h0) { wsum[64] = 4 * tid; wsum[65] = need - b0; wsum[66] = h0; }
+    else if (b1 < need && need <= b1 + h1) { wsum[64] = 4 * tid + 1; wsum[65] = need - b1; wsum[66] = h1; }
+    else if (b2 < need && need <= b2 + h2) { wsum[64] = 4 * tid + 2; wsum[65] = need - b2; wsum[66] = h2; }
+    else if (b3 < need && need <= b3 + h3) { wsum[64] = 4 * tid + 3; wsum[65] = need - b3; wsum[66] = h3; }
+    __syncthreads();
+    prefix |= (unsigned long long)wsum[64] << shift;
+    mask |= (unsigned long long)(kTopkBins - 1) << shift;
+    need = wsum[65];
+    in_bin = wsum[66];
+    __syncthreads();
+    if (in_bin == need) break;
+  }
+  if (tid == 0) sm.count = 0;
+  __syncthreads();
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+    if (have[j] && (u[j] & mask) <= prefix) sm.keys[atomicAdd(&sm.count, 1u)] = u[j];
+  __syncthreads();
+  const int got = (int)sm.count;
+  const int n_pad = next_pow2(got);
+  for (int i = got + tid; i < n_pad; i += 1024) sm.keys[i] = kKeyMax;
+  __syncthreads();
+  block_bitonic_sort(sm.keys, n_pad);
+  return got;
+}
+
 }  // namespace lsa

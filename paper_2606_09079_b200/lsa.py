@@ -29,7 +29,7 @@ STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_E
           -4: "LSA_ERR_OOM", -5: "LSA_ERR_STATE", -6: "LSA_ERR_UNSUPPORTED"}
 
 EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit_tables",
-           "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_set_chunk_emb",
+           "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_step_host_async", "lsa_host_wait", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
            "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats", "lsa_export_chunks",
@@ -91,6 +91,8 @@ def _load() -> C.CDLL:
     lib.lsa_decode_attention.argtypes = [vp, vp, vp, f32p]
     lib.lsa_step.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.lsa_step_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.lsa_step_host_async.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(C.c_uint64)]
+    lib.lsa_host_wait.argtypes = [vp, C.c_uint64]
     lib.lsa_set_chunk_emb.argtypes = [vp, C.c_int32, vp]
     lib.lsa_get_page_table.argtypes = [vp, C.c_int32, C.c_int32, i32p, i32p, i32p]
     lib.lsa_get_residency.argtypes = [vp, C.c_int32, i32p]
@@ -155,7 +157,18 @@ def _ids(seq_ids: Sequence[int]):
 
 
 class LsaContext:
-    """Owns one lsa_ctx.  See include/lsa.h for the meaning of every argument."""
+    """Owns one lsa_ctx.  See include/lsa.h for the meaning of every argument.
+
+    Stream contract (include/lsa.h "Conventions"): results are written on the library's streams - `out` / `lse` on
+    stream_compute, `sel_idx` / `sel_score` on stream_fetch - NOT on torch's current stream.  Tensors this wrapper
+    allocates for them are marked with record_stream(), so the caching allocator cannot hand their memory out again
+    while the library still writes it; a caller that reads them on another stream orders that stream behind the
+    library's (ctx.stream_compute / ctx.stream_fetch, or ctx.sync())."""
+
+    def _on(self, t, stream):
+        if t is not None:
+            t.record_stream(stream)
+        return t
 
     def __init__(self, *, dtype: int, H: int, D: int, C_: int, W: int, Dh: int, E: int, k: int, tau: int,
                  hot_pool: torch.Tensor, W_q: torch.Tensor, seqs: Sequence[dict], recall_lag: int = 1,
@@ -230,7 +243,7 @@ class LsaContext:
         sc = torch.empty((n, self.k), dtype=torch.float32, device=h.device) if want_scores else None
         self._check(_lib.lsa_index_select(self._h, _dev_ptr(h, self.tdtype, "h"), arr, n, sel.data_ptr(),
                                           None if sc is None else sc.data_ptr()))
-        return sel, sc
+        return self._on(sel, self.stream_fetch), self._on(sc, self.stream_fetch)
 
     def l1_init(self, layers: Sequence[dict], index_k: Sequence[Sequence[torch.Tensor]], d_c: int, c_I: int = 128,
                 n_h: int = 64, threshold: float = 0.5):
@@ -270,7 +283,7 @@ class LsaContext:
         sc = torch.empty((self.B, self.k2), dtype=torch.float32, device=q_idx.device) if want_entries else None
         self._check(_lib.lsa_l2_select(self._h, _dev_ptr(q_idx, self.tdtype, "q_idx"), _dev_ptr(w_idx, torch.float32, "w_idx"),
                                        None if sel is None else sel.data_ptr(), None if sc is None else sc.data_ptr()))
-        return sel, sc
+        return self._on(sel, self.stream_compute), self._on(sc, self.stream_compute)
 
     def l2_mask(self, seq: int):
         """Blocking: the row mask of the last Level-2 selection, as a bool array [k][C = 128]."""
@@ -281,7 +294,7 @@ class LsaContext:
         return bits.reshape(self.k, 128).astype(bool)
 
     def step_l2(self, q, h, k_new, v_new, q_idx, w_idx, out=None):
-        out = torch.empty_like(q) if out is None else out
+        out = self._on(torch.empty_like(q), self.stream_compute) if out is None else out
         self._check(_lib.lsa_step_l2(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(h, self.tdtype, "h"),
                                      _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
                                      _dev_ptr(q_idx, self.tdtype, "q_idx"), _dev_ptr(w_idx, torch.float32, "w_idx"),
@@ -297,7 +310,7 @@ class LsaContext:
         sc = torch.empty((n, self.k), dtype=torch.float32, device=h.device) if want_scores else None
         self._check(_lib.lsa_l1_select(self._h, _dev_ptr(h, self.tdtype, "h"), arr, n, sel.data_ptr(),
                                        None if sc is None else sc.data_ptr()))
-        return sel, sc
+        return self._on(sel, self.stream_fetch), self._on(sc, self.stream_fetch)
 
     def fetch_chunks(self, seq_ids: Sequence[int], sel_idx: torch.Tensor):
         arr, n = _ids(seq_ids)
@@ -307,14 +320,14 @@ class LsaContext:
         self._check(_lib.lsa_commit_tables(self._h))
 
     def decode_attention(self, q: torch.Tensor, out: Optional[torch.Tensor] = None, want_lse: bool = False):
-        out = torch.empty_like(q) if out is None else out
-        lse = torch.empty((self.B, self.H), dtype=torch.float32, device=q.device) if want_lse else None
+        out = self._on(torch.empty_like(q), self.stream_compute) if out is None else out
+        lse = self._on(torch.empty((self.B, self.H), dtype=torch.float32, device=q.device), self.stream_compute) if want_lse else None
         self._check(_lib.lsa_decode_attention(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(out, self.tdtype, "out"),
                                               None if lse is None else lse.data_ptr()))
         return (out, lse) if want_lse else out
 
     def step(self, q, h, k_new=None, v_new=None, out=None):
-        out = torch.empty_like(q) if out is None else out
+        out = self._on(torch.empty_like(q), self.stream_compute) if out is None else out
         self._check(_lib.lsa_step(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(h, self.tdtype, "h"),
                                   _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
                                   _dev_ptr(out, self.tdtype, "out")))
@@ -326,7 +339,7 @@ class LsaContext:
 
     def step_graph(self, q, h, k_new=None, v_new=None, out=None):
         """lsa_step with the non-trigger step replayed from a CUDA graph (keep q / k_new / v_new / out at fixed addresses)."""
-        out = torch.empty_like(q) if out is None else out
+        out = self._on(torch.empty_like(q), self.stream_compute) if out is None else out
         self._check(_lib.lsa_step_graph(self._h, _dev_ptr(q, self.tdtype, "q"), _dev_ptr(h, self.tdtype, "h"),
                                         _dev_ptr(k_new, self.tdtype, "k_new"), _dev_ptr(v_new, self.tdtype, "v_new"),
                                         _dev_ptr(out, self.tdtype, "out")))
@@ -342,6 +355,17 @@ class LsaContext:
                                        _host_ptr(k_new, self.tdtype, "k_new"), _host_ptr(v_new, self.tdtype, "v_new"),
                                        _host_ptr(out, self.tdtype, "out")))
         return out
+
+    def step_host_async(self, q, h, k_new, v_new, out) -> int:
+        """lsa_step_host without the wait; returns the ticket for host_wait (buffers must stay untouched until then)."""
+        t = C.c_uint64(0)
+        self._check(_lib.lsa_step_host_async(self._h, _host_ptr(q, self.tdtype, "q"), _host_ptr(h, self.tdtype, "h"),
+                                             _host_ptr(k_new, self.tdtype, "k_new"), _host_ptr(v_new, self.tdtype, "v_new"),
+                                             _host_ptr(out, self.tdtype, "out"), C.byref(t)))
+        return t.value
+
+    def host_wait(self, ticket: int):
+        self._check(_lib.lsa_host_wait(self._h, ticket))
 
     # -- support -----------------------------------------------------------------------------
     def set_chunk_emb(self, seq: int, emb: torch.Tensor):

@@ -436,6 +436,39 @@ def test_step_host_equals_step(pinned_out):
     a.ctx.close(); b_.ctx.close()
 
 
+def test_step_host_async_tickets_equal_step():
+    """lsa_step_host_async (step_overlap = 1): several steps in flight, each with pinned inputs and a pinned output of its own,
+    tickets waited for out of lock-step with the calls; outputs, page tables and counters must equal those of lsa_step on a
+    second context fed the same inputs.  Trigger and swap steps are part of the run."""
+    cfg = make_config(2, B=2, L=[16384 + 4 * 37, 8192], W=1024, k=6, hot_pages=32, steps=44, name="cfg2_host_async", q_gain=16.0, tau=8)
+    wl = LsaWorkload(cfg)
+    a, b_ = GpuRig(wl, step_overlap=1), GpuRig(wl, step_overlap=1)
+    pinh = lambda x: to_torch(x, cfg.dtype).pin_memory()
+    ins = [(pinh(wl.q(t)), pinh(wl.h(t)), pinh(wl.kv_new(t)[0]), pinh(wl.kv_new(t)[1])) for t in range(cfg.steps)]
+    outs = [torch.empty((cfg.B, cfg.H, cfg.D), dtype=torch.bfloat16).pin_memory() for _ in range(cfg.steps)]
+    refs, tickets = [], []
+    for t in range(cfg.steps):
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t)
+        refs.append(a.ctx.step(a.dev(q), a.dev(h), a.dev(kn), a.dev(vn)))
+        tickets.append(b_.ctx.step_host_async(ins[t][0], ins[t][1], ins[t][2], ins[t][3], outs[t]))
+        assert tickets[-1] > 0, "the overlapped path must hand out real tickets"
+        if t >= 5 and t % 3 == 0:                       # wait for an older step while newer ones are in flight
+            b_.ctx.host_wait(tickets[t - 5])
+            a.ctx.sync()
+            assert torch.equal(refs[t - 5].cpu(), outs[t - 5]), f"step {t - 5}"
+    for t in range(cfg.steps):
+        b_.ctx.host_wait(tickets[t])
+    a.ctx.sync()
+    for t in range(cfg.steps):
+        assert torch.equal(refs[t].cpu(), outs[t]), f"step {t}"
+    for s_ in range(cfg.B):
+        assert a.ctx.page_table(s_) == b_.ctx.page_table(s_)
+    sa, sb = a.ctx.stats(), b_.ctx.stats()
+    assert (sa["hits"], sa["misses"], sa["bytes_fetched"]) == (sb["hits"], sb["misses"], sb["bytes_fetched"])
+    a.ctx.close(); b_.ctx.close()
+
+
 def test_recall_lag_deeper_than_one_step_flagship_shape_and_bounds():
     """recall_lag in 2..tau-1 (a longer fetch hides behind more steps; default stays the paper's t+1): lock-step on
     the tcgen05 path - the swap then rides on the attention launch lag steps after the trigger - and the init bound."""
