@@ -56,6 +56,7 @@ struct lsa_ctx {
   unsigned int host_flag_seq = 0;
   bool host_flag_armed = false;        // the launch just enqueued will write host_flag_seq to the flag
   bool next_alone = false;             // the caller will block on the step being enqueued
+  int qtower_tc = 1;                   // S1 on tensor cores when 8..16 sequences fire together
   unsigned int* gather_ctr = nullptr;  // DEVICE: finished blocks of the gather kernels of lsa_step_host_async
   unsigned int gather_total = 0;       // as enqueued
   bool inputs_by_counter = false;      // the next attention launch waits for gather_total instead of for the stream
@@ -260,7 +261,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   if ((rc = dev_alloc(c, &c->pool.counters, 8))) return rc;
   if ((rc = dev_alloc(c, &c->pool.epoch, 1))) return rc;
   // ---- index scratch ----
-  if ((rc = dev_alloc(c, &c->d_z, (size_t)B * cfg->E))) return rc;
+  if ((rc = dev_alloc(c, &c->d_z, (size_t)std::max(B, 16 * std::max(1, cfg->Dh / 512)) * cfg->E))) return rc;   // or [Dh/512][16][E] partials
   if ((rc = dev_alloc(c, &c->d_scores, (size_t)B * std::max(c->n_chunks_max, 1)))) return rc;
   if ((rc = dev_alloc(c, &c->d_sel, (size_t)B * k))) return rc;
 
@@ -339,17 +340,28 @@ extern "C" int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs, l
 static int index_select_impl(lsa_ctx* c, const void* h, const int* ids, const int* rows, int n, int32_t* sel_idx,
                              float* sel_score) {
   const lsa_config& cfg = c->cfg;
-  for (int off = 0; off < n; off += kFireMax) {
-    const int m = std::min(kFireMax, n - off);
+  for (int off = 0; off < n;) {
+    // 8..16 sequences firing together with consecutive rows of h: the projection is a GEMM on tensor cores
+    int m = std::min(kFireMax, n - off);
+    const int m_tc = std::min(16, n - off);
+    const bool tc = c->qtower_tc != 0 && qtower_tc_usable(cfg.dtype, cfg.E, cfg.Dh, m_tc, rows + off);
+    if (tc) m = m_tc;
     FireList fire{}, hrows{};
     fire.n = hrows.n = m;
     for (int i = 0; i < m; ++i) { fire.ids[i] = ids[off + i]; hrows.ids[i] = rows[off + i]; }
     ProfScope prof(c, LSA_PH_INDEX, c->sf);
-    LSA_CUDA(c, launch_qtower(cfg.dtype, cfg.W_q, h, hrows, c->d_z, cfg.E, cfg.Dh, c->sf));
-    LSA_CUDA(c, launch_scores(cfg.dtype, c->d_seqs, fire, c->d_z, c->d_scores, cfg.E, std::max(c->n_chunks_max, 1), c->sf));
+    if (tc) {
+      LSA_CUDA(c, launch_qtower_tc(cfg.W_q, h, rows[off], m, c->d_z, cfg.E, cfg.Dh, c->sf));
+      LSA_CUDA(c, launch_scores(cfg.dtype, c->d_seqs, fire, c->d_z, c->d_scores, cfg.E, std::max(c->n_chunks_max, 1), c->sf,
+                                qtower_tc_splits(cfg.Dh)));
+    } else {
+      LSA_CUDA(c, launch_qtower(cfg.dtype, cfg.W_q, h, hrows, c->d_z, cfg.E, cfg.Dh, c->sf));
+      LSA_CUDA(c, launch_scores(cfg.dtype, c->d_seqs, fire, c->d_z, c->d_scores, cfg.E, std::max(c->n_chunks_max, 1), c->sf));
+    }
     LSA_CUDA(c, launch_topk(c->d_seqs, fire, c->d_scores, std::max(c->n_chunks_max, 1), c->k,
                             sel_idx + (size_t)off * c->k, sel_score ? sel_score + (size_t)off * c->k : nullptr, c->sf));
     c->index_launches += 3;
+    off += m;
   }
   return LSA_OK;
 }

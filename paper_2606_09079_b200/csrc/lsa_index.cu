@@ -71,7 +71,7 @@ constexpr int kScWarps = 8;
 template <typename T>
 __global__ void __launch_bounds__(kScWarps * 32)
 score_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __restrict__ z,
-             float* __restrict__ scores, int E, int n_chunks_max) {
+             float* __restrict__ scores, int E, int n_chunks_max, int n_part) {
   extern __shared__ float zs[];           // [E]
   __shared__ float red[kScWarps];
   __shared__ float inv_norm_s;
@@ -85,7 +85,10 @@ score_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __rest
   if (c0 >= sq.n_chunks) return;
   float ss = 0.f;
   for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    // z arrives as n_part partial sums over slices of Dh (the batched tensor-core tower, lsa_index_tc.cu), added here in
+    // a fixed order; n_part = 1: the GEMV's complete sums
     float v = z[(size_t)i * E + e];
+    for (int pz = 1; pz < n_part; ++pz) v += z[((size_t)pz * fire.n + i) * E + e];
     zs[e] = v;
     ss = fmaf(v, v, ss);
   }
@@ -149,12 +152,12 @@ cudaError_t launch_qtower(int dtype, const void* W, const void* h, const FireLis
 }
 
 cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, const float* z, float* scores,
-                          int E, int n_chunks_max, cudaStream_t st) {
+                          int E, int n_chunks_max, cudaStream_t st, int n_part) {
   dim3 grid((n_chunks_max + kScWarps - 1) / kScWarps, fire.n);
   size_t smem = (size_t)E * sizeof(float);
   if (dtype == 0)
-    return launch_pdl(score_kernel<float>, grid, dim3(kScWarps * 32), smem, st, seqs, fire, z, scores, E, n_chunks_max);
-  return launch_pdl(score_kernel<__nv_bfloat16>, grid, dim3(kScWarps * 32), smem, st, seqs, fire, z, scores, E, n_chunks_max);
+    return launch_pdl(score_kernel<float>, grid, dim3(kScWarps * 32), smem, st, seqs, fire, z, scores, E, n_chunks_max, n_part);
+  return launch_pdl(score_kernel<__nv_bfloat16>, grid, dim3(kScWarps * 32), smem, st, seqs, fire, z, scores, E, n_chunks_max, n_part);
 }
 
 cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores, int n_chunks_max, int k,

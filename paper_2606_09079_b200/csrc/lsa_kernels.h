@@ -17,8 +17,13 @@ struct AttnGeom {          // host-computed split geometry of one S7 launch
 cudaError_t launch_qtower(int dtype, const void* W, const void* h, const FireList& rows, float* z, int E,
                           int Dh, cudaStream_t st);
 // scores[i][c] = (z_i . Emb_{b_i}[c]) / max(||z_i||, 1e-12)
+// (z may be n_part partial sums [n_part][fire.n][E], added in order)
 cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, const float* z,
-                          float* scores, int E, int n_chunks_max, cudaStream_t st);
+                          float* scores, int E, int n_chunks_max, cudaStream_t st, int n_part = 1);
+// S1 for 8..16 sequences firing together, bf16, on tensor cores (lsa_index_tc.cu): z_part [Dh / 512][n][E]
+bool qtower_tc_usable(int dtype, int E, int Dh, int n, const int* hrows);
+int qtower_tc_splits(int Dh);
+cudaError_t launch_qtower_tc(const void* W, const void* h, int h_row0, int n, float* z_part, int E, int Dh, cudaStream_t st);
 // sel_idx[i][0..k) / sel_score: first k_eff by (score desc, chunk idx asc), rest -1 / -inf
 cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores,
                         int n_chunks_max, int k, int32_t* sel_idx, float* sel_score, cudaStream_t st);

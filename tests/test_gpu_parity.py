@@ -24,6 +24,32 @@ def _lsa():
 
 
 # ------------------------------------------------------------------------------- S1-S3
+@pytest.mark.parametrize("n_fire", [1, 3, 8, 11, 16, 20])
+def test_index_select_batched_tower_on_tensor_cores(n_fire):
+    """S1 for 8..16 sequences firing together is one tcgen05 GEMM (lsa_index_tc.cu: W_q streamed once, the sequences on N,
+    partial sums over slices of Dh added in a fixed order by the scoring kernel); fewer sequences, or a batch of 20 (16 + 4),
+    take the GEMV.  Scores element by element and the selection against the oracle at the BASELINE shape Dh = 4096, E = 512;
+    the 8 sequences of a batched call must also get exactly the chunks they get when they fire alone."""
+    cfg = make_small_config("bf16", B=20, L=[4096 + 512 * b for b in range(20)], C=16, H=8, D=64, E=512, Dh=4096, k=12, hot_pages=600, W=64)
+    wl = LsaWorkload(cfg)
+    rig = GpuRig(wl)
+    h = wl.h(0)
+    ids = list(range(n_fire))
+    sel, sc = rig.ctx.index_select(rig.dev(h[:n_fire]), ids)
+    rig.ctx.sync()
+    sel, sc = sel.cpu().numpy(), sc.cpu().numpy().astype(np.float64)
+    for i, b in enumerate(ids):
+        ref = chunk_scores(query_tower(wl.W_q, h[b]), wl.chunk_emb(b, 0))
+        assert validate_selection(sel[i], ref, cfg.k) is None
+        np.testing.assert_allclose(sc[i][sel[i] >= 0], ref[sel[i][sel[i] >= 0]], atol=2e-6)
+    if n_fire >= 8:
+        for b in (0, n_fire - 1):
+            alone, _ = rig.ctx.index_select(rig.dev(h[b:b + 1]), [b])
+            rig.ctx.sync()
+            assert np.array_equal(alone.cpu().numpy()[0], sel[b])
+    rig.ctx.close()
+
+
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 def test_index_select_matches_oracle_order(dtype):
     cfg = make_small_config(dtype, B=3, L=[65536, 32768, 1024], C=16, E=128, Dh=512, k=24, hot_pages=256)
