@@ -58,9 +58,15 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
       }
       __syncthreads();
       block_bitonic_sort(sm.sel.keys, n_pad);
+      // valid ids sort first: their number = keys that are not the sentinel (one block-wide count, not a serial scan)
+      int mine = 0;
+      for (int i = tid; i < k; i += blockDim.x) mine += sm.sel.keys[i] != kKeyMax;
+      mine = __reduce_add_sync(0xffffffffu, mine);
+      if (lane == 0) sm.warp_cnt[warp] = mine;
+      __syncthreads();
       if (tid == 0) {
         int n = 0;
-        while (n < k && sm.sel.keys[n] != kKeyMax) ++n;
+        for (int w = 0; w < 32; ++w) n += sm.warp_cnt[w];
         sm.n_sel = n;
         sm.tick = pool.counters[C_TICK] + 1;     // committed below, once the pass is known to succeed
         sm.epoch = ++(*pool.epoch);              // scratch stamp of pin_mark: harmless if the pass is abandoned
@@ -184,7 +190,6 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
       pool.counters[C_HITS] += n_sel - n_miss;
       pool.counters[C_BYTES] += (unsigned long long)n_miss * (unsigned long long)page_bytes;
     }
-    __threadfence();
     __syncthreads();
   }
 }
