@@ -333,6 +333,21 @@ class LsaContext:
                                   _dev_ptr(out, self.tdtype, "out")))
         return out
 
+    def bind_step(self, q, h, k_new, v_new, out):
+        """lsa_step on fixed buffers: the arguments are checked and converted once, the returned callable only makes the
+        C call (a decode loop that reuses its buffers pays the marshalling once instead of every step)."""
+        args = (self._h, C.c_void_p(_dev_ptr(q, self.tdtype, "q")), C.c_void_p(_dev_ptr(h, self.tdtype, "h")),
+                C.c_void_p(_dev_ptr(k_new, self.tdtype, "k_new")), C.c_void_p(_dev_ptr(v_new, self.tdtype, "v_new")),
+                C.c_void_p(_dev_ptr(out, self.tdtype, "out")))
+        keep = (q, h, k_new, v_new, out)
+        fn, check = _lib.lsa_step, self._check
+
+        def call(_keep=keep):
+            rc = fn(*args)
+            if rc:
+                check(rc)
+        return call
+
     def export_chunks(self, seq: int, first_chunk: int, src: torch.Tensor):
         """KV export (VRAM -> pinned cold pool): src = [n][2][C][D] CUDA tensor of page images for chunks first_chunk.."""
         self._check(_lib.lsa_export_chunks(self._h, seq, first_chunk, int(src.shape[0]), _dev_ptr(src, self.tdtype, "src")))

@@ -510,3 +510,61 @@ class L2Inputs:
         c = self.cfg
         g = _rng(c.seed, self.tag, 3, step)
         return ((0.5 + g.standard_normal((c.B, self.n_h))) / self.n_h).astype(np.float32)
+
+
+# --------------------------------------------------------------------------------------
+# NEXT-4 second half: the compressed history grows during decode ("all actively
+# decoded tokens' CSA chunks" are an always-resident tier).  Inputs only: the entries a model's
+# CSA / HCA compressors would hand over, and the embedding row of every chunk they complete.
+# --------------------------------------------------------------------------------------
+class GrowthInputs:
+    """Seeded stand-ins for what DeepSeek-V4's compressors emit while decoding (they need the model):
+
+    * before decode step t (t > 0, t % csa_every == 0) one CSA entry (K row, V row) per sequence - csa_every = 4 is the
+      paper's "4:1" reading (R4); * before step t (t > 0, t % hca_every == 0) one HCA entry - 128:1 (P:31);
+    * when an entry completes a chunk, that chunk's embedding row: a random unit row, or (with probability `hot_frac`) a
+      row planted at cosine `needle_cos` with the sequence's query direction, so that some completed chunks are recalled
+      again later and their exported cold copy is really read.
+    Capacities are what the caller must allocate: `cap_csa(b)` entries, `cap_hca(b)` rows."""
+
+    def __init__(self, wl: "LsaWorkload", steps: int, csa_every: int = 4, hca_every: int = 128, hot_frac: float = 0.5,
+                 tag: int = 1300):
+        self.wl, self.steps, self.csa_every, self.hca_every, self.hot_frac, self.tag = wl, steps, csa_every, hca_every, hot_frac, tag
+
+    def cap_csa(self, b: int) -> int:
+        c = self.wl.cfg
+        n = c.n_csa(b) + self.steps // self.csa_every + 1
+        return -(-n // c.C) * c.C                      # whole chunks: the cold pool is allocated in pages
+
+    def cap_hca(self, b: int) -> int:
+        return self.wl.cfg.n_hca(b) + self.steps // self.hca_every + 1
+
+    def csa_due(self, step: int) -> bool:
+        return step > 0 and step % self.csa_every == 0
+
+    def hca_due(self, step: int) -> bool:
+        return step > 0 and step % self.hca_every == 0
+
+    def csa_entry(self, step: int) -> Tuple[np.ndarray, np.ndarray]:
+        """(K [B, D], V [B, D]) stored dtype: the entry handed over before decode step `step`."""
+        c = self.wl.cfg
+        g = _rng(c.seed, self.tag, 1, step)
+        s = 1.0 / math.sqrt(c.D)
+        return _randn_stored(g, (c.B, c.D), s, c.dtype), _randn_stored(g, (c.B, c.D), s, c.dtype)
+
+    def hca_entry(self, step: int) -> Tuple[np.ndarray, np.ndarray]:
+        c = self.wl.cfg
+        g = _rng(c.seed, self.tag, 2, step)
+        s = 1.0 / math.sqrt(c.D)
+        return _randn_stored(g, (c.B, c.D), s, c.dtype), _randn_stored(g, (c.B, c.D), s, c.dtype)
+
+    def emb_row(self, b: int, chunk: int) -> np.ndarray:
+        """Embedding row [E] (stored dtype) of the chunk with id `chunk` of sequence b, handed over when it completes."""
+        c = self.wl.cfg
+        g = _rng(c.seed, self.tag, 3, b + c.seq_offset, chunk)
+        r = g.standard_normal((1, c.E))
+        if g.uniform() < self.hot_frac:
+            row = LsaWorkload._plant(self.wl.u[b], r, np.full(1, c.needle_cos))
+        else:
+            row = _unit_rows(r)
+        return store(row[0].astype(np.float32), c.dtype)

@@ -22,6 +22,59 @@ def make_oracle(wl: LsaWorkload, trigger_idx: int = 0, **over) -> LsaOracle:
     return LsaOracle(**kw)
 
 
+def growth_arrays(wl: LsaWorkload, gi):
+    """Capacity-sized copies of the workload's arrays for a run whose compressed history grows (NEXT-4): the cold pool,
+    the embedding table and the HCA arrays with room for what `gi` (workloads.GrowthInputs) will hand over."""
+    c = wl.cfg
+    cold, emb, hk, hv = [], [], [], []
+    for b in range(c.B):
+        cap_ch = gi.cap_csa(b) // c.C
+        x = np.zeros((cap_ch,) + wl.cold_csa[b].shape[1:], dtype=wl.cold_csa[b].dtype)
+        x[: c.n_chunks(b)] = wl.cold_csa[b]
+        cold.append(x)
+        e0 = wl.chunk_emb(b, 0)
+        e = np.zeros((cap_ch, c.E), dtype=e0.dtype)
+        e[: c.n_chunks(b)] = e0
+        emb.append(e)
+        for src, dst in ((wl.hca_k[b], hk), (wl.hca_v[b], hv)):
+            y = np.zeros((gi.cap_hca(b), c.D), dtype=src.dtype)
+            y[: c.n_hca(b)] = src
+            dst.append(y)
+    return cold, emb, hk, hv
+
+
+def make_growing_oracle(wl: LsaWorkload, gi, **over):
+    from oracle.growth_oracle import GrowingLsaOracle
+    c = wl.cfg
+    cold, emb, hk, hv = growth_arrays(wl, gi)
+    kw = dict(
+        dtype=c.dtype, H=c.H, D=c.D, C=c.C, W=c.W, k=c.k, tau=c.tau, recall_lag=c.recall_lag,
+        hot_pages=c.hot_pages, W_q=wl.W_q, cold_csa=cold, n_csa=[c.n_csa(b) for b in range(c.B)],
+        n_hca=[c.n_hca(b) for b in range(c.B)], chunk_emb=emb, hca_k=hk, hca_v=hv, win_k=wl.win_k, win_v=wl.win_v,
+        w_len=[min(c.W, c.L[b]) for b in range(c.B)], w_head=[min(c.W, c.L[b]) % c.W for b in range(c.B)],
+        step0=[c.step0(b) for b in range(c.B)])
+    kw.update(over)
+    return GrowingLsaOracle(**kw)
+
+
+def oracle_appends(orc, gi, t: int):
+    """Hand the entries due before decode step t to the oracle (R29).  Returns [(b, chunk)] completed by them."""
+    c = orc
+    done = []
+    hca = gi.hca_entry(t) if gi.hca_due(t) else None
+    csa = gi.csa_entry(t) if gi.csa_due(t) else None
+    if hca is None and csa is None:
+        return done
+    for b in range(orc.B):
+        emb_row = None
+        if csa is not None and orc.n_csa[b] % orc.C == orc.C - 1:
+            emb_row = gi.emb_row(b, orc.n_csa[b] // orc.C)
+        if orc.append_compressed(b, None if csa is None else csa[0][b], None if csa is None else csa[1][b],
+                                 None if hca is None else hca[0][b], None if hca is None else hca[1][b], emb_row):
+            done.append((b, orc.n_chunks[b] - 1))
+    return done
+
+
 def apply_emb_updates(wl: LsaWorkload, oracle: LsaOracle, global_step: int, gpu_embs=None):
     """Needle drift (cfg 2-4): rewrite embedding rows before the trigger at `global_step`."""
     import torch
