@@ -39,7 +39,7 @@
 extern "C" {
 #endif
 
-#define LSA_VERSION 2
+#define LSA_VERSION 3
 
 typedef struct lsa_ctx lsa_ctx; /* opaque */
 
@@ -107,6 +107,12 @@ typedef struct lsa_seq_desc {
   int32_t w_len;         /* filled ring rows [0, w_len) are attended                            */
   int32_t w_head;        /* next ring slot to be written by lsa_step(k_new, v_new)              */
   int64_t step0;         /* initial decode-step counter (staggered triggers, R26)               */
+  /* NEXT-4 growth (lsa_append_compressed); 0 = the compressed history of this sequence is static.  When cap_csa > 0:
+   * cold_csa and chunk_emb hold ceil(cap_csa / C) chunks / rows (cold_csa writable), hca_k / hca_v hold cap_hca rows
+   * (writable; the library zeroes rows [n_hca, cap_hca) at init), cap_csa >= n_csa, cap_hca >= n_hca.  Either every
+   * sequence of a context grows or none does. */
+  int64_t cap_csa;
+  int64_t cap_hca;
 } lsa_seq_desc;
 
 typedef struct lsa_stats {
@@ -122,6 +128,9 @@ typedef struct lsa_stats {
   int32_t attn_impl;      /* implementation actually in use (lsa_attn_impl)                      */
   int32_t attn_ctas;      /* CTAs of the last S7 launch                                          */
   int32_t reserved;
+  uint64_t csa_appended;  /* CSA entries handed over by lsa_append_compressed (all sequences)    */
+  uint64_t hca_appended;  /* HCA entries handed over                                            */
+  uint64_t chunks_exported;/* chunks completed by an append and mirrored to the cold pool         */
 } lsa_stats;
 
 /* Create a context.  All pages start FREE, every chunk starts in the cold pool, the attended
@@ -280,6 +289,27 @@ int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, c
  * later trigger's fetch.  Meant for admission, before the chunks are first selected: a chunk that is already resident
  * keeps its old hot copy until it is evicted.  Enqueues and returns; bit-exact. */
 int lsa_export_chunks(lsa_ctx* ctx, int32_t seq, int32_t first_chunk, int32_t n_chunks, const void* src);
+
+/* NEXT-4 (second half; "all actively decoded tokens' CSA chunks" are an always-resident tier; P:179 VRAM -> DRAM;
+ * DESIGN.md R29-R33): hand over already-compressed entries of the tokens decoded since the last call - at most one CSA
+ * entry and one HCA entry per listed sequence - BEFORE the lsa_step that first attends them.  The compressors themselves
+ * belong to the model; the library takes their output, as it takes k_new / v_new.
+ *   seq_ids HOST [n] strictly ascending; csa_k / csa_v DEVICE [n][D] (both or neither); hca_k / hca_v DEVICE [n][D] (both
+ *   or neither); emb_rows DEVICE [n][E]: row i is read only if sequence seq_ids[i]'s CSA entry completes a chunk (it is
+ *   that chunk's embedding, L2-normalised by the producer) - may be NULL when no listed sequence completes one.
+ * Effect per sequence, in stream order on stream_compute: the HCA entry becomes row n_hca of hca_k / hca_v (n_hca += 1);
+ * the CSA entry becomes row n_csa % C of the TAIL chunk n_csa / C, which lives in a reserved page of the hot pool (the last
+ * 2 B pages: page hot_pages - 2 B + 2 b + (chunk % 2); the LRU manages the pages before them) and is attended with its valid
+ * rows through an entry at the end of the page table (n_csa += 1).  When the entry completes the chunk: emb row -> chunk_emb,
+ * the page image is exported to the cold pool (stream_fetch), the chunk becomes a candidate of the indexer from the next
+ * trigger on, and it stays attended through the table until a table becomes current whose trigger saw it as a candidate;
+ * from then on it is attended iff recalled.  Two of the k table slots are the tier's: at most k - 2 chunks are recalled.
+ * Only the dual-encoder indexer supports growth (Level 1 / Level 2 contexts: LSA_ERR_UNSUPPORTED).
+ * Errors: INVALID_ARG (ids, null pairs, capacity exceeded, missing emb_rows at a completion), STATE (the context was not
+ * created with cap_csa > 0; or a third chunk would enter the tier before the oldest one left it - needs the table of a
+ * trigger that saw it, i.e. chunks must not complete faster than every tau + recall_lag steps).  Enqueues and returns. */
+int lsa_append_compressed(lsa_ctx* ctx, const int32_t* seq_ids, int32_t n, const void* csa_k, const void* csa_v,
+                          const void* hca_k, const void* hca_v, const void* emb_rows);
 
 /* Replace the embedding table pointer of one sequence (DEVICE [n_chunks][E]). */
 int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb);

@@ -96,6 +96,14 @@ struct lsa_ctx {
   int ktime_cap = 0;
   // bookkeeping
   unsigned long long n_steps = 0, attn_launches = 0, index_launches = 0;
+  // NEXT-4 growth (lsa_append_compressed; DESIGN R29-R33)
+  bool growth = false;
+  int k_sel = 0;                       // recalled chunks per table at most: k, or k - 2 when the context grows
+  int P_lru = 0;                       // pages the LRU manages: hot_pages, or hot_pages - 2 B
+  std::vector<long long> cap_csa;
+  std::vector<int> ncand_cur, ncand_nxt;   // candidates seen by the trigger of the current / the staged table (host mirror)
+  cudaEvent_t ev_roll = nullptr;       // fetch-stream position a roll (chunk completed / new tail) must wait for
+  unsigned long long csa_appended = 0, hca_appended = 0, chunks_exported = 0;
   int last_attn_ctas = 0;
   std::string err;
 };
@@ -164,6 +172,7 @@ extern "C" void lsa_destroy(lsa_ctx* ctx) {
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->ev_fetch) cudaEventDestroy(ctx->ev_fetch);
   if (ctx->ev_compute) cudaEventDestroy(ctx->ev_compute);
+  if (ctx->ev_roll) cudaEventDestroy(ctx->ev_roll);
   for (auto& v : ctx->prof_ev)
     for (cudaEvent_t e : v) cudaEventDestroy(e);
   delete ctx;
@@ -195,17 +204,32 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   c->n_tbl[0].assign(B, 0);
   c->n_tbl[1].assign(B, 0);
   c->app_count.assign(B, 0u);
+  c->growth = seqs[0].cap_csa > 0;
+  c->k_sel = c->growth ? k - 2 : k;
+  c->P_lru = (int)cfg->hot_pages - (c->growth ? 2 * B : 0);
+  c->cap_csa.assign(B, 0);
+  c->ncand_cur.assign(B, 0);
+  c->ncand_nxt.assign(B, 0);
+  if (c->growth && k < 3) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "a growing context needs k >= 3 (two table slots belong to the decode tier)");
+  if (c->growth) LSA_CUDA(c, cudaEventCreateWithFlags(&c->ev_roll, cudaEventDisableTiming));
   long long sum_k = 0, total_keys_max = 0, n_keys_max = 0;
   for (int b = 0; b < B; ++b) {
     const lsa_seq_desc& s = seqs[b];
+    if ((s.cap_csa > 0) != c->growth) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: either every sequence grows (cap_csa > 0) or none", b);
+    if (c->growth && (s.cap_csa < s.n_csa || s.cap_hca < s.n_hca || s.cap_hca > (1ll << 30)))
+      LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: cap_csa / cap_hca below n_csa / n_hca", b);
     if (s.n_csa < 0 || s.n_hca < 0 || s.w_len < 0 || s.w_len > cfg->W || s.w_head < 0 || s.w_head >= std::max(cfg->W, 1))
       LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: bad n_csa/n_hca/w_len/w_head", b);
-    const long long n_chunks = (s.n_csa + C - 1) / C;
-    if (n_chunks > 0 && (!s.cold_csa || !s.chunk_emb)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null cold_csa/chunk_emb", b);
+    // candidates of the indexer: every chunk (a partial last one included, R22); for a growing sequence the FULL chunks
+    // only - the partial one is the tail of the decode tier (R30).  cap_chunks: what the caller's arrays can hold.
+    const long long cap_chunks = c->growth ? (s.cap_csa + C - 1) / C : (s.n_csa + C - 1) / C;
+    const long long n_chunks = c->growth ? s.n_csa / C : cap_chunks;
+    c->cap_csa[b] = c->growth ? s.cap_csa : s.n_csa;
+    if (cap_chunks > 0 && (!s.cold_csa || !s.chunk_emb)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null cold_csa/chunk_emb", b);
     if (s.n_hca > 0 && (!s.hca_k || !s.hca_v)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null hca_k/hca_v", b);
     if (cfg->W > 0 && (!s.win_k || !s.win_v)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: null win_k/win_v", b);
     SeqDev d{};
-    if (n_chunks > 0) {
+    if (cap_chunks > 0) {
       cudaPointerAttributes at{};
       cudaError_t e = cudaPointerGetAttributes(&at, s.cold_csa);
       if (e != cudaSuccess || at.type != cudaMemoryTypeHost || !at.devicePointer) {
@@ -222,24 +246,27 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
     d.n_csa = s.n_csa;
     d.n_chunks = (int)n_chunks;
     d.n_hca = (int)s.n_hca;
-    d.k_eff = (int)std::min<long long>(k, n_chunks);
+    d.cap_hca = c->growth ? (int)s.cap_hca : (int)s.n_hca;
+    d.tier_page0 = c->growth ? c->P_lru + 2 * b : -1;
+    d.k_eff = (int)std::min<long long>(c->k_sel, n_chunks);
     d.page_of_off = c->total_chunks;
     d.w_len = s.w_len;
     d.w_head = s.w_head;
-    c->total_chunks += (int)n_chunks;
-    c->n_chunks_max = std::max(c->n_chunks_max, (int)n_chunks);
+    c->ncand_cur[b] = c->ncand_nxt[b] = (int)n_chunks;
+    c->total_chunks += (int)cap_chunks;
+    c->n_chunks_max = std::max(c->n_chunks_max, (int)cap_chunks);
     c->seq_host[b] = d;
     c->step[b] = s.step0;
     c->k_eff[b] = d.k_eff;
     c->w_head[b] = s.w_head;
-    sum_k += d.k_eff;
-    const long long nk = s.n_hca + (long long)d.k_eff * C + cfg->W;
+    sum_k += std::min<long long>(c->k_sel, cap_chunks);
+    const long long nk = d.cap_hca + (long long)(c->growth ? k : d.k_eff) * C + cfg->W;
     total_keys_max += nk;
     n_keys_max = std::max(n_keys_max, nk);
   }
-  if (cfg->hot_pages < 2 * sum_k)
-    LSA_FAIL(c, LSA_ERR_INVALID_ARG, "hot_pages=%lld < 2*sum_b min(k,n_chunks_b)=%lld (current + staged tables are pinned)",
-             (long long)cfg->hot_pages, 2 * sum_k);
+  if (c->P_lru < 2 * sum_k)
+    LSA_FAIL(c, LSA_ERR_INVALID_ARG, "hot_pages=%lld%s < 2*sum_b min(k,n_chunks_b)=%lld (current + staged tables are pinned)",
+             (long long)c->P_lru, c->growth ? " (after the 2 B pages of the decode tier)" : "", 2 * sum_k);
   if (cfg->hot_pages > (1ll << kPageBits)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "hot_pages > 2^%d", kPageBits);
 
   // ---- device state ----
@@ -260,6 +287,29 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   if ((rc = dev_alloc(c, &c->pool.fetch_page, (size_t)B * k))) return rc;
   if ((rc = dev_alloc(c, &c->pool.counters, 8))) return rc;
   if ((rc = dev_alloc(c, &c->pool.epoch, 1))) return rc;
+  if (c->growth) {
+    // decode tier (DESIGN R30, R32): HCA rows not in use yet must be finite (the tensor-core path multiplies them by
+    // P = 0); a partial last chunk of the prompt is the first tail chunk - its rows are copied from the cold pool into the
+    // sequence's reserved page and listed in the (otherwise empty) attended table
+    for (int b = 0; b < B; ++b) {
+      SeqDev& d = c->seq_host[b];
+      if (d.cap_hca > d.n_hca) {
+        const size_t off = (size_t)d.n_hca * D * c->elem, nb = (size_t)(d.cap_hca - d.n_hca) * D * c->elem;
+        LSA_CUDA(c, cudaMemset((char*)const_cast<void*>(d.hca_k) + off, 0, nb));
+        LSA_CUDA(c, cudaMemset((char*)const_cast<void*>(d.hca_v) + off, 0, nb));
+      }
+      if (d.n_csa % C) {
+        const int ch = (int)(d.n_csa / C), page = d.tier_page0 + (ch & 1);
+        LSA_CUDA(c, cudaMemcpy((char*)cfg->hot_pool + (long long)page * c->page_bytes,
+                               (const char*)seqs[b].cold_csa + (long long)ch * c->page_bytes, (size_t)c->page_bytes, cudaMemcpyHostToDevice));
+        LSA_CUDA(c, cudaMemcpy(c->pool.tbl_chunk + (size_t)b * 2 * k, &ch, sizeof(int), cudaMemcpyHostToDevice));
+        LSA_CUDA(c, cudaMemcpy(c->pool.tbl_page + (size_t)b * 2 * k, &page, sizeof(int), cudaMemcpyHostToDevice));
+        d.n_tbl[0] = 1;
+        c->n_tbl[0][b] = 1;
+      }
+    }
+    LSA_CUDA(c, cudaMemcpy(c->d_seqs, c->seq_host.data(), sizeof(SeqDev) * B, cudaMemcpyHostToDevice));
+  }
   // ---- index scratch ----
   if ((rc = dev_alloc(c, &c->d_z, (size_t)std::max(B, 16 * std::max(1, cfg->Dh / 512)) * cfg->E))) return rc;   // or [Dh/512][16][E] partials
   if ((rc = dev_alloc(c, &c->d_scores, (size_t)B * std::max(c->n_chunks_max, 1)))) return rc;
@@ -288,7 +338,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
     if ((rc = dev_alloc(c, &c->part_ml, (size_t)B * c->geom.s_max * H * 2, false))) return rc;
   } else {
     std::vector<long long> nk(B);
-    for (int b = 0; b < B; ++b) nk[b] = seqs[b].n_hca + (long long)c->k_eff[b] * C + cfg->W;
+    for (int b = 0; b < B; ++b) nk[b] = c->seq_host[b].cap_hca + (long long)(c->growth ? k : c->k_eff[b]) * C + cfg->W;
     TcInit ti{};
     ti.B = B; ti.k = k; ti.W = cfg->W; ti.P = P; ti.n_sms = c->n_sms; ti.max_ctas = cfg->max_ctas;
     ti.fuse_combine = cfg->merge_mode == LSA_MERGE_FUSED ? 1 : 0;
@@ -459,8 +509,8 @@ static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx,
     for (int i = 0; i < m; ++i) fire.ids[i] = ids[off + i];
     {
       ProfScope prof(c, LSA_PH_RESIDENCY, c->sf);
-      LSA_CUDA(c, launch_residency(c->d_seqs, c->pool, fire, sel_idx + (size_t)off * c->k, c->B, c->k, (int)cfg.hot_pages,
-                                   c->page_bytes, c->sf));
+      LSA_CUDA(c, launch_residency(c->d_seqs, c->pool, fire, sel_idx + (size_t)off * c->k, c->B, c->k, c->P_lru,
+                                   c->page_bytes, c->sf, c->k_sel, c->growth ? cfg.C : 0));
     }
     {
       ProfScope prof(c, LSA_PH_FETCH, c->sf);
@@ -472,7 +522,11 @@ static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx,
   for (int i = 0; i < n; ++i) {
     c->pending[ids[i]] = 1;
     c->visible_at[ids[i]] = c->step[ids[i]] + cfg.recall_lag;
-    c->n_tbl[1 - c->cur_buf[ids[i]]][ids[i]] = sel_is_topk ? c->k_eff[ids[i]] : -1;
+    const int b = ids[i];
+    // entries of the staged table: the recalled chunks, then the tail chunk of a growing sequence if it holds rows
+    const int tail = (c->growth && c->seq_host[b].n_csa % cfg.C) ? 1 : 0;
+    c->n_tbl[1 - c->cur_buf[b]][b] = sel_is_topk ? c->k_eff[b] + tail : -1;
+    c->ncand_nxt[b] = c->seq_host[b].n_chunks;
   }
   return LSA_OK;
 }
@@ -496,6 +550,7 @@ static bool due_mask(lsa_ctx* c, bool force, uint32_t words[32]) {
       words[b >> 5] |= 1u << (b & 31);
       c->pending[b] = 0;
       c->cur_buf[b] ^= 1;                         // the device flips its record under the same condition
+      c->ncand_cur[b] = c->ncand_nxt[b];
       any = true;
     }
   }
@@ -554,7 +609,7 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
     if (prof) cudaEventRecord(c->prof_ev[LSA_PH_ATTENTION][2 * ia], c->sc);
     long long tiles = 0;                          // host mirror: HCA + selected pages + window, in 128-key tiles
     for (int b = 0; b < c->B; ++b)
-      tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->seq_host[b].w_len + 127) / 128;
+      tiles += (c->seq_host[b].n_hca + 127) / 128 + c->k_eff[b] + (c->growth ? 2 : 0) + (c->seq_host[b].w_len + 127) / 128;
     int rc;
     if (c->cfg.step_overlap && tc_small_supported(c->tc) && !c->l2_armed && !c->no_small) {
       // small batches whose steps do not depend on one another (lsa_config.step_overlap): one launch per step that
@@ -709,7 +764,7 @@ extern "C" int lsa_step_graph(lsa_ctx* ctx, const void* q, const void* h, const 
   lsa_ctx* c = ctx;
   if (!q || !out) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null q / out");
   if ((k_new == nullptr) != (v_new == nullptr)) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "k_new and v_new must both be given or both NULL");
-  bool plain = c->attn_impl != LSA_ATTN_TCGEN05 || c->prof_cap > 0 || c->cfg.merge_mode == LSA_MERGE_FUSED || (k_new && c->cfg.W < 1);
+  bool plain = c->growth || c->attn_impl != LSA_ATTN_TCGEN05 || c->prof_cap > 0 || c->cfg.merge_mode == LSA_MERGE_FUSED || (k_new && c->cfg.W < 1);
   for (int b = 0; b < c->B && !plain; ++b)
     plain = (c->step[b] % c->cfg.tau == 0) || (c->pending[b] && c->step[b] >= c->visible_at[b]);   // trigger, or a swap is due
   c->no_small = true;             // the captured launch reads the device records: this context stays on the general kernels
@@ -1008,6 +1063,86 @@ extern "C" int lsa_export_chunks(lsa_ctx* ctx, int32_t seq, int32_t first_chunk,
   return LSA_OK;
 }
 
+// ---- NEXT-4 (second half): decoded tokens' compressed entries ---------------------------------------------------
+extern "C" int lsa_append_compressed(lsa_ctx* ctx, const int32_t* seq_ids, int32_t n, const void* csa_k, const void* csa_v,
+                                     const void* hca_k, const void* hca_v, const void* emb_rows) {
+  if (!ctx) return LSA_ERR_STATE;
+  lsa_ctx* c = ctx;
+  if (!c->growth) LSA_FAIL(c, LSA_ERR_STATE, "the context was created without growth capacity (lsa_seq_desc.cap_csa)");
+  if (c->l1 || c->l2) LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "growth is only built for the dual-encoder indexer (no Level-1 / Level-2 index keys are appended)");
+  if ((csa_k == nullptr) != (csa_v == nullptr) || (hca_k == nullptr) != (hca_v == nullptr))
+    LSA_FAIL(c, LSA_ERR_INVALID_ARG, "csa_k / csa_v and hca_k / hca_v must be given in pairs");
+  int rc = check_ids(c, seq_ids, n);
+  if (rc) return rc;
+  if (!csa_k && !hca_k) return LSA_OK;
+  const int C = c->cfg.C;
+  bool roll = false, any_done = false;
+  for (int i = 0; i < n; ++i) {                     // validate everything before anything is enqueued
+    const int b = seq_ids[i];
+    const SeqDev& s = c->seq_host[b];
+    if (hca_k && s.n_hca >= s.cap_hca) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: HCA capacity %d exceeded", b, s.cap_hca);
+    if (!csa_k) continue;
+    if (s.n_csa >= c->cap_csa[b]) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: CSA capacity %lld exceeded", b, c->cap_csa[b]);
+    const int ch = (int)(s.n_csa / C), r = (int)(s.n_csa % C);
+    if (r == 0) {
+      // chunks [ncand_cur, ch) are still attended through the tier: a third one would need the reserved page of the oldest
+      if (ch - c->ncand_cur[b] >= 2)
+        LSA_FAIL(c, LSA_ERR_STATE, "seq %d: chunk %d would be the third chunk of the decode tier (chunks complete faster than tables turn over)", b, ch);
+      if (c->n_tbl[c->cur_buf[b]][b] < 0 || (c->pending[b] && c->n_tbl[1 - c->cur_buf[b]][b] < 0))
+        LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "seq %d: growth needs tables staged from the library's own top-k (lsa_step), not from lsa_fetch_chunks", b);
+      roll = true;
+    }
+    if (r == C - 1) {
+      if (!emb_rows) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: the entry completes chunk %d, emb_rows is required", b, ch);
+      roll = any_done = true;
+    }
+  }
+  if (roll) {
+    // a completed chunk / a new tail changes what the side band reads (candidates, the staged table): let the side band
+    // and earlier exports finish first.  Rare: twice per C entries.
+    LSA_CUDA(c, cudaEventRecord(c->ev_roll, c->sf));
+    LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_roll, 0));
+  }
+  for (int off = 0; off < n; off += kFireMax) {
+    AppendList list{};
+    list.n = std::min(kFireMax, n - off);
+    for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[off + i];
+    LSA_CUDA(c, launch_append_compressed(c->cfg.dtype, c->d_seqs, c->pool, c->cfg.hot_pool, list, off, csa_k, csa_v, hca_k, hca_v, emb_rows,
+                                         c->cfg.D, c->cfg.E, C, c->k, c->k_sel, c->page_bytes, c->sc));
+    c->attn_launches += 1;
+  }
+  c->serialize_next = true;                          // the next attention launch reads what these kernels wrote
+  if (any_done) {
+    LSA_CUDA(c, cudaEventRecord(c->ev_compute, c->sc));
+    LSA_CUDA(c, cudaStreamWaitEvent(c->sf, c->ev_compute, 0));
+  }
+  for (int i = 0; i < n; ++i) {                     // host mirrors + export of completed chunks (P:179 direction)
+    const int b = seq_ids[i];
+    SeqDev& s = c->seq_host[b];
+    if (hca_k) { s.n_hca += 1; c->hca_appended += 1; }
+    if (!csa_k) continue;
+    const int ch = (int)(s.n_csa / C), r = (int)(s.n_csa % C);
+    if (r == 0) {
+      c->n_tbl[c->cur_buf[b]][b] += 1;
+      if (c->pending[b]) c->n_tbl[1 - c->cur_buf[b]][b] += 1;
+    }
+    s.n_csa += 1;
+    c->csa_appended += 1;
+    if (r == C - 1) {
+      s.n_chunks = ch + 1;
+      s.k_eff = std::min(c->k_sel, ch + 1);
+      c->k_eff[b] = s.k_eff;
+      const unsigned char* src = static_cast<const unsigned char*>(c->cfg.hot_pool) + (long long)(s.tier_page0 + (ch & 1)) * c->page_bytes;
+      void* dst = const_cast<unsigned char*>(reinterpret_cast<const unsigned char*>(s.cold)) + (long long)ch * c->page_bytes;
+      const int ctas = (int)std::max<long long>(1, std::min<long long>(c->fetch_ctas, (c->page_bytes + 16383) / 16384));
+      LSA_CUDA(c, launch_export(src, dst, c->page_bytes, ctas, c->sf));
+      c->index_launches += 1;
+      c->chunks_exported += 1;
+    }
+  }
+  return LSA_OK;
+}
+
 // ---- support --------------------------------------------------------------------------------------
 extern "C" int lsa_set_chunk_emb(lsa_ctx* ctx, int32_t seq, const void* chunk_emb) {
   if (!ctx) return LSA_ERR_STATE;
@@ -1077,6 +1212,9 @@ extern "C" int lsa_get_stats(lsa_ctx* ctx, lsa_stats* out) {
   out->index_launches = ctx->index_launches;
   out->attn_impl = ctx->attn_impl;
   out->attn_ctas = ctx->last_attn_ctas;
+  out->csa_appended = ctx->csa_appended;
+  out->hca_appended = ctx->hca_appended;
+  out->chunks_exported = ctx->chunks_exported;
   return LSA_OK;
 }
 

@@ -407,7 +407,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
   for (int b = 0; b < init.B; ++b) {
     const SeqDev& s = init.seq_host[b];
     const void* ptrs[4] = {s.hca_k, s.hca_v, s.win_k, s.win_v};
-    const uint64_t rows[4] = {(uint64_t)s.n_hca, (uint64_t)s.n_hca, (uint64_t)init.W, (uint64_t)init.W};
+    const uint64_t rows[4] = {(uint64_t)s.cap_hca, (uint64_t)s.cap_hca, (uint64_t)init.W, (uint64_t)init.W};   // cap_hca = n_hca unless the history grows
     for (int j = 0; j < 4; ++j) {
       const bool none = rows[j] == 0 || ptrs[j] == nullptr;     // never referenced: point at the pool
       if (!encode_rows(pl->encode, &maps[(size_t)b * 4 + j], none ? init.hot_pool : ptrs[j], none ? kTcTile : rows[j], kTcTile, 2, msg)) {
@@ -431,7 +431,7 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
     for (int b = 0; b < init.B; ++b) {
       const SeqDev& s = init.seq_host[b];
       const void* ptrs[4] = {s.hca_k, s.hca_v, s.win_k, s.win_v};
-      const uint64_t rows[4] = {(uint64_t)s.n_hca, (uint64_t)s.n_hca, (uint64_t)init.W, (uint64_t)init.W};
+      const uint64_t rows[4] = {(uint64_t)s.cap_hca, (uint64_t)s.cap_hca, (uint64_t)init.W, (uint64_t)init.W};   // cap_hca = n_hca unless the history grows
       for (int j = 0; j < 4; ++j) {
         maps8[(size_t)b * 8 + j] = maps[(size_t)b * 4 + j];
         const bool none = rows[j] == 0 || ptrs[j] == nullptr;

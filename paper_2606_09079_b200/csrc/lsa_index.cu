@@ -128,8 +128,10 @@ topk_kernel(const SeqDev* __restrict__ seqs, FireList fire, const float* __restr
     return ((unsigned long long)(~float_to_ordered(sc[c])) << 32) | (unsigned)c;
   };
   // n <= 4096: histogram select + sort of the k winners; larger tables: radix select over the keys in global memory
-  const int m = sq.n_chunks <= 4096 ? block_topk_select(sc, sq.n_chunks, min(k, sq.n_chunks), sm)
-                                    : block_select_smallest(keyf, sq.n_chunks, min(k, sq.n_chunks), sm);
+  // k_eff = min(recalled chunks per table, n_chunks): k for a static context, k - 2 for a growing one (DESIGN R33)
+  const int kk = min(k, sq.k_eff);
+  const int m = sq.n_chunks <= 4096 ? block_topk_select(sc, sq.n_chunks, kk, sm)
+                                    : block_select_smallest(keyf, sq.n_chunks, kk, sm);
   for (int j = threadIdx.x; j < k; j += blockDim.x) {
     int idx = -1;
     float val = -INFINITY;

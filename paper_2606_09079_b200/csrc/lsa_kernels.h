@@ -29,8 +29,16 @@ cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* s
                         int n_chunks_max, int k, int32_t* sel_idx, float* sel_score, cudaStream_t st);
 
 // ---- S4-S6 (lsa_residency.cu) -----------------------------------------------------------
+// P = pages managed by the LRU; k_cap = recalled chunks per table at most (0: k); C = entries per chunk (tail entry of a
+// growing sequence, 0: static context)
 cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, const int32_t* sel_idx,
-                             int B, int k, int P, long long page_bytes, cudaStream_t st);
+                             int B, int k, int P, long long page_bytes, cudaStream_t st, int k_cap = 0, int C = 0);
+// NEXT-4 (second half): one block per listed sequence writes the handed-over CSA / HCA entries and, when a chunk completes
+// or a new tail chunk starts, updates the records and page tables (lsa_residency.cu: append_compressed_kernel)
+struct AppendList { int n; int ids[kFireMax]; };
+cudaError_t launch_append_compressed(int dtype, SeqDev* seqs, PoolDev pool, void* hot_pool, const AppendList& list, int row0,
+                                     const void* csa_k, const void* csa_v, const void* hca_k, const void* hca_v, const void* emb_rows,
+                                     int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st);
 cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas,
                          cudaStream_t st);
 // NEXT-4: copy `bytes` (multiple of 16) from device memory into the mapped pinned cold pool

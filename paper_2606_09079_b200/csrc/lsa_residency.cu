@@ -35,7 +35,9 @@ struct ResSmem {
 
 __global__ void __launch_bounds__(1024)
 residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const int32_t* __restrict__ sel_idx,
-                 int B, int k, int P, long long page_bytes) {
+                 int B, int k, int P, long long page_bytes, int k_cap, int C) {
+  // P = pages the LRU manages, k_cap = recalled chunks per table at most (a growing context keeps 2 B pages and two table
+  // slots per sequence for the decode tier, DESIGN R32 / R33)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ResSmem& sm = *reinterpret_cast<ResSmem*>(smem_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -78,6 +80,11 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
     const int n_sel = sm.n_sel;
     const unsigned long long tick = sm.tick;
     const unsigned int epoch = sm.epoch;
+    if (n_sel > k_cap) {                           // an explicit selection larger than the table's recalled share
+      if (tid == 0) pool.counters[C_ERROR] = 2;
+      __syncthreads();
+      continue;
+    }
 
     // ---- pin every page of a current table and of other sequences' staged tables ----
     for (int idx = tid; idx < B * 2 * k; idx += blockDim.x) {
@@ -183,7 +190,16 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
       pool.tbl_page[((size_t)b * 2 + buf) * k + tid] = sm.next_page[tid];
     }
     if (tid == 0) {
-      sq.n_tbl[buf] = n_sel;
+      int n_tbl = n_sel;
+      if (sq.tier_page0 >= 0 && sq.n_csa % C != 0) {
+        // the tail chunk (being filled by lsa_append_compressed) is always attended: its entry follows the recalled ones.
+        // Chunks completed since are not listed: this trigger saw them as candidates (DESIGN R31).
+        const int c = (int)(sq.n_csa / C);
+        pool.tbl_chunk[((size_t)b * 2 + buf) * k + n_tbl] = c;
+        pool.tbl_page[((size_t)b * 2 + buf) * k + n_tbl] = sq.tier_page0 + (c & 1);
+        n_tbl += 1;
+      }
+      sq.n_tbl[buf] = n_tbl;
       sq.pending = 1;
       pool.counters[C_FETCH_COUNT] += n_miss;
       pool.counters[C_MISSES] += n_miss;
@@ -293,8 +309,88 @@ prestep_kernel_v(SeqDev* __restrict__ seqs, int D, int W, SwapWords sw, int use_
   }
 }
 
+// ---- NEXT-4 (second half): decoded tokens' compressed entries (P:185 tier 3; DESIGN R29-R33) ------------------
+// One block per listed sequence; row = row0 + blockIdx.x of the caller's [n][D] / [n][E] arrays.  The entry becomes row
+// n_csa % C of the tail chunk's reserved page; a new tail chunk gets its table entries (current table, and the staged one
+// if a swap is pending: the host has made the side band finish first); a completed chunk gets its embedding row and
+// becomes a candidate.  The records change after the rows are written; readers are later launches on the same stream.
+template <typename T>
+__global__ void __launch_bounds__(128)
+append_compressed_kernel(SeqDev* __restrict__ seqs, PoolDev pool, unsigned char* __restrict__ hot_pool, AppendList list, int row0,
+                         const T* __restrict__ csa_k, const T* __restrict__ csa_v, const T* __restrict__ hca_k,
+                         const T* __restrict__ hca_v, const T* __restrict__ emb_rows, int D, int E, int C, int k, int k_sel,
+                         long long page_bytes) {
+  const int b = list.ids[blockIdx.x], row = row0 + blockIdx.x;
+  SeqDev& sq = seqs[b];
+  constexpr int V = Elem<T>::kVec;
+  const long long n = sq.n_csa;
+  const int c = (int)(n / C), i = (int)(n % C);
+  if (hca_k) {
+    T* kd = reinterpret_cast<T*>(const_cast<void*>(sq.hca_k)) + (size_t)sq.n_hca * D;
+    T* vd = reinterpret_cast<T*>(const_cast<void*>(sq.hca_v)) + (size_t)sq.n_hca * D;
+    for (int d = threadIdx.x * V; d < D; d += blockDim.x * V) {
+      *reinterpret_cast<uint4*>(kd + d) = *reinterpret_cast<const uint4*>(hca_k + (size_t)row * D + d);
+      *reinterpret_cast<uint4*>(vd + d) = *reinterpret_cast<const uint4*>(hca_v + (size_t)row * D + d);
+    }
+  }
+  const int page = sq.tier_page0 + (c & 1);
+  if (csa_k) {
+    T* pg = reinterpret_cast<T*>(hot_pool + (long long)page * page_bytes);
+    T* kd = pg + (size_t)i * D;
+    T* vd = pg + (size_t)C * D + (size_t)i * D;
+    for (int d = threadIdx.x * V; d < D; d += blockDim.x * V) {
+      *reinterpret_cast<uint4*>(kd + d) = *reinterpret_cast<const uint4*>(csa_k + (size_t)row * D + d);
+      *reinterpret_cast<uint4*>(vd + d) = *reinterpret_cast<const uint4*>(csa_v + (size_t)row * D + d);
+    }
+    if (i == C - 1) {                           // the entry completes chunk c: its embedding row
+      T* ed = reinterpret_cast<T*>(const_cast<void*>(sq.emb)) + (size_t)c * E;
+      for (int e = threadIdx.x * V; e < E; e += blockDim.x * V)
+        *reinterpret_cast<uint4*>(ed + e) = *reinterpret_cast<const uint4*>(emb_rows + (size_t)row * E + e);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (hca_k) sq.n_hca += 1;
+    if (csa_k) {
+      if (i == 0) {                             // a new tail chunk: listed after everything else (its id is the largest)
+        const int cur = sq.cur_buf;
+        int m = sq.n_tbl[cur];
+        pool.tbl_chunk[((size_t)b * 2 + cur) * k + m] = c;
+        pool.tbl_page[((size_t)b * 2 + cur) * k + m] = page;
+        sq.n_tbl[cur] = m + 1;
+        if (sq.pending) {
+          m = sq.n_tbl[1 - cur];
+          pool.tbl_chunk[((size_t)b * 2 + 1 - cur) * k + m] = c;
+          pool.tbl_page[((size_t)b * 2 + 1 - cur) * k + m] = page;
+          sq.n_tbl[1 - cur] = m + 1;
+        }
+      }
+      sq.n_csa = n + 1;
+      if (i == C - 1) {
+        sq.n_chunks = c + 1;
+        sq.k_eff = min(k_sel, c + 1);
+      }
+    }
+  }
+}
+
+cudaError_t launch_append_compressed(int dtype, SeqDev* seqs, PoolDev pool, void* hot_pool, const AppendList& list, int row0,
+                                     const void* csa_k, const void* csa_v, const void* hca_k, const void* hca_v, const void* emb_rows,
+                                     int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st) {
+  unsigned char* hp = reinterpret_cast<unsigned char*>(hot_pool);
+  if (dtype == 0)
+    append_compressed_kernel<float><<<list.n, 128, 0, st>>>(seqs, pool, hp, list, row0, (const float*)csa_k, (const float*)csa_v,
+                                                            (const float*)hca_k, (const float*)hca_v, (const float*)emb_rows, D, E,
+                                                            C, k, k_sel, page_bytes);
+  else
+    append_compressed_kernel<__nv_bfloat16><<<list.n, 128, 0, st>>>(
+        seqs, pool, hp, list, row0, (const __nv_bfloat16*)csa_k, (const __nv_bfloat16*)csa_v, (const __nv_bfloat16*)hca_k,
+        (const __nv_bfloat16*)hca_v, (const __nv_bfloat16*)emb_rows, D, E, C, k, k_sel, page_bytes);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, const int32_t* sel_idx, int B, int k,
-                             int P, long long page_bytes, cudaStream_t st) {
+                             int P, long long page_bytes, cudaStream_t st, int k_cap, int C) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(residency_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -302,7 +398,8 @@ cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, c
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  return launch_pdl(residency_kernel, dim3(1), dim3(1024), sizeof(ResSmem), st, seqs, pool, fire, sel_idx, B, k, P, page_bytes);
+  return launch_pdl(residency_kernel, dim3(1), dim3(1024), sizeof(ResSmem), st, seqs, pool, fire, sel_idx, B, k, P, page_bytes, k_cap > 0 ? k_cap : k,
+                    C > 0 ? C : 1);
 }
 
 cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas, cudaStream_t st) {

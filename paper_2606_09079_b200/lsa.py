@@ -33,7 +33,7 @@ EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
            "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats", "lsa_export_chunks",
-           "lsa_last_error", "lsa_destroy", "lsa_version"]
+           "lsa_append_compressed", "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
 class LsaError(RuntimeError):
@@ -54,14 +54,16 @@ class lsa_config(C.Structure):
 class lsa_seq_desc(C.Structure):
     _fields_ = [("cold_csa", C.c_void_p), ("n_csa", C.c_int64), ("chunk_emb", C.c_void_p),
                 ("hca_k", C.c_void_p), ("hca_v", C.c_void_p), ("n_hca", C.c_int64), ("win_k", C.c_void_p),
-                ("win_v", C.c_void_p), ("w_len", C.c_int32), ("w_head", C.c_int32), ("step0", C.c_int64)]
+                ("win_v", C.c_void_p), ("w_len", C.c_int32), ("w_head", C.c_int32), ("step0", C.c_int64),
+                ("cap_csa", C.c_int64), ("cap_hca", C.c_int64)]
 
 
 class lsa_stats(C.Structure):
     _fields_ = [("triggers", C.c_uint64), ("hits", C.c_uint64), ("misses", C.c_uint64),
                 ("evictions", C.c_uint64), ("bytes_fetched", C.c_uint64), ("steps", C.c_uint64),
                 ("attn_launches", C.c_uint64), ("index_launches", C.c_uint64), ("pool_error", C.c_int32),
-                ("attn_impl", C.c_int32), ("attn_ctas", C.c_int32), ("reserved", C.c_int32)]
+                ("attn_impl", C.c_int32), ("attn_ctas", C.c_int32), ("reserved", C.c_int32),
+                ("csa_appended", C.c_uint64), ("hca_appended", C.c_uint64), ("chunks_exported", C.c_uint64)]
 
 
 class lsa_l1_layer(C.Structure):
@@ -108,6 +110,7 @@ def _load() -> C.CDLL:
     lib.lsa_l2_select.argtypes = [vp, vp, vp, vp, vp]
     lib.lsa_l2_get_mask.argtypes = [vp, C.c_int32, vp]
     lib.lsa_export_chunks.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, vp]
+    lib.lsa_append_compressed.argtypes = [vp, C.POINTER(C.c_int32), C.c_int32, vp, vp, vp, vp, vp]
     lib.lsa_step_graph.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.lsa_graph_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.lsa_step_l2.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
@@ -207,12 +210,14 @@ class LsaContext:
             d.chunk_emb = _dev_ptr(s.get("chunk_emb"), td, "chunk_emb")
             d.hca_k = _dev_ptr(s.get("hca_k"), td, "hca_k")
             d.hca_v = _dev_ptr(s.get("hca_v"), td, "hca_v")
-            d.n_hca = 0 if s.get("hca_k") is None else s["hca_k"].shape[0]
+            d.n_hca = int(s["n_hca"]) if "n_hca" in s else (0 if s.get("hca_k") is None else s["hca_k"].shape[0])
             d.win_k = _dev_ptr(s.get("win_k"), td, "win_k")
             d.win_v = _dev_ptr(s.get("win_v"), td, "win_v")
             d.w_len = int(s.get("w_len", 0))
             d.w_head = int(s.get("w_head", 0))
             d.step0 = int(s.get("step0", 0))
+            d.cap_csa = int(s.get("cap_csa", 0))
+            d.cap_hca = int(s.get("cap_hca", 0))
         handle = C.c_void_p()
         rc = _lib.lsa_init_pools(C.byref(cfg), descs, C.byref(handle))
         if rc != 0:
@@ -351,6 +356,16 @@ class LsaContext:
     def export_chunks(self, seq: int, first_chunk: int, src: torch.Tensor):
         """KV export (VRAM -> pinned cold pool): src = [n][2][C][D] CUDA tensor of page images for chunks first_chunk.."""
         self._check(_lib.lsa_export_chunks(self._h, seq, first_chunk, int(src.shape[0]), _dev_ptr(src, self.tdtype, "src")))
+
+    def append_compressed(self, seq_ids: Sequence[int], csa_k=None, csa_v=None, hca_k=None, hca_v=None, emb_rows=None):
+        """Hand over the compressed entries of the tokens decoded since the last call (NEXT-4): csa_k / csa_v [n][D],
+        hca_k / hca_v [n][D], emb_rows [n][E] CUDA tensors (row i belongs to seq_ids[i])."""
+        arr, n = _ids(seq_ids)
+        self._check(_lib.lsa_append_compressed(self._h, arr, n, _dev_ptr(csa_k, self.tdtype, "csa_k"), _dev_ptr(csa_v, self.tdtype, "csa_v"),
+                                               _dev_ptr(hca_k, self.tdtype, "hca_k"), _dev_ptr(hca_v, self.tdtype, "hca_v"),
+                                               _dev_ptr(emb_rows, self.tdtype, "emb_rows")))
+        for t in (csa_k, csa_v, hca_k, hca_v, emb_rows):
+            self._on(t, self.stream_compute)
 
     def step_graph(self, q, h, k_new=None, v_new=None, out=None):
         """lsa_step with the non-trigger step replayed from a CUDA graph (keep q / k_new / v_new / out at fixed addresses)."""

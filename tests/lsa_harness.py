@@ -243,3 +243,129 @@ def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=
             n_checked += 1
     rig.ctx.sync()
     return dict(checked=n_checked, max_abs_err=max_err, oracle=orc, tie_triggers=n_ties)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-4 second half: lock-step run with a growing compressed history
+# ------------------------------------------------------------------------------------------
+class GrowthRig(GpuRig):
+    """GpuRig whose per-sequence arrays have the capacity GrowthInputs asks for (lsa_seq_desc.cap_csa / cap_hca)."""
+
+    def __init__(self, wl: LsaWorkload, gi, device="cuda:0", **ctx_over):
+        import torch
+        from paper_2606_09079_b200 import lsa
+        from paper_2606_09079_b200.workloads import to_torch
+        c = wl.cfg
+        self.wl, self.cfg, self.device, self.gi = wl, c, torch.device(device), gi
+        dt = c.dtype
+        tdt = torch.float32 if dt == "f32" else torch.bfloat16
+        dev = self.device
+        cold, emb, hk, hv = growth_arrays(wl, gi)
+        self.hot_pool = torch.zeros((c.hot_pages, 2, c.C, c.D), dtype=tdt, device=dev)
+        self.W_q = to_torch(wl.W_q, dt).to(dev)
+        self.cold = [to_torch(x, dt).pin_memory() for x in cold]
+        self.emb = [to_torch(x, dt).to(dev) for x in emb]
+        self.hca_k = [to_torch(x, dt).to(dev) for x in hk]
+        self.hca_v = [to_torch(x, dt).to(dev) for x in hv]
+        self.win_k = [to_torch(x, dt).to(dev) for x in wl.win_k]
+        self.win_v = [to_torch(x, dt).to(dev) for x in wl.win_v]
+        seqs = []
+        for b in range(c.B):
+            seqs.append(dict(cold_csa=self.cold[b], n_csa=c.n_csa(b), chunk_emb=self.emb[b], hca_k=self.hca_k[b], hca_v=self.hca_v[b],
+                             n_hca=c.n_hca(b), win_k=self.win_k[b], win_v=self.win_v[b], w_len=min(c.W, c.L[b]),
+                             w_head=min(c.W, c.L[b]) % c.W, step0=c.step0(b), cap_csa=gi.cap_csa(b), cap_hca=gi.cap_hca(b)))
+        kw = dict(dtype=lsa.LSA_F32 if dt == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W, Dh=c.Dh, E=c.E,
+                  k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=self.W_q, seqs=seqs, recall_lag=c.recall_lag)
+        kw.update(ctx_over)
+        self.ctx = lsa.LsaContext(**kw)
+        self.tdt = tdt
+
+
+def run_growth_lockstep(wl: LsaWorkload, gi, rig: "GrowthRig", steps: int, check_attention_at=None, check_tables_every: int = 1):
+    """lsa_append_compressed + lsa_step against GrowingLsaOracle: the recalled part of every staged table is validated
+    against the oracle's scores and fed back (tolerance cascade), then tables (recalled + tier entries), residency, counters,
+    fetched bytes, exported cold-pool bytes and the tier pages' valid rows are compared bit for bit, attention within tolerance."""
+    import torch
+    from oracle import validate_selection
+    from paper_2606_09079_b200.workloads import from_torch
+    c = wl.cfg
+    orc = make_growing_oracle(wl, gi)
+    tol = attn_tolerance(c.dtype)
+    n_checked, max_err, n_recalled_grown = 0, 0.0, 0
+    ids = list(range(c.B))
+    for t in range(steps):
+        # ---- hand over what is due before step t (R29), both sides ----
+        hca = gi.hca_entry(t) if gi.hca_due(t) else None
+        csa = gi.csa_entry(t) if gi.csa_due(t) else None
+        if hca is not None or csa is not None:
+            emb_rows = None
+            if csa is not None:
+                rows = np.zeros((c.B, c.E), dtype=wl.W_q.dtype)
+                need = False
+                for b in range(c.B):
+                    if orc.n_csa[b] % c.C == c.C - 1:
+                        rows[b] = gi.emb_row(b, orc.n_csa[b] // c.C)
+                        need = True
+                emb_rows = rig.dev(rows) if need else None
+            rig.ctx.append_compressed(ids, None if csa is None else rig.dev(csa[0]), None if csa is None else rig.dev(csa[1]),
+                                      None if hca is None else rig.dev(hca[0]), None if hca is None else rig.dev(hca[1]), emb_rows)
+            done = oracle_appends(orc, gi, t)
+            if done:
+                rig.ctx.sync()
+                for b, ch in done:                                  # export: the cold pool's copy, bit for bit
+                    got = from_torch(rig.cold[b][ch], c.dtype)
+                    assert np.array_equal(got, orc.cold[b][ch]), f"step {t} seq {b}: exported chunk {ch} differs"
+                    got_e = from_torch(rig.emb[b][ch].cpu(), c.dtype)
+                    assert np.array_equal(got_e, orc.chunk_emb[b][ch]), f"step {t} seq {b}: embedding row {ch}"
+        q, h = wl.q(t), wl.h(t)
+        kn, vn = wl.kv_new(t)
+        firing = [b for b in range(c.B) if orc.step[b] % c.tau == 0]
+        out_gpu = rig.ctx.step(rig.dev(q), rig.dev(h), rig.dev(kn), rig.dev(vn))
+        which = 0 if c.recall_lag == 0 else 1
+        forced = {}
+        for b in firing:
+            chunks, pages = rig.ctx.page_table(b, which)
+            rec = [ch for ch, p in zip(chunks, pages) if p < orc.P_lru]
+            sc = orc.scores(b, h[b])
+            order = sorted(rec, key=lambda ch: (-sc[ch], ch))
+            padded = np.full(orc.k_sel, -1, dtype=np.int64); padded[: len(order)] = order
+            msg = validate_selection(padded, sc, orc.k_sel)
+            assert msg is None, f"step {t} seq {b}: {msg}"
+            forced[b] = rec
+        orc.step_begin(h, forced_selection=forced if firing else None)
+        for b in firing:
+            chunks, pages = rig.ctx.page_table(b, which)
+            assert list(zip(chunks, pages)) == orc.table(b, which), f"step {t} seq {b}: staged table {list(zip(chunks, pages))} vs {orc.table(b, which)}"
+            n = orc.n_chunks[b]
+            assert rig.ctx.residency(b, n) == orc.pool.page_of[b][:n], f"step {t} seq {b}: residency mismatch"
+            n_recalled_grown += sum(1 for ch in forced[b] if ch >= c.n_csa(b) // c.C)
+        if firing:
+            st = rig.ctx.stats()
+            assert (st["hits"], st["misses"], st["evictions"], st["bytes_fetched"], st["pool_error"], st["chunks_exported"]) == \
+                   (orc.pool.hits, orc.pool.misses, orc.pool.evictions, orc.pool.bytes_fetched, 0, orc.exported), f"step {t}: counters"
+            hot_np = from_torch(rig.hot_pool.cpu(), c.dtype)
+            owned = [p for p, o in enumerate(orc.pool.owner) if o is not None]
+            assert np.array_equal(hot_np[owned], orc.pool.hot[owned]), f"step {t}: fetched bytes differ"
+        if t % check_tables_every == 0:
+            for b in range(c.B):
+                chunks, pages = rig.ctx.page_table(b, 0)
+                assert list(zip(chunks, pages)) == orc.table(b, 0), f"step {t} seq {b}: current table {list(zip(chunks, pages))} vs {orc.table(b, 0)}"
+            hot_np = from_torch(rig.hot_pool.cpu(), c.dtype)
+            for b in range(c.B):
+                for ch in orc.tier(b):                             # the tier pages' valid rows
+                    p, v = orc.tier_page(b, ch), orc.valid_rows(b, ch)
+                    assert np.array_equal(hot_np[p][:, :v], orc.pool.hot[p][:, :v]), f"step {t} seq {b}: tier chunk {ch}"
+        attend = check_attention_at is None or t in check_attention_at
+        res = orc.step_end(q, kn, vn, attend=attend)
+        if attend:
+            got = rig.host(out_gpu)
+            np.testing.assert_allclose(got, res[0], err_msg=f"attention mismatch at step {t}", **tol)
+            max_err = max(max_err, float(np.max(np.abs(got - res[0]))))
+            n_checked += 1
+    rig.ctx.sync()
+    st = rig.ctx.stats()
+    for b in range(c.B):
+        hk = from_torch(rig.hca_k[b].cpu(), c.dtype)
+        assert np.array_equal(hk[: orc.n_hca[b]], orc.hca_k[b][: orc.n_hca[b]])
+    return dict(checked=n_checked, max_abs_err=max_err, oracle=orc, exported=st["chunks_exported"], csa_appended=st["csa_appended"],
+                hca_appended=st["hca_appended"], recalled_grown=n_recalled_grown)

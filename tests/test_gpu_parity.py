@@ -756,3 +756,69 @@ def test_small_batch_step_overlap_lockstep():
     r = run_lockstep(wl, rig, cfg.steps)
     assert r["checked"] == cfg.steps
     rig.ctx.close()
+
+
+# ---- NEXT-4 second half: the compressed history grows while decoding (DESIGN R29-R33) ------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("lag", [0, 1, 2])
+def test_growth_lockstep_small_f32(lag):
+    """SIMT path, every step checked: a CSA entry every step, an HCA entry every 16, chunks of 16 entries, so in 200 steps 12
+    chunks per sequence complete, are exported, become candidates and some are recalled again from their cold copy.  The
+    window (24 rows) wraps 8 times: the decoded tokens really move from the window into CSA / HCA entries."""
+    from lsa_harness import GrowthRig, run_growth_lockstep
+    from paper_2606_09079_b200.workloads import GrowthInputs
+    cfg = make_small_config("f32", B=2, L=[4096 + 24, 2432], C=16, W=24, k=5, tau=4, steps=0, hot_pages=20, needle_period=10 ** 9,
+                            recall_lag=lag)
+    wl = LsaWorkload(cfg)
+    gi = GrowthInputs(wl, steps=200, csa_every=1, hca_every=16, hot_frac=1.0)
+    rig = GrowthRig(wl, gi)
+    res = run_growth_lockstep(wl, gi, rig, 200)
+    assert res["checked"] == 200 and res["exported"] >= 24 and res["recalled_grown"] > 0
+    assert res["csa_appended"] == 2 * 199 and res["hca_appended"] == 2 * 12
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("overlap", [0, 1])
+def test_growth_lockstep_tcgen05(overlap):
+    """Tensor-core path at the BASELINE shape (bf16, H 64, D 512, C 128) with the paper's cadences (one CSA entry per 4 tokens,
+    one HCA entry per 128), 1100 steps > W = 512: two chunks complete per sequence; B = 2 with a ragged start (one sequence
+    begins inside a chunk).  step_overlap 1 takes the small-batch kernel, 0 the large-grid kernel + combine."""
+    from lsa_harness import GrowthRig, run_growth_lockstep
+    from paper_2606_09079_b200.workloads import GrowthInputs
+    cfg = make_small_config("bf16", B=2, L=[32768 + 4 * 50, 16384], H=64, D=512, C=128, W=512, Dh=256, E=128, k=6, tau=64,
+                            steps=0, hot_pages=24, needle_period=10 ** 9, n_needles=3)
+    wl = LsaWorkload(cfg)
+    gi = GrowthInputs(wl, steps=1100, csa_every=4, hca_every=128, hot_frac=1.0)
+    rig = GrowthRig(wl, gi, step_overlap=overlap)
+    check = set(range(0, 1100, 37)) | set(range(300, 330)) | set(range(508, 520)) | {1099}
+    res = run_growth_lockstep(wl, gi, rig, 1100, check_attention_at=check, check_tables_every=16)
+    assert res["exported"] == 2 + 2 and res["csa_appended"] == 2 * 274 and res["hca_appended"] == 2 * 8
+    from paper_2606_09079_b200 import lsa
+    assert rig.ctx.stats()["attn_impl"] == lsa.LSA_ATTN_TCGEN05
+
+
+@pytest.mark.gpu
+def test_growth_argument_errors():
+    from paper_2606_09079_b200 import lsa
+    from lsa_harness import GrowthRig, GpuRig
+    from paper_2606_09079_b200.workloads import GrowthInputs
+    cfg = make_small_config("f32", B=2, L=[4096, 2432], C=16, W=24, k=5, tau=4, steps=0, hot_pages=20, needle_period=10 ** 9)
+    wl = LsaWorkload(cfg)
+    gi = GrowthInputs(wl, steps=8, csa_every=1)
+    rig = GrowthRig(wl, gi)
+    z = torch.zeros((2, cfg.D), device="cuda")
+    with pytest.raises(lsa.LsaError):                       # a pair must be complete
+        rig.ctx.append_compressed([0, 1], csa_k=z)
+    with pytest.raises(lsa.LsaError):                       # ids ascending
+        rig.ctx.append_compressed([1, 0], csa_k=z, csa_v=z)
+    for _ in range(15):
+        rig.ctx.append_compressed([0, 1], csa_k=z, csa_v=z)
+    with pytest.raises(lsa.LsaError):                       # the 16th entry completes a chunk: emb_rows required
+        rig.ctx.append_compressed([0, 1], csa_k=z, csa_v=z)
+    rig.ctx.append_compressed([0, 1], csa_k=z, csa_v=z, emb_rows=torch.zeros((2, cfg.E), device="cuda"))
+    with pytest.raises(lsa.LsaError):                       # capacity: cap_csa = n_csa + 8 + 1 rounded up to a chunk
+        for _ in range(40):
+            rig.ctx.append_compressed([0, 1], csa_k=z, csa_v=z, emb_rows=torch.zeros((2, cfg.E), device="cuda"))
+    static = GpuRig(LsaWorkload(make_small_config("f32")))
+    with pytest.raises(lsa.LsaError):                       # a context without capacity cannot grow
+        static.ctx.append_compressed([0], csa_k=z[:1], csa_v=z[:1])
