@@ -38,6 +38,7 @@ import subprocess
 import sys
 import threading
 import time
+import types
 
 import numpy as np
 import torch
@@ -309,6 +310,7 @@ def main():
     ap.add_argument("--dry-run", action="store_true", help="CPU only: launcher, sharding and reductions with a gloo group")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
     ap.add_argument("--export", action="store_true", help="also time lsa_export_chunks (NEXT-4: KV export HBM -> pinned cold pool)")
+    ap.add_argument("--growth", action="store_true", help="also time the step with a growing compressed history (NEXT-4: lsa_append_compressed)")
     ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
     ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
     ap.add_argument("--l2-k2", type=int, default=2048, help="Level-2 Top-k (entries per sequence and step)")
@@ -744,6 +746,80 @@ def main():
                       mode="device kernel storing over the mapped pinned cold pool")
         del src, dstp
 
+    # ---- optional: the step with a growing compressed history (NEXT-4, second half): lsa_append_compressed every 4th step
+    # (CSA entry; HCA entry every 128th), chunks completing every 512 steps and being exported, against the static loop ----
+    growth = None
+    if args.growth and rank == 0:
+        n_gr = max(2048, min(args.steps, 8192))
+        n_gr += (-n_gr) % (R * c.tau)
+        per_rep = (R * c.tau * 2 + n_gr) // R + 8
+        extra = per_rep // (c.csa_ratio * c.C) + 2
+        cold_cap = []
+        for b in range(c.B):                                # one capacity-sized cold pool per sequence, shared by the replicas
+            x = torch.zeros((c.n_chunks(b) + extra,) + tuple(shared["cold"][b].shape[1:]), dtype=tdt).pin_memory()
+            x[: c.n_chunks(b)] = shared["cold"][b]
+            cold_cap.append(x)
+        greps = []
+        for ridx in range(R):
+            g_ = types.SimpleNamespace()
+            g_.hot_pool = torch.zeros((c.hot_pages + 2 * c.B, 2, c.C, c.D), dtype=tdt, device=dev)
+            g_.emb = [torch.cat([e, torch.zeros((extra, c.E), dtype=tdt, device=dev)]) for e in shared["emb"]]
+            g_.hca_k = [torch.cat([x, torch.zeros((per_rep // c.hca_ratio + 2, c.D), dtype=tdt, device=dev)]) for x in shared["hca_k"]]
+            g_.hca_v = [torch.cat([x, torch.zeros((per_rep // c.hca_ratio + 2, c.D), dtype=tdt, device=dev)]) for x in shared["hca_v"]]
+            g_.win_k = [x.clone() for x in shared["win_k"]]
+            g_.win_v = [x.clone() for x in shared["win_v"]]
+            phase = (c.tau - ridx * (c.tau // R)) % c.tau
+            seqs = [dict(cold_csa=cold_cap[b], n_csa=c.n_csa(b), n_hca=c.n_hca(b), chunk_emb=g_.emb[b], hca_k=g_.hca_k[b],
+                         hca_v=g_.hca_v[b], win_k=g_.win_k[b], win_v=g_.win_v[b], w_len=min(c.W, c.L[b]), w_head=0, step0=c.step0(b) + phase,
+                         cap_csa=(c.n_chunks(b) + extra) * c.C, cap_hca=int(g_.hca_k[b].shape[0])) for b in range(c.B)]
+            g_.ctx = lsa.LsaContext(dtype=lsa.LSA_F32 if c.dtype == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W, Dh=c.Dh,
+                                    E=c.E, k=c.k + 2, tau=c.tau, hot_pool=g_.hot_pool, W_q=shared["W_q"], seqs=seqs,
+                                    recall_lag=c.recall_lag, stream_compute=sc, stream_fetch=sf, attn_impl=shared["attn_impl"],
+                                    step_overlap=args.overlap)
+            g_.step, g_.bound = phase, {}
+            greps.append(g_)
+        ids_all = list(range(c.B))
+        emb_new = torch.nn.functional.normalize(torch.randn((c.B, c.E), device=dev, generator=torch.Generator(dev).manual_seed(c.seed)), dim=-1).to(tdt)
+        n_app = [0, 0]
+
+        def grow_step(i):
+            r = greps[i % R]
+            t = r.step - ((c.tau - (i % R) * (c.tau // R)) % c.tau)          # decode steps this replica has made
+            j = i % NIN
+            if t > 0 and t % c.csa_ratio == 0:
+                hk = t % c.hca_ratio == 0
+                r.ctx.append_compressed(ids_all, kns[j], vns[j], kns[j] if hk else None, vns[j] if hk else None, emb_new)
+                n_app[0] += c.B; n_app[1] += c.B if hk else 0
+            key = (j, (r.step // c.tau) % NIN)
+            fn = r.bound.get(key)
+            if fn is None:
+                fn = r.bound[key] = r.ctx.bind_step(qs[j], hs[key[1]], kns[j], vns[j], out)
+            fn()
+            r.step += 1
+
+        for i in range(2 * R * c.tau):
+            grow_step(i)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a0 = list(n_app)
+        e0.record(sc)
+        for i in range(n_gr):
+            grow_step(2 * R * c.tau + i)
+        sc.wait_stream(sf)
+        e1.record(sc)
+        sf.synchronize(); sc.synchronize()
+        gms = e0.elapsed_time(e1) / n_gr
+        gst = [r.ctx.stats() for r in greps]
+        growth = dict(value=per_step_units / (gms * 1e-3), unit=unit, ms_per_step=gms, steps=n_gr, static_ms_per_step=ms / args.steps,
+                      csa_entries_in_region=n_app[0] - a0[0], hca_entries_in_region=n_app[1] - a0[1],
+                      chunks_exported=sum(s_["chunks_exported"] for s_ in gst), k=c.k + 2,
+                      note="k + 2 table slots and 2 B more pages, so the same k chunks are recalled as in the static loop and the tail "
+                           "chunk is attended on top; an append that only writes rows runs beside the previous attention launch and the next "
+                           "launch waits for its counter; a completed chunk / new tail (twice per 512 steps) is stream-ordered")
+        for r in greps:
+            r.ctx.close()
+        del greps, cold_cap
+
     # ---- optional: lsa_step_graph (NEXT-3) through the same replica rotation, fixed input buffers ----
     graph = None
     if args.graph and rank == 0 and stats["attn_impl"] == 2:
@@ -795,7 +871,7 @@ def main():
                     tie_triggers_seen=n_tie_triggers[0], clocks=clocks, roofline=roofline, dependent_inputs=dependent,
                     cpu_baseline=cpu_baseline, cpu_baseline_1t=cpu_baseline_1t,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases_ms.items()},
-                    fetch=fetch, side_band=side_band, l1_indexer=l1, level2=level2, step_graph=graph, export=export, wall_s=wall,
+                    fetch=fetch, side_band=side_band, l1_indexer=l1, level2=level2, step_graph=graph, export=export, growth=growth, wall_s=wall,
                     host_enqueue_ms_per_step=enq_free * 1e3 / n_free, host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=(units_job if tokens else units_job * (cfg.B if sharded else c.B)) / (ms * 1e-3))
         print(json.dumps(line))

@@ -104,6 +104,8 @@ struct lsa_ctx {
   std::vector<int> ncand_cur, ncand_nxt;   // candidates seen by the trigger of the current / the staged table (host mirror)
   cudaEvent_t ev_roll = nullptr;       // fetch-stream position a roll (chunk completed / new tail) must wait for
   unsigned long long csa_appended = 0, hca_appended = 0, chunks_exported = 0;
+  std::vector<unsigned int> grow_count;    // lsa_append_compressed calls per sequence (mirror of SeqDev::grow_epoch as enqueued)
+  bool grow_wait_next = false;         // an append kernel was enqueued beside the previous attention launch
   int last_attn_ctas = 0;
   std::string err;
 };
@@ -210,6 +212,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   c->cap_csa.assign(B, 0);
   c->ncand_cur.assign(B, 0);
   c->ncand_nxt.assign(B, 0);
+  c->grow_count.assign(B, 0u);
   if (c->growth && k < 3) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "a growing context needs k >= 3 (two table slots belong to the decode tier)");
   if (c->growth) LSA_CUDA(c, cudaEventCreateWithFlags(&c->ev_roll, cudaEventDisableTiming));
   long long sum_k = 0, total_keys_max = 0, n_keys_max = 0;
@@ -624,7 +627,10 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
         q_.w_len = c->seq_host[b].w_len;
         q_.app_slot = app ? (c->w_head[b] == 0 ? c->cfg.W - 1 : c->w_head[b] - 1) : -1;
         q_.app_count = app ? c->app_count[b] - 1u : c->app_count[b];
+        q_.grow_count = c->grow_count[b];
       }
+      stp.grow_wait = c->grow_wait_next ? 1 : 0;
+      c->grow_wait_next = false;
       stp.swap = pre ? pre->swap[0] : 0u;
       stp.k_new = app ? pre->k_new : nullptr;
       stp.v_new = app ? pre->v_new : nullptr;
@@ -1103,15 +1109,27 @@ extern "C" int lsa_append_compressed(lsa_ctx* ctx, const int32_t* seq_ids, int32
     LSA_CUDA(c, cudaEventRecord(c->ev_roll, c->sf));
     LSA_CUDA(c, cudaStreamWaitEvent(c->sc, c->ev_roll, 0));
   }
+  // Independent steps on the small-batch path: an append that only writes rows (no table entry, no new candidate) runs
+  // BESIDE the previous attention launch - nothing in flight reads those rows unmasked - and the next launch waits for
+  // SeqDev::grow_epoch instead of for the stream.  Everything else is stream-ordered (the next launch does not start early).
+  const bool beside = !roll && c->cfg.step_overlap && c->attn_impl == LSA_ATTN_TCGEN05 && tc_small_supported(c->tc) && !c->no_small &&
+                      !c->serialize_next && c->prof_cap == 0;
   for (int off = 0; off < n; off += kFireMax) {
     AppendList list{};
     list.n = std::min(kFireMax, n - off);
-    for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[off + i];
+    for (int i = 0; i < list.n; ++i) {
+      const int b = seq_ids[off + i];
+      list.ids[i] = b;
+      list.n_csa[i] = c->seq_host[b].n_csa;
+      list.n_hca[i] = c->seq_host[b].n_hca;
+      list.epoch[i] = ++c->grow_count[b];
+    }
     LSA_CUDA(c, launch_append_compressed(c->cfg.dtype, c->d_seqs, c->pool, c->cfg.hot_pool, list, off, csa_k, csa_v, hca_k, hca_v, emb_rows,
-                                         c->cfg.D, c->cfg.E, C, c->k, c->k_sel, c->page_bytes, c->sc));
+                                         c->cfg.D, c->cfg.E, C, c->k, c->k_sel, c->page_bytes, c->sc, beside));
     c->attn_launches += 1;
   }
-  c->serialize_next = true;                          // the next attention launch reads what these kernels wrote
+  if (beside) c->grow_wait_next = true;
+  else c->serialize_next = true;                     // the next attention launch reads what these kernels wrote
   if (any_done) {
     LSA_CUDA(c, cudaEventRecord(c->ev_compute, c->sc));
     LSA_CUDA(c, cudaStreamWaitEvent(c->sf, c->ev_compute, 0));

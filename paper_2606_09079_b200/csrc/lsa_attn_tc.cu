@@ -568,6 +568,7 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
     const TcSmallSeq& h = step.seq[b];
     SmSeq& d = prm.seq[b];
     d.n_hca = s.n_hca; d.cur = h.cur; d.n_cur = h.n_cur; d.w_len = h.w_len; d.app_slot = h.app_slot; d.app_count = h.app_count;
+    d.grow_count = h.grow_count;
     d.n_csa = s.n_csa;
     halves += (s.n_hca + kSmHalf - 1) / kSmHalf + 2 * (h.n_cur >= 0 ? h.n_cur : s.k_eff) + (h.w_len + kSmHalf - 1) / kSmHalf;
   }
@@ -601,6 +602,7 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   prm.k_new = (const __nv_bfloat16*)step.k_new; prm.v_new = (const __nv_bfloat16*)step.v_new;
   prm.ktime = ktime;
   prm.wait_inputs = step.wait_inputs;
+  prm.grow_wait = step.grow_wait;
   prm.in_ctr = step.in_ctr; prm.in_need = step.in_need;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

@@ -45,6 +45,7 @@ struct TcSmallSeq {
   int w_len;                // attended ring rows, this launch's append included
   int app_slot;             // ring slot written by this launch, or -1
   unsigned int app_count;   // appends enqueued before this launch
+  unsigned int grow_count;  // lsa_append_compressed calls enqueued for the sequence before this launch
 };
 struct TcSmallStep {
   TcSmallSeq seq[4];
@@ -56,6 +57,7 @@ struct TcSmallStep {
   int wait_inputs;          // 1: q / k_new / v_new may have been produced by the kernel just before this launch
   const unsigned int* in_ctr;   // q / k_new / v_new are complete once *in_ctr has reached in_need (null: see wait_inputs)
   unsigned int in_need;
+  int grow_wait;            // 1: an append kernel runs beside the previous launch: wait for grow_count before HCA / page rows
   int alone;                // 1: the caller blocks on this step (no neighbour launch to share the SMs with): use them all
   unsigned int* host_flag;  // PINNED HOST word (device alias) set to host_flag_val when `out` is complete, or null
   unsigned int host_flag_val;

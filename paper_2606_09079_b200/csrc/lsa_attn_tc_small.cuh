@@ -51,6 +51,7 @@ struct SmSeq {
   int w_len;                // attended ring rows, this launch's append included
   int app_slot;             // ring slot this launch writes k_new / v_new to, or -1
   unsigned int app_count;   // appends enqueued before this launch: SeqDev::app_epoch reaches it before ring rows are read
+  unsigned int grow_count;  // lsa_append_compressed calls enqueued before this launch (SeqDev::grow_epoch), see grow_wait
   long long n_csa;
 };
 
@@ -83,6 +84,8 @@ struct SmParams {
   int W;                         // ring capacity
   const __nv_bfloat16* k_new;    // [B][D] or null
   const __nv_bfloat16* v_new;
+  int grow_wait;                 // 1: an append kernel (lsa_append_compressed) runs beside the previous launch: HCA / page rows
+                                 // are read only after SeqDev::grow_epoch has reached seq[b].grow_count
   int wait_inputs;               // 1: griddepcontrol.wait before q / k_new / v_new are read
   const unsigned int* in_ctr;    // lsa_step_host_async: q / k_new / v_new are staged by a gather kernel that runs beside the
   unsigned int in_need;          // previous step; they are complete once this counter (its finished blocks) reaches in_need
@@ -375,7 +378,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     {
       SubCursor c0(sm, p.B, cta, n_cta);
       SubTile s0;
-      const bool early = c0.next(s0) && s0.kind == 0;
+      const bool early = c0.next(s0) && s0.kind == 0 && !p.grow_wait;
       if (lane == 0) sm.k0_early = early ? 1 : 0;
       if (early && elect_one()) {
         const uint64_t pol = l2_policy_evict_first();
@@ -410,10 +413,13 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         // window rows in the range: ring rows appended by earlier launches are visible once app_epoch has caught
         // up with the host's count (normally it has)
         if (lane == b && f1 > base + pg_b && f0 < end_b) wait_counter(&p.seqs[b].app_epoch, q.app_count, 50);
+        // HCA / tail-page rows handed over by an append kernel that runs beside the previous launch
+        if (p.grow_wait && lane == b && f0 < end_b && f1 > end_b - g_b) wait_counter(&p.seqs[b].grow_epoch, q.grow_count, 57);
         if (b > 0 && f0 < end_b && f1 > end_b - g_b && lane < 8) prefetch_tmap(p.seq_maps + b * 8 + lane);
       }
     }
     if (lane == 0) sm.pg_cnt = min(cnt, 32);
+    if (p.grow_wait) fence_proxy_async_all();          // the rows were written by generic stores, TMA reads them
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm.setup);
   } else if (warp == 1) {

@@ -36,6 +36,7 @@ struct SeqDev {
   // -- growth (lsa_append_compressed, DESIGN R29-R33); static contexts: cap_hca = n_hca, tier_page0 = -1 --
   int cap_hca;             // rows hca_k / hca_v can hold (tensor maps are made over this many)
   int tier_page0;          // first of this sequence's two reserved hot-pool pages, or -1
+  unsigned int grow_epoch; // lsa_append_compressed calls applied to this sequence so far (released after the rows are written)
   unsigned int app_epoch;  // ring rows appended so far; bumped with release semantics AFTER the row is written, so a
                            // launch that does not wait for its predecessor (lsa_attn_tc_small.cuh) can order its reads
 };

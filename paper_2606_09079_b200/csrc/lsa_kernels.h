@@ -35,10 +35,16 @@ cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, c
                              int B, int k, int P, long long page_bytes, cudaStream_t st, int k_cap = 0, int C = 0);
 // NEXT-4 (second half): one block per listed sequence writes the handed-over CSA / HCA entries and, when a chunk completes
 // or a new tail chunk starts, updates the records and page tables (lsa_residency.cu: append_compressed_kernel)
-struct AppendList { int n; int ids[kFireMax]; };
+struct AppendList {
+  int n;
+  int ids[kFireMax];
+  long long n_csa[kFireMax];      // host mirrors BEFORE the call: the kernel does not depend on an earlier append having landed
+  int n_hca[kFireMax];
+  unsigned int epoch[kFireMax];   // value released to SeqDev::grow_epoch once the rows are written
+};
 cudaError_t launch_append_compressed(int dtype, SeqDev* seqs, PoolDev pool, void* hot_pool, const AppendList& list, int row0,
                                      const void* csa_k, const void* csa_v, const void* hca_k, const void* hca_v, const void* emb_rows,
-                                     int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st);
+                                     int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st, bool beside_previous);
 cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas,
                          cudaStream_t st);
 // NEXT-4: copy `bytes` (multiple of 16) from device memory into the mapped pinned cold pool

@@ -323,11 +323,12 @@ append_compressed_kernel(SeqDev* __restrict__ seqs, PoolDev pool, unsigned char*
   const int b = list.ids[blockIdx.x], row = row0 + blockIdx.x;
   SeqDev& sq = seqs[b];
   constexpr int V = Elem<T>::kVec;
-  const long long n = sq.n_csa;
+  const long long n = list.n_csa[blockIdx.x];
+  const int n_hca = list.n_hca[blockIdx.x];
   const int c = (int)(n / C), i = (int)(n % C);
   if (hca_k) {
-    T* kd = reinterpret_cast<T*>(const_cast<void*>(sq.hca_k)) + (size_t)sq.n_hca * D;
-    T* vd = reinterpret_cast<T*>(const_cast<void*>(sq.hca_v)) + (size_t)sq.n_hca * D;
+    T* kd = reinterpret_cast<T*>(const_cast<void*>(sq.hca_k)) + (size_t)n_hca * D;
+    T* vd = reinterpret_cast<T*>(const_cast<void*>(sq.hca_v)) + (size_t)n_hca * D;
     for (int d = threadIdx.x * V; d < D; d += blockDim.x * V) {
       *reinterpret_cast<uint4*>(kd + d) = *reinterpret_cast<const uint4*>(hca_k + (size_t)row * D + d);
       *reinterpret_cast<uint4*>(vd + d) = *reinterpret_cast<const uint4*>(hca_v + (size_t)row * D + d);
@@ -348,9 +349,11 @@ append_compressed_kernel(SeqDev* __restrict__ seqs, PoolDev pool, unsigned char*
         *reinterpret_cast<uint4*>(ed + e) = *reinterpret_cast<const uint4*>(emb_rows + (size_t)row * E + e);
     }
   }
+  asm volatile("fence.proxy.async;" ::: "memory");   // the rows are read by TMA (async proxy) in later launches
+  __threadfence();
   __syncthreads();
   if (threadIdx.x == 0) {
-    if (hca_k) sq.n_hca += 1;
+    if (hca_k) sq.n_hca = n_hca + 1;
     if (csa_k) {
       if (i == 0) {                             // a new tail chunk: listed after everything else (its id is the largest)
         const int cur = sq.cur_buf;
@@ -371,13 +374,20 @@ append_compressed_kernel(SeqDev* __restrict__ seqs, PoolDev pool, unsigned char*
         sq.k_eff = min(k_sel, c + 1);
       }
     }
+    // a launch that runs beside this kernel (lsa_attn_tc_small.cuh, grow_wait) reads the rows only after this
+    __threadfence();
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&sq.grow_epoch), "r"(list.epoch[blockIdx.x]) : "memory");
   }
 }
 
 cudaError_t launch_append_compressed(int dtype, SeqDev* seqs, PoolDev pool, void* hot_pool, const AppendList& list, int row0,
                                      const void* csa_k, const void* csa_v, const void* hca_k, const void* hca_v, const void* emb_rows,
-                                     int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st) {
+                                     int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st, bool beside_previous) {
   unsigned char* hp = reinterpret_cast<unsigned char*>(hot_pool);
+  if (beside_previous && dtype != 0)          // no griddepcontrol.wait inside: it touches nothing a launch in flight reads unmasked
+    return launch_pdl(append_compressed_kernel<__nv_bfloat16>, dim3(list.n), dim3(128), 0, st, seqs, pool, hp, list, row0,
+                      (const __nv_bfloat16*)csa_k, (const __nv_bfloat16*)csa_v, (const __nv_bfloat16*)hca_k, (const __nv_bfloat16*)hca_v,
+                      (const __nv_bfloat16*)emb_rows, D, E, C, k, k_sel, page_bytes);
   if (dtype == 0)
     append_compressed_kernel<float><<<list.n, 128, 0, st>>>(seqs, pool, hp, list, row0, (const float*)csa_k, (const float*)csa_v,
                                                             (const float*)hca_k, (const float*)hca_v, (const float*)emb_rows, D, E,
