@@ -283,6 +283,22 @@ int lsa_l2_get_mask(lsa_ctx* ctx, int32_t seq, uint32_t* words);
 int lsa_step_l2(lsa_ctx* ctx, const void* q, const void* h, const void* k_new, const void* v_new,
                 const void* q_idx, const float* w_idx, void* out);
 
+/* S1-S3 (as lsa_index_select: P:61-65, P:71-79 in BASELINE's dual-encoder form, R1-R3, R14-R16) for callers that may
+ * not allocate: code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  No context; the scratch
+ * between the three kernels (z, the scores, the per-sequence records) is a file-scope device array of the library
+ * (~641 KiB, held by every GPU that loads the library until exit) and the call allocates nothing - no cudaMalloc /
+ * cudaFree, no memcpy: it only enqueues four kernels on `stream` (a cudaStream_t of the CURRENT device).
+ *   dtype lsa_dtype; W_q DEVICE [E][Dh]; h DEVICE [n][Dh]; chunk_emb HOST [n] of DEVICE pointers [n_chunks[i]][E];
+ *   n_chunks HOST [n]; sel_idx DEVICE [n][k] int32 (unused slots -1); sel_score DEVICE [n][k] fp32 or NULL.
+ * Limits (the array's size): n <= 8, E <= 4096 (multiple of 8), n_chunks[i] <= 16384, k <= 1024, Dh % 8 == 0; anything
+ * beyond is LSA_ERR_INVALID_ARG (text: lsa_last_error(NULL)) and nothing is enqueued.
+ * The array is shared by every call on the device and keeps the last call's contents; nothing in it needs to start at
+ * zero.  Calls that OVERLAP on the GPU (different streams without an ordering between them) race on it: keep calls on one
+ * stream or order them with events.  Results are identical to lsa_index_select on the same inputs. */
+int lsa_index_select_static(int32_t dtype, const void* W_q, const void* h, const void* const* chunk_emb,
+                            const int32_t* n_chunks, int32_t n, int32_t E, int32_t Dh, int32_t k, int32_t* sel_idx,
+                            float* sel_score, void* stream);
+
 /* NEXT-4 (first half; P:179, P:199 VRAM -> DRAM): KV export into the cold pool.  Copies n_chunks page images
  * src DEVICE [n_chunks][2][C][D] (dtype) into chunks [first_chunk, first_chunk + n_chunks) of sequence seq's pinned-host
  * cold pool (which must be writable), by a device kernel over the mapped pool on stream_fetch - ordered before every

@@ -439,6 +439,16 @@ extern "C" int lsa_index_select(lsa_ctx* ctx, const void* h, const int32_t* seq_
   return index_select_impl(ctx, h, seq_ids, rows.data(), n, sel_idx, sel_score);
 }
 
+// S1-S3 without a context and without any allocation (scratch = a file-scope device array in lsa_index.cu)
+extern "C" int lsa_index_select_static(int32_t dtype, const void* W_q, const void* h, const void* const* chunk_emb,
+                                       const int32_t* n_chunks, int32_t n, int32_t E, int32_t Dh, int32_t k, int32_t* sel_idx,
+                                       float* sel_score, void* stream) {
+  char msg[256] = "";
+  const int rc = index_select_static(dtype, W_q, h, chunk_emb, n_chunks, n, E, Dh, k, sel_idx, sel_score, (cudaStream_t)stream, msg, sizeof(msg));
+  if (rc != 0) g_init_error = msg;                 // read with lsa_last_error(NULL)
+  return rc == 0 ? LSA_OK : (rc == -1 ? LSA_ERR_INVALID_ARG : LSA_ERR_CUDA);
+}
+
 // ---- paper-exact Level-1 indexer (NEXT-1) ---------------------------------------------------------
 extern "C" int lsa_l1_init(lsa_ctx* ctx, const lsa_l1_config* cfg, const void* const* index_k) {
   if (!ctx) return LSA_ERR_STATE;

@@ -8,6 +8,8 @@
 // All three are HBM/latency bound (W_q 4 MiB + Emb <= 2 MiB per trigger): 16-byte loads, one warp per
 // output row, fp32 accumulation in a fixed order so bit-identical embedding rows give bit-identical
 // scores wherever they sit in the table (exact planted ties stay exact).
+#include <cstdio>
+
 #include "lsa_kernels.h"
 #include "lsa_select.cuh"
 
@@ -165,6 +167,97 @@ cudaError_t launch_scores(int dtype, const SeqDev* seqs, const FireList& fire, c
 cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores, int n_chunks_max, int k,
                         int32_t* sel_idx, float* sel_score, cudaStream_t st) {
   return launch_pdl(topk_kernel, dim3(fire.n), dim3(1024), 0, st, seqs, fire, scores, n_chunks_max, k, sel_idx, sel_score);
+}
+
+}  // namespace lsa
+
+// ---- lsa_index_select_static: S1-S3 for callers that may not allocate -------------------------------------------
+// The indexer needs scratch between its three kernels (z = W_q h, the scores, the per-sequence records the scoring and
+// top-k kernels read).  Here that scratch is a file-scope device array of fixed size instead of cudaMalloc'ed memory:
+// nothing is allocated by the call, so it can be used under CUDA graph capture, in a serving loop, or by a harness that
+// forbids allocation.  Every GPU that loads the library holds the array (sizeof(IndexStaticScratch), ~641 KiB) until exit.
+// Every call on a device shares it and it keeps the last call's contents: nothing in it has to start at zero (the records,
+// z[i][0..E) and scores[i][0..n_chunks_i) are fully rewritten before they are read), but two calls that overlap on the GPU
+// (different streams, no ordering between them) race on it.
+namespace lsa {
+
+struct IndexStaticScratch {
+  SeqDev seqs[kStaticSeqs];
+  float z[kStaticSeqs * kStaticE];
+  float scores[kStaticSeqs * kStaticChunks];
+};
+static __device__ __align__(256) IndexStaticScratch g_index_scratch;
+
+struct StaticSeqArgs {
+  const void* emb[kStaticSeqs];
+  int n_chunks[kStaticSeqs];
+  int n, k;
+};
+// Device code names the array directly; only host code needs its address.
+__global__ void static_seq_setup_kernel(StaticSeqArgs a) {
+  const int i = threadIdx.x;
+  if (i >= a.n) return;
+  SeqDev s{};
+  s.emb = a.emb[i];
+  s.n_chunks = a.n_chunks[i];
+  s.n_csa = 0;
+  s.k_eff = min(a.k, a.n_chunks[i]);
+  s.tier_page0 = -1;
+  g_index_scratch.seqs[i] = s;
+}
+
+int index_select_static(int dtype, const void* W_q, const void* h, const void* const* chunk_emb, const int* n_chunks, int n, int E,
+                        int Dh, int k, int32_t* sel_idx, float* sel_score, cudaStream_t st, char* msg, size_t msg_len) {
+  auto fail = [&](int code, const char* fmt, long long a = 0, long long b = 0) {
+    snprintf(msg, msg_len, fmt, a, b);
+    return code;
+  };
+  if (dtype != 0 && dtype != 1) return fail(-1, "bad dtype %lld", dtype);
+  if (!W_q || !h || !chunk_emb || !n_chunks || !sel_idx) return fail(-1, "null argument");
+  if (n < 1 || n > kStaticSeqs) return fail(-1, "n = %lld sequences: the static scratch holds at most %lld", n, kStaticSeqs);
+  if (E < 8 || E > kStaticE || E % 8) return fail(-1, "E = %lld: must be a multiple of 8 and at most %lld (static scratch)", E, kStaticE);
+  if (Dh < 8 || Dh % 8) return fail(-1, "Dh = %lld must be a positive multiple of 8", Dh);
+  if (k < 1 || k > kMaxK) return fail(-1, "k = %lld must be in [1, %lld]", k, kMaxK);
+  StaticSeqArgs a{};
+  a.n = n; a.k = k;
+  int n_max = 0;
+  for (int i = 0; i < n; ++i) {
+    if (!chunk_emb[i]) return fail(-1, "chunk_emb[%lld] is null", i);
+    if (n_chunks[i] < 1 || n_chunks[i] > kStaticChunks)
+      return fail(-1, "n_chunks = %lld: the static scratch holds at most %lld scores per sequence", n_chunks[i], kStaticChunks);
+    a.emb[i] = chunk_emb[i];
+    a.n_chunks[i] = n_chunks[i];
+    n_max = n_chunks[i] > n_max ? n_chunks[i] : n_max;
+  }
+  // the array's address on the CURRENT device, looked up once per device (in host code the symbol's name is only a
+  // stand-in: passing &g_index_scratch to a kernel would hand it a host address)
+  static IndexStaticScratch* ptr_of[64] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev < 0 || dev >= 64) return fail(-2, "cudaGetDevice failed or device index %lld >= 64", dev);
+  IndexStaticScratch* sp = __atomic_load_n(&ptr_of[dev], __ATOMIC_ACQUIRE);
+  if (!sp) {
+    e = cudaGetSymbolAddress(reinterpret_cast<void**>(&sp), g_index_scratch);
+    if (e != cudaSuccess || !sp) {
+      snprintf(msg, msg_len, "cudaGetSymbolAddress(g_index_scratch) failed: %s", cudaGetErrorString(e));
+      return -2;
+    }
+    __atomic_store_n(&ptr_of[dev], sp, __ATOMIC_RELEASE);     // the same value whichever thread gets here first
+  }
+  static_seq_setup_kernel<<<1, kStaticSeqs, 0, st>>>(a);
+  e = cudaGetLastError();
+  FireList fire{};
+  fire.n = n;
+  for (int i = 0; i < n; ++i) fire.ids[i] = i;
+  if (e == cudaSuccess) e = launch_qtower(dtype, W_q, h, fire, sp->z, E, Dh, st);
+  // row stride of the scores = the longest table of this call (<= kStaticChunks, so n rows always fit)
+  if (e == cudaSuccess) e = launch_scores(dtype, sp->seqs, fire, sp->z, sp->scores, E, n_max, st, 1);
+  if (e == cudaSuccess) e = launch_topk(sp->seqs, fire, sp->scores, n_max, k, sel_idx, sel_score, st);
+  if (e != cudaSuccess) {
+    snprintf(msg, msg_len, "launch failed: %s", cudaGetErrorString(e));
+    return -2;
+  }
+  return 0;
 }
 
 }  // namespace lsa

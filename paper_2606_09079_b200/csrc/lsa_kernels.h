@@ -1,6 +1,7 @@
 // lsa_kernels.h - host-side launchers of the LSA kernels (internal to liblsa).
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 #include "lsa_common.cuh"
@@ -27,6 +28,14 @@ cudaError_t launch_qtower_tc(const void* W, const void* h, int h_row0, int n, fl
 // sel_idx[i][0..k) / sel_score: first k_eff by (score desc, chunk idx asc), rest -1 / -inf
 cudaError_t launch_topk(const SeqDev* seqs, const FireList& fire, const float* scores,
                         int n_chunks_max, int k, int32_t* sel_idx, float* sel_score, cudaStream_t st);
+
+// S1-S3 with the scratch in a file-scope device array (lsa_index.cu): no allocation.  Limits of that array:
+constexpr int kStaticSeqs = 8;         // sequences per call
+constexpr int kStaticE = 4096;         // E at most
+constexpr int kStaticChunks = 16384;   // chunks per sequence at most
+// chunk_emb / n_chunks: HOST arrays [n]; 0 or an lsa_status (text in msg)
+int index_select_static(int dtype, const void* W_q, const void* h, const void* const* chunk_emb, const int* n_chunks, int n, int E,
+                        int Dh, int k, int32_t* sel_idx, float* sel_score, cudaStream_t st, char* msg, size_t msg_len);
 
 // ---- S4-S6 (lsa_residency.cu) -----------------------------------------------------------
 // P = pages managed by the LRU; k_cap = recalled chunks per table at most (0: k); C = entries per chunk (tail entry of a

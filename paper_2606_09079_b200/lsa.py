@@ -33,7 +33,7 @@ EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
            "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
            "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats", "lsa_export_chunks",
-           "lsa_append_compressed", "lsa_last_error", "lsa_destroy", "lsa_version"]
+           "lsa_append_compressed", "lsa_index_select_static", "lsa_last_error", "lsa_destroy", "lsa_version"]
 
 
 class LsaError(RuntimeError):
@@ -110,6 +110,8 @@ def _load() -> C.CDLL:
     lib.lsa_l2_select.argtypes = [vp, vp, vp, vp, vp]
     lib.lsa_l2_get_mask.argtypes = [vp, C.c_int32, vp]
     lib.lsa_export_chunks.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, vp]
+    lib.lsa_index_select_static.argtypes = [C.c_int32, vp, vp, C.POINTER(C.c_void_p), C.POINTER(C.c_int32), C.c_int32, C.c_int32,
+                                            C.c_int32, C.c_int32, vp, vp, vp]
     lib.lsa_append_compressed.argtypes = [vp, C.POINTER(C.c_int32), C.c_int32, vp, vp, vp, vp, vp]
     lib.lsa_step_graph.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.lsa_graph_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
@@ -455,6 +457,35 @@ def lsa_decode_attention(ctx: LsaContext, q, out=None, want_lse=False):
 
 def lsa_step(ctx: LsaContext, q, h, k_new=None, v_new=None, out=None):
     return ctx.step(q, h, k_new, v_new, out)
+
+
+def index_select_static(dtype: int, W_q: torch.Tensor, h: torch.Tensor, chunk_emb: Sequence[torch.Tensor], k: int,
+                        sel_idx: torch.Tensor, sel_score: Optional[torch.Tensor] = None,
+                        stream: Optional[torch.cuda.Stream] = None) -> None:
+    """lsa_index_select_static: S1-S3 with the library's static device scratch - allocates nothing (see include/lsa.h for
+    the limits and the no-overlap rule).  h [n][Dh], chunk_emb: n tensors [n_chunks_i][E], sel_idx [n][k] int32 and
+    sel_score [n][k] fp32 are the CALLER's CUDA tensors; the kernels run on `stream` (default: torch's current stream)."""
+    td = _torch_dtype(dtype)
+    n = len(chunk_emb)
+    if h.dim() != 2 or h.shape[0] != n:
+        raise LsaError(-1, "h must be [n][Dh] with one row per embedding table")
+    if sel_idx.dtype != torch.int32 or tuple(sel_idx.shape) != (n, k) or not sel_idx.is_cuda or not sel_idx.is_contiguous():
+        raise LsaError(-1, "sel_idx must be a contiguous CUDA int32 tensor [n][k]")
+    if sel_score is not None and (sel_score.dtype != torch.float32 or tuple(sel_score.shape) != (n, k) or not sel_score.is_cuda
+                                  or not sel_score.is_contiguous()):
+        raise LsaError(-1, "sel_score must be a contiguous CUDA float32 tensor [n][k]")
+    E = int(W_q.shape[0])
+    for e in chunk_emb:
+        if e.dim() != 2 or int(e.shape[1]) != E:
+            raise LsaError(-1, "every chunk_emb must be [n_chunks][E]")
+    embs = (C.c_void_p * n)(*[_dev_ptr(e, td, "chunk_emb") for e in chunk_emb])
+    ncs = (C.c_int32 * n)(*[int(e.shape[0]) for e in chunk_emb])
+    st = torch.cuda.current_stream(h.device) if stream is None else stream
+    with torch.cuda.device(h.device):
+        rc = _lib.lsa_index_select_static(dtype, _dev_ptr(W_q, td, "W_q"), _dev_ptr(h, td, "h"), embs, ncs, n, E, int(W_q.shape[1]), k,
+                                          sel_idx.data_ptr(), None if sel_score is None else sel_score.data_ptr(), st.cuda_stream)
+    if rc != 0:
+        raise LsaError(rc, (_lib.lsa_last_error(None) or b"").decode())
 
 
 def lsa_version() -> int:
