@@ -153,7 +153,10 @@ class ResidencyOracle:
     copied from the cold pool.  nxt[b] = [(c, page)] in ascending c (R13)."""
 
     def __init__(self, n_seqs: int, n_chunks: Sequence[int], hot_pages: int,
-                 cold: Optional[Sequence[np.ndarray]] = None):
+                 cold: Optional[Sequence[np.ndarray]] = None, cold_page_nbytes: Optional[int] = None):
+        """cold_page_nbytes: bytes one page occupies in the cold pool when that differs from the hot image (FP8 cold pages,
+        DESIGN R34: `cold` then holds the DEQUANTISED page images, which is what a recall writes into the hot pool)."""
+        self.cold_page_nbytes = cold_page_nbytes
         self.P = int(hot_pages)
         self.owner: List[Optional[Tuple[int, int]]] = [None] * self.P
         self.last_used = [0] * self.P
@@ -211,7 +214,7 @@ class ResidencyOracle:
             fetch_list.append((c, p))
             if self.hot is not None:
                 self.hot[p] = self.cold[b][c]   # byte copy of one page
-                self.bytes_fetched += self.cold[b][c].nbytes
+                self.bytes_fetched += self.cold_page_nbytes or self.cold[b][c].nbytes
         self.nxt[b] = [(c, self.page_of[b][c]) for c in sel_up]
         self.visible_at[b] = step_b + recall_lag
         return fetch_list
@@ -246,7 +249,7 @@ class LsaOracle:
                  cold_csa: Sequence[np.ndarray], n_csa: Sequence[int],
                  chunk_emb: Sequence[np.ndarray], hca_k, hca_v, win_k, win_v,
                  w_len: Sequence[int], w_head: Sequence[int], step0: Sequence[int],
-                 sm_scale: float = 0.0):
+                 sm_scale: float = 0.0, cold_page_nbytes: Optional[int] = None):
         self.dtype, self.H, self.D, self.C, self.W = dtype, H, D, C, W
         self.k, self.tau, self.recall_lag = k, tau, recall_lag
         self.sm_scale = sm_scale if sm_scale > 0 else 1.0 / math.sqrt(D)
@@ -261,7 +264,7 @@ class LsaOracle:
         self.win_v = [x.copy() for x in win_v]
         self.w_len, self.w_head = list(w_len), list(w_head)
         self.step = [int(s) for s in step0]
-        self.pool = ResidencyOracle(self.B, self.n_chunks, hot_pages, self.cold)
+        self.pool = ResidencyOracle(self.B, self.n_chunks, hot_pages, self.cold, cold_page_nbytes)
 
     # -- S1-S3 ---------------------------------------------------------------------------
     def scores(self, b: int, h_b: np.ndarray) -> np.ndarray:

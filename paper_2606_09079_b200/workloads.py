@@ -568,3 +568,50 @@ class GrowthInputs:
         else:
             row = _unit_rows(r)
         return store(row[0].astype(np.float32), c.dtype)
+
+
+# --------------------------------------------------------------------------------------
+# FP8 cold pool (NEXT-4 "FP8 KV pages", the host-link half): seeded e4m3 CODES and block scales.  Inputs only - the
+# generator draws bytes, it never encodes or decodes a value (that arithmetic is the kernels' and the oracle's).
+# --------------------------------------------------------------------------------------
+class Fp8ColdInputs:
+    """Per sequence: codes uint8 [n_chunks][2][C][D] and scales float32 [n_chunks][2] (K block, V block).
+
+    A code byte is sign(1) | exponent(4) | mantissa(3).  Bytes are drawn so that the decoded magnitudes look like what a
+    quantiser leaves of Gaussian rows: exponent fields concentrated in the top binades (field 15 - g, g geometric with
+    p = 1/2, clipped at 0 = subnormals), uniform mantissa and sign; the NaN pattern (field 15, mantissa 7) is redrawn as
+    mantissa 6.  Scales are powers of two 2^(-12 - (c mod 3)) (magnitudes around 1/sqrt(D) for D = 512), different per
+    chunk and block so that a wrong scale index shows.  cfg 4/5-sized pools tile a base block like LsaWorkload does."""
+
+    def __init__(self, wl: "LsaWorkload", tag: int = 1400):
+        c = wl.cfg
+        self.codes: List[np.ndarray] = []
+        self.scales: List[np.ndarray] = []
+        base = None
+        if c.kv_base_chunks > 0:
+            base = self._draw(_rng(c.seed, tag, 0), (c.kv_base_chunks, 2, c.C, c.D))
+        for b in range(c.B):
+            nch, gb = c.n_chunks(b), b + c.seq_offset
+            if base is None:
+                codes = self._draw(_rng(c.seed, tag, 1, gb), (nch, 2, c.C, c.D))
+            else:
+                idx = (np.arange(nch, dtype=np.int64) * 7 + 13 * gb) % c.kv_base_chunks
+                codes = base[idx].copy()
+                codes[:, 0, 0, 0] = (np.arange(nch) % 120 + 1).astype(np.uint8)      # a unique tag per chunk (a wrong copy shows)
+            tail = nch * c.C - c.n_csa(b)
+            if tail:
+                codes[nch - 1, :, c.C - tail:, :] = 0                               # rows past n_csa: zero
+            sc = np.empty((nch, 2), dtype=np.float32)
+            sc[:, 0] = 2.0 ** (-12.0 - (np.arange(nch) % 3))
+            sc[:, 1] = 2.0 ** (-12.0 - ((np.arange(nch) + 1) % 3))
+            self.codes.append(codes)
+            self.scales.append(sc)
+
+    @staticmethod
+    def _draw(g: np.random.Generator, shape) -> np.ndarray:
+        n = int(np.prod(shape))
+        expo = 15 - np.minimum(g.geometric(0.5, size=n) - 1, 15)
+        mant = g.integers(0, 8, size=n)
+        mant = np.where((expo == 15) & (mant == 7), 6, mant)
+        sign = g.integers(0, 2, size=n)
+        return ((sign << 7) | (expo << 3) | mant).astype(np.uint8).reshape(shape)
