@@ -39,7 +39,7 @@
 extern "C" {
 #endif
 
-#define LSA_VERSION 3
+#define LSA_VERSION 4
 
 typedef struct lsa_ctx lsa_ctx; /* opaque */
 
@@ -62,6 +62,15 @@ enum lsa_attn_impl { LSA_ATTN_AUTO = 0, LSA_ATTN_SIMT = 1, LSA_ATTN_TCGEN05 = 2 
  * attention kernel behind a grid-wide arrival counter: one launch per step; measured slower than KERNEL on
  * B200, kept as a tested alternative. */
 enum lsa_merge_mode { LSA_MERGE_AUTO = 0, LSA_MERGE_KERNEL = 1, LSA_MERGE_FUSED = 2 };
+
+/* Cold-pool page format (NEXT-4 "FP8 KV pages", the host-link half; R34-R36).  NATIVE: a cold page is the hot
+ * page image (dtype).  FP8_E4M3 (dtype must be LSA_BF16): a cold page is [2][C][D] e4m3 codes (1 byte each: sign, 4
+ * exponent bits with bias 7, 3 mantissa bits, no infinities, S.1111.111 = NaN which must not occur) and the sequence has
+ * one fp32 scale per block in lsa_seq_desc.cold_scale.  S5 dequantises while it copies: hot element = bf16_rne(fp32(code)
+ * * scale) - exact when the scale is a power of two - so a recall moves HALF the bytes over the host link and everything
+ * behind it (hot pool, S7) is unchanged.  lsa_export_chunks quantises: per block e = exponent of the largest magnitude - 7,
+ * scale = 2^e, code = e4m3 round-to-nearest-even of x * 2^-e (all-zero block: scale 1); it writes codes and scales. */
+enum lsa_cold_format { LSA_COLD_NATIVE = 0, LSA_COLD_FP8_E4M3 = 1 };
 
 /* Shape and resources of one LSA layer shared by B sequences (BJ configs). */
 typedef struct lsa_config {
@@ -91,12 +100,15 @@ typedef struct lsa_config {
                          /* the previous step's S8 instead of after it              */
   int32_t max_ctas;      /* 0 -> one split-K wave sized from the SM count                       */
   int32_t merge_mode;    /* lsa_merge_mode: where S8 runs (tcgen05 path)                        */
+  int32_t cold_format;   /* lsa_cold_format: how a page is stored in the cold pool (host link)  */
+  int32_t reserved0;
 } lsa_config;
 
 /* One sequence (CPU cold mirror + always-resident tiers).  n_chunks = ceil(n_csa/C);
  * the last chunk may be partial: rows >= n_csa - c*C of it are never attended (R22). */
 typedef struct lsa_seq_desc {
-  const void* cold_csa;  /* PINNED HOST [n_chunks][2][C][D]: chunk c = one page image            */
+  const void* cold_csa;  /* PINNED HOST [n_chunks][2][C][D]: chunk c = one page image (dtype; or  */
+                         /* e4m3 codes, 1 byte each, with lsa_config.cold_format = FP8_E4M3)    */
   int64_t n_csa;         /* valid compressed (CSA) entries                                      */
   const void* chunk_emb; /* DEVICE [n_chunks][E], rows L2-normalised by the producer (R3)        */
   const void* hca_k;     /* DEVICE [n_hca][D] heavily-compressed (128:1) keys, always resident   */
@@ -113,6 +125,9 @@ typedef struct lsa_seq_desc {
    * sequence of a context grows or none does. */
   int64_t cap_csa;
   int64_t cap_hca;
+  /* LSA_COLD_FP8_E4M3 only: DEVICE [n_chunks][2] fp32, (K scale, V scale) of every cold page; positive, finite.  Read by S5,
+   * written by lsa_export_chunks.  NULL otherwise. */
+  void* cold_scale;
 } lsa_seq_desc;
 
 typedef struct lsa_stats {

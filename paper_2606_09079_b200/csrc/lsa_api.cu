@@ -29,6 +29,7 @@ struct lsa_ctx {
   int B = 0, k = 0;
   float sm_scale = 0.f;
   long long page_bytes = 0;
+  long long cold_page_bytes = 0;       // = page_bytes, or half of it with FP8 cold pages (lsa_config.cold_format)
   int elem = 0;
   cudaStream_t sc = nullptr, sf = nullptr;
   cudaEvent_t ev_fetch = nullptr, ev_compute = nullptr;
@@ -187,6 +188,10 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   c->k = k;
   c->elem = cfg->dtype == LSA_F32 ? 4 : 2;
   c->page_bytes = 2ll * C * D * c->elem;
+  const bool fp8_cold = cfg->cold_format == LSA_COLD_FP8_E4M3;
+  c->cold_page_bytes = fp8_cold ? 2ll * C * D : c->page_bytes;
+  if (fp8_cold && (cfg->dtype != LSA_BF16 || (C * (long long)D) % 16))
+    LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "FP8 cold pages need dtype = LSA_BF16 and C * D a multiple of 16");
   c->sm_scale = cfg->sm_scale > 0.f ? cfg->sm_scale : 1.0f / std::sqrt((float)D);
   c->sc = (cudaStream_t)cfg->stream_compute;
   c->sf = (cudaStream_t)cfg->stream_fetch;
@@ -218,6 +223,9 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   long long sum_k = 0, total_keys_max = 0, n_keys_max = 0;
   for (int b = 0; b < B; ++b) {
     const lsa_seq_desc& s = seqs[b];
+    if (fp8_cold && s.n_csa > 0 && !s.cold_scale) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: cold_scale is NULL with FP8 cold pages", b);
+    if (fp8_cold && s.cap_csa > 0)
+      LSA_FAIL(c, LSA_ERR_UNSUPPORTED, "a growing compressed history (cap_csa) with FP8 cold pages is not built");
     if ((s.cap_csa > 0) != c->growth) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: either every sequence grows (cap_csa > 0) or none", b);
     if (c->growth && (s.cap_csa < s.n_csa || s.cap_hca < s.n_hca || s.cap_hca > (1ll << 30)))
       LSA_FAIL(c, LSA_ERR_INVALID_ARG, "seq %d: cap_csa / cap_hca below n_csa / n_hca", b);
@@ -242,6 +250,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
       d.cold = at.devicePointer;
     }
     d.emb = s.chunk_emb;
+    d.cold_scale = fp8_cold ? static_cast<const float*>(s.cold_scale) : nullptr;
     d.hca_k = s.hca_k;
     d.hca_v = s.hca_v;
     d.win_k = s.win_k;
@@ -288,6 +297,7 @@ static int init_impl(lsa_ctx* c, const lsa_config* cfg, const lsa_seq_desc* seqs
   if ((rc = dev_alloc(c, &c->pool.tbl_page, (size_t)B * 2 * k))) return rc;
   if ((rc = dev_alloc(c, &c->pool.fetch_src, (size_t)B * k))) return rc;
   if ((rc = dev_alloc(c, &c->pool.fetch_page, (size_t)B * k))) return rc;
+  if (fp8_cold && (rc = dev_alloc(c, &c->pool.fetch_scale, (size_t)B * k))) return rc;
   if ((rc = dev_alloc(c, &c->pool.counters, 8))) return rc;
   if ((rc = dev_alloc(c, &c->pool.epoch, 1))) return rc;
   if (c->growth) {
@@ -374,6 +384,8 @@ extern "C" int lsa_init_pools(const lsa_config* cfg, const lsa_seq_desc* seqs, l
   if (cfg->hot_pages < 1) LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "hot_pages must be >= 1");
   if (cfg->merge_mode < LSA_MERGE_AUTO || cfg->merge_mode > LSA_MERGE_FUSED)
     LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad merge_mode");
+  if (cfg->cold_format != LSA_COLD_NATIVE && cfg->cold_format != LSA_COLD_FP8_E4M3)
+    LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "bad cold_format");
   if (cfg->step_overlap != 0 && cfg->step_overlap != 1)
     LSA_FAIL((lsa_ctx*)nullptr, LSA_ERR_INVALID_ARG, "step_overlap must be 0 or 1");
   lsa_ctx* c = new (std::nothrow) lsa_ctx();
@@ -522,12 +534,13 @@ static int fetch_impl(lsa_ctx* c, const int* ids, int n, const int32_t* sel_idx,
     for (int i = 0; i < m; ++i) fire.ids[i] = ids[off + i];
     {
       ProfScope prof(c, LSA_PH_RESIDENCY, c->sf);
+      // (the residency pass only uses the page size on the COLD side: source offsets and the byte counter)
       LSA_CUDA(c, launch_residency(c->d_seqs, c->pool, fire, sel_idx + (size_t)off * c->k, c->B, c->k, c->P_lru,
-                                   c->page_bytes, c->sf, c->k_sel, c->growth ? cfg.C : 0));
+                                   c->cold_page_bytes, c->sf, c->k_sel, c->growth ? cfg.C : 0));
     }
     {
       ProfScope prof(c, LSA_PH_FETCH, c->sf);
-      LSA_CUDA(c, launch_fetch(c->pool, cfg.hot_pool, c->page_bytes, c->fetch_ctas, c->sf));
+      LSA_CUDA(c, launch_fetch(c->pool, cfg.hot_pool, c->page_bytes, c->fetch_ctas, c->sf, c->cold_page_bytes));
     }
     c->index_launches += 2;
   }
@@ -1071,6 +1084,13 @@ extern "C" int lsa_export_chunks(lsa_ctx* ctx, int32_t seq, int32_t first_chunk,
     LSA_FAIL(c, LSA_ERR_INVALID_ARG, "chunks [%d, %d) outside the sequence's %d chunks", first_chunk, first_chunk + n_chunks, c->seq_host[seq].n_chunks);
   if (n_chunks == 0) return LSA_OK;
   if (!src) LSA_FAIL(c, LSA_ERR_INVALID_ARG, "null src");
+  if (c->cold_page_bytes != c->page_bytes) {       // FP8 cold pages: quantise; one block per (page, K | V block)
+    void* dst8 = const_cast<unsigned char*>(reinterpret_cast<const unsigned char*>(c->seq_host[seq].cold)) + (long long)first_chunk * c->cold_page_bytes;
+    float* sc = const_cast<float*>(c->seq_host[seq].cold_scale) + 2ll * first_chunk;
+    LSA_CUDA(c, launch_export_fp8(src, dst8, sc, 2ll * n_chunks, (long long)c->cfg.C * c->cfg.D, c->sf));
+    c->index_launches += 1;
+    return LSA_OK;
+  }
   const long long bytes = (long long)n_chunks * c->page_bytes;
   void* dst = const_cast<unsigned char*>(reinterpret_cast<const unsigned char*>(c->seq_host[seq].cold)) + (long long)first_chunk * c->page_bytes;
   const int ctas = (int)std::max<long long>(1, std::min<long long>(c->fetch_ctas > 0 ? c->fetch_ctas : 64, (bytes + 16383) / 16384));

@@ -36,6 +36,7 @@ struct SeqDev {
   // -- growth (lsa_append_compressed, DESIGN R29-R33); static contexts: cap_hca = n_hca, tier_page0 = -1 --
   int cap_hca;             // rows hca_k / hca_v can hold (tensor maps are made over this many)
   int tier_page0;          // first of this sequence's two reserved hot-pool pages, or -1
+  const float* cold_scale; // FP8 cold pool: [n_chunks][2] (K scale, V scale), else null
   unsigned int grow_epoch; // lsa_append_compressed calls applied to this sequence so far (released after the rows are written)
   unsigned int app_epoch;  // ring rows appended so far; bumped with release semantics AFTER the row is written, so a
                            // launch that does not wait for its predecessor (lsa_attn_tc_small.cuh) can order its reads
@@ -52,6 +53,7 @@ struct PoolDev {
   // fetch list of the current trigger launch
   const void** fetch_src;       // [B*k]
   int* fetch_page;              // [B*k]
+  const float** fetch_scale;    // [B*k] FP8 cold pool: the page's two block scales
   // scalars
   unsigned long long* counters; // [8]: tick, triggers, hits, misses, evictions, bytes, fetch_count, error
   unsigned int* epoch;

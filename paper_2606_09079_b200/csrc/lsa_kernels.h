@@ -54,8 +54,11 @@ struct AppendList {
 cudaError_t launch_append_compressed(int dtype, SeqDev* seqs, PoolDev pool, void* hot_pool, const AppendList& list, int row0,
                                      const void* csa_k, const void* csa_v, const void* hca_k, const void* hca_v, const void* emb_rows,
                                      int D, int E, int C, int k, int k_sel, long long page_bytes, cudaStream_t st, bool beside_previous);
+// cold_page_bytes != page_bytes: FP8 cold pages (half the bytes), dequantised while copied
 cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas,
-                         cudaStream_t st);
+                         cudaStream_t st, long long cold_page_bytes);
+// quantise n_blocks blocks of block_elems bf16 elements into e4m3 codes in the mapped cold pool + one scale per block
+cudaError_t launch_export_fp8(const void* src, void* dst_mapped, float* scales, long long n_blocks, long long block_elems, cudaStream_t st);
 // NEXT-4: copy `bytes` (multiple of 16) from device memory into the mapped pinned cold pool
 cudaError_t launch_export(const void* src, void* dst_mapped, long long bytes, int n_ctas, cudaStream_t st);
 // swap tables of sequences whose bit is set in swap_mask; append k_new/v_new rows to the ring

@@ -16,6 +16,8 @@
 // semantics are sequential in ascending sequence id, so there is no parallelism across sequences;
 // inside one sequence every pass (pin marking, hit lookup, victim selection, table write) is
 // block-parallel.
+#include <cuda_fp16.h>
+
 #include "lsa_kernels.h"
 #include "lsa_select.cuh"
 
@@ -174,6 +176,7 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
         sm.next_page[tid] = p;
         pool.fetch_src[base + r] = reinterpret_cast<const unsigned char*>(sq.cold) + (long long)c * page_bytes;
         pool.fetch_page[base + r] = p;
+        if (sq.cold_scale) pool.fetch_scale[base + r] = sq.cold_scale + 2 * (size_t)c;
       }
     }
     __syncthreads();
@@ -245,6 +248,113 @@ fetch_kernel(PoolDev pool, unsigned char* __restrict__ hot_pool, long long page_
       if (off < left) *reinterpret_cast<uint4*>(dst + off) = v[u];
     }
   }
+}
+
+// ---- S5 with FP8 (e4m3) cold pages (DESIGN R34): half the bytes cross the host link, the hot page is bf16 as before ----
+// hot element = bf16_rne(fp32(code) * scale): the code is widened exactly (e4m3 -> f16 -> f32), one fp32 multiply, one
+// rounding.  16 codes per 16-byte load become two 16-byte stores.
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t two_codes, float scale) {
+  uint32_t h2;
+  asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"((unsigned short)two_codes));
+  const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h2));
+  const __nv_bfloat162 b = __floats2bfloat162_rn(f.x * scale, f.y * scale);
+  return *reinterpret_cast<const uint32_t*>(&b);
+}
+
+__global__ void __launch_bounds__(kFetchThreads)
+fetch_fp8_kernel(PoolDev pool, unsigned char* __restrict__ hot_pool, long long page_bytes, long long cold_page_bytes) {
+  pdl_wait();                      // the fetch list of the residency pass is complete
+  const int n_fetch = (int)pool.counters[C_FETCH_COUNT];
+  const int slices = (int)((cold_page_bytes + kFetchSlice - 1) / kFetchSlice);
+  const long long items = (long long)n_fetch * slices, half = cold_page_bytes / 2;     // K block | V block
+  for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+    const int f = (int)(it / slices), s = (int)(it % slices);
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(pool.fetch_src[f]) + (long long)s * kFetchSlice;
+    unsigned char* dst = hot_pool + (long long)pool.fetch_page[f] * page_bytes + 2ll * s * kFetchSlice;
+    const long long left = cold_page_bytes - (long long)s * kFetchSlice;
+    const float sk = __ldg(pool.fetch_scale[f]), sv = __ldg(pool.fetch_scale[f] + 1);
+    uint4 v[kFetchUnroll];
+#pragma unroll
+    for (int u = 0; u < kFetchUnroll; ++u) {
+      long long off = ((long long)u * kFetchThreads + threadIdx.x) * 16;
+      if (off < left) v[u] = ld_stream16(reinterpret_cast<const uint4*>(src + off));
+    }
+#pragma unroll
+    for (int u = 0; u < kFetchUnroll; ++u) {
+      long long off = ((long long)u * kFetchThreads + threadIdx.x) * 16;
+      if (off < left) {
+        const float sc = ((long long)s * kFetchSlice + off) < half ? sk : sv;
+        const uint32_t w[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+        uint32_t o[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          o[2 * j] = e4m3x2_to_bf16x2(w[j] & 0xffffu, sc);
+          o[2 * j + 1] = e4m3x2_to_bf16x2(w[j] >> 16, sc);
+        }
+        uint4* d = reinterpret_cast<uint4*>(dst + 2 * off);
+        d[0] = make_uint4(o[0], o[1], o[2], o[3]);
+        d[1] = make_uint4(o[4], o[5], o[6], o[7]);
+      }
+    }
+  }
+}
+
+// ---- export with FP8 cold pages: quantise (DESIGN R35).  One block per (page, K | V block): the largest magnitude's
+// exponent field gives e (max * 2^-e in [128, 256)), scale = 2^e, code = e4m3_rne(x * 2^-e) (the product is exact).
+__global__ void __launch_bounds__(256)
+export_fp8_kernel(const __nv_bfloat16* __restrict__ src, unsigned char* __restrict__ dst, float* __restrict__ scales, long long block_elems) {
+  __shared__ unsigned int wmax[8];
+  __shared__ float s_inv, s_scale;
+  const long long blk = blockIdx.x;
+  const __nv_bfloat16* x = src + blk * block_elems;
+  unsigned char* out = dst + blk * block_elems;
+  unsigned int mx = 0;                                     // |x| as bf16 bits: integer order = magnitude order
+  for (long long i = (long long)threadIdx.x * 8; i < block_elems; i += 256 * 8) {
+    const uint4 r = *reinterpret_cast<const uint4*>(x + i);
+    const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { mx = max(mx, w[j] & 0x7fffu); mx = max(mx, (w[j] >> 16) & 0x7fffu); }
+  }
+  mx = __reduce_max_sync(0xffffffffu, mx);
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned int m = 0;
+    for (int w = 0; w < 8; ++w) m = max(m, wmax[w]);
+    const int field = (int)(m >> 7) & 0xff;                // bf16: 8 exponent bits above 7 mantissa bits
+    int e = field == 0 ? 0 : field - 127 - 7;
+    e = max(-120, min(120, e));
+    s_scale = __uint_as_float((unsigned)(e + 127) << 23);
+    s_inv = __uint_as_float((unsigned)(127 - e) << 23);
+    scales[blk] = s_scale;
+  }
+  __syncthreads();
+  const float inv = s_inv;
+  for (long long i = (long long)threadIdx.x * 16; i < block_elems; i += 256 * 16) {
+    const uint4 r0 = *reinterpret_cast<const uint4*>(x + i), r1 = *reinterpret_cast<const uint4*>(x + i + 8);
+    const uint32_t w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+    uint32_t o[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      uint32_t acc = 0;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const uint32_t ww = w[2 * j + h];
+        const float lo = __uint_as_float(ww << 16) * inv, hi = __uint_as_float(ww & 0xffff0000u) * inv;
+        unsigned short c2;
+        asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(c2) : "f"(hi), "f"(lo));   // first operand -> upper byte
+        acc |= (uint32_t)c2 << (16 * h);
+      }
+      o[j] = acc;
+    }
+    *reinterpret_cast<uint4*>(out + i) = make_uint4(o[0], o[1], o[2], o[3]);
+  }
+}
+
+cudaError_t launch_export_fp8(const void* src, void* dst_mapped, float* scales, long long n_blocks, long long block_elems, cudaStream_t st) {
+  export_fp8_kernel<<<(unsigned)n_blocks, 256, 0, st>>>(reinterpret_cast<const __nv_bfloat16*>(src), reinterpret_cast<unsigned char*>(dst_mapped),
+                                                        scales, block_elems);
+  return cudaGetLastError();
 }
 
 // ---- NEXT-4 (first half): KV export, HBM -> pinned-host cold pool ("P-server streams full KV into D's pinned host
@@ -412,7 +522,10 @@ cudaError_t launch_residency(SeqDev* seqs, PoolDev pool, const FireList& fire, c
                     C > 0 ? C : 1);
 }
 
-cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas, cudaStream_t st) {
+cudaError_t launch_fetch(PoolDev pool, void* hot_pool, long long page_bytes, int n_ctas, cudaStream_t st, long long cold_page_bytes) {
+  if (cold_page_bytes != page_bytes)
+    return launch_pdl(fetch_fp8_kernel, dim3(n_ctas), dim3(kFetchThreads), 0, st, pool, reinterpret_cast<unsigned char*>(hot_pool), page_bytes,
+                      cold_page_bytes);
   return launch_pdl(fetch_kernel, dim3(n_ctas), dim3(kFetchThreads), 0, st, pool, reinterpret_cast<unsigned char*>(hot_pool), page_bytes);
 }
 

@@ -23,6 +23,7 @@ LIB_PATH = os.path.join(_HERE, "liblsa.so")
 LSA_F32, LSA_BF16 = 0, 1
 LSA_ATTN_AUTO, LSA_ATTN_SIMT, LSA_ATTN_TCGEN05 = 0, 1, 2
 LSA_MERGE_AUTO, LSA_MERGE_KERNEL, LSA_MERGE_FUSED = 0, 1, 2
+LSA_COLD_NATIVE, LSA_COLD_FP8_E4M3 = 0, 1
 LSA_INDEXER_DUAL_ENCODER, LSA_INDEXER_LEVEL1 = 0, 1
 
 STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_ERR_POOL_EXHAUSTED",
@@ -48,14 +49,15 @@ class lsa_config(C.Structure):
                 ("k", C.c_int32), ("tau", C.c_int32), ("recall_lag", C.c_int32), ("sm_scale", C.c_float),
                 ("hot_pages", C.c_int64), ("hot_pool", C.c_void_p), ("W_q", C.c_void_p),
                 ("stream_compute", C.c_void_p), ("stream_fetch", C.c_void_p), ("attn_impl", C.c_int32),
-                ("step_overlap", C.c_int32), ("max_ctas", C.c_int32), ("merge_mode", C.c_int32)]
+                ("step_overlap", C.c_int32), ("max_ctas", C.c_int32), ("merge_mode", C.c_int32),
+                ("cold_format", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class lsa_seq_desc(C.Structure):
     _fields_ = [("cold_csa", C.c_void_p), ("n_csa", C.c_int64), ("chunk_emb", C.c_void_p),
                 ("hca_k", C.c_void_p), ("hca_v", C.c_void_p), ("n_hca", C.c_int64), ("win_k", C.c_void_p),
                 ("win_v", C.c_void_p), ("w_len", C.c_int32), ("w_head", C.c_int32), ("step0", C.c_int64),
-                ("cap_csa", C.c_int64), ("cap_hca", C.c_int64)]
+                ("cap_csa", C.c_int64), ("cap_hca", C.c_int64), ("cold_scale", C.c_void_p)]
 
 
 class lsa_stats(C.Structure):
@@ -179,7 +181,7 @@ class LsaContext:
                  hot_pool: torch.Tensor, W_q: torch.Tensor, seqs: Sequence[dict], recall_lag: int = 1,
                  sm_scale: float = 0.0, stream_compute: Optional[torch.cuda.Stream] = None,
                  stream_fetch: Optional[torch.cuda.Stream] = None, attn_impl: int = LSA_ATTN_AUTO,
-                 step_overlap: int = 0, max_ctas: int = 0, merge_mode: int = LSA_MERGE_AUTO):
+                 step_overlap: int = 0, max_ctas: int = 0, merge_mode: int = LSA_MERGE_AUTO, cold_format: int = 0):
         if not torch.cuda.is_available():
             raise LsaError(-2, "no CUDA device: the LSA path has no CPU fallback")
         td = _torch_dtype(dtype)
@@ -201,13 +203,15 @@ class LsaContext:
         cfg.stream_compute = self.stream_compute.cuda_stream
         cfg.stream_fetch = self.stream_fetch.cuda_stream
         cfg.attn_impl, cfg.step_overlap, cfg.max_ctas, cfg.merge_mode = attn_impl, step_overlap, max_ctas, merge_mode
+        cfg.cold_format = cold_format
         descs = (lsa_seq_desc * self.B)()
         for b, s in enumerate(seqs):
             d = descs[b]
             cold = s.get("cold_csa")
             if cold is not None and not cold.is_pinned():
                 raise LsaError(-1, f"seq {b}: cold_csa must be pinned host memory")
-            d.cold_csa = _host_ptr(cold, td, "cold_csa")
+            d.cold_csa = _host_ptr(cold, torch.uint8 if cold_format == LSA_COLD_FP8_E4M3 else td, "cold_csa")
+            d.cold_scale = _dev_ptr(s.get("cold_scale"), torch.float32, "cold_scale")
             d.n_csa = int(s["n_csa"])
             d.chunk_emb = _dev_ptr(s.get("chunk_emb"), td, "chunk_emb")
             d.hca_k = _dev_ptr(s.get("hca_k"), td, "hca_k")

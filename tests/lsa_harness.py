@@ -175,14 +175,14 @@ def apply_tie_triggers(wl: LsaWorkload, oracle: LsaOracle, rig, global_step: int
 
 
 def run_lockstep(wl: LsaWorkload, rig: "GpuRig", steps: int, check_attention_at=None, with_kv_new: bool = True,
-                 l1=None, l1_band: float = 3e-2, step_fn=None):
+                 l1=None, l1_band: float = 3e-2, step_fn=None, oracle=None):
     """Drive lsa_step and the oracle in lock-step: validate the GPU's
     selection against the oracle's scores, feed it to the oracle's residency model, then compare page
     tables / residency / fetched bytes bit-exactly and attention outputs within tolerance."""
     import torch
     from oracle import validate_selection
     c = wl.cfg
-    orc = make_oracle(wl)
+    orc = make_oracle(wl) if oracle is None else oracle
     tol = attn_tolerance(c.dtype)
     n_checked, max_err, n_ties, tie_state = 0, 0.0, 0, {}
     for t in range(steps):
@@ -369,3 +369,50 @@ def run_growth_lockstep(wl: LsaWorkload, gi, rig: "GrowthRig", steps: int, check
         assert np.array_equal(hk[: orc.n_hca[b]], orc.hca_k[b][: orc.n_hca[b]])
     return dict(checked=n_checked, max_abs_err=max_err, oracle=orc, exported=st["chunks_exported"], csa_appended=st["csa_appended"],
                 hca_appended=st["hca_appended"], recalled_grown=n_recalled_grown)
+
+
+# ------------------------------------------------------------------------------------------
+# FP8 (e4m3) cold pages: the cold pool holds codes + block scales, a recall dequantises (DESIGN R34)
+# ------------------------------------------------------------------------------------------
+def make_fp8_oracle(wl: LsaWorkload, fp8, **over) -> LsaOracle:
+    """The oracle of a run whose cold pool is `fp8` (workloads.Fp8ColdInputs): its cold pages are what a recall must write
+    into the hot pool - the codes dequantised by oracle/fp8_oracle.py - and a page costs C*D*2 bytes on the host link."""
+    from oracle.fp8_oracle import dequant_page
+    c = wl.cfg
+    cold = []
+    for b in range(c.B):
+        pages = np.empty(fp8.codes[b].shape, dtype=np.uint16)
+        for ch in range(pages.shape[0]):
+            pages[ch] = dequant_page(fp8.codes[b][ch], fp8.scales[b][ch])
+        cold.append(pages)
+    return make_oracle(wl, cold_csa=cold, cold_page_nbytes=2 * c.C * c.D, **over)
+
+
+class Fp8Rig(GpuRig):
+    """GpuRig with lsa_config.cold_format = FP8_E4M3: pinned uint8 code pools, device scale arrays."""
+
+    def __init__(self, wl: LsaWorkload, fp8, device="cuda:0", **ctx_over):
+        import torch
+        from paper_2606_09079_b200 import lsa
+        from paper_2606_09079_b200.workloads import to_torch
+        c = wl.cfg
+        assert c.dtype == "bf16"
+        self.wl, self.cfg, self.device, self.fp8 = wl, c, torch.device(device), fp8
+        dev, tdt = self.device, torch.bfloat16
+        self.hot_pool = torch.zeros((c.hot_pages, 2, c.C, c.D), dtype=tdt, device=dev)
+        self.W_q = to_torch(wl.W_q, "bf16").to(dev)
+        self.cold = [torch.from_numpy(x.copy()).pin_memory() for x in fp8.codes]
+        self.cold_scale = [torch.from_numpy(x.copy()).to(dev) for x in fp8.scales]
+        self.emb = [to_torch(wl.chunk_emb(b, 0), "bf16").to(dev) for b in range(c.B)]
+        self.hca_k = [to_torch(x, "bf16").to(dev) for x in wl.hca_k]
+        self.hca_v = [to_torch(x, "bf16").to(dev) for x in wl.hca_v]
+        self.win_k = [to_torch(x, "bf16").to(dev) for x in wl.win_k]
+        self.win_v = [to_torch(x, "bf16").to(dev) for x in wl.win_v]
+        seqs = [dict(cold_csa=self.cold[b], cold_scale=self.cold_scale[b], n_csa=c.n_csa(b), chunk_emb=self.emb[b], hca_k=self.hca_k[b],
+                     hca_v=self.hca_v[b], win_k=self.win_k[b], win_v=self.win_v[b], w_len=min(c.W, c.L[b]),
+                     w_head=min(c.W, c.L[b]) % c.W, step0=c.step0(b)) for b in range(c.B)]
+        kw = dict(dtype=lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W, Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pool=self.hot_pool,
+                  W_q=self.W_q, seqs=seqs, recall_lag=c.recall_lag, cold_format=lsa.LSA_COLD_FP8_E4M3)
+        kw.update(ctx_over)
+        self.ctx = lsa.LsaContext(**kw)
+        self.tdt = tdt

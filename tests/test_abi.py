@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol(lib_path):
     for n in _declared():
         assert hasattr(lib, n), f"liblsa.so does not export {n}"
     lib.lsa_version.restype = ctypes.c_int
-    assert lib.lsa_version() == 3
+    assert lib.lsa_version() == 4
 
 
 def test_binding_lists_the_same_symbols(lib_path):
