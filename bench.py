@@ -47,7 +47,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_2606_09079_b200.dist import max_over_ranks, shard_sequences, sum_over_ranks  # noqa: E402
-from paper_2606_09079_b200.workloads import LsaWorkload, make_config, plant_boundary_ties, shard_config, to_torch  # noqa: E402
+from paper_2606_09079_b200.workloads import Fp8ColdInputs, LsaWorkload, make_config, plant_boundary_ties, shard_config, to_torch  # noqa: E402
 
 METRIC = {1: ("lsa_decode_steps_per_s_8k_ctx_fp32", "steps/s"),
           2: ("lsa_decode_steps_per_s_128k_ctx", "steps/s"),
@@ -240,13 +240,15 @@ class Replica:
         self.hca_v = [x.clone() for x in shared["hca_v"]]
         self.win_k = [x.clone() for x in shared["win_k"]]
         self.win_v = [x.clone() for x in shared["win_v"]]
-        seqs = [dict(cold_csa=shared["cold"][b], n_csa=c.n_csa(b), chunk_emb=self.emb[b], hca_k=self.hca_k[b],
+        fp8 = shared.get("cold_scale") is not None
+        seqs = [dict(cold_csa=shared["cold"][b], cold_scale=shared["cold_scale"][b] if fp8 else None, n_csa=c.n_csa(b), chunk_emb=self.emb[b], hca_k=self.hca_k[b],
                      hca_v=self.hca_v[b], win_k=self.win_k[b], win_v=self.win_v[b], w_len=min(c.W, c.L[b]), w_head=0,
                      step0=c.step0(b) + phase) for b in range(c.B)]
         self.ctx = lsa.LsaContext(dtype=lsa.LSA_F32 if c.dtype == "f32" else lsa.LSA_BF16, H=c.H, D=c.D, C_=c.C, W=c.W,
                                   Dh=c.Dh, E=c.E, k=c.k, tau=c.tau, hot_pool=self.hot_pool, W_q=shared["W_q"], seqs=seqs,
                                   recall_lag=c.recall_lag, stream_compute=sc, stream_fetch=sf,
-                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0), step_overlap=overlap)
+                                  attn_impl=shared["attn_impl"], max_ctas=shared.get("max_ctas", 0), step_overlap=overlap,
+                                  cold_format=lsa.LSA_COLD_FP8_E4M3 if fp8 else lsa.LSA_COLD_NATIVE)
         self.step = phase                # global step index of the workload this replica is at (wl.fires / wl.trigger_index)
         self.bound = {}                  # lsa_step bound to fixed input buffers (LsaContext.bind_step)
         self.tie_emb = {}                # cfg 5: sequences whose alternate (tie-carrying) embedding table is installed
@@ -310,6 +312,7 @@ def main():
     ap.add_argument("--dry-run", action="store_true", help="CPU only: launcher, sharding and reductions with a gloo group")
     ap.add_argument("--l1", action="store_true", help="also time the paper-exact Level-1 indexer (NEXT-1)")
     ap.add_argument("--export", action="store_true", help="also time lsa_export_chunks (NEXT-4: KV export HBM -> pinned cold pool)")
+    ap.add_argument("--cold-fp8", action="store_true", help="FP8 (e4m3) cold pages: half the bytes per recall over the host link (not BASELINE's config: reported under run.cold_format)")
     ap.add_argument("--growth", action="store_true", help="also time the step with a growing compressed history (NEXT-4: lsa_append_compressed)")
     ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
     ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
@@ -361,8 +364,10 @@ def main():
             return n_steps
         return sum_over_ranks(n_steps * per_step_units, dev)
 
+    fp8 = Fp8ColdInputs(wl) if args.cold_fp8 else None            # --cold-fp8: e4m3 codes + block scales in the cold pool
     shared = dict(dev=dev, tdt=tdt, attn_impl=attn_impl, max_ctas=args.max_ctas, W_q=to_torch(wl.W_q, c.dtype).to(dev),
-                  cold=[to_torch(x, c.dtype).pin_memory() for x in wl.cold_csa],
+                  cold=([torch.from_numpy(x).pin_memory() for x in fp8.codes] if fp8 else [to_torch(x, c.dtype).pin_memory() for x in wl.cold_csa]),
+                  cold_scale=[torch.from_numpy(x).to(dev) for x in fp8.scales] if fp8 else None,
                   emb=[to_torch(wl.chunk_emb(b, 0), c.dtype).to(dev) for b in range(c.B)],
                   hca_k=[to_torch(x, c.dtype).to(dev) for x in wl.hca_k], hca_v=[to_torch(x, c.dtype).to(dev) for x in wl.hca_v],
                   win_k=[to_torch(x, c.dtype).to(dev) for x in wl.win_k], win_v=[to_torch(x, c.dtype).to(dev) for x in wl.win_v])
@@ -726,7 +731,7 @@ def main():
 
     # ---- optional: KV export into the cold pool (NEXT-4, first half) against the pinned D2H copy rate ----
     export = None
-    if args.export and rank == 0:
+    if args.export and rank == 0 and not args.cold_fp8:
         n_ch = min(c.n_chunks(0), max(1, (256 * 2**20) // c.page_bytes))
         src = shared["cold"][0][:n_ch].to(dev)                   # the same bytes go back: the pool's content is unchanged
         nb = src.numel() * src.element_size()
@@ -749,7 +754,7 @@ def main():
     # ---- optional: the step with a growing compressed history (NEXT-4, second half): lsa_append_compressed every 4th step
     # (CSA entry; HCA entry every 128th), chunks completing every 512 steps and being exported, against the static loop ----
     growth = None
-    if args.growth and rank == 0:
+    if args.growth and rank == 0 and not args.cold_fp8:
         n_gr = max(2048, min(args.steps, 8192))
         n_gr += (-n_gr) % (R * c.tau)
         per_rep = (R * c.tau * 2 + n_gr) // R + 8
@@ -861,7 +866,7 @@ def main():
         line = dict(metric=name, value=value, unit=unit, n_gpus=world, steps=args.steps, steps_requested=steps_requested, warmup=warmup,
                     ms_per_step=ms / args.steps, higher_is_better=True, scaling="strong" if sharded else "weak", vs_baseline=None,
                     dtype=c.dtype, data="synthetic", config=workload_config(cfg, world, l2),
-                    run=dict(step_overlap=args.overlap, attn_impl={1: "simt", 2: "tcgen05"}.get(stats["attn_impl"], "?"), attn_ctas=stats["attn_ctas"],
+                    run=dict(step_overlap=args.overlap, cold_format="fp8_e4m3" if args.cold_fp8 else "native", attn_impl={1: "simt", 2: "tcgen05"}.get(stats["attn_impl"], "?"), attn_ctas=stats["attn_ctas"],
                              replicas=R, replica_trigger_phases=phases, sequences_this_rank=c.B,
                              note="step_overlap = 1: the timed steps belong to independent layer-state replicas and their inputs are staged before the loop"),
                     e2e=dict(value=e2e_value, unit=unit, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=n_e2e,
