@@ -33,6 +33,10 @@ struct ResSmem {
   int n_miss;
   unsigned long long tick;
   unsigned int epoch;
+  // several sequences firing together on a full pool (P <= kSortCap): the unpinned pages sorted ONCE by (last_used, page)
+  int order[kSortCap];    // their page ids in that order
+  int victim[kMaxK];      // pages taken by the current sequence's misses, in miss order
+  int n_order, cursor, use_order, took, advance;
 };
 
 __global__ void __launch_bounds__(1024)
@@ -48,13 +52,91 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
   if (tid == 0) pool.counters[C_FETCH_COUNT] = 0;
   __syncthreads();
 
+  // ---- several sequences fire together and never-used pages will not cover them: order the unpinned pages ONCE ----
+  // A pass only ever touches pages it then lists in its staged table, and staged tables are pinned for every later pass
+  // of the launch; untouched pages keep their (last_used, page) key.  So the victims of the whole launch are consumed
+  // front to back from ONE sorted list of the pages that are unpinned when the launch starts: sequence b takes the first
+  // n_miss(b) entries behind the cursor that have not been pinned since (its own hits, which may sit anywhere in the
+  // list).  The per-sequence work shrinks to a hit pass and one scan of a window of the list; the result is the
+  // sequential one (DESIGN R12).  Needs: no firing sequence with an unswapped staged table of its own (that table would
+  // have to be unpinned for its own pass only - the general path below handles it).
+  if (tid == 0) {
+    bool ok = fire.n >= 2 && P <= kSortCap && blockDim.x == 1024;
+    const long long n_used = (long long)(pool.counters[C_MISSES] - pool.counters[C_EVICTIONS]);
+    if (ok && n_used + (long long)fire.n * k_cap <= (long long)P) ok = false;        // index arithmetic will do
+    for (int fi = 0; ok && fi < fire.n; ++fi) ok = seqs[fire.ids[fi]].pending == 0;
+    sm.use_order = ok ? 1 : 0;
+    if (ok) sm.epoch = ++(*pool.epoch);
+    sm.cursor = 0;
+  }
+  __syncthreads();
+  const bool use_order = sm.use_order != 0;
+  if (use_order) {
+    const unsigned int epoch = sm.epoch;
+    for (int idx = tid; idx < B * 2 * k; idx += blockDim.x) {
+      int bb = idx / (2 * k), r = idx % (2 * k), buf = r / k, j = r % k;
+      const SeqDev& o = seqs[bb];
+      const bool live = buf == o.cur_buf || o.pending != 0;
+      if (live && j < o.n_tbl[buf]) {
+        const int pg = pool.tbl_page[((size_t)bb * 2 + buf) * k + j];
+        if (pg < P) pool.pin_mark[pg] = epoch;                    // (tier pages of a growing context lie beyond P)
+      }
+    }
+    __syncthreads();
+    const int n_pad = next_pow2(P);
+    int mine = 0;
+    for (int i = tid; i < n_pad; i += blockDim.x) {
+      unsigned long long key = kKeyMax;
+      if (i < P && pool.pin_mark[i] != epoch) { key = (pool.last_used[i] << kPageBits) | (unsigned long long)i; ++mine; }
+      sm.sel.keys[i] = key;
+    }
+    mine = __reduce_add_sync(0xffffffffu, mine);
+    if (lane == 0) sm.warp_cnt[warp] = mine;
+    __syncthreads();
+    block_bitonic_sort(sm.sel.keys, n_pad);
+    if (tid == 0) {
+      int n = 0;
+      for (int w = 0; w < 32; ++w) n += sm.warp_cnt[w];
+      sm.n_order = n;
+    }
+    for (int i = tid; i < n_pad; i += blockDim.x) sm.order[i] = (int)(sm.sel.keys[i] & ((1ull << kPageBits) - 1));
+    __syncthreads();
+  }
+  // ... and all the selections in one go: key = (position in the fire list, chunk id), invalid ids last in their segment
+  const int k_pad = next_pow2(k);
+  const bool pre_sorted = use_order && fire.n * k_pad <= kSortCap;
+  if (pre_sorted) {
+    const int total = fire.n * k_pad, total_pad = next_pow2(total);
+    for (int i = tid; i < total_pad; i += blockDim.x) {
+      unsigned long long key = kKeyMax;
+      if (i < total) {
+        const int fi = i / k_pad, j = i - fi * k_pad;
+        const int c = j < k ? sel_idx[(size_t)fi * k + j] : -1;
+        const bool valid = c >= 0 && c < seqs[fire.ids[fi]].n_chunks;
+        key = ((unsigned long long)fi << 32) | (valid ? (unsigned)c : 0xffffffffu);
+      }
+      sm.sel.keys[i] = key;
+    }
+    __syncthreads();
+    block_bitonic_sort(sm.sel.keys, total_pad);
+  }
+
   for (int fi = 0; fi < fire.n; ++fi) {
     const int b = fire.ids[fi];
     SeqDev& sq = seqs[b];
     const int* my_sel = sel_idx + (size_t)fi * k;
 
     // ---- selection -> ascending chunk id (R13) ----
-    {
+    if (pre_sorted) {
+      const bool valid = tid < k_pad && (unsigned)sm.sel.keys[fi * k_pad + tid] != 0xffffffffu;
+      const int n = __syncthreads_count(valid);            // valid ids sort first inside the segment
+      if (valid) sm.sel_up[tid] = (int)(unsigned)sm.sel.keys[fi * k_pad + tid];
+      if (tid == 0) {
+        sm.n_sel = n;
+        sm.tick = pool.counters[C_TICK] + 1;
+      }
+      __syncthreads();
+    } else {
       int n_pad = next_pow2(k);
       for (int i = tid; i < n_pad; i += blockDim.x) {
         int c = (i < k) ? my_sel[i] : -1;
@@ -73,7 +155,7 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
         for (int w = 0; w < 32; ++w) n += sm.warp_cnt[w];
         sm.n_sel = n;
         sm.tick = pool.counters[C_TICK] + 1;     // committed below, once the pass is known to succeed
-        sm.epoch = ++(*pool.epoch);              // scratch stamp of pin_mark: harmless if the pass is abandoned
+        if (!use_order) sm.epoch = ++(*pool.epoch);   // scratch stamp of pin_mark: harmless if the pass is abandoned
       }
       __syncthreads();
       for (int i = tid; i < sm.n_sel; i += blockDim.x) sm.sel_up[i] = (int)sm.sel.keys[i];
@@ -89,7 +171,7 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
     }
 
     // ---- pin every page of a current table and of other sequences' staged tables ----
-    for (int idx = tid; idx < B * 2 * k; idx += blockDim.x) {
+    for (int idx = tid; !use_order && idx < B * 2 * k; idx += blockDim.x) {
       int bb = idx / (2 * k), r = idx % (2 * k), buf = r / k, j = r % k;
       const SeqDev& o = seqs[bb];
       bool is_cur = (buf == o.cur_buf);
@@ -137,7 +219,63 @@ residency_kernel(SeqDev* __restrict__ seqs, PoolDev pool, FireList fire, const i
     // enough never-used pages are left, the victims are simply the next n_miss indices (no scan of the pool).
     bool fast = true;
     long long n_used = 0;
-    if (n_miss > 0) {
+    if (n_miss > 0 && use_order) {
+      // the first n_miss entries behind the cursor that are still unpinned, window by window
+      int need = n_miss, got = 0;
+      bool short_of_pages = false;
+      while (need > 0) {
+        const int cur = sm.cursor, pos = cur + tid;
+        const bool in = pos < sm.n_order;
+        const int pg = in ? sm.order[pos] : -1;
+        const bool free_pg = in && pool.pin_mark[pg] != epoch;
+        const unsigned balf = __ballot_sync(0xffffffffu, free_pg);
+        const int wpre_f = __popc(balf & ((1u << lane) - 1));
+        __syncthreads();                                   // warp_cnt / took / advance of the previous round are consumed
+        if (lane == 0) sm.warp_cnt[warp] = __popc(balf);
+        __syncthreads();
+        int below = 0;
+        for (int w = 0; w < warp; ++w) below += sm.warp_cnt[w];
+        const int rank = below + wpre_f;
+        if (free_pg && rank < need) sm.victim[got + rank] = pg;
+        if (free_pg && rank == need - 1) sm.advance = tid + 1;      // the window is satisfied here
+        if (tid == 1023) { sm.took = rank + (free_pg ? 1 : 0); }
+        __syncthreads();
+        const int took = min(sm.took, need);
+        if (sm.took >= need) { if (tid == 0) sm.cursor = cur + sm.advance; need = 0; }
+        else {
+          if (cur + 1024 >= sm.n_order) { short_of_pages = true; break; }
+          if (tid == 0) sm.cursor = cur + 1024;
+          need -= took; got += took;
+        }
+        __syncthreads();
+      }
+      if (short_of_pages) {
+        if (tid == 0) pool.counters[C_ERROR] = 1;
+        __syncthreads();
+        continue;
+      }
+      __syncthreads();
+      const unsigned long long base = pool.counters[C_FETCH_COUNT];
+      if (tid < n_sel && sm.miss_rank[tid] >= 0) {
+        const int r = sm.miss_rank[tid];
+        const int c = sm.sel_up[tid];
+        const int p = sm.victim[r];
+        const int ob = pool.owner_seq[p];
+        if (ob >= 0) {
+          pool.page_of[seqs[ob].page_of_off + pool.owner_chunk[p]] = -1;
+          atomicAdd(&pool.counters[C_EVICTIONS], 1ull);
+        }
+        pool.owner_seq[p] = b;
+        pool.owner_chunk[p] = c;
+        pool.page_of[sq.page_of_off + c] = p;
+        pool.last_used[p] = tick;
+        pool.pin_mark[p] = epoch;
+        sm.next_page[tid] = p;
+        pool.fetch_src[base + r] = reinterpret_cast<const unsigned char*>(sq.cold) + (long long)c * page_bytes;
+        pool.fetch_page[base + r] = p;
+        if (sq.cold_scale) pool.fetch_scale[base + r] = sq.cold_scale + 2 * (size_t)c;
+      }
+    } else if (n_miss > 0) {
       n_used = (long long)(pool.counters[C_MISSES] - pool.counters[C_EVICTIONS]);
       fast = n_used + n_miss <= (long long)P;
       if (!fast) {
