@@ -280,7 +280,7 @@ struct TcWorkspace;
 struct TcPlan {
   TcInit init{};
   EncodeTiledFn encode = nullptr;
-  CUtensorMap map_pool{}, map_pool64{}, map_q{}, map_part{};
+  CUtensorMap map_pool{}, map_pool64{}, map_q{}, map_part{}, map_part_small{};
   const void* q_cached = nullptr;
   CUtensorMap* d_maps = nullptr;
   CUtensorMap* d_maps8 = nullptr;      // small path: [B][8], 128-row and 64-row boxes
@@ -463,6 +463,13 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { *msg = "cuTensorMapEncodeTiled (partials) failed"; return -2; }
+    // the small-batch path's merge: both workspace buffers as one tensor [2 * slots][H*D/2]; box = the 256 B of one unit
+    // (4 heads x 32 d, fp16) of 32 consecutive slots
+    cuuint64_t dims2[2] = {(cuuint64_t)kTcH * kTcD / 2, (cuuint64_t)pl->ws->slots * 2};
+    cuuint32_t box2[2] = {64, 32};
+    r = pl->encode(&pl->map_part_small, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, pl->ws->part_o, dims2, strides, box2, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { *msg = "cuTensorMapEncodeTiled (partials, small path) failed"; return -2; }
   }
   p.part_o = pl->ws->part_o; p.part_s = pl->ws->part_s; p.part_m = pl->ws->part_m; p.part_l = pl->ws->part_l; p.piece_info = pl->ws->piece_info;
   TC_CUDA(cudaMalloc(&p.grid_ctr, sizeof(unsigned int)));
@@ -589,6 +596,7 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   prm.part_m = ws->part_m + (size_t)buf * ws->slots * kTcH;              // [64][slots]
   prm.part_l = ws->part_l + (size_t)buf * ws->slots * kTcH;
   prm.n_slots = (int)ws->slots;
+  prm.slot_row0 = buf * (int)ws->slots;
   prm.piece_info = ws->piece_info + (size_t)buf * ws->grid_max;
   prm.arr_ctr = ws->ctrs + buf; prm.arr_target = (ws->arr_total[buf] += (unsigned)n_attn);
   prm.done_ctr = ws->ctrs + 2;
@@ -610,7 +618,7 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   cudaLaunchConfig_t lc{};
   lc.gridDim = dim3(n_attn); lc.blockDim = dim3(kTcThreads); lc.dynamicSmemBytes = sizeof(SmSmem) + 1024; lc.stream = st;
   lc.attrs = attr; lc.numAttrs = (step.serialize || first_after_general) ? 0 : 1;
-  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel, pl->map_pool, pl->map_pool64, pl->map_q, pl->maps0, prm));
+  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel, pl->map_pool, pl->map_pool64, pl->map_q, pl->map_part_small, pl->maps0, prm));
   if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
   if (ev_mid1) TC_CUDA(cudaEventRecord(ev_mid1, st));
   ws->n_small += 1;

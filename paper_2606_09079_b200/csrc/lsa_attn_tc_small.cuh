@@ -68,6 +68,7 @@ struct SmParams {
   float* part_m;                 // S8 reads one head (block) of EVERY slot, which is then one coalesced line per 32 slots
   float* part_l;
   int n_slots;                   // row length of the transposed arrays
+  int slot_row0;                 // first row of this launch's workspace buffer in the partials' tensor map (S8's TMA)
   int2* piece_info;
   unsigned int* arr_ctr;         // arrival counter of this launch's workspace buffer (cumulative over its launches)
   unsigned int arr_target;       // its value once every CTA of this launch has arrived
@@ -110,7 +111,7 @@ struct SmSmem {
   int pg_off[kSmB], pg_cnt;                                   // entry of (sequence b, table position t) = pg_off[b] + t
   int k0_early;                                               // the setup already requested K of the first sub-tile
   uint64_t full[kTcStages], empty[kTcStages];
-  uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup, app_done;
+  uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup, app_done, mrg_full;
   uint32_t tmem_base;
 };
 
@@ -226,93 +227,104 @@ __device__ __forceinline__ float sm_w_of(float m, float M) { return m == -INFINI
 
 // S8 (see the header, item 3).  Called by the 256 softmax threads (t = 0..255) of every CTA once all partials of the
 // launch are visible.  Unit = (sequence b, 32 consecutive uint2 columns cc of the partial layout) = 4 heads x 32 d, 256
-// per sequence; CTA c takes units [c * NU / n_cta, (c + 1) * NU / n_cta), two at a time: warps 0-3 the first, warps 4-7
-// the second, warp (w & 3) the slots of CTAs (w & 3), (w & 3) + 4, ...  EVERYTHING a pair of units needs is requested
-// before anything is waited for - the fp16 columns of all slots, and (lane l: CTAs l, l + 32, ...) piece_info, m, l and
-// the block scale, which every warp fetches for itself so that no weight crosses a warp - so the merge is one memory
-// round trip deep.  Inactive slots get scale 0 and are selected away, never multiplied.
-// scratch: >= 4 KiB of shared memory the attention phase no longer uses (the Q tile buffer).
-constexpr int kMrgData = 40;                  // slots per warp: kSG * 40 >= n_cta
-// kSG = warps per unit: 4 (two units at a time, n_cta <= 160) or 2 (four units at a time, n_cta <= 80)
-template <int kSG>
-__device__ __noinline__ void small_merge(const SmParams& p, unsigned char* scratch, int cta, int n_cta, int t) {
-  constexpr int kMrgW = kSG == 4 ? 5 : 3;     // slots per lane: ceil(n_cta max / 32)
-  constexpr int kPer = 8 / kSG;               // units per iteration
-  const int w = t >> 5, lane = t & 31, sg = w % kSG, half = w / kSG;
-  float4* red = reinterpret_cast<float4*>(scratch);              // [units per iteration][kSG slot groups][32 lanes]
+// per sequence; CTA c takes units [c * NU / n_cta, (c + 1) * NU / n_cta), kMuPer at a time.  The merge runs ONCE per
+// launch, so its cost is its code size as much as its data: an unrolled register version (40 loads in flight per thread)
+// was 27 KB of straight-line code fetched cold by every CTA (ncu: "no_instructions" the top stall reason, a third of all
+// samples inside the merge).  Here one thread requests the fp16 columns of all slots by TMA (2-D boxes of 32 slots x
+// 256 B into the shared memory the attention phase has left behind), one warp per unit meanwhile computes the weights
+// (lane l: slots l, l + 32, ...; the m / l / scale rows are contiguous along the slots), and the weighted sum is a short
+// rolled loop over shared memory.  Slots without a partial for the sequence get weight 0 and are skipped, never multiplied.
+constexpr int kMuPer = 4;                     // units per round
+constexpr int kMuSlots = 160;                 // n_cta at most
+__device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CUtensorMap* map_part, int cta, int n_cta, int t) {
+  const int w = t >> 5, lane = t & 31;
+  unsigned char* land = sm.q;                                    // [kMuPer][rows][256 B]; q + stage are contiguous (192 KiB)
+  float4* wbuf = reinterpret_cast<float4*>(sm.p);                // [kMuPer][kMuSlots]: weight x block scale per head (10 KiB)
+  float4* ml = reinterpret_cast<float4*>(sm.ones);               // [kMuPer][2]: M, L
+  float4* red = ml + 2 * kMuPer;                                 // [kMuPer][32]
   const int NU = p.B * 256;
   const int u0 = (int)((unsigned)cta * (unsigned)NU / (unsigned)n_cta), u1 = (int)((unsigned)(cta + 1) * (unsigned)NU / (unsigned)n_cta);
-  for (int ub = u0; ub < u1; ub += kPer) {
-    const int u = ub + half;
-    const bool on = u < u1;
-    const int b = on ? u >> 8 : 0, cc = u & 255;
-    const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
-    // ---- requests ----
-    const uint2* col = p.part_o + (size_t)b * (kTcH * kTcD / 4) + cc * 32 + lane;      // slot (c + b), this lane's column
-    uint2 v[kMrgData];
-#pragma unroll
-    for (int j = 0; j < kMrgData; ++j)
-      v[j] = (on && sg + kSG * j < n_cta) ? *(col + (size_t)(sg + kSG * j) * (kTcH * kTcD / 4)) : make_uint2(0u, 0u);
-    float4 mj[kMrgW], lj[kMrgW];
-    float sj[kMrgW];
-#pragma unroll
-    for (int r = 0; r < kMrgW; ++r) {
-      const int c = lane + 32 * r;
-      mj[r] = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY); lj[r] = make_float4(0.f, 0.f, 0.f, 0.f); sj[r] = 0.f;
-      if (on && c < n_cta) {
-        const size_t s = (size_t)c + b, ns = (size_t)p.n_slots;
+  const int n_box = (n_cta + 31) >> 5, rows = n_box * 32;
+  const size_t ns = (size_t)p.n_slots;
+  int round = 0;
+  for (int ub = u0; ub < u1; ub += kMuPer, ++round) {
+    const int nu = min(kMuPer, u1 - ub);
+    if (t == 0) {
+      fence_proxy_async_all();                                   // the partials were written by generic stores of other CTAs
+      mbar_arrive_expect_tx(&sm.mrg_full, (uint32_t)(nu * rows * 256));
+#pragma unroll 1
+      for (int i = 0; i < nu; ++i) {
+        const int u = ub + i, b = u >> 8, cc = u & 255;
+#pragma unroll 1
+        for (int bx = 0; bx < n_box; ++bx)
+          tma_load_2d(land + (size_t)(i * rows + bx * 32) * 256, map_part, cc * 64, p.slot_row0 + b + bx * 32, &sm.mrg_full);
+      }
+    }
+    if (w < nu) {                                                // weights of unit ub + w
+      const int u = ub + w, b = u >> 8, cc = u & 255;
+      const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
+      float4 M = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+#pragma unroll 1
+      for (int c = lane; c < n_cta; c += 32) {
+        const size_t s_ = (size_t)c + b;
         const int2 info = p.piece_info[c];
-        const float* pm = p.part_m + (size_t)h0 * ns + s;
-        const float* pl = p.part_l + (size_t)h0 * ns + s;
-        const float4 m4 = make_float4(pm[0], pm[ns], pm[2 * ns], pm[3 * ns]);
-        const float4 l4 = make_float4(pl[0], pl[ns], pl[2 * ns], pl[3 * ns]);
-        const float s1 = p.part_s[(size_t)((m * 2 + hh) * 4 + dq) * ns + s];
+        const float* pm = p.part_m + (size_t)h0 * ns + s_;
+        float4 m4 = make_float4(pm[0], pm[ns], pm[2 * ns], pm[3 * ns]);
         // CTA c wrote a partial for sequence b, and the piece had an attended key (else it wrote no O)
-        if (info.x <= b && b < info.x + info.y && m4.x != -INFINITY) { mj[r] = m4; lj[r] = l4; sj[r] = s1; }
+        if (!(info.x <= b && b < info.x + info.y) || m4.x == -INFINITY) m4 = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+        wbuf[w * kMuSlots + c] = m4;                             // parked: becomes the weight below
+        M.x = fmaxf(M.x, m4.x); M.y = fmaxf(M.y, m4.y); M.z = fmaxf(M.z, m4.z); M.w = fmaxf(M.w, m4.w);
       }
-    }
-    // ---- weights (every warp for itself) ----
-    float4 M = mj[0];
-#pragma unroll
-    for (int r = 1; r < kMrgW; ++r) { M.x = fmaxf(M.x, mj[r].x); M.y = fmaxf(M.y, mj[r].y); M.z = fmaxf(M.z, mj[r].z); M.w = fmaxf(M.w, mj[r].w); }
-    M = sm_warp_max4(M);
-    float4 L = make_float4(0.f, 0.f, 0.f, 0.f), ws[kMrgW];
-#pragma unroll
-    for (int r = 0; r < kMrgW; ++r) {
-      const float4 wj = make_float4(sm_w_of(mj[r].x, M.x), sm_w_of(mj[r].y, M.y), sm_w_of(mj[r].z, M.z), sm_w_of(mj[r].w, M.w));
-      L.x = fmaf(wj.x, lj[r].x, L.x); L.y = fmaf(wj.y, lj[r].y, L.y); L.z = fmaf(wj.z, lj[r].z, L.z); L.w = fmaf(wj.w, lj[r].w, L.w);
-      ws[r] = make_float4(wj.x * sj[r], wj.y * sj[r], wj.z * sj[r], wj.w * sj[r]);
-    }
-    L = sm_warp_sum4(L);
-    // ---- weighted sum of this warp's slots ----
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-    for (int j = 0; j < kMrgData; ++j) {
-      constexpr int kRound = 32 / kSG;                           // slot sg + kSG j is held by lane src, round j / kRound
-      const int src = (sg + kSG * j) & 31;
-      const float fx = __shfl_sync(0xffffffffu, ws[j / kRound].x, src), fy = __shfl_sync(0xffffffffu, ws[j / kRound].y, src);
-      const float fz = __shfl_sync(0xffffffffu, ws[j / kRound].z, src), fw = __shfl_sync(0xffffffffu, ws[j / kRound].w, src);
-      const float sc = __shfl_sync(0xffffffffu, sj[j / kRound], src);
-      if (sc != 0.f) {
-        const float2 a01 = unpack_f16x2(v[j].x), a23 = unpack_f16x2(v[j].y);
-        acc.x = fmaf(fx, a01.x, acc.x); acc.y = fmaf(fy, a01.y, acc.y);
-        acc.z = fmaf(fz, a23.x, acc.z); acc.w = fmaf(fw, a23.y, acc.w);
+      M = sm_warp_max4(M);
+      float4 L = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
+      for (int c = lane; c < n_cta; c += 32) {
+        const size_t s_ = (size_t)c + b;
+        const float4 m4 = wbuf[w * kMuSlots + c];
+        float4 wj = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (m4.x != -INFINITY) {
+          const float* pl = p.part_l + (size_t)h0 * ns + s_;
+          const float s1 = p.part_s[(size_t)((m * 2 + hh) * 4 + dq) * ns + s_];
+          const float4 e = make_float4(sm_w_of(m4.x, M.x), sm_w_of(m4.y, M.y), sm_w_of(m4.z, M.z), sm_w_of(m4.w, M.w));
+          L.x = fmaf(e.x, pl[0], L.x); L.y = fmaf(e.y, pl[ns], L.y); L.z = fmaf(e.z, pl[2 * ns], L.z); L.w = fmaf(e.w, pl[3 * ns], L.w);
+          wj = make_float4(e.x * s1, e.y * s1, e.z * s1, e.w * s1);
+        }
+        wbuf[w * kMuSlots + c] = wj;
       }
+      L = sm_warp_sum4(L);
+      if (lane == 0) { ml[2 * w] = M; ml[2 * w + 1] = L; }
     }
-    red[(half * kSG + sg) * 32 + lane] = acc;
     named_bar_sync(2, 256);
-    if (sg == 0 && on) {                                         // one warp per unit: 4 heads x 32 d
-      float4 num = red[(half * kSG) * 32 + lane];
-#pragma unroll
-      for (int i = 1; i < kSG; ++i) {
-        const float4 a = red[(half * kSG + i) * 32 + lane];
-        num.x += a.x; num.y += a.y; num.z += a.z; num.w += a.w;
+    mbar_wait(&sm.mrg_full, round & 1, 57);
+    // weighted sum: warps i and i + 4 share unit i, half of the slots each; lane = one uint2 column (4 heads of one d)
+    const int i = w & 3, half = w >> 2;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (i < nu) {
+      const int s_lo = half * (rows >> 1), s_hi = min(n_cta, s_lo + (rows >> 1));
+      const unsigned char* lp = land + (size_t)i * rows * 256 + lane * 8;
+#pragma unroll 4
+      for (int sl = s_lo; sl < s_hi; ++sl) {
+        const float4 f = wbuf[i * kMuSlots + sl];
+        if (f.x != 0.f || f.y != 0.f || f.z != 0.f || f.w != 0.f) {
+          const uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
+          const float2 a01 = unpack_f16x2(v.x), a23 = unpack_f16x2(v.y);
+          acc.x = fmaf(f.x, a01.x, acc.x); acc.y = fmaf(f.y, a01.y, acc.y);
+          acc.z = fmaf(f.z, a23.x, acc.z); acc.w = fmaf(f.w, a23.y, acc.w);
+        }
       }
+      if (half == 1) red[i * 32 + lane] = acc;
+    }
+    named_bar_sync(2, 256);
+    if (half == 0 && i < nu) {                                   // one warp per unit writes 4 heads x 32 d
+      const int u = ub + i, b = u >> 8, cc = u & 255;
+      const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
+      const float4 a = red[i * 32 + lane], M = ml[2 * i], L = ml[2 * i + 1];
+      acc.x += a.x; acc.y += a.y; acc.z += a.z; acc.w += a.w;
       __nv_bfloat16* o = p.out + ((size_t)b * kTcH + h0) * kTcD + m * 128 + dq * 32 + lane;
-      o[0] = __float2bfloat16_rn(L.x > 0.f ? num.x / L.x : 0.f);
-      o[kTcD] = __float2bfloat16_rn(L.y > 0.f ? num.y / L.y : 0.f);
-      o[2 * kTcD] = __float2bfloat16_rn(L.z > 0.f ? num.z / L.z : 0.f);
-      o[3 * kTcD] = __float2bfloat16_rn(L.w > 0.f ? num.w / L.w : 0.f);
+      o[0] = __float2bfloat16_rn(L.x > 0.f ? acc.x / L.x : 0.f);
+      o[kTcD] = __float2bfloat16_rn(L.y > 0.f ? acc.y / L.y : 0.f);
+      o[2 * kTcD] = __float2bfloat16_rn(L.z > 0.f ? acc.z / L.z : 0.f);
+      o[3 * kTcD] = __float2bfloat16_rn(L.w > 0.f ? acc.w / L.w : 0.f);
       if (p.lse && m == 0 && dq == 0 && lane == 0) {
         float* ls = p.lse + (size_t)b * kTcH + h0;
         ls[0] = L.x > 0.f ? (M.x + log2f(L.x)) * 0.6931471805599453f : -INFINITY;
@@ -321,13 +333,14 @@ __device__ __noinline__ void small_merge(const SmParams& p, unsigned char* scrat
         ls[3] = L.w > 0.f ? (M.w + log2f(L.w)) * 0.6931471805599453f : -INFINITY;
       }
     }
-    named_bar_sync(2, 256);                                      // `red` is reused by the next pair
+    named_bar_sync(2, 256);                                      // landing buffer, wbuf, red are reused by the next round
   }
 }
 
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_constant__ CUtensorMap map_pool64,
-                     const __grid_constant__ CUtensorMap map_q, const __grid_constant__ SmMaps0 maps0, const __grid_constant__ SmParams p) {
+                     const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_part,
+                     const __grid_constant__ SmMaps0 maps0, const __grid_constant__ SmParams p) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   SmSmem& sm = *reinterpret_cast<SmSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -341,10 +354,12 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     for (int i = 0; i < 4; ++i) mbar_init(&sm.o_full[i], 1);
     mbar_init(&sm.setup, kTcThreads / 32);
     mbar_init(&sm.app_done, kTcSoftmaxWarps);
+    mbar_init(&sm.mrg_full, 1);
     fence_mbar_init();
     prefetch_tmap(&map_pool);
     prefetch_tmap(&map_pool64);
     prefetch_tmap(&map_q);
+    prefetch_tmap(&map_part);
   }
   __syncthreads();
   griddep_launch_dependents();    // the combine blocks of this step (and, behind them, the next step's CTAs) may be placed
@@ -803,8 +818,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     }
   }
   if (warp >= 2) {
-    if (n_cta <= 80) small_merge<2>(p, sm.q, cta, n_cta, tid - 64);
-    else small_merge<4>(p, sm.q, cta, n_cta, tid - 64);
+    small_merge(p, sm, &map_part, cta, n_cta, tid - 64);
   }
   __syncthreads();
   if (tid == 0) {
