@@ -110,6 +110,8 @@ struct SmSmem {
   int pg_page[32], pg_chunk[32];                              // table entries of the pages in this CTA's range
   int pg_off[kSmB], pg_cnt;                                   // entry of (sequence b, table position t) = pg_off[b] + t
   int k0_early;                                               // the setup already requested K of the first sub-tile
+  int q_early;                                                // ... and the Q tile of the first piece
+  int f0, f1;                                                 // this CTA's half tiles [f0, f1) of the flat list
   uint64_t full[kTcStages], empty[kTcStages];
   uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup, app_done, mrg_full;
   uint32_t tmem_base;
@@ -120,6 +122,12 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -155,12 +163,11 @@ struct SubTile {
 struct SubCursor {
   const SmSmem& sm;
   int B, f, f1, b, prev_b;
-  __device__ SubCursor(const SmSmem& sm_, int B_, int cta, int n_cta) : sm(sm_), B(B_) {
-    const unsigned T = (unsigned)sm_.gpre[B_];
-    f = (int)((unsigned)cta * T / (unsigned)n_cta);
-    f1 = (int)((unsigned)(cta + 1) * T / (unsigned)n_cta);
+  __device__ SubCursor(const SmSmem& sm_, int B_) : sm(sm_), B(B_) {
+    f = sm_.f0; f1 = sm_.f1;                   // this CTA's share of the flat list (computed once by the setup)
     b = 0; prev_b = -1;
   }
+  // out of line on purpose: four roles walk the list, one copy of the code stays hot in the instruction cache
   __device__ bool next(SubTile& s) {
     if (f >= f1) return false;
     while (sm.gpre[b + 1] <= f) ++b;
@@ -387,14 +394,21 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     if (lane == 0) sm.gpre[0] = 0;
     const unsigned T = (unsigned)__shfl_sync(0xffffffffu, incl, p.B - 1);
     const int f0 = (int)((unsigned)cta * T / (unsigned)n_cta), f1 = (int)((unsigned)(cta + 1) * T / (unsigned)n_cta);
+    if (lane == 0) { sm.f0 = f0; sm.f1 = f1; }
     __syncwarp();
     // A range that starts in HCA rows needs nothing from global memory: its first K sub-tile is requested right here,
     // ahead of the table / counter look-ups below (sm.k0_early tells the producer loop)
     {
-      SubCursor c0(sm, p.B, cta, n_cta);
+      SubCursor c0(sm, p.B);
       SubTile s0;
-      const bool early = c0.next(s0) && s0.kind == 0 && !p.grow_wait;
-      if (lane == 0) sm.k0_early = early ? 1 : 0;
+      const bool any0 = c0.next(s0);
+      const bool early = any0 && s0.kind == 0 && !p.grow_wait;
+      const bool q_early = any0 && !p.wait_inputs && !p.in_ctr;   // q is ready: nothing to wait for before its tile is requested
+      if (lane == 0) { sm.k0_early = early ? 1 : 0; sm.q_early = q_early ? 1 : 0; }
+      if (q_early && elect_one()) {
+        mbar_arrive_expect_tx(&sm.q_full, 65536);
+        tma_load_3d(sm.q, &map_q, 0, s0.b * kTcH, 0, &sm.q_full);
+      }
       if (early && elect_one()) {
         const uint64_t pol = l2_policy_evict_first();
         const CUtensorMap* mk = (s0.b == 0 ? maps0.m : p.seq_maps + s0.b * 8) + (s0.rows == kTcTile ? 0 : 4);
@@ -406,30 +420,40 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
       }
     }
     int cnt = 0;                                       // page slots of this CTA's range, all sequences
-#pragma unroll
-    for (int b = 0; b < kSmB; ++b) {
+    // (rolled, and only over the sequences there are: this code runs once per CTA, instruction-cache cold)
+#pragma unroll 1
+    for (int b = 0; b < p.B; ++b) {
       const int end_b = __shfl_sync(0xffffffffu, incl, b), g_b = __shfl_sync(0xffffffffu, g, b);
       const int hca_b = __shfl_sync(0xffffffffu, hca, b), pg_b = __shfl_sync(0xffffffffu, pg, b), cur_b = __shfl_sync(0xffffffffu, q.cur, b);
-      if (b < p.B) {
+      {
         const int base = end_b - g_b + hca_b;          // first page half tile of sequence b in the flat list
         const int lo = max(f0, base), hi = min(f1, base + pg_b);
-        int off = -(1 << 30);
+        int off = -(1 << 30), vp = 0, vc = 0;
+        bool have = false;
         if (lo < hi) {
           const int t_lo = (lo - base) >> 1, n = ((hi - 1 - base) >> 1) - t_lo + 1;
           off = cnt - t_lo;
           if (lane >= cnt && lane < cnt + n) {
             const size_t e = ((size_t)b * 2 + cur_b) * p.k + t_lo + lane - cnt;
-            sm.pg_page[lane] = __ldcg(p.tbl_page + e);
-            sm.pg_chunk[lane] = __ldcg(p.tbl_chunk + e);
+            vp = __ldcg(p.tbl_page + e);
+            vc = __ldcg(p.tbl_chunk + e);
+            have = true;
           }
           cnt += n;
         }
+        // window rows in the range: ring rows appended by earlier launches are visible once app_epoch has caught up with
+        // the host's count (normally it has); HCA / tail-page rows handed over by an append kernel that runs beside the
+        // previous launch: grow_epoch.  Both counters are probed while the table loads are in flight - one round trip.
+        const bool need_app = lane == b && f1 > base + pg_b && f0 < end_b;
+        const bool need_grow = p.grow_wait && lane == b && f0 < end_b && f1 > end_b - g_b;
+        unsigned probe_a = 0, probe_g = 0;
+        if (need_app) probe_a = ld_relaxed_u32(&p.seqs[b].app_epoch);
+        if (need_grow) probe_g = ld_relaxed_u32(&p.seqs[b].grow_epoch);
+        if (have) { sm.pg_page[lane] = vp; sm.pg_chunk[lane] = vc; }
         if (lane == 0) sm.pg_off[b] = off;
-        // window rows in the range: ring rows appended by earlier launches are visible once app_epoch has caught
-        // up with the host's count (normally it has)
-        if (lane == b && f1 > base + pg_b && f0 < end_b) wait_counter(&p.seqs[b].app_epoch, q.app_count, 50);
-        // HCA / tail-page rows handed over by an append kernel that runs beside the previous launch
-        if (p.grow_wait && lane == b && f0 < end_b && f1 > end_b - g_b) wait_counter(&p.seqs[b].grow_epoch, q.grow_count, 57);
+        if (need_app && (int)(probe_a - q.app_count) < 0) wait_counter(&p.seqs[b].app_epoch, q.app_count, 50);
+        if (need_grow && (int)(probe_g - q.grow_count) < 0) wait_counter(&p.seqs[b].grow_epoch, q.grow_count, 57);
+        if (need_app || need_grow) fence_acq_rel_gpu();      // the relaxed probe becomes an acquire
         if (b > 0 && f0 < end_b && f1 > end_b - g_b && lane < 8) prefetch_tmap(p.seq_maps + b * 8 + lane);
       }
     }
@@ -454,7 +478,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   if (warp == 0) {
     // =========================== TMA producer ===========================
     if (elect_one()) {
-      SubCursor cur(sm, p.B, cta, n_cta);
+      SubCursor cur(sm, p.B);
       SubTile s, nx;
       uint32_t ring = sm.k0_early ? 4u : 0u;
       int item = 0;
@@ -500,12 +524,13 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
           app_gate(s);
           if (!k0_pending) issue4(mk, rk, s.rows);         // K of the piece's first sub-tile: in flight before Q is known
           k0_pending = false;
-          if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 10);
-          if (p.wait_inputs && !waited) { griddep_wait(); waited = true; }   // q is the caller's: whatever the stream ran last
-          if (p.in_ctr && !waited) { wait_counter(p.in_ctr, p.in_need, 55); fence_proxy_async_all(); waited = true; }
-                                                    // after griddep_wait
-          mbar_arrive_expect_tx(&sm.q_full, 65536);
-          tma_load_3d(sm.q, &map_q, 0, s.b * kTcH, 0, &sm.q_full);
+          if (item > 0 || !sm.q_early) {
+            if (item > 0) mbar_wait(&sm.q_empty, (item - 1) & 1, 10);
+            if (p.wait_inputs && !waited) { griddep_wait(); waited = true; }   // q is the caller's: whatever the stream ran last
+            if (p.in_ctr && !waited) { wait_counter(p.in_ctr, p.in_need, 55); fence_proxy_async_all(); waited = true; }
+            mbar_arrive_expect_tx(&sm.q_full, 65536);
+            tma_load_3d(sm.q, &map_q, 0, s.b * kTcH, 0, &sm.q_full);
+          }
         }
         have = cur.next(nx);
         if (!s.last) {                                     // K runs one sub-tile ahead of V inside a piece
@@ -537,7 +562,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
       const uint64_t dq0 = make_sdesc(smem_u32(sm.q), 16, 1024, kLayoutSw128);
       const uint64_t dp0 = make_sdesc(smem_u32(sm.p), 16384, 1024, kLayoutSw128);
       const uint64_t ones_desc = make_sdesc(smem_u32(sm.ones), 128, 256, kLayoutNone);
-      SubCursor cur(sm, p.B, cta, n_cta);
+      SubCursor cur(sm, p.B);
       SubTile s, nx;
       uint32_t ring = 0, n_s = 0, n_pv = 0;
       int item = 0;
@@ -626,7 +651,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     if (p.k_new) {
       // window append ("decoded tokens stay resident"; DESIGN R6): the CTA that owns the sub-tile holding
       // ring slot w_head of a sequence writes k_new / v_new there before its producer loads that sub-tile
-      SubCursor pc(sm, p.B, cta, n_cta);
+      SubCursor pc(sm, p.B);
       SubTile a;
       const int t = tid - 64;
       bool waited = false;
@@ -645,7 +670,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
       __syncwarp();
       if (lane == 0) mbar_arrive(&sm.app_done);
     }
-    SubCursor cur(sm, p.B, cta, n_cta);
+    SubCursor cur(sm, p.B);
     SubTile s;
     uint32_t tcount = 0, piece = 0;
     int b_first = -1, b_last = -1;
