@@ -290,6 +290,7 @@ struct TcPlan {
   TcParams params{};
   unsigned long long grid_total = 0;   // host mirror of the fused-S8 arrival counter
   int grid_max = 0;
+  int small_mergers = 32;              // small path: merging CTAs of a launch that shares the machine (measured: 16 / 24 / 48 / 64 are slower)
   size_t smem = 0;
   TcWorkspace* ws = nullptr;
 };
@@ -302,20 +303,22 @@ struct TcPlan {
 // written back to HBM between uses.  A context whose grid or batch does not fit an existing workspace of its
 // stream gets a new one.  Slots that a launch does not write are never read with effect (the combine kernels
 // skip slots that piece_info does not mark), so nothing is cleared between users.
+constexpr int kWsBufs = 3;              // a launch's partials are merged while the next two launches write theirs
 struct TcWorkspace {
   int device = 0;
   cudaStream_t stream = nullptr;
   size_t slots = 0, grid_max = 0;
   int refs = 0;
-  uint2* part_o = nullptr;              // two buffers of `slots` each: the small path alternates, the general path uses the first
+  uint2* part_o = nullptr;              // kWsBufs buffers of `slots` each: the small path rotates, the general path uses the first
   float *part_s = nullptr, *part_m = nullptr, *part_l = nullptr;
-  int2* piece_info = nullptr;           // two buffers of grid_max
-  // small path (lsa_attn_tc_small.cuh): launches so far; the CTAs that arrive per buffer / leave in total, as the
-  // host has enqueued them (the kernels wait for these totals)
-  unsigned int* ctrs = nullptr;         // DEVICE [3]: arrivals buffer 0, arrivals buffer 1, CTAs that have left
+  int2* piece_info = nullptr;           // kWsBufs buffers of grid_max
+  // small path (lsa_attn_tc_small.cuh): launches so far; the CTAs that arrive per buffer / the mergers that have finished
+  // in total, as the host has enqueued them (the kernels wait for these totals)
+  unsigned int* ctrs = nullptr;         // DEVICE [kWsBufs + 1]: arrivals per buffer, then the mergers that have finished
   unsigned long long n_small = 0;
-  unsigned int arr_total[2] = {0, 0};
-  unsigned int done_total = 0, done_total_prev = 0;     // after the last launch / after the one before it
+  unsigned int arr_total[kWsBufs] = {};
+  unsigned int done_total = 0;          // after the last launch
+  unsigned int done_hist[kWsBufs] = {}; // after each of the last kWsBufs launches (index: launch number mod kWsBufs)
   bool last_small = false;              // the last launch on this workspace did not wait for its predecessor
 };
 static std::mutex g_ws_mu;
@@ -334,16 +337,16 @@ static TcWorkspace* ws_acquire(cudaStream_t st, size_t slots, size_t grid_max, s
     if (w->device == device && w->stream == st && w->slots >= slots && w->grid_max >= grid_max) { ++w->refs; return w; }
   TcWorkspace* w = new TcWorkspace();
   w->device = device; w->stream = st; w->slots = slots; w->grid_max = grid_max; w->refs = 1;
-  cudaError_t e = cudaMalloc(&w->part_o, 2 * slots * (kTcH * kTcD / 4) * sizeof(uint2));
-  if (e == cudaSuccess) e = cudaMalloc(&w->part_s, 2 * slots * kTcPartScales * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&w->part_m, 2 * slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&w->part_l, 2 * slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, 2 * grid_max * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMalloc(&w->ctrs, 3 * sizeof(unsigned int));
-  if (e == cudaSuccess) e = cudaMemset(w->part_m, 0, 2 * slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMemset(w->part_l, 0, 2 * slots * kTcH * sizeof(float));
-  if (e == cudaSuccess) e = cudaMemset(w->piece_info, 0, 2 * grid_max * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMemset(w->ctrs, 0, 3 * sizeof(unsigned int));
+  cudaError_t e = cudaMalloc(&w->part_o, kWsBufs * slots * (kTcH * kTcD / 4) * sizeof(uint2));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_s, kWsBufs * slots * kTcPartScales * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_m, kWsBufs * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&w->part_l, kWsBufs * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, kWsBufs * grid_max * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMalloc(&w->ctrs, (kWsBufs + 1) * sizeof(unsigned int));
+  if (e == cudaSuccess) e = cudaMemset(w->part_m, 0, kWsBufs * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemset(w->part_l, 0, kWsBufs * slots * kTcH * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemset(w->piece_info, 0, kWsBufs * grid_max * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMemset(w->ctrs, 0, (kWsBufs + 1) * sizeof(unsigned int));
   if (e != cudaSuccess) {
     *msg = std::string("split-K workspace: ") + cudaGetErrorString(e);
     ws_free(w);
@@ -463,9 +466,9 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { *msg = "cuTensorMapEncodeTiled (partials) failed"; return -2; }
-    // the small-batch path's merge: both workspace buffers as one tensor [2 * slots][H*D/2]; box = the 256 B of one unit
-    // (4 heads x 32 d, fp16) of 32 consecutive slots
-    cuuint64_t dims2[2] = {(cuuint64_t)kTcH * kTcD / 2, (cuuint64_t)pl->ws->slots * 2};
+    // the small-batch path's merge: all workspace buffers as one tensor [kWsBufs * slots][H*D/2]; box = the 256 B of one
+    // unit (4 heads x 32 d, fp16) of 32 consecutive slots
+    cuuint64_t dims2[2] = {(cuuint64_t)kTcH * kTcD / 2, (cuuint64_t)pl->ws->slots * kWsBufs};
     cuuint32_t box2[2] = {64, 32};
     r = pl->encode(&pl->map_part_small, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, pl->ws->part_o, dims2, strides, box2, es,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -587,7 +590,11 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   const long long g_cap = (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 20) / 2);
   const long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
   const int n_attn = (int)std::max<long long>(1, std::min<long long>(g_cap, (halves + per - 1) / per));
-  const int buf = (int)(ws->n_small & 1);
+  const int buf = (int)(ws->n_small % kWsBufs);
+  // S8: the launch's last n_mrg CTAs to arrive merge its partials (8 units of 4 heads x 32 d each per round), the others
+  // leave their SM to the next launch at once; a launch that has the machine to itself lets every CTA merge
+  const int n_units = B * 256;
+  const int n_mrg = alone ? n_attn : std::min(n_attn, std::max(pl->small_mergers, (n_units + 15) / 16));
   const bool first_after_general = !ws->last_small;  // the general path's combine may still read buffer 0: wait for the stream
   prm.seqs = pl->init.d_seqs; prm.tbl_chunk = pl->init.pool.tbl_chunk; prm.tbl_page = pl->init.pool.tbl_page; prm.seq_maps = pl->d_maps8;
   prm.B = B; prm.k = pl->init.k; prm.n_attn = n_attn; prm.scale_log2 = pl->params.scale_log2;
@@ -599,11 +606,12 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   prm.slot_row0 = buf * (int)ws->slots;
   prm.piece_info = ws->piece_info + (size_t)buf * ws->grid_max;
   prm.arr_ctr = ws->ctrs + buf; prm.arr_target = (ws->arr_total[buf] += (unsigned)n_attn);
-  prm.done_ctr = ws->ctrs + 2;
-  prm.done_need_buf = ws->done_total_prev;           // the launch two back (same buffer) has been merged
+  prm.n_mrg = n_mrg;
+  prm.done_ctr = ws->ctrs + kWsBufs;
+  prm.done_need_buf = ws->done_hist[buf];            // the launch kWsBufs back (same buffer) has been merged
   prm.done_need_prev = ws->done_total;               // the previous launch has been merged
-  ws->done_total_prev = ws->done_total;
-  ws->done_total += (unsigned)n_attn;
+  ws->done_total += (unsigned)n_mrg;
+  ws->done_hist[buf] = ws->done_total;
   prm.done_after = ws->done_total;
   prm.host_flag = step.host_flag; prm.host_flag_val = step.host_flag_val;
   prm.out = (__nv_bfloat16*)out; prm.lse = lse; prm.swap = step.swap; prm.W = pl->init.W;

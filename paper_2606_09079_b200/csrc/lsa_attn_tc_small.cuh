@@ -24,15 +24,20 @@
 //
 // 3. S8 runs inside the launch.  A second kernel in the programmatic chain must sit resident and wait for the attention
 //    grid; measured, those waiting blocks pile up on the SMs the next step's CTAs need, and the host pays a second
-//    launch.  Instead every CTA publishes its partials, arrives at a counter (one per workspace buffer), waits for the
-//    launch's other CTAs and merges its share of the output: unit = 4 heads x 32 d; the 8 softmax warps take partials
-//    w, w+8, ... of every CTA of the launch (inactive ones are selected away, so no list is built first) - one
-//    round trip of loads per unit.  A second counter (done_ctr) is bumped on exit: it protects the reuse of the
-//    buffer two launches later and orders the merges of consecutive launches (records, `out`).  All CTAs of a
-//    launch are resident at the same time (grid <= SM count, one CTA per SM; a programmatically dependent launch
-//    starts only after every CTA of its predecessor has started), so the counter barrier cannot starve; waits are
-//    bounded and trap.  Contexts that run CONCURRENTLY on different streams could each hold part of the SMs and
-//    wait for the rest: such contexts must share stream_compute (they then share the workspace) or be run in turn.
+//    launch.  Instead every CTA publishes its partials and takes an arrival number from a counter (one per workspace
+//    buffer).  The launch's LAST n_mrg arrivals (32 of 64 at cfg 3) stay and merge: they wait for the stragglers among
+//    themselves, request the fp16 partials of their output units by TMA, weigh and sum them (unit = 4 heads x 32 d, one
+//    per warp and round).  Every earlier arrival LEAVES at once and its SM goes to the next launch's CTA.  A per-CTA
+//    timeline (%globaltimer at ten points, %smid) showed why: with every CTA waiting at a barrier for the slowest and
+//    then merging, a CTA spent 10 of its 26 us of residence not streaming, and the step time was SM residence / 148,
+//    not bytes / bandwidth (cfg 3: 12.45 -> 11.1 us per step).  A second counter (done_ctr, mergers only) orders the
+//    merges of consecutive launches (records, `out`) and protects the reuse of a workspace buffer three launches later.
+//    Mergers wait only for CTAs of their own launch and for mergers of EARLIER launches; every CTA of a launch has
+//    started before the next launch's first CTA starts (programmatic launch), and two launches together leave SMs free
+//    (grid <= (SMs - 20) / 2 unless the launch runs alone), so an unstarted CTA always finds an SM: the waits cannot
+//    starve; they are bounded and trap.  Contexts that run CONCURRENTLY on different streams could each hold part of
+//    the SMs and wait for the rest: such contexts must share stream_compute (they then share the workspace) or be run
+//    in turn.
 #pragma once
 #include <type_traits>
 
@@ -72,10 +77,11 @@ struct SmParams {
   int2* piece_info;
   unsigned int* arr_ctr;         // arrival counter of this launch's workspace buffer (cumulative over its launches)
   unsigned int arr_target;       // its value once every CTA of this launch has arrived
-  unsigned int* done_ctr;        // CTAs that have left, all launches of the workspace
+  int n_mrg;                     // the last n_mrg CTAs of the launch to arrive merge its partials (1 .. n_attn)
+  unsigned int* done_ctr;        // merging CTAs that have finished, all launches of the workspace
   unsigned int done_need_buf;    // value it has reached once the launch that used this buffer last has been merged
   unsigned int done_need_prev;   // value it has reached once the previous launch has been merged
-  unsigned int done_after;       // its value once this launch's last CTA has left
+  unsigned int done_after;       // its value once this launch's last merger has finished
   unsigned int* host_flag;       // lsa_step_host: PINNED HOST word (mapped) that receives host_flag_val when the launch's
   unsigned int host_flag_val;    // last CTA leaves, i.e. when `out` is complete - the host spins on it instead of
                                  // synchronising the stream; null otherwise
@@ -112,6 +118,7 @@ struct SmSmem {
   int k0_early;                                               // the setup already requested K of the first sub-tile
   int q_early;                                                // ... and the Q tile of the first piece
   int f0, f1;                                                 // this CTA's half tiles [f0, f1) of the flat list
+  int rank;                                                   // this CTA's arrival index among the launch's CTAs (S8)
   uint64_t full[kTcStages], empty[kTcStages];
   uint64_t q_full, q_empty, s_full[2], s_empty[2], p_full, pv_done, o_full[4], o_empty, setup, app_done, mrg_full;
   uint32_t tmem_base;
@@ -232,101 +239,110 @@ __device__ __forceinline__ float4 sm_warp_sum4(float4 v) {
 }
 __device__ __forceinline__ float sm_w_of(float m, float M) { return m == -INFINITY ? 0.f : exp2f(m - M); }
 
-// S8 (see the header, item 3).  Called by the 256 softmax threads (t = 0..255) of every CTA once all partials of the
-// launch are visible.  Unit = (sequence b, 32 consecutive uint2 columns cc of the partial layout) = 4 heads x 32 d, 256
-// per sequence; CTA c takes units [c * NU / n_cta, (c + 1) * NU / n_cta), kMuPer at a time.  The merge runs ONCE per
-// launch, so its cost is its code size as much as its data: an unrolled register version (40 loads in flight per thread)
-// was 27 KB of straight-line code fetched cold by every CTA (ncu: "no_instructions" the top stall reason, a third of all
-// samples inside the merge).  Here one thread requests the fp16 columns of all slots by TMA (2-D boxes of 32 slots x
-// 256 B into the shared memory the attention phase has left behind), one warp per unit meanwhile computes the weights
-// (lane l: slots l, l + 32, ...; the m / l / scale rows are contiguous along the slots), and the weighted sum is a short
-// rolled loop over shared memory.  Slots without a partial for the sequence get weight 0 and are skipped, never multiplied.
-constexpr int kMuPer = 4;                     // units per round
-constexpr int kMuSlots = 160;                 // n_cta at most
-__device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CUtensorMap* map_part, int cta, int n_cta, int t) {
+// S8 (see the header, item 3).  Called by the 256 softmax threads (t = 0..255) of the launch's MERGING CTAs once all
+// partials of the launch are visible.  Unit = (sequence b, 32 consecutive uint2 columns cc of the partial layout) = 4 heads
+// x 32 d, 256 per sequence; merger mi of n_mrg takes units [mi * NU / n_mrg, (mi + 1) * NU / n_mrg), one unit per warp and
+// round.  The merge runs ONCE per launch, so its cost is its latency chain and its code size as much as its data: one
+// thread requests the fp16 columns of all slots by TMA (2-D boxes of 32 slots x 256 B into the shared memory the attention
+// phase has left behind); meanwhile every warp fetches m / l / block scale of all slots of its unit in ONE round trip
+// (lane l: slots l, l + 32, ...; the rows are contiguous along the slots), parks them in shared memory, turns them into
+// weights, and then runs the weighted sum as a short rolled loop over shared memory.  Slots without a partial for the
+// sequence get weight 0 and are skipped, never multiplied.
+constexpr int kMuLandBytes = 160 * 1024;      // landing area at the start of q + stage (192 KiB contiguous); weights behind it
+struct MergePlan {
+  int n_box, rows, per;                       // 32-slot boxes per unit, their rows, units per round
+  int u0, u1;                                 // this merger's units
+};
+__device__ __forceinline__ MergePlan merge_plan(const SmParams& p, int mi, int n_mrg) {
+  MergePlan mp;
+  mp.n_box = (p.n_attn + 31) >> 5; mp.rows = mp.n_box * 32;
+  mp.per = mp.rows <= 64 ? 8 : 4;             // per * rows * 256 B <= kMuLandBytes
+  const unsigned NU = (unsigned)p.B * 256u;
+  mp.u0 = (int)((unsigned)mi * NU / (unsigned)n_mrg); mp.u1 = (int)((unsigned)(mi + 1) * NU / (unsigned)n_mrg);
+  return mp;
+}
+// one thread: request the fp16 columns of units [ub, ub + nu) of every slot of the launch
+__device__ __forceinline__ void merge_request(const SmParams& p, SmSmem& sm, const CUtensorMap* map_part, const MergePlan& mp, int ub, int nu) {
+  fence_proxy_async_all();                    // the partials were written by generic stores of other CTAs
+  mbar_arrive_expect_tx(&sm.mrg_full, (uint32_t)(nu * mp.rows * 256));
+#pragma unroll 1
+  for (int i = 0; i < nu; ++i) {
+    const int u = ub + i, b = u >> 8, cc = u & 255;
+#pragma unroll 1
+    for (int bx = 0; bx < mp.n_box; ++bx)
+      tma_load_2d(sm.q + (size_t)(i * mp.rows + bx * 32) * 256, map_part, cc * 64, p.slot_row0 + b + bx * 32, &sm.mrg_full);
+  }
+}
+// the 256 softmax threads; round 0 has been requested by the thread that saw the last arrival
+__device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CUtensorMap* map_part, int mi, int n_mrg, int t) {
   const int w = t >> 5, lane = t & 31;
-  unsigned char* land = sm.q;                                    // [kMuPer][rows][256 B]; q + stage are contiguous (192 KiB)
-  float4* wbuf = reinterpret_cast<float4*>(sm.p);                // [kMuPer][kMuSlots]: weight x block scale per head (10 KiB)
-  float4* ml = reinterpret_cast<float4*>(sm.ones);               // [kMuPer][2]: M, L
-  float4* red = ml + 2 * kMuPer;                                 // [kMuPer][32]
-  const int NU = p.B * 256;
-  const int u0 = (int)((unsigned)cta * (unsigned)NU / (unsigned)n_cta), u1 = (int)((unsigned)(cta + 1) * (unsigned)NU / (unsigned)n_cta);
-  const int n_box = (n_cta + 31) >> 5, rows = n_box * 32;
+  const int n_cta = p.n_attn;
+  const MergePlan mp = merge_plan(p, mi, n_mrg);
+  const int rows = mp.rows, per = mp.per;
+  unsigned char* land = sm.q;                                    // [per][rows][256 B]
+  float4* mbuf = reinterpret_cast<float4*>(sm.q + kMuLandBytes); // [per][rows]: m per head, then weight x block scale (<= 10 KiB)
+  float4* lbuf = mbuf + per * rows;                              // [per][rows]: l per head
+  float* sbuf = reinterpret_cast<float*>(lbuf + per * rows);     // [per][rows]: block scale
   const size_t ns = (size_t)p.n_slots;
   int round = 0;
-  for (int ub = u0; ub < u1; ub += kMuPer, ++round) {
-    const int nu = min(kMuPer, u1 - ub);
-    if (t == 0) {
-      fence_proxy_async_all();                                   // the partials were written by generic stores of other CTAs
-      mbar_arrive_expect_tx(&sm.mrg_full, (uint32_t)(nu * rows * 256));
-#pragma unroll 1
-      for (int i = 0; i < nu; ++i) {
-        const int u = ub + i, b = u >> 8, cc = u & 255;
-#pragma unroll 1
-        for (int bx = 0; bx < n_box; ++bx)
-          tma_load_2d(land + (size_t)(i * rows + bx * 32) * 256, map_part, cc * 64, p.slot_row0 + b + bx * 32, &sm.mrg_full);
-      }
-    }
-    if (w < nu) {                                                // weights of unit ub + w
-      const int u = ub + w, b = u >> 8, cc = u & 255;
-      const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
-      float4 M = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
-#pragma unroll 1
+  for (int ub = mp.u0; ub < mp.u1; ub += per, ++round) {
+    const int nu = min(per, mp.u1 - ub);
+    if (t == 0 && round > 0) merge_request(p, sm, map_part, mp, ub, nu);
+    const bool mine = w < nu;                                    // warp w: unit ub + w, start to finish
+    const int u = ub + (mine ? w : 0), b = u >> 8, cc = u & 255;
+    const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
+    float4 M = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+    float4 L = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (mine) {
+      float4* mw = mbuf + w * rows;
+      float4* lw = lbuf + w * rows;
+      float* sw = sbuf + w * rows;
+#pragma unroll 2
       for (int c = lane; c < n_cta; c += 32) {
         const size_t s_ = (size_t)c + b;
-        const int2 info = p.piece_info[c];
+        const int2 info = __ldcg(p.piece_info + c);
         const float* pm = p.part_m + (size_t)h0 * ns + s_;
-        float4 m4 = make_float4(pm[0], pm[ns], pm[2 * ns], pm[3 * ns]);
+        const float* pl = p.part_l + (size_t)h0 * ns + s_;
+        float4 m4 = make_float4(__ldcg(pm), __ldcg(pm + ns), __ldcg(pm + 2 * ns), __ldcg(pm + 3 * ns));
+        const float4 l4 = make_float4(__ldcg(pl), __ldcg(pl + ns), __ldcg(pl + 2 * ns), __ldcg(pl + 3 * ns));
+        const float s1 = __ldcg(p.part_s + (size_t)((m * 2 + hh) * 4 + dq) * ns + s_);
         // CTA c wrote a partial for sequence b, and the piece had an attended key (else it wrote no O)
         if (!(info.x <= b && b < info.x + info.y) || m4.x == -INFINITY) m4 = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
-        wbuf[w * kMuSlots + c] = m4;                             // parked: becomes the weight below
+        mw[c] = m4; lw[c] = l4; sw[c] = s1;
         M.x = fmaxf(M.x, m4.x); M.y = fmaxf(M.y, m4.y); M.z = fmaxf(M.z, m4.z); M.w = fmaxf(M.w, m4.w);
       }
       M = sm_warp_max4(M);
-      float4 L = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
       for (int c = lane; c < n_cta; c += 32) {
-        const size_t s_ = (size_t)c + b;
-        const float4 m4 = wbuf[w * kMuSlots + c];
+        const float4 m4 = mw[c];
         float4 wj = make_float4(0.f, 0.f, 0.f, 0.f);
         if (m4.x != -INFINITY) {
-          const float* pl = p.part_l + (size_t)h0 * ns + s_;
-          const float s1 = p.part_s[(size_t)((m * 2 + hh) * 4 + dq) * ns + s_];
+          const float4 l4 = lw[c];
+          const float s1 = sw[c];
           const float4 e = make_float4(sm_w_of(m4.x, M.x), sm_w_of(m4.y, M.y), sm_w_of(m4.z, M.z), sm_w_of(m4.w, M.w));
-          L.x = fmaf(e.x, pl[0], L.x); L.y = fmaf(e.y, pl[ns], L.y); L.z = fmaf(e.z, pl[2 * ns], L.z); L.w = fmaf(e.w, pl[3 * ns], L.w);
+          L.x = fmaf(e.x, l4.x, L.x); L.y = fmaf(e.y, l4.y, L.y); L.z = fmaf(e.z, l4.z, L.z); L.w = fmaf(e.w, l4.w, L.w);
           wj = make_float4(e.x * s1, e.y * s1, e.z * s1, e.w * s1);
         }
-        wbuf[w * kMuSlots + c] = wj;
+        mw[c] = wj;
       }
       L = sm_warp_sum4(L);
-      if (lane == 0) { ml[2 * w] = M; ml[2 * w + 1] = L; }
-    }
-    named_bar_sync(2, 256);
-    mbar_wait(&sm.mrg_full, round & 1, 57);
-    // weighted sum: warps i and i + 4 share unit i, half of the slots each; lane = one uint2 column (4 heads of one d)
-    const int i = w & 3, half = w >> 2;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (i < nu) {
-      const int s_lo = half * (rows >> 1), s_hi = min(n_cta, s_lo + (rows >> 1));
-      const unsigned char* lp = land + (size_t)i * rows * 256 + lane * 8;
-#pragma unroll 4
-      for (int sl = s_lo; sl < s_hi; ++sl) {
-        const float4 f = wbuf[i * kMuSlots + sl];
-        if (f.x != 0.f || f.y != 0.f || f.z != 0.f || f.w != 0.f) {
-          const uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
-          const float2 a01 = unpack_f16x2(v.x), a23 = unpack_f16x2(v.y);
-          acc.x = fmaf(f.x, a01.x, acc.x); acc.y = fmaf(f.y, a01.y, acc.y);
-          acc.z = fmaf(f.z, a23.x, acc.z); acc.w = fmaf(f.w, a23.y, acc.w);
-        }
+      __syncwarp();
+      mbar_wait(&sm.mrg_full, round & 1, 57);
+      // weighted sum: lane = one uint2 column (4 heads of one d); a slot of weight 0 is selected away, never multiplied
+      const unsigned char* lp = land + (size_t)w * rows * 256 + lane * 8;
+#pragma unroll 8
+      for (int sl = 0; sl < n_cta; ++sl) {
+        const float4 f = mw[sl];
+        uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
+        if (f.x == 0.f && f.y == 0.f && f.z == 0.f && f.w == 0.f) v = make_uint2(0u, 0u);
+        const float2 a01 = unpack_f16x2(v.x), a23 = unpack_f16x2(v.y);
+        acc.x = fmaf(f.x, a01.x, acc.x); acc.y = fmaf(f.y, a01.y, acc.y);
+        acc.z = fmaf(f.z, a23.x, acc.z); acc.w = fmaf(f.w, a23.y, acc.w);
       }
-      if (half == 1) red[i * 32 + lane] = acc;
     }
-    named_bar_sync(2, 256);
-    if (half == 0 && i < nu) {                                   // one warp per unit writes 4 heads x 32 d
-      const int u = ub + i, b = u >> 8, cc = u & 255;
-      const int dq = cc & 3, g = (cc >> 2) & 7, hh = (cc >> 5) & 1, m = cc >> 6, h0 = hh * 32 + g * 4;
-      const float4 a = red[i * 32 + lane], M = ml[2 * i], L = ml[2 * i + 1];
-      acc.x += a.x; acc.y += a.y; acc.z += a.z; acc.w += a.w;
+    if (round == 0) named_bar_sync(4, 288);                      // the previous launch has been merged: `out` may be written
+    if (mine) {
       __nv_bfloat16* o = p.out + ((size_t)b * kTcH + h0) * kTcD + m * 128 + dq * 32 + lane;
       o[0] = __float2bfloat16_rn(L.x > 0.f ? acc.x / L.x : 0.f);
       o[kTcD] = __float2bfloat16_rn(L.y > 0.f ? acc.y / L.y : 0.f);
@@ -340,7 +356,10 @@ __device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CU
         ls[3] = L.w > 0.f ? (M.w + log2f(L.w)) * 0.6931471805599453f : -INFINITY;
       }
     }
-    named_bar_sync(2, 256);                                      // landing buffer, wbuf, red are reused by the next round
+    if (ub + per < mp.u1) {                                      // the landing buffer and the weights are reused by the next round
+      if (!mine) mbar_wait(&sm.mrg_full, round & 1, 58);         // (idle warps keep up with the barrier's phase)
+      named_bar_sync(2, 256);
+    }
   }
 }
 
@@ -469,8 +488,6 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   } else {
     for (int i = tid - 64; i < 2048; i += kTcThreads - 64) reinterpret_cast<uint16_t*>(sm.ones)[i] = 0x3f80;   // bf16 1.0
     fence_proxy_async_smem();
-    // the partials of two launches ago (same buffer) have been merged
-    if (tid == 64) wait_counter(p.done_ctr, p.done_need_buf, 51);
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm.setup);
   }
@@ -544,7 +561,6 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (s.last) ++item;
         s = nx;
       }
-                                                    // all loads issued
     }
   } else if (warp == 1) {
     // =========================== MMA issuer ===========================
@@ -636,7 +652,6 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (s.last) ++item;
         s = nx;
       }
-                                                    // last PV issued (last V landed)
     }
   } else {
     // =========================== softmax + epilogue (8 warps) ===========================
@@ -648,6 +663,9 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
     const uint32_t tS = tmem, tO = tmem + 128, tL = tmem + 384;
+    // the launch that used this workspace buffer last (three launches ago) has been merged: normally long ago.  The
+    // other softmax warps meet this one at the named barrier of their first sub-tile, before any of them writes a partial.
+    if (tid == 64) wait_counter(p.done_ctr, p.done_need_buf, 51);
     if (p.k_new) {
       // window append ("decoded tokens stay resident"; DESIGN R6): the CTA that owns the sub-tile holding
       // ring slot w_head of a sequence writes k_new / v_new there before its producer loads that sub-tile
@@ -819,37 +837,57 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     }
     if (tid == 64) p.piece_info[cta] = make_int2(b_first < 0 ? 0 : b_first, b_first < 0 ? 0 : b_last - b_first + 1);
   }
-  // ---- S8: publish, meet the other CTAs of the launch, merge this CTA's share ----
+  // ---- S8: publish; the launch's last n_mrg CTAs to arrive merge its partials, the others leave their SM at once ----
   tc_fence_before();
-  if (warp >= 2) __threadfence();                   // this thread's partial stores are visible device-wide
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(sm.tmem_base, 512);
   }
   if (tid == 0) {
-    red_release_add_u32(p.arr_ctr, 1u);
-    wait_counter(p.arr_ctr, p.arr_target, 53);      // every partial of the launch is visible from here on
-    wait_counter(p.done_ctr, p.done_need_prev, 54); // the previous launch has been merged (records, `out`)
+    __threadfence();                                // cumulative: the partial stores of every thread of this CTA (ordered before
+    const unsigned int old = atomicAdd(p.arr_ctr, 1u);   // this thread by the barrier) are visible before the arrival is
+    sm.rank = (int)(old - (p.arr_target - (unsigned)n_cta));   // arrival index inside this launch, 0 .. n_cta - 1
   }
   __syncthreads();
-  if (cta == 0 && tid < p.B) {                      // the per-sequence record catches up with the launch's view
-    SeqDev& sd = p.seqs[tid];
-    if (((p.swap >> tid) & 1u) && sd.pending) { sd.cur_buf = 1 - sd.cur_buf; sd.pending = 0; }
-    if (p.k_new) {
-      const int slot = sd.w_head;
-      sd.w_head = (slot + 1 == p.W) ? 0 : slot + 1;
-      sd.w_len = min(p.W, sd.w_len + 1);
-    }
+  const int mi = sm.rank - (n_cta - p.n_mrg);       // the last n_mrg arrivals are the mergers 0 .. n_mrg - 1
+  if (mi < 0) {
+    if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
+    return;
   }
-  if (warp >= 2) {
-    small_merge(p, sm, &map_part, cta, n_cta, tid - 64);
+  // mergers: warp 0 sees the last arrival, requests the first round of partials and then waits for the previous launch's
+  // merge (records, `out`); the softmax warps start on the weights as soon as the partials are visible
+  if (warp == 0) {
+    if (lane == 0) {
+      wait_counter(p.arr_ctr, p.arr_target, 53);    // every partial of the launch is visible from here on
+      const MergePlan mp = merge_plan(p, mi, p.n_mrg);
+      merge_request(p, sm, &map_part, mp, mp.u0, min(mp.per, mp.u1 - mp.u0));
+    }
+    __syncwarp();
+    named_bar_sync(3, 288);
+    if (lane == 0) {
+      wait_counter(p.done_ctr, p.done_need_prev, 54);   // the previous launch has been merged
+    }
+    __syncwarp();
+    if (mi == 0 && lane < p.B) {                    // the per-sequence record catches up with the launch's view
+      SeqDev& sd = p.seqs[lane];
+      if (((p.swap >> lane) & 1u) && sd.pending) { sd.cur_buf = 1 - sd.cur_buf; sd.pending = 0; }
+      if (p.k_new) {
+        const int slot = sd.w_head;
+        sd.w_head = (slot + 1 == p.W) ? 0 : slot + 1;
+        sd.w_len = min(p.W, sd.w_len + 1);
+      }
+    }
+    named_bar_sync(4, 288);
+  } else if (warp >= 2) {
+    named_bar_sync(3, 288);
+    small_merge(p, sm, &map_part, mi, p.n_mrg, tid - 64);
   }
   __syncthreads();
   if (tid == 0) {
     if (p.host_flag) {
       // `out` may live in pinned host memory: this CTA's rows are visible system-wide before it is counted, and the
-      // CTA that completes the count tells the host
+      // merger that completes the count tells the host
       __threadfence_system();
       const unsigned int old = atomicAdd(p.done_ctr, 1u);
       if (old + 1u == p.done_after) {
