@@ -582,13 +582,17 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
     d.n_csa = s.n_csa;
     halves += (s.n_hca + kSmHalf - 1) / kSmHalf + 2 * (h.n_cur >= 0 ? h.n_cur : s.k_eff) + (h.w_len + kSmHalf - 1) / kSmHalf;
   }
-  // Two launches are in flight at a time (the next one starts on the SMs this one leaves free), so a launch takes just
-  // under half the SMs - the rest is headroom for the trigger side band - and every CTA the same number of half tiles
-  // (a launch that waits for the stream anyway - trigger-free swap steps, host-synchronous steps - has no neighbour to
-  // share the machine with and takes every SM)
+  // About three launches are in flight at a time (a launch's CTAs start on the SMs its predecessors' CTAs leave), so a
+  // launch takes a third of the SMs and every CTA the same, EVEN number of half tiles where the list allows it (an even
+  // share keeps the two halves of a 128-row tile together; a lone half is a 64-row box that still costs M = 128 MMAs).
+  // Fewer, longer pieces amortise what a CTA pays once - its set-up, the wait for its first rows, the hand-over of the SM
+  // (~9 us against ~1.3 us per half tile) - and the step time is SM residence / SM count; measured at cfg 3 (us per
+  // step): 32 CTAs 11.2, 48: 10.5, 55: 10.6, 64: 10.85.  A launch that waits for the stream anyway - trigger-free swap
+  // steps, host-synchronous steps - has no neighbour to share the machine with and takes every SM.
   const bool alone = step.serialize || step.alone;
-  const long long g_cap = (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 20) / 2);
-  const long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
+  const long long g_cap = (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 4) / 3);
+  long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
+  if (!alone && per > 1 && (per & 1)) ++per;
   const int n_attn = (int)std::max<long long>(1, std::min<long long>(g_cap, (halves + per - 1) / per));
   const int buf = (int)(ws->n_small % kWsBufs);
   // S8: the launch's last n_mrg CTAs to arrive merge its partials (8 units of 4 heads x 32 d each per round), the others
