@@ -298,19 +298,31 @@ __device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CU
       float4* mw = mbuf + w * rows;
       float4* lw = lbuf + w * rows;
       float* sw = sbuf + w * rows;
-#pragma unroll 2
-      for (int c = lane; c < n_cta; c += 32) {
-        const size_t s_ = (size_t)c + b;
-        const int2 info = __ldcg(p.piece_info + c);
-        const float* pm = p.part_m + (size_t)h0 * ns + s_;
-        const float* pl = p.part_l + (size_t)h0 * ns + s_;
-        float4 m4 = make_float4(__ldcg(pm), __ldcg(pm + ns), __ldcg(pm + 2 * ns), __ldcg(pm + 3 * ns));
-        const float4 l4 = make_float4(__ldcg(pl), __ldcg(pl + ns), __ldcg(pl + 2 * ns), __ldcg(pl + 3 * ns));
-        const float s1 = __ldcg(p.part_s + (size_t)((m * 2 + hh) * 4 + dq) * ns + s_);
+      // two slots per lane and trip (all of them at up to 64 CTAs), every load issued before the first store
+#pragma unroll 1
+      for (int c = lane; c < n_cta; c += 64) {
+        const bool two = c + 32 < n_cta;
+        const int c2 = two ? c + 32 : c;
+        const size_t sa = (size_t)c + b, sb = (size_t)c2 + b;
+        const float* pm = p.part_m + (size_t)h0 * ns;
+        const float* pl = p.part_l + (size_t)h0 * ns;
+        const float* ps = p.part_s + (size_t)((m * 2 + hh) * 4 + dq) * ns;
+        const int2 ia = __ldcg(p.piece_info + c), ib = __ldcg(p.piece_info + c2);
+        float4 ma = make_float4(__ldcg(pm + sa), __ldcg(pm + ns + sa), __ldcg(pm + 2 * ns + sa), __ldcg(pm + 3 * ns + sa));
+        float4 mb = make_float4(__ldcg(pm + sb), __ldcg(pm + ns + sb), __ldcg(pm + 2 * ns + sb), __ldcg(pm + 3 * ns + sb));
+        const float4 la = make_float4(__ldcg(pl + sa), __ldcg(pl + ns + sa), __ldcg(pl + 2 * ns + sa), __ldcg(pl + 3 * ns + sa));
+        const float4 lb = make_float4(__ldcg(pl + sb), __ldcg(pl + ns + sb), __ldcg(pl + 2 * ns + sb), __ldcg(pl + 3 * ns + sb));
+        const float s1a = __ldcg(ps + sa), s1b = __ldcg(ps + sb);
         // CTA c wrote a partial for sequence b, and the piece had an attended key (else it wrote no O)
-        if (!(info.x <= b && b < info.x + info.y) || m4.x == -INFINITY) m4 = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
-        mw[c] = m4; lw[c] = l4; sw[c] = s1;
-        M.x = fmaxf(M.x, m4.x); M.y = fmaxf(M.y, m4.y); M.z = fmaxf(M.z, m4.z); M.w = fmaxf(M.w, m4.w);
+        const float4 none = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+        if (!(ia.x <= b && b < ia.x + ia.y) || ma.x == -INFINITY) ma = none;
+        if (!(ib.x <= b && b < ib.x + ib.y) || mb.x == -INFINITY) mb = none;
+        mw[c] = ma; lw[c] = la; sw[c] = s1a;
+        M.x = fmaxf(M.x, ma.x); M.y = fmaxf(M.y, ma.y); M.z = fmaxf(M.z, ma.z); M.w = fmaxf(M.w, ma.w);
+        if (two) {
+          mw[c2] = mb; lw[c2] = lb; sw[c2] = s1b;
+          M.x = fmaxf(M.x, mb.x); M.y = fmaxf(M.y, mb.y); M.z = fmaxf(M.z, mb.z); M.w = fmaxf(M.w, mb.w);
+        }
       }
       M = sm_warp_max4(M);
 #pragma unroll 1
@@ -329,13 +341,14 @@ __device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CU
       L = sm_warp_sum4(L);
       __syncwarp();
       mbar_wait(&sm.mrg_full, round & 1, 57);
-      // weighted sum: lane = one uint2 column (4 heads of one d); a slot of weight 0 is selected away, never multiplied
+      // weighted sum: lane = one uint2 column (4 heads of one d).  A slot without a partial for this sequence has weight 0
+      // and holds what an earlier launch left there, which is finite fp16 (the workspace is zeroed when it is created and
+      // partials are scaled into the fp16 range before they are stored), so 0 x stale = 0: no select in the loop
       const unsigned char* lp = land + (size_t)w * rows * 256 + lane * 8;
 #pragma unroll 8
       for (int sl = 0; sl < n_cta; ++sl) {
         const float4 f = mw[sl];
-        uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
-        if (f.x == 0.f && f.y == 0.f && f.z == 0.f && f.w == 0.f) v = make_uint2(0u, 0u);
+        const uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
         const float2 a01 = unpack_f16x2(v.x), a23 = unpack_f16x2(v.y);
         acc.x = fmaf(f.x, a01.x, acc.x); acc.y = fmaf(f.y, a01.y, acc.y);
         acc.z = fmaf(f.z, a23.x, acc.z); acc.w = fmaf(f.w, a23.y, acc.w);
@@ -860,11 +873,21 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   if (warp == 0) {
     if (lane == 0) {
       wait_counter(p.arr_ctr, p.arr_target, 53);    // every partial of the launch is visible from here on
-      const MergePlan mp = merge_plan(p, mi, p.n_mrg);
-      merge_request(p, sm, &map_part, mp, mp.u0, min(mp.per, mp.u1 - mp.u0));
     }
     __syncwarp();
-    named_bar_sync(3, 288);
+    named_bar_sync(3, 288);                         // the softmax warps start on the weights
+    {                                               // round 0 of the partials: one 32-slot box per lane
+      const MergePlan mp = merge_plan(p, mi, p.n_mrg);
+      const int nu = min(mp.per, mp.u1 - mp.u0);
+      if (lane == 0) mbar_arrive_expect_tx(&sm.mrg_full, (uint32_t)(nu * mp.rows * 256));
+      __syncwarp();
+      if (lane < nu * mp.n_box) {
+        const int i = lane / mp.n_box, bx = lane - i * mp.n_box;
+        const int u = mp.u0 + i, b = u >> 8, cc = u & 255;
+        fence_proxy_async_all();                    // the partials were written by generic stores of other CTAs
+        tma_load_2d(sm.q + (size_t)(i * mp.rows + bx * 32) * 256, &map_part, cc * 64, p.slot_row0 + b + bx * 32, &sm.mrg_full);
+      }
+    }
     if (lane == 0) {
       wait_counter(p.done_ctr, p.done_need_prev, 54);   // the previous launch has been merged
     }
