@@ -590,9 +590,10 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   // share keeps the two halves of a 128-row tile together; a lone half is a 64-row box that still costs M = 128 MMAs).
   // Fewer, longer pieces amortise what a CTA pays once - its set-up, the wait for its first rows, the hand-over of the SM
   // (~9 us against ~1.3 us per half tile) - and the step time is SM residence / SM count; measured at cfg 3 (us per
-  // step): 32 CTAs 11.2, 48: 10.5, 55: 10.6, 64: 10.85.  A launch that waits for the stream anyway - trigger-free swap
-  // steps, host-synchronous steps - has no neighbour to share the machine with and takes every SM.
-  const bool alone = step.serialize || step.alone;
+  // step): 32 CTAs 11.2, 48: 10.5, 55: 10.6, 64: 10.85.  A launch the host blocks on has no neighbour to share the
+  // machine with and takes every SM; a launch that merely waits for the stream (a swap step: the fetch event) keeps the
+  // shared size, because the launches BEHIND it overlap it again (all SMs there: 10.2 us per step, shared size: 10.0).
+  const bool alone = step.alone;
   const long long g_cap = (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 4) / 3);
   long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
   if (!alone && per > 1 && (per & 1)) ++per;

@@ -25,19 +25,20 @@
 // 3. S8 runs inside the launch.  A second kernel in the programmatic chain must sit resident and wait for the attention
 //    grid; measured, those waiting blocks pile up on the SMs the next step's CTAs need, and the host pays a second
 //    launch.  Instead every CTA publishes its partials and takes an arrival number from a counter (one per workspace
-//    buffer).  The launch's LAST n_mrg arrivals (32 of 64 at cfg 3) stay and merge: they wait for the stragglers among
+//    buffer).  The launch's LAST n_mrg arrivals (32 of 48 at cfg 3) stay and merge: they wait for the stragglers among
 //    themselves, request the fp16 partials of their output units by TMA, weigh and sum them (unit = 4 heads x 32 d, one
 //    per warp and round).  Every earlier arrival LEAVES at once and its SM goes to the next launch's CTA.  A per-CTA
 //    timeline (%globaltimer at ten points, %smid) showed why: with every CTA waiting at a barrier for the slowest and
 //    then merging, a CTA spent 10 of its 26 us of residence not streaming, and the step time was SM residence / 148,
-//    not bytes / bandwidth (cfg 3: 12.45 -> 11.1 us per step).  A second counter (done_ctr, mergers only) orders the
-//    merges of consecutive launches (records, `out`) and protects the reuse of a workspace buffer three launches later.
+//    not bytes / bandwidth (cfg 3: 12.45 -> 10.85 us per step, 10.0 with the changes that followed).
+//    A second counter (done_ctr, mergers only) orders the merges of consecutive launches (records, `out`) and protects
+//    the reuse of a workspace buffer three launches later.
 //    Mergers wait only for CTAs of their own launch and for mergers of EARLIER launches; every CTA of a launch has
-//    started before the next launch's first CTA starts (programmatic launch), and two launches together leave SMs free
-//    (grid <= (SMs - 20) / 2 unless the launch runs alone), so an unstarted CTA always finds an SM: the waits cannot
-//    starve; they are bounded and trap.  Contexts that run CONCURRENTLY on different streams could each hold part of
-//    the SMs and wait for the rest: such contexts must share stream_compute (they then share the workspace) or be run
-//    in turn.
+//    started before the next launch's first CTA starts (programmatic launch), so the only CTAs that can hold an SM
+//    while an unstarted CTA still needs one are that launch's own mergers - at most 32 SMs - and the waits cannot
+//    starve (a launch that runs alone lets all its CTAs merge: grid <= SM count, one CTA per SM, all resident);
+//    they are bounded and trap.  Contexts that run CONCURRENTLY on different streams could each hold part of the SMs
+//    and wait for the rest: such contexts must share stream_compute (they then share the workspace) or be run in turn.
 #pragma once
 #include <type_traits>
 
