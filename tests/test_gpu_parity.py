@@ -747,6 +747,37 @@ def test_small_batch_steps_back_to_back_without_sync(overlap):
         r["ctx"].close()
 
 
+@pytest.mark.parametrize("max_ctas,n_rows,w_len", [(0, [11200], [900]), (40, [3333], [1100]), (100, [11000], [1000]),
+                                                   (100, [7000, 5000], [1000, 160]), (0, [3000, 2000, 1500, 800], [500, 64, 0, 129])])
+def test_small_batch_last_arrivals_merge(max_ctas, n_rows, w_len):
+    """S8 of the small-batch kernel (step_overlap = 1): only the launch's last arrivals merge, the other CTAs leave.
+    Shapes and CTA caps that give (a) 48 CTAs with 32 mergers of one round each, (b) 36 CTAs and a ragged last piece,
+    (c) 94 CTAs: more than 64 partial slots (3 boxes of 32 slots, 4 units per round), 32 mergers of two rounds each beside
+    62 leavers, (d) two sequences: 16 units per merger, (e) four sequences: every CTA merges, four rounds each.  Seven
+    launches back to back walk twice through the three workspace buffers; every output against the oracle's attention."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 1200
+    g = torch.Generator().manual_seed(41)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    B = len(n_rows)
+    hk, hv = [rnd(n, D) for n in n_rows], [rnd(n, D) for n in n_rows]
+    wk, wv = [rnd(W, D) for _ in range(B)], [rnd(W, D) for _ in range(B)]
+    qs = [rnd(B, H, D) for _ in range(7)]
+    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.05, max_ctas=max_ctas,
+                      attn_impl=lsa.LSA_ATTN_TCGEN05, step_overlap=1)
+    res = [ctx.decode_attention(q, want_lse=True) for q in qs]      # no synchronisation in between
+    ctx.sync()
+    for q, (out, lse) in zip(qs, res):
+        for b in range(B):
+            K = np.concatenate([hk[b].double().cpu().numpy(), wk[b][: w_len[b]].double().cpu().numpy()])
+            V = np.concatenate([hv[b].double().cpu().numpy(), wv[b][: w_len[b]].double().cpu().numpy()])
+            ref, ref_lse, _ = attention(q[b].double().cpu().numpy(), K, V, 0.05)
+            np.testing.assert_allclose(out[b].double().cpu().numpy(), ref, err_msg=f"seq {b}", **attn_tolerance("bf16"))
+            np.testing.assert_allclose(lse[b].cpu().numpy(), ref_lse, atol=2e-2, rtol=1e-3)
+    ctx.close()
+
+
 def test_small_batch_step_overlap_lockstep():
     """lsa_config.step_overlap = 1 (inputs independent of the previous step's output): the whole path in lock-step with
     the oracle over several trigger periods - triggers, swaps (serialised launches) and the overlapped steps between them."""
