@@ -89,6 +89,53 @@ def stored_traffic(config_id, overlap):
     return d["traffic_bytes"], f"ncu --set full, commit {d.get('commit')} ({d.get('file')})"
 
 
+def summarise_timeline(records, step_ms):
+    """Per-CTA timeline of the small-batch attention launches (include/lsa.h LSA_TL_*): records = one uint64 array
+    [launch record][CTA][event] per context.  Means over all stamped CTAs, in microseconds: where a CTA's residence on its SM
+    goes, how long an SM stays empty between two CTAs, and the step time that SM residence alone would give."""
+    import numpy as np
+    ENTRY, SETUP, FIRST_S, LAST_PV, EPI, ARRIVED, ALL_ARR, MERGED, EXIT, SMID, NCTAS, SEQ = range(12)
+    rows = []
+    n_launches = 0
+    for rec in records:
+        a = rec.astype(np.int64)
+        for l in range(a.shape[0]):
+            n = int(a[l, 0, NCTAS])
+            if n <= 0 or n > a.shape[1] or (a[l, :n, EXIT] <= a[l, :n, ENTRY]).any():
+                continue                            # never written, or overwritten while it was read
+            rows.append(a[l, :n])
+            n_launches += 1
+    if not rows:
+        return None
+    e = np.concatenate(rows)
+    mrg = e[:, MERGED] > 0
+    us = lambda x: float(np.mean(x)) / 1e3
+    res = e[:, EXIT] - e[:, ENTRY]
+    by_sm = {}
+    for r_ in e:
+        by_sm.setdefault(int(r_[SMID]), []).append((int(r_[ENTRY]), int(r_[EXIT])))
+    gaps = []
+    for v in by_sm.values():
+        v.sort()
+        gaps += [b0 - a1 for (_, a1), (b0, _) in zip(v, v[1:]) if 0 <= b0 - a1 < 8000]     # consecutive CTAs on one SM
+    sm_us_per_launch = float(res.sum()) / 1e3 / n_launches
+    handover = float(np.median(gaps)) / 1e3 if gaps else None
+    ctas = len(e) / n_launches
+    out = dict(launches=n_launches, ctas_per_launch=ctas, mergers_per_launch=float(mrg.sum()) / n_launches, sms_seen=len(by_sm),
+               step_us=step_ms * 1e3,
+               all_ctas_us=dict(entry_to_setup=us(e[:, SETUP] - e[:, ENTRY]), entry_to_first_s=us(e[:, FIRST_S] - e[:, ENTRY]),
+                                first_s_to_last_pv=us(e[:, LAST_PV] - e[:, FIRST_S]), last_pv_to_epilogue=us(e[:, EPI] - e[:, LAST_PV]),
+                                epilogue_to_arrived=us(e[:, ARRIVED] - e[:, EPI])),
+               leavers_us=dict(residence=us(res[~mrg])) if (~mrg).any() else None,
+               mergers_us=dict(arrived_to_all_arrived=us(e[mrg, ALL_ARR] - e[mrg, ARRIVED]), all_arrived_to_merged=us(e[mrg, MERGED] - e[mrg, ALL_ARR]),
+                               residence=us(res[mrg])),
+               sm_residence_us_per_launch=sm_us_per_launch, handover_us_median=handover,
+               step_us_if_sm_bound=(sm_us_per_launch + ctas * (handover or 0.0)) / 148.0,
+               note="stamps of %globaltimer by one thread per CTA; step_us is the step time of the stamped stretch (the stamps cost a little); "
+                    "step_us_if_sm_bound = (summed residence + hand-over per CTA) / 148 SMs")
+    return out
+
+
 def replicas_for(c, l2_bytes):
     return max(1, math.ceil(2 * l2_bytes / c.attn_bytes_per_step()))
 
@@ -314,6 +361,7 @@ def main():
     ap.add_argument("--export", action="store_true", help="also time lsa_export_chunks (NEXT-4: KV export HBM -> pinned cold pool)")
     ap.add_argument("--cold-fp8", action="store_true", help="FP8 (e4m3) cold pages: half the bytes per recall over the host link (not BASELINE's config: reported under run.cold_format)")
     ap.add_argument("--growth", action="store_true", help="also time the step with a growing compressed history (NEXT-4: lsa_append_compressed)")
+    ap.add_argument("--timeline", action="store_true", help="also stamp a per-CTA timeline of the small-batch attention launches (lsa_timeline_*) over a separate stretch of steps and summarise it")
     ap.add_argument("--graph", action="store_true", help="also time lsa_step_graph (NEXT-3: the non-trigger step replayed from a CUDA graph)")
     ap.add_argument("--l2", action="store_true", help="also time the step with Level 2 (native Top-k inside the resident set, NEXT-2)")
     ap.add_argument("--l2-k2", type=int, default=2048, help="Level-2 Top-k (entries per sequence and step)")
@@ -853,6 +901,22 @@ def main():
                      captures=sum(g_["captures"] for g_ in gs), replays=sum(g_["replays"] for g_ in gs),
                      note="lsa_step_graph: steps without a trigger or a table swap replay one captured graph (attention + combine) per context")
 
+    # ---- per-CTA timeline of the small-batch launches (lsa_timeline_*; DESIGN 7.3): a stretch of its own, after every timed leg
+    timeline = None
+    if args.timeline and args.overlap and c.B <= 4 and stats["attn_impl"] == 2:
+        for r in reps:
+            r.ctx.timeline_enable(True)
+        n_tl = 2 * R * c.tau
+        for i in range(R * 8):                      # the stamps themselves are part of what is measured: settle first
+            one_step(i_next + i)
+        i_next += R * 8
+        ms_tl, _, _, _ = timed(n_tl, i0=i_next)
+        i_next += n_tl
+        tl = [r.ctx.timeline_read()[0] for r in reps]
+        for r in reps:
+            r.ctx.timeline_enable(False)
+        timeline = summarise_timeline(tl, ms_tl / n_tl)
+
     cpu_baseline = cpu_baseline_1t = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n, secs, threads = oracle_sample(wl, budget_s=12.0, max_steps=24)
@@ -876,7 +940,7 @@ def main():
                     tie_triggers_seen=n_tie_triggers[0], clocks=clocks, roofline=roofline, dependent_inputs=dependent,
                     cpu_baseline=cpu_baseline, cpu_baseline_1t=cpu_baseline_1t,
                     phases_ms={k_: (v["ms"] / v["count"] if v["count"] else None) for k_, v in phases_ms.items()},
-                    fetch=fetch, side_band=side_band, l1_indexer=l1, level2=level2, step_graph=graph, export=export, growth=growth, wall_s=wall,
+                    fetch=fetch, side_band=side_band, timeline=timeline, l1_indexer=l1, level2=level2, step_graph=graph, export=export, growth=growth, wall_s=wall,
                     host_enqueue_ms_per_step=enq_free * 1e3 / n_free, host_enqueue_ms_per_step_e2e=enq_e2e * 1e3 / n_e2e,
                     tokens_per_s=(units_job if tokens else units_job * (cfg.B if sharded else c.B)) / (ms * 1e-3))
         print(json.dumps(line))

@@ -366,6 +366,35 @@ enum lsa_phase { LSA_PH_PRESTEP = 0, LSA_PH_ATTENTION = 1, LSA_PH_COMBINE = 2, L
                  LSA_PH_COUNT = 7 };
 int lsa_profile_enable(lsa_ctx* ctx, int32_t capacity);
 int lsa_profile_read(lsa_ctx* ctx, double* ms_sum /* HOST [LSA_PH_COUNT] */, int64_t* count /* HOST [LSA_PH_COUNT] */);
+
+/* Per-CTA timeline of the small-batch attention launches (B <= 4 with lsa_config.step_overlap; DESIGN.md 7.3 explains what
+ * it showed: the step time of that path is the CTAs' summed residence / SM count, not bytes / bandwidth).
+ * lsa_timeline_enable(ctx, 1) allocates, once, a device ring of LSA_TL_LAUNCHES launch records and makes every small-batch
+ * launch of the context stamp %globaltimer (nanoseconds) at the points below, one row per CTA, into record (launch number mod
+ * LSA_TL_LAUNCHES); (ctx, 0) stops the stamping (the ring is kept).  Off, the launches run a kernel without any of it.
+ * lsa_timeline_read blocks on both streams, copies the ring to HOST dst[LSA_TL_LAUNCHES][LSA_TL_CTAS][LSA_TL_EVENTS]
+ * (uint64; rows of CTAs a launch did not have, and records never written, are 0) and stores the number of launches
+ * stamped so far in *n_launches (may be NULL).  Launches of more than LSA_TL_CTAS CTAs are not stamped.
+ * Errors: LSA_ERR_STATE (null ctx), LSA_ERR_INVALID_ARG (null dst), LSA_ERR_OOM, LSA_ERR_CUDA. */
+#define LSA_TL_LAUNCHES 16
+#define LSA_TL_CTAS 160
+#define LSA_TL_EVENTS 12
+enum lsa_tl_event {
+  LSA_TL_ENTRY = 0,        /* the CTA's barriers are initialised, its roles start                                      */
+  LSA_TL_SETUP = 1,        /* warp 0 has the piece boundaries, the table entries and the counters of its range         */
+  LSA_TL_FIRST_S = 2,      /* Q and the first K sub-tile have landed, the first S^T = K Q^T has been issued             */
+  LSA_TL_LAST_PV = 3,      /* the last O^T += V^T P^T has been issued (every K / V row of the piece has landed)         */
+  LSA_TL_EPILOGUE = 4,     /* the partial (O^T, l, m) of the last piece has been stored                                 */
+  LSA_TL_ARRIVED = 5,      /* the CTA has published its partials and taken its arrival number                          */
+  LSA_TL_ALL_ARRIVED = 6,  /* mergers only (0 for a CTA that left): every CTA of the launch has arrived                 */
+  LSA_TL_MERGED = 7,       /* mergers only: this CTA's share of `out` has been written                                  */
+  LSA_TL_EXIT = 8,         /* the CTA returns                                                                          */
+  LSA_TL_SMID = 9,         /* %smid, not a time                                                                        */
+  LSA_TL_NCTAS = 10,       /* CTAs of the launch, not a time                                                           */
+  LSA_TL_SEQ = 11          /* number of the launch among the context's stamped launches, not a time                    */
+};
+int lsa_timeline_enable(lsa_ctx* ctx, int32_t on);
+int lsa_timeline_read(lsa_ctx* ctx, uint64_t* dst /* HOST */, uint64_t* n_launches /* HOST, may be NULL */);
 int lsa_get_step(lsa_ctx* ctx, int32_t seq, int64_t* step);
 int lsa_sync(lsa_ctx* ctx);                      /* waits for both streams, reports device errors */
 const char* lsa_last_error(lsa_ctx* ctx);        /* ctx may be NULL: last init error             */

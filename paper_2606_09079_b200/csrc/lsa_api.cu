@@ -93,6 +93,9 @@ struct lsa_ctx {
   int prof_cap = 0;
   std::vector<cudaEvent_t> prof_ev[LSA_PH_COUNT];   // 2*cap events per phase
   int prof_n[LSA_PH_COUNT] = {0, 0, 0, 0, 0, 0, 0};
+  unsigned long long* d_tl = nullptr;               // lsa_timeline_enable: [LSA_TL_LAUNCHES][LSA_TL_CTAS][LSA_TL_EVENTS]
+  bool tl_on = false;
+  unsigned long long tl_seq = 0;                    // launches stamped so far
   unsigned long long* d_ktime = nullptr;            // [prof_cap][2] attention-kernel globaltimer stamps
   int ktime_cap = 0;
   // bookkeeping
@@ -665,6 +668,11 @@ static int attention_impl(lsa_ctx* c, const void* q, void* out, float* lse, cons
       c->serialize_next = false;
       c->inputs_from_prev_kernel = false;
       c->next_alone = false;
+      if (c->tl_on) {                               // lsa_timeline_enable: this launch's record of the ring
+        stp.tl = c->d_tl + (size_t)(c->tl_seq % LSA_TL_LAUNCHES) * LSA_TL_CTAS * LSA_TL_EVENTS;
+        stp.tl_seq = (unsigned int)c->tl_seq;
+        c->tl_seq += 1;
+      }
       if (c->host_flag_dev) {                       // lsa_step_host spins on the flag instead of synchronising the stream
         stp.host_flag = c->host_flag_dev;
         stp.host_flag_val = ++c->host_flag_seq;
@@ -1270,6 +1278,29 @@ extern "C" int lsa_get_step(lsa_ctx* ctx, int32_t seq, int64_t* step) {
   if (!ctx) return LSA_ERR_STATE;
   if (seq < 0 || seq >= ctx->B || !step) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "bad argument");
   *step = ctx->step[seq];
+  return LSA_OK;
+}
+
+extern "C" int lsa_timeline_enable(lsa_ctx* ctx, int32_t on) {
+  if (!ctx) return LSA_ERR_STATE;
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  if (on && !ctx->d_tl) {
+    int rc = dev_alloc(ctx, &ctx->d_tl, (size_t)LSA_TL_LAUNCHES * LSA_TL_CTAS * LSA_TL_EVENTS);   // zeroed
+    if (rc) return rc;
+  }
+  ctx->tl_on = on != 0;
+  return LSA_OK;
+}
+
+extern "C" int lsa_timeline_read(lsa_ctx* ctx, uint64_t* dst, uint64_t* n_launches) {
+  if (!ctx) return LSA_ERR_STATE;
+  if (!dst) LSA_FAIL(ctx, LSA_ERR_INVALID_ARG, "null dst");
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sf));
+  LSA_CUDA(ctx, cudaStreamSynchronize(ctx->sc));
+  const size_t bytes = (size_t)LSA_TL_LAUNCHES * LSA_TL_CTAS * LSA_TL_EVENTS * sizeof(uint64_t);
+  if (ctx->d_tl) LSA_CUDA(ctx, cudaMemcpy(dst, ctx->d_tl, bytes, cudaMemcpyDeviceToHost));
+  else memset(dst, 0, bytes);
+  if (n_launches) *n_launches = ctx->tl_seq;
   return LSA_OK;
 }
 

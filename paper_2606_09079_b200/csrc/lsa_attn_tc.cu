@@ -450,7 +450,8 @@ int tc_create(const TcInit& init, TcPlan** out, std::string* msg) {
     for (int j = 0; j < 8; ++j) pl->maps0.m[j] = maps8[j];
     TC_CUDA(cudaMalloc(&pl->d_maps8, maps8.size() * sizeof(CUtensorMap)));
     TC_CUDA(cudaMemcpy(pl->d_maps8, maps8.data(), maps8.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
-    TC_CUDA(cudaFuncSetAttribute(attn_tc_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(SmSmem) + 1024)));
+    TC_CUDA(cudaFuncSetAttribute(attn_tc_small_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(SmSmem) + 1024)));
+    TC_CUDA(cudaFuncSetAttribute(attn_tc_small_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(SmSmem) + 1024)));
     pl->small_ok = true;
   }
   const size_t slots = (size_t)pl->grid_max + init.B;
@@ -625,6 +626,7 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   prm.out = (__nv_bfloat16*)out; prm.lse = lse; prm.swap = step.swap; prm.W = pl->init.W;
   prm.k_new = (const __nv_bfloat16*)step.k_new; prm.v_new = (const __nv_bfloat16*)step.v_new;
   prm.ktime = ktime;
+  prm.tl = n_attn <= kTlCtas ? step.tl : nullptr; prm.tl_seq = step.tl_seq;
   prm.wait_inputs = step.wait_inputs;
   prm.grow_wait = step.grow_wait;
   prm.in_ctr = step.in_ctr; prm.in_need = step.in_need;
@@ -634,7 +636,8 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   cudaLaunchConfig_t lc{};
   lc.gridDim = dim3(n_attn); lc.blockDim = dim3(kTcThreads); lc.dynamicSmemBytes = sizeof(SmSmem) + 1024; lc.stream = st;
   lc.attrs = attr; lc.numAttrs = (step.serialize || first_after_general) ? 0 : 1;
-  TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel, pl->map_pool, pl->map_pool64, pl->map_q, pl->map_part_small, pl->maps0, prm));
+  if (prm.tl) TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel<true>, pl->map_pool, pl->map_pool64, pl->map_q, pl->map_part_small, pl->maps0, prm));
+  else TC_CUDA(cudaLaunchKernelEx(&lc, attn_tc_small_kernel<false>, pl->map_pool, pl->map_pool64, pl->map_q, pl->map_part_small, pl->maps0, prm));
   if (ev_mid0) TC_CUDA(cudaEventRecord(ev_mid0, st));
   if (ev_mid1) TC_CUDA(cudaEventRecord(ev_mid1, st));
   ws->n_small += 1;

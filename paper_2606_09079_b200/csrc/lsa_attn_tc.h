@@ -61,6 +61,8 @@ struct TcSmallStep {
   int alone;                // 1: the caller blocks on this step (no neighbour launch to share the SMs with): use them all
   unsigned int* host_flag;  // PINNED HOST word (device alias) set to host_flag_val when `out` is complete, or null
   unsigned int host_flag_val;
+  unsigned long long* tl;   // DEVICE timeline record of this launch ([160 CTAs][12 stamps], include/lsa.h LSA_TL_*) or null
+  unsigned int tl_seq;
 };
 bool tc_small_supported(const TcPlan* plan);
 int tc_attention_small(TcPlan* plan, const void* q, void* out, float* lse, const TcSmallStep& step, cudaStream_t st,

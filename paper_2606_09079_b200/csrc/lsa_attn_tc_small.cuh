@@ -98,7 +98,15 @@ struct SmParams {
   const unsigned int* in_ctr;    // lsa_step_host_async: q / k_new / v_new are staged by a gather kernel that runs beside the
   unsigned int in_need;          // previous step; they are complete once this counter (its finished blocks) reaches in_need
   unsigned long long* ktime;     // profiling only, see TcParams
+  unsigned long long* tl;        // lsa_timeline_enable: this launch's record [kTlCtas][kTlEvents] of %globaltimer stamps, or null
+  unsigned int tl_seq;           // ... and its number among the context's traced launches
 };
+
+// Per-CTA timeline (include/lsa.h: lsa_timeline_*, LSA_TL_*): an instantiation of its own (kTl), so that the kernel that runs
+// when nothing is stamped carries none of it (eleven `if (p.tl)` in the one kernel cost 0.3 us per step at cfg 3, measured).
+constexpr int kTlCtas = 160, kTlEvents = 12;
+enum { kTlEntry = 0, kTlSetup, kTlFirstS, kTlLastPV, kTlEpilogue, kTlArrived, kTlAllArrived, kTlMerged, kTlExit, kTlSmid, kTlNCtas, kTlSeq };
+#define LSA_TL(ev) do { if constexpr (kTl) p.tl[(size_t)blockIdx.x * kTlEvents + (ev)] = gtime(); } while (0)
 
 // the eight tensor maps of sequence 0 travel with the launch (param space: no descriptor fetch from global memory
 // in front of the first TMA); sequences 1.. use SmParams::seq_maps
@@ -377,6 +385,7 @@ __device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CU
   }
 }
 
+template <bool kTl>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_constant__ CUtensorMap map_pool64,
                      const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_part,
@@ -404,6 +413,12 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   __syncthreads();
   griddep_launch_dependents();    // the combine blocks of this step (and, behind them, the next step's CTAs) may be placed
   if (p.ktime && tid == 0) atomicMin(p.ktime, gtime());
+  if (kTl && tid == 0) {
+    unsigned long long* r = p.tl + (size_t)cta * kTlEvents;
+    unsigned int smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    r[kTlEntry] = gtime(); r[kTlAllArrived] = 0; r[kTlMerged] = 0; r[kTlSmid] = smid; r[kTlNCtas] = (unsigned)n_cta; r[kTlSeq] = p.tl_seq;
+  }
   if (warp == 0) {
     // per-sequence shape -> half tiles per segment and their prefix (B <= 4).  Everything this CTA needs from global
     // memory before its first TMA is requested in ONE round trip: the table entries of the pages in its range, the
@@ -493,7 +508,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     if (lane == 0) sm.pg_cnt = min(cnt, 32);
     if (p.grow_wait) fence_proxy_async_all();          // the rows were written by generic stores, TMA reads them
     __syncwarp();
-    if (lane == 0) mbar_arrive(&sm.setup);
+    if (lane == 0) { LSA_TL(kTlSetup); mbar_arrive(&sm.setup); }
   } else if (warp == 1) {
     tmem_alloc(&sm.tmem_base, 512);
     tc_fence_before();
@@ -658,6 +673,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
           mbar_wait(&sm.q_full, item & 1, 20);
           tc_fence_after();
           issue_s(s.rows, s.last);
+          if (item == 0) LSA_TL(kTlFirstS);
         }
         have = cur.next(nx);
         if (!s.last) issue_s(nx.rows, nx.last);
@@ -666,6 +682,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
         if (s.last) ++item;
         s = nx;
       }
+      LSA_TL(kTlLastPV);
     }
   } else {
     // =========================== softmax + epilogue (8 warps) ===========================
@@ -849,6 +866,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
       if (lane == 0) mbar_arrive(&sm.o_empty);
       ++piece;
     }
+    if (tid == 64) LSA_TL(kTlEpilogue);
     if (tid == 64) p.piece_info[cta] = make_int2(b_first < 0 ? 0 : b_first, b_first < 0 ? 0 : b_last - b_first + 1);
   }
   // ---- S8: publish; the launch's last n_mrg CTAs to arrive merge its partials, the others leave their SM at once ----
@@ -862,10 +880,12 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     __threadfence();                                // cumulative: the partial stores of every thread of this CTA (ordered before
     const unsigned int old = atomicAdd(p.arr_ctr, 1u);   // this thread by the barrier) are visible before the arrival is
     sm.rank = (int)(old - (p.arr_target - (unsigned)n_cta));   // arrival index inside this launch, 0 .. n_cta - 1
+    LSA_TL(kTlArrived);
   }
   __syncthreads();
   const int mi = sm.rank - (n_cta - p.n_mrg);       // the last n_mrg arrivals are the mergers 0 .. n_mrg - 1
   if (mi < 0) {
+    if (tid == 0) LSA_TL(kTlExit);
     if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
     return;
   }
@@ -874,6 +894,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
   if (warp == 0) {
     if (lane == 0) {
       wait_counter(p.arr_ctr, p.arr_target, 53);    // every partial of the launch is visible from here on
+      LSA_TL(kTlAllArrived);
     }
     __syncwarp();
     named_bar_sync(3, 288);                         // the softmax warps start on the weights
@@ -908,6 +929,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
     small_merge(p, sm, &map_part, mi, p.n_mrg, tid - 64);
   }
   __syncthreads();
+  if (tid == 0) LSA_TL(kTlMerged);
   if (tid == 0) {
     if (p.host_flag) {
       // `out` may live in pinned host memory: this CTA's rows are visible system-wide before it is counted, and the
@@ -923,6 +945,7 @@ attn_tc_small_kernel(const __grid_constant__ CUtensorMap map_pool, const __grid_
       red_release_add_u32(p.done_ctr, 1u);
     }
   }
+  if (tid == 0) LSA_TL(kTlExit);
   if (p.ktime && tid == 0) atomicMax(p.ktime + 1, gtime());
 }
 

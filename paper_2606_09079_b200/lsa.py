@@ -32,7 +32,7 @@ STATUS = {0: "LSA_OK", -1: "LSA_ERR_INVALID_ARG", -2: "LSA_ERR_CUDA", -3: "LSA_E
 EXPORTS = ["lsa_init_pools", "lsa_index_select", "lsa_fetch_chunks", "lsa_commit_tables",
            "lsa_decode_attention", "lsa_step", "lsa_step_host", "lsa_step_host_async", "lsa_host_wait", "lsa_set_chunk_emb",
            "lsa_get_page_table", "lsa_get_residency", "lsa_get_stats", "lsa_get_step", "lsa_sync",
-           "lsa_profile_enable", "lsa_profile_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
+           "lsa_profile_enable", "lsa_profile_read", "lsa_timeline_enable", "lsa_timeline_read", "lsa_l1_init", "lsa_l1_select", "lsa_set_indexer",
            "lsa_l2_init", "lsa_l2_select", "lsa_step_l2", "lsa_l2_get_mask", "lsa_step_graph", "lsa_graph_stats", "lsa_export_chunks",
            "lsa_append_compressed", "lsa_index_select_static", "lsa_last_error", "lsa_destroy", "lsa_version"]
 
@@ -105,6 +105,8 @@ def _load() -> C.CDLL:
     lib.lsa_sync.argtypes = [vp]
     lib.lsa_profile_enable.argtypes = [vp, C.c_int32]
     lib.lsa_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    lib.lsa_timeline_enable.argtypes = [vp, C.c_int32]
+    lib.lsa_timeline_read.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
     lib.lsa_l1_init.argtypes = [vp, C.POINTER(lsa_l1_config), C.POINTER(vp)]
     lib.lsa_l1_select.argtypes = [vp, vp, i32p, C.c_int32, vp, f32p]
     lib.lsa_set_indexer.argtypes = [vp, C.c_int32]
@@ -435,6 +437,20 @@ class LsaContext:
 
     def profile_enable(self, capacity: int):
         self._check(_lib.lsa_profile_enable(self._h, capacity))
+
+    TL_SHAPE = (16, 160, 12)      # LSA_TL_LAUNCHES, LSA_TL_CTAS, LSA_TL_EVENTS
+    TL_EVENTS = ("entry", "setup", "first_s", "last_pv", "epilogue", "arrived", "all_arrived", "merged", "exit", "smid", "n_ctas", "seq")
+
+    def timeline_enable(self, on: bool = True):
+        self._check(_lib.lsa_timeline_enable(self._h, 1 if on else 0))
+
+    def timeline_read(self):
+        """(uint64 array [launch record][CTA][event] of %globaltimer nanoseconds, launches stamped so far); include/lsa.h LSA_TL_*"""
+        import numpy as np
+        buf = np.zeros(self.TL_SHAPE, dtype=np.uint64)
+        n = C.c_uint64(0)
+        self._check(_lib.lsa_timeline_read(self._h, buf.ctypes.data_as(C.c_void_p), C.byref(n)))
+        return buf, int(n.value)
 
     def profile_read(self) -> dict:
         ms, cnt = (C.c_double * 7)(), (C.c_int64 * 7)()

@@ -778,6 +778,47 @@ def test_small_batch_last_arrivals_merge(max_ctas, n_rows, w_len):
     ctx.close()
 
 
+def test_small_batch_timeline():
+    """lsa_timeline_*: every CTA of a stamped launch has ordered stamps, the launch's last 32 arrivals (all of them if it has
+    fewer CTAs) carry merger stamps, and stamping does not change the result."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 1200
+    g = torch.Generator().manual_seed(43)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    hk, hv, wk, wv = [rnd(11200, D)], [rnd(11200, D)], [rnd(W, D)], [rnd(W, D)]
+    q = rnd(1, H, D)
+    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, [900], W, sm_scale=0.05, attn_impl=lsa.LSA_ATTN_TCGEN05, step_overlap=1)
+    ref = ctx.decode_attention(q)
+    tl0, n0 = ctx.timeline_read()                                 # (waits for both streams)
+    assert n0 == 0 and not tl0.any()
+    ctx.timeline_enable(True)
+    outs = [ctx.decode_attention(q) for _ in range(5)]            # an output buffer each
+    ctx.timeline_enable(False)
+    ctx.decode_attention(q)                                       # not stamped
+    tl, n = ctx.timeline_read()
+    assert n == 5
+    for o in outs:
+        assert torch.equal(o, ref)
+    E = {name: i for i, name in enumerate(ctx.TL_EVENTS)}
+    for l in range(5):
+        rec = tl[l].astype(np.int64)
+        n_cta = int(rec[0, E["n_ctas"]])
+        assert n_cta == 48 and (rec[:n_cta, E["seq"]] == l).all() and not rec[n_cta:].any()
+        r = rec[:n_cta]
+        for a_, b_ in [("entry", "setup"), ("entry", "first_s"), ("first_s", "last_pv"), ("last_pv", "epilogue"), ("epilogue", "arrived"), ("arrived", "exit")]:
+            assert (r[:, E[a_]] <= r[:, E[b_]]).all(), (a_, b_)
+        mrg = r[:, E["merged"]] > 0
+        assert mrg.sum() == 32
+        assert (r[mrg, E["arrived"]] <= r[mrg, E["all_arrived"]]).all() and (r[mrg, E["all_arrived"]] <= r[mrg, E["merged"]]).all()
+        assert (r[mrg, E["merged"]] <= r[mrg, E["exit"]]).all() and (r[~mrg, E["all_arrived"]] == 0).all()
+        # the mergers are the LAST arrivals (a stamp is taken after the arrival, so two near-simultaneous ones may swap)
+        assert r[mrg, E["arrived"]].min() + 2000 >= r[~mrg, E["arrived"]].max()
+        assert (r[:, E["smid"]] < 256).all()
+    assert not tl[5:].any()
+    ctx.close()
+
+
 def test_small_batch_step_overlap_lockstep():
     """lsa_config.step_overlap = 1 (inputs independent of the previous step's output): the whole path in lock-step with
     the oracle over several trigger periods - triggers, swaps (serialised launches) and the overlapped steps between them."""
