@@ -707,6 +707,23 @@ def main():
                      residency_ms_per_trigger=pr["residency"]["ms"] / max(pr["residency"]["count"], 1))
         del src, dst
 
+    # ---- per-CTA timeline of the small-batch launches (lsa_timeline_*; DESIGN 7.3): a stretch of its own, after the timed legs of the main
+    # contexts (and before the legs that move them to other kernels: lsa_step_graph keeps a context on the general path)
+    timeline = None
+    if args.timeline and args.overlap and c.B <= 4 and stats["attn_impl"] == 2:
+        for r in reps:
+            r.ctx.timeline_enable(True)
+        n_tl = 2 * R * c.tau
+        for i in range(R * 8):                      # the stamps themselves are part of what is measured: settle first
+            one_step(i_next + i)
+        i_next += R * 8
+        ms_tl, _, _, _ = timed(n_tl, i0=i_next)
+        i_next += n_tl
+        tl = [r.ctx.timeline_read()[0] for r in reps]
+        for r in reps:
+            r.ctx.timeline_enable(False)
+        timeline = summarise_timeline(tl, ms_tl / n_tl)
+
     # ---- optional: the paper-exact Level-1 indexer (NEXT-1) at this config's context length ----
     l1 = None
     if args.l1 and rank == 0 and c.dtype == "bf16" and c.C == 128:
@@ -900,22 +917,6 @@ def main():
         graph = dict(value=per_step_units / (g_ms * 1e-3), unit=unit, ms_per_step=g_ms, host_enqueue_ms_per_step=enq_g * 1e3 / n_g,
                      captures=sum(g_["captures"] for g_ in gs), replays=sum(g_["replays"] for g_ in gs),
                      note="lsa_step_graph: steps without a trigger or a table swap replay one captured graph (attention + combine) per context")
-
-    # ---- per-CTA timeline of the small-batch launches (lsa_timeline_*; DESIGN 7.3): a stretch of its own, after every timed leg
-    timeline = None
-    if args.timeline and args.overlap and c.B <= 4 and stats["attn_impl"] == 2:
-        for r in reps:
-            r.ctx.timeline_enable(True)
-        n_tl = 2 * R * c.tau
-        for i in range(R * 8):                      # the stamps themselves are part of what is measured: settle first
-            one_step(i_next + i)
-        i_next += R * 8
-        ms_tl, _, _, _ = timed(n_tl, i0=i_next)
-        i_next += n_tl
-        tl = [r.ctx.timeline_read()[0] for r in reps]
-        for r in reps:
-            r.ctx.timeline_enable(False)
-        timeline = summarise_timeline(tl, ms_tl / n_tl)
 
     cpu_baseline = cpu_baseline_1t = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
