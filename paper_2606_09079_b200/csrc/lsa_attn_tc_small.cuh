@@ -5,14 +5,14 @@
 // from the general kernel (lsa_attn_tc_kernel.cuh), whose tcgen05 / TMA pipeline this kernel keeps:
 //
 // 1. Pieces are cut at HALF tiles (64 rows).  The flat list of 64-row half tiles (per sequence: HCA rows, two
-//    halves per page of the current table, window rows) is cut into gridDim.x contiguous ranges, so all 148 SMs
-//    pull from HBM (whole 128-row tiles allow only 96 equal shares at cfg 3).  Adjacent halves of one source are
+//    halves per page of the current table, window rows) is cut into gridDim.x contiguous ranges of equal length (whole
+//    128-row tiles allow only 96 equal shares at cfg 3; the host picks an even length where it can).  Adjacent halves of one source are
 //    merged back into a 128-row sub-tile; a lone half is a 64-row TMA box (its own tensor map) that fills the
 //    first half of a stage: S^T is still one M = 128 MMA per k-step (rows 64.. are stale shared memory, masked by
 //    the softmax threads), PV and the row sums run 4 instead of 8 k-steps.
 //
 // 2. Nothing the LIBRARY wrote for the previous step is read before the K/V stream starts: the per-sequence shape
-//    arrives BY VALUE from the host's deterministic mirrors (SmSeq), the split partials alternate between two
+//    arrives BY VALUE from the host's deterministic mirrors (SmSeq), the split partials rotate through three
 //    workspace buffers, and the one true cross-launch dependency - the window row the previous step appended
 //     - is ordered by a release / acquire counter in the sequence record (SeqDev::app_epoch).  Launched with
 //    programmatic stream serialization, its CTAs start on an SM the moment the previous step's CTA leaves it and

@@ -698,7 +698,7 @@ def test_small_batch_half_tile_split_edge_cases(max_ctas, overlap):
 
 @pytest.mark.parametrize("overlap", [0, 1])
 def test_small_batch_steps_back_to_back_without_sync(overlap):
-    """The small-batch launches do not wait for the previous step's merge (double-buffered partials, the ring row
+    """The small-batch launches do not wait for the previous step's merge (partials in rotating workspace buffers, the ring row
     ordered by SeqDev::app_epoch): 48 steps of two contexts interleaved on one stream, each with its own q and its
     own output buffer, no host synchronisation in between; every output is then compared with the oracle, which
     sees the window grow by one row per step."""
