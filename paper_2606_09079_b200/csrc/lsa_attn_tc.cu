@@ -595,7 +595,8 @@ int tc_attention_small(TcPlan* pl, const void* q, void* out, float* lse, const T
   // machine with and takes every SM; a launch that merely waits for the stream (a swap step: the fetch event) keeps the
   // shared size, because the launches BEHIND it overlap it again (all SMs there: 10.2 us per step, shared size: 10.0).
   const bool alone = step.alone;
-  const long long g_cap = (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 4) / 3);
+  // (the in-launch merge lands at most 160 partial slots per output unit in shared memory: lsa_attn_tc_small.cuh kMuLandBytes)
+  const long long g_cap = std::min<long long>(160, (pl->init.max_ctas > 0 || alone) ? pl->grid_max : std::max(1, (pl->init.n_sms - 4) / 3));
   long long per = std::max<long long>(1, (halves + g_cap - 1) / g_cap);
   if (!alone && per > 1 && (per & 1)) ++per;
   const int n_attn = (int)std::max<long long>(1, std::min<long long>(g_cap, (halves + per - 1) / per));
