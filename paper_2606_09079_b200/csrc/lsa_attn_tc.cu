@@ -343,7 +343,7 @@ static TcWorkspace* ws_acquire(cudaStream_t st, size_t slots, size_t grid_max, s
   if (e == cudaSuccess) e = cudaMalloc(&w->part_l, kWsBufs * slots * kTcH * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&w->piece_info, kWsBufs * grid_max * sizeof(int2));
   if (e == cudaSuccess) e = cudaMalloc(&w->ctrs, (kWsBufs + 1) * sizeof(unsigned int));
-  // (a slot that holds no partial for a sequence is weighed with 0, not skipped: what it holds must be finite)
+  // (the workspace starts defined: a slot no launch has written yet is still landed by the merge's TMA boxes)
   if (e == cudaSuccess) e = cudaMemset(w->part_o, 0, kWsBufs * slots * (kTcH * kTcD / 4) * sizeof(uint2));
   if (e == cudaSuccess) e = cudaMemset(w->part_s, 0, kWsBufs * slots * kTcPartScales * sizeof(float));
   if (e == cudaSuccess) e = cudaMemset(w->part_m, 0, kWsBufs * slots * kTcH * sizeof(float));

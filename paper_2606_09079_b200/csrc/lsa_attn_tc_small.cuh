@@ -350,14 +350,15 @@ __device__ __noinline__ void small_merge(const SmParams& p, SmSmem& sm, const CU
       L = sm_warp_sum4(L);
       __syncwarp();
       mbar_wait(&sm.mrg_full, round & 1, 57);
-      // weighted sum: lane = one uint2 column (4 heads of one d).  A slot without a partial for this sequence has weight 0
-      // and holds what an earlier launch left there, which is finite fp16 (the workspace is zeroed when it is created and
-      // partials are scaled into the fp16 range before they are stored), so 0 x stale = 0: no select in the loop
+      // weighted sum: lane = one uint2 column (4 heads of one d).  A slot of weight 0 (no partial for this sequence: it
+      // holds what an earlier launch left there, possibly of another sequence) is selected away, never multiplied - a NaN
+      // a caller fed into one sequence must not reach another; a select, not a branch, so the loads of a trip stay batched
       const unsigned char* lp = land + (size_t)w * rows * 256 + lane * 8;
 #pragma unroll 8
       for (int sl = 0; sl < n_cta; ++sl) {
         const float4 f = mw[sl];
-        const uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
+        uint2 v = *reinterpret_cast<const uint2*>(lp + (size_t)sl * 256);
+        if (f.x == 0.f && f.y == 0.f && f.z == 0.f && f.w == 0.f) v = make_uint2(0u, 0u);
         const float2 a01 = unpack_f16x2(v.x), a23 = unpack_f16x2(v.y);
         acc.x = fmaf(f.x, a01.x, acc.x); acc.y = fmaf(f.y, a01.y, acc.y);
         acc.z = fmaf(f.z, a23.x, acc.z); acc.w = fmaf(f.w, a23.y, acc.w);

@@ -778,6 +778,34 @@ def test_small_batch_last_arrivals_merge(max_ctas, n_rows, w_len):
     ctx.close()
 
 
+@pytest.mark.parametrize("overlap", [0, 1])
+def test_small_batch_merge_never_multiplies_a_foreign_slot(overlap):
+    """Partial slot = CTA + sequence, so the slots a sequence's merge walks include other sequences' partials (weight 0).
+    They are selected away, not multiplied: a NaN fed into sequence 0 leaves sequence 1's output exact
+    (step_overlap 1: the in-launch merge; 0: the large-grid kernel + combine kernel)."""
+    lsa = _lsa()
+    dev = torch.device("cuda:0")
+    H, D, W = 64, 512, 700
+    g = torch.Generator().manual_seed(47)
+    rnd = lambda *s: torch.randn(*s, generator=g).to(torch.bfloat16).to(dev)
+    n_rows, w_len = [5000, 4000], [600, 333]
+    hk, hv = [rnd(n, D) for n in n_rows], [rnd(n, D) for n in n_rows]
+    wk, wv = [rnd(W, D) for _ in range(2)], [rnd(W, D) for _ in range(2)]
+    hv[0][1234, 77] = float("nan")
+    hk[0][4000, 5] = float("nan")
+    q = rnd(2, H, D)
+    ctx = _direct_ctx("bf16", H, D, 128, hk, hv, wk, wv, w_len, W, sm_scale=0.05, attn_impl=lsa.LSA_ATTN_TCGEN05, step_overlap=overlap)
+    outs = [ctx.decode_attention(q) for _ in range(5)]
+    ctx.sync()
+    K = np.concatenate([hk[1].double().cpu().numpy(), wk[1][: w_len[1]].double().cpu().numpy()])
+    V = np.concatenate([hv[1].double().cpu().numpy(), wv[1][: w_len[1]].double().cpu().numpy()])
+    ref, _, _ = attention(q[1].double().cpu().numpy(), K, V, 0.05)
+    for out in outs:                                  # (what sequence 0 itself gets for NaN inputs is not specified)
+        assert torch.isfinite(out[1]).all()
+        np.testing.assert_allclose(out[1].double().cpu().numpy(), ref, **attn_tolerance("bf16"))
+    ctx.close()
+
+
 def test_small_batch_timeline():
     """lsa_timeline_*: every CTA of a stamped launch has ordered stamps, the launch's last 32 arrivals (all of them if it has
     fewer CTAs) carry merger stamps, and stamping does not change the result."""
